@@ -1,0 +1,387 @@
+"""TEST INFRASTRUCTURE -- CPU oracle for the Tangram hot path (PAPER.md = arxiv/paper_2606_06302).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may
+import this.  It shares no code with the CUDA/C++ product (paper_2606_06302_b200/csrc): own
+source, own address arithmetic, plain Python / numpy fp64 (the attention part is plain C in
+attention_oracle.c, called through ctypes).
+
+What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.md §Readings):
+  O2 reserve_budgets      Eq. 5 (:158)  B = min(1, mu + alpha*sigma);  Eq. 4 (:154) n = ceil(B N);
+                          overflow truncation (:176)
+  O3 build_ragged_tables  Budget-Aware Clustering (:192-194, :227-233), per-group page table sized
+                          by the group's max budget (:190), slack use (:235)
+  O4 split_map            Algorithm 1 (:196-225)
+     plan_partitions      modes SPLITMAP (Alg. 1 expanded, reading A16), BALANCED (north_star's
+                          equal-bytes work list, reading A2), STATIC_EVEN (FlashDecoding-style
+                          uniform num_splits, :120)
+  O5 merge                log-sum-exp merge of split-KV partials (implied by split-KV :91, :120)
+  O1 attention*           plain softmax(q K~^T / sqrt(d)) V~ through the page tables (Eq. 1 :57)
+
+Pins (every function is pinned; nothing here is "parity unpinned"): tests/test_oracle_pins.py.
+Fidelity to the authors' unseen code for the rounding mode of Alg. 1 line 10 (reading A14) and
+for how S maps to CTAs (reading A16) cannot be pinned from the paper; they are pinned to the
+DESIGN.md readings.
+"""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import math
+import os
+import subprocess
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+FLAG_FILL_GROUP = 1
+MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
+
+
+# --------------------------------------------------------------------------------------------
+# O2  Budget Reservation  (Eq. 5 :158, Eq. 4 :154, overflow :176)
+# --------------------------------------------------------------------------------------------
+def reserve_budgets(mu, sigma, alpha: float, ctx_len, demand=None):
+    """Returns (B [H] f64, reserved [R][H] i32, kv_len [R][H] i32).
+
+    B_h = min(1, mu_h + alpha*sigma_h) evaluated as one fp64 multiply then one fp64 add
+    (reading A9; Python floats never fuse).  reserved = ceil(B_h * N_r) clamped to [1, N_r].
+    kv_len = min(demand, reserved) (the overflow rule, :176) or reserved if demand is None."""
+    H, R = len(mu), len(ctx_len)
+    B = np.empty(H, dtype=np.float64)
+    for h in range(H):
+        prod = float(alpha) * float(sigma[h])
+        b = float(mu[h]) + prod
+        b = min(1.0, b)
+        if not (b > 0.0):
+            raise ValueError(f"budget ratio of head {h} is not in (0,1] (reading A11)")
+        B[h] = b
+    reserved = np.empty((R, H), dtype=np.int32)
+    kv_len = np.empty((R, H), dtype=np.int32)
+    for r in range(R):
+        N = int(ctx_len[r])
+        if N < 1:
+            raise ValueError("ctx_len < 1")
+        for h in range(H):
+            n = int(math.ceil(float(B[h]) * float(N)))
+            n = max(1, min(N, n))
+            reserved[r, h] = n
+            if demand is None:
+                kv_len[r, h] = n
+            else:
+                dm = int(demand[r][h])
+                if dm < 0:
+                    raise ValueError("demand < 0")
+                kv_len[r, h] = min(dm, n)
+    return B, reserved, kv_len
+
+
+# --------------------------------------------------------------------------------------------
+# O3  Budget-Aware Clustering + per-(request, cluster) page tables  (§4.2 :190-235)
+# --------------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class Tables:
+    R: int
+    H: int
+    C: int
+    Hp: int
+    P: int
+    perm: np.ndarray        # [H]  pi: sorted position -> head
+    cluster_of: np.ndarray  # [H]  head -> cluster
+    slot_of: np.ndarray     # [H]  head -> slot inside the cluster's pages
+    tbl_indptr: np.ndarray  # [R*C+1] int64, row = r*C + c
+    tbl_pages: np.ndarray   # [n_pages_used] int32
+    n_pages_used: int
+
+
+def cluster_heads(B, n_clusters: int):
+    """pi = heads stably sorted by B ascending (ties keep head order, reading A6);
+    group i = H_p consecutive heads of the sorted order (:231-233)."""
+    H = len(B)
+    if n_clusters <= 0 or H % n_clusters != 0:
+        raise ValueError("H must be a multiple of n_clusters (reading A17)")
+    Hp = H // n_clusters
+    perm = sorted(range(H), key=lambda h: (float(B[h]), h))
+    cluster_of = [0] * H
+    slot_of = [0] * H
+    for j, h in enumerate(perm):
+        cluster_of[h] = j // Hp
+        slot_of[h] = j % Hp
+    return (np.array(perm, dtype=np.int32), np.array(cluster_of, dtype=np.int32),
+            np.array(slot_of, dtype=np.int32))
+
+
+def build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages,
+                        flags: int = 0, kv_len=None):
+    """Returns (Tables, kv_len').  Row (r, c) of the tables has ceil(max_{h in c} reserved / P)
+    pages (:190) and takes the next entries of `free_pages` in order (reading A27).  With
+    FLAG_FILL_GROUP every head's kv_len is raised to its cluster's max reserved (:235)."""
+    reserved = np.asarray(reserved)
+    R, H = reserved.shape
+    if page_size <= 0:
+        raise ValueError("page_size <= 0")
+    perm, cluster_of, slot_of = cluster_heads(B, n_clusters)
+    C, Hp = n_clusters, H // n_clusters
+    indptr = [0]
+    pages: List[int] = []
+    cursor = 0
+    gmax = np.zeros((R, C), dtype=np.int64)
+    for r in range(R):
+        for c in range(C):
+            members = [int(perm[c * Hp + k]) for k in range(Hp)]
+            mx = max(int(reserved[r, h]) for h in members)
+            gmax[r, c] = mx
+            n_pg = -(-mx // page_size)
+            if cursor + n_pg > len(free_pages):
+                raise MemoryError("out of pages")
+            pages.extend(int(free_pages[cursor + i]) for i in range(n_pg))
+            cursor += n_pg
+            indptr.append(cursor)
+    kv_out = None if kv_len is None else np.array(kv_len, dtype=np.int32, copy=True)
+    if (flags & FLAG_FILL_GROUP) and kv_out is not None:
+        for r in range(R):
+            for h in range(H):
+                kv_out[r, h] = gmax[r, cluster_of[h]]
+    t = Tables(R=R, H=H, C=C, Hp=Hp, P=page_size, perm=perm, cluster_of=cluster_of,
+               slot_of=slot_of, tbl_indptr=np.array(indptr, dtype=np.int64),
+               tbl_pages=np.array(pages, dtype=np.int32), n_pages_used=cursor)
+    return t, kv_out
+
+
+# --------------------------------------------------------------------------------------------
+# O4  AoT plans
+# --------------------------------------------------------------------------------------------
+def split_map(B, perm, Hp: int, n_cta: int) -> np.ndarray:
+    """Algorithm 1 (:196-225) for one layer, de-garbled per reading A13:
+    Omega = sum_h B_h; if Omega = 0: S = 1; tau = Omega / N_CTA;
+    Phi_i = sum_{h in G_i} B_h;  S_i = max(1, round(Phi_i / tau)), round = half-up (A14)."""
+    H = len(B)
+    C = H // Hp
+    S = [1] * C
+    omega = 0.0
+    for h in range(H):           # head-index order
+        omega += float(B[h])
+    if omega == 0.0:
+        return np.array(S, dtype=np.int32)
+    tau = omega / float(n_cta)
+    for i in range(C):
+        phi = 0.0
+        for k in range(Hp):      # perm order inside the group
+            phi += float(B[int(perm[i * Hp + k])])
+        S[i] = max(1, int(math.floor(phi / tau + 0.5)))
+    return np.array(S, dtype=np.int32)
+
+
+@dataclasses.dataclass
+class Plan:
+    W: int
+    mode: int
+    split_map: np.ndarray       # [C] int32 (SPLITMAP: Alg. 1; STATIC_EVEN: constant; BALANCED: Alg. 1, informational)
+    items: np.ndarray           # [n_items, 8] int32: req, kv_head, cluster, slot, tok_begin, tok_end, part_slot, n_parts
+    worker_indptr: np.ndarray   # [W+1] int64
+    part_indptr: np.ndarray     # [R*H+1] int64, seq = r*H + h
+    n_items: int
+    n_part_slots: int
+
+
+def _finish(raw: List[Tuple[int, int, int, int, int]], t: Tables, W: int, mode: int, S) -> Plan:
+    """raw: (worker, r, h, tok_begin, tok_end) in plan order.  Assigns part_slot / n_parts and
+    lays the items out worker-major, plan order kept inside a worker."""
+    R, H = t.R, t.H
+    count = [0] * (R * H)
+    for (_, r, h, _, _) in raw:
+        count[r * H + h] += 1
+    part_indptr = [0] * (R * H + 1)
+    for s in range(R * H):
+        part_indptr[s + 1] = part_indptr[s] + count[s]
+    # ordinal of an item inside its sequence = token order
+    by_seq: dict = {}
+    for idx, (_, r, h, tb, _) in enumerate(raw):
+        by_seq.setdefault(r * H + h, []).append((tb, idx))
+    ordinal = [0] * len(raw)
+    for s, lst in by_seq.items():
+        for o, (_, idx) in enumerate(sorted(lst)):
+            ordinal[idx] = o
+    per_worker: List[List[int]] = [[] for _ in range(W)]
+    for idx, it in enumerate(raw):
+        per_worker[it[0]].append(idx)
+    items = np.zeros((len(raw), 8), dtype=np.int32)
+    worker_indptr = [0]
+    k = 0
+    for w in range(W):
+        for idx in per_worker[w]:
+            _, r, h, tb, te = raw[idx]
+            s = r * H + h
+            items[k] = (r, h, int(t.cluster_of[h]), int(t.slot_of[h]), tb, te,
+                        part_indptr[s] + ordinal[idx], count[s])
+            k += 1
+        worker_indptr.append(k)
+    return Plan(W=W, mode=mode, split_map=np.asarray(S, dtype=np.int32), items=items,
+                worker_indptr=np.array(worker_indptr, dtype=np.int64),
+                part_indptr=np.array(part_indptr, dtype=np.int64), n_items=len(raw),
+                n_part_slots=part_indptr[-1])
+
+
+def plan_partitions(t: Tables, B, kv_len, n_workers: int, granule: int, overhead_granules: int,
+                    mode: int, static_splits: int = 0) -> Plan:
+    """Offline deterministic planner (§4.3).  Sequences are visited r-major, then in `perm`
+    order, so neighbours share a page table."""
+    kv_len = np.asarray(kv_len)
+    R, H, W, g, c0 = t.R, t.H, int(n_workers), int(granule), int(overhead_granules)
+    if W < 1 or g < 1 or g % t.P != 0 or c0 < 0:
+        raise ValueError("bad planner arguments (granule must be a positive multiple of P)")
+    S_alg1 = split_map(B, t.perm, t.Hp, W)
+    seqs = [(r, int(t.perm[j])) for r in range(R) for j in range(H)]
+    raw: List[Tuple[int, int, int, int, int]] = []
+
+    if mode == MODE_BALANCED:
+        # north_star: "splits every (request, KV head) sequence into chunks of near-equal KV
+        # bytes per CTA".  Cost of a sequence = its granules + c0 granules of fixed overhead.
+        u = [-(-int(kv_len[r, h]) // g) for (r, h) in seqs]
+        w = [ui + (c0 if ui > 0 else 0) for ui in u]
+        T = sum(w)
+        b = [(k * T) // W for k in range(W + 1)]
+        a = 0
+        k = 0
+        for i, (r, h) in enumerate(seqs):
+            n = int(kv_len[r, h])
+            run_start = None
+            run_worker = None
+            for j in range(u[i]):
+                pos = a + c0 + j
+                while b[k + 1] <= pos:      # worker k owns positions b_k <= pos < b_{k+1}
+                    k += 1
+                if run_worker != k:
+                    if run_start is not None:
+                        raw.append((run_worker, r, h, run_start * g, min(n, j * g)))
+                    run_start, run_worker = j, k
+            if run_start is not None:
+                raw.append((run_worker, r, h, run_start * g, n))
+            a += w[i]
+        return _finish(raw, t, W, mode, S_alg1)
+
+    if mode == MODE_SPLITMAP:
+        S = S_alg1
+    elif mode == MODE_STATIC_EVEN:
+        s = int(static_splits)
+        if s <= 0:                      # smallest S with R*H*S >= W
+            s = max(1, -(-W // (R * H)))
+        S = np.full(t.C, s, dtype=np.int32)
+    else:
+        raise ValueError("mode")
+    kk = 0
+    for (r, h) in seqs:
+        n = int(kv_len[r, h])
+        npg = -(-n // g)                # granules of this sequence
+        Sc = int(S[int(t.cluster_of[h])])
+        for j in range(Sc):
+            lo = (j * npg) // Sc
+            hi = ((j + 1) * npg) // Sc
+            tb, te = lo * g, min(n, hi * g)
+            if te <= tb:
+                continue                # empty chunk dropped
+            raw.append((kk % W, r, h, tb, te))
+            kk += 1
+    return _finish(raw, t, W, mode, S)
+
+
+# --------------------------------------------------------------------------------------------
+# O5  log-sum-exp merge  (textbook; implied by split-KV :91)
+# --------------------------------------------------------------------------------------------
+def merge(parts: Sequence[Tuple[np.ndarray, float]]):
+    """parts: (o_i normalised within its chunk [d] f64, lse_i).  L = m* + ln sum e^{lse_i-m*};
+    out = sum e^{lse_i - L} o_i.  Parts with lse = -inf contribute nothing."""
+    live = [(np.asarray(o, dtype=np.float64), float(l)) for (o, l) in parts if l != -math.inf]
+    if not live:
+        d = len(parts[0][0]) if parts else 0
+        return np.zeros(d, dtype=np.float64), -math.inf
+    mstar = max(l for (_, l) in live)
+    tot = 0.0
+    for (_, l) in live:
+        tot += math.exp(l - mstar)
+    L = mstar + math.log(tot)
+    out = np.zeros_like(live[0][0])
+    for (o, l) in live:
+        out = out + math.exp(l - L) * o
+    return out, L
+
+
+# --------------------------------------------------------------------------------------------
+# O1  attention through the page tables (plain C, fp64; attention_oracle.c)
+# --------------------------------------------------------------------------------------------
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle_attention.so")
+_lib = None
+
+
+def build_c(force: bool = False) -> str:
+    src = os.path.join(_HERE, "attention_oracle.c")
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
+                               "-o", _SO, src, "-lm"])
+    return _SO
+
+
+def _c():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build_c())
+        _lib.tangram_oracle_attention_pairs.restype = ctypes.c_int
+    return _lib
+
+
+def _u16(x) -> np.ndarray:
+    """bf16 torch tensor (or uint16 ndarray) -> contiguous uint16 ndarray of the raw bits."""
+    if isinstance(x, np.ndarray):
+        assert x.dtype == np.uint16
+        return np.ascontiguousarray(x)
+    import torch
+    assert x.dtype == torch.bfloat16 and x.device.type == "cpu"
+    return x.contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def attention_pairs(q, pool, t: Tables, kv_len, Hq: int, d: int, pairs, n_threads: int = 0):
+    """Attention for the listed (r, j) pairs.  Returns (out [n,d] f64, lse [n] f64, threads)."""
+    qb, pb = _u16(q), _u16(pool)
+    pairs = np.ascontiguousarray(np.asarray(pairs, dtype=np.int32).reshape(-1, 2))
+    kv = np.ascontiguousarray(np.asarray(kv_len, dtype=np.int32))
+    n = pairs.shape[0]
+    out = np.zeros((n, d), dtype=np.float64)
+    lse = np.zeros(n, dtype=np.float64)
+    ip = np.ascontiguousarray(t.tbl_indptr, dtype=np.int64)
+    pg = np.ascontiguousarray(t.tbl_pages, dtype=np.int32)
+    co = np.ascontiguousarray(t.cluster_of, dtype=np.int32)
+    so = np.ascontiguousarray(t.slot_of, dtype=np.int32)
+    used = _c().tangram_oracle_attention_pairs(
+        _p(qb), _p(pb), _p(ip), _p(pg), _p(co), _p(so), _p(kv),
+        ctypes.c_int32(t.R), ctypes.c_int32(t.H), ctypes.c_int32(Hq), ctypes.c_int32(t.C),
+        ctypes.c_int32(t.Hp), ctypes.c_int32(t.P), ctypes.c_int32(d), _p(pairs),
+        ctypes.c_int64(n), _p(out), _p(lse), ctypes.c_int32(n_threads))
+    return out, lse, int(used)
+
+
+def attention(q, pool, t: Tables, kv_len, Hq: int, d: int, n_threads: int = 0):
+    """Whole batch: out [R][Hq][d] f64, lse [R][Hq] f64."""
+    pairs = [(r, j) for r in range(t.R) for j in range(Hq)]
+    out, lse, used = attention_pairs(q, pool, t, kv_len, Hq, d, pairs, n_threads)
+    return out.reshape(t.R, Hq, d), lse.reshape(t.R, Hq), used
+
+
+def attend_range(q, pool, t: Tables, Hq: int, d: int, r: int, j: int, t0: int, t1: int):
+    """Attention of (r, j) over tokens [t0, t1) only: (o [d] normalised in the range, lse)."""
+    qb, pb = _u16(q), _u16(pool)
+    out = np.zeros(d, dtype=np.float64)
+    lse = ctypes.c_double(0.0)
+    ip = np.ascontiguousarray(t.tbl_indptr, dtype=np.int64)
+    pg = np.ascontiguousarray(t.tbl_pages, dtype=np.int32)
+    co = np.ascontiguousarray(t.cluster_of, dtype=np.int32)
+    so = np.ascontiguousarray(t.slot_of, dtype=np.int32)
+    _c().tangram_oracle_attend_range(
+        _p(qb), _p(pb), _p(ip), _p(pg), _p(co), _p(so),
+        ctypes.c_int32(t.R), ctypes.c_int32(t.H), ctypes.c_int32(Hq), ctypes.c_int32(t.C),
+        ctypes.c_int32(t.Hp), ctypes.c_int32(t.P), ctypes.c_int32(d), ctypes.c_int32(r),
+        ctypes.c_int32(j), ctypes.c_int32(t0), ctypes.c_int32(t1), _p(out), ctypes.byref(lse))
+    return out, float(lse.value)

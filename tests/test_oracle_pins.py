@@ -1,0 +1,427 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no product
+code).  Each pin is chosen so that a plausible mistake in the oracle (dropped term, wrong sign
+or index, transposed operand, wrong scale) fails at least one of them.  SURVEY.md §8(c) "Pins".
+"""
+import itertools
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import tangram_oracle as O
+from paper_2606_06302_b200 import inputs as I
+
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "hand_examples.json")))
+
+
+def bf16(x):
+    return torch.as_tensor(np.asarray(x), dtype=torch.float32).bfloat16()
+
+
+# ---------------------------------------------------------------------------- helpers
+def scatter_dense_into_pool(K, V, kv_len, t, n_pool_pages, fill=None, seed=0):
+    """Independent inverse of the oracle's gather: write dense K,V [R][H][n][d] (bf16 tensors)
+    page by page into a pool laid out [page][slot][kv][token][d].  Unwritten slots get random
+    garbage (or `fill`)."""
+    R, H, P = t.R, t.H, t.P
+    d = K[0][0].shape[-1]
+    g = torch.Generator().manual_seed(seed)
+    pool = torch.randn(n_pool_pages, t.Hp, 2, P, d, generator=g).bfloat16()
+    if fill is not None:
+        pool[:] = fill
+    for r in range(R):
+        for h in range(H):
+            n = int(kv_len[r][h])
+            row = t.tbl_pages[t.tbl_indptr[r * t.C + t.cluster_of[h]]:
+                              t.tbl_indptr[r * t.C + t.cluster_of[h] + 1]]
+            for pi in range((n + P - 1) // P):
+                lo, hi = pi * P, min(n, (pi + 1) * P)
+                pool[int(row[pi]), int(t.slot_of[h]), 0, :hi - lo] = K[r][h][lo:hi]
+                pool[int(row[pi]), int(t.slot_of[h]), 1, :hi - lo] = V[r][h][lo:hi]
+    return pool
+
+
+def simple_tables(kv_len, H, C, P, B=None, free=None):
+    """Tables sized exactly by kv_len (reserved := kv_len)."""
+    kv_len = np.asarray(kv_len, dtype=np.int32)
+    R = kv_len.shape[0]
+    if B is None:
+        B = np.linspace(0.1, 1.0, H)
+    n_pages = int(sum(-(-int(kv_len[r].max()) // P) for r in range(R)) * C + 8)
+    if free is None:
+        free = np.random.default_rng(1).permutation(n_pages).astype(np.int32)
+    t, _ = O.build_ragged_tables(B, kv_len, C, P, free)
+    return t, n_pages
+
+
+def dense_case(R, H, G, d, lens, seed, C=1, P=16, B=None):
+    g = torch.Generator().manual_seed(seed)
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    K = [[torch.randn(int(lens[r][h]), d, generator=g).bfloat16() for h in range(H)] for r in range(R)]
+    V = [[torch.randn(int(lens[r][h]), d, generator=g).bfloat16() for h in range(H)] for r in range(R)]
+    t, n_pages = simple_tables(lens, H, C, P, B=B)
+    pool = scatter_dense_into_pool(K, V, lens, t, n_pages, seed=seed + 1)
+    return q, K, V, t, pool
+
+
+# ---------------------------------------------------------------------------- O2 reserve
+@pytest.mark.parametrize("case", GOLD["reserve"])
+def test_reserve_golden(case):
+    B, res, kv = O.reserve_budgets(case["mu"], case["sigma"], case["alpha"], case["ctx_len"])
+    assert B.tolist() == case["B"]
+    assert res.tolist() == case["reserved"]
+    assert kv.tolist() == case["reserved"]
+
+
+def test_reserve_invariants_and_overflow():
+    rng = np.random.default_rng(3)
+    mu = rng.uniform(0.01, 1.0, 16)
+    sg = rng.uniform(0, 0.1, 16)
+    N = rng.integers(1, 5000, 9)
+    dem = rng.integers(0, 5000, (9, 16))
+    B, res, kv = O.reserve_budgets(mu, sg, 2.0, N, dem)
+    assert np.all((B > 0) & (B <= 1))
+    assert np.all(res >= 1) and np.all(res <= N[:, None])
+    assert np.all(kv <= res) and np.all(kv <= dem) and np.all((kv == res) | (kv == dem))
+    # monotone in B for a fixed N
+    order = np.argsort(B)
+    assert np.all(np.diff(res[:, order], axis=1) >= 0)
+    # sigma = 0: sum_h ceil(B N) within [rho H N, rho H N + H)   (:160, "approximately")
+    B0, res0, _ = O.reserve_budgets(mu, np.zeros(16), 2.0, N)
+    exact = N[:, None] * mu[None, :]
+    slack = res0.sum(1) - exact.sum(1)
+    assert np.all(slack >= -1e-9) and np.all(slack < 16)
+    with pytest.raises(ValueError):
+        O.reserve_budgets([0.0], [0.0], 2.0, [10])
+    with pytest.raises(ValueError):
+        O.reserve_budgets([0.5], [0.0], 2.0, [0])
+
+
+# ---------------------------------------------------------------------------- O3 clustering / tables
+def test_cluster_properties_and_ties():
+    B = np.array([0.5, 0.1, 0.5, 0.9, 0.1, 0.3, 1.0, 0.3])
+    perm, cl, sl = O.cluster_heads(B, 4)
+    assert sorted(perm.tolist()) == list(range(8))
+    assert perm.tolist() == [1, 4, 5, 7, 0, 2, 3, 6]          # stable: ties keep head order
+    assert cl.tolist() == [2, 0, 2, 3, 0, 1, 3, 1]
+    assert sl.tolist() == [0, 0, 1, 0, 1, 0, 1, 1]
+    for c in range(3):                                          # max of group i <= min of group i+1
+        assert B[perm[2 * c:2 * c + 2]].max() <= B[perm[2 * c + 2:2 * c + 4]].min()
+    p2, c2, s2 = O.cluster_heads(np.full(8, 0.4), 2)            # equal budgets => identity
+    assert p2.tolist() == list(range(8)) and c2.tolist() == [0] * 4 + [1] * 4
+    with pytest.raises(ValueError):
+        O.cluster_heads(B, 3)
+
+
+@pytest.mark.parametrize("H,Hp", [(4, 2), (6, 2), (6, 3), (8, 4), (8, 2)])
+def test_sorted_grouping_minimises_allocation_bruteforce(H, Hp):
+    """Sorted-consecutive grouping minimises sum_c H_p * max_c B over ALL equal-size partitions
+    (the claim behind Budget-Aware Clustering)."""
+    rng = np.random.default_rng(H * 10 + Hp)
+    B = rng.uniform(0.01, 1.0, H)
+    perm, cl, _ = O.cluster_heads(B, H // Hp)
+    ours = sum(Hp * B[perm[c * Hp:(c + 1) * Hp]].max() for c in range(H // Hp))
+
+    def parts(rest):
+        if not rest:
+            yield []
+            return
+        first = rest[0]
+        for combo in itertools.combinations(rest[1:], Hp - 1):
+            grp = (first,) + combo
+            left = [x for x in rest if x not in grp]
+            for p in parts(left):
+                yield [grp] + p
+
+    best = min(sum(Hp * max(B[list(g)]) for g in p) for p in parts(list(range(H))))
+    assert ours <= best + 1e-12
+
+
+def test_tables_structure():
+    wl = I.make_workload("8b", R=3, ctx_div=16)
+    B, res, kv = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    free = I.make_free_pages(wl, 4000)
+    t, kv2 = O.build_ragged_tables(B, res, wl.C, wl.P, free, 0, kv)
+    assert np.array_equal(kv2, kv)
+    assert len(set(t.tbl_pages.tolist())) == len(t.tbl_pages) == t.n_pages_used
+    assert np.array_equal(t.tbl_pages, free[:t.n_pages_used])         # prefix of the free list, in order
+    for r in range(wl.R):
+        for c in range(wl.C):
+            members = t.perm[c * t.Hp:(c + 1) * t.Hp]
+            want = -(-int(res[r, members].max()) // wl.P)
+            assert t.tbl_indptr[r * wl.C + c + 1] - t.tbl_indptr[r * wl.C + c] == want
+    # H_p = H: one table per request sized by the global max (the monolithic page, :89/:188)
+    t1, _ = O.build_ragged_tables(B, res, 1, wl.P, free)
+    assert [int(x) for x in np.diff(t1.tbl_indptr)] == [-(-int(res[r].max()) // wl.P) for r in range(wl.R)]
+    assert t1.n_pages_used * t1.Hp >= t.n_pages_used * t.Hp - wl.R * wl.C * t.Hp   # bytes: ragged <= monolithic (+ page rounding)
+    # FILL_GROUP (:235)
+    _, kvf = O.build_ragged_tables(B, res, wl.C, wl.P, free, O.FLAG_FILL_GROUP, kv)
+    for r in range(wl.R):
+        for h in range(wl.H):
+            members = t.perm[t.cluster_of[h] * t.Hp:(t.cluster_of[h] + 1) * t.Hp]
+            assert kvf[r, h] == res[r, members].max() <= wl.ctx_len[r]
+    with pytest.raises(MemoryError):
+        O.build_ragged_tables(B, res, wl.C, wl.P, free[:t.n_pages_used - 1])
+
+
+# ---------------------------------------------------------------------------- O4 plans
+@pytest.mark.parametrize("case", GOLD["split_map"])
+def test_split_map_golden(case):
+    B = np.array(case["B"])
+    perm, _, _ = O.cluster_heads(B, len(B) // case["Hp"])
+    assert O.split_map(B, perm, case["Hp"], case["n_cta"]).tolist() == case["S"]
+
+
+def test_split_map_scale_invariance_and_zero():
+    B = np.array([0.05, 0.05, 0.1, 0.1, 0.2, 0.3, 0.9, 1.0])
+    perm, _, _ = O.cluster_heads(B, 4)
+    for lam in (0.5, 0.25, 0.125):            # ratios only (:254); dyadic lam keeps fp exact
+        assert O.split_map(lam * B, perm, 2, 108).tolist() == O.split_map(B, perm, 2, 108).tolist()
+    assert O.split_map(np.zeros(8), perm, 2, 108).tolist() == [1, 1, 1, 1]
+
+
+def _one_request_tables(lens, P=16):
+    H = len(lens)
+    B = np.linspace(0.1, 0.9, H)              # increasing => identity perm, seq i = head i
+    t, _ = simple_tables([lens], H, 1, P, B=B)
+    return t, B
+
+
+@pytest.mark.parametrize("case", GOLD["balanced"])
+def test_balanced_golden(case):
+    t, B = _one_request_tables(case["kv_len"])
+    pl = O.plan_partitions(t, B, [case["kv_len"]], case["W"], case["g"], case["c0"], O.MODE_BALANCED)
+    got = [[[int(it[1]), int(it[4]), int(it[5])] for it in pl.items[pl.worker_indptr[w]:pl.worker_indptr[w + 1]]]
+           for w in range(case["W"])]
+    assert got == case["workers"]
+
+
+def check_plan_valid(pl, t, kv_len, g):
+    """Every token of every (r, h) is covered exactly once; slots and counts are consistent."""
+    kv_len = np.asarray(kv_len)
+    cover = {}
+    for it in pl.items:
+        r, h, c, s, tb, te, slot, npart = (int(x) for x in it)
+        assert c == t.cluster_of[h] and s == t.slot_of[h]
+        assert 0 <= tb < te <= kv_len[r, h]
+        assert tb % g == 0 and (te % g == 0 or te == kv_len[r, h])
+        cover.setdefault((r, h), []).append((tb, te, slot, npart))
+    seen_slots = set()
+    for r in range(t.R):
+        for h in range(t.H):
+            lst = sorted(cover.get((r, h), []))
+            n = int(kv_len[r, h])
+            seq = r * t.H + h
+            assert pl.part_indptr[seq + 1] - pl.part_indptr[seq] == len(lst)
+            pos = 0
+            for o, (tb, te, slot, npart) in enumerate(lst):
+                assert tb == pos and npart == len(lst) and slot == pl.part_indptr[seq] + o
+                assert slot not in seen_slots
+                seen_slots.add(slot)
+                pos = te
+            assert pos == n
+    assert pl.n_part_slots == pl.part_indptr[-1] == pl.n_items == len(pl.items)
+    assert pl.worker_indptr[0] == 0 and pl.worker_indptr[-1] == pl.n_items
+    assert np.all(np.diff(pl.worker_indptr) >= 0)
+
+
+@pytest.mark.parametrize("mode", [O.MODE_BALANCED, O.MODE_SPLITMAP, O.MODE_STATIC_EVEN])
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("8b", dict(R=4, ctx_div=8)), ("skew", dict(R=2, ctx_div=8)),
+                                     ("uniform", dict(R=8, ctx_div=4)), ("32b", dict(R=5, ctx_div=8))])
+def test_plan_invariants(name, kw, mode):
+    wl = I.make_workload(name, **kw)
+    B, res, kv = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    t, _ = O.build_ragged_tables(B, res, wl.C, wl.P, np.arange(200000, dtype=np.int32))
+    for W, c0 in ((4, 0), (37, 1), (296, 2)):
+        pl = O.plan_partitions(t, B, kv, W, wl.granule, c0, mode)
+        check_plan_valid(pl, t, kv, wl.granule)
+        pl2 = O.plan_partitions(t, B, kv, W, wl.granule, c0, mode)
+        assert pl.items.tobytes() == pl2.items.tobytes()             # deterministic
+        if mode == O.MODE_BALANCED:
+            assert pl.n_items <= wl.R * wl.H + W - 1
+            u = -(-kv.astype(np.int64) // wl.granule)
+            T = int((u + np.where(u > 0, c0, 0)).sum())
+            for w in range(W):
+                its = pl.items[pl.worker_indptr[w]:pl.worker_indptr[w + 1]]
+                gran = sum(-(-(int(it[5]) - int(it[4])) // wl.granule) for it in its)
+                assert gran <= T / W + 1                              # never more than the fair share (+ rounding)
+                assert gran >= T // W - (c0 * (len(its) + 1)) - 1     # overhead positions carry no tokens
+
+
+def test_balanced_equal_lengths_even_tokens():
+    lens = [[256] * 8] * 4                     # 32 sequences x 4 granules = 128; W = 16 divides it
+    B = np.full(8, 0.5)
+    t, _ = simple_tables(lens, 8, 2, 16, B=B)
+    pl = O.plan_partitions(t, B, lens, 16, 64, 0, O.MODE_BALANCED)
+    tok = [sum(int(it[5] - it[4]) for it in pl.items[pl.worker_indptr[w]:pl.worker_indptr[w + 1]]) for w in range(16)]
+    assert tok == [512] * 16
+    plw = O.plan_partitions(t, B, lens, 1000, 64, 0, O.MODE_BALANCED)   # W > T: empty workers allowed
+    check_plan_valid(plw, t, np.array(lens), 64)
+    assert plw.n_items == 128
+
+
+def test_static_even_default_and_splitmap_expansion():
+    lens = [[640, 64, 100, 0]]
+    B = np.array([0.9, 0.1, 0.2, 0.05])
+    t, _ = simple_tables(lens, 4, 2, 16, B=B)
+    pl = O.plan_partitions(t, B, lens, 16, 64, 0, O.MODE_STATIC_EVEN)      # S = ceil(16/4) = 4
+    assert pl.split_map.tolist() == [4, 4]
+    check_plan_valid(pl, t, np.array(lens), 64)
+    by = {}
+    for it in pl.items:
+        by.setdefault(int(it[1]), []).append((int(it[4]), int(it[5])))
+    assert sorted(by[0]) == [(0, 128), (128, 320), (320, 448), (448, 640)]   # 10 granules -> 2,3,2,3
+    assert by[1] == [(0, 64)] and sorted(by[2]) == [(0, 64), (64, 100)] and 3 not in by
+    # SPLITMAP: perm = [3,1,2,0]; Phi = [.15, 1.1]; tau = 1.25/16 -> S = [2, 14]
+    pls = O.plan_partitions(t, B, lens, 16, 64, 0, O.MODE_SPLITMAP)
+    assert pls.split_map.tolist() == [2, 14]
+    check_plan_valid(pls, t, np.array(lens), 64)
+    # items dealt round-robin in global order: item k -> worker k mod W
+    assert [int(x) for x in np.diff(pls.worker_indptr)] == [1] * pls.n_items + [0] * (16 - pls.n_items)
+
+
+# ---------------------------------------------------------------------------- O5 merge
+def test_merge_properties():
+    rng = np.random.default_rng(5)
+    parts = [(rng.normal(size=8), float(rng.normal())) for _ in range(5)]
+    o, L = O.merge(parts)
+    o1, L1 = O.merge([parts[0]])
+    assert np.array_equal(o1, parts[0][0]) and L1 == parts[0][1]           # one part is returned unchanged
+    o2, L2 = O.merge(parts[::-1])                                          # commutative
+    assert np.allclose(o, o2, rtol=0, atol=1e-14) and abs(L - L2) < 1e-14
+    oa, La = O.merge([O.merge(parts[:2]), O.merge(parts[2:])])             # associative
+    assert np.allclose(o, oa, rtol=0, atol=1e-14) and abs(L - La) < 1e-14
+    oi, Li = O.merge(parts + [(np.full(8, np.nan), -math.inf)])            # -inf part is the identity
+    assert np.array_equal(o, oi) and L == Li
+    # independent closed form: weights softmax(lse)
+    lses = np.array([p[1] for p in parts])
+    w = np.exp(lses) / np.exp(lses).sum()
+    assert np.allclose(o, sum(wi * p[0] for wi, p in zip(w, parts)), atol=1e-14)
+    assert abs(L - math.log(np.exp(lses).sum())) < 1e-14
+    z, Lz = O.merge([(np.zeros(4), -math.inf)])
+    assert np.all(z == 0) and Lz == -math.inf
+
+
+# ---------------------------------------------------------------------------- O1 attention
+def test_attention_vs_dense_library_equal_budgets():
+    """(i) all budgets equal => dense fp64 softmax(QK^T/sqrt(d))V on contiguous arrays (torch)."""
+    R, H, G, d, n = 3, 4, 3, 64, 197
+    lens = [[n] * H] * R
+    q, K, V, t, pool = dense_case(R, H, G, d, lens, seed=11, C=2, B=np.full(H, 0.5))
+    out, lse, _ = O.attention(q, pool, t, lens, H * G, d)
+    Kd = torch.stack([torch.stack(K[r]) for r in range(R)]).double()      # [R,H,n,d]
+    Vd = torch.stack([torch.stack(V[r]) for r in range(R)]).double()
+    qd = q.double().view(R, H, G, d)
+    ref = torch.nn.functional.scaled_dot_product_attention(qd, Kd, Vd)      # [R,H,G,d], scale 1/sqrt(d)
+    s = torch.einsum("rhgd,rhnd->rhgn", qd, Kd) / math.sqrt(d)
+    assert np.allclose(out, ref.reshape(R, H * G, d).numpy(), rtol=0, atol=1e-12)
+    assert np.allclose(lse, torch.logsumexp(s, -1).reshape(R, H * G).numpy(), rtol=0, atol=1e-12)
+
+
+def test_attention_vs_bruteforce_ragged():
+    """(ii) brute force without max-subtraction, pure Python loops, ragged lengths, GQA 5."""
+    R, H, G, d = 2, 4, 5, 64
+    lens = [[33, 1, 16, 50], [7, 64, 0, 17]]
+    q, K, V, t, pool = dense_case(R, H, G, d, lens, seed=12, C=2)
+    out, lse, _ = O.attention(q, pool, t, lens, H * G, d)
+    for r in range(R):
+        for j in range(H * G):
+            h = j // G
+            n = lens[r][h]
+            if n == 0:
+                assert np.all(out[r, j] == 0) and lse[r, j] == -math.inf
+                continue
+            qv = q[r, j].double().numpy()
+            Kn, Vn = K[r][h].double().numpy(), V[r][h].double().numpy()
+            e = [math.exp(sum(qv[x] * Kn[tk][x] for x in range(d)) / math.sqrt(d)) for tk in range(n)]
+            Z = sum(e)
+            ref = [sum(e[tk] * Vn[tk][x] for tk in range(n)) / Z for x in range(d)]
+            assert np.allclose(out[r, j], ref, rtol=0, atol=1e-12)
+            assert abs(lse[r, j] - math.log(Z)) < 1e-12
+
+
+def test_attention_closed_forms():
+    cf = GOLD["attention_closed_forms"]
+    d, H, G = 64, 2, 2
+    # n = 1  =>  out = v0, lse = q.k0/sqrt(d)
+    q, K, V, t, pool = dense_case(1, H, G, d, [[1, 1]], seed=13)
+    out, lse, _ = O.attention(q, pool, t, [[1, 1]], H * G, d)
+    for j in range(H * G):
+        assert np.array_equal(out[0, j], V[0][j // G][0].double().numpy())
+        want = float(q[0, j].double() @ K[0][j // G][0].double()) / 8.0
+        assert abs(lse[0, j] - want) < 1e-13
+    # q = 0 => out = mean(v), lse = ln n
+    n = 512
+    q, K, V, t, pool = dense_case(1, H, G, d, [[n, n]], seed=14)
+    out, lse, _ = O.attention(torch.zeros_like(q), pool, t, [[n, n]], H * G, d)
+    assert np.allclose(lse, cf[1]["lse_n512"], rtol=0, atol=1e-12)
+    assert np.allclose(out[0, 0], V[0][0].double().mean(0).numpy(), atol=1e-13)
+    # pins the 1/sqrt(d) scale and the natural log: q = 8 e0, k0 = e0, k1 = 0, v0 = 1, v1 = 0
+    qq = torch.zeros(1, H * G, d).bfloat16()
+    qq[0, :, 0] = 8.0
+    Kc = [[torch.zeros(2, d).bfloat16() for _ in range(H)]]
+    Vc = [[torch.zeros(2, d).bfloat16() for _ in range(H)]]
+    for h in range(H):
+        Kc[0][h][0, 0] = 1.0
+        Vc[0][h][0, :] = 1.0
+    t2, npg = simple_tables([[2, 2]], H, 1, 16)
+    pool2 = scatter_dense_into_pool(Kc, Vc, [[2, 2]], t2, npg)
+    out, lse, _ = O.attention(qq, pool2, t2, [[2, 2]], H * G, d)
+    assert np.allclose(out, cf[0]["w0"], rtol=0, atol=1e-15) and np.allclose(lse, cf[0]["lse"], rtol=0, atol=1e-15)
+    # V_h == h + 1 => out_j = floor(j / G) + 1 (pins the GQA map, reading A20) -- G = 3, H = 4
+    H4, G3 = 4, 3
+    lens = [[40, 9, 23, 31]]
+    q, K, V, t, pool = dense_case(1, H4, G3, d, lens, seed=15, C=2)
+    Vh = [[torch.full((lens[0][h], d), float(h + 1)).bfloat16() for h in range(H4)]]
+    pool = scatter_dense_into_pool(K, Vh, lens, t, pool.shape[0])
+    out, _, _ = O.attention(q, pool, t, lens, H4 * G3, d)
+    for j in range(H4 * G3):
+        assert np.allclose(out[0, j], j // G3 + 1, rtol=0, atol=1e-12)
+
+
+def test_split_then_merge_equals_unsplit():
+    """(iv) any partition of [0, n) merged by O5 equals the unsplit result."""
+    R, H, G, d = 2, 2, 4, 128
+    lens = [[300, 45], [77, 129]]
+    q, K, V, t, pool = dense_case(R, H, G, d, lens, seed=16)
+    out, lse, _ = O.attention(q, pool, t, lens, H * G, d)
+    rng = np.random.default_rng(17)
+    for r in range(R):
+        for j in range(H * G):
+            n = lens[r][j // G]
+            cuts = sorted(set(rng.integers(0, n + 1, size=4).tolist()) | {0, n})
+            parts = [O.attend_range(q, pool, t, H * G, d, r, j, a, b) for a, b in zip(cuts[:-1], cuts[1:])]
+            parts.append(O.attend_range(q, pool, t, H * G, d, r, j, n, n))         # an empty part
+            o, L = O.merge(parts)
+            assert np.allclose(o, out[r, j], rtol=0, atol=1e-12) and abs(L - lse[r, j]) < 1e-12
+
+
+def test_page_permutation_invariance():
+    """(v) same logical KV under a different physical page assignment: bit-identical in fp64."""
+    R, H, G, d = 2, 4, 2, 64
+    lens = np.array([[100, 20, 64, 3], [16, 90, 33, 48]], dtype=np.int32)
+    g = torch.Generator().manual_seed(18)
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    K = [[torch.randn(int(lens[r][h]), d, generator=g).bfloat16() for h in range(H)] for r in range(R)]
+    V = [[torch.randn(int(lens[r][h]), d, generator=g).bfloat16() for h in range(H)] for r in range(R)]
+    B = np.array([0.9, 0.2, 0.6, 0.3])
+    res = []
+    for seed in (1, 2):
+        free = np.random.default_rng(seed).permutation(64).astype(np.int32)
+        t, _ = O.build_ragged_tables(B, lens, 2, 16, free)
+        pool = scatter_dense_into_pool(K, V, lens, t, 64, seed=seed)               # different garbage too
+        res.append(O.attention(q, pool, t, lens, H * G, d)[:2])
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+def test_slack_is_never_read():
+    """NaN in every slot outside [0, kv_len) must not reach the output (reading A28)."""
+    R, H, G, d = 1, 4, 2, 64
+    lens = [[70, 5, 33, 16]]
+    q, K, V, t, _ = dense_case(R, H, G, d, lens, seed=19, C=2)
+    pool = scatter_dense_into_pool(K, V, lens, t, 32, fill=float("nan"))
+    out, lse, _ = O.attention(q, pool, t, lens, H * G, d)
+    assert np.all(np.isfinite(out)) and np.all(np.isfinite(lse))
