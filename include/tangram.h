@@ -1,0 +1,199 @@
+/*
+ * tangram.h -- C ABI of the B200-native Tangram hot path (arxiv/paper_2606_06302; citations are
+ * lines of the paper text, PAPER.md, with the section / equation / algorithm they fall in).
+ *
+ * The path: decode-step attention over a KV cache that was compressed non-uniformly (every KV
+ * head keeps its own token budget), stored through Ragged Paging (§4.2) and
+ * executed from an Ahead-of-Time work list (§4.3), followed by a log-sum-exp
+ * merge of the split-KV partials.
+ *
+ * Conventions
+ *  - Every call returns TANGRAM_OK (0) or a negative TANGRAM_ERR_* code; a description of the last
+ *    error of the calling thread is returned by tangram_last_error().  Nothing throws across the ABI.
+ *  - The CALLER owns every buffer, host and device.  The library allocates no device memory.
+ *  - "host" / "device" is stated per pointer.  Host calls (reserve, build tables, plan) are pure,
+ *    deterministic functions of their arguments, thread-safe, and need no CUDA context.
+ *  - Variable-size outputs use query-then-fill: call with the output array NULL to get the counts
+ *    in the struct, allocate, call again.
+ *  - fp64 expressions are evaluated exactly as written (no FMA contraction); integer results are
+ *    bit-exact against the CPU oracle (oracle/tangram_oracle.py).
+ */
+#ifndef TANGRAM_H_
+#define TANGRAM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TANGRAM_OK 0
+#define TANGRAM_ERR_INVALID_ARG (-1)
+#define TANGRAM_ERR_OUT_OF_PAGES (-2)
+#define TANGRAM_ERR_BUFFER_TOO_SMALL (-3)
+#define TANGRAM_ERR_CUDA (-4)
+
+/* Thread-local, never NULL; valid until the next failing call on the same thread. */
+const char* tangram_last_error(void);
+
+/* ------------------------------------------------------------------------------------------------
+ * a1  Budget Reservation -- PAPER.md:156-158 (Eq. 5: B = min(1, mu + alpha*sigma)), :152-154
+ *     (Eq. 4: per-head top-ceil(B N)), :172-174 (Precise Page Allocation: the scheduler reserves
+ *     exactly the post-compression footprint at admission), :176 (overflow: a head that demands
+ *     more than its budget keeps the top entries within capacity).
+ *
+ *   mu, sigma    host [H] f64   calibrated mean / std of each KV head's implicit retention ratio
+ *   alpha        safety-margin coefficient (the paper uses 2, :262)
+ *   ctx_len      host [R] i32   pre-compression context length N_r >= 1
+ *   demand       host [R][H] i32 or NULL: tokens the compressor would retain for this input (>= 0)
+ *   B_out        host [H] f64   B_h = min(1.0, mu_h + alpha*sigma_h), one multiply then one add
+ *   reserved_out host [R][H] i32  ceil(B_h * N_r) clamped to [1, N_r]
+ *   kv_len_out   host [R][H] i32  min(demand, reserved), or reserved if demand == NULL
+ * Errors: INVALID_ARG if H < 1, R < 1, ctx_len < 1, demand < 0, or mu + alpha*sigma <= 0 (B must
+ * be in (0,1], :152); nothing is written then. */
+int tangram_reserve_budgets(const double* mu, const double* sigma, double alpha, int32_t H,
+                            const int32_t* ctx_len, int32_t R, const int32_t* demand,
+                            double* B_out, int32_t* reserved_out, int32_t* kv_len_out);
+
+/* ------------------------------------------------------------------------------------------------
+ * a2  Ragged Paging -- PAPER.md:190 (a page holds H_p x 2 x P x d elements of one head group in
+ *     one layer; each group owns a page table sized by its max budget), :192-194 and :227-233
+ *     (Budget-Aware Clustering: sort heads by budget ascending, H_p consecutive heads = group),
+ *     :235 (slack: smaller-budget heads may keep extra KV up to the group's budget).
+ *
+ * Heads are stably sorted by B (ties keep head order); cluster c = sorted positions
+ * [c*H_p, (c+1)*H_p); row (r, c) of the tables has ceil(max_{h in c} reserved[r][h] / P) pages and
+ * takes the next entries of free_pages in order, rows visited r-major then c.  Page layout in the
+ * pool (bf16): pool[page][slot][kv][token][d], kv 0 = K, 1 = V, slot = slot_of[head].
+ *
+ *   B            host [H] f64 (from a1)            reserved  host [R][H] i32 (from a1)
+ *   free_pages   host [n_free] i32 page ids the caller's allocator hands out (not modified)
+ *   flags        TANGRAM_FILL_GROUP: kv_len_inout[r][h] := max reserved of h's cluster (:235)
+ *   kv_len_inout host [R][H] i32 or NULL (only touched with TANGRAM_FILL_GROUP)
+ *   out          caller-filled: perm/cluster_of/slot_of [H], tbl_indptr [R*C+1], tbl_pages
+ *                [tbl_pages_cap] (or tbl_pages == NULL to query: only n_pages_used is written).
+ *                On success R,H,C,Hp,P, the arrays and n_pages_used are written.
+ * Errors: INVALID_ARG (H % n_clusters != 0, page_size <= 0, ...); OUT_OF_PAGES if the free list is
+ * too short (n_pages_used = pages needed; arrays untouched); BUFFER_TOO_SMALL if tbl_pages_cap <
+ * pages needed (n_pages_used = pages needed). */
+#define TANGRAM_FILL_GROUP 1u
+typedef struct tangram_tables {
+    int32_t R, H, C, Hp, P;
+    int32_t* perm;        /* host [H]  sorted position -> head (pi of :229) */
+    int32_t* cluster_of;  /* host [H]  head -> cluster */
+    int32_t* slot_of;     /* host [H]  head -> slot inside the cluster's pages */
+    int64_t* tbl_indptr;  /* host [R*C+1]  CSR row pointer, row = r*C + c */
+    int32_t* tbl_pages;   /* host [tbl_pages_cap]  page ids, row after row */
+    int64_t tbl_pages_cap;
+    int64_t n_pages_used;
+} tangram_tables;
+int tangram_build_ragged_tables(const double* B, const int32_t* reserved, int32_t R, int32_t H,
+                                int32_t n_clusters, int32_t page_size, const int32_t* free_pages,
+                                int64_t n_free, uint32_t flags, int32_t* kv_len_inout,
+                                tangram_tables* out);
+
+/* ------------------------------------------------------------------------------------------------
+ * a3  AoT Load Balancing -- PAPER.md:196-225 (Algorithm 1: S_i = max(1, round(Phi_i / tau)),
+ *     tau = Omega / N_CTA), :250-256 (the split map is computed offline from budget ratios; zero
+ *     runtime planning), :120 (static uniform num_splits is the straggler baseline).
+ *
+ * Offline, host-side, deterministic work-list builder.  Sequences (r, h) are visited r-major then
+ * in perm order.  A sequence of n = kv_len[r][h] tokens has ceil(n / g) granules.
+ *   TANGRAM_MODE_BALANCED   (primary; BASELINE.json north_star "chunks of near-equal KV bytes per
+ *       CTA"): the sequences are laid end to end, each preceded by `overhead_granules` cost units;
+ *       worker k owns positions [floor(k T / W), floor((k+1) T / W)); every maximal run of one
+ *       sequence's granules inside one worker is one item.
+ *   TANGRAM_MODE_SPLITMAP   (Algorithm 1, literal): every sequence of cluster c is cut into
+ *       split_map[c] granule-aligned chunks; item k (global order) goes to worker k mod W.
+ *   TANGRAM_MODE_STATIC_EVEN (baseline of :120): as SPLITMAP with the same split count for every
+ *       head: static_splits, or if <= 0 the smallest S with R*H*S >= W.
+ * Items of a worker are stored contiguously (worker_indptr), plan order kept.  part_slot numbers
+ * the items of a sequence in token order from part_indptr[r*H + h]; n_parts = their count
+ * (n_parts == 1: the decode kernel writes the final output directly, no merge).
+ *
+ *   t        tables from a2 (host)      B host [H]      kv_len host [R][H] i32 (<= cluster capacity)
+ *   n_workers W >= 1 (persistent CTAs, from tangram_query_max_ctas)
+ *   granule_tokens g: positive multiple of t->P;  overhead_granules c0 >= 0
+ *   out      caller-filled: split_map [C], worker_indptr [W+1], part_indptr [R*H+1], items
+ *            [items_cap] (or items == NULL to query: n_items / n_part_slots only).
+ *            split_map always receives Algorithm 1's S (the constant S for STATIC_EVEN).
+ * Errors: INVALID_ARG; BUFFER_TOO_SMALL (n_items = needed). */
+#define TANGRAM_MODE_BALANCED 0
+#define TANGRAM_MODE_SPLITMAP 1
+#define TANGRAM_MODE_STATIC_EVEN 2
+typedef struct tangram_item { /* 32 bytes */
+    int32_t req, kv_head, cluster, slot, tok_begin, tok_end, part_slot, n_parts;
+} tangram_item;
+typedef struct tangram_plan {
+    int32_t W, mode;
+    int64_t n_items, n_part_slots;
+    int32_t* split_map;     /* host [C] */
+    tangram_item* items;    /* host [items_cap], worker-major */
+    int64_t items_cap;
+    int64_t* worker_indptr; /* host [W+1] */
+    int64_t* part_indptr;   /* host [R*H+1], seq = r*H + h */
+} tangram_plan;
+int tangram_plan_partitions(const tangram_tables* t, const double* B, const int32_t* kv_len,
+                            int32_t n_workers, int32_t granule_tokens, int32_t overhead_granules,
+                            int32_t mode, int32_t static_splits, tangram_plan* out);
+
+/* ------------------------------------------------------------------------------------------------
+ * Device side.  One upload of tables + plan per (batch, layer); then one
+ * tangram_decode_attention per decode step with no host planning (:254 "zero runtime planning").
+ */
+
+/* N_CTA of :252 ("CUDAMaxOccupancy API ... CTAs the GPU can execute concurrently for the attention
+ * kernel") = SM count x resident CTAs per SM of the decode kernel for this head_dim / GQA group.
+ * Needs a CUDA device.  head_dim in {64, 128}, 1 <= gqa <= 8. */
+int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa, int32_t* n_cta_out);
+
+/* Bytes of the device blob that tangram_upload fills for these tables + plan. */
+size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan* p);
+
+/* Host-side view of an uploaded plan: sizes plus DEVICE pointers into the blob.  Plain data; valid
+ * as long as the blob is. */
+typedef struct tangram_device_plan {
+    int32_t R, H, C, Hp, P, W, mode, reserved_;
+    int64_t n_items, n_part_slots;
+    const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
+    const int64_t* worker_indptr; /* device [W+1] */
+    const int64_t* part_indptr;   /* device [R*H+1] */
+    const int32_t* tbl_pages;     /* device page ids */
+} tangram_device_plan;
+
+/* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte
+ * aligned) with cudaMemcpyAsync on `stream` (a cudaStream_t, may be NULL); fills *dp.  The host
+ * arrays may be freed when the call returns. */
+int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
+                   void* stream, tangram_device_plan* dp);
+
+/* Workspace for the split-KV partials: n_part_slots x G x (d + 1) fp32, rounded up. */
+size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_dim);
+
+/* a4 + a5  One layer, whole batch: split-KV decode kernel over the work list, then the LSE merge
+ * kernel.  Asynchronous on `stream`; CUDA-graph capturable; no host work besides the two launches.
+ *
+ *   dp        from tangram_upload (host struct holding device pointers)
+ *   q         device [R][Hq][d] bf16, 16-byte aligned
+ *   kv_pool   device [n_pool_pages][Hp][2][P][d] bf16, 128-byte aligned (Ragged page, :190)
+ *   Hq        query heads, Hq % H == 0, G = Hq / H <= 8 (query head j uses KV head floor(j / G))
+ *   d         64 or 128;  P must be 16
+ *   sm_scale  softmax scale; 0 means 1/sqrt(d)
+ *   out       device [R][Hq][d] bf16;  lse device [R][Hq] f32 (natural log of sum exp(scaled score);
+ *             -inf and out = 0 for a head with kv_len 0)
+ *   workspace device, >= tangram_workspace_bytes(dp->n_part_slots, G, d), 16-byte aligned
+ *   worker_ns device [W][2] u64 or NULL: if given, every worker CTA stores its globaltimer start /
+ *             end (the per-CTA elapsed-time spread of BASELINE.json is measured from these).
+ * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
+ * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
+ * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G), BUFFER_TOO_SMALL (workspace), CUDA. */
+int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                             int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                             float* lse, void* workspace, size_t workspace_bytes,
+                             uint64_t* worker_ns, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TANGRAM_H_ */

@@ -1,0 +1,244 @@
+"""Thin ctypes binding over libtangram.so (C ABI declared in include/tangram.h).
+
+Argument marshalling only: every step of the path (Budget Reservation, Ragged Paging tables, the
+AoT planner, the decode and merge kernels) runs inside the library.  Names mirror the C entry
+points.  There is no CPU fallback: if the library is missing this module raises on import, and the
+device calls raise TangramError on any CUDA problem.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtangram.so")
+
+OK, ERR_INVALID_ARG, ERR_OUT_OF_PAGES, ERR_BUFFER_TOO_SMALL, ERR_CUDA = 0, -1, -2, -3, -4
+FILL_GROUP = 1
+MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
+MODE_NAMES = {MODE_BALANCED: "balanced", MODE_SPLITMAP: "splitmap", MODE_STATIC_EVEN: "static_even"}
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_06302_b200.build` "
+                      "(there is no fallback path)")
+_lib = C.CDLL(LIB_PATH)
+
+
+class TangramError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"tangram error {code}: {msg}")
+        self.code = code
+
+
+class _Tables(C.Structure):
+    _fields_ = [("R", C.c_int32), ("H", C.c_int32), ("C", C.c_int32), ("Hp", C.c_int32), ("P", C.c_int32),
+                ("perm", C.c_void_p), ("cluster_of", C.c_void_p), ("slot_of", C.c_void_p),
+                ("tbl_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("tbl_pages_cap", C.c_int64),
+                ("n_pages_used", C.c_int64)]
+
+
+class _Plan(C.Structure):
+    _fields_ = [("W", C.c_int32), ("mode", C.c_int32), ("n_items", C.c_int64), ("n_part_slots", C.c_int64),
+                ("split_map", C.c_void_p), ("items", C.c_void_p), ("items_cap", C.c_int64),
+                ("worker_indptr", C.c_void_p), ("part_indptr", C.c_void_p)]
+
+
+class _DevicePlan(C.Structure):
+    _fields_ = [("R", C.c_int32), ("H", C.c_int32), ("C", C.c_int32), ("Hp", C.c_int32), ("P", C.c_int32),
+                ("W", C.c_int32), ("mode", C.c_int32), ("reserved_", C.c_int32), ("n_items", C.c_int64),
+                ("n_part_slots", C.c_int64), ("items", C.c_void_p), ("worker_indptr", C.c_void_p),
+                ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p)]
+
+
+_lib.tangram_last_error.restype = C.c_char_p
+_lib.tangram_blob_bytes.restype = C.c_size_t
+_lib.tangram_workspace_bytes.restype = C.c_size_t
+_lib.tangram_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
+for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
+              "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention"):
+    getattr(_lib, _name).restype = C.c_int
+
+EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
+           "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
+           "tangram_workspace_bytes", "tangram_decode_attention")
+
+
+def _check(rc: int):
+    if rc != OK:
+        raise TangramError(rc, _lib.tangram_last_error().decode())
+
+
+def _np(a, dtype) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=dtype))
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+# ------------------------------------------------------------------------------------------ a1
+def tangram_reserve_budgets(mu, sigma, alpha: float, ctx_len, demand=None):
+    """-> (B [H] f64, reserved [R,H] i32, kv_len [R,H] i32).  Eq. 5 / Eq. 4 / overflow rule."""
+    mu, sigma, ctx = _np(mu, np.float64), _np(sigma, np.float64), _np(ctx_len, np.int32)
+    H, R = mu.shape[0], ctx.shape[0]
+    dem = None if demand is None else _np(demand, np.int32).reshape(R, H)
+    B = np.zeros(H, np.float64)
+    reserved = np.zeros((R, H), np.int32)
+    kv_len = np.zeros((R, H), np.int32)
+    _check(_lib.tangram_reserve_budgets(_ptr(mu), _ptr(sigma), C.c_double(alpha), C.c_int32(H), _ptr(ctx),
+                                        C.c_int32(R), _ptr(dem), _ptr(B), _ptr(reserved), _ptr(kv_len)))
+    return B, reserved, kv_len
+
+
+# ------------------------------------------------------------------------------------------ a2
+@dataclasses.dataclass
+class Tables:
+    R: int
+    H: int
+    C: int
+    Hp: int
+    P: int
+    perm: np.ndarray
+    cluster_of: np.ndarray
+    slot_of: np.ndarray
+    tbl_indptr: np.ndarray
+    tbl_pages: np.ndarray
+    n_pages_used: int
+
+    def _c(self) -> _Tables:
+        return _Tables(self.R, self.H, self.C, self.Hp, self.P, _ptr(self.perm), _ptr(self.cluster_of),
+                       _ptr(self.slot_of), _ptr(self.tbl_indptr), _ptr(self.tbl_pages), len(self.tbl_pages),
+                       self.n_pages_used)
+
+
+def tangram_pages_needed(B, reserved, n_clusters: int, page_size: int) -> int:
+    """Query form of tangram_build_ragged_tables: pages the batch needs (no free list consumed)."""
+    B, reserved = _np(B, np.float64), _np(reserved, np.int32)
+    R, H = reserved.shape
+    t = _Tables()
+    rc = _lib.tangram_build_ragged_tables(_ptr(B), _ptr(reserved), C.c_int32(R), C.c_int32(H), C.c_int32(n_clusters),
+                                          C.c_int32(page_size), None, C.c_int64(0), C.c_uint32(0), None, C.byref(t))
+    if rc not in (OK, ERR_OUT_OF_PAGES):
+        _check(rc)
+    return int(t.n_pages_used)
+
+
+def tangram_build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages, flags: int = 0,
+                                kv_len=None):
+    """-> (Tables, kv_len').  kv_len' is a copy of kv_len (raised to the cluster capacity with FILL_GROUP)."""
+    B, reserved = _np(B, np.float64), _np(reserved, np.int32)
+    free = _np(free_pages, np.int32)
+    R, H = reserved.shape
+    kv = None if kv_len is None else _np(kv_len, np.int32).reshape(R, H).copy()
+    need = tangram_pages_needed(B, reserved, n_clusters, page_size)
+    t = Tables(R, H, n_clusters, H // max(1, n_clusters), page_size, np.zeros(H, np.int32), np.zeros(H, np.int32),
+               np.zeros(H, np.int32), np.zeros(R * n_clusters + 1, np.int64), np.zeros(max(need, 1), np.int32), 0)
+    ct = t._c()
+    _check(_lib.tangram_build_ragged_tables(_ptr(B), _ptr(reserved), C.c_int32(R), C.c_int32(H),
+                                            C.c_int32(n_clusters), C.c_int32(page_size), _ptr(free),
+                                            C.c_int64(free.shape[0]), C.c_uint32(flags), _ptr(kv), C.byref(ct)))
+    t.n_pages_used = int(ct.n_pages_used)
+    t.tbl_pages = t.tbl_pages[:t.n_pages_used]
+    t.Hp, t.C = int(ct.Hp), int(ct.C)
+    return t, kv
+
+
+# ------------------------------------------------------------------------------------------ a3
+@dataclasses.dataclass
+class Plan:
+    W: int
+    mode: int
+    split_map: np.ndarray      # [C]
+    items: np.ndarray          # [n_items, 8] i32: req, kv_head, cluster, slot, tok_begin, tok_end, part_slot, n_parts
+    worker_indptr: np.ndarray  # [W+1] i64
+    part_indptr: np.ndarray    # [R*H+1] i64
+    n_items: int
+    n_part_slots: int
+
+    def _c(self) -> _Plan:
+        return _Plan(self.W, self.mode, self.n_items, self.n_part_slots, _ptr(self.split_map), _ptr(self.items),
+                     self.items.shape[0], _ptr(self.worker_indptr), _ptr(self.part_indptr))
+
+
+def tangram_plan_partitions(t: Tables, B, kv_len, n_workers: int, granule_tokens: int, overhead_granules: int,
+                            mode: int, static_splits: int = 0) -> Plan:
+    B, kv = _np(B, np.float64), _np(kv_len, np.int32)
+    ct = t._c()
+    split_map = np.zeros(t.C, np.int32)
+    q = _Plan(0, 0, 0, 0, _ptr(split_map), None, 0, None, None)
+    args = (C.byref(ct), _ptr(B), _ptr(kv), C.c_int32(n_workers), C.c_int32(granule_tokens),
+            C.c_int32(overhead_granules), C.c_int32(mode), C.c_int32(static_splits))
+    _check(_lib.tangram_plan_partitions(*args, C.byref(q)))
+    pl = Plan(n_workers, mode, split_map, np.zeros((max(int(q.n_items), 1), 8), np.int32),
+              np.zeros(n_workers + 1, np.int64), np.zeros(t.R * t.H + 1, np.int64), int(q.n_items),
+              int(q.n_part_slots))
+    cp = pl._c()
+    _check(_lib.tangram_plan_partitions(*args, C.byref(cp)))
+    pl.items = pl.items[:pl.n_items]
+    return pl
+
+
+# ------------------------------------------------------------------------------------------ device side
+def tangram_query_max_ctas(device: int, head_dim: int, gqa: int) -> int:
+    n = C.c_int32(0)
+    _check(_lib.tangram_query_max_ctas(C.c_int(device), C.c_int32(head_dim), C.c_int32(gqa), C.byref(n)))
+    return int(n.value)
+
+
+def tangram_blob_bytes(t: Tables, p: Plan) -> int:
+    ct, cp = t._c(), p._c()
+    return int(_lib.tangram_blob_bytes(C.byref(ct), C.byref(cp)))
+
+
+def tangram_workspace_bytes(n_part_slots: int, gqa: int, head_dim: int) -> int:
+    return int(_lib.tangram_workspace_bytes(n_part_slots, gqa, head_dim))
+
+
+class DevicePlan:
+    """Uploaded tables + plan.  Keeps the device blob (a torch uint8 tensor) alive."""
+
+    def __init__(self, t: Tables, p: Plan, device="cuda", stream=None):
+        import torch
+        self.tables, self.plan = t, p
+        nbytes = tangram_blob_bytes(t, p)
+        self.blob = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        self.c = _DevicePlan()
+        ct, cp = t._c(), p._c()
+        sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+        _check(_lib.tangram_upload(C.byref(ct), C.byref(cp), C.c_void_p(self.blob.data_ptr()), C.c_size_t(nbytes), sp,
+                                   C.byref(self.c)))
+
+
+def tangram_upload(t: Tables, p: Plan, device="cuda", stream=None) -> DevicePlan:
+    return DevicePlan(t, p, device, stream)
+
+
+def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, workspace=None, sm_scale: float = 0.0,
+                             worker_ns=None, stream=None):
+    """q [R,Hq,d] bf16 cuda, kv_pool [n_pages,Hp,2,P,d] bf16 cuda -> (out [R,Hq,d] bf16, lse [R,Hq] f32).
+    Asynchronous on the current (or given) torch stream."""
+    import torch
+    assert q.is_cuda and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
+    assert q.is_contiguous() and kv_pool.is_contiguous()
+    R, Hq, d = q.shape
+    n_pages = kv_pool.shape[0]
+    assert tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d) and R == dp.c.R
+    G = Hq // dp.c.H
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty(R, Hq, dtype=torch.float32, device=q.device)
+    need = tangram_workspace_bytes(int(dp.c.n_part_slots), G, d)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    wn = C.c_void_p(worker_ns.data_ptr()) if worker_ns is not None else None
+    _check(_lib.tangram_decode_attention(C.byref(dp.c), C.c_void_p(q.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
+                                         C.c_int64(n_pages), C.c_int32(Hq), C.c_int32(d), C.c_float(sm_scale),
+                                         C.c_void_p(out.data_ptr()), C.c_void_p(lse.data_ptr()),
+                                         C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), wn, sp))
+    return out, lse

@@ -1,0 +1,625 @@
+// Tangram decode attention for B200 (sm_100a): split-KV decode kernel driven by the Ahead-of-Time
+// work list (a4) and the log-sum-exp merge kernel (a5).  Contract: include/tangram.h.
+//
+// Decode kernel, one persistent CTA per worker (one per SM):
+//   * warp 8 is the producer.  Lane 0 hands every item's descriptor and query group to the consumers
+//     through a 2-slot ring (cp.async.bulk of the contiguous G x d bf16 block).  Lanes 0-7 each feed
+//     the private tile ring of one consumer warp: one TMA tensor copy (cp.async.bulk.tensor, 128-byte
+//     swizzle) per (page, head) brings the page's K rows and V rows -- one contiguous 2*P*d*2-byte run
+//     of the ragged page pool[page][slot][kv][token][d] -- into shared memory and completes on that
+//     stage's mbarrier.  Page ids are read one round ahead; the producer runs ahead across item
+//     boundaries, so the HBM stream never drains between items.
+//   * warps 0-7 are consumers.  Tile i of an item goes to warp (i + rot) % 8.  Per tile (16 tokens):
+//     S = Q K^T with mma.sync m16n8k16 (bf16 in, fp32 accumulate; the GQA group sits in rows 0..G-1 of
+//     the 16-row A operand), fp32 online softmax in the exp2 domain with a warp-uniform lazy rescale,
+//     O += P V with V fragments from ldmatrix.trans.  At the end of an item the eight (m, l, O)
+//     states are combined through shared memory and the CTA writes either the final bf16 output
+//     (n_parts == 1) or an fp32 partial (o, lse).
+// The path is HBM-bound (4*d bytes per token-head against 4*d*G flop); the tensor cores are used
+// because at G = 4..5 the CUDA-core formulation would need ~50 warp instructions per 512 bytes and
+// B200 has only ~7 bytes of HBM bandwidth per issue slot.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+#include "tangram.h"
+#include "tangram_internal.h"
+
+namespace tangram {
+
+constexpr int kPage = 16;          // tokens per page the kernels are specialised for
+constexpr int kNW = 8;             // consumer warps
+constexpr int kThreads = (kNW + 1) * 32;
+constexpr int kQSlots = 2;         // item / query ring depth
+constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime <= this)
+constexpr int kMaxG = 8;
+constexpr int kSmemLimit = 232448; // 227 KB opt-in limit per CTA
+
+struct DecodeParams {
+    const DeviceItem* items;
+    const int64_t* worker_indptr;
+    const int32_t* tbl_pages;
+    const __nv_bfloat16* q;
+    __nv_bfloat16* out;
+    float* lse;
+    float* part_o;
+    float* part_lse;
+    unsigned long long* worker_ns;
+    int32_t Hq, G, Hp, n_stages;
+    float scale_log2;
+};
+
+// ------------------------------------------------------------------ shared-memory carve-up
+template <int D>
+struct Smem {
+    static constexpr int kTile = 2 * kPage * D * 2;          // K rows + V rows of one (page, head)
+    static constexpr int kHalf = 2 * kPage * 128;            // one 64-element column block of the tile
+    static constexpr int kRowF = D + 8;                      // padded fp32 row of the merge scratch
+    __host__ __device__ static int q_slot(int G) { return (G * D * 2 + 127) & ~127; }
+    __host__ __device__ static int off_q(int ns) { return kNW * ns * kTile; }
+    __host__ __device__ static int off_desc(int ns, int G) { return off_q(ns) + kQSlots * q_slot(G); }
+    __host__ __device__ static int off_scratch(int ns, int G) { return off_desc(ns, G) + kQSlots * 32; }
+    __host__ __device__ static int off_ml(int ns, int G) { return off_scratch(ns, G) + kNW * G * kRowF * 4; }
+    __host__ __device__ static int off_bar(int ns, int G) { return (off_ml(ns, G) + kNW * G * 8 + 15) & ~15; }
+    __host__ __device__ static int total(int ns, int G) {
+        return off_bar(ns, G) + (2 * kNW * kMaxStages + 2 * kQSlots) * 8 + 1024 /* base alignment slack */;
+    }
+    static int max_stages(int G) {
+        int ns = kMaxStages;
+        while (ns > 1 && total(ns, G) > kSmemLimit) --ns;
+        return ns;
+    }
+};
+
+// ------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_tile(uint32_t dst, const CUtensorMap* map, uint32_t bar, int row,
+                                              uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst),
+        "l"(map), "r"(0), "r"(row), "r"(0), "r"(bar), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr)
+                 : "memory");
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr)
+                 : "memory");
+}
+// D(16x8) += A(16x16) B(16x8), bf16 inputs, fp32 accumulate.  Only rows 0..7 of A are populated
+// (the GQA group), so a1 = a3 = 0 and the row 8..15 halves of the accumulator are discarded.
+__device__ __forceinline__ void mma_rows07(float& c0, float& c1, uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
+    float d2, d3;
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%10,%10};"
+        : "+f"(c0), "+f"(c1), "=f"(d2), "=f"(d3)
+        : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1), "f"(0.f));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+__device__ __forceinline__ void named_bar_sync(int id, int threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ unsigned long long globaltimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// ------------------------------------------------------------------ a4: split-KV decode kernel
+template <int D, bool TIMED>
+__global__ void __launch_bounds__(kThreads, 1)
+tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeParams p) {
+    using L = Smem<D>;
+    constexpr int kTile = L::kTile, kHalf = L::kHalf, kRowF = L::kRowF;
+    extern __shared__ uint8_t smem_raw[];
+    // 128-byte-swizzled TMA tiles need a 1024-byte aligned base
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+
+    const int NS = p.n_stages, G = p.G;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t it_begin = p.worker_indptr[blockIdx.x];
+    const int n_items = static_cast<int>(p.worker_indptr[blockIdx.x + 1] - it_begin);
+
+    const uint32_t tiles = smem_u32(smem);
+    uint8_t* q_ring = smem + L::off_q(NS);
+    uint8_t* desc_ring = smem + L::off_desc(NS, G);
+    float* scratch_o = reinterpret_cast<float*>(smem + L::off_scratch(NS, G));
+    float* scratch_ml = reinterpret_cast<float*>(smem + L::off_ml(NS, G));
+    const uint32_t bars = smem_u32(smem + L::off_bar(NS, G));
+    const int q_slot_bytes = L::q_slot(G);
+    auto full_bar = [&](int w, int s) { return bars + (w * kMaxStages + s) * 8; };
+    auto empty_bar = [&](int w, int s) { return bars + (kNW * kMaxStages + w * kMaxStages + s) * 8; };
+    auto qfull_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + s) * 8; };
+    auto qempty_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + kQSlots + s) * 8; };
+
+    if (TIMED && threadIdx.x == 0) p.worker_ns[2 * blockIdx.x] = globaltimer();
+    if (threadIdx.x == 0) {
+        for (int w = 0; w < kNW; ++w)
+            for (int s = 0; s < NS; ++s) {
+                mbar_init(full_bar(w, s), 1);
+                mbar_init(empty_bar(w, s), 1);
+            }
+        for (int s = 0; s < kQSlots; ++s) {
+            mbar_init(qfull_bar(s), 1);
+            mbar_init(qempty_bar(s), kNW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == kNW) {
+        // ============================== producer warp ==============================
+        uint64_t policy;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+        uint32_t stage = 0, phase = 0;  // lane w < 8 tracks consumer warp w's ring
+        int rot = 0;
+        DeviceItem next;
+        if (n_items > 0) next = p.items[it_begin];
+        for (int it = 0; it < n_items; ++it) {
+            const DeviceItem item = next;
+            if (it + 1 < n_items) next = p.items[it_begin + it + 1];
+            const int qs = it % kQSlots;
+            const uint32_t qpar = (it / kQSlots) & 1;
+            if (lane == 0) {
+                mbar_wait(qempty_bar(qs), qpar ^ 1);
+                *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = item;
+                const uint32_t qbytes = static_cast<uint32_t>(G * D * 2);
+                mbar_arrive_expect_tx(qfull_bar(qs), qbytes);
+                bulk_load(smem_u32(q_ring + qs * q_slot_bytes),
+                          p.q + (static_cast<size_t>(item.req) * p.Hq + static_cast<size_t>(item.kv_head) * G) * D,
+                          qbytes, qfull_bar(qs));
+            }
+            const int n_tiles = (item.tok_end - item.tok_begin + kPage - 1) / kPage;
+            if (lane < kNW) {
+                const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
+                int i = (lane - rot) & (kNW - 1);
+                int pid = i < n_tiles ? __ldg(ids + i) : 0;
+                while (i < n_tiles) {
+                    const int i_next = i + kNW;
+                    const int pid_next = i_next < n_tiles ? __ldg(ids + i_next) : 0;
+                    mbar_wait(empty_bar(lane, stage), phase ^ 1);
+                    mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
+                    tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
+                                  (pid * p.Hp + item.slot) * (2 * kPage), policy);
+                    if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
+                    i = i_next, pid = pid_next;
+                }
+            }
+            __syncwarp();
+            rot = (rot + n_tiles) & (kNW - 1);
+        }
+        return;
+    }
+
+    // ================================ consumer warps ================================
+    const int row = lane >> 2;  // query head inside the GQA group held by this quad (valid if < G)
+    const int qd = lane & 3;
+    const bool row_ok = row < G;
+    uint32_t stage = 0, phase = 0;
+    int rot = 0;
+    constexpr float kNegInf = -INFINITY;
+
+    for (int it = 0; it < n_items; ++it) {
+        const int qs = it % kQSlots;
+        mbar_wait(qfull_bar(qs), (it / kQSlots) & 1);
+        const DeviceItem item = *reinterpret_cast<const DeviceItem*>(desc_ring + qs * 32);
+        uint32_t qa[D / 16][2];
+        {
+            const uint8_t* qrow = q_ring + qs * q_slot_bytes + row * D * 2;
+#pragma unroll
+            for (int ks = 0; ks < D / 16; ++ks) {
+                qa[ks][0] = row_ok ? *reinterpret_cast<const uint32_t*>(qrow + (ks * 16 + qd * 2) * 2) : 0u;
+                qa[ks][1] = row_ok ? *reinterpret_cast<const uint32_t*>(qrow + (ks * 16 + 8 + qd * 2) * 2) : 0u;
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(qempty_bar(qs));
+
+        const int n_tok = item.tok_end - item.tok_begin;
+        const int n_tiles = (n_tok + kPage - 1) / kPage;
+        float m = kNegInf, l = 0.f;
+        float o[D / 8][2];
+#pragma unroll
+        for (int nt = 0; nt < D / 8; ++nt) o[nt][0] = o[nt][1] = 0.f;
+
+        for (int i = (warp - rot) & (kNW - 1); i < n_tiles; i += kNW) {
+            mbar_wait(full_bar(warp, stage), phase);
+            const uint32_t tb = tiles + (warp * NS + stage) * kTile;
+            const int valid = min(kPage, n_tok - i * kPage);
+            if (valid < kPage) {
+                // ragged tail: V rows of tokens that are not retained may hold anything (NaN
+                // included) and 0 * NaN would poison the PV product -- zero them.
+                if (lane < 8 * (D / 64))
+                    for (int rr = kPage + valid; rr < 2 * kPage; ++rr)
+                        asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(tb + (lane >> 3) * kHalf + rr * 128 +
+                                                                                   (lane & 7) * 16),
+                                     "r"(0u)
+                                     : "memory");
+                __syncwarp();
+            }
+            // ---- S = Q K^T : 16 (8 used) query rows x 16 tokens
+            float s[2][2] = {{0.f, 0.f}, {0.f, 0.f}};
+            {
+                const int tok = ((lane >> 4) << 3) + (lane & 7);
+                const uint32_t rbase = tb + tok * 128;
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const int ck = ((ks & 3) << 1) + ((lane >> 3) & 1);
+                    uint32_t b0, b1, b2, b3;
+                    ldsm_x4(rbase + (ks >> 2) * kHalf + ((ck ^ (tok & 7)) << 4), b0, b1, b2, b3);
+                    mma_rows07(s[0][0], s[0][1], qa[ks][0], qa[ks][1], b0, b1);
+                    mma_rows07(s[1][0], s[1][1], qa[ks][0], qa[ks][1], b2, b3);
+                }
+            }
+            // ---- online softmax (exp2 domain)
+            float tmax = kNegInf;
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const float x = s[nt][e] * p.scale_log2;
+                    s[nt][e] = (nt * 8 + qd * 2 + e < valid) ? x : kNegInf;
+                    tmax = fmaxf(tmax, s[nt][e]);
+                }
+            tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
+            tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
+            const float m_new = fmaxf(m, tmax);
+            if (__any_sync(0xffffffffu, m_new > m)) {
+                const float corr = exp2f(m - m_new);  // m = -inf on the first tile -> 0
+                l *= corr;
+#pragma unroll
+                for (int nt = 0; nt < D / 8; ++nt) o[nt][0] *= corr, o[nt][1] *= corr;
+                m = m_new;
+            }
+            const float p00 = exp2f(s[0][0] - m), p01 = exp2f(s[0][1] - m);
+            const float p10 = exp2f(s[1][0] - m), p11 = exp2f(s[1][1] - m);
+            l += (p00 + p01) + (p10 + p11);
+            const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);
+            // ---- O += P V
+            {
+                const int vrow = kPage + (((lane >> 3) & 1) << 3) + (lane & 7);
+                const uint32_t rbase = tb + vrow * 128;
+#pragma unroll
+                for (int cg = 0; cg < D / 8; cg += 2) {
+                    const int ck = (cg & 7) + (lane >> 4);
+                    uint32_t v0, v1, v2, v3;
+                    ldsm_x4_t(rbase + (cg >> 3) * kHalf + ((ck ^ (vrow & 7)) << 4), v0, v1, v2, v3);
+                    mma_rows07(o[cg][0], o[cg][1], pa0, pa2, v0, v1);
+                    mma_rows07(o[cg + 1][0], o[cg + 1][1], pa0, pa2, v2, v3);
+                }
+            }
+            if (valid < kPage) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(warp, stage));
+            if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
+        }
+        rot = (rot + n_tiles) & (kNW - 1);
+
+        // ---- combine the eight warp states of this item
+        l += __shfl_xor_sync(0xffffffffu, l, 1);
+        l += __shfl_xor_sync(0xffffffffu, l, 2);
+        if (row_ok) {
+            float* so = scratch_o + (warp * G + row) * kRowF + qd * 2;
+#pragma unroll
+            for (int nt = 0; nt < D / 8; ++nt) *reinterpret_cast<float2*>(so + nt * 8) = make_float2(o[nt][0], o[nt][1]);
+            if (qd == 0) *reinterpret_cast<float2*>(scratch_ml + (warp * G + row) * 2) = make_float2(m, l);
+        }
+        named_bar_sync(1, kNW * 32);
+        for (int idx = threadIdx.x; idx < G * (D / 2); idx += kNW * 32) {
+            const int g = idx / (D / 2), c2 = idx % (D / 2);
+            float mw[kNW], M = kNegInf;
+#pragma unroll
+            for (int w = 0; w < kNW; ++w) {
+                mw[w] = scratch_ml[(w * G + g) * 2];
+                M = fmaxf(M, mw[w]);
+            }
+            float Lsum = 0.f, ax = 0.f, ay = 0.f;
+#pragma unroll
+            for (int w = 0; w < kNW; ++w) {
+                const float e = exp2f(mw[w] - M);  // warps without a tile have m = -inf -> weight 0
+                Lsum += e * scratch_ml[(w * G + g) * 2 + 1];
+                const float2 v = *reinterpret_cast<const float2*>(scratch_o + (w * G + g) * kRowF + c2 * 2);
+                ax += e * v.x, ay += e * v.y;
+            }
+            const float inv = 1.f / Lsum;
+            const float lse_nat = (M + log2f(Lsum)) * 0.6931471805599453f;
+            if (item.n_parts == 1) {
+                const size_t hq = static_cast<size_t>(item.req) * p.Hq + static_cast<size_t>(item.kv_head) * G + g;
+                *reinterpret_cast<__nv_bfloat162*>(p.out + hq * D + c2 * 2) = __floats2bfloat162_rn(ax * inv, ay * inv);
+                if (c2 == 0) p.lse[hq] = lse_nat;
+            } else {
+                const size_t ps = static_cast<size_t>(item.part_slot) * G + g;
+                *reinterpret_cast<float2*>(p.part_o + ps * D + c2 * 2) = make_float2(ax * inv, ay * inv);
+                if (c2 == 0) p.part_lse[ps] = lse_nat;
+            }
+        }
+        named_bar_sync(1, kNW * 32);  // scratch may be overwritten by the next item
+    }
+    if (TIMED && threadIdx.x == 0) p.worker_ns[2 * blockIdx.x + 1] = globaltimer();
+}
+
+// ------------------------------------------------------------------ a5: LSE merge kernel
+// One warp per (request, query head).  Sequences with one part were written by the decode kernel;
+// sequences with no retained token get out = 0, lse = -inf.
+template <int D>
+__global__ void __launch_bounds__(128)
+tangram_merge_kernel(const int64_t* __restrict__ part_indptr, const float* __restrict__ part_o,
+                     const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
+                     float* __restrict__ lse, int R, int H, int G) {
+    constexpr int V = D / 32;  // floats per lane
+    const int Hq = H * G;
+    const int gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (gw >= R * Hq) return;
+    const int r = gw / Hq, j = gw % Hq, h = j / G, gi = j % G;
+    const int64_t p0 = part_indptr[static_cast<int64_t>(r) * H + h];
+    const int n = static_cast<int>(part_indptr[static_cast<int64_t>(r) * H + h + 1] - p0);
+    if (n == 1) return;
+    __nv_bfloat16* dst = out + static_cast<size_t>(gw) * D + lane * V;
+    if (n == 0) {
+#pragma unroll
+        for (int e = 0; e < V; ++e) dst[e] = __float2bfloat16(0.f);
+        if (lane == 0) lse[gw] = -INFINITY;
+        return;
+    }
+    float M = -INFINITY;
+    for (int i = lane; i < n; i += 32) M = fmaxf(M, part_lse[(p0 + i) * G + gi]);
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, s));
+    float acc[V], tot = 0.f;
+#pragma unroll
+    for (int e = 0; e < V; ++e) acc[e] = 0.f;
+    for (int i = 0; i < n; ++i) {
+        const float w = __expf(part_lse[(p0 + i) * G + gi] - M);
+        tot += w;
+        const float* src = part_o + ((p0 + i) * G + gi) * D + lane * V;
+        if constexpr (V == 4) {
+            const float4 v = *reinterpret_cast<const float4*>(src);
+            acc[0] += w * v.x, acc[1] += w * v.y, acc[2] += w * v.z, acc[3] += w * v.w;
+        } else {
+            const float2 v = *reinterpret_cast<const float2*>(src);
+            acc[0] += w * v.x, acc[1] += w * v.y;
+        }
+    }
+    const float inv = 1.f / tot;
+#pragma unroll
+    for (int e = 0; e < V; e += 2)
+        *reinterpret_cast<__nv_bfloat162*>(dst + e) = __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
+    if (lane == 0) lse[gw] = M + __logf(tot);
+}
+
+// ------------------------------------------------------------------ host-side launch helpers
+static int cuda_fail(cudaError_t e, const char* what) {
+    return fail(TANGRAM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess)
+            sym = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(sym);
+    }();
+    return fn;
+}
+
+// The pool [n_pages][Hp][2][P][d] bf16 seen as rows of d elements: dim0 = 64 elements (128 B, the
+// swizzle span), dim1 = row, dim2 = which 64-element half of the row.  One box = the 2P rows (K then
+// V) of one (page, slot).
+static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages, int Hp, int d) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return fail(TANGRAM_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    const cuuint64_t rows = static_cast<cuuint64_t>(n_pool_pages) * Hp * 2 * kPage;
+    const cuuint64_t gdim[3] = {64, rows, static_cast<cuuint64_t>(d / 64)};
+    const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(d) * 2, 128};
+    const cuuint32_t box[3] = {64, 2 * kPage, static_cast<cuuint32_t>(d / 64)};
+    const cuuint32_t estride[3] = {1, 1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(pool), gdim, gstride, box,
+                           estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(TANGRAM_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return TANGRAM_OK;
+}
+
+template <int D>
+static int launch_decode(const tangram_device_plan* dp, const DecodeParams& prm, const CUtensorMap& map,
+                         cudaStream_t stream) {
+    using L = Smem<D>;
+    const int smem = L::total(prm.n_stages, prm.G);
+    cudaError_t e;
+    if (prm.worker_ns) {
+        e = cudaFuncSetAttribute(tangram_decode_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+        tangram_decode_kernel<D, true><<<dp->W, kThreads, smem, stream>>>(map, prm);
+    } else {
+        e = cudaFuncSetAttribute(tangram_decode_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+        tangram_decode_kernel<D, false><<<dp->W, kThreads, smem, stream>>>(map, prm);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
+    const int n_rows = dp->R * prm.Hq;
+    tangram_merge_kernel<D><<<(n_rows + 3) / 4, 128, 0, stream>>>(dp->part_indptr, prm.part_o, prm.part_lse, prm.out,
+                                                                prm.lse, dp->R, dp->H, prm.G);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
+    return TANGRAM_OK;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace tangram
+
+using namespace tangram;
+
+extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa, int32_t* n_cta_out) {
+    if (!n_cta_out || (head_dim != 64 && head_dim != 128) || gqa < 1 || gqa > kMaxG)
+        return fail(TANGRAM_ERR_INVALID_ARG, "query_max_ctas: head_dim=%d gqa=%d", head_dim, gqa);
+    int sms = 0, per_sm = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    if (head_dim == 128) {
+        const int smem = Smem<128>::total(Smem<128>::max_stages(gqa), gqa);
+        e = cudaFuncSetAttribute(tangram_decode_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<128, false>, kThreads, smem);
+    } else {
+        const int smem = Smem<64>::total(Smem<64>::max_stages(gqa), gqa);
+        e = cudaFuncSetAttribute(tangram_decode_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<64, false>, kThreads, smem);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "occupancy query");
+    *n_cta_out = sms * per_sm;
+    return TANGRAM_OK;
+}
+
+extern "C" size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan* p) {
+    if (!t || !p) return 0;
+    size_t b = 0;
+    b += align_up(sizeof(DeviceItem) * (size_t)p->n_items, 256);
+    b += align_up(sizeof(int64_t) * ((size_t)p->W + 1), 256);
+    b += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
+    b += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
+    return b + 256;
+}
+
+extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
+                              void* stream, tangram_device_plan* dp) {
+    if (!t || !p || !dev_blob || !dp || !p->items || !p->worker_indptr || !p->part_indptr || !t->tbl_pages ||
+        !t->tbl_indptr)
+        return fail(TANGRAM_ERR_INVALID_ARG, "upload: NULL argument");
+    const size_t need = tangram_blob_bytes(t, p);
+    if (bytes < need) return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "upload: blob %zu < %zu bytes", bytes, need);
+    if (reinterpret_cast<uintptr_t>(dev_blob) % 256 != 0)
+        return fail(TANGRAM_ERR_INVALID_ARG, "upload: dev_blob must be 256-byte aligned");
+    std::vector<uint8_t> host(need, 0);
+    size_t off = 0;
+    const size_t off_items = off;
+    DeviceItem* di = reinterpret_cast<DeviceItem*>(host.data() + off);
+    for (int64_t i = 0; i < p->n_items; ++i) {
+        const tangram_item& s = p->items[i];
+        const int64_t row_off = t->tbl_indptr[(int64_t)s.req * t->C + s.cluster];
+        if (row_off > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: page table larger than 2^31 entries");
+        di[i] = DeviceItem{s.req, s.kv_head, (int32_t)row_off, s.slot, s.tok_begin, s.tok_end, s.part_slot, s.n_parts};
+    }
+    off += align_up(sizeof(DeviceItem) * (size_t)p->n_items, 256);
+    const size_t off_windptr = off;
+    std::memcpy(host.data() + off, p->worker_indptr, sizeof(int64_t) * ((size_t)p->W + 1));
+    off += align_up(sizeof(int64_t) * ((size_t)p->W + 1), 256);
+    const size_t off_pindptr = off;
+    std::memcpy(host.data() + off, p->part_indptr, sizeof(int64_t) * ((size_t)t->R * t->H + 1));
+    off += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
+    const size_t off_pages = off;
+    std::memcpy(host.data() + off, t->tbl_pages, sizeof(int32_t) * (size_t)t->n_pages_used);
+    // pageable source: the runtime stages it before returning, so `host` may die at scope exit
+    cudaError_t e = cudaMemcpyAsync(dev_blob, host.data(), need, cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e, "upload: cudaMemcpyAsync");
+    e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e, "upload: cudaStreamSynchronize");
+    uint8_t* base = static_cast<uint8_t*>(dev_blob);
+    dp->R = t->R, dp->H = t->H, dp->C = t->C, dp->Hp = t->Hp, dp->P = t->P, dp->W = p->W, dp->mode = p->mode;
+    dp->reserved_ = 0;
+    dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
+    dp->items = base + off_items;
+    dp->worker_indptr = reinterpret_cast<const int64_t*>(base + off_windptr);
+    dp->part_indptr = reinterpret_cast<const int64_t*>(base + off_pindptr);
+    dp->tbl_pages = reinterpret_cast<const int32_t*>(base + off_pages);
+    return TANGRAM_OK;
+}
+
+extern "C" size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_dim) {
+    if (n_part_slots < 0 || gqa < 1 || head_dim < 1) return 0;
+    return align_up((size_t)n_part_slots * gqa * head_dim * 4, 256) + align_up((size_t)n_part_slots * gqa * 4, 256) + 256;
+}
+
+extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                                        int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                                        float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
+                                        void* stream) {
+    if (!dp || !q || !kv_pool || !out || !lse) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
+    if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128}", d);
+    if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d (kernels need 16)", dp->P);
+    if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > kMaxG)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d)", Hq,
+                    dp->H, kMaxG);
+    if (n_pool_pages < 1 || dp->W < 1) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool or plan");
+    if (reinterpret_cast<uintptr_t>(q) % 16 || reinterpret_cast<uintptr_t>(kv_pool) % 128 ||
+        reinterpret_cast<uintptr_t>(out) % 16 || reinterpret_cast<uintptr_t>(workspace) % 16)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: misaligned pointer");
+    const int G = Hq / dp->H;
+    const size_t need = tangram_workspace_bytes(dp->n_part_slots, G, d);
+    if (dp->n_part_slots > 0 && (!workspace || workspace_bytes < need))
+        return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "decode_attention: workspace %zu < %zu bytes", workspace_bytes, need);
+
+    CUtensorMap map;
+    int rc = make_kv_map(&map, kv_pool, n_pool_pages, dp->Hp, d);
+    if (rc != TANGRAM_OK) return rc;
+
+    DecodeParams prm;
+    prm.items = static_cast<const DeviceItem*>(dp->items);
+    prm.worker_indptr = dp->worker_indptr;
+    prm.tbl_pages = dp->tbl_pages;
+    prm.q = static_cast<const __nv_bfloat16*>(q);
+    prm.out = static_cast<__nv_bfloat16*>(out);
+    prm.lse = lse;
+    prm.part_o = static_cast<float*>(workspace);
+    prm.part_lse = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) +
+                                            align_up((size_t)dp->n_part_slots * G * d * 4, 256));
+    prm.worker_ns = reinterpret_cast<unsigned long long*>(worker_ns);
+    prm.Hq = Hq, prm.G = G, prm.Hp = dp->Hp;
+    prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);
+    const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
+    prm.scale_log2 = scale * 1.4426950408889634f;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return d == 128 ? launch_decode<128>(dp, prm, map, st) : launch_decode<64>(dp, prm, map, st);
+}

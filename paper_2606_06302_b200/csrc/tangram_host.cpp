@@ -1,0 +1,269 @@
+// Host side of the Tangram hot path: Budget Reservation (a1), Ragged Paging tables (a2) and the
+// Ahead-of-Time partition planner (a3).  Pure integer / fp64 code, no CUDA.  See include/tangram.h
+// for the contract of every entry point and the PAPER.md passages they implement.
+// Compiled with -ffp-contract=off: fp64 expressions are evaluated exactly as written.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <vector>
+
+#include "tangram.h"
+#include "tangram_internal.h"
+
+namespace tangram {
+
+static thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+// Algorithm 1 for one layer.  round() is half-up.
+static void algorithm1(const double* B, const int32_t* perm, int32_t H, int32_t Hp, int32_t n_cta,
+                       int32_t* S) {
+    const int32_t C = H / Hp;
+    std::fill(S, S + C, 1);
+    double omega = 0.0;
+    for (int32_t h = 0; h < H; ++h) omega += B[h];
+    if (omega == 0.0) return;
+    const double tau = omega / static_cast<double>(n_cta);
+    for (int32_t i = 0; i < C; ++i) {
+        double phi = 0.0;
+        for (int32_t k = 0; k < Hp; ++k) phi += B[perm[i * Hp + k]];
+        const double s = std::floor(phi / tau + 0.5);
+        S[i] = s < 1.0 ? 1 : static_cast<int32_t>(s);
+    }
+}
+
+struct RawItem {
+    int32_t worker, r, h, tb, te;
+};
+
+}  // namespace tangram
+
+using namespace tangram;
+
+extern "C" const char* tangram_last_error(void) { return g_err; }
+
+extern "C" int tangram_reserve_budgets(const double* mu, const double* sigma, double alpha, int32_t H,
+                                       const int32_t* ctx_len, int32_t R, const int32_t* demand,
+                                       double* B_out, int32_t* reserved_out, int32_t* kv_len_out) {
+    if (!mu || !sigma || !ctx_len || !B_out || !reserved_out || !kv_len_out)
+        return fail(TANGRAM_ERR_INVALID_ARG, "reserve_budgets: NULL argument");
+    if (H < 1 || R < 1) return fail(TANGRAM_ERR_INVALID_ARG, "reserve_budgets: H=%d R=%d", H, R);
+    std::vector<double> B(H);
+    for (int32_t h = 0; h < H; ++h) {
+        const double margin = alpha * sigma[h];
+        const double b = std::min(1.0, mu[h] + margin);  // Eq. 5
+        if (!(b > 0.0))
+            return fail(TANGRAM_ERR_INVALID_ARG, "reserve_budgets: head %d has B=%g, not in (0,1]", h, b);
+        B[h] = b;
+    }
+    for (int32_t r = 0; r < R; ++r) {
+        if (ctx_len[r] < 1)
+            return fail(TANGRAM_ERR_INVALID_ARG, "reserve_budgets: ctx_len[%d]=%d < 1", r, ctx_len[r]);
+        if (demand)
+            for (int32_t h = 0; h < H; ++h)
+                if (demand[(size_t)r * H + h] < 0)
+                    return fail(TANGRAM_ERR_INVALID_ARG, "reserve_budgets: demand[%d][%d] < 0", r, h);
+    }
+    std::copy(B.begin(), B.end(), B_out);
+    for (int32_t r = 0; r < R; ++r) {
+        const double N = static_cast<double>(ctx_len[r]);
+        for (int32_t h = 0; h < H; ++h) {
+            const double want = std::ceil(B[h] * N);  // Eq. 4: ceil(B N)
+            int32_t n = want > N ? ctx_len[r] : static_cast<int32_t>(want);
+            n = std::max(1, std::min(ctx_len[r], n));
+            const size_t i = (size_t)r * H + h;
+            reserved_out[i] = n;
+            kv_len_out[i] = demand ? std::min(demand[i], n) : n;  // overflow truncation, :176
+        }
+    }
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_build_ragged_tables(const double* B, const int32_t* reserved, int32_t R,
+                                           int32_t H, int32_t n_clusters, int32_t page_size,
+                                           const int32_t* free_pages, int64_t n_free, uint32_t flags,
+                                           int32_t* kv_len_inout, tangram_tables* out) {
+    if (!B || !reserved || !out) return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: NULL argument");
+    if (R < 1 || H < 1 || n_clusters < 1 || H % n_clusters != 0)
+        return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: H=%d not a multiple of n_clusters=%d (R=%d)", H,
+                    n_clusters, R);
+    if (page_size <= 0) return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: page_size=%d", page_size);
+    if (n_free < 0 || (n_free > 0 && !free_pages))
+        return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: bad free list");
+    const int32_t C = n_clusters, Hp = H / C;
+
+    // Budget-Aware Clustering (:227-233): stable ascending sort on B only.
+    std::vector<int32_t> order(H);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return B[a] < B[b]; });
+
+    // capacity of every (request, cluster) row: the cluster's largest reservation (:190)
+    std::vector<int32_t> cap((size_t)R * C);
+    int64_t need = 0;
+    for (int32_t r = 0; r < R; ++r)
+        for (int32_t c = 0; c < C; ++c) {
+            int32_t mx = 0;
+            for (int32_t k = 0; k < Hp; ++k) {
+                const int32_t v = reserved[(size_t)r * H + order[c * Hp + k]];
+                if (v < 0) return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: reserved < 0");
+                mx = std::max(mx, v);
+            }
+            cap[(size_t)r * C + c] = mx;
+            need += (mx + page_size - 1) / page_size;
+        }
+    out->R = R, out->H = H, out->C = C, out->Hp = Hp, out->P = page_size;
+    out->n_pages_used = need;
+    if (need > n_free)
+        return fail(TANGRAM_ERR_OUT_OF_PAGES, "build_ragged_tables: need %lld pages, free list has %lld",
+                    (long long)need, (long long)n_free);
+    if (!out->tbl_pages) return TANGRAM_OK;  // query
+    if (!out->perm || !out->cluster_of || !out->slot_of || !out->tbl_indptr)
+        return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: NULL output array");
+    if (out->tbl_pages_cap < need)
+        return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "build_ragged_tables: tbl_pages_cap %lld < %lld",
+                    (long long)out->tbl_pages_cap, (long long)need);
+    for (int32_t j = 0; j < H; ++j) {
+        out->perm[j] = order[j];
+        out->cluster_of[order[j]] = j / Hp;
+        out->slot_of[order[j]] = j % Hp;
+    }
+    int64_t cur = 0;
+    out->tbl_indptr[0] = 0;
+    for (int64_t row = 0; row < (int64_t)R * C; ++row) {
+        const int64_t n = (cap[row] + page_size - 1) / page_size;
+        std::memcpy(out->tbl_pages + cur, free_pages + cur, sizeof(int32_t) * (size_t)n);
+        cur += n;
+        out->tbl_indptr[row + 1] = cur;
+    }
+    if ((flags & TANGRAM_FILL_GROUP) && kv_len_inout)
+        for (int32_t r = 0; r < R; ++r)
+            for (int32_t h = 0; h < H; ++h)
+                kv_len_inout[(size_t)r * H + h] = cap[(size_t)r * C + out->cluster_of[h]];
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_plan_partitions(const tangram_tables* t, const double* B, const int32_t* kv_len,
+                                       int32_t n_workers, int32_t granule_tokens,
+                                       int32_t overhead_granules, int32_t mode, int32_t static_splits,
+                                       tangram_plan* out) {
+    if (!t || !B || !kv_len || !out) return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: NULL argument");
+    if (!t->perm || !t->cluster_of || !t->slot_of || !t->tbl_indptr)
+        return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: tables not filled");
+    const int32_t R = t->R, H = t->H, C = t->C, Hp = t->Hp, P = t->P;
+    const int32_t W = n_workers, g = granule_tokens, c0 = overhead_granules;
+    if (W < 1 || g < 1 || P < 1 || g % P != 0 || c0 < 0)
+        return fail(TANGRAM_ERR_INVALID_ARG,
+                    "plan_partitions: W=%d granule=%d (must be a positive multiple of P=%d) overhead=%d", W, g, P, c0);
+    if (mode != TANGRAM_MODE_BALANCED && mode != TANGRAM_MODE_SPLITMAP && mode != TANGRAM_MODE_STATIC_EVEN)
+        return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: mode=%d", mode);
+    for (int32_t r = 0; r < R; ++r)
+        for (int32_t h = 0; h < H; ++h) {
+            const int64_t row = (int64_t)r * C + t->cluster_of[h];
+            const int64_t cap_tokens = (t->tbl_indptr[row + 1] - t->tbl_indptr[row]) * (int64_t)P;
+            const int32_t n = kv_len[(size_t)r * H + h];
+            if (n < 0 || n > cap_tokens)
+                return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: kv_len[%d][%d]=%d exceeds its table (%lld tokens)",
+                            r, h, n, (long long)cap_tokens);
+        }
+
+    std::vector<int32_t> S(C);
+    algorithm1(B, t->perm, H, Hp, W, S.data());
+    std::vector<RawItem> raw;
+    const int64_t n_seq = (int64_t)R * H;
+    raw.reserve((size_t)(n_seq + W));
+
+    if (mode == TANGRAM_MODE_BALANCED) {
+        // Lay the sequences end to end on a cost axis (granules, plus c0 per non-empty sequence) and
+        // cut the axis at b_k = floor(k T / W).
+        int64_t T = 0;
+        for (int32_t r = 0; r < R; ++r)
+            for (int32_t h = 0; h < H; ++h) {
+                const int64_t u = (kv_len[(size_t)r * H + h] + (int64_t)g - 1) / g;
+                T += u + (u > 0 ? c0 : 0);
+            }
+        auto cut = [&](int64_t k) { return (k * T) / W; };
+        int64_t pos = 0;   // cost position where the current sequence starts
+        int64_t k = 0;     // current worker
+        for (int32_t r = 0; r < R; ++r)
+            for (int32_t j = 0; j < H; ++j) {
+                const int32_t h = t->perm[j];
+                const int32_t n = kv_len[(size_t)r * H + h];
+                const int64_t u = (n + (int64_t)g - 1) / g;
+                if (u == 0) continue;
+                const int64_t first = pos + c0, last = first + u;  // granule positions [first, last)
+                int64_t p = first;
+                while (p < last) {
+                    while (cut(k + 1) <= p) ++k;
+                    const int64_t stop = std::min(last, cut(k + 1));
+                    const int64_t tb = (p - first) * g;
+                    const int64_t te = std::min<int64_t>(n, (stop - first) * g);
+                    raw.push_back({(int32_t)k, r, h, (int32_t)tb, (int32_t)te});
+                    p = stop;
+                }
+                pos = last;
+            }
+    } else {
+        int32_t s_even = static_splits;
+        if (mode == TANGRAM_MODE_STATIC_EVEN) {
+            if (s_even <= 0) s_even = (int32_t)std::max<int64_t>(1, (W + n_seq - 1) / n_seq);
+            std::fill(S.begin(), S.end(), s_even);
+        }
+        int64_t dealt = 0;
+        for (int32_t r = 0; r < R; ++r)
+            for (int32_t j = 0; j < H; ++j) {
+                const int32_t h = t->perm[j];
+                const int32_t n = kv_len[(size_t)r * H + h];
+                const int64_t u = (n + (int64_t)g - 1) / g;
+                const int64_t Sc = S[t->cluster_of[h]];
+                for (int64_t c = 0; c < Sc; ++c) {
+                    const int64_t lo = (c * u) / Sc, hi = ((c + 1) * u) / Sc;
+                    const int64_t tb = lo * g, te = std::min<int64_t>(n, hi * g);
+                    if (te <= tb) continue;
+                    raw.push_back({(int32_t)(dealt % W), r, h, (int32_t)tb, (int32_t)te});
+                    ++dealt;
+                }
+            }
+    }
+
+    out->W = W, out->mode = mode;
+    out->n_items = (int64_t)raw.size();
+    out->n_part_slots = (int64_t)raw.size();
+    if (out->split_map) std::copy(S.begin(), S.end(), out->split_map);
+    if (!out->items) return TANGRAM_OK;  // query
+    if (!out->worker_indptr || !out->part_indptr || !out->split_map)
+        return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: NULL output array");
+    if (out->items_cap < out->n_items)
+        return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "plan_partitions: items_cap %lld < %lld", (long long)out->items_cap,
+                    (long long)out->n_items);
+
+    // parts per sequence; raw is already in token order inside every sequence
+    std::vector<int64_t> cnt((size_t)n_seq, 0);
+    for (const RawItem& it : raw) ++cnt[(size_t)it.r * H + it.h];
+    out->part_indptr[0] = 0;
+    for (int64_t s = 0; s < n_seq; ++s) out->part_indptr[s + 1] = out->part_indptr[s] + cnt[(size_t)s];
+    std::vector<int64_t> wcount((size_t)W + 1, 0);
+    for (const RawItem& it : raw) ++wcount[(size_t)it.worker + 1];
+    for (int32_t w = 0; w < W; ++w) wcount[(size_t)w + 1] += wcount[(size_t)w];
+    std::copy(wcount.begin(), wcount.end(), out->worker_indptr);
+    std::vector<int64_t> wcur(wcount.begin(), wcount.end() - 1);
+    std::vector<int64_t> ord((size_t)n_seq, 0);
+    for (const RawItem& it : raw) {
+        const size_t s = (size_t)it.r * H + it.h;
+        tangram_item& o = out->items[wcur[(size_t)it.worker]++];
+        o.req = it.r, o.kv_head = it.h, o.cluster = t->cluster_of[it.h], o.slot = t->slot_of[it.h];
+        o.tok_begin = it.tb, o.tok_end = it.te;
+        o.part_slot = (int32_t)(out->part_indptr[s] + ord[s]++);
+        o.n_parts = (int32_t)cnt[s];
+    }
+    return TANGRAM_OK;
+}

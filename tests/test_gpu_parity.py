@@ -1,0 +1,226 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json's: bf16 outputs max |err| <= 2e-2 and relative
+L2 <= 5e-3, per-head LSE within 1e-3.  Integer results (tables, plans) are compared bit-exactly in
+tests/test_host_vs_oracle.py; here the plans that drive the kernel are the product's own."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import tangram_oracle as O
+from paper_2606_06302_b200 import binding as T
+from paper_2606_06302_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, REL_L2, LSE_TOL = 2e-2, 5e-3, 1e-3
+
+
+def setup(wl, flags=0, identity=False):
+    B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    need = T.tangram_pages_needed(B, res, wl.C, wl.P)
+    n_pool = int(math.ceil(1.05 * need))
+    free = I.make_free_pages(wl, n_pool, identity=identity)
+    t, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, free, flags, kv)
+    return B, res, kv, t, n_pool
+
+
+def oracle_tables(t):
+    return O.Tables(R=t.R, H=t.H, C=t.C, Hp=t.Hp, P=t.P, perm=t.perm, cluster_of=t.cluster_of, slot_of=t.slot_of,
+                    tbl_indptr=t.tbl_indptr, tbl_pages=t.tbl_pages, n_pages_used=t.n_pages_used)
+
+
+def check(out, lse, ref_out, ref_lse, what=""):
+    out = out.float().cpu().numpy().astype(np.float64).reshape(ref_out.shape)
+    lse = lse.cpu().numpy().astype(np.float64).reshape(ref_lse.shape)
+    assert np.all(np.isfinite(out)), what
+    err = np.abs(out - ref_out).max()
+    rel = np.linalg.norm(out - ref_out) / max(np.linalg.norm(ref_out), 1e-30)
+    fin = np.isfinite(ref_lse)
+    assert np.array_equal(np.isneginf(lse), np.isneginf(ref_lse)), what
+    dl = np.abs(lse[fin] - ref_lse[fin]).max() if fin.any() else 0.0
+    assert err <= MAX_ABS and rel <= REL_L2 and dl <= LSE_TOL, f"{what}: max|err|={err:.3e} relL2={rel:.3e} dLSE={dl:.3e}"
+    return err, rel, dl
+
+
+def run_modes(wl, B, kv, t, q, pool, Ws, modes=(T.MODE_BALANCED, T.MODE_SPLITMAP, T.MODE_STATIC_EVEN), c0=1):
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    for W in Ws:
+        for mode in modes:
+            pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, c0, mode)
+            dp = T.tangram_upload(t, pl)
+            out, lse = T.tangram_decode_attention(dp, q, pool)
+            torch.cuda.synchronize()
+            check(out, lse, ref_out, ref_lse, f"{wl.name} W={W} mode={T.MODE_NAMES[mode]}")
+    return ref_out, ref_lse
+
+
+def n_cta(wl):
+    return T.tangram_query_max_ctas(0, wl.d, wl.G)
+
+
+def test_query_max_ctas():
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    for d, g in ((64, 2), (128, 4), (128, 5), (128, 8)):
+        n = T.tangram_query_max_ctas(0, d, g)
+        assert n >= sms and n % sms == 0
+
+
+def test_tiny_full_config():
+    wl = I.make_workload("tiny")
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    run_modes(wl, B, kv, t, q, pool, Ws=(1, 4, n_cta(wl)))
+
+
+@pytest.mark.parametrize("name,kw", [("8b", dict(R=4, ctx_div=8)), ("32b", dict(R=6, ctx_div=8)),
+                                     ("skew", dict(R=2, ctx_div=8)), ("uniform", dict(R=16, ctx_div=4))])
+def test_scaled_configs(name, kw):
+    """Scaled-down BASELINE configs: many tiles per item, ragged tails, GQA 4 and 5, H_p 2/4/8."""
+    wl = I.make_workload(name, **kw)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    run_modes(wl, B, kv, t, q, pool, Ws=(7, n_cta(wl)))
+
+
+@pytest.mark.parametrize("seed,R,H,G,d,C", [(1, 3, 4, 1, 64, 2), (2, 2, 4, 2, 128, 4), (3, 3, 2, 3, 128, 1),
+                                            (4, 2, 6, 5, 128, 3), (5, 2, 2, 8, 64, 1), (6, 1, 8, 7, 128, 2),
+                                            (7, 4, 4, 6, 64, 4), (8, 2, 2, 8, 128, 2)])
+def test_random_shapes(seed, R, H, G, d, C):
+    wl = I.make_random_workload(seed, R=R, H=H, G=G, d=d, C=C, max_ctx=900)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    run_modes(wl, B, kv, t, q, pool, Ws=(3, 40))
+
+
+def test_empty_and_one_token_sequences():
+    wl = I.make_random_workload(11, R=3, H=4, G=2, d=128, C=2, max_ctx=300)
+    wl.demand[:, 1] = 0          # a head that retains nothing: out = 0, lse = -inf
+    wl.demand[1, :] = 1          # single-token sequences: out = v0
+    wl.demand[2, :] = 0          # a request with no KV at all
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    ref_out, ref_lse = run_modes(wl, B, kv, t, q, pool, Ws=(5,))
+    assert np.isneginf(ref_lse[2]).all() and np.all(ref_out[2] == 0)
+
+
+def test_slack_poisoned_with_nan():
+    """Every pool slot outside [0, kv_len) of its head is NaN: output unchanged and finite (the kernel
+    never lets unretained slots reach the result; SURVEY §8(c) "Kernel-only" pin, reading A28)."""
+    wl = I.make_workload("skew", R=2, ctx_div=16)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    keep = torch.zeros(pool.shape[:4], dtype=torch.bool)         # [page][slot][kv][token]
+    for r in range(wl.R):
+        for h in range(wl.H):
+            row = t.tbl_pages[t.tbl_indptr[r * t.C + t.cluster_of[h]]:t.tbl_indptr[r * t.C + t.cluster_of[h] + 1]]
+            n = int(kv[r, h])
+            for pi in range(-(-n // wl.P)):
+                keep[int(row[pi]), int(t.slot_of[h]), :, :min(wl.P, n - pi * wl.P)] = True
+    pool = torch.where(keep.to(pool.device)[..., None], pool, torch.full_like(pool, float("nan")))
+    run_modes(wl, B, kv, t, q, pool, Ws=(9, n_cta(wl)), modes=(T.MODE_BALANCED, T.MODE_STATIC_EVEN))
+
+
+def test_fill_group_policy():
+    wl = I.make_workload("8b", R=2, ctx_div=16)
+    B, res, kv, t, n_pool = setup(wl, flags=T.FILL_GROUP, identity=True)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    run_modes(wl, B, kv, t, q, pool, Ws=(n_cta(wl),), modes=(T.MODE_BALANCED,))
+
+
+def test_page_permutation_invariance_and_determinism():
+    """Same logical KV under two physical page assignments: identical output bits; and two runs of the
+    same plan are bit-identical (fixed work list, no atomics)."""
+    wl = I.make_workload("8b", R=2, ctx_div=16)
+    B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    n_pool = T.tangram_pages_needed(B, res, wl.C, wl.P) + 50
+    outs = []
+    base_pool = None
+    for identity in (True, False):
+        free = I.make_free_pages(wl, n_pool, identity=identity)
+        t, _ = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, free, 0, kv)
+        if base_pool is None:
+            q, base_pool = I.make_q_and_pool(wl, n_pool, "cuda")
+            pool, t0 = base_pool, t
+        else:                      # move every logical page to its new physical id
+            pool = torch.randn_like(base_pool.float()).bfloat16()
+            pool[torch.as_tensor(t.tbl_pages, dtype=torch.long, device="cuda")] = \
+                base_pool[torch.as_tensor(t0.tbl_pages, dtype=torch.long, device="cuda")]
+        pl = T.tangram_plan_partitions(t, B, kv, 24, wl.granule, 1, T.MODE_BALANCED)
+        dp = T.tangram_upload(t, pl)
+        o1, l1 = T.tangram_decode_attention(dp, q, pool)
+        o2, l2 = T.tangram_decode_attention(dp, q, pool)
+        torch.cuda.synchronize()
+        assert torch.equal(o1, o2) and torch.equal(l1, l2)
+        outs.append((o1, l1))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+
+
+def test_cuda_graph_capture_and_worker_timestamps():
+    wl = I.make_workload("32b", R=4, ctx_div=8)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    W = n_cta(wl)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED)
+    dp = T.tangram_upload(t, pl)
+    out, lse = T.tangram_decode_attention(dp, q, pool)
+    ws = torch.empty(T.tangram_workspace_bytes(pl.n_part_slots, wl.G, wl.d), dtype=torch.uint8, device="cuda")
+    out_g, lse_g = torch.zeros_like(out), torch.zeros_like(lse)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        T.tangram_decode_attention(dp, q, pool, out_g, lse_g, ws, stream=s)      # warm-up outside capture
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            T.tangram_decode_attention(dp, q, pool, out_g, lse_g, ws, stream=s)
+    out_g.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, out_g) and torch.equal(lse, lse_g)
+    ns = torch.zeros(W, 2, dtype=torch.int64, device="cuda")
+    out_t, _ = T.tangram_decode_attention(dp, q, pool, worker_ns=ns)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out_t)
+    ns = ns.cpu().numpy()
+    assert np.all(ns[:, 1] >= ns[:, 0]) and np.all(ns[:, 0] > 0)
+
+
+def test_device_error_contract():
+    wl = I.make_workload("tiny")
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    pl = T.tangram_plan_partitions(t, B, kv, 4, wl.granule, 0, T.MODE_STATIC_EVEN, 3)
+    dp = T.tangram_upload(t, pl)
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_decode_attention(dp, q, pool, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == T.ERR_BUFFER_TOO_SMALL
+    q3 = torch.randn(wl.R, 3 * wl.H * 3, wl.d, device="cuda").bfloat16()          # G = 9 > 8
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_decode_attention(dp, q3, pool)
+    assert e.value.code == T.ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("name", ["8b", "32b", "skew", "uniform"])
+def test_full_size_sampled(name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (W = N_CTA, BALANCED,
+    c0 = 1), checked on sampled (request, query head) outputs the oracle computes one by one, plus a
+    property that holds at any size: every lse is finite and every output row is finite."""
+    wl = I.make_workload(name)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    W = n_cta(wl)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED)
+    dp = T.tangram_upload(t, pl)
+    out, lse = T.tangram_decode_attention(dp, q, pool)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out.float()).all() and torch.isfinite(lse).all()
+    rng = np.random.default_rng(wl.seed)
+    pairs = {(int(rng.integers(wl.R)), int(rng.integers(wl.Hq))) for _ in range(48)}
+    longest = np.unravel_index(np.argmax(kv), kv.shape)                 # always include the longest sequence
+    pairs.add((int(longest[0]), int(longest[1]) * wl.G))
+    pairs = sorted(pairs)
+    ref_out, ref_lse, _ = O.attention_pairs(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d, pairs)
+    idx_r = torch.as_tensor([p[0] for p in pairs], device="cuda")
+    idx_j = torch.as_tensor([p[1] for p in pairs], device="cuda")
+    check(out[idx_r, idx_j], lse[idx_r, idx_j], ref_out, ref_lse, f"{name} full size")

@@ -1,0 +1,138 @@
+"""Host side of the product (C ABI: reserve / tables / planner) against the CPU oracle: bit-exact
+budgets, page tables and plans on the five BASELINE configs (full size) and on random shapes, the
+error contract, and the exported symbols.  No GPU needed: these calls are host-pure."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+from hypothesis import given, settings, strategies as st
+
+from oracle import tangram_oracle as O
+from paper_2606_06302_b200 import binding as T
+from paper_2606_06302_b200 import inputs as I
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "tangram.h")).read()
+    declared = set(re.findall(r"\b(tangram_[a-z_]+)\s*\(", hdr))
+    assert declared == set(T.EXPORTS)
+    lib = ctypes.CDLL(T.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def both_sides(wl, n_pool_pages=None, flags=0, identity=False):
+    Bo, reso, kvo = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    Bp, resp, kvp = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    assert Bo.tobytes() == Bp.tobytes() and np.array_equal(reso, resp) and np.array_equal(kvo, kvp)
+    need = T.tangram_pages_needed(Bp, resp, wl.C, wl.P)
+    n_pool = n_pool_pages or int(np.ceil(1.05 * need))
+    free = I.make_free_pages(wl, n_pool, identity=identity)
+    to, kvo2 = O.build_ragged_tables(Bo, reso, wl.C, wl.P, free, flags, kvo)
+    tp, kvp2 = T.tangram_build_ragged_tables(Bp, resp, wl.C, wl.P, free, flags, kvp)
+    assert need == to.n_pages_used == tp.n_pages_used
+    for f in ("perm", "cluster_of", "slot_of", "tbl_indptr", "tbl_pages"):
+        a, b = getattr(to, f), getattr(tp, f)
+        assert a.dtype == b.dtype and np.array_equal(a, b), f
+    assert (to.R, to.H, to.C, to.Hp, to.P) == (tp.R, tp.H, tp.C, tp.Hp, tp.P)
+    assert np.array_equal(kvo2, kvp2)
+    return Bo, kvo2, to, tp
+
+
+def plans_equal(po, pp):
+    assert (po.W, po.mode, po.n_items, po.n_part_slots) == (pp.W, pp.mode, pp.n_items, pp.n_part_slots)
+    assert np.array_equal(po.split_map, pp.split_map)
+    assert po.items.shape == pp.items.shape and np.array_equal(po.items, pp.items)
+    assert np.array_equal(po.worker_indptr, pp.worker_indptr)
+    assert np.array_equal(po.part_indptr, pp.part_indptr)
+
+
+@pytest.mark.parametrize("name", I.CONFIG_NAMES)
+def test_full_configs_bit_exact(name):
+    wl = I.make_workload(name)
+    B, kv, to, tp = both_sides(wl)
+    for mode in (O.MODE_BALANCED, O.MODE_SPLITMAP, O.MODE_STATIC_EVEN):
+        for W, c0 in ((148, 1), (296, 0)):
+            po = O.plan_partitions(to, B, kv, W, wl.granule, c0, mode)
+            pp = T.tangram_plan_partitions(tp, B, kv, W, wl.granule, c0, mode)
+            plans_equal(po, pp)
+
+
+def test_fill_group_and_identity_free_list():
+    wl = I.make_workload("skew", R=2, ctx_div=16)
+    B, kv, to, tp = both_sides(wl, flags=O.FLAG_FILL_GROUP, identity=True)
+    assert kv[0, 7] == kv[0, 0] == wl.ctx_len[0] and kv[0, 1] < 100   # the short heads sharing the long head's cluster fill up
+    po = O.plan_partitions(to, B, kv, 8, 64, 1, O.MODE_BALANCED)
+    plans_equal(po, T.tangram_plan_partitions(tp, B, kv, 8, 64, 1, T.MODE_BALANCED))
+
+
+@settings(max_examples=60, deadline=None)
+@given(seed=st.integers(0, 10**6), R=st.integers(1, 5), Hp=st.integers(1, 4), C=st.integers(1, 4),
+       W=st.integers(1, 40), c0=st.integers(0, 3), gmul=st.integers(1, 4), mode=st.integers(0, 2),
+       splits=st.integers(0, 5))
+def test_random_shapes_bit_exact(seed, R, Hp, C, W, c0, gmul, mode, splits):
+    wl = I.make_random_workload(seed, R=R, H=Hp * C, G=1, d=64, C=C, max_ctx=700)
+    B, kv, to, tp = both_sides(wl)
+    g = wl.P * gmul
+    po = O.plan_partitions(to, B, kv, W, g, c0, mode, splits)
+    pp = T.tangram_plan_partitions(tp, B, kv, W, g, c0, mode, splits)
+    plans_equal(po, pp)
+
+
+def test_zero_length_sequences():
+    wl = I.make_random_workload(5, R=3, H=4, G=1, d=64, C=2)
+    wl.demand[:, 1] = 0
+    wl.demand[2, :] = 0
+    B, kv, to, tp = both_sides(wl)
+    assert kv[2].sum() == 0
+    for mode in range(3):
+        plans_equal(O.plan_partitions(to, B, kv, 7, 64, 1, mode), T.tangram_plan_partitions(tp, B, kv, 7, 64, 1, mode))
+
+
+def test_error_contract():
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_reserve_budgets([0.0], [0.0], 2.0, [10])
+    assert e.value.code == T.ERR_INVALID_ARG and "B=" in str(e.value)
+    with pytest.raises(T.TangramError):
+        T.tangram_reserve_budgets([0.5], [0.0], 2.0, [0])
+    with pytest.raises(T.TangramError):
+        T.tangram_reserve_budgets([0.5], [0.0], 2.0, [5], [[-1]])
+    B, res, kv = T.tangram_reserve_budgets([0.5, 0.25, 0.5], [0, 0, 0], 2.0, [100])
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_build_ragged_tables(B, res, 2, 16, np.arange(100))           # H % C != 0
+    assert e.value.code == T.ERR_INVALID_ARG
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_build_ragged_tables(B, res, 3, 0, np.arange(100))            # page_size <= 0
+    assert e.value.code == T.ERR_INVALID_ARG
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_build_ragged_tables(B, res, 3, 16, np.arange(3))             # needs 4+2+4 pages
+    assert e.value.code == T.ERR_OUT_OF_PAGES
+    t, _ = T.tangram_build_ragged_tables(B, res, 3, 16, np.arange(100))
+    with pytest.raises(T.TangramError) as e:
+        T.tangram_plan_partitions(t, B, kv, 4, 24, 0, T.MODE_BALANCED)          # granule % P != 0
+    assert e.value.code == T.ERR_INVALID_ARG
+    with pytest.raises(T.TangramError):
+        T.tangram_plan_partitions(t, B, kv, 0, 64, 0, T.MODE_BALANCED)
+    with pytest.raises(T.TangramError):
+        T.tangram_plan_partitions(t, B, kv + 1000, 4, 64, 0, T.MODE_BALANCED)   # kv_len beyond the table
+    with pytest.raises(T.TangramError):
+        T.tangram_plan_partitions(t, B, kv, 4, 64, 0, 7)
+
+
+def test_skew_balance_numbers():
+    """SURVEY §8(d) scratch check: Skew, W=296, g=64 -> at most R*H+W-1 items, token spread < 1 %; STATIC_EVEN S=3 leaves 43 691-token
+    chunks next to a ~7.3K-token fair share."""
+    wl = I.make_workload("skew")
+    B, kv, to, tp = both_sides(wl)
+    pl = T.tangram_plan_partitions(tp, B, kv, 296, 64, 0, T.MODE_BALANCED)
+    assert 296 <= pl.n_items <= wl.R * wl.H + 296 - 1
+    tok = np.array([sum(int(it[5] - it[4]) for it in pl.items[pl.worker_indptr[w]:pl.worker_indptr[w + 1]])
+                    for w in range(296)])
+    assert (tok.max() - tok.min()) / tok.mean() < 0.01
+    ps = T.tangram_plan_partitions(tp, B, kv, 296, 64, 0, T.MODE_STATIC_EVEN)
+    assert ps.split_map.tolist() == [3, 3]
+    assert max(int(it[5] - it[4]) for it in ps.items) == 43712           # ceil(2048/3)=683 granules * 64
