@@ -193,6 +193,19 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
                              float* lse, void* workspace, size_t workspace_bytes,
                              uint64_t* worker_ns, void* stream);
 
+/* The two kernels of tangram_decode_attention as separate calls (same arguments, same checks):
+ * a4 alone (split-KV decode kernel: final outputs of single-part sequences, fp32 partials of the
+ * others into `workspace`) and a5 alone (LSE merge of the partials in `workspace` into out / lse;
+ * zero-length sequences get out = 0, lse = -inf).  decode_partials followed by merge_partials on the
+ * same stream is exactly tangram_decode_attention; they exist so that each kernel can be timed and
+ * profiled on its own. */
+int tangram_decode_partials(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                            int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                            float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
+                            void* stream);
+int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d, void* out, float* lse,
+                           void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

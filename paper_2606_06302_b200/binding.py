@@ -59,12 +59,13 @@ _lib.tangram_blob_bytes.restype = C.c_size_t
 _lib.tangram_workspace_bytes.restype = C.c_size_t
 _lib.tangram_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
 for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
-              "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention"):
+              "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
+              "tangram_merge_partials"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
-           "tangram_workspace_bytes", "tangram_decode_attention")
+           "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials")
 
 
 def _check(rc: int):
@@ -218,7 +219,7 @@ def tangram_upload(t: Tables, p: Plan, device="cuda", stream=None) -> DevicePlan
 
 
 def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, workspace=None, sm_scale: float = 0.0,
-                             worker_ns=None, stream=None):
+                             worker_ns=None, stream=None, _entry="tangram_decode_attention"):
     """q [R,Hq,d] bf16 cuda, kv_pool [n_pages,Hp,2,P,d] bf16 cuda -> (out [R,Hq,d] bf16, lse [R,Hq] f32).
     Asynchronous on the current (or given) torch stream."""
     import torch
@@ -237,8 +238,26 @@ def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, wor
         workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     wn = C.c_void_p(worker_ns.data_ptr()) if worker_ns is not None else None
-    _check(_lib.tangram_decode_attention(C.byref(dp.c), C.c_void_p(q.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
+    _check(getattr(_lib, _entry)(C.byref(dp.c), C.c_void_p(q.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
                                          C.c_int64(n_pages), C.c_int32(Hq), C.c_int32(d), C.c_float(sm_scale),
                                          C.c_void_p(out.data_ptr()), C.c_void_p(lse.data_ptr()),
                                          C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), wn, sp))
+    return out, lse
+
+
+def tangram_decode_partials(dp: DevicePlan, q, kv_pool, out=None, lse=None, workspace=None, sm_scale: float = 0.0,
+                            worker_ns=None, stream=None):
+    """a4 alone: the split-KV decode kernel (see include/tangram.h)."""
+    return tangram_decode_attention(dp, q, kv_pool, out, lse, workspace, sm_scale, worker_ns, stream,
+                                    _entry="tangram_decode_partials")
+
+
+def tangram_merge_partials(dp: DevicePlan, out, lse, workspace, stream=None):
+    """a5 alone: the LSE merge kernel over the partials in `workspace`."""
+    import torch
+    R, Hq, d = out.shape
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    _check(_lib.tangram_merge_partials(C.byref(dp.c), C.c_int32(Hq), C.c_int32(d), C.c_void_p(out.data_ptr()),
+                                       C.c_void_p(lse.data_ptr()), C.c_void_p(workspace.data_ptr()),
+                                       C.c_size_t(workspace.numel()), sp))
     return out, lse

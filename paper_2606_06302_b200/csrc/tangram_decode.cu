@@ -39,6 +39,7 @@ constexpr int kQSlots = 2;         // item / query ring depth
 constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime <= this)
 constexpr int kMaxG = 8;
 constexpr int kSmemLimit = 232448; // 227 KB opt-in limit per CTA
+constexpr int kRunSplit = 1, kRunMerge = 2;
 
 struct DecodeParams {
     const DeviceItem* items;
@@ -472,11 +473,12 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
 
 template <int D>
 static int launch_decode(const tangram_device_plan* dp, const DecodeParams& prm, const CUtensorMap& map,
-                         cudaStream_t stream) {
+                         cudaStream_t stream, int which) {
     using L = Smem<D>;
     const int smem = L::total(prm.n_stages, prm.G);
     cudaError_t e;
-    if (prm.worker_ns) {
+    if (!(which & kRunSplit)) {
+    } else if (prm.worker_ns) {
         e = cudaFuncSetAttribute(tangram_decode_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
         tangram_decode_kernel<D, true><<<dp->W, kThreads, smem, stream>>>(map, prm);
@@ -487,6 +489,7 @@ static int launch_decode(const tangram_device_plan* dp, const DecodeParams& prm,
     }
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
+    if (!(which & kRunMerge)) return TANGRAM_OK;
     const int n_rows = dp->R * prm.Hq;
     tangram_merge_kernel<D><<<(n_rows + 3) / 4, 128, 0, stream>>>(dp->part_indptr, prm.part_o, prm.part_lse, prm.out,
                                                                 prm.lse, dp->R, dp->H, prm.G);
@@ -582,10 +585,9 @@ extern "C" size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int
     return align_up((size_t)n_part_slots * gqa * head_dim * 4, 256) + align_up((size_t)n_part_slots * gqa * 4, 256) + 256;
 }
 
-extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
-                                        int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
-                                        float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
-                                        void* stream) {
+static int run_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool, int64_t n_pool_pages,
+                         int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
+                         size_t workspace_bytes, uint64_t* worker_ns, void* stream, int which) {
     if (!dp || !q || !kv_pool || !out || !lse) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
     if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128}", d);
     if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d (kernels need 16)", dp->P);
@@ -602,8 +604,11 @@ extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const voi
         return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "decode_attention: workspace %zu < %zu bytes", workspace_bytes, need);
 
     CUtensorMap map;
-    int rc = make_kv_map(&map, kv_pool, n_pool_pages, dp->Hp, d);
-    if (rc != TANGRAM_OK) return rc;
+    std::memset(&map, 0, sizeof map);
+    if (which & kRunSplit) {
+        const int rc = make_kv_map(&map, kv_pool, n_pool_pages, dp->Hp, d);
+        if (rc != TANGRAM_OK) return rc;
+    }
 
     DecodeParams prm;
     prm.items = static_cast<const DeviceItem*>(dp->items);
@@ -621,5 +626,28 @@ extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const voi
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
     prm.scale_log2 = scale * 1.4426950408889634f;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    return d == 128 ? launch_decode<128>(dp, prm, map, st) : launch_decode<64>(dp, prm, map, st);
+    return d == 128 ? launch_decode<128>(dp, prm, map, st, which) : launch_decode<64>(dp, prm, map, st, which);
+}
+
+extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                                        int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                                        float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
+                                        void* stream) {
+    return run_attention(dp, q, kv_pool, n_pool_pages, Hq, d, sm_scale, out, lse, workspace, workspace_bytes,
+                         worker_ns, stream, kRunSplit | kRunMerge);
+}
+
+extern "C" int tangram_decode_partials(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                                       int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                                       float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
+                                       void* stream) {
+    return run_attention(dp, q, kv_pool, n_pool_pages, Hq, d, sm_scale, out, lse, workspace, workspace_bytes,
+                         worker_ns, stream, kRunSplit);
+}
+
+extern "C" int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d, void* out, float* lse,
+                                      void* workspace, size_t workspace_bytes, void* stream) {
+    // q / kv_pool are not read by the merge kernel; pass aligned dummies through the shared validation
+    return run_attention(dp, out, out, 1, Hq, d, 0.f, out, lse, workspace, workspace_bytes, nullptr, stream,
+                         kRunMerge);
 }
