@@ -130,7 +130,7 @@ def algorithmic_bytes(wl, kv, plan, t):
             "total": kv_bytes + qo + partials + page_ids}
 
 
-def setup_workload(T, I, name, device, W=None, mode=None, c0=1):
+def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None):
     import torch
     wl = I.make_workload(name)
     t0 = time.perf_counter()
@@ -144,25 +144,32 @@ def setup_workload(T, I, name, device, W=None, mode=None, c0=1):
     if W is None:
         W = T.tangram_query_max_ctas(torch.cuda.current_device(), wl.d, wl.G)
     t3 = time.perf_counter()
-    plan = T.tangram_plan_partitions(tb, B, kv, W, wl.granule, c0, T.MODE_BALANCED if mode is None else mode)
+    dyn = (T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS) if dyn is None else dyn
+    plan = T.tangram_plan_partitions(tb, B, kv, W, wl.granule, c0, T.MODE_BALANCED if mode is None else mode, 0,
+                                     dyn[0], dyn[1])
     t4 = time.perf_counter()
     q, pool = I.make_q_and_pool(wl, n_pool, device)
     host_ms = {"reserve_ms": (t1 - t0) * 1e3, "tables_ms": (t2 - t1) * 1e3, "plan_ms": (t4 - t3) * 1e3}
     return dict(wl=wl, B=B, res=res, kv=kv, tables=tb, plan=plan, W=W, q=q, pool=pool, n_pool=n_pool,
-                host_ms=host_ms, c0=c0)
+                host_ms=host_ms, c0=c0, dyn=dyn)
 
 
 class L2Flusher:
-    """Writes a buffer larger than the 126 MB L2 between timed iterations."""
+    """Flushes the 126 MB L2 between timed iterations: writes a 256 MB buffer (evicts everything the
+    previous step left), then reads a second 256 MB buffer so that the dirty lines of the write are
+    themselves written back BEFORE the timed region starts -- otherwise up to ~126 MB of write-back
+    traffic from the flush would be charged to the step being timed."""
 
     def __init__(self, device, nbytes=256 << 20):
         import torch
         self.buf = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        self.rd = torch.zeros(nbytes // 4, dtype=torch.int32, device=device)
         self.v = 0
 
     def __call__(self):
         self.v = (self.v + 1) & 0x7F
         self.buf.fill_(self.v)
+        self.rd.max()
 
 
 def time_steps(fn, steps, warmup, flush, torch):
@@ -286,7 +293,7 @@ def reference_arm(args):
 def spread_of(T, S, torch, reps=5):
     """Per-CTA elapsed-time spread (max - min) / mean of the worker CTAs' busy time, from the
     globaltimer stamps of the instrumented build (median over reps)."""
-    W = S["W"]
+    W = S["plan"].n_static
     ns = torch.zeros(W, 2, dtype=torch.int64, device=S["q"].device)
     dp = S["dp"]
     vals = []
@@ -295,7 +302,7 @@ def spread_of(T, S, torch, reps=5):
         torch.cuda.synchronize()
         a = ns.cpu().numpy().astype(np.float64)
         busy = a[:, 1] - a[:, 0]
-        busy = busy[np.diff(S["plan"].worker_indptr) > 0]
+        busy = busy[np.diff(S["plan"].worker_indptr)[:W] > 0]
         vals.append(float((busy.max() - busy.min()) / busy.mean()))
     return float(np.median(vals))
 
@@ -310,10 +317,10 @@ def prepare(T, S, torch):
     S["bytes"] = algorithmic_bytes(wl, S["kv"], plan, S["tables"])
 
 
-def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, compare=True):
+def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, compare=True, dyn=None):
     """µs per layer-step, achieved TB/s, kernel-only roofline, spread, and the same kernel run from the
     STATIC_EVEN and SPLITMAP plans."""
-    S = setup_workload(T, I, name, device)
+    S = setup_workload(T, I, name, device, dyn=dyn)
     prepare(T, S, torch)
     step = lambda: T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"])
     ms = time_steps(step, steps, warmup, flush, torch)
@@ -328,7 +335,7 @@ def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, co
            "pct_of_measured_copy": 100 * b["total"] / (us * 1e-6) / 1e9 / peak_gbs,
            "decode_kernel_us": kus, "decode_kernel_gbs": b["total"] / (kus * 1e-6) / 1e9,
            "algorithmic_bytes": b, "W": S["W"], "items": int(S["plan"].n_items), "granule": S["wl"].granule,
-           "c0": S["c0"], "n_stages_smem": None, "host_ms": S["host_ms"],
+           "c0": S["c0"], "dyn_permille": S["dyn"][0], "dyn_rounds": S["dyn"][1], "host_ms": S["host_ms"],
            "cta_spread": spread_of(T, S, torch)}
     if compare:
         for mode, key in ((T.MODE_STATIC_EVEN, "static_even"), (T.MODE_SPLITMAP, "splitmap")):
@@ -373,6 +380,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the other configs' summary lines")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dyn-permille", type=int, default=None, help="dynamic-tail share of the BALANCED plan")
+    ap.add_argument("--dyn-rounds", type=int, default=None)
     args = ap.parse_args()
     if args.impl == "reference":
         reference_arm(args)
@@ -393,7 +402,8 @@ def main():
     peak_gbs, peak_src = measured_peak()
     flush = L2Flusher(device)
 
-    S = setup_workload(T, I, args.workload, device)
+    dyn = None if args.dyn_permille is None else (args.dyn_permille, args.dyn_rounds or 0)
+    S = setup_workload(T, I, args.workload, device, dyn=dyn)
     prepare(T, S, torch)
     step = lambda: T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"])
     for _ in range(args.warmup):
@@ -436,10 +446,11 @@ def main():
         "pct_of_measured_copy_peak": 100 * tbs * 1e3 / world / peak_gbs,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": args.workload, "R": S["wl"].R, "Hq": S["wl"].Hq, "H": S["wl"].H, "d": S["wl"].d,
-                   "page_size": S["wl"].P, "clusters": S["wl"].C, "plan": "balanced", "W": S["W"],
+                   "page_size": S["wl"].P, "clusters": S["wl"].C, "plan": "balanced", "W": S["W"], "dyn_permille": S["dyn"][0],
+                   "dyn_rounds": S["dyn"][1], "work_lists": int(S["plan"].W),
                    "granule": S["wl"].granule, "c0": S["c0"], "items": int(S["plan"].n_items),
                    "kv_bytes": b["kv"], "algorithmic_bytes": b["total"], "pool_bytes": S["pool"].numel() * 2,
-                   "l2": "inputs larger than L2 and a 256 MB L2 flush before every timed step",
+                   "l2": "inputs larger than L2 and an L2 flush (256 MB write, then 256 MB read) before every timed step",
                    "multi_gpu": "replicas only (path shards by request, no collective)"},
         "e2e": {"value": e_bytes / (e_ms * 1e-3) / 1e12, "unit": "TB/s", "us_per_layer_step": e_ms * 1e3,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -461,7 +472,7 @@ def main():
         del S
         torch.cuda.empty_cache()
         for name in ("tiny", "8b", "32b", "skew", "uniform"):
-            S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs)
+            S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs, dyn=dyn)
             if name == args.workload and not args.no_cpu_baseline:
                 from oracle import tangram_oracle as O
                 O.build_c()

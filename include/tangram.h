@@ -113,8 +113,16 @@ int tangram_build_ragged_tables(const double* B, const int32_t* reserved, int32_
  * (n_parts == 1: the decode kernel writes the final output directly, no merge).
  *
  *   t        tables from a2 (host)      B host [H]      kv_len host [R][H] i32 (<= cluster capacity)
- *   n_workers W >= 1 (persistent CTAs, from tangram_query_max_ctas)
+ *   n_workers >= 1 (persistent CTAs = launch grid, from tangram_query_max_ctas)
  *   granule_tokens g: positive multiple of t->P;  overhead_granules c0 >= 0
+ *   dyn_permille, dyn_rounds (BALANCED only; both 0 = every CTA owns exactly one list, the purely
+ *       static plan): the last dyn_permille/1000 of the cost axis is not pre-assigned to a CTA but
+ *       cut into dyn_rounds rounds of n_workers lists each -- round j < dyn_rounds takes 2^-j of
+ *       that share, the last round the rest -- which the CTAs claim in list order when they run
+ *       out of work.  Everything is still computed offline; the claim only decides WHICH CTA runs
+ *       a precomputed list, which is what absorbs the stable +-15 % per-SM bandwidth differences
+ *       measured on B200.  List k covers cost positions [b_k, b_{k+1}),
+ *       b_k = floor(T * cumw_k / cumw_W) with the integer list weights of DESIGN.md §Planner.
  *   out      caller-filled: split_map [C], worker_indptr [W+1], part_indptr [R*H+1], items
  *            [items_cap] (or items == NULL to query: n_items / n_part_slots only).
  *            split_map always receives Algorithm 1's S (the constant S for STATIC_EVEN).
@@ -126,7 +134,9 @@ typedef struct tangram_item { /* 32 bytes */
     int32_t req, kv_head, cluster, slot, tok_begin, tok_end, part_slot, n_parts;
 } tangram_item;
 typedef struct tangram_plan {
-    int32_t W, mode;
+    int32_t W;        /* work lists in total = n_static * (1 + dyn_rounds) */
+    int32_t n_static; /* = n_workers: lists 0..n_static-1 belong to CTA 0..n_static-1 (the launch grid) */
+    int32_t mode, reserved_;
     int64_t n_items, n_part_slots;
     int32_t* split_map;     /* host [C] */
     tangram_item* items;    /* host [items_cap], worker-major */
@@ -136,7 +146,8 @@ typedef struct tangram_plan {
 } tangram_plan;
 int tangram_plan_partitions(const tangram_tables* t, const double* B, const int32_t* kv_len,
                             int32_t n_workers, int32_t granule_tokens, int32_t overhead_granules,
-                            int32_t mode, int32_t static_splits, tangram_plan* out);
+                            int32_t mode, int32_t static_splits, int32_t dyn_permille, int32_t dyn_rounds,
+                            tangram_plan* out);
 
 /* ------------------------------------------------------------------------------------------------
  * Device side.  One upload of tables + plan per (batch, layer); then one
@@ -154,12 +165,16 @@ size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan* p);
 /* Host-side view of an uploaded plan: sizes plus DEVICE pointers into the blob.  Plain data; valid
  * as long as the blob is. */
 typedef struct tangram_device_plan {
-    int32_t R, H, C, Hp, P, W, mode, reserved_;
+    int32_t R, H, C, Hp, P, W /* work lists */, mode, n_static /* launch grid */;
     int64_t n_items, n_part_slots;
+    int64_t n_merge_seqs;       /* sequences whose part count is not 1 (they need the merge kernel) */
+    const int32_t* merge_seqs;  /* device [n_merge_seqs]: r * H + h */
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
     const int64_t* worker_indptr; /* device [W+1] */
     const int64_t* part_indptr;   /* device [R*H+1] */
     const int32_t* tbl_pages;     /* device page ids */
+    int32_t* sched;               /* device [2]: list-claim counter and CTAs-done counter of the dynamic
+                                     tail; zero between launches (the kernel re-arms them itself) */
 } tangram_device_plan;
 
 /* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte

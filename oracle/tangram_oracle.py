@@ -173,7 +173,8 @@ def split_map(B, perm, Hp: int, n_cta: int) -> np.ndarray:
 
 @dataclasses.dataclass
 class Plan:
-    W: int
+    W: int                      # work lists in total (= n_static * (1 + dyn_rounds) with a dynamic tail)
+    n_static: int               # lists 0..n_static-1 are the CTAs' own
     mode: int
     split_map: np.ndarray       # [C] int32 (SPLITMAP: Alg. 1; STATIC_EVEN: constant; BALANCED: Alg. 1, informational)
     items: np.ndarray           # [n_items, 8] int32: req, kv_head, cluster, slot, tok_begin, tok_end, part_slot, n_parts
@@ -183,7 +184,8 @@ class Plan:
     n_part_slots: int
 
 
-def _finish(raw: List[Tuple[int, int, int, int, int]], t: Tables, W: int, mode: int, S) -> Plan:
+def _finish(raw: List[Tuple[int, int, int, int, int]], t: Tables, W: int, mode: int, S,
+            n_static: Optional[int] = None) -> Plan:
     """raw: (worker, r, h, tok_begin, tok_end) in plan order.  Assigns part_slot / n_parts and
     lays the items out worker-major, plan order kept inside a worker."""
     R, H = t.R, t.H
@@ -215,20 +217,38 @@ def _finish(raw: List[Tuple[int, int, int, int, int]], t: Tables, W: int, mode: 
                         part_indptr[s] + ordinal[idx], count[s])
             k += 1
         worker_indptr.append(k)
-    return Plan(W=W, mode=mode, split_map=np.asarray(S, dtype=np.int32), items=items,
+    return Plan(W=W, n_static=W if n_static is None else n_static, mode=mode,
+                split_map=np.asarray(S, dtype=np.int32), items=items,
                 worker_indptr=np.array(worker_indptr, dtype=np.int64),
                 part_indptr=np.array(part_indptr, dtype=np.int64), n_items=len(raw),
                 n_part_slots=part_indptr[-1])
 
 
+def list_weights(n_workers: int, dyn_permille: int, dyn_rounds: int) -> List[int]:
+    """Relative sizes of the BALANCED work lists.  No dynamic tail: n_workers
+    lists of weight 1.  With a tail of dyn_permille/1000 of the cost handed out in J = dyn_rounds
+    rounds (round j < J takes 2^-j of the tail, the last round the rest): the n_workers static
+    lists weigh (1000 - dyn) 2^(J-1) each, a list of round j < J weighs dyn 2^(J-1-j), a list of the
+    last round weighs dyn."""
+    if dyn_rounds == 0:
+        return [1] * n_workers
+    J = dyn_rounds
+    w = [(1000 - dyn_permille) * 2 ** (J - 1)] * n_workers
+    for j in range(1, J + 1):
+        w += [dyn_permille * 2 ** (J - 1 - j) if j < J else dyn_permille] * n_workers
+    return w
+
+
 def plan_partitions(t: Tables, B, kv_len, n_workers: int, granule: int, overhead_granules: int,
-                    mode: int, static_splits: int = 0) -> Plan:
+                    mode: int, static_splits: int = 0, dyn_permille: int = 0, dyn_rounds: int = 0) -> Plan:
     """Offline deterministic planner (§4.3).  Sequences are visited r-major, then in `perm`
     order, so neighbours share a page table."""
     kv_len = np.asarray(kv_len)
     R, H, W, g, c0 = t.R, t.H, int(n_workers), int(granule), int(overhead_granules)
     if W < 1 or g < 1 or g % t.P != 0 or c0 < 0:
         raise ValueError("bad planner arguments (granule must be a positive multiple of P)")
+    if not (0 <= dyn_permille < 1000 and 0 <= dyn_rounds <= 16 and (dyn_permille > 0) == (dyn_rounds > 0)):
+        raise ValueError("bad dynamic-tail arguments")
     S_alg1 = split_map(B, t.perm, t.Hp, W)
     seqs = [(r, int(t.perm[j])) for r in range(R) for j in range(H)]
     raw: List[Tuple[int, int, int, int, int]] = []
@@ -239,7 +259,12 @@ def plan_partitions(t: Tables, B, kv_len, n_workers: int, granule: int, overhead
         u = [-(-int(kv_len[r, h]) // g) for (r, h) in seqs]
         w = [ui + (c0 if ui > 0 else 0) for ui in u]
         T = sum(w)
-        b = [(k * T) // W for k in range(W + 1)]
+        lw = list_weights(W, dyn_permille, dyn_rounds)
+        n_static, W = W, len(lw)
+        cum = [0]
+        for x in lw:
+            cum.append(cum[-1] + x)
+        b = [(T * cum[k]) // cum[W] for k in range(W + 1)]   # list k owns positions [b_k, b_{k+1})
         a = 0
         k = 0
         for i, (r, h) in enumerate(seqs):
@@ -257,7 +282,7 @@ def plan_partitions(t: Tables, B, kv_len, n_workers: int, granule: int, overhead
             if run_start is not None:
                 raw.append((run_worker, r, h, run_start * g, n))
             a += w[i]
-        return _finish(raw, t, W, mode, S_alg1)
+        return _finish(raw, t, W, mode, S_alg1, n_static)
 
     if mode == MODE_SPLITMAP:
         S = S_alg1

@@ -20,6 +20,8 @@ LIB_PATH = os.path.join(_HERE, "libtangram.so")
 OK, ERR_INVALID_ARG, ERR_OUT_OF_PAGES, ERR_BUFFER_TOO_SMALL, ERR_CUDA = 0, -1, -2, -3, -4
 FILL_GROUP = 1
 MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
+# dynamic tail of the BALANCED plan used by bench.py / smoke (tuned on B200)
+DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 250, 4
 MODE_NAMES = {MODE_BALANCED: "balanced", MODE_SPLITMAP: "splitmap", MODE_STATIC_EVEN: "static_even"}
 
 if not os.path.exists(LIB_PATH):
@@ -42,16 +44,18 @@ class _Tables(C.Structure):
 
 
 class _Plan(C.Structure):
-    _fields_ = [("W", C.c_int32), ("mode", C.c_int32), ("n_items", C.c_int64), ("n_part_slots", C.c_int64),
+    _fields_ = [("W", C.c_int32), ("n_static", C.c_int32), ("mode", C.c_int32), ("reserved_", C.c_int32),
+                ("n_items", C.c_int64), ("n_part_slots", C.c_int64),
                 ("split_map", C.c_void_p), ("items", C.c_void_p), ("items_cap", C.c_int64),
                 ("worker_indptr", C.c_void_p), ("part_indptr", C.c_void_p)]
 
 
 class _DevicePlan(C.Structure):
     _fields_ = [("R", C.c_int32), ("H", C.c_int32), ("C", C.c_int32), ("Hp", C.c_int32), ("P", C.c_int32),
-                ("W", C.c_int32), ("mode", C.c_int32), ("reserved_", C.c_int32), ("n_items", C.c_int64),
-                ("n_part_slots", C.c_int64), ("items", C.c_void_p), ("worker_indptr", C.c_void_p),
-                ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p)]
+                ("W", C.c_int32), ("mode", C.c_int32), ("n_static", C.c_int32), ("n_items", C.c_int64),
+                ("n_part_slots", C.c_int64), ("n_merge_seqs", C.c_int64), ("merge_seqs", C.c_void_p),
+                ("items", C.c_void_p), ("worker_indptr", C.c_void_p),
+                ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p)]
 
 
 _lib.tangram_last_error.restype = C.c_char_p
@@ -151,7 +155,8 @@ def tangram_build_ragged_tables(B, reserved, n_clusters: int, page_size: int, fr
 # ------------------------------------------------------------------------------------------ a3
 @dataclasses.dataclass
 class Plan:
-    W: int
+    W: int                     # work lists in total
+    n_static: int              # launch grid: lists 0..n_static-1 are the CTAs' own
     mode: int
     split_map: np.ndarray      # [C]
     items: np.ndarray          # [n_items, 8] i32: req, kv_head, cluster, slot, tok_begin, tok_end, part_slot, n_parts
@@ -161,21 +166,23 @@ class Plan:
     n_part_slots: int
 
     def _c(self) -> _Plan:
-        return _Plan(self.W, self.mode, self.n_items, self.n_part_slots, _ptr(self.split_map), _ptr(self.items),
+        return _Plan(self.W, self.n_static, self.mode, 0, self.n_items, self.n_part_slots, _ptr(self.split_map),
+                     _ptr(self.items),
                      self.items.shape[0], _ptr(self.worker_indptr), _ptr(self.part_indptr))
 
 
 def tangram_plan_partitions(t: Tables, B, kv_len, n_workers: int, granule_tokens: int, overhead_granules: int,
-                            mode: int, static_splits: int = 0) -> Plan:
+                            mode: int, static_splits: int = 0, dyn_permille: int = 0, dyn_rounds: int = 0) -> Plan:
     B, kv = _np(B, np.float64), _np(kv_len, np.int32)
     ct = t._c()
     split_map = np.zeros(t.C, np.int32)
-    q = _Plan(0, 0, 0, 0, _ptr(split_map), None, 0, None, None)
+    q = _Plan(0, 0, 0, 0, 0, 0, _ptr(split_map), None, 0, None, None)
     args = (C.byref(ct), _ptr(B), _ptr(kv), C.c_int32(n_workers), C.c_int32(granule_tokens),
-            C.c_int32(overhead_granules), C.c_int32(mode), C.c_int32(static_splits))
+            C.c_int32(overhead_granules), C.c_int32(mode), C.c_int32(static_splits), C.c_int32(dyn_permille),
+            C.c_int32(dyn_rounds))
     _check(_lib.tangram_plan_partitions(*args, C.byref(q)))
-    pl = Plan(n_workers, mode, split_map, np.zeros((max(int(q.n_items), 1), 8), np.int32),
-              np.zeros(n_workers + 1, np.int64), np.zeros(t.R * t.H + 1, np.int64), int(q.n_items),
+    pl = Plan(int(q.W), int(q.n_static), mode, split_map, np.zeros((max(int(q.n_items), 1), 8), np.int32),
+              np.zeros(int(q.W) + 1, np.int64), np.zeros(t.R * t.H + 1, np.int64), int(q.n_items),
               int(q.n_part_slots))
     cp = pl._c()
     _check(_lib.tangram_plan_partitions(*args, C.byref(cp)))

@@ -22,9 +22,12 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstdint>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include "tangram.h"
@@ -51,7 +54,8 @@ struct DecodeParams {
     float* part_o;
     float* part_lse;
     unsigned long long* worker_ns;
-    int32_t Hq, G, Hp, n_stages;
+    int* sched;  // [0] next list to claim (relative to gridDim.x), [1] CTAs done; both 0 between launches
+    int32_t Hq, G, Hp, n_stages, n_lists;
     float scale_log2;
 };
 
@@ -162,9 +166,6 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
 
     const int NS = p.n_stages, G = p.G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t it_begin = p.worker_indptr[blockIdx.x];
-    const int n_items = static_cast<int>(p.worker_indptr[blockIdx.x + 1] - it_begin);
-
     const uint32_t tiles = smem_u32(smem);
     uint8_t* q_ring = smem + L::off_q(NS);
     uint8_t* desc_ring = smem + L::off_desc(NS, G);
@@ -191,47 +192,86 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    asm volatile("griddepcontrol.launch_dependents;");  // lets the merge grid's launch overlap this kernel
 
     if (warp == kNW) {
         // ============================== producer warp ==============================
         uint64_t policy;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
         uint32_t stage = 0, phase = 0;  // lane w < 8 tracks consumer warp w's ring
-        int rot = 0;
+        // Work lists: list blockIdx.x is this CTA's own; with a dynamic tail (n_lists > gridDim.x) further
+        // lists are claimed from a global counter, two lists ahead so that neither the atomic nor the
+        // dependent loads (list range -> first item -> page ids) ever stall the TMA issue.
+        const bool dynamic = p.n_lists > static_cast<int>(gridDim.x);
+        auto claim = [&]() {
+            int v = 0;
+            if (lane == 0) v = atomicAdd(p.sched, 1) + static_cast<int>(gridDim.x);
+            return v;
+        };
+        int nxt = p.n_lists;
+        if (dynamic) nxt = __shfl_sync(0xffffffffu, claim(), 0);
+        int64_t cb = p.worker_indptr[blockIdx.x], ce = p.worker_indptr[blockIdx.x + 1];
+        int64_t nb = 0, ne = 0;
+        if (nxt < p.n_lists) nb = p.worker_indptr[nxt], ne = p.worker_indptr[nxt + 1];
         DeviceItem next;
-        if (n_items > 0) next = p.items[it_begin];
-        for (int it = 0; it < n_items; ++it) {
-            const DeviceItem item = next;
-            if (it + 1 < n_items) next = p.items[it_begin + it + 1];
-            const int qs = it % kQSlots;
-            const uint32_t qpar = (it / kQSlots) & 1;
-            if (lane == 0) {
-                mbar_wait(qempty_bar(qs), qpar ^ 1);
-                *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = item;
-                const uint32_t qbytes = static_cast<uint32_t>(G * D * 2);
-                mbar_arrive_expect_tx(qfull_bar(qs), qbytes);
-                bulk_load(smem_u32(q_ring + qs * q_slot_bytes),
-                          p.q + (static_cast<size_t>(item.req) * p.Hq + static_cast<size_t>(item.kv_head) * G) * D,
-                          qbytes, qfull_bar(qs));
-            }
-            const int n_tiles = (item.tok_end - item.tok_begin + kPage - 1) / kPage;
-            if (lane < kNW) {
-                const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
-                int i = (lane - rot) & (kNW - 1);
-                int pid = i < n_tiles ? __ldg(ids + i) : 0;
-                while (i < n_tiles) {
-                    const int i_next = i + kNW;
-                    const int pid_next = i_next < n_tiles ? __ldg(ids + i_next) : 0;
-                    mbar_wait(empty_bar(lane, stage), phase ^ 1);
-                    mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
-                    tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
-                                  (pid * p.Hp + item.slot) * (2 * kPage), policy);
-                    if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
-                    i = i_next, pid = pid_next;
+        if (cb < ce) next = p.items[cb];
+        int seq = 0;  // running item number = position in the item / query ring
+        for (;;) {
+            int fut = p.n_lists;
+            if (dynamic && nxt < p.n_lists) fut = claim();  // consumed when this list is done
+            for (int64_t it = cb; it < ce; ++it, ++seq) {
+                const DeviceItem item = next;
+                if (it + 1 < ce) next = p.items[it + 1];
+                else if (nb < ne) next = p.items[nb];
+                const int qs = seq % kQSlots;
+                const uint32_t qpar = (seq / kQSlots) & 1;
+                if (lane == 0) {
+                    mbar_wait(qempty_bar(qs), qpar ^ 1);
+                    *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = item;
+                    const uint32_t qbytes = static_cast<uint32_t>(G * D * 2);
+                    mbar_arrive_expect_tx(qfull_bar(qs), qbytes);
+                    bulk_load(smem_u32(q_ring + qs * q_slot_bytes),
+                              p.q + (static_cast<size_t>(item.req) * p.Hq + static_cast<size_t>(item.kv_head) * G) * D,
+                              qbytes, qfull_bar(qs));
                 }
+                const int n_tiles = (item.tok_end - item.tok_begin + kPage - 1) / kPage;
+                const int rot = item.part_slot & (kNW - 1);  // which warp gets the item's first tile
+                if (lane < kNW) {
+                    const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
+                    int i = (lane - rot) & (kNW - 1);
+                    int pid = i < n_tiles ? __ldg(ids + i) : 0;
+                    while (i < n_tiles) {
+                        const int i_next = i + kNW;
+                        const int pid_next = i_next < n_tiles ? __ldg(ids + i_next) : 0;
+                        mbar_wait(empty_bar(lane, stage), phase ^ 1);
+                        mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
+                        tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
+                                      (pid * p.Hp + item.slot) * (2 * kPage), policy);
+                        if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
+                        i = i_next, pid = pid_next;
+                    }
+                }
+                __syncwarp();
             }
-            __syncwarp();
-            rot = (rot + n_tiles) & (kNW - 1);
+            if (cb == ce && nb < ne) next = p.items[nb];
+            if (nxt >= p.n_lists) break;
+            cb = nb, ce = ne;
+            nxt = dynamic ? __shfl_sync(0xffffffffu, fut, 0) : p.n_lists;
+            nb = ne = 0;
+            if (nxt < p.n_lists) nb = p.worker_indptr[nxt], ne = p.worker_indptr[nxt + 1];
+        }
+        if (lane == 0) {
+            // end-of-work sentinel for the consumers
+            const int qs = seq % kQSlots;
+            mbar_wait(qempty_bar(qs), ((seq / kQSlots) & 1) ^ 1);
+            DeviceItem stop{};
+            stop.n_parts = -1;
+            *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = stop;
+            mbar_arrive(qfull_bar(qs));
+            if (dynamic) {
+                // the last CTA to finish re-arms the counters for the next launch on this plan
+                if (atomicAdd(p.sched + 1, 1) == static_cast<int>(gridDim.x) - 1) p.sched[0] = 0, p.sched[1] = 0;
+            }
         }
         return;
     }
@@ -241,13 +281,13 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     const int qd = lane & 3;
     const bool row_ok = row < G;
     uint32_t stage = 0, phase = 0;
-    int rot = 0;
     constexpr float kNegInf = -INFINITY;
 
-    for (int it = 0; it < n_items; ++it) {
+    for (int it = 0;; ++it) {
         const int qs = it % kQSlots;
         mbar_wait(qfull_bar(qs), (it / kQSlots) & 1);
         const DeviceItem item = *reinterpret_cast<const DeviceItem*>(desc_ring + qs * 32);
+        if (item.n_parts < 0) break;  // producer's end-of-work sentinel
         uint32_t qa[D / 16][2];
         {
             const uint8_t* qrow = q_ring + qs * q_slot_bytes + row * D * 2;
@@ -262,6 +302,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
 
         const int n_tok = item.tok_end - item.tok_begin;
         const int n_tiles = (n_tok + kPage - 1) / kPage;
+        const int rot = item.part_slot & (kNW - 1);  // a function of the item only: results do not depend on which CTA runs it
         float m = kNegInf, l = 0.f;
         float o[D / 8][2];
 #pragma unroll
@@ -338,7 +379,6 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             if (lane == 0) mbar_arrive(empty_bar(warp, stage));
             if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
         }
-        rot = (rot + n_tiles) & (kNW - 1);
 
         // ---- combine the eight warp states of this item
         l += __shfl_xor_sync(0xffffffffu, l, 1);
@@ -384,52 +424,85 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
 }
 
 // ------------------------------------------------------------------ a5: LSE merge kernel
-// One warp per (request, query head).  Sequences with one part were written by the decode kernel;
-// sequences with no retained token get out = 0, lse = -inf.
+// One CTA of 8 warps per (sequence that needs a merge, query head of its group).  `merge_seqs` lists
+// the sequences (r * H + h) whose part count is not 1 (built at upload time): sequences with one
+// part were written by the decode kernel; sequences with no retained token get out = 0, lse = -inf.
+// Warp w accumulates parts w, w + 8, ... (four loads in flight per lane), then the eight warp sums are
+// combined in a fixed order, so the result is deterministic.
+constexpr int kMergeWarps = 8;
 template <int D>
-__global__ void __launch_bounds__(128)
-tangram_merge_kernel(const int64_t* __restrict__ part_indptr, const float* __restrict__ part_o,
-                     const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
-                     float* __restrict__ lse, int R, int H, int G) {
+__global__ void __launch_bounds__(kMergeWarps * 32)
+tangram_merge_kernel(const int32_t* __restrict__ merge_seqs, const int64_t* __restrict__ part_indptr,
+                     const float* __restrict__ part_o, const float* __restrict__ part_lse,
+                     __nv_bfloat16* __restrict__ out, float* __restrict__ lse, int H, int G) {
     constexpr int V = D / 32;  // floats per lane
-    const int Hq = H * G;
-    const int gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (gw >= R * Hq) return;
-    const int r = gw / Hq, j = gw % Hq, h = j / G, gi = j % G;
-    const int64_t p0 = part_indptr[static_cast<int64_t>(r) * H + h];
-    const int n = static_cast<int>(part_indptr[static_cast<int64_t>(r) * H + h + 1] - p0);
-    if (n == 1) return;
-    __nv_bfloat16* dst = out + static_cast<size_t>(gw) * D + lane * V;
+    using VecT = typename std::conditional<V == 4, float4, float2>::type;
+    __shared__ float s_red[kMergeWarps];
+    __shared__ float s_acc[kMergeWarps][D + 1];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int seq = merge_seqs[blockIdx.x / G], gi = blockIdx.x % G;
+    const int r = seq / H, h = seq % H;
+    const int64_t p0 = part_indptr[seq];
+    const int n = static_cast<int>(part_indptr[seq + 1] - p0);
+    const size_t row = (static_cast<size_t>(r) * H + h) * G + gi;  // = r * Hq + h * G + gi
+    // everything above reads plan data only; the partials / outputs need the decode grid to be done
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (n == 0) {
-#pragma unroll
-        for (int e = 0; e < V; ++e) dst[e] = __float2bfloat16(0.f);
-        if (lane == 0) lse[gw] = -INFINITY;
+        if (threadIdx.x < D / 2)
+            reinterpret_cast<__nv_bfloat162*>(out + row * D)[threadIdx.x] = __floats2bfloat162_rn(0.f, 0.f);
+        if (threadIdx.x == 0) lse[row] = -INFINITY;
         return;
     }
     float M = -INFINITY;
-    for (int i = lane; i < n; i += 32) M = fmaxf(M, part_lse[(p0 + i) * G + gi]);
+    for (int i = threadIdx.x; i < n; i += kMergeWarps * 32) M = fmaxf(M, part_lse[(p0 + i) * G + gi]);
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, s));
+    if (lane == 0) s_red[warp] = M;
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < kMergeWarps; ++w) M = fmaxf(M, s_red[w]);
+    __syncthreads();
+
     float acc[V], tot = 0.f;
 #pragma unroll
     for (int e = 0; e < V; ++e) acc[e] = 0.f;
-    for (int i = 0; i < n; ++i) {
-        const float w = __expf(part_lse[(p0 + i) * G + gi] - M);
-        tot += w;
-        const float* src = part_o + ((p0 + i) * G + gi) * D + lane * V;
-        if constexpr (V == 4) {
-            const float4 v = *reinterpret_cast<const float4*>(src);
-            acc[0] += w * v.x, acc[1] += w * v.y, acc[2] += w * v.z, acc[3] += w * v.w;
-        } else {
-            const float2 v = *reinterpret_cast<const float2*>(src);
-            acc[0] += w * v.x, acc[1] += w * v.y;
+    const size_t stride = static_cast<size_t>(G) * D;
+    const float* src = part_o + (p0 * G + gi) * D + lane * V;
+    for (int i = warp; i < n; i += 4 * kMergeWarps) {
+        VecT v[4];
+        float w[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int ii = i + u * kMergeWarps;
+            const bool ok = ii < n;
+            v[u] = *reinterpret_cast<const VecT*>(src + (ok ? ii : i) * stride);
+            w[u] = ok ? __expf(part_lse[(p0 + ii) * G + gi] - M) : 0.f;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            tot += w[u];
+            if constexpr (V == 4) {
+                acc[0] += w[u] * v[u].x, acc[1] += w[u] * v[u].y, acc[2] += w[u] * v[u].z, acc[3] += w[u] * v[u].w;
+            } else {
+                acc[0] += w[u] * v[u].x, acc[1] += w[u] * v[u].y;
+            }
         }
     }
-    const float inv = 1.f / tot;
 #pragma unroll
-    for (int e = 0; e < V; e += 2)
-        *reinterpret_cast<__nv_bfloat162*>(dst + e) = __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
-    if (lane == 0) lse[gw] = M + __logf(tot);
+    for (int e = 0; e < V; ++e) s_acc[warp][lane * V + e] = acc[e];
+    if (lane == 0) s_red[warp] = tot;
+    __syncthreads();
+    if (threadIdx.x < D / 2) {
+        float t = 0.f, x = 0.f, y = 0.f;
+#pragma unroll
+        for (int w = 0; w < kMergeWarps; ++w) {
+            t += s_red[w];
+            x += s_acc[w][2 * threadIdx.x], y += s_acc[w][2 * threadIdx.x + 1];
+        }
+        const float inv = 1.f / t;
+        reinterpret_cast<__nv_bfloat162*>(out + row * D)[threadIdx.x] = __floats2bfloat162_rn(x * inv, y * inv);
+        if (threadIdx.x == 0) lse[row] = M + __logf(t);
+    }
 }
 
 // ------------------------------------------------------------------ host-side launch helpers
@@ -481,18 +554,29 @@ static int launch_decode(const tangram_device_plan* dp, const DecodeParams& prm,
     } else if (prm.worker_ns) {
         e = cudaFuncSetAttribute(tangram_decode_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
-        tangram_decode_kernel<D, true><<<dp->W, kThreads, smem, stream>>>(map, prm);
+        tangram_decode_kernel<D, true><<<dp->n_static, kThreads, smem, stream>>>(map, prm);
     } else {
         e = cudaFuncSetAttribute(tangram_decode_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
-        tangram_decode_kernel<D, false><<<dp->W, kThreads, smem, stream>>>(map, prm);
+        tangram_decode_kernel<D, false><<<dp->n_static, kThreads, smem, stream>>>(map, prm);
     }
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
     if (!(which & kRunMerge)) return TANGRAM_OK;
-    const int n_rows = dp->R * prm.Hq;
-    tangram_merge_kernel<D><<<(n_rows + 3) / 4, 128, 0, stream>>>(dp->part_indptr, prm.part_o, prm.part_lse, prm.out,
-                                                                prm.lse, dp->R, dp->H, prm.G);
+    if (dp->n_merge_seqs == 0) return TANGRAM_OK;
+    // Programmatic dependent launch: the merge grid is scheduled while the decode grid drains and
+    // blocks in griddepcontrol.wait until the decode grid has completed and flushed its writes.
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(dp->n_merge_seqs * prm.G)), cfg.blockDim = dim3(kMergeWarps * 32), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr, cfg.numAttrs = 1;
+    const float* po = prm.part_o;
+    const float* pl = prm.part_lse;
+    e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, dp->part_indptr, po, pl, prm.out, prm.lse,
+                           (int)dp->H, (int)prm.G);
+    if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
     return TANGRAM_OK;
@@ -533,7 +617,8 @@ extern "C" size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan
     b += align_up(sizeof(int64_t) * ((size_t)p->W + 1), 256);
     b += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
     b += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
-    return b + 256;
+    b += align_up(sizeof(int32_t) * (size_t)t->R * t->H, 256);  // merge_seqs (upper bound)
+    return b + 256 /* scheduler counters */ + 256;
 }
 
 extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
@@ -564,6 +649,14 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     off += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
     const size_t off_pages = off;
     std::memcpy(host.data() + off, t->tbl_pages, sizeof(int32_t) * (size_t)t->n_pages_used);
+    off += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
+    const size_t off_mseq = off;
+    int32_t* mseq = reinterpret_cast<int32_t*>(host.data() + off);
+    int64_t n_mseq = 0;
+    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)
+        if (p->part_indptr[sq + 1] - p->part_indptr[sq] != 1) mseq[n_mseq++] = (int32_t)sq;
+    off += align_up(sizeof(int32_t) * (size_t)t->R * t->H, 256);
+    const size_t off_sched = off;
     // pageable source: the runtime stages it before returning, so `host` may die at scope exit
     cudaError_t e = cudaMemcpyAsync(dev_blob, host.data(), need, cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "upload: cudaMemcpyAsync");
@@ -571,7 +664,10 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     if (e != cudaSuccess) return cuda_fail(e, "upload: cudaStreamSynchronize");
     uint8_t* base = static_cast<uint8_t*>(dev_blob);
     dp->R = t->R, dp->H = t->H, dp->C = t->C, dp->Hp = t->Hp, dp->P = t->P, dp->W = p->W, dp->mode = p->mode;
-    dp->reserved_ = 0;
+    dp->n_static = p->n_static;
+    dp->sched = reinterpret_cast<int32_t*>(base + off_sched);
+    dp->merge_seqs = reinterpret_cast<const int32_t*>(base + off_mseq);
+    dp->n_merge_seqs = n_mseq;
     dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
     dp->items = base + off_items;
     dp->worker_indptr = reinterpret_cast<const int64_t*>(base + off_windptr);
@@ -594,7 +690,7 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > kMaxG)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d)", Hq,
                     dp->H, kMaxG);
-    if (n_pool_pages < 1 || dp->W < 1) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool or plan");
+    if (n_pool_pages < 1 || dp->W < 1 || dp->n_static < 1 || dp->n_static > dp->W) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool or plan");
     if (reinterpret_cast<uintptr_t>(q) % 16 || reinterpret_cast<uintptr_t>(kv_pool) % 128 ||
         reinterpret_cast<uintptr_t>(out) % 16 || reinterpret_cast<uintptr_t>(workspace) % 16)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: misaligned pointer");
@@ -622,7 +718,10 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
                                             align_up((size_t)dp->n_part_slots * G * d * 4, 256));
     prm.worker_ns = reinterpret_cast<unsigned long long*>(worker_ns);
     prm.Hq = Hq, prm.G = G, prm.Hp = dp->Hp;
+    prm.n_lists = dp->W;
+    prm.sched = dp->sched;
     prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);
+    if (const char* dbg = getenv("TANGRAM_DEBUG_STAGES")) prm.n_stages = std::min(prm.n_stages, atoi(dbg));
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
     prm.scale_log2 = scale * 1.4426950408889634f;
     cudaStream_t st = static_cast<cudaStream_t>(stream);

@@ -155,15 +155,22 @@ extern "C" int tangram_build_ragged_tables(const double* B, const int32_t* reser
 extern "C" int tangram_plan_partitions(const tangram_tables* t, const double* B, const int32_t* kv_len,
                                        int32_t n_workers, int32_t granule_tokens,
                                        int32_t overhead_granules, int32_t mode, int32_t static_splits,
-                                       tangram_plan* out) {
+                                       int32_t dyn_permille, int32_t dyn_rounds, tangram_plan* out) {
     if (!t || !B || !kv_len || !out) return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: NULL argument");
     if (!t->perm || !t->cluster_of || !t->slot_of || !t->tbl_indptr)
         return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: tables not filled");
     const int32_t R = t->R, H = t->H, C = t->C, Hp = t->Hp, P = t->P;
-    const int32_t W = n_workers, g = granule_tokens, c0 = overhead_granules;
-    if (W < 1 || g < 1 || P < 1 || g % P != 0 || c0 < 0)
+    const int32_t NW = n_workers, g = granule_tokens, c0 = overhead_granules;
+    if (NW < 1 || g < 1 || P < 1 || g % P != 0 || c0 < 0)
         return fail(TANGRAM_ERR_INVALID_ARG,
-                    "plan_partitions: W=%d granule=%d (must be a positive multiple of P=%d) overhead=%d", W, g, P, c0);
+                    "plan_partitions: W=%d granule=%d (must be a positive multiple of P=%d) overhead=%d", NW, g, P, c0);
+    if (dyn_permille < 0 || dyn_permille >= 1000 || dyn_rounds < 0 || dyn_rounds > 16 ||
+        (dyn_permille > 0) != (dyn_rounds > 0))
+        return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: dyn_permille=%d dyn_rounds=%d", dyn_permille, dyn_rounds);
+    // Work-list slots: the first NW are the CTAs' own lists; with a dynamic tail (BALANCED only) they
+    // are followed by dyn_rounds rounds of NW smaller lists that the CTAs claim in order at run time.
+    const bool tail = mode == TANGRAM_MODE_BALANCED && dyn_rounds > 0;
+    const int32_t W = tail ? NW * (1 + dyn_rounds) : NW;
     if (mode != TANGRAM_MODE_BALANCED && mode != TANGRAM_MODE_SPLITMAP && mode != TANGRAM_MODE_STATIC_EVEN)
         return fail(TANGRAM_ERR_INVALID_ARG, "plan_partitions: mode=%d", mode);
     for (int32_t r = 0; r < R; ++r)
@@ -177,7 +184,7 @@ extern "C" int tangram_plan_partitions(const tangram_tables* t, const double* B,
         }
 
     std::vector<int32_t> S(C);
-    algorithm1(B, t->perm, H, Hp, W, S.data());
+    algorithm1(B, t->perm, H, Hp, NW, S.data());
     std::vector<RawItem> raw;
     const int64_t n_seq = (int64_t)R * H;
     raw.reserve((size_t)(n_seq + W));
@@ -191,7 +198,22 @@ extern "C" int tangram_plan_partitions(const tangram_tables* t, const double* B,
                 const int64_t u = (kv_len[(size_t)r * H + h] + (int64_t)g - 1) / g;
                 T += u + (u > 0 ? c0 : 0);
             }
-        auto cut = [&](int64_t k) { return (k * T) / W; };
+        // Relative size of list k: (1000 - dyn) 2^(J-1) for the NW static lists; dyn 2^(J-1-j) for the
+        // lists of round j = 1..J-1 and dyn for the last round J (each round hands out half of what is
+        // left, the last one all of it).  b_k = floor(T cumw_k / cumw_W).
+        std::vector<int64_t> cumw((size_t)W + 1, 0);
+        for (int32_t k = 0; k < W; ++k) {
+            int64_t w = 1;
+            if (tail) {
+                const int32_t J = dyn_rounds, round = k / NW;  // 0 = static
+                if (round == 0) w = (int64_t)(1000 - dyn_permille) << (J - 1);
+                else if (round < J) w = (int64_t)dyn_permille << (J - 1 - round);
+                else w = dyn_permille;
+            }
+            cumw[(size_t)k + 1] = cumw[(size_t)k] + w;
+        }
+        const int64_t totw = cumw[(size_t)W];
+        auto cut = [&](int64_t k) { return (int64_t)(((__int128)T * cumw[(size_t)k]) / totw); };
         int64_t pos = 0;   // cost position where the current sequence starts
         int64_t k = 0;     // current worker
         for (int32_t r = 0; r < R; ++r)
@@ -235,7 +257,7 @@ extern "C" int tangram_plan_partitions(const tangram_tables* t, const double* B,
             }
     }
 
-    out->W = W, out->mode = mode;
+    out->W = W, out->n_static = NW, out->mode = mode;
     out->n_items = (int64_t)raw.size();
     out->n_part_slots = (int64_t)raw.size();
     if (out->split_map) std::copy(S.begin(), S.end(), out->split_map);

@@ -15,6 +15,7 @@ from paper_2606_06302_b200 import inputs as I
 pytestmark = pytest.mark.gpu
 
 MAX_ABS, REL_L2, LSE_TOL = 2e-2, 5e-3, 1e-3
+DYN_PERMILLE, DYN_ROUNDS = T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS     # bench.py's launch configuration
 
 
 def setup(wl, flags=0, identity=False):
@@ -48,11 +49,13 @@ def run_modes(wl, B, kv, t, q, pool, Ws, modes=(T.MODE_BALANCED, T.MODE_SPLITMAP
     ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
     for W in Ws:
         for mode in modes:
-            pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, c0, mode)
-            dp = T.tangram_upload(t, pl)
-            out, lse = T.tangram_decode_attention(dp, q, pool)
-            torch.cuda.synchronize()
-            check(out, lse, ref_out, ref_lse, f"{wl.name} W={W} mode={T.MODE_NAMES[mode]}")
+            for dyn, J in (((0, 0), (300, 3)) if mode == T.MODE_BALANCED else ((0, 0),)):
+                pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, c0, mode, 0, dyn, J)
+                dp = T.tangram_upload(t, pl)
+                for rep in range(2 if J else 1):      # twice: the dynamic-tail counters re-arm themselves
+                    out, lse = T.tangram_decode_attention(dp, q, pool)
+                    torch.cuda.synchronize()
+                    check(out, lse, ref_out, ref_lse, f"{wl.name} W={W} mode={T.MODE_NAMES[mode]} dyn={dyn}/{J}")
     return ref_out, ref_lse
 
 
@@ -147,7 +150,7 @@ def test_page_permutation_invariance_and_determinism():
             pool = torch.randn_like(base_pool.float()).bfloat16()
             pool[torch.as_tensor(t.tbl_pages, dtype=torch.long, device="cuda")] = \
                 base_pool[torch.as_tensor(t0.tbl_pages, dtype=torch.long, device="cuda")]
-        pl = T.tangram_plan_partitions(t, B, kv, 24, wl.granule, 1, T.MODE_BALANCED)
+        pl = T.tangram_plan_partitions(t, B, kv, 24, wl.granule, 1, T.MODE_BALANCED, 0, 250, 2)
         dp = T.tangram_upload(t, pl)
         o1, l1 = T.tangram_decode_attention(dp, q, pool)
         o2, l2 = T.tangram_decode_attention(dp, q, pool)
@@ -162,7 +165,7 @@ def test_cuda_graph_capture_and_worker_timestamps():
     B, res, kv, t, n_pool = setup(wl)
     q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
     W = n_cta(wl)
-    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, 250, 3)
     dp = T.tangram_upload(t, pl)
     out, lse = T.tangram_decode_attention(dp, q, pool)
     ws = torch.empty(T.tangram_workspace_bytes(pl.n_part_slots, wl.G, wl.d), dtype=torch.uint8, device="cuda")
@@ -178,7 +181,7 @@ def test_cuda_graph_capture_and_worker_timestamps():
     g.replay()
     torch.cuda.synchronize()
     assert torch.equal(out, out_g) and torch.equal(lse, lse_g)
-    ns = torch.zeros(W, 2, dtype=torch.int64, device="cuda")
+    ns = torch.zeros(pl.n_static, 2, dtype=torch.int64, device="cuda")
     out_t, _ = T.tangram_decode_attention(dp, q, pool, worker_ns=ns)
     torch.cuda.synchronize()
     assert torch.equal(out, out_t)
@@ -210,7 +213,7 @@ def test_full_size_sampled(name):
     B, res, kv, t, n_pool = setup(wl)
     q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
     W = n_cta(wl)
-    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
     dp = T.tangram_upload(t, pl)
     out, lse = T.tangram_decode_attention(dp, q, pool)
     torch.cuda.synchronize()

@@ -44,7 +44,8 @@ def both_sides(wl, n_pool_pages=None, flags=0, identity=False):
 
 
 def plans_equal(po, pp):
-    assert (po.W, po.mode, po.n_items, po.n_part_slots) == (pp.W, pp.mode, pp.n_items, pp.n_part_slots)
+    assert (po.W, po.n_static, po.mode, po.n_items, po.n_part_slots) == \
+        (pp.W, pp.n_static, pp.mode, pp.n_items, pp.n_part_slots)
     assert np.array_equal(po.split_map, pp.split_map)
     assert po.items.shape == pp.items.shape and np.array_equal(po.items, pp.items)
     assert np.array_equal(po.worker_indptr, pp.worker_indptr)
@@ -60,6 +61,11 @@ def test_full_configs_bit_exact(name):
             po = O.plan_partitions(to, B, kv, W, wl.granule, c0, mode)
             pp = T.tangram_plan_partitions(tp, B, kv, W, wl.granule, c0, mode)
             plans_equal(po, pp)
+    for dyn, J in ((250, 4), (100, 1), (999, 16)):
+        po = O.plan_partitions(to, B, kv, 148, wl.granule, 1, O.MODE_BALANCED, 0, dyn, J)
+        pp = T.tangram_plan_partitions(tp, B, kv, 148, wl.granule, 1, T.MODE_BALANCED, 0, dyn, J)
+        plans_equal(po, pp)
+        assert pp.W == 148 * (1 + J) and pp.n_static == 148
 
 
 def test_fill_group_and_identity_free_list():
@@ -73,13 +79,15 @@ def test_fill_group_and_identity_free_list():
 @settings(max_examples=60, deadline=None)
 @given(seed=st.integers(0, 10**6), R=st.integers(1, 5), Hp=st.integers(1, 4), C=st.integers(1, 4),
        W=st.integers(1, 40), c0=st.integers(0, 3), gmul=st.integers(1, 4), mode=st.integers(0, 2),
-       splits=st.integers(0, 5))
-def test_random_shapes_bit_exact(seed, R, Hp, C, W, c0, gmul, mode, splits):
+       splits=st.integers(0, 5), dyn=st.integers(0, 999), J=st.integers(0, 6))
+def test_random_shapes_bit_exact(seed, R, Hp, C, W, c0, gmul, mode, splits, dyn, J):
+    if dyn == 0 or J == 0:
+        dyn = J = 0
     wl = I.make_random_workload(seed, R=R, H=Hp * C, G=1, d=64, C=C, max_ctx=700)
     B, kv, to, tp = both_sides(wl)
     g = wl.P * gmul
-    po = O.plan_partitions(to, B, kv, W, g, c0, mode, splits)
-    pp = T.tangram_plan_partitions(tp, B, kv, W, g, c0, mode, splits)
+    po = O.plan_partitions(to, B, kv, W, g, c0, mode, splits, dyn, J)
+    pp = T.tangram_plan_partitions(tp, B, kv, W, g, c0, mode, splits, dyn, J)
     plans_equal(po, pp)
 
 
@@ -121,6 +129,10 @@ def test_error_contract():
         T.tangram_plan_partitions(t, B, kv + 1000, 4, 64, 0, T.MODE_BALANCED)   # kv_len beyond the table
     with pytest.raises(T.TangramError):
         T.tangram_plan_partitions(t, B, kv, 4, 64, 0, 7)
+    for dyn, J in ((250, 0), (0, 2), (1000, 2), (100, 17)):
+        with pytest.raises(T.TangramError) as e:
+            T.tangram_plan_partitions(t, B, kv, 4, 64, 0, T.MODE_BALANCED, 0, dyn, J)
+        assert e.value.code == T.ERR_INVALID_ARG
 
 
 def test_skew_balance_numbers():

@@ -199,6 +199,45 @@ def test_balanced_golden(case):
     assert got == case["workers"]
 
 
+@pytest.mark.parametrize("case", GOLD["balanced_dynamic"])
+def test_balanced_dynamic_tail_golden(case):
+    assert O.list_weights(case["W"], case["dyn_permille"], case["dyn_rounds"]) == case["weights"]
+    if "lists" not in case:
+        return
+    t, B = _one_request_tables(case["kv_len"])
+    pl = O.plan_partitions(t, B, [case["kv_len"]], case["W"], case["g"], case["c0"], O.MODE_BALANCED, 0,
+                           case["dyn_permille"], case["dyn_rounds"])
+    assert pl.n_static == case["W"] and pl.W == len(case["weights"])
+    got = [[[int(it[1]), int(it[4]), int(it[5])] for it in pl.items[pl.worker_indptr[w]:pl.worker_indptr[w + 1]]]
+           for w in range(pl.W)]
+    assert got == case["lists"]
+    check_plan_valid(pl, t, np.array([case["kv_len"]]), case["g"])
+
+
+def test_dynamic_tail_shares_and_validity():
+    wl = I.make_workload("8b", R=6, ctx_div=4)
+    B, res, kv = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    t, _ = O.build_ragged_tables(B, res, wl.C, wl.P, np.arange(200000, dtype=np.int32))
+    W = 16
+    pl = O.plan_partitions(t, B, kv, W, 64, 1, O.MODE_BALANCED, 0, 200, 3)
+    check_plan_valid(pl, t, kv, 64)
+    assert pl.W == W * 4 and pl.n_static == W
+    tok = np.array([sum(int(it[5] - it[4]) for it in pl.items[pl.worker_indptr[w]:pl.worker_indptr[w + 1]])
+                    for w in range(pl.W)], dtype=float)
+    tot = tok.sum()
+    share = [tok[r * W:(r + 1) * W].sum() / tot for r in range(4)]
+    assert np.allclose(share, [0.8, 0.1, 0.05, 0.05], atol=0.01)
+    # no tail requested => identical to the static plan; tail args are ignored by the other modes
+    p0 = O.plan_partitions(t, B, kv, W, 64, 1, O.MODE_BALANCED)
+    assert p0.W == p0.n_static == W
+    for mode in (O.MODE_SPLITMAP, O.MODE_STATIC_EVEN):
+        a = O.plan_partitions(t, B, kv, W, 64, 1, mode)
+        b = O.plan_partitions(t, B, kv, W, 64, 1, mode, 0, 200, 3)
+        assert a.items.tobytes() == b.items.tobytes() and b.W == W
+    with pytest.raises(ValueError):
+        O.plan_partitions(t, B, kv, W, 64, 1, O.MODE_BALANCED, 0, 200, 0)
+
+
 def check_plan_valid(pl, t, kv_len, g):
     """Every token of every (r, h) is covered exactly once; slots and counts are consistent."""
     kv_len = np.asarray(kv_len)
