@@ -167,8 +167,10 @@ size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan* p);
 typedef struct tangram_device_plan {
     int32_t R, H, C, Hp, P, W /* work lists */, mode, n_static /* launch grid */;
     int64_t n_items, n_part_slots;
-    int64_t n_merge_seqs;       /* sequences whose part count is not 1 (they need the merge kernel) */
-    const int32_t* merge_seqs;  /* device [n_merge_seqs]: r * H + h */
+    int64_t n_merge_seqs;       /* sequences whose part count is not 1 */
+    int64_t n_empty_seqs;       /* of these, the first n_empty_seqs have no part at all (kv_len 0) */
+    const int32_t* merge_seqs;  /* device [n_merge_seqs][4]: {r * H + h, first part slot, parts, 0}, empty
+                                   sequences first */
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
     const int64_t* worker_indptr; /* device [W+1] */
     const int64_t* part_indptr;   /* device [R*H+1] */

@@ -71,8 +71,9 @@ struct Smem {
     __host__ __device__ static int off_scratch(int ns, int G) { return off_desc(ns, G) + kQSlots * 32; }
     __host__ __device__ static int off_ml(int ns, int G) { return off_scratch(ns, G) + kNW * G * kRowF * 4; }
     __host__ __device__ static int off_bar(int ns, int G) { return (off_ml(ns, G) + kNW * G * 8 + 15) & ~15; }
+    __host__ __device__ static int off_flag(int ns, int G) { return off_bar(ns, G) + (2 * kNW * kMaxStages + 2 * kQSlots) * 8; }
     __host__ __device__ static int total(int ns, int G) {
-        return off_bar(ns, G) + (2 * kNW * kMaxStages + 2 * kQSlots) * 8 + 1024 /* base alignment slack */;
+        return off_flag(ns, G) + 16 + 1024 /* base alignment slack */;
     }
     static int max_stages(int G) {
         int ns = kMaxStages;
@@ -139,6 +140,7 @@ __device__ __forceinline__ void mma_rows07(float& c0, float& c1, uint32_t a0, ui
     asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%10,%10};"
         : "+f"(c0), "+f"(c1), "=f"(d2), "=f"(d3)
         : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1), "f"(0.f));
+    (void)d2, (void)d3;
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     uint32_t r;
@@ -424,84 +426,82 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
 }
 
 // ------------------------------------------------------------------ a5: LSE merge kernel
-// One CTA of 8 warps per (sequence that needs a merge, query head of its group).  `merge_seqs` lists
-// the sequences (r * H + h) whose part count is not 1 (built at upload time): sequences with one
-// part were written by the decode kernel; sequences with no retained token get out = 0, lse = -inf.
-// Warp w accumulates parts w, w + 8, ... (four loads in flight per lane), then the eight warp sums are
-// combined in a fixed order, so the result is deterministic.
-constexpr int kMergeWarps = 8;
+// One CTA of 512 threads per sequence that needs a merge.  `merge_seqs` lists the sequences
+// (r * H + h) whose part count is not 1 (built at upload time, empty sequences first): sequences with
+// one part were written by the decode kernel; sequences with no retained token get out = 0,
+// lse = -inf.  A thread owns four adjacent output elements (one float4 of a partial row; a warp reads
+// 512 contiguous bytes) of query head g and, if G * D / 4 < 512, one of PG part groups (parts
+// k, k + PG, ...), eight loads in flight; the PG group sums are then combined in group order.  The
+// summation order is a function of (n, G, D) only, so the result is deterministic.
+constexpr int kMergeThreads = 512;
 template <int D>
-__global__ void __launch_bounds__(kMergeWarps * 32)
-tangram_merge_kernel(const int32_t* __restrict__ merge_seqs, const int64_t* __restrict__ part_indptr,
-                     const float* __restrict__ part_o, const float* __restrict__ part_lse,
-                     __nv_bfloat16* __restrict__ out, float* __restrict__ lse, int H, int G) {
-    constexpr int V = D / 32;  // floats per lane
-    using VecT = typename std::conditional<V == 4, float4, float2>::type;
-    __shared__ float s_red[kMergeWarps];
-    __shared__ float s_acc[kMergeWarps][D + 1];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int seq = merge_seqs[blockIdx.x / G], gi = blockIdx.x % G;
-    const int r = seq / H, h = seq % H;
-    const int64_t p0 = part_indptr[seq];
-    const int n = static_cast<int>(part_indptr[seq + 1] - p0);
-    const size_t row = (static_cast<size_t>(r) * H + h) * G + gi;  // = r * Hq + h * G + gi
+__global__ void __launch_bounds__(kMergeThreads)
+tangram_merge_kernel(const int32_t* __restrict__ merge_recs, const float* __restrict__ part_o,
+                     const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
+                     float* __restrict__ lse, int G) {
+    __shared__ float s_part[kMergeThreads][6];
+    const int4 rec = reinterpret_cast<const int4*>(merge_recs)[blockIdx.x];  // {seq, first part slot, parts, -}
+    const int seq = rec.x, n = rec.z;
+    const int64_t p0 = rec.y;
+    const size_t row0 = static_cast<size_t>(seq) * G;  // (r * H + h) * G = r * Hq + h * G
+    const int n_elem = G * (D / 4);                     // float4 elements of the G output rows
     // everything above reads plan data only; the partials / outputs need the decode grid to be done
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (n == 0) {
-        if (threadIdx.x < D / 2)
-            reinterpret_cast<__nv_bfloat162*>(out + row * D)[threadIdx.x] = __floats2bfloat162_rn(0.f, 0.f);
-        if (threadIdx.x == 0) lse[row] = -INFINITY;
+        if (threadIdx.x < n_elem) reinterpret_cast<uint2*>(out + row0 * D)[threadIdx.x] = make_uint2(0u, 0u);
+        if (threadIdx.x < G) lse[row0 + threadIdx.x] = -INFINITY;
         return;
     }
-    float M = -INFINITY;
-    for (int i = threadIdx.x; i < n; i += kMergeWarps * 32) M = fmaxf(M, part_lse[(p0 + i) * G + gi]);
+    const int PG = kMergeThreads / n_elem;  // part groups (>= 1 since G * D / 4 <= 256)
+    const int e4 = threadIdx.x % n_elem, grp = threadIdx.x / n_elem;
+    const int g = e4 / (D / 4), c4 = e4 % (D / 4);
+    // online (running-max) accumulation: one pass, no separate max pass, any number of parts
+    float m = -INFINITY, tot = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    if (grp < PG) {
+        const float* pl = part_lse + p0 * G + g;  // [part][g]
+        const float* po = part_o + (p0 * G + g) * D + c4 * 4;
+        const size_t stride = static_cast<size_t>(G) * D;
+        for (int i = grp; i < n; i += 8 * PG) {
+            float4 v[8];
+            float w[8];
 #pragma unroll
-    for (int s = 16; s > 0; s >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, s));
-    if (lane == 0) s_red[warp] = M;
-    __syncthreads();
+            for (int u = 0; u < 8; ++u) {
+                const int ii = i + u * PG;
+                const int ic = ii < n ? ii : i;
+                v[u] = *reinterpret_cast<const float4*>(po + ic * stride);
+                w[u] = ii < n ? pl[ic * G] : -INFINITY;
+            }
+            float m_new = m;
 #pragma unroll
-    for (int w = 0; w < kMergeWarps; ++w) M = fmaxf(M, s_red[w]);
-    __syncthreads();
-
-    float acc[V], tot = 0.f;
+            for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
+            const float resc = __expf(m - m_new);  // m = -inf on the first batch -> 0; m_new is finite (part i exists)
+            tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
+            m = m_new;
 #pragma unroll
-    for (int e = 0; e < V; ++e) acc[e] = 0.f;
-    const size_t stride = static_cast<size_t>(G) * D;
-    const float* src = part_o + (p0 * G + gi) * D + lane * V;
-    for (int i = warp; i < n; i += 4 * kMergeWarps) {
-        VecT v[4];
-        float w[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int ii = i + u * kMergeWarps;
-            const bool ok = ii < n;
-            v[u] = *reinterpret_cast<const VecT*>(src + (ok ? ii : i) * stride);
-            w[u] = ok ? __expf(part_lse[(p0 + ii) * G + gi] - M) : 0.f;
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            tot += w[u];
-            if constexpr (V == 4) {
-                acc[0] += w[u] * v[u].x, acc[1] += w[u] * v[u].y, acc[2] += w[u] * v[u].z, acc[3] += w[u] * v[u].w;
-            } else {
-                acc[0] += w[u] * v[u].x, acc[1] += w[u] * v[u].y;
+            for (int u = 0; u < 8; ++u) {
+                const float e = __expf(w[u] - m);  // -inf -> 0
+                tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
             }
         }
+        float* sp = s_part[threadIdx.x];
+        sp[0] = m, sp[1] = tot, sp[2] = a0, sp[3] = a1, sp[4] = a2, sp[5] = a3;
     }
-#pragma unroll
-    for (int e = 0; e < V; ++e) s_acc[warp][lane * V + e] = acc[e];
-    if (lane == 0) s_red[warp] = tot;
     __syncthreads();
-    if (threadIdx.x < D / 2) {
-        float t = 0.f, x = 0.f, y = 0.f;
-#pragma unroll
-        for (int w = 0; w < kMergeWarps; ++w) {
-            t += s_red[w];
-            x += s_acc[w][2 * threadIdx.x], y += s_acc[w][2 * threadIdx.x + 1];
+    if (grp == 0) {
+        float M = m;
+        for (int k = 1; k < PG; ++k) M = fmaxf(M, s_part[k * n_elem + e4][0]);
+        float sc = __expf(m - M);
+        tot *= sc, a0 *= sc, a1 *= sc, a2 *= sc, a3 *= sc;
+        for (int k = 1; k < PG; ++k) {
+            const float* sp = s_part[k * n_elem + e4];
+            sc = __expf(sp[0] - M);  // a group without parts has m = -inf -> 0
+            tot += sc * sp[1], a0 += sc * sp[2], a1 += sc * sp[3], a2 += sc * sp[4], a3 += sc * sp[5];
         }
-        const float inv = 1.f / t;
-        reinterpret_cast<__nv_bfloat162*>(out + row * D)[threadIdx.x] = __floats2bfloat162_rn(x * inv, y * inv);
-        if (threadIdx.x == 0) lse[row] = M + __logf(t);
+        const float inv = 1.f / tot;
+        const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
+        reinterpret_cast<uint2*>(out + (row0 + g) * D)[c4] =
+            make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
+        if (c4 == 0) lse[row0 + g] = M + __logf(tot);
     }
 }
 
@@ -567,15 +567,14 @@ static int launch_decode(const tangram_device_plan* dp, const DecodeParams& prm,
     // Programmatic dependent launch: the merge grid is scheduled while the decode grid drains and
     // blocks in griddepcontrol.wait until the decode grid has completed and flushed its writes.
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)(dp->n_merge_seqs * prm.G)), cfg.blockDim = dim3(kMergeWarps * 32), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
+    cfg.gridDim = dim3((unsigned)dp->n_merge_seqs), cfg.blockDim = dim3(kMergeThreads), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr, cfg.numAttrs = 1;
     const float* po = prm.part_o;
     const float* pl = prm.part_lse;
-    e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, dp->part_indptr, po, pl, prm.out, prm.lse,
-                           (int)dp->H, (int)prm.G);
+    e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, po, pl, prm.out, prm.lse, (int)prm.G);
     if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
@@ -617,7 +616,7 @@ extern "C" size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan
     b += align_up(sizeof(int64_t) * ((size_t)p->W + 1), 256);
     b += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
     b += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
-    b += align_up(sizeof(int32_t) * (size_t)t->R * t->H, 256);  // merge_seqs (upper bound)
+    b += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);  // merge records (upper bound)
     return b + 256 /* scheduler counters */ + 256;
 }
 
@@ -653,9 +652,18 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     const size_t off_mseq = off;
     int32_t* mseq = reinterpret_cast<int32_t*>(host.data() + off);
     int64_t n_mseq = 0;
-    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)
-        if (p->part_indptr[sq + 1] - p->part_indptr[sq] != 1) mseq[n_mseq++] = (int32_t)sq;
-    off += align_up(sizeof(int32_t) * (size_t)t->R * t->H, 256);
+    int64_t n_empty = 0;
+    auto push = [&](int64_t sq) {  // record = {sequence, first part slot, parts, 0}
+        int32_t* rec = mseq + 4 * n_mseq++;
+        rec[0] = (int32_t)sq, rec[1] = (int32_t)p->part_indptr[sq];
+        rec[2] = (int32_t)(p->part_indptr[sq + 1] - p->part_indptr[sq]), rec[3] = 0;
+    };
+    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // empty sequences first ...
+        if (p->part_indptr[sq + 1] - p->part_indptr[sq] == 0) push(sq);
+    n_empty = n_mseq;
+    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // ... then the multi-part ones
+        if (p->part_indptr[sq + 1] - p->part_indptr[sq] > 1) push(sq);
+    off += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);
     const size_t off_sched = off;
     // pageable source: the runtime stages it before returning, so `host` may die at scope exit
     cudaError_t e = cudaMemcpyAsync(dev_blob, host.data(), need, cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream));
@@ -668,6 +676,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->sched = reinterpret_cast<int32_t*>(base + off_sched);
     dp->merge_seqs = reinterpret_cast<const int32_t*>(base + off_mseq);
     dp->n_merge_seqs = n_mseq;
+    dp->n_empty_seqs = n_empty;
     dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
     dp->items = base + off_items;
     dp->worker_indptr = reinterpret_cast<const int64_t*>(base + off_windptr);
@@ -720,6 +729,7 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.Hq = Hq, prm.G = G, prm.Hp = dp->Hp;
     prm.n_lists = dp->W;
     prm.sched = dp->sched;
+
     prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);
     if (const char* dbg = getenv("TANGRAM_DEBUG_STAGES")) prm.n_stages = std::min(prm.n_stages, atoi(dbg));
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));

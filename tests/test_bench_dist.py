@@ -1,0 +1,49 @@
+"""The N>1 plumbing of bench.py (barrier, max-over-ranks of the device time, sum of the processed
+bytes) on CPU with the gloo backend, world_size 2.  The hot path itself has no collective: ranks are
+independent replicas."""
+import os
+import socket
+import sys
+
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      LOCAL_RANK=str(rank))
+    import bench
+    assert bench.dist_env() == (rank, rank, world)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dist.barrier()
+    ms, units = bench.aggregate(1.0 + rank, 100.0 * (rank + 1), world, device="cpu")
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, ms, units))
+
+
+def test_aggregate_world_size_2():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    # every rank sees max time (2.0 ms) and the summed units (300): value = units / time is whole-job
+    assert res == [(0, 2.0, 300.0), (1, 2.0, 300.0)]
+
+
+def test_aggregate_single_rank_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.aggregate(3.5, 7.0, 1) == (3.5, 7.0)

@@ -125,6 +125,29 @@ def test_slack_poisoned_with_nan():
     run_modes(wl, B, kv, t, q, pool, Ws=(9, n_cta(wl)), modes=(T.MODE_BALANCED, T.MODE_STATIC_EVEN))
 
 
+def test_split_then_merge_entry_points():
+    """tangram_decode_partials + tangram_merge_partials (the two kernels on their own) give the same
+    result, within tolerance, as tangram_decode_attention (which launches both)."""
+    wl = I.make_workload("skew", R=2, ctx_div=8)
+    wl.demand[1, 3] = 0                                   # an empty sequence for the merge kernel's zero path
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    for dyn, J in ((0, 0), (400, 3)):
+        pl = T.tangram_plan_partitions(t, B, kv, 21, wl.granule, 1, T.MODE_BALANCED, 0, dyn, J)
+        dp = T.tangram_upload(t, pl)
+        ws = torch.zeros(T.tangram_workspace_bytes(pl.n_part_slots, wl.G, wl.d), dtype=torch.uint8, device="cuda")
+        out = torch.full_like(q, float("nan"))
+        lse = torch.full((wl.R, wl.Hq), float("nan"), device="cuda")
+        T.tangram_decode_partials(dp, q, pool, out, lse, ws)
+        T.tangram_merge_partials(dp, out, lse, ws)
+        torch.cuda.synchronize()
+        check(out, lse, ref_out, ref_lse, f"split+merge dyn={dyn}")
+        out2, lse2 = T.tangram_decode_attention(dp, q, pool)
+        torch.cuda.synchronize()
+        check(out2, lse2, ref_out, ref_lse, f"decode_attention dyn={dyn}")
+
+
 def test_fill_group_policy():
     wl = I.make_workload("8b", R=2, ctx_div=16)
     B, res, kv, t, n_pool = setup(wl, flags=T.FILL_GROUP, identity=True)
