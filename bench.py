@@ -315,7 +315,7 @@ def spread_of(T, S, torch, reps=5):
     """Per-CTA elapsed-time spread (max - min) / mean of the worker CTAs' busy time, from the
     globaltimer stamps of the instrumented build (median over reps)."""
     W = S["plan"].n_static
-    ns = torch.zeros(W, 2, dtype=torch.int64, device=S["q"].device)
+    ns = torch.zeros(W, 4, dtype=torch.int64, device=S["q"].device)
     dp = S["dp"]
     vals = []
     for _ in range(reps):

@@ -169,14 +169,17 @@ typedef struct tangram_device_plan {
     int64_t n_items, n_part_slots;
     int64_t n_merge_seqs;       /* sequences whose part count is not 1 */
     int64_t n_empty_seqs;       /* of these, the first n_empty_seqs have no part at all (kv_len 0) */
+    int64_t n_big_merge_seqs;   /* ... and the last n_big_merge_seqs have more than 32 parts */
     const int32_t* merge_seqs;  /* device [n_merge_seqs][4]: {r * H + h, first part slot, parts, 0}, empty
-                                   sequences first */
+                                   sequences first, then by part count <= 32 / > 32 */
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
     const int64_t* worker_indptr; /* device [W+1] */
+    const void* list_heads;       /* device [W] 128-byte list heads: item range, first item, its first 16 page ids */
     const int64_t* part_indptr;   /* device [R*H+1] */
     const int32_t* tbl_pages;     /* device page ids */
-    int32_t* sched;               /* device [2]: list-claim counter and CTAs-done counter of the dynamic
-                                     tail; zero between launches (the kernel re-arms them itself) */
+    int32_t* sched;               /* device [4]: list-claim / CTAs-done counters of the dynamic tail and the
+                                     grid-barrier counters of the in-kernel merge; zero between launches
+                                     (the kernel re-arms them itself) */
 } tangram_device_plan;
 
 /* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte
@@ -200,8 +203,10 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *   out       device [R][Hq][d] bf16;  lse device [R][Hq] f32 (natural log of sum exp(scaled score);
  *             -inf and out = 0 for a head with kv_len 0)
  *   workspace device, >= tangram_workspace_bytes(dp->n_part_slots, G, d), 16-byte aligned
- *   worker_ns device [W][2] u64 or NULL: if given, every worker CTA stores its globaltimer start /
- *             end (the per-CTA elapsed-time spread of BASELINE.json is measured from these).
+ *   worker_ns device [n_static][4] u64 or NULL: if given, every CTA stores its globaltimer stamps
+ *             {start, end of its work lists, grid barrier passed, merges done} (the last two only when
+ *             the merge runs inside the decode grid); the per-CTA elapsed-time spread of BASELINE.json
+ *             is measured from the first two.
  * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
  * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G), BUFFER_TOO_SMALL (workspace), CUDA. */

@@ -21,7 +21,7 @@ OK, ERR_INVALID_ARG, ERR_OUT_OF_PAGES, ERR_BUFFER_TOO_SMALL, ERR_CUDA = 0, -1, -
 FILL_GROUP = 1
 MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
 # dynamic tail of the BALANCED plan used by bench.py / smoke (tuned on B200)
-DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 750, 4
+DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 900, 7
 MODE_NAMES = {MODE_BALANCED: "balanced", MODE_SPLITMAP: "splitmap", MODE_STATIC_EVEN: "static_even"}
 
 if not os.path.exists(LIB_PATH):
@@ -53,9 +53,9 @@ class _Plan(C.Structure):
 class _DevicePlan(C.Structure):
     _fields_ = [("R", C.c_int32), ("H", C.c_int32), ("C", C.c_int32), ("Hp", C.c_int32), ("P", C.c_int32),
                 ("W", C.c_int32), ("mode", C.c_int32), ("n_static", C.c_int32), ("n_items", C.c_int64),
-                ("n_part_slots", C.c_int64), ("n_merge_seqs", C.c_int64), ("n_empty_seqs", C.c_int64),
+                ("n_part_slots", C.c_int64), ("n_merge_seqs", C.c_int64), ("n_empty_seqs", C.c_int64), ("n_big_merge_seqs", C.c_int64),
                 ("merge_seqs", C.c_void_p),
-                ("items", C.c_void_p), ("worker_indptr", C.c_void_p),
+                ("items", C.c_void_p), ("worker_indptr", C.c_void_p), ("list_heads", C.c_void_p),
                 ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p)]
 
 

@@ -54,8 +54,12 @@ struct DecodeParams {
     float* part_o;
     float* part_lse;
     unsigned long long* worker_ns;
-    int* sched;  // [0] next list to claim (relative to gridDim.x), [1] CTAs done; both 0 between launches
+    int* sched;  // [0] next list to claim (relative to gridDim.x), [1] CTAs done claiming, [2] grid-barrier
+                 // arrivals, [3] CTAs done merging; all 0 between launches (the kernel re-arms them)
+    const int32_t* merge_recs;  // merge records (see a5)
+    const void* list_heads;     // [n_lists] 128-byte list heads
     int32_t Hq, G, Hp, n_stages, n_lists;
+    int32_t tail_merge, n_merge_units, n_merge_small;
     float scale_log2;
 };
 
@@ -69,7 +73,11 @@ struct Smem {
     __host__ __device__ static int off_q(int ns) { return kNW * ns * kTile; }
     __host__ __device__ static int off_desc(int ns, int G) { return off_q(ns) + kQSlots * q_slot(G); }
     __host__ __device__ static int off_scratch(int ns, int G) { return off_desc(ns, G) + kQSlots * 32; }
-    __host__ __device__ static int off_ml(int ns, int G) { return off_scratch(ns, G) + kNW * G * kRowF * 4; }
+    // merge scratch: 8 warp states of G padded rows; also reused by the tail merge (256 threads x 6 floats)
+    __host__ __device__ static int scratch_bytes(int G) {
+        return kNW * G * kRowF * 4 > kNW * 32 * 6 * 4 ? kNW * G * kRowF * 4 : kNW * 32 * 6 * 4;
+    }
+    __host__ __device__ static int off_ml(int ns, int G) { return off_scratch(ns, G) + scratch_bytes(G); }
     __host__ __device__ static int off_bar(int ns, int G) { return (off_ml(ns, G) + kNW * G * 8 + 15) & ~15; }
     __host__ __device__ static int off_flag(int ns, int G) { return off_bar(ns, G) + (2 * kNW * kMaxStages + 2 * kQSlots) * 8; }
     __host__ __device__ static int total(int ns, int G) {
@@ -156,6 +164,113 @@ __device__ __forceinline__ unsigned long long globaltimer() {
     return t;
 }
 
+// ------------------------------------------------------------------ a5: LSE merge
+// The merge records list the sequences (r * H + h) whose part count is not 1 (built at upload time:
+// empty sequences first, then sequences with at most kMergeBigParts parts, then the "big" ones).
+// Sequences with one part were written by the decode kernel; sequences with no retained token get
+// out = 0, lse = -inf.  A merge UNIT is a whole small record (all G query heads) or one query head of a
+// big record; unit u of a launch is decoded by unit_of().  Within a unit a thread owns four adjacent
+// output elements (one float4 of a partial row, so a row is read by D/4 adjacent threads) and one of
+// PG part groups (parts k, k + PG, ...) with eight loads in flight and running-max accumulation (one
+// pass); the group sums are then combined in group order.  The summation order is a function of
+// (n, G, D, thread count) only, so the result is deterministic.
+constexpr int kMergeThreads = 512;
+constexpr int kMergeBigParts = 32;
+
+struct MergeUnit {
+    int seq, p0, n, g;  // g < 0: all query heads of the group
+};
+__device__ __forceinline__ MergeUnit unit_of(const int32_t* __restrict__ recs, int n_small, int u, int G) {
+    const int r = u < n_small ? u : n_small + (u - n_small) / G;
+    const int4 rec = reinterpret_cast<const int4*>(recs)[r];  // {seq, first part slot, parts, -}
+    return MergeUnit{rec.x, rec.y, rec.z, u < n_small ? -1 : (u - n_small) % G};
+}
+
+template <int D, int NT, bool NAMED_BAR>
+__device__ __forceinline__ void merge_unit(const MergeUnit mu, int G, const float* __restrict__ part_o,
+                                           const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
+                                           float* __restrict__ lse, float (*s_part)[6], int tid) {
+    auto sync = [] {
+        if constexpr (NAMED_BAR) named_bar_sync(1, NT);
+        else __syncthreads();
+    };
+    const int rows = mu.g < 0 ? G : 1;
+    const int n_elem = rows * (D / 4);  // float4 elements of the unit's output rows (<= 256)
+    const size_t row0 = static_cast<size_t>(mu.seq) * G + (mu.g < 0 ? 0 : mu.g);  // (r*H + h)*G + g = r*Hq + h*G + g
+    const int n = mu.n;
+    if (n == 0) {
+        if (tid < n_elem) reinterpret_cast<uint2*>(out + row0 * D)[tid] = make_uint2(0u, 0u);
+        if (tid < rows) lse[row0 + tid] = -INFINITY;
+        return;
+    }
+    const int PG = NT / n_elem;  // part groups
+    const int e4 = tid % n_elem, grp = tid / n_elem;
+    const int gl = e4 / (D / 4), c4 = e4 % (D / 4);  // row inside the unit, float4 column
+    const int g = mu.g < 0 ? gl : mu.g;
+    float m = -INFINITY, tot = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    if (grp < PG) {
+        const float* pl = part_lse + static_cast<size_t>(mu.p0) * G + g;  // [part][g]
+        const float* po = part_o + (static_cast<size_t>(mu.p0) * G + g) * D + c4 * 4;
+        const size_t stride = static_cast<size_t>(G) * D;
+        for (int i = grp; i < n; i += 8 * PG) {
+            float4 v[8];
+            float w[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int ii = i + u * PG;
+                const int ic = ii < n ? ii : i;
+                v[u] = __ldcg(reinterpret_cast<const float4*>(po + ic * stride));
+                w[u] = ii < n ? __ldcg(pl + ic * G) : -INFINITY;
+            }
+            float m_new = m;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
+            const float resc = __expf(m - m_new);  // m = -inf on the first batch -> 0; m_new is finite (part i exists)
+            tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
+            m = m_new;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float e = __expf(w[u] - m);  // -inf -> 0
+                tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
+            }
+        }
+        float* sp = s_part[tid];
+        sp[0] = m, sp[1] = tot, sp[2] = a0, sp[3] = a1, sp[4] = a2, sp[5] = a3;
+    }
+    sync();
+    if (grp == 0) {
+        float M = m;
+        for (int k = 1; k < PG; ++k) M = fmaxf(M, s_part[k * n_elem + e4][0]);
+        float sc = __expf(m - M);
+        tot *= sc, a0 *= sc, a1 *= sc, a2 *= sc, a3 *= sc;
+        for (int k = 1; k < PG; ++k) {
+            const float* sp = s_part[k * n_elem + e4];
+            sc = __expf(sp[0] - M);  // a group without parts has m = -inf -> 0
+            tot += sc * sp[1], a0 += sc * sp[2], a1 += sc * sp[3], a2 += sc * sp[4], a3 += sc * sp[5];
+        }
+        const float inv = 1.f / tot;
+        const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
+        reinterpret_cast<uint2*>(out + (row0 + gl) * D)[c4] =
+            make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
+        if (c4 == 0) lse[row0 + gl] = M + __logf(tot);
+    }
+    sync();  // s_part may be reused by the next unit
+}
+
+// Stand-alone merge kernel (tangram_merge_partials, and the fallback of tangram_decode_attention when
+// the grid cannot be launched cooperatively): one CTA per unit.
+template <int D>
+__global__ void __launch_bounds__(kMergeThreads)
+tangram_merge_kernel(const int32_t* __restrict__ merge_recs, int n_small, const float* __restrict__ part_o,
+                     const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
+                     float* __restrict__ lse, int G) {
+    __shared__ float s_part[kMergeThreads][6];
+    const MergeUnit mu = unit_of(merge_recs, n_small, blockIdx.x, G);
+    // everything above reads plan data only; the partials / outputs need the decode grid to be done
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    merge_unit<D, kMergeThreads, false>(mu, G, part_o, part_lse, out, lse, s_part, threadIdx.x);
+}
+
 // ------------------------------------------------------------------ a4: split-KV decode kernel
 template <int D, bool TIMED>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -180,7 +295,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     auto qfull_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + s) * 8; };
     auto qempty_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + kQSlots + s) * 8; };
 
-    if (TIMED && threadIdx.x == 0) p.worker_ns[2 * blockIdx.x] = globaltimer();
+    if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x] = globaltimer();
     if (threadIdx.x == 0) {
         for (int w = 0; w < kNW; ++w)
             for (int s = 0; s < NS; ++s) {
@@ -202,29 +317,44 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
         uint32_t stage = 0, phase = 0;  // lane w < 8 tracks consumer warp w's ring
         // Work lists: list blockIdx.x is this CTA's own; with a dynamic tail (n_lists > gridDim.x) further
-        // lists are claimed from a global counter, two lists ahead so that neither the atomic nor the
-        // dependent loads (list range -> first item -> page ids) ever stall the TMA issue.
+        // lists are claimed from a global counter.  The claim is issued as late as possible -- when the
+        // producer starts the LAST item of the current list -- so that a CTA never sits on a list another
+        // CTA could already run; its latency is covered by that item's TMA issue, and the consumers still
+        // hold a full ring (192 KB) of tiles while the next list's range and first item are fetched.
         const bool dynamic = p.n_lists > static_cast<int>(gridDim.x);
         auto claim = [&]() {
             int v = 0;
             if (lane == 0) v = atomicAdd(p.sched, 1) + static_cast<int>(gridDim.x);
             return v;
         };
-        int nxt = p.n_lists;
-        if (dynamic) nxt = __shfl_sync(0xffffffffu, claim(), 0);
-        int64_t cb = p.worker_indptr[blockIdx.x], ce = p.worker_indptr[blockIdx.x + 1];
-        int64_t nb = 0, ne = 0;
-        if (nxt < p.n_lists) nb = p.worker_indptr[nxt], ne = p.worker_indptr[nxt + 1];
+        // One 128-byte list head (a single coalesced load, lane L reads word L) carries the list's item
+        // range, its first item and that item's first 16 page ids, so the first TMA of a list is two
+        // dependent memory round trips away from the claim instead of four.
+        int64_t cb, ce;
         DeviceItem next;
-        if (cb < ce) next = p.items[cb];
+        int head_pid_lo = 0, head_pid_hi = 0;  // page ids of tiles (lane - rot) & 7 and that + 8 of the list's first item
+        auto load_head = [&](int list) {
+            const int w = __ldg(reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(list) * 32 + lane);
+            cb = __shfl_sync(0xffffffffu, w, 0);
+            ce = cb + __shfl_sync(0xffffffffu, w, 1);
+            next.req = __shfl_sync(0xffffffffu, w, 4), next.kv_head = __shfl_sync(0xffffffffu, w, 5);
+            next.tbl_row = __shfl_sync(0xffffffffu, w, 6), next.slot = __shfl_sync(0xffffffffu, w, 7);
+            next.tok_begin = __shfl_sync(0xffffffffu, w, 8), next.tok_end = __shfl_sync(0xffffffffu, w, 9);
+            next.part_slot = __shfl_sync(0xffffffffu, w, 10), next.n_parts = __shfl_sync(0xffffffffu, w, 11);
+            const int i0 = (lane - (next.part_slot & (kNW - 1))) & (kNW - 1);
+            head_pid_lo = __shfl_sync(0xffffffffu, w, 12 + i0);
+            head_pid_hi = __shfl_sync(0xffffffffu, w, 20 + i0);
+        };
+        load_head(blockIdx.x);
         int seq = 0;  // running item number = position in the item / query ring
         for (;;) {
-            int fut = p.n_lists;
-            if (dynamic && nxt < p.n_lists) fut = claim();  // consumed when this list is done
+            int fut = 0;
+            if (dynamic && cb == ce) fut = claim();
             for (int64_t it = cb; it < ce; ++it, ++seq) {
                 const DeviceItem item = next;
+                const bool head_item = it == cb;
                 if (it + 1 < ce) next = p.items[it + 1];
-                else if (nb < ne) next = p.items[nb];
+                else if (dynamic) fut = claim();
                 const int qs = seq % kQSlots;
                 const uint32_t qpar = (seq / kQSlots) & 1;
                 if (lane == 0) {
@@ -241,10 +371,11 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 if (lane < kNW) {
                     const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
                     int i = (lane - rot) & (kNW - 1);
-                    int pid = i < n_tiles ? __ldg(ids + i) : 0;
+                    int pid = head_item ? head_pid_lo : (i < n_tiles ? __ldg(ids + i) : 0);
                     while (i < n_tiles) {
                         const int i_next = i + kNW;
-                        const int pid_next = i_next < n_tiles ? __ldg(ids + i_next) : 0;
+                        const int pid_next =
+                            head_item && i_next < 2 * kNW ? head_pid_hi : (i_next < n_tiles ? __ldg(ids + i_next) : 0);
                         mbar_wait(empty_bar(lane, stage), phase ^ 1);
                         mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
                         tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
@@ -255,12 +386,10 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 }
                 __syncwarp();
             }
-            if (cb == ce && nb < ne) next = p.items[nb];
+            if (!dynamic) break;
+            const int nxt = __shfl_sync(0xffffffffu, fut, 0);
             if (nxt >= p.n_lists) break;
-            cb = nb, ce = ne;
-            nxt = dynamic ? __shfl_sync(0xffffffffu, fut, 0) : p.n_lists;
-            nb = ne = 0;
-            if (nxt < p.n_lists) nb = p.worker_indptr[nxt], ne = p.worker_indptr[nxt + 1];
+            load_head(nxt);
         }
         if (lane == 0) {
             // end-of-work sentinel for the consumers
@@ -422,86 +551,32 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         }
         named_bar_sync(1, kNW * 32);  // scratch may be overwritten by the next item
     }
-    if (TIMED && threadIdx.x == 0) p.worker_ns[2 * blockIdx.x + 1] = globaltimer();
-}
+    if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 1] = globaltimer();
 
-// ------------------------------------------------------------------ a5: LSE merge kernel
-// One CTA of 512 threads per sequence that needs a merge.  `merge_seqs` lists the sequences
-// (r * H + h) whose part count is not 1 (built at upload time, empty sequences first): sequences with
-// one part were written by the decode kernel; sequences with no retained token get out = 0,
-// lse = -inf.  A thread owns four adjacent output elements (one float4 of a partial row; a warp reads
-// 512 contiguous bytes) of query head g and, if G * D / 4 < 512, one of PG part groups (parts
-// k, k + PG, ...), eight loads in flight; the PG group sums are then combined in group order.  The
-// summation order is a function of (n, G, D) only, so the result is deterministic.
-constexpr int kMergeThreads = 512;
-template <int D>
-__global__ void __launch_bounds__(kMergeThreads)
-tangram_merge_kernel(const int32_t* __restrict__ merge_recs, const float* __restrict__ part_o,
-                     const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
-                     float* __restrict__ lse, int G) {
-    __shared__ float s_part[kMergeThreads][6];
-    const int4 rec = reinterpret_cast<const int4*>(merge_recs)[blockIdx.x];  // {seq, first part slot, parts, -}
-    const int seq = rec.x, n = rec.z;
-    const int64_t p0 = rec.y;
-    const size_t row0 = static_cast<size_t>(seq) * G;  // (r * H + h) * G = r * Hq + h * G
-    const int n_elem = G * (D / 4);                     // float4 elements of the G output rows
-    // everything above reads plan data only; the partials / outputs need the decode grid to be done
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (n == 0) {
-        if (threadIdx.x < n_elem) reinterpret_cast<uint2*>(out + row0 * D)[threadIdx.x] = make_uint2(0u, 0u);
-        if (threadIdx.x < G) lse[row0 + threadIdx.x] = -INFINITY;
-        return;
-    }
-    const int PG = kMergeThreads / n_elem;  // part groups (>= 1 since G * D / 4 <= 256)
-    const int e4 = threadIdx.x % n_elem, grp = threadIdx.x / n_elem;
-    const int g = e4 / (D / 4), c4 = e4 % (D / 4);
-    // online (running-max) accumulation: one pass, no separate max pass, any number of parts
-    float m = -INFINITY, tot = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-    if (grp < PG) {
-        const float* pl = part_lse + p0 * G + g;  // [part][g]
-        const float* po = part_o + (p0 * G + g) * D + c4 * 4;
-        const size_t stride = static_cast<size_t>(G) * D;
-        for (int i = grp; i < n; i += 8 * PG) {
-            float4 v[8];
-            float w[8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int ii = i + u * PG;
-                const int ic = ii < n ? ii : i;
-                v[u] = *reinterpret_cast<const float4*>(po + ic * stride);
-                w[u] = ii < n ? pl[ic * G] : -INFINITY;
-            }
-            float m_new = m;
-#pragma unroll
-            for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
-            const float resc = __expf(m - m_new);  // m = -inf on the first batch -> 0; m_new is finite (part i exists)
-            tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
-            m = m_new;
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const float e = __expf(w[u] - m);  // -inf -> 0
-                tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
-            }
+    if (p.tail_merge) {
+        // a5 inside the persistent grid (cooperative launch: all CTAs are co-resident).  Grid barrier over
+        // the consumer threads, then CTA b merges units b, b + gridDim.x, ... -- no second launch, and the
+        // merges of many sequences run on all SMs at once.
+        __threadfence();
+        named_bar_sync(1, kNW * 32);
+        if (threadIdx.x == 0) {
+            atomicAdd(p.sched + 2, 1);
+            int seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
+                if (seen < static_cast<int>(gridDim.x)) __nanosleep(64);
+            } while (seen < static_cast<int>(gridDim.x));
+            __threadfence();
         }
-        float* sp = s_part[threadIdx.x];
-        sp[0] = m, sp[1] = tot, sp[2] = a0, sp[3] = a1, sp[4] = a2, sp[5] = a3;
-    }
-    __syncthreads();
-    if (grp == 0) {
-        float M = m;
-        for (int k = 1; k < PG; ++k) M = fmaxf(M, s_part[k * n_elem + e4][0]);
-        float sc = __expf(m - M);
-        tot *= sc, a0 *= sc, a1 *= sc, a2 *= sc, a3 *= sc;
-        for (int k = 1; k < PG; ++k) {
-            const float* sp = s_part[k * n_elem + e4];
-            sc = __expf(sp[0] - M);  // a group without parts has m = -inf -> 0
-            tot += sc * sp[1], a0 += sc * sp[2], a1 += sc * sp[3], a2 += sc * sp[4], a3 += sc * sp[5];
-        }
-        const float inv = 1.f / tot;
-        const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
-        reinterpret_cast<uint2*>(out + (row0 + g) * D)[c4] =
-            make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
-        if (c4 == 0) lse[row0 + g] = M + __logf(tot);
+        named_bar_sync(1, kNW * 32);
+        if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
+        float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
+        for (int u = blockIdx.x; u < p.n_merge_units; u += gridDim.x)
+            merge_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, u, G), G, p.part_o, p.part_lse, p.out,
+                                          p.lse, s_part, threadIdx.x);
+        if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
+        if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == static_cast<int>(gridDim.x) - 1)
+            p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
     }
 }
 
@@ -544,39 +619,67 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
     return TANGRAM_OK;
 }
 
-template <int D>
-static int launch_decode(const tangram_device_plan* dp, const DecodeParams& prm, const CUtensorMap& map,
-                         cudaStream_t stream, int which) {
+// CTAs of the decode kernel that can be co-resident on the current device (SMs x occupancy).
+template <int D, bool TIMED>
+static int max_coresident(int smem) {
+    int dev = 0, sms = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED>, kThreads, smem) !=
+        cudaSuccess)
+        return 0;
+    return sms * per_sm;
+}
+
+template <int D, bool TIMED>
+static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map, cudaStream_t stream,
+                        bool want_tail_merge, bool* merged) {
     using L = Smem<D>;
     const int smem = L::total(prm.n_stages, prm.G);
-    cudaError_t e;
-    if (!(which & kRunSplit)) {
-    } else if (prm.worker_ns) {
-        e = cudaFuncSetAttribute(tangram_decode_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
-        tangram_decode_kernel<D, true><<<dp->n_static, kThreads, smem, stream>>>(map, prm);
-    } else {
-        e = cudaFuncSetAttribute(tangram_decode_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
-        tangram_decode_kernel<D, false><<<dp->n_static, kThreads, smem, stream>>>(map, prm);
-    }
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
-    if (!(which & kRunMerge)) return TANGRAM_OK;
-    if (dp->n_merge_seqs == 0) return TANGRAM_OK;
-    // Programmatic dependent launch: the merge grid is scheduled while the decode grid drains and
-    // blocks in griddepcontrol.wait until the decode grid has completed and flushed its writes.
+    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, TIMED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    // The tail merge needs a grid barrier, i.e. a cooperative launch with every CTA resident.
+    static thread_local int cached_smem = -1, cached_max = 0;
+    if (want_tail_merge && cached_smem != smem) cached_max = max_coresident<D, TIMED>(smem), cached_smem = smem;
+    prm.tail_merge = want_tail_merge && dp->n_static <= cached_max;
+    *merged = prm.tail_merge;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)dp->n_merge_seqs), cfg.blockDim = dim3(kMergeThreads), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
+    cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
+    cfg.attrs = attr, cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+    if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
+    return TANGRAM_OK;
+}
+
+template <int D>
+static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map,
+                         cudaStream_t stream, int which) {
+    const int n_small = (int)(dp->n_merge_seqs - dp->n_big_merge_seqs);
+    const int n_units = n_small + (int)dp->n_big_merge_seqs * prm.G;
+    prm.merge_recs = dp->merge_seqs, prm.n_merge_small = n_small, prm.n_merge_units = n_units;
+    bool merged = false;
+    if (which & kRunSplit) {
+        const bool want = (which & kRunMerge) && n_units > 0;
+        const int rc = prm.worker_ns ? launch_split<D, true>(dp, prm, map, stream, want, &merged)
+                                     : launch_split<D, false>(dp, prm, map, stream, want, &merged);
+        if (rc != TANGRAM_OK) return rc;
+    }
+    if (!(which & kRunMerge) || merged || n_units == 0) return TANGRAM_OK;
+    // Stand-alone merge kernel by programmatic dependent launch: its grid is scheduled while the decode
+    // grid drains and blocks in griddepcontrol.wait until that grid has completed and flushed its writes.
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)n_units), cfg.blockDim = dim3(kMergeThreads), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr, cfg.numAttrs = 1;
     const float* po = prm.part_o;
     const float* pl = prm.part_lse;
-    e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, po, pl, prm.out, prm.lse, (int)prm.G);
-    if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
-    e = cudaGetLastError();
+    cudaError_t e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, n_small, po, pl, prm.out, prm.lse,
+                                       (int)prm.G);
     if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
     return TANGRAM_OK;
 }
@@ -617,6 +720,7 @@ extern "C" size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan
     b += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
     b += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
     b += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);  // merge records (upper bound)
+    b += align_up(128 * (size_t)p->W, 256);                          // list heads
     return b + 256 /* scheduler counters */ + 256;
 }
 
@@ -625,6 +729,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     if (!t || !p || !dev_blob || !dp || !p->items || !p->worker_indptr || !p->part_indptr || !t->tbl_pages ||
         !t->tbl_indptr)
         return fail(TANGRAM_ERR_INVALID_ARG, "upload: NULL argument");
+    if (p->n_items > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: more than 2^31 items");
     const size_t need = tangram_blob_bytes(t, p);
     if (bytes < need) return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "upload: blob %zu < %zu bytes", bytes, need);
     if (reinterpret_cast<uintptr_t>(dev_blob) % 256 != 0)
@@ -661,9 +766,30 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // empty sequences first ...
         if (p->part_indptr[sq + 1] - p->part_indptr[sq] == 0) push(sq);
     n_empty = n_mseq;
-    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // ... then the multi-part ones
-        if (p->part_indptr[sq + 1] - p->part_indptr[sq] > 1) push(sq);
+    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq) {  // ... then the small multi-part ones
+        const int64_t np = p->part_indptr[sq + 1] - p->part_indptr[sq];
+        if (np > 1 && np <= kMergeBigParts) push(sq);
+    }
+    const int64_t n_not_big = n_mseq;
+    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // ... then the big ones (one merge unit per query head)
+        if (p->part_indptr[sq + 1] - p->part_indptr[sq] > kMergeBigParts) push(sq);
     off += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);
+    const size_t off_heads = off;
+    {   // list head = {item_begin, n_items, 0, 0, first item (8 words), its first 16 page ids, 0 x 4}
+        int32_t* hd = reinterpret_cast<int32_t*>(host.data() + off);
+        for (int32_t k = 0; k < p->W; ++k, hd += 32) {
+            const int64_t ib = p->worker_indptr[k], ie = p->worker_indptr[k + 1];
+            hd[0] = (int32_t)ib, hd[1] = (int32_t)(ie - ib);
+            if (ie > ib) {
+                std::memcpy(hd + 4, &di[ib], sizeof(DeviceItem));
+                const DeviceItem& f = di[ib];
+                const int64_t first_pg = (int64_t)f.tbl_row + f.tok_begin / kPage;
+                const int64_t n_tiles = (f.tok_end - f.tok_begin + kPage - 1) / kPage;
+                for (int64_t i = 0; i < 16 && i < n_tiles; ++i) hd[12 + i] = t->tbl_pages[first_pg + i];
+            }
+        }
+    }
+    off += align_up(128 * (size_t)p->W, 256);
     const size_t off_sched = off;
     // pageable source: the runtime stages it before returning, so `host` may die at scope exit
     cudaError_t e = cudaMemcpyAsync(dev_blob, host.data(), need, cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream));
@@ -677,6 +803,8 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->merge_seqs = reinterpret_cast<const int32_t*>(base + off_mseq);
     dp->n_merge_seqs = n_mseq;
     dp->n_empty_seqs = n_empty;
+    dp->list_heads = base + off_heads;
+    dp->n_big_merge_seqs = n_mseq - n_not_big;
     dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
     dp->items = base + off_items;
     dp->worker_indptr = reinterpret_cast<const int64_t*>(base + off_windptr);
@@ -726,8 +854,10 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.part_lse = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) +
                                             align_up((size_t)dp->n_part_slots * G * d * 4, 256));
     prm.worker_ns = reinterpret_cast<unsigned long long*>(worker_ns);
+    prm.tail_merge = 0, prm.merge_recs = nullptr, prm.n_merge_units = 0, prm.n_merge_small = 0;
     prm.Hq = Hq, prm.G = G, prm.Hp = dp->Hp;
     prm.n_lists = dp->W;
+    prm.list_heads = dp->list_heads;
     prm.sched = dp->sched;
 
     prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);

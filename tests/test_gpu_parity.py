@@ -204,7 +204,7 @@ def test_cuda_graph_capture_and_worker_timestamps():
     g.replay()
     torch.cuda.synchronize()
     assert torch.equal(out, out_g) and torch.equal(lse, lse_g)
-    ns = torch.zeros(pl.n_static, 2, dtype=torch.int64, device="cuda")
+    ns = torch.zeros(pl.n_static, 4, dtype=torch.int64, device="cuda")
     out_t, _ = T.tangram_decode_attention(dp, q, pool, worker_ns=ns)
     torch.cuda.synchronize()
     assert torch.equal(out, out_t)
