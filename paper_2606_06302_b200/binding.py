@@ -21,7 +21,7 @@ OK, ERR_INVALID_ARG, ERR_OUT_OF_PAGES, ERR_BUFFER_TOO_SMALL, ERR_CUDA = 0, -1, -
 FILL_GROUP = 1
 MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
 # dynamic tail of the BALANCED plan used by bench.py / smoke (tuned on B200)
-DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 900, 7
+DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 500, 6
 MODE_NAMES = {MODE_BALANCED: "balanced", MODE_SPLITMAP: "splitmap", MODE_STATIC_EVEN: "static_even"}
 
 if not os.path.exists(LIB_PATH):

@@ -43,6 +43,10 @@ constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime
 constexpr int kMaxG = 8;
 constexpr int kSmemLimit = 232448; // 227 KB opt-in limit per CTA
 constexpr int kRunSplit = 1, kRunMerge = 2;
+#ifndef TANGRAM_CLAIM_TILES
+#define TANGRAM_CLAIM_TILES 16
+#endif
+constexpr int kClaimTiles = TANGRAM_CLAIM_TILES;  // how many tiles before the end of a list its successor is claimed
 
 struct DecodeParams {
     const DeviceItem* items;
@@ -257,6 +261,52 @@ __device__ __forceinline__ void merge_unit(const MergeUnit mu, int G, const floa
     sync();  // s_part may be reused by the next unit
 }
 
+// A small record (at most kMergeBigParts parts) merged by G * D/4 threads, one float4 element each, every
+// part visited in order: no shared memory, no barrier, so the sub-groups of a CTA merge different
+// records at the same time.
+template <int D>
+__device__ __forceinline__ void merge_small(const int4 rec, int G, const float* __restrict__ part_o,
+                                            const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
+                                            float* __restrict__ lse, int e4) {
+    const int n = rec.z, g = e4 / (D / 4), c4 = e4 % (D / 4);
+    const size_t row = static_cast<size_t>(rec.x) * G + g;
+    if (n == 0) {
+        reinterpret_cast<uint2*>(out + row * D)[c4] = make_uint2(0u, 0u);
+        if (c4 == 0) lse[row] = -INFINITY;
+        return;
+    }
+    const float* pl = part_lse + static_cast<size_t>(rec.y) * G + g;
+    const float* po = part_o + (static_cast<size_t>(rec.y) * G + g) * D + c4 * 4;
+    const size_t stride = static_cast<size_t>(G) * D;
+    float m = -INFINITY, tot = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    for (int i = 0; i < n; i += 8) {
+        float4 v[8];
+        float w[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int ic = i + u < n ? i + u : i;
+            v[u] = __ldcg(reinterpret_cast<const float4*>(po + ic * stride));
+            w[u] = i + u < n ? __ldcg(pl + ic * G) : -INFINITY;
+        }
+        float m_new = m;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
+        const float resc = __expf(m - m_new);
+        tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
+        m = m_new;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const float e = __expf(w[u] - m);
+            tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
+        }
+    }
+    const float inv = 1.f / tot;
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
+    reinterpret_cast<uint2*>(out + row * D)[c4] =
+        make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
+    if (c4 == 0) lse[row] = m + __logf(tot);
+}
+
 // Stand-alone merge kernel (tangram_merge_partials, and the fallback of tangram_decode_attention when
 // the grid cannot be launched cooperatively): one CTA per unit.
 template <int D>
@@ -354,7 +404,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 const DeviceItem item = next;
                 const bool head_item = it == cb;
                 if (it + 1 < ce) next = p.items[it + 1];
-                else if (dynamic) fut = claim();
+                const bool claim_here = dynamic && it + 1 == ce;  // last item of the list: claim the next list
                 const int qs = seq % kQSlots;
                 const uint32_t qpar = (seq / kQSlots) & 1;
                 if (lane == 0) {
@@ -372,7 +422,15 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
                     int i = (lane - rot) & (kNW - 1);
                     int pid = head_item ? head_pid_lo : (i < n_tiles ? __ldg(ids + i) : 0);
+                    // lane 0 issues the claim kClaimTiles tiles before the end of the item's TMA issue: late
+                    // enough that the CTA does not hoard a list, early enough to cover the claim -> list
+                    // head -> first TMA chain (~3 us) with tiles that are still being issued
+                    bool to_claim = claim_here && lane == 0;
                     while (i < n_tiles) {
+                        if (to_claim && i + kClaimTiles >= n_tiles) {
+                            fut = atomicAdd(p.sched, 1) + static_cast<int>(gridDim.x);
+                            to_claim = false;
+                        }
                         const int i_next = i + kNW;
                         const int pid_next =
                             head_item && i_next < 2 * kNW ? head_pid_hi : (i_next < n_tiles ? __ldg(ids + i_next) : 0);
@@ -383,6 +441,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                         if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
                         i = i_next, pid = pid_next;
                     }
+                    if (to_claim) fut = atomicAdd(p.sched, 1) + static_cast<int>(gridDim.x);
                 }
                 __syncwarp();
             }
@@ -557,6 +616,17 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         // a5 inside the persistent grid (cooperative launch: all CTAs are co-resident).  Grid barrier over
         // the consumer threads, then CTA b merges units b, b + gridDim.x, ... -- no second launch, and the
         // merges of many sequences run on all SMs at once.
+        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*gridDim.x)*K + sub, no
+        // barrier inside; the first record is fetched BEFORE the grid barrier (plan data).  Big records
+        // (more than kMergeBigParts parts) go first, one query head per unit, CTAs 0 .. n_big_units-1 ...
+        const int n_elem = G * (D / 4), K = (kNW * 32) / n_elem, sub = threadIdx.x / n_elem;
+        const int n_big_units = p.n_merge_units - p.n_merge_small;
+        const int grid = static_cast<int>(gridDim.x);
+        // ... so the small records start at the CTA after the last one holding a big unit
+        const int first = (static_cast<int>(blockIdx.x) - n_big_units % grid + grid) % grid;
+        int sidx = first * K + sub;
+        int4 rec = make_int4(0, 0, 0, 0);
+        if (sub < K && sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
         __threadfence();
         named_bar_sync(1, kNW * 32);
         if (threadIdx.x == 0) {
@@ -564,16 +634,22 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             int seen;
             do {
                 asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
-                if (seen < static_cast<int>(gridDim.x)) __nanosleep(64);
-            } while (seen < static_cast<int>(gridDim.x));
+                if (seen < grid) __nanosleep(32);
+            } while (seen < grid);
             __threadfence();
         }
         named_bar_sync(1, kNW * 32);
         if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
         float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
-        for (int u = blockIdx.x; u < p.n_merge_units; u += gridDim.x)
-            merge_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, u, G), G, p.part_o, p.part_lse, p.out,
-                                          p.lse, s_part, threadIdx.x);
+        for (int u = blockIdx.x; u < n_big_units; u += grid)
+            merge_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G), G, p.part_o,
+                                          p.part_lse, p.out, p.lse, s_part, threadIdx.x);
+        if (sub < K)
+            for (; sidx < p.n_merge_small; sidx += grid * K) {
+                merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
+                if (sidx + grid * K < p.n_merge_small)
+                    rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
+            }
         if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
         if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == static_cast<int>(gridDim.x) - 1)
             p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
