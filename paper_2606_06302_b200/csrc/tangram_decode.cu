@@ -937,7 +937,6 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.sched = dp->sched;
 
     prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);
-    if (const char* dbg = getenv("TANGRAM_DEBUG_STAGES")) prm.n_stages = std::min(prm.n_stages, atoi(dbg));
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
     prm.scale_log2 = scale * 1.4426950408889634f;
     cudaStream_t st = static_cast<cudaStream_t>(stream);

@@ -10,6 +10,12 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    # The built libraries are git-ignored: (re)build them in-tree before any test imports the binding.
+    # nvcc cross-compiles sm_100a without a GPU; the oracle is plain C (gcc).
+    from paper_2606_06302_b200 import build as _build
+    _build.build(force=False)
+    from oracle import tangram_oracle as _oracle
+    _oracle.build_c()
 
 
 def pytest_collection_modifyitems(config, items):
