@@ -15,6 +15,8 @@ What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.
                           equal-bytes work list, reading A2), STATIC_EVEN (FlashDecoding-style
                           uniform num_splits, :120)
   O5 merge                log-sum-exp merge of split-KV partials (implied by split-KV :91, :120)
+  O6 append_kv            one decode step's new K/V rows written into the ragged pages (NEXT-1;
+                          page layout :190, capacity bound :176, reading A29)
   O1 attention*           plain softmax(q K~^T / sqrt(d)) V~ through the page tables (Eq. 1 :57)
 
 Pins (every function is pinned; nothing here is "parity unpinned"): tests/test_oracle_pins.py.
@@ -328,6 +330,37 @@ def merge(parts: Sequence[Tuple[np.ndarray, float]]):
     for (o, l) in live:
         out = out + math.exp(l - L) * o
     return out, L
+
+
+# --------------------------------------------------------------------------------------------
+# O6  KV append of one decode step (NEXT-1; page layout :190, capacity bound :176)
+# --------------------------------------------------------------------------------------------
+def append_kv(pool_bits: np.ndarray, t: Tables, kv_len, k_new_bits: np.ndarray, v_new_bits: np.ndarray):
+    """One decode step's new K/V row of every (request, KV head) written behind its retained tokens.
+
+    pool_bits  uint16 [n_pages][Hp][2][P][d] (raw bf16 bits; a modified COPY is returned)
+    k_new_bits, v_new_bits  uint16 [R][H][d]
+    Rule (reading A29): the row goes to token index n = kv_len[r][h] of head h, i.e. to
+    pool[tbl_pages[tbl_indptr[r*C + c] + n // P]][slot][kv][n % P]; kv_len[r][h] becomes n + 1.  The
+    reserved budget is a hard capacity bound (:176): if n already equals the capacity of the
+    (request, cluster) table (its pages x P) the row is dropped and counted as an overflow.
+    Returns (pool', kv_len', n_overflow)."""
+    pool = np.array(pool_bits, dtype=np.uint16, copy=True)
+    kv = np.array(kv_len, dtype=np.int32, copy=True)
+    over = 0
+    for r in range(t.R):
+        for h in range(t.H):
+            c, s = int(t.cluster_of[h]), int(t.slot_of[h])
+            lo, hi = int(t.tbl_indptr[r * t.C + c]), int(t.tbl_indptr[r * t.C + c + 1])
+            n = int(kv[r, h])
+            if n >= (hi - lo) * t.P:
+                over += 1
+                continue
+            page = int(t.tbl_pages[lo + n // t.P])
+            pool[page, s, 0, n % t.P, :] = k_new_bits[r, h, :]
+            pool[page, s, 1, n % t.P, :] = v_new_bits[r, h, :]
+            kv[r, h] = n + 1
+    return pool, kv, over
 
 
 # --------------------------------------------------------------------------------------------

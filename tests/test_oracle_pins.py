@@ -464,3 +464,50 @@ def test_slack_is_never_read():
     pool = scatter_dense_into_pool(K, V, lens, t, 32, fill=float("nan"))
     out, lse, _ = O.attention(q, pool, t, lens, H * G, d)
     assert np.all(np.isfinite(out)) and np.all(np.isfinite(lse))
+
+
+# ---------------------------------------------------------------------------- O6 KV append (NEXT-1)
+def test_append_kv_round_trip_against_dense_attention():
+    """Tokens appended one decode step at a time into empty sequences are found again, in order, by the
+    (already pinned) gather of O1: attention over the appended cache equals dense library attention over
+    the appended rows.  Also: bytes outside the written rows never change, kv_len counts the rows, and
+    rows beyond the table capacity are dropped and counted."""
+    R, H, G, d, P, steps = 2, 4, 2, 64, 16, 37
+    B = np.array([0.9, 0.2, 0.6, 0.3])
+    cap_tokens = np.array([[48, 16, 32, 16], [32, 16, 48, 32]], dtype=np.int32)     # reservation per head
+    free = np.random.default_rng(3).permutation(40).astype(np.int32)
+    t, _ = O.build_ragged_tables(B, cap_tokens, 2, P, free)
+    g = torch.Generator().manual_seed(21)
+    pool0 = torch.randn(40, t.Hp, 2, P, d, generator=g).bfloat16()
+    bits = pool0.view(torch.int16).numpy().view(np.uint16).copy()
+    kv = np.zeros((R, H), dtype=np.int32)
+    Ks = torch.randn(steps, R, H, d, generator=g).bfloat16()
+    Vs = torch.randn(steps, R, H, d, generator=g).bfloat16()
+    total_over = 0
+    for sidx in range(steps):
+        kb = Ks[sidx].view(torch.int16).numpy().view(np.uint16)
+        vb = Vs[sidx].view(torch.int16).numpy().view(np.uint16)
+        new_bits, new_kv, over = O.append_kv(bits, t, kv, kb, vb)
+        assert np.array_equal(new_kv - kv, (new_kv > kv).astype(np.int32)) and over == int((new_kv == kv).sum())
+        assert (new_bits != bits).sum() <= int((new_kv > kv).sum()) * 2 * d        # only the written rows change
+        bits, kv, total_over = new_bits, new_kv, total_over + over
+    # capacity of head h = pages of its cluster x P (cluster = pair of heads sorted by B: (1,3) and (2,0))
+    cap = np.zeros((R, H), dtype=np.int32)
+    for r in range(R):
+        for h in range(H):
+            c = t.cluster_of[h]
+            cap[r, h] = (t.tbl_indptr[r * 2 + c + 1] - t.tbl_indptr[r * 2 + c]) * P
+    assert np.array_equal(kv, np.minimum(steps, cap)) and total_over == int((steps - kv).sum())
+    assert cap[0].tolist() == [48, 16, 48, 16]                                      # cluster max, page-rounded
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    pool = torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16)
+    out, lse, _ = O.attention(q, pool, t, kv, H * G, d)
+    for r in range(R):
+        for j in range(H * G):
+            h = j // G
+            n = int(kv[r, h])
+            Kd, Vd = Ks[:n, r, h].double(), Vs[:n, r, h].double()
+            sc = (Kd @ q[r, j].double()) / math.sqrt(d)
+            ref = torch.softmax(sc, 0) @ Vd
+            assert np.allclose(out[r, j], ref.numpy(), rtol=0, atol=1e-12)
+            assert abs(lse[r, j] - float(torch.logsumexp(sc, 0))) < 1e-12
