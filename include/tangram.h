@@ -175,6 +175,7 @@ typedef struct tangram_device_plan {
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
     const int64_t* worker_indptr; /* device [W+1] */
     const void* list_heads;       /* device [W] 128-byte list heads: item range, first item, its first 16 page ids */
+    const int32_t* seq_info;      /* device [R*H][4]: {page-table row offset, capacity in tokens, slot, 0} */
     const int64_t* part_indptr;   /* device [R*H+1] */
     const int32_t* tbl_pages;     /* device page ids */
     int32_t* sched;               /* device [4]: list-claim / CTAs-done counters of the dynamic tail and the
@@ -197,6 +198,11 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *   dp        from tangram_upload (host struct holding device pointers)
  *   q         device [R][Hq][d] bf16, 16-byte aligned
  *   kv_pool   device [n_pool_pages][Hp][2][P][d] bf16, 128-byte aligned (Ragged page, :190)
+ *   kv_len_dev device [R][H] i32 or NULL.  NULL: the items are executed exactly as planned.  Otherwise the
+ *             plan is OPEN-ENDED: every item covers tokens [tok_begin, min(tok_end, kv_len_dev[r][h])), so a
+ *             plan built once for lengths >= the run-time ones (e.g. the tables' capacity) serves every
+ *             decode step while tangram_append_kv grows the cache; items beyond the current length are
+ *             empty and a head with length 0 yields out = 0, lse = -inf.
  *   Hq        query heads, Hq % H == 0, G = Hq / H <= 8 (query head j uses KV head floor(j / G))
  *   d         64 or 128;  P must be 16
  *   sm_scale  softmax scale; 0 means 1/sqrt(d)
@@ -211,7 +217,8 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
  * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G), BUFFER_TOO_SMALL (workspace), CUDA. */
 int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
-                             int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                             int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d,
+                             float sm_scale, void* out,
                              float* lse, void* workspace, size_t workspace_bytes,
                              uint64_t* worker_ns, void* stream);
 
@@ -222,11 +229,28 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
  * same stream is exactly tangram_decode_attention; they exist so that each kernel can be timed and
  * profiled on its own. */
 int tangram_decode_partials(const tangram_device_plan* dp, const void* q, const void* kv_pool,
-                            int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                            int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d,
+                            float sm_scale, void* out,
                             float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
                             void* stream);
 int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d, void* out, float* lse,
                            void* workspace, size_t workspace_bytes, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-1  KV append of one decode step.  The new K row and V row of every (request,
+ * KV head) are written behind its retained tokens in the ragged pages (:190 page layout), and its length
+ * grows by one.  The reserved budget is a hard capacity bound (:176): a head whose (request, cluster)
+ * table is full (pages x P tokens) keeps its length, its row is dropped and counted.
+ *
+ *   dp            from tangram_upload (uses the tables only)
+ *   k_new, v_new  device [R][H][d] bf16, 16-byte aligned
+ *   kv_pool       device [n_pool_pages][Hp][2][P][d] bf16 (written)
+ *   kv_len_dev    device [R][H] i32, read and incremented
+ *   overflow_dev  device i32 or NULL: incremented once per dropped row
+ * Asynchronous on `stream`; graph capturable.  Errors: INVALID_ARG, CUDA. */
+int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const void* v_new, void* kv_pool,
+                      int64_t n_pool_pages, int32_t d, int32_t* kv_len_dev, int32_t* overflow_dev,
+                      void* stream);
 
 #ifdef __cplusplus
 }

@@ -56,7 +56,7 @@ class _DevicePlan(C.Structure):
                 ("n_part_slots", C.c_int64), ("n_merge_seqs", C.c_int64), ("n_empty_seqs", C.c_int64), ("n_big_merge_seqs", C.c_int64),
                 ("merge_seqs", C.c_void_p),
                 ("items", C.c_void_p), ("worker_indptr", C.c_void_p), ("list_heads", C.c_void_p),
-                ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p)]
+                ("seq_info", C.c_void_p), ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p)]
 
 
 _lib.tangram_last_error.restype = C.c_char_p
@@ -65,12 +65,12 @@ _lib.tangram_workspace_bytes.restype = C.c_size_t
 _lib.tangram_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
 for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
-              "tangram_merge_partials"):
+              "tangram_merge_partials", "tangram_append_kv"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
-           "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials")
+           "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv")
 
 
 def _check(rc: int):
@@ -227,7 +227,7 @@ def tangram_upload(t: Tables, p: Plan, device="cuda", stream=None) -> DevicePlan
 
 
 def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, workspace=None, sm_scale: float = 0.0,
-                             worker_ns=None, stream=None, _entry="tangram_decode_attention"):
+                             worker_ns=None, stream=None, kv_len=None, _entry="tangram_decode_attention"):
     """q [R,Hq,d] bf16 cuda, kv_pool [n_pages,Hp,2,P,d] bf16 cuda -> (out [R,Hq,d] bf16, lse [R,Hq] f32).
     Asynchronous on the current (or given) torch stream."""
     import torch
@@ -246,17 +246,20 @@ def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, wor
         workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     wn = C.c_void_p(worker_ns.data_ptr()) if worker_ns is not None else None
+    if kv_len is not None:
+        assert kv_len.is_cuda and kv_len.dtype == torch.int32 and kv_len.is_contiguous() and kv_len.numel() == R * dp.c.H
+    kvl = C.c_void_p(kv_len.data_ptr()) if kv_len is not None else None
     _check(getattr(_lib, _entry)(C.byref(dp.c), C.c_void_p(q.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
-                                         C.c_int64(n_pages), C.c_int32(Hq), C.c_int32(d), C.c_float(sm_scale),
+                                         C.c_int64(n_pages), kvl, C.c_int32(Hq), C.c_int32(d), C.c_float(sm_scale),
                                          C.c_void_p(out.data_ptr()), C.c_void_p(lse.data_ptr()),
                                          C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), wn, sp))
     return out, lse
 
 
 def tangram_decode_partials(dp: DevicePlan, q, kv_pool, out=None, lse=None, workspace=None, sm_scale: float = 0.0,
-                            worker_ns=None, stream=None):
+                            worker_ns=None, stream=None, kv_len=None):
     """a4 alone: the split-KV decode kernel (see include/tangram.h)."""
-    return tangram_decode_attention(dp, q, kv_pool, out, lse, workspace, sm_scale, worker_ns, stream,
+    return tangram_decode_attention(dp, q, kv_pool, out, lse, workspace, sm_scale, worker_ns, stream, kv_len,
                                     _entry="tangram_decode_partials")
 
 
@@ -269,3 +272,20 @@ def tangram_merge_partials(dp: DevicePlan, out, lse, workspace, stream=None):
                                        C.c_void_p(lse.data_ptr()), C.c_void_p(workspace.data_ptr()),
                                        C.c_size_t(workspace.numel()), sp))
     return out, lse
+
+
+def tangram_append_kv(dp: DevicePlan, k_new, v_new, kv_pool, kv_len, overflow=None, stream=None):
+    """NEXT-1: append one decode step's K/V rows ([R,H,d] bf16 each) into the ragged pages; kv_len
+    ([R,H] int32, cuda) is incremented in place; `overflow` (int32[1], cuda) counts dropped rows."""
+    import torch
+    R, H, d = k_new.shape
+    assert k_new.is_cuda and v_new.is_cuda and kv_pool.is_cuda and kv_len.is_cuda
+    assert k_new.dtype == torch.bfloat16 and v_new.dtype == torch.bfloat16 and kv_len.dtype == torch.int32
+    assert k_new.is_contiguous() and v_new.is_contiguous() and kv_len.is_contiguous()
+    assert (R, H) == (dp.c.R, dp.c.H) and tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d)
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    ov = C.c_void_p(overflow.data_ptr()) if overflow is not None else None
+    _check(_lib.tangram_append_kv(C.byref(dp.c), C.c_void_p(k_new.data_ptr()), C.c_void_p(v_new.data_ptr()),
+                                  C.c_void_p(kv_pool.data_ptr()), C.c_int64(kv_pool.shape[0]), C.c_int32(d),
+                                  C.c_void_p(kv_len.data_ptr()), ov, sp))
+    return kv_len

@@ -62,6 +62,8 @@ struct DecodeParams {
                  // arrivals, [3] CTAs done merging; all 0 between launches (the kernel re-arms them)
     const int32_t* merge_recs;  // merge records (see a5)
     const void* list_heads;     // [n_lists] 128-byte list heads
+    const int32_t* kv_len;      // [R*H] run-time lengths (open-ended plan) or nullptr: items are taken as planned
+    int32_t H;
     int32_t Hq, G, Hp, n_stages, n_lists;
     int32_t tail_merge, n_merge_units, n_merge_small;
     float scale_log2;
@@ -229,12 +231,12 @@ __device__ __forceinline__ void merge_unit(const MergeUnit mu, int G, const floa
             float m_new = m;
 #pragma unroll
             for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
-            const float resc = __expf(m - m_new);  // m = -inf on the first batch -> 0; m_new is finite (part i exists)
+            const float resc = m_new == -INFINITY ? 1.f : __expf(m - m_new);  // m = -inf on the first batch -> 0
             tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
             m = m_new;
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
-                const float e = __expf(w[u] - m);  // -inf -> 0
+                const float e = m == -INFINITY ? 0.f : __expf(w[u] - m);  // -inf -> 0; all parts empty so far -> 0
                 tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
             }
         }
@@ -245,18 +247,18 @@ __device__ __forceinline__ void merge_unit(const MergeUnit mu, int G, const floa
     if (grp == 0) {
         float M = m;
         for (int k = 1; k < PG; ++k) M = fmaxf(M, s_part[k * n_elem + e4][0]);
-        float sc = __expf(m - M);
+        float sc = M == -INFINITY ? 0.f : __expf(m - M);
         tot *= sc, a0 *= sc, a1 *= sc, a2 *= sc, a3 *= sc;
         for (int k = 1; k < PG; ++k) {
             const float* sp = s_part[k * n_elem + e4];
-            sc = __expf(sp[0] - M);  // a group without parts has m = -inf -> 0
+            sc = M == -INFINITY ? 0.f : __expf(sp[0] - M);  // a group without parts has m = -inf -> 0
             tot += sc * sp[1], a0 += sc * sp[2], a1 += sc * sp[3], a2 += sc * sp[4], a3 += sc * sp[5];
         }
-        const float inv = 1.f / tot;
+        const float inv = tot > 0.f ? 1.f / tot : 0.f;
         const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
         reinterpret_cast<uint2*>(out + (row0 + gl) * D)[c4] =
             make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
-        if (c4 == 0) lse[row0 + gl] = M + __logf(tot);
+        if (c4 == 0) lse[row0 + gl] = tot > 0.f ? M + __logf(tot) : -INFINITY;
     }
     sync();  // s_part may be reused by the next unit
 }
@@ -291,20 +293,20 @@ __device__ __forceinline__ void merge_small(const int4 rec, int G, const float* 
         float m_new = m;
 #pragma unroll
         for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
-        const float resc = __expf(m - m_new);
+        const float resc = m_new == -INFINITY ? 1.f : __expf(m - m_new);
         tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
         m = m_new;
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const float e = __expf(w[u] - m);
+            const float e = m == -INFINITY ? 0.f : __expf(w[u] - m);  // parts of an open-ended plan may be empty
             tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
         }
     }
-    const float inv = 1.f / tot;
+    const float inv = tot > 0.f ? 1.f / tot : 0.f;
     const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
     reinterpret_cast<uint2*>(out + row * D)[c4] =
         make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
-    if (c4 == 0) lse[row] = m + __logf(tot);
+    if (c4 == 0) lse[row] = tot > 0.f ? m + __logf(tot) : -INFINITY;
 }
 
 // Stand-alone merge kernel (tangram_merge_partials, and the fallback of tangram_decode_attention when
@@ -391,6 +393,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             next.tbl_row = __shfl_sync(0xffffffffu, w, 6), next.slot = __shfl_sync(0xffffffffu, w, 7);
             next.tok_begin = __shfl_sync(0xffffffffu, w, 8), next.tok_end = __shfl_sync(0xffffffffu, w, 9);
             next.part_slot = __shfl_sync(0xffffffffu, w, 10), next.n_parts = __shfl_sync(0xffffffffu, w, 11);
+            if (p.kv_len) next.tok_end = min(next.tok_end, __ldg(p.kv_len + next.req * p.H + next.kv_head));
             const int i0 = (lane - (next.part_slot & (kNW - 1))) & (kNW - 1);
             head_pid_lo = __shfl_sync(0xffffffffu, w, 12 + i0);
             head_pid_hi = __shfl_sync(0xffffffffu, w, 20 + i0);
@@ -403,7 +406,11 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             for (int64_t it = cb; it < ce; ++it, ++seq) {
                 const DeviceItem item = next;
                 const bool head_item = it == cb;
-                if (it + 1 < ce) next = p.items[it + 1];
+                if (it + 1 < ce) {
+                    next = p.items[it + 1];
+                    // open-ended plan: the item ends where the sequence ends NOW (it may be empty)
+                    if (p.kv_len) next.tok_end = min(next.tok_end, __ldg(p.kv_len + next.req * p.H + next.kv_head));
+                }
                 const bool claim_here = dynamic && it + 1 == ce;  // last item of the list: claim the next list
                 const int qs = seq % kQSlots;
                 const uint32_t qpar = (seq / kQSlots) & 1;
@@ -416,7 +423,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                               p.q + (static_cast<size_t>(item.req) * p.Hq + static_cast<size_t>(item.kv_head) * G) * D,
                               qbytes, qfull_bar(qs));
                 }
-                const int n_tiles = (item.tok_end - item.tok_begin + kPage - 1) / kPage;
+                const int n_tiles = max(0, item.tok_end - item.tok_begin + kPage - 1) / kPage;
                 const int rot = item.part_slot & (kNW - 1);  // which warp gets the item's first tile
                 if (lane < kNW) {
                     const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
@@ -490,7 +497,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         __syncwarp();
         if (lane == 0) mbar_arrive(qempty_bar(qs));
 
-        const int n_tok = item.tok_end - item.tok_begin;
+        const int n_tok = max(0, item.tok_end - item.tok_begin);  // 0: an open-ended item beyond the current length
         const int n_tiles = (n_tok + kPage - 1) / kPage;
         const int rot = item.part_slot & (kNW - 1);  // a function of the item only: results do not depend on which CTA runs it
         float m = kNegInf, l = 0.f;
@@ -588,16 +595,17 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 mw[w] = scratch_ml[(w * G + g) * 2];
                 M = fmaxf(M, mw[w]);
             }
+            const bool none = M == kNegInf;  // no tile at all (empty open-ended item): o = 0, lse = -inf
             float Lsum = 0.f, ax = 0.f, ay = 0.f;
 #pragma unroll
             for (int w = 0; w < kNW; ++w) {
-                const float e = exp2f(mw[w] - M);  // warps without a tile have m = -inf -> weight 0
+                const float e = none ? 0.f : exp2f(mw[w] - M);  // warps without a tile have m = -inf -> weight 0
                 Lsum += e * scratch_ml[(w * G + g) * 2 + 1];
                 const float2 v = *reinterpret_cast<const float2*>(scratch_o + (w * G + g) * kRowF + c2 * 2);
                 ax += e * v.x, ay += e * v.y;
             }
-            const float inv = 1.f / Lsum;
-            const float lse_nat = (M + log2f(Lsum)) * 0.6931471805599453f;
+            const float inv = none ? 0.f : 1.f / Lsum;
+            const float lse_nat = none ? kNegInf : (M + log2f(Lsum)) * 0.6931471805599453f;
             if (item.n_parts == 1) {
                 const size_t hq = static_cast<size_t>(item.req) * p.Hq + static_cast<size_t>(item.kv_head) * G + g;
                 *reinterpret_cast<__nv_bfloat162*>(p.out + hq * D + c2 * 2) = __floats2bfloat162_rn(ax * inv, ay * inv);
@@ -654,6 +662,37 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == static_cast<int>(gridDim.x) - 1)
             p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
     }
+}
+
+// ------------------------------------------------------------------ NEXT-1: KV append
+// One warp per (request, KV head): the new K row and V row (d bf16 each) go to token index
+// n = kv_len[r][h] of the head's ragged pages; kv_len becomes n + 1.  A head whose table is full keeps its
+// length (the reserved budget is a hard capacity bound) and the row is counted in *overflow.
+__global__ void __launch_bounds__(128)
+tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ tbl_pages,
+                      const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, uint4* __restrict__ pool,
+                      int32_t* __restrict__ kv_len, int32_t* __restrict__ overflow, int n_seq, int Hp, int d) {
+    const int seq = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (seq >= n_seq) return;
+    const int4 si = seq_info[seq];  // {table row offset, capacity tokens, slot, -}
+    const int n = kv_len[seq];
+    if (n >= si.y) {
+        if (lane == 0 && overflow) atomicAdd(overflow, 1);
+        return;
+    }
+    const int chunks = d / 8;  // 16-byte chunks per row
+    const int page = tbl_pages[si.x + n / kPage];
+    // pool[page][slot][kv][token][d]
+    const size_t row_k = ((static_cast<size_t>(page) * Hp + si.z) * 2 + 0) * kPage + n % kPage;
+    const size_t row_v = ((static_cast<size_t>(page) * Hp + si.z) * 2 + 1) * kPage + n % kPage;
+    for (int c = lane; c < 2 * chunks; c += 32) {
+        const bool is_v = c >= chunks;
+        const int cc = is_v ? c - chunks : c;
+        const uint4 val = (is_v ? v_new : k_new)[static_cast<size_t>(seq) * chunks + cc];
+        pool[(is_v ? row_v : row_k) * chunks + cc] = val;
+    }
+    __syncwarp();
+    if (lane == 0) kv_len[seq] = n + 1;
 }
 
 // ------------------------------------------------------------------ host-side launch helpers
@@ -797,13 +836,14 @@ extern "C" size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan
     b += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
     b += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);  // merge records (upper bound)
     b += align_up(128 * (size_t)p->W, 256);                          // list heads
+    b += align_up(16 * (size_t)t->R * t->H, 256);                    // per-sequence table info (KV append)
     return b + 256 /* scheduler counters */ + 256;
 }
 
 extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
                               void* stream, tangram_device_plan* dp) {
     if (!t || !p || !dev_blob || !dp || !p->items || !p->worker_indptr || !p->part_indptr || !t->tbl_pages ||
-        !t->tbl_indptr)
+        !t->tbl_indptr || !t->cluster_of || !t->slot_of)
         return fail(TANGRAM_ERR_INVALID_ARG, "upload: NULL argument");
     if (p->n_items > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: more than 2^31 items");
     const size_t need = tangram_blob_bytes(t, p);
@@ -866,6 +906,18 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
         }
     }
     off += align_up(128 * (size_t)p->W, 256);
+    const size_t off_seqinfo = off;
+    {   // {page-table row offset, capacity in tokens, slot, 0} of every (request, KV head)
+        int32_t* si = reinterpret_cast<int32_t*>(host.data() + off);
+        for (int32_t r = 0; r < t->R; ++r)
+            for (int32_t h = 0; h < t->H; ++h, si += 4) {
+                const int64_t row = (int64_t)r * t->C + t->cluster_of[h];
+                si[0] = (int32_t)t->tbl_indptr[row];
+                si[1] = (int32_t)((t->tbl_indptr[row + 1] - t->tbl_indptr[row]) * t->P);
+                si[2] = t->slot_of[h], si[3] = 0;
+            }
+    }
+    off += align_up(16 * (size_t)t->R * t->H, 256);
     const size_t off_sched = off;
     // pageable source: the runtime stages it before returning, so `host` may die at scope exit
     cudaError_t e = cudaMemcpyAsync(dev_blob, host.data(), need, cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream));
@@ -880,6 +932,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->n_merge_seqs = n_mseq;
     dp->n_empty_seqs = n_empty;
     dp->list_heads = base + off_heads;
+    dp->seq_info = reinterpret_cast<const int32_t*>(base + off_seqinfo);
     dp->n_big_merge_seqs = n_mseq - n_not_big;
     dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
     dp->items = base + off_items;
@@ -895,7 +948,7 @@ extern "C" size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int
 }
 
 static int run_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool, int64_t n_pool_pages,
-                         int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
+                         const int32_t* kv_len_dev, int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
                          size_t workspace_bytes, uint64_t* worker_ns, void* stream, int which) {
     if (!dp || !q || !kv_pool || !out || !lse) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
     if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128}", d);
@@ -935,6 +988,7 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.n_lists = dp->W;
     prm.list_heads = dp->list_heads;
     prm.sched = dp->sched;
+    prm.kv_len = kv_len_dev, prm.H = dp->H;
 
     prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
@@ -944,24 +998,44 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
 }
 
 extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
-                                        int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                                        int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d, float sm_scale, void* out,
                                         float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
                                         void* stream) {
-    return run_attention(dp, q, kv_pool, n_pool_pages, Hq, d, sm_scale, out, lse, workspace, workspace_bytes,
-                         worker_ns, stream, kRunSplit | kRunMerge);
+    return run_attention(dp, q, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, workspace,
+                         workspace_bytes, worker_ns, stream, kRunSplit | kRunMerge);
 }
 
 extern "C" int tangram_decode_partials(const tangram_device_plan* dp, const void* q, const void* kv_pool,
-                                       int64_t n_pool_pages, int32_t Hq, int32_t d, float sm_scale, void* out,
+                                       int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d, float sm_scale, void* out,
                                        float* lse, void* workspace, size_t workspace_bytes, uint64_t* worker_ns,
                                        void* stream) {
-    return run_attention(dp, q, kv_pool, n_pool_pages, Hq, d, sm_scale, out, lse, workspace, workspace_bytes,
-                         worker_ns, stream, kRunSplit);
+    return run_attention(dp, q, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, workspace,
+                         workspace_bytes, worker_ns, stream, kRunSplit);
 }
 
 extern "C" int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d, void* out, float* lse,
                                       void* workspace, size_t workspace_bytes, void* stream) {
     // q / kv_pool are not read by the merge kernel; pass aligned dummies through the shared validation
-    return run_attention(dp, out, out, 1, Hq, d, 0.f, out, lse, workspace, workspace_bytes, nullptr, stream,
+    return run_attention(dp, out, out, 1, nullptr, Hq, d, 0.f, out, lse, workspace, workspace_bytes, nullptr, stream,
                          kRunMerge);
+}
+
+extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const void* v_new, void* kv_pool,
+                                 int64_t n_pool_pages, int32_t d, int32_t* kv_len_dev, int32_t* overflow_dev,
+                                 void* stream) {
+    if (!dp || !k_new || !v_new || !kv_pool || !kv_len_dev)
+        return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: NULL argument");
+    if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: head_dim %d not in {64, 128}", d);
+    if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: page size %d (kernels need 16)", dp->P);
+    if (n_pool_pages < 1) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: empty pool");
+    if (reinterpret_cast<uintptr_t>(k_new) % 16 || reinterpret_cast<uintptr_t>(v_new) % 16 ||
+        reinterpret_cast<uintptr_t>(kv_pool) % 16)
+        return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: misaligned pointer");
+    const int n_seq = dp->R * dp->H;
+    tangram_append_kernel<<<(n_seq + 3) / 4, 128, 0, static_cast<cudaStream_t>(stream)>>>(
+        reinterpret_cast<const int4*>(dp->seq_info), dp->tbl_pages, static_cast<const uint4*>(k_new),
+        static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
+    return TANGRAM_OK;
 }

@@ -250,3 +250,93 @@ def test_full_size_sampled(name):
     idx_r = torch.as_tensor([p[0] for p in pairs], device="cuda")
     idx_j = torch.as_tensor([p[1] for p in pairs], device="cuda")
     check(out[idx_r, idx_j], lse[idx_r, idx_j], ref_out, ref_lse, f"{name} full size")
+
+
+# ------------------------------------------------------------------------------------ NEXT-1
+def bits(x):
+    return x.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def test_append_kv_bit_exact_and_open_ended_plan():
+    """KV append (byte work: pool and lengths bit-exact against oracle O6, overflow counted) and a plan
+    built ONCE for the tables' capacity that serves every decode step through the run-time lengths."""
+    wl = I.make_workload("8b", R=3, ctx_div=32)
+    B, res, kv0, t, n_pool = setup(wl)
+    ot = oracle_tables(t)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    cap = np.zeros_like(kv0)
+    for r in range(wl.R):
+        for h in range(wl.H):
+            row = r * t.C + t.cluster_of[h]
+            cap[r, h] = (t.tbl_indptr[row + 1] - t.tbl_indptr[row]) * wl.P
+    W = n_cta(wl)
+    plan = T.tangram_plan_partitions(t, B, cap, W, wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dp = T.tangram_upload(t, plan)
+    start = np.maximum(cap - 5, 0).astype(np.int32)          # five steps to capacity, then overflow
+    start[0, 0] = 0                                            # an empty head that grows from nothing
+    start[1, :] = np.minimum(start[1, :], 40)
+    kv_dev = torch.as_tensor(start, device="cuda")
+    over_dev = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ref_bits, ref_kv, ref_over = bits(pool), start.copy(), 0
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    for step in range(8):
+        out, lse = T.tangram_decode_attention(dp, q, pool, kv_len=kv_dev)          # attends the CURRENT lengths
+        torch.cuda.synchronize()
+        pool_ref_t = torch.from_numpy(ref_bits.view(np.int16)).view(torch.bfloat16)
+        ro, rl, _ = O.attention(q.cpu(), pool_ref_t, ot, ref_kv, wl.Hq, wl.d)
+        check(out, lse, ro, rl, f"open-ended plan, step {step}")
+        k_new = torch.randn(wl.R, wl.H, wl.d, generator=gen, device="cuda").bfloat16()
+        v_new = torch.randn(wl.R, wl.H, wl.d, generator=gen, device="cuda").bfloat16()
+        T.tangram_append_kv(dp, k_new, v_new, pool, kv_dev, over_dev)
+        torch.cuda.synchronize()
+        ref_bits, ref_kv, o = O.append_kv(ref_bits, ot, ref_kv, bits(k_new), bits(v_new))
+        ref_over += o
+        assert np.array_equal(bits(pool), ref_bits) and np.array_equal(kv_dev.cpu().numpy(), ref_kv)
+        assert int(over_dev.item()) == ref_over
+    assert ref_over > 0 and np.array_equal(ref_kv[0, 1:], cap[0, 1:]) and ref_kv[0, 0] == 8
+
+
+def test_open_ended_plan_all_empty_and_shorter_lengths():
+    wl = I.make_workload("skew", R=2, ctx_div=16)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    ot = oracle_tables(t)
+    for dyn, J in ((0, 0), (500, 4)):
+        plan = T.tangram_plan_partitions(t, B, kv, 33, wl.granule, 1, T.MODE_BALANCED, 0, dyn, J)
+        dp = T.tangram_upload(t, plan)
+        rng = np.random.default_rng(9)
+        for trial in range(3):
+            cur = (kv * rng.uniform(0, 1, size=kv.shape)).astype(np.int32)
+            cur[0, trial] = 0
+            if trial == 2:
+                cur[:] = 0                                     # nothing retained anywhere
+            out, lse = T.tangram_decode_attention(dp, q, pool, kv_len=torch.as_tensor(cur, device="cuda"))
+            torch.cuda.synchronize()
+            ro, rl, _ = O.attention(q.cpu(), pool.cpu(), ot, cur, wl.Hq, wl.d)
+            check(out, lse, ro, rl, f"run-time lengths trial {trial} dyn={dyn}")
+
+
+def test_no_write_outside_the_output_buffers():
+    """compute-sanitizer is closed on this pool, so bounds are checked with guard regions: out, lse and the
+    workspace sit inside larger buffers filled with a sentinel that must survive the call."""
+    wl = I.make_workload("32b", R=3, ctx_div=16)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    plan = T.tangram_plan_partitions(t, B, kv, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dp = T.tangram_upload(t, plan)
+    pad = 4096
+    n_out, n_lse = q.numel() * 2, wl.R * wl.Hq * 4
+    n_ws = T.tangram_workspace_bytes(plan.n_part_slots, wl.G, wl.d)
+    big = torch.full((pad + n_out + pad + n_lse + pad + n_ws + pad,), 0x5A, dtype=torch.uint8, device="cuda")
+    o0, l0, w0 = pad, pad + n_out + pad, pad + n_out + pad + n_lse + pad
+    out = big[o0:o0 + n_out].view(torch.bfloat16).view(wl.R, wl.Hq, wl.d)
+    lse = big[l0:l0 + n_lse].view(torch.float32).view(wl.R, wl.Hq)
+    ws = big[w0:w0 + n_ws]
+    pool_before = pool.clone()
+    T.tangram_decode_attention(dp, q, pool, out, lse, ws)
+    torch.cuda.synchronize()
+    for a, b in ((0, o0), (o0 + n_out, l0), (l0 + n_lse, w0), (w0 + n_ws, big.numel())):
+        assert bool((big[a:b] == 0x5A).all()), (a, b)
+    assert torch.equal(pool.view(torch.int16), pool_before.view(torch.int16))     # the cache is read-only here
+    ro, rl, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    check(out, lse, ro, rl, "guarded buffers")
