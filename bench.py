@@ -147,9 +147,9 @@ def algorithmic_bytes(wl, kv, plan, t):
             "total": kv_bytes + qo + partials + page_ids}
 
 
-def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None):
+def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None, layer=0, plan_capacity=False):
     import torch
-    wl = I.make_workload(name)
+    wl = I.make_workload(name, layer=layer)
     t0 = time.perf_counter()
     B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
     need = T.tangram_pages_needed(B, res, wl.C, wl.P)
@@ -162,7 +162,11 @@ def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None):
         W = T.tangram_query_max_ctas(torch.cuda.current_device(), wl.d, wl.G)
     t3 = time.perf_counter()
     dyn = (T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS) if dyn is None else dyn
-    plan = T.tangram_plan_partitions(tb, B, kv, W, wl.granule, c0, T.MODE_BALANCED if mode is None else mode, 0,
+    kv_plan = kv
+    if plan_capacity:      # open-ended plan: built once for the tables' capacity, serves every decode step
+        rows = np.arange(wl.R)[:, None] * tb.C + tb.cluster_of[None, :]
+        kv_plan = ((tb.tbl_indptr[rows + 1] - tb.tbl_indptr[rows]) * wl.P).astype(np.int32)
+    plan = T.tangram_plan_partitions(tb, B, kv_plan, W, wl.granule, c0, T.MODE_BALANCED if mode is None else mode, 0,
                                      dyn[0], dyn[1])
     t4 = time.perf_counter()
     q, pool = I.make_q_and_pool(wl, n_pool, device)
@@ -310,6 +314,58 @@ def reference_arm(args):
 
 
 # ------------------------------------------------------------------------------------------------
+# NEXT-1: a real decode loop -- L layers x (KV append + attention) per step under ONE CUDA graph
+# ------------------------------------------------------------------------------------------------
+def decode_loop(T, I, name, device, layers, steps, torch):
+    """Every layer has its own budgets, clusters, tables and an open-ended plan built once for the
+    tables' capacity; one decode step = for each layer: tangram_append_kv, then tangram_decode_attention
+    on the run-time lengths.  The L-layer step is captured in one CUDA graph and replayed: zero host
+    planning across steps and layers.  The layers' pools are distinct and far larger than
+    L2 together, so no flush is needed between layer-steps."""
+    Ls = []
+    for l in range(layers):
+        S = setup_workload(T, I, name, device, layer=l, plan_capacity=True)
+        prepare(T, S, torch)
+        S["kv_dev"] = torch.as_tensor(S["kv"], device=device)
+        g = torch.Generator(device=device).manual_seed(S["wl"].seed + 17)
+        S["k_new"] = torch.randn(S["wl"].R, S["wl"].H, S["wl"].d, generator=g, device=device).bfloat16()
+        S["v_new"] = torch.randn(S["wl"].R, S["wl"].H, S["wl"].d, generator=g, device=device).bfloat16()
+        Ls.append(S)
+
+    def one_step(stream=None):
+        for S in Ls:
+            T.tangram_append_kv(S["dp"], S["k_new"], S["v_new"], S["pool"], S["kv_dev"], stream=stream)
+            T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"], kv_len=S["kv_dev"],
+                                       stream=stream)
+
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        one_step(st)                                  # warm-up outside the capture
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=st):
+            one_step(st)
+        for _ in range(3):
+            graph.replay()
+        st.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            a.record(st)
+            graph.replay()
+            b.record(st)
+        st.synchronize()
+    torch.cuda.current_stream().wait_stream(st)
+    ms = np.array([a.elapsed_time(b) for a, b in evs])
+    kv_bytes = float(np.mean([int(S["kv_dev"].sum().item()) * 4 * S["wl"].d for S in Ls]))
+    us_layer = float(np.median(ms)) * 1e3 / layers
+    return {"layers": layers, "steps": steps, "us_per_layer_step": us_layer, "us_per_decode_step": us_layer * layers,
+            "tbs": kv_bytes / (us_layer * 1e-6) / 1e12, "pct_of_8tbs": 100 * kv_bytes / (us_layer * 1e-6) / 1e12 / NOMINAL_TBS,
+            "launches_per_layer_step": 2, "host_planning_per_step_ms": 0.0,
+            "note": "append + attention per layer, open-ended plans built once, whole L-layer step in one CUDA graph; "
+                    "kv bytes = retained K/V at the end of the loop (the lengths grow by one token per step)"}
+
+
+# ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
 def spread_of(T, S, torch, reps=5):
@@ -404,6 +460,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dyn-permille", type=int, default=None, help="dynamic-tail share of the BALANCED plan")
     ap.add_argument("--dyn-rounds", type=int, default=None)
+    ap.add_argument("--decode-loop-layers", type=int, default=8,
+                    help="layers of the multi-layer decode loop summary (0 = skip)")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_arm(args)
@@ -506,6 +564,8 @@ def main():
             del S2
             torch.cuda.empty_cache()
         line["per_config"] = per
+        if args.decode_loop_layers > 0:
+            line["decode_loop"] = decode_loop(T, I, args.workload, device, args.decode_loop_layers, 30, torch)
     elif not args.no_cpu_baseline and world == 1:
         from oracle import tangram_oracle as O
         O.build_c()

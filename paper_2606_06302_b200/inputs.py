@@ -65,12 +65,17 @@ def _jitter(rng: np.random.Generator, ratio_h: np.ndarray, R: int, hw: float) ->
     return np.minimum(1.0, ratio_h[None, :] * (1.0 + u))
 
 
-def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1) -> Workload:
+def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1, layer: int = 0) -> Workload:
     """Build config `name` (one of CONFIG_NAMES).  `R` overrides the batch size and
     `ctx_div` divides every context length (scaled-down parity cases); the default
-    arguments give the full BASELINE.json configuration."""
+    arguments give the full BASELINE.json configuration.  `layer` > 0 draws another layer of the
+    same shape (its own head ratios, i.e. its own budgets, clusters and plan) for multi-layer
+    decode loops: seed + 1000 * layer; the context lengths of layer 0 are kept (same requests)."""
     idx = CONFIG_NAMES.index(name)
     seed = SEED_BASE + idx
+    if layer:
+        base = make_workload(name, R=R, ctx_div=ctx_div)
+        seed += 1000 * layer
     rng = np.random.default_rng(seed)
     P, alpha, g = 16, 2.0, 64
 
@@ -116,6 +121,8 @@ def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1) -> Wo
         raise ValueError(name)
 
     ctx = np.maximum(ctx, 1).astype(np.int32)
+    if layer:
+        ctx = base.ctx_len.copy()
     ratio_rh = _jitter(rng, ratio_h, R_, hw)
     mu = ratio_h.astype(np.float64).copy()
     sigma = (hw * mu / math.sqrt(3.0)) if hw > 0 else np.zeros(H)

@@ -340,3 +340,53 @@ def test_no_write_outside_the_output_buffers():
     assert torch.equal(pool.view(torch.int16), pool_before.view(torch.int16))     # the cache is read-only here
     ro, rl, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
     check(out, lse, ro, rl, "guarded buffers")
+
+
+def test_multi_layer_decode_loop_under_one_cuda_graph():
+    """L layers x (append + attention) captured in one CUDA graph and replayed for several decode steps:
+    every layer's output after the last replay matches the oracle run on the oracle-side cache."""
+    L, steps = 3, 4
+    layers = []
+    for l in range(L):
+        wl = I.make_workload("32b", R=2, ctx_div=32, layer=l)
+        B, res, kv, t, n_pool = setup(wl)
+        q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+        rows = np.arange(wl.R)[:, None] * t.C + t.cluster_of[None, :]
+        cap = ((t.tbl_indptr[rows + 1] - t.tbl_indptr[rows]) * wl.P).astype(np.int32)
+        plan = T.tangram_plan_partitions(t, B, cap, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+        dp = T.tangram_upload(t, plan)
+        g = torch.Generator(device="cuda").manual_seed(100 + l)
+        layers.append(dict(wl=wl, t=t, kv=kv.copy(), q=q, pool=pool, dp=dp, kv_dev=torch.as_tensor(kv, device="cuda"),
+                           k=torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16(),
+                           v=torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16(),
+                           out=torch.empty_like(q), lse=torch.empty(wl.R, wl.Hq, device="cuda"),
+                           ws=torch.empty(T.tangram_workspace_bytes(plan.n_part_slots, wl.G, wl.d), dtype=torch.uint8,
+                                          device="cuda"),
+                           ref_bits=bits(pool)))
+    assert (not np.array_equal(layers[0]["t"].perm, layers[1]["t"].perm)
+            or not np.array_equal(layers[0]["kv"], layers[1]["kv"]))          # the layers really differ
+
+    def step(st):
+        for S in layers:
+            T.tangram_append_kv(S["dp"], S["k"], S["v"], S["pool"], S["kv_dev"], stream=st)
+            T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"], kv_len=S["kv_dev"], stream=st)
+
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        step(st)                                                               # decode step 1 (eager)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=st):
+            step(st)
+        for _ in range(steps - 1):                                             # decode steps 2 .. steps
+            graph.replay()
+    torch.cuda.synchronize()
+    for S in layers:
+        ot = oracle_tables(S["t"])
+        rb, rk = S["ref_bits"], S["kv"]
+        for _ in range(steps):
+            rb, rk, _ = O.append_kv(rb, ot, rk, bits(S["k"]), bits(S["v"]))
+        assert np.array_equal(bits(S["pool"]), rb) and np.array_equal(S["kv_dev"].cpu().numpy(), rk)
+        ro, rl, _ = O.attention(S["q"].cpu(), torch.from_numpy(rb.view(np.int16)).view(torch.bfloat16), ot, rk,
+                                S["wl"].Hq, S["wl"].d)
+        check(S["out"], S["lse"], ro, rl, "multi-layer graph loop")
