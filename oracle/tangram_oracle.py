@@ -15,6 +15,8 @@ What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.
                           equal-bytes work list, reading A2), STATIC_EVEN (FlashDecoding-style
                           uniform num_splits, :120)
   O5 merge                log-sum-exp merge of split-KV partials (implied by split-KV :91, :120)
+  O7 topk_indices /       per-head Top-ceil(B N) selection (Eq. 4 :154) and K~ = K[I,:], V~ = V[I,:] (Eq. 1
+     compact_topk         :57) written into the ragged pages (NEXT-2; tie rule = reading A30)
   O6 append_kv            one decode step's new K/V rows written into the ragged pages (NEXT-1;
                           page layout :190, capacity bound :176, reading A29)
   O1 attention*           plain softmax(q K~^T / sqrt(d)) V~ through the page tables (Eq. 1 :57)
@@ -361,6 +363,48 @@ def append_kv(pool_bits: np.ndarray, t: Tables, kv_len, k_new_bits: np.ndarray, 
             pool[page, s, 1, n % t.P, :] = v_new_bits[r, h, :]
             kv[r, h] = n + 1
     return pool, kv, over
+
+
+# --------------------------------------------------------------------------------------------
+# O7  per-head Top-k selection + compaction into the ragged pages (NEXT-2; Eq. 4 :154, Eq. 1 :57)
+# --------------------------------------------------------------------------------------------
+def topk_indices(scores, k: int) -> np.ndarray:
+    """I = Top(k, s) (Eq. 4): the k highest-scoring token indices, returned in ascending token order
+    (storage order = logical order, reading A22).  Scores are compared as the fp32 values they are;
+    among equal scores the lower token index wins (reading A30: the paper does not break ties)."""
+    s = np.asarray(scores, dtype=np.float32)
+    order = sorted(range(len(s)), key=lambda i: (-float(s[i]), i))
+    return np.array(sorted(order[:k]), dtype=np.int64)
+
+
+def compact_topk(pool_bits: np.ndarray, t: Tables, scores, k_dense_bits, v_dense_bits, ctx_len, keep):
+    """K~ = K[I,:], V~ = V[I,:] (Eq. 1) with I = Top(keep[r][h], s_{r,h}[:N_r]) (Eq. 4) written into the
+    ragged pages of head h in token order.
+
+    pool_bits              uint16 [n_pages][Hp][2][P][d] (a modified COPY is returned)
+    scores                 float32 [R][H][n_max]   (entries >= ctx_len[r] are ignored)
+    k_dense_bits, v_dense_bits  uint16 [R][H][n_max][d]  the uncompressed cache
+    keep                   int [R][H]  tokens to retain (= kv_len of a1; <= ctx_len and <= table capacity)
+    Returns (pool', indices) with indices[r][h] the retained token indices."""
+    pool = np.array(pool_bits, dtype=np.uint16, copy=True)
+    out_idx = [[None] * t.H for _ in range(t.R)]
+    for r in range(t.R):
+        N = int(ctx_len[r])
+        for h in range(t.H):
+            k = int(keep[r][h])
+            if k > N:
+                raise ValueError("keep > ctx_len")
+            c, sl = int(t.cluster_of[h]), int(t.slot_of[h])
+            lo, hi = int(t.tbl_indptr[r * t.C + c]), int(t.tbl_indptr[r * t.C + c + 1])
+            if k > (hi - lo) * t.P:
+                raise ValueError("keep exceeds the table capacity")
+            idx = topk_indices(np.asarray(scores[r][h])[:N], k)
+            out_idx[r][h] = idx
+            for pos, tok in enumerate(idx):
+                page = int(t.tbl_pages[lo + pos // t.P])
+                pool[page, sl, 0, pos % t.P, :] = k_dense_bits[r, h, tok, :]
+                pool[page, sl, 1, pos % t.P, :] = v_dense_bits[r, h, tok, :]
+    return pool, out_idx
 
 
 # --------------------------------------------------------------------------------------------

@@ -511,3 +511,60 @@ def test_append_kv_round_trip_against_dense_attention():
             ref = torch.softmax(sc, 0) @ Vd
             assert np.allclose(out[r, j], ref.numpy(), rtol=0, atol=1e-12)
             assert abs(lse[r, j] - float(torch.logsumexp(sc, 0))) < 1e-12
+
+
+# ---------------------------------------------------------------------------- O7 Top-k + compaction (NEXT-2)
+def test_topk_indices_definition_and_ties():
+    """Brute-force definition: token i is retained iff fewer than k tokens beat it, where j beats i when
+    s_j > s_i, or s_j == s_i and j < i.  Includes heavy ties, negative scores, +-0 and infinities."""
+    rng = np.random.default_rng(31)
+    cases = [rng.normal(size=40).astype(np.float32),
+             rng.integers(0, 4, size=50).astype(np.float32),                # many ties
+             np.array([0.0, -0.0, 1.0, -1.0, np.inf, -np.inf, 1.0, 0.0], dtype=np.float32),
+             np.full(9, 2.5, dtype=np.float32)]
+    for s in cases:
+        n = len(s)
+        for k in (0, 1, n // 3, n - 1, n):
+            want = [i for i in range(n)
+                    if sum(1 for j in range(n) if s[j] > s[i] or (s[j] == s[i] and j < i)) < k]
+            got = O.topk_indices(s, k)
+            assert got.tolist() == want
+            if 0 < k < n:
+                dropped = np.setdiff1d(np.arange(n), got)
+                assert s[got].min() >= s[dropped].max()
+    assert O.topk_indices(np.array([3, 1, 2], dtype=np.float32), 2).tolist() == [0, 2]   # ascending token order
+
+
+def test_compact_topk_round_trip_against_dense_attention():
+    """Eq. 1 through the pages: attention over the compacted cache (pinned gather O1) equals dense library
+    attention over K[I,:], V[I,:] with I from the brute-force-pinned selection; untouched pool bytes survive."""
+    R, H, G, d, P, n_max = 2, 4, 2, 64, 16, 90
+    ctx = np.array([90, 57], dtype=np.int32)
+    keep = np.array([[90, 20, 45, 1], [57, 0, 30, 16]], dtype=np.int32)
+    B = np.array([1.0, 0.25, 0.5, 0.2])
+    t, _ = O.build_ragged_tables(B, keep, 2, P, np.random.default_rng(4).permutation(60).astype(np.int32))
+    g = torch.Generator().manual_seed(33)
+    scores = torch.randn(R, H, n_max, generator=g).numpy()
+    Kd = torch.randn(R, H, n_max, d, generator=g).bfloat16()
+    Vd = torch.randn(R, H, n_max, d, generator=g).bfloat16()
+    pool0 = torch.randn(60, t.Hp, 2, P, d, generator=g).bfloat16()
+    b0 = pool0.view(torch.int16).numpy().view(np.uint16)
+    kb = Kd.view(torch.int16).numpy().view(np.uint16)
+    vb = Vd.view(torch.int16).numpy().view(np.uint16)
+    b1, idx = O.compact_topk(b0, t, scores, kb, vb, ctx, keep)
+    assert (b1 != b0).sum() <= int(keep.sum()) * 2 * d
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    out, lse, _ = O.attention(q, torch.from_numpy(b1.view(np.int16)).view(torch.bfloat16), t, keep, H * G, d)
+    for r in range(R):
+        for j in range(H * G):
+            h = j // G
+            I_ = idx[r][h]
+            assert len(I_) == keep[r, h] and (len(I_) == 0 or I_.max() < ctx[r])
+            if len(I_) == 0:
+                assert np.all(out[r, j] == 0) and lse[r, j] == -math.inf
+                continue
+            sc = (Kd[r, h, I_].double() @ q[r, j].double()) / math.sqrt(d)
+            ref = torch.softmax(sc, 0) @ Vd[r, h, I_].double()
+            assert np.allclose(out[r, j], ref.numpy(), rtol=0, atol=1e-12)
+    with pytest.raises(ValueError):
+        O.compact_topk(b0, t, scores, kb, vb, ctx, keep + 100)
