@@ -252,6 +252,36 @@ int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const vo
                       int64_t n_pool_pages, int32_t d, int32_t* kv_len_dev, int32_t* overflow_dev,
                       void* stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-2  Per-head Top-k selection + compaction into the ragged pages.
+ * PAPER.md:152-154 (Eq. 4: I_{l,h} = Top(ceil(B_{l,h} N), s_{l,h}) -- every head selects on its own scores
+ * with its own static budget), :57-58 (Eq. 1: K~ = K[I,:], V~ = V[I,:]), :190 (the retained rows live in
+ * the ragged pages of the head's group), :176 (the reserved budget is a hard capacity bound).
+ *
+ * For every (request r, KV head h): the keep[r][h] highest-scoring tokens among the first ctx_len[r] are
+ * selected -- scores compared as the fp32 values they are (-0 == +0), among equal scores the lower token
+ * index wins -- and their K rows and V rows are written, in ascending token order, to token slots
+ * 0 .. keep-1 of head h's pages: pool[tbl_pages[row(r, cluster_of[h]) + pos / P]][slot_of[h]][kv][pos % P][:].
+ * Nothing else in the pool is written.  Scores must not be NaN (their order is then unspecified).
+ *
+ *   dp            from tangram_upload (uses the tables only)
+ *   scores        device [R][H][n_max] f32   importance of every token (entries >= ctx_len[r] are ignored)
+ *   k_dense, v_dense  device [R][H][n_max][d] bf16, 16-byte aligned: the uncompressed cache
+ *   ctx_len_dev   device [R] i32, 1 <= ctx_len[r] <= n_max
+ *   keep_dev      device [R][H] i32  tokens to retain (= kv_len of a1).  A value outside
+ *                 [0, min(ctx_len[r], pages(r, cluster) x P)] is clamped into it and the head is counted
+ *   kv_pool       device [n_pool_pages][Hp][2][P][d] bf16 (written)
+ *   idx_out       device [R][H][n_max] i32: the first keep[r][h] entries of row (r, h) receive the retained
+ *                 token indices in ascending order (the set I of Eq. 4); the rest is not touched
+ *   clamped_dev   device i32 or NULL: incremented by the number of clamped heads
+ *   workspace     device, >= tangram_compact_workspace_bytes(R, H), 16-byte aligned
+ * Asynchronous on `stream` (three launches); graph capturable.  Errors: INVALID_ARG, BUFFER_TOO_SMALL, CUDA. */
+size_t tangram_compact_workspace_bytes(int32_t R, int32_t H);
+int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
+                         const void* v_dense, int64_t n_max, const int32_t* ctx_len_dev, const int32_t* keep_dev,
+                         void* kv_pool, int64_t n_pool_pages, int32_t d, int32_t* idx_out, int32_t* clamped_dev,
+                         void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

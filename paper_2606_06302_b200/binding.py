@@ -63,14 +63,17 @@ _lib.tangram_last_error.restype = C.c_char_p
 _lib.tangram_blob_bytes.restype = C.c_size_t
 _lib.tangram_workspace_bytes.restype = C.c_size_t
 _lib.tangram_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
+_lib.tangram_compact_workspace_bytes.restype = C.c_size_t
+_lib.tangram_compact_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
 for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
-              "tangram_merge_partials", "tangram_append_kv"):
+              "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
-           "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv")
+           "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
+           "tangram_compact_workspace_bytes", "tangram_compact_topk")
 
 
 def _check(rc: int):
@@ -289,3 +292,36 @@ def tangram_append_kv(dp: DevicePlan, k_new, v_new, kv_pool, kv_len, overflow=No
                                   C.c_void_p(kv_pool.data_ptr()), C.c_int64(kv_pool.shape[0]), C.c_int32(d),
                                   C.c_void_p(kv_len.data_ptr()), ov, sp))
     return kv_len
+
+
+def tangram_compact_workspace_bytes(R: int, H: int) -> int:
+    return int(_lib.tangram_compact_workspace_bytes(R, H))
+
+
+def tangram_compact_topk(dp: DevicePlan, scores, k_dense, v_dense, ctx_len, keep, kv_pool, idx_out=None,
+                         clamped=None, workspace=None, stream=None):
+    """NEXT-2: per-head Top-keep[r][h] selection on `scores` ([R,H,n_max] f32) and compaction of the selected
+    K/V rows ([R,H,n_max,d] bf16 each) into the ragged pages.  ctx_len [R] / keep [R,H] int32 cuda.
+    -> idx_out [R,H,n_max] int32 (first keep[r][h] entries of each row = retained token indices, ascending)."""
+    import torch
+    R, H, n_max, d = k_dense.shape
+    assert scores.is_cuda and k_dense.is_cuda and v_dense.is_cuda and kv_pool.is_cuda and ctx_len.is_cuda and keep.is_cuda
+    assert scores.dtype == torch.float32 and tuple(scores.shape) == (R, H, n_max) and scores.is_contiguous()
+    assert k_dense.dtype == torch.bfloat16 and v_dense.dtype == torch.bfloat16 and v_dense.shape == k_dense.shape
+    assert k_dense.is_contiguous() and v_dense.is_contiguous() and kv_pool.is_contiguous()
+    assert ctx_len.dtype == torch.int32 and keep.dtype == torch.int32 and ctx_len.numel() == R and keep.numel() == R * H
+    assert ctx_len.is_contiguous() and keep.is_contiguous()
+    assert (R, H) == (dp.c.R, dp.c.H) and tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d)
+    if idx_out is None:
+        idx_out = torch.empty(R, H, n_max, dtype=torch.int32, device=scores.device)
+    need = tangram_compact_workspace_bytes(R, H)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=scores.device)
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    cl = C.c_void_p(clamped.data_ptr()) if clamped is not None else None
+    _check(_lib.tangram_compact_topk(C.byref(dp.c), C.c_void_p(scores.data_ptr()), C.c_void_p(k_dense.data_ptr()),
+                                     C.c_void_p(v_dense.data_ptr()), C.c_int64(n_max), C.c_void_p(ctx_len.data_ptr()),
+                                     C.c_void_p(keep.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
+                                     C.c_int64(kv_pool.shape[0]), C.c_int32(d), C.c_void_p(idx_out.data_ptr()), cl,
+                                     C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), sp))
+    return idx_out

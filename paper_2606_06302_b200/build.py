@@ -10,7 +10,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtangram.so")
-SOURCES = [os.path.join(CSRC, "tangram_decode.cu"), os.path.join(CSRC, "tangram_host.cpp")]
+SOURCES = [os.path.join(CSRC, "tangram_decode.cu"), os.path.join(CSRC, "tangram_compact.cu"),
+           os.path.join(CSRC, "tangram_host.cpp")]
 HEADERS = [os.path.join(ROOT, "include", "tangram.h"), os.path.join(CSRC, "tangram_internal.h")]
 
 

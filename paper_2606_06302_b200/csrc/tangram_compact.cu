@@ -1,0 +1,322 @@
+// NEXT-2 of SURVEY.md §8(f): per-head Top-k selection (Eq. 4: I = Top(ceil(B N), s)) and
+// compaction K~ = K[I,:], V~ = V[I,:] (Eq. 1) into the ragged pages (:190).  Contract:
+// include/tangram.h (tangram_compact_topk).  Three launches on the caller's stream:
+//
+//   1. compact_prepare_kernel   one CTA: clamps keep[r][h] to [0, min(N_r, table capacity)] (the reserved
+//      budget is a hard capacity bound, :176), counts the clamped heads, and scans ceil(keep / P) into a
+//      tile index (tile = the P token slots of one (page, head)); zeroes the gather kernel's chunk counter.
+//   2. topk_select_kernel       one 1024-thread CTA per (request, KV head): radix select (4 passes of 8 bits,
+//      per-warp histograms) over a monotone integer image of the fp32 score finds the threshold key T
+//      and how many of the entries equal to T are kept (the lowest token indices first, reading A30); an
+//      ordered pass then writes the retained token indices in ascending order: the entry at token i goes to
+//      position (#greater before i) + min(#equal before i, need).  Integer work on fp32 bit patterns: the
+//      result is the unique Top-k under the tie rule, bit-exact against the sort-based oracle.
+//   3. compact_gather_kernel    persistent grid, warps claim chunks of tiles from a global counter (the same
+//      run-time balancing as the decode kernel's dynamic tail: per-SM bandwidth differs on B200).  A warp
+//      moves one tile: up to P K rows and P V rows of d bf16 each, gathered with 16-byte loads (16 in
+//      flight per lane) and stored as two contiguous runs of the page.  HBM-bound: 4*d bytes read +
+//      4*d bytes written per retained token-head.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "tangram.h"
+#include "tangram_internal.h"
+
+namespace tangram {
+
+constexpr int kCPage = 16;           // tokens per page (the kernels are specialised for P = 16)
+constexpr int kSelThreads = 1024;
+constexpr int kSelWarps = kSelThreads / 32;
+constexpr int kGatherThreads = 256;
+constexpr int kGatherChunk = 8;      // tiles claimed at once
+
+// Workspace (int32 words): [0] chunk counter, [1] total tiles, [2..3] pad, then keep_eff[n_seq],
+// then tile_indptr[n_seq + 1].
+struct CompactWs {
+    int32_t* counter;
+    int32_t* keep_eff;
+    int32_t* tile_indptr;
+};
+static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 4 + (size_t)n_seq + (size_t)n_seq + 1; }
+
+// fp32 score -> uint32 key with the same order (larger score = larger key); -0.0 and +0.0 compare equal
+// as they do as fp32 values.
+__device__ __forceinline__ uint32_t score_key(float x) {
+    uint32_t u = __float_as_uint(x);
+    if ((u << 1) == 0u) u = 0u;
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+__global__ void __launch_bounds__(1024)
+compact_prepare_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ ctx_len,
+                       const int32_t* __restrict__ keep, int n_seq, int H, int32_t* __restrict__ counter,
+                       int32_t* __restrict__ keep_eff, int32_t* __restrict__ tile_indptr, int32_t* __restrict__ clamped) {
+    __shared__ int s_warp[32];
+    __shared__ int s_run, s_bad;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_run = 0, s_bad = 0;
+    __syncthreads();
+    for (int base = 0; base < n_seq; base += blockDim.x) {
+        const int seq = base + tid;
+        int tiles = 0, bad = 0;
+        if (seq < n_seq) {
+            const int want = keep[seq];
+            const int cap = min(ctx_len[seq / H], seq_info[seq].y);  // {table row offset, capacity tokens, slot, -}
+            const int k = max(0, min(want, cap));
+            bad = k != want;
+            keep_eff[seq] = k;
+            tiles = (k + kCPage - 1) / kCPage;
+        }
+        int incl = tiles;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        const unsigned badmask = __ballot_sync(0xffffffffu, bad);
+        if (lane == 0 && badmask) atomicAdd(&s_bad, __popc(badmask));
+        __syncthreads();
+        int before = s_run;
+        for (int w = 0; w < warp; ++w) before += s_warp[w];
+        if (seq < n_seq) tile_indptr[seq] = before + incl - tiles;
+        __syncthreads();
+        if (tid == blockDim.x - 1) s_run = before + incl;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        tile_indptr[n_seq] = s_run;
+        counter[0] = 0, counter[1] = s_run;
+        if (clamped && s_bad) atomicAdd(clamped, s_bad);
+    }
+}
+
+__global__ void __launch_bounds__(kSelThreads)
+topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len,
+                   const int32_t* __restrict__ keep_eff, int H, int32_t* __restrict__ idx_out) {
+    __shared__ uint32_t s_hist[kSelWarps][256];
+    __shared__ uint32_t s_total[256];
+    __shared__ uint32_t s_prefix, s_krem;
+    __shared__ uint32_t s_wgt[kSelWarps], s_weq[kSelWarps];
+    const int seq = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = ctx_len[seq / H];
+    const int k = keep_eff[seq];
+    if (k <= 0) return;
+    const float* s = scores + static_cast<size_t>(seq) * n_max;
+    int32_t* idx = idx_out + static_cast<size_t>(seq) * n_max;
+    if (k >= N) {  // everything is retained
+        for (int i = tid; i < N; i += kSelThreads) idx[i] = i;
+        return;
+    }
+    // ---- radix select of the k-th largest key
+    uint32_t prefix = 0, mask = 0, krem = static_cast<uint32_t>(k);
+    for (int pass = 0; pass < 4; ++pass) {
+        const int shift = 24 - 8 * pass;
+        for (int b = tid; b < kSelWarps * 256; b += kSelThreads) (&s_hist[0][0])[b] = 0u;
+        __syncthreads();
+        for (int i = tid; i < N; i += kSelThreads) {
+            const uint32_t key = score_key(__ldg(s + i));
+            if ((key & mask) == prefix) atomicAdd(&s_hist[warp][(key >> shift) & 255u], 1u);
+        }
+        __syncthreads();
+        if (tid < 256) {
+            uint32_t t = 0;
+#pragma unroll 8
+            for (int w = 0; w < kSelWarps; ++w) t += s_hist[w][tid];
+            s_total[tid] = t;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            // lane owns bins [8 lane, 8 lane + 8); `above` = entries in the bins of higher lanes
+            uint32_t c[8], mine = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) c[j] = s_total[8 * lane + j], mine += c[j];
+            uint32_t incl = mine;  // inclusive suffix sum over lanes
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t v = __shfl_down_sync(0xffffffffu, incl, o);
+                if (lane + o < 32) incl += v;
+            }
+            uint32_t gt = incl - mine;
+#pragma unroll
+            for (int j = 7; j >= 0; --j) {
+                if (gt < krem && krem <= gt + c[j]) {  // exactly one (lane, j) satisfies this
+                    s_prefix = prefix | (static_cast<uint32_t>(8 * lane + j) << shift);
+                    s_krem = krem - gt;
+                }
+                gt += c[j];
+            }
+        }
+        __syncthreads();
+        prefix = s_prefix, krem = s_krem;
+        mask |= 255u << shift;
+    }
+    const uint32_t T = prefix, need = krem;  // keep every key > T and the first `need` entries with key == T
+    // ---- ordered pass: position of token i = #greater before i + min(#equal before i, need)
+    uint32_t run_gt = 0, run_eq = 0;
+    for (int base = 0; base < N; base += kSelThreads) {
+        const int i = base + tid;
+        uint32_t key = 0;
+        bool gt = false, eq = false;
+        if (i < N) {
+            key = score_key(__ldg(s + i));
+            gt = key > T, eq = key == T;
+        }
+        const unsigned bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
+        if (lane == 0) s_wgt[warp] = __popc(bg), s_weq[warp] = __popc(be);
+        __syncthreads();
+        // every warp scans the 32 warp counts redundantly
+        uint32_t wg = s_wgt[lane], we = s_weq[lane];
+        uint32_t ig = wg, ie = we;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t vg = __shfl_up_sync(0xffffffffu, ig, o), ve = __shfl_up_sync(0xffffffffu, ie, o);
+            if (lane >= o) ig += vg, ie += ve;
+        }
+        const uint32_t tot_g = __shfl_sync(0xffffffffu, ig, 31), tot_e = __shfl_sync(0xffffffffu, ie, 31);
+        const uint32_t warp_g = __shfl_sync(0xffffffffu, ig - wg, warp), warp_e = __shfl_sync(0xffffffffu, ie - we, warp);
+        const uint32_t lt = (1u << lane) - 1u;
+        const uint32_t gt_before = run_gt + warp_g + __popc(bg & lt);
+        const uint32_t eq_before = run_eq + warp_e + __popc(be & lt);
+        if (gt || (eq && eq_before < need)) idx[gt_before + min(eq_before, need)] = i;
+        run_gt += tot_g, run_eq += tot_e;
+        __syncthreads();  // s_wgt / s_weq are rewritten by the next chunk
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(kGatherThreads, 2)
+compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ tbl_pages,
+                      const int32_t* __restrict__ idx, int64_t n_max, const uint4* __restrict__ k_dense,
+                      const uint4* __restrict__ v_dense, uint4* __restrict__ pool, int Hp, int n_seq,
+                      int32_t* __restrict__ counter, const int32_t* __restrict__ keep_eff,
+                      const int32_t* __restrict__ tile_indptr) {
+    constexpr int kChunks = D / 8;           // 16-byte chunks per row
+    constexpr int kRowsPerLd = 32 / kChunks;  // rows one warp-wide load covers
+    constexpr int kLds = kCPage / kRowsPerLd; // loads per lane for the K rows of a tile (same for V)
+    const int lane = threadIdx.x & 31;
+    const int sub = lane / kChunks, ch = lane % kChunks;
+    const int total = __ldg(counter + 1);
+    for (;;) {
+        int first = 0;
+        if (lane == 0) first = atomicAdd(counter, kGatherChunk);
+        first = __shfl_sync(0xffffffffu, first, 0);
+        if (first >= total) break;
+        const int last = min(first + kGatherChunk, total);
+        // sequence of the chunk's first tile: largest seq with tile_indptr[seq] <= first
+        int lo = 0, hi = n_seq;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(tile_indptr + mid) <= first) lo = mid;
+            else hi = mid;
+        }
+        int seq = lo;
+        int seq_end = __ldg(tile_indptr + seq + 1);
+        for (int tile = first; tile < last; ++tile) {
+            while (tile >= seq_end) ++seq, seq_end = __ldg(tile_indptr + seq + 1);  // skips heads that keep nothing
+            const int tl = tile - __ldg(tile_indptr + seq);  // tile inside the sequence = index of its page in the table row
+            const int4 si = __ldg(seq_info + seq);           // {table row offset, capacity tokens, slot, -}
+            const int n_rows = min(kCPage, __ldg(keep_eff + seq) - tl * kCPage);
+            const int page = __ldg(tbl_pages + si.x + tl);
+            int my_tok = 0;
+            if (lane < n_rows) my_tok = __ldg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
+            uint4 kreg[kLds], vreg[kLds];
+#pragma unroll
+            for (int j = 0; j < kLds; ++j) {
+                const int row = j * kRowsPerLd + sub;
+                const int tok = __shfl_sync(0xffffffffu, my_tok, row);
+                if (row < n_rows) {
+                    const size_t src = (static_cast<size_t>(seq) * n_max + tok) * kChunks + ch;
+                    kreg[j] = __ldcs(k_dense + src);
+                    vreg[j] = __ldcs(v_dense + src);
+                }
+            }
+            // pool[page][slot][kv][token][d]
+            const size_t dst_k = ((static_cast<size_t>(page) * Hp + si.z) * 2) * kCPage * kChunks;
+            const size_t dst_v = dst_k + static_cast<size_t>(kCPage) * kChunks;
+#pragma unroll
+            for (int j = 0; j < kLds; ++j) {
+                const int row = j * kRowsPerLd + sub;
+                if (row < n_rows) {
+                    pool[dst_k + row * kChunks + ch] = kreg[j];
+                    pool[dst_v + row * kChunks + ch] = vreg[j];
+                }
+            }
+        }
+    }
+}
+
+static int cuda_fail2(cudaError_t e, const char* what) {
+    return fail(TANGRAM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+}  // namespace tangram
+
+using namespace tangram;
+
+extern "C" size_t tangram_compact_workspace_bytes(int32_t R, int32_t H) {
+    if (R < 1 || H < 1) return 0;
+    return (compact_ws_words((int64_t)R * H) * 4 + 255) / 256 * 256;
+}
+
+extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
+                                    const void* v_dense, int64_t n_max, const int32_t* ctx_len_dev,
+                                    const int32_t* keep_dev, void* kv_pool, int64_t n_pool_pages, int32_t d,
+                                    int32_t* idx_out, int32_t* clamped_dev, void* workspace, size_t workspace_bytes,
+                                    void* stream) {
+    if (!dp || !scores || !k_dense || !v_dense || !ctx_len_dev || !keep_dev || !kv_pool || !idx_out || !workspace)
+        return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: NULL argument");
+    if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: head_dim %d not in {64, 128}", d);
+    if (dp->P != kCPage) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: page size %d (kernels need 16)", dp->P);
+    if (n_max < 1 || n_max > INT32_MAX || n_pool_pages < 1)
+        return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: n_max=%lld n_pool_pages=%lld", (long long)n_max,
+                    (long long)n_pool_pages);
+    if (reinterpret_cast<uintptr_t>(k_dense) % 16 || reinterpret_cast<uintptr_t>(v_dense) % 16 ||
+        reinterpret_cast<uintptr_t>(kv_pool) % 16 || reinterpret_cast<uintptr_t>(workspace) % 16)
+        return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: misaligned pointer");
+    const int64_t n_seq64 = (int64_t)dp->R * dp->H;
+    if (n_seq64 < 1 || n_seq64 > (1 << 24)) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: R*H=%lld", (long long)n_seq64);
+    const int n_seq = (int)n_seq64;
+    const size_t need = tangram_compact_workspace_bytes(dp->R, dp->H);
+    if (workspace_bytes < need)
+        return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "compact_topk: workspace %zu < %zu bytes", workspace_bytes, need);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int32_t* ws = static_cast<int32_t*>(workspace);
+    CompactWs w{ws, ws + 4, ws + 4 + n_seq};
+    const int4* seq_info = reinterpret_cast<const int4*>(dp->seq_info);
+
+    compact_prepare_kernel<<<1, 1024, 0, st>>>(seq_info, ctx_len_dev, keep_dev, n_seq, dp->H, w.counter, w.keep_eff,
+                                               w.tile_indptr, clamped_dev);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
+    topk_select_kernel<<<n_seq, kSelThreads, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail2(e, "top-k select launch");
+
+    static thread_local int grid128 = 0, grid64 = 0;
+    int& grid = d == 128 ? grid128 : grid64;
+    if (grid == 0) {
+        int dev = 0, sms = 0, per_sm = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail2(e, "cudaGetDevice");
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+            return cuda_fail2(e, "cudaDeviceGetAttribute");
+        e = d == 128 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, compact_gather_kernel<128>, kGatherThreads, 0)
+                     : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, compact_gather_kernel<64>, kGatherThreads, 0);
+        if (e != cudaSuccess) return cuda_fail2(e, "occupancy query");
+        grid = sms * (per_sm > 0 ? per_sm : 1);
+    }
+    const uint4* kd = static_cast<const uint4*>(k_dense);
+    const uint4* vd = static_cast<const uint4*>(v_dense);
+    uint4* pool = static_cast<uint4*>(kv_pool);
+    if (d == 128)
+        compact_gather_kernel<128><<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool,
+                                                                    dp->Hp, n_seq, w.counter, w.keep_eff, w.tile_indptr);
+    else
+        compact_gather_kernel<64><<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool,
+                                                                   dp->Hp, n_seq, w.counter, w.keep_eff, w.tile_indptr);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail2(e, "compact gather launch");
+    return TANGRAM_OK;
+}

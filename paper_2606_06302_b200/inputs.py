@@ -170,3 +170,24 @@ def make_q_and_pool(wl: Workload, n_pool_pages: int, device: str = "cpu", *, poi
         pool[p0:p1] = torch.randn((p1 - p0,) + shape[1:], generator=gen, device=device,
                                   dtype=torch.float32).bfloat16()
     return q, pool
+
+
+def make_scores_and_dense_kv(wl: Workload, n_max: int, device: str = "cpu", *, ties: str = "bf16"):
+    """Inputs of the per-head Top-k compaction (NEXT-2): importance scores [R, H, n_max] f32 and the
+    uncompressed cache K, V [R, H, n_max, d] bf16 ~ N(0,1).  Scores are log-normal (attention-mass-like:
+    positive, heavy tail); with ties="bf16" they are rounded to bf16 precision first, as a scoring function
+    running in bf16 would leave them, so equal scores are common; ties="none" keeps full fp32 values.
+    Stands in for the scores of the paper's compression methods, which need model weights."""
+    import torch
+
+    gen = torch.Generator(device=device)
+    gen.manual_seed(wl.seed + 4242)
+    scores = torch.randn(wl.R, wl.H, n_max, generator=gen, device=device, dtype=torch.float32).exp_()
+    if ties == "bf16":
+        scores = scores.bfloat16().float()
+    k = torch.empty(wl.R, wl.H, n_max, wl.d, dtype=torch.bfloat16, device=device)
+    v = torch.empty_like(k)
+    for dst in (k, v):
+        for r in range(wl.R):  # one request at a time: bounded fp32 scratch
+            dst[r] = torch.randn(wl.H, n_max, wl.d, generator=gen, device=device, dtype=torch.float32).bfloat16()
+    return scores, k, v

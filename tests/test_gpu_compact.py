@@ -1,0 +1,183 @@
+"""GPU parity of NEXT-2 (per-head Top-k selection, Eq. 4, and compaction into the ragged pages,
+Eq. 1) against oracle O7.  Index and byte work: bit-exact, including every pool byte the
+compaction must NOT touch."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import tangram_oracle as O
+from paper_2606_06302_b200 import binding as T
+from paper_2606_06302_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+
+def bits(x):
+    return x.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def otables(t):
+    return O.Tables(R=t.R, H=t.H, C=t.C, Hp=t.Hp, P=t.P, perm=t.perm, cluster_of=t.cluster_of, slot_of=t.slot_of,
+                    tbl_indptr=t.tbl_indptr, tbl_pages=t.tbl_pages, n_pages_used=t.n_pages_used)
+
+
+def setup(wl):
+    B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    n_pool = int(math.ceil(1.05 * T.tangram_pages_needed(B, res, wl.C, wl.P))) + 1
+    t, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, I.make_free_pages(wl, n_pool), 0, kv)
+    pl = T.tangram_plan_partitions(t, B, kv, 8, wl.granule, 1, T.MODE_BALANCED)
+    return B, res, kv, t, n_pool, T.tangram_upload(t, pl)
+
+
+def run_and_compare(wl, t, dp, n_pool, keep, scores, kd, vd, n_max):
+    _, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    before = bits(pool).copy()
+    keep_dev = torch.from_numpy(np.ascontiguousarray(keep, dtype=np.int32)).cuda()
+    ctx_dev = torch.from_numpy(wl.ctx_len.astype(np.int32)).cuda()
+    idx_out = torch.full((wl.R, wl.H, n_max), -7, dtype=torch.int32, device="cuda")
+    clamped = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T.tangram_compact_topk(dp, scores, kd, vd, ctx_dev, keep_dev, pool, idx_out=idx_out, clamped=clamped)
+    torch.cuda.synchronize()
+    assert int(clamped.item()) == 0
+    ref_pool, ref_idx = O.compact_topk(before, otables(t), scores.cpu().numpy(), bits(kd), bits(vd), wl.ctx_len, keep)
+    got_idx = idx_out.cpu().numpy()
+    for r in range(wl.R):
+        for h in range(wl.H):
+            k = int(keep[r][h])
+            assert np.array_equal(got_idx[r, h, :k], ref_idx[r][h]), (r, h, k)
+            assert np.all(got_idx[r, h, k:] == -7)                      # nothing written behind the retained set
+    assert np.array_equal(bits(pool), ref_pool)                          # every byte, slack included
+    return pool, ref_pool
+
+
+@pytest.mark.parametrize("seed,R,H,d,C,max_ctx,ties", [(21, 3, 4, 128, 2, 3000, "bf16"), (22, 2, 6, 64, 3, 2500, "none"),
+                                                       (23, 4, 2, 128, 1, 700, "bf16"), (24, 2, 8, 64, 8, 5000, "bf16"),
+                                                       (25, 1, 4, 128, 4, 40, "none")])
+def test_compact_random_shapes_bit_exact(seed, R, H, d, C, max_ctx, ties):
+    wl = I.make_random_workload(seed, R=R, H=H, G=1, d=d, C=C, max_ctx=max_ctx)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    n_max = int(wl.ctx_len.max()) + 3
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda", ties=ties)
+    run_and_compare(wl, t, dp, n_pool, kv, scores, kd, vd, n_max)
+
+
+def test_compact_edge_keeps_and_heavy_ties():
+    """keep in {0, 1, N-1, N, page multiples}; scores with four distinct values only, +-0, +-inf."""
+    wl = I.make_random_workload(31, R=3, H=4, G=1, d=64, C=2, max_ctx=1500)
+    wl.ctx_len[:] = [1500, 1024, 33]
+    wl.mu[:] = 1.0                                     # capacity = the whole context for every head
+    wl.demand = np.array([[0, 1, 1499, 1500], [1024, 16, 17, 512], [33, 32, 31, 2]], dtype=np.int32)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    assert np.array_equal(kv, wl.demand)
+    n_max = 1504
+    g = torch.Generator(device="cuda").manual_seed(5)
+    scores = torch.randint(0, 4, (3, 4, n_max), generator=g, device="cuda").float()
+    scores[0, 2, ::7] = 0.0
+    scores[0, 2, 3::7] = -0.0
+    scores[0, 3, 5] = math.inf
+    scores[1, 3, 11::13] = -math.inf
+    scores[1, 1] = 2.5                                 # all equal: the first 16 tokens win
+    scores[2, 2] = -scores[2, 2]
+    _, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    run_and_compare(wl, t, dp, n_pool, kv, scores, kd, vd, n_max)
+
+
+def test_compact_clamps_to_capacity_and_counts():
+    """:176 -- the reserved budget is a hard capacity bound: a keep beyond min(N_r, pages x P) is clamped and
+    counted (the oracle refuses such a call; with the clamped value the two agree bit for bit)."""
+    wl = I.make_random_workload(41, R=2, H=4, G=1, d=128, C=2, max_ctx=900)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    cap = np.zeros_like(kv)
+    for r in range(wl.R):
+        for h in range(wl.H):
+            row = r * t.C + int(t.cluster_of[h])
+            cap[r, h] = min(int(wl.ctx_len[r]), int(t.tbl_indptr[row + 1] - t.tbl_indptr[row]) * t.P)
+    want = kv.copy()
+    want[0, 1] = cap[0, 1] + 5
+    want[1, 2] = 10 ** 9
+    want[1, 0] = -3
+    with pytest.raises(ValueError):
+        O.compact_topk(np.zeros((n_pool, t.Hp, 2, t.P, wl.d), np.uint16), otables(t), scores.cpu().numpy(), bits(kd),
+                       bits(vd), wl.ctx_len, np.maximum(want, 0))
+    _, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    before = bits(pool).copy()
+    clamped = torch.zeros(1, dtype=torch.int32, device="cuda")
+    idx = T.tangram_compact_topk(dp, scores, kd, vd, torch.from_numpy(wl.ctx_len).cuda(),
+                                 torch.from_numpy(want.astype(np.int32)).cuda(), pool, clamped=clamped)
+    torch.cuda.synchronize()
+    assert int(clamped.item()) == 3
+    eff = np.clip(want, 0, cap)
+    ref_pool, ref_idx = O.compact_topk(before, otables(t), scores.cpu().numpy(), bits(kd), bits(vd), wl.ctx_len, eff)
+    assert np.array_equal(bits(pool), ref_pool)
+    assert np.array_equal(idx.cpu().numpy()[1, 2, :eff[1, 2]], ref_idx[1][2])
+
+
+def test_compact_then_decode_attention_matches_oracle_pipeline():
+    """The step before the path feeding the path: compaction (CUDA) -> decode attention (CUDA) against
+    oracle compaction -> oracle attention."""
+    wl = I.make_workload("8b", R=3, ctx_div=8)
+    B, res, kv, t, n_pool = setup(wl)[:5]
+    W = T.tangram_query_max_ctas(0, wl.d, wl.G)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, T.DEFAULT_DYN_PERMILLE,
+                                   T.DEFAULT_DYN_ROUNDS)
+    dp = T.tangram_upload(t, pl)
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    pool, ref_pool = run_and_compare(wl, t, dp, n_pool, kv, scores, kd, vd, n_max)
+    q, _ = I.make_q_and_pool(wl, 1, "cuda")
+    out, lse = T.tangram_decode_attention(dp, q, pool)
+    torch.cuda.synchronize()
+    ref_out, ref_lse, _ = O.attention(q.cpu(), torch.from_numpy(ref_pool.view(np.int16)).view(torch.bfloat16),
+                                      otables(t), kv, wl.Hq, wl.d)
+    got = out.float().cpu().numpy().astype(np.float64)
+    assert np.abs(got - ref_out).max() <= 2e-2
+    assert np.linalg.norm(got - ref_out) / np.linalg.norm(ref_out) <= 5e-3
+    assert np.abs(lse.cpu().numpy() - ref_lse).max() <= 1e-3
+
+
+def test_compact_full_size_sampled_and_properties():
+    """8b at BASELINE size (bench.py's configuration): sampled (request, head) index sets against the oracle;
+    for every head the properties that hold at any size -- ascending unique indices below N_r, every kept
+    score >= every dropped score, ties resolved towards the lower index, pool rows = dense rows at I."""
+    wl = I.make_workload("8b")
+    B, res, kv, t, n_pool, dp = setup(wl)
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    pool = torch.zeros(n_pool, t.Hp, 2, t.P, wl.d, dtype=torch.bfloat16, device="cuda")
+    idx = T.tangram_compact_topk(dp, scores, kd, vd, torch.from_numpy(wl.ctx_len).cuda(),
+                                 torch.from_numpy(kv.astype(np.int32)).cuda(), pool)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(9)
+    sc = scores.cpu().numpy()
+    ix = idx.cpu().numpy()
+    sample = {(int(rng.integers(wl.R)), int(rng.integers(wl.H))) for _ in range(6)}
+    for r in range(wl.R):
+        N = int(wl.ctx_len[r])
+        for h in range(wl.H):
+            k = int(kv[r, h])
+            I_ = ix[r, h, :k].astype(np.int64)
+            assert np.all(np.diff(I_) > 0) and (k == 0 or (I_[0] >= 0 and I_[-1] < N))
+            keep_mask = np.zeros(N, bool)
+            keep_mask[I_] = True
+            s = sc[r, h, :N]
+            if 0 < k < N:
+                thr = s[keep_mask].min()
+                assert thr >= s[~keep_mask].max()
+                tie = np.flatnonzero(s == thr)
+                kept_tie = keep_mask[tie]
+                assert np.all(kept_tie[:kept_tie.sum()])               # the kept ties are the lowest indices
+            if (r, h) in sample:
+                assert np.array_equal(I_, O.topk_indices(s, k))
+            # pool rows = dense rows at I (Eq. 1), checked on the device
+            row = r * t.C + int(t.cluster_of[h])
+            pages = torch.from_numpy(t.tbl_pages[int(t.tbl_indptr[row]):int(t.tbl_indptr[row]) + (k + t.P - 1) // t.P]
+                                     .astype(np.int64)).cuda()
+            sl = int(t.slot_of[h])
+            got_k = pool[pages, sl, 0].reshape(-1, wl.d)[:k]
+            got_v = pool[pages, sl, 1].reshape(-1, wl.d)[:k]
+            It = torch.from_numpy(I_).cuda()
+            assert torch.equal(got_k, kd[r, h, It]) and torch.equal(got_v, vd[r, h, It])
