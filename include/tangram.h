@@ -267,7 +267,7 @@ int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const vo
  *   dp            from tangram_upload (uses the tables only)
  *   scores        device [R][H][n_max] f32   importance of every token (entries >= ctx_len[r] are ignored)
  *   k_dense, v_dense  device [R][H][n_max][d] bf16, 16-byte aligned: the uncompressed cache
- *   ctx_len_dev   device [R] i32, 1 <= ctx_len[r] <= n_max
+ *   ctx_len_dev   device [R] i32, 1 <= ctx_len[r] <= n_max <= 2^30
  *   keep_dev      device [R][H] i32  tokens to retain (= kv_len of a1).  A value outside
  *                 [0, min(ctx_len[r], pages(r, cluster) x P)] is clamped into it and the head is counted
  *   kv_pool       device [n_pool_pages][Hp][2][P][d] bf16 (written)

@@ -5,12 +5,13 @@
 //   1. compact_prepare_kernel   one CTA: clamps keep[r][h] to [0, min(N_r, table capacity)] (the reserved
 //      budget is a hard capacity bound, :176), counts the clamped heads, and scans ceil(keep / P) into a
 //      tile index (tile = the P token slots of one (page, head)); zeroes the gather kernel's chunk counter.
-//   2. topk_select_kernel       one 1024-thread CTA per (request, KV head): radix select (4 passes of 8 bits,
-//      per-warp histograms) over a monotone integer image of the fp32 score finds the threshold key T
-//      and how many of the entries equal to T are kept (the lowest token indices first, reading A30); an
-//      ordered pass then writes the retained token indices in ascending order: the entry at token i goes to
-//      position (#greater before i) + min(#equal before i, need).  Integer work on fp32 bit patterns: the
-//      result is the unique Top-k under the tie rule, bit-exact against the sort-based oracle.
+//   2. topk_select_kernel       one CTA (512 or 1024 threads, by row length) per (request, KV head): radix select (digits of 11, 11
+//      and 10 bits, shared-memory atomic histograms, 16-byte loads) over a monotone integer image of the
+//      fp32 score finds the threshold key T and how many of the entries equal to T are kept (the lowest
+//      token indices first, reading A30).  An ordered pass then writes the retained token indices in ascending order: the entry at token i goes
+//      to position (#greater before i) + min(#equal before i, need); every warp owns a contiguous segment,
+//      so that pass needs one block barrier in total.  Integer work on fp32 bit patterns: the result is the
+//      unique Top-k under the tie rule, bit-exact against the sort-based oracle.
 //   3. compact_gather_kernel    persistent grid, warps claim chunks of tiles from a global counter (the same
 //      run-time balancing as the decode kernel's dynamic tail: per-SM bandwidth differs on B200).  A warp
 //      moves one tile: up to P K rows and P V rows of d bf16 each, gathered with 16-byte loads (16 in
@@ -27,8 +28,8 @@
 namespace tangram {
 
 constexpr int kCPage = 16;           // tokens per page (the kernels are specialised for P = 16)
-constexpr int kSelThreads = 1024;
-constexpr int kSelWarps = kSelThreads / 32;
+constexpr int kSelBins = 2048;        // 11-bit digits
+constexpr int kSelLongRow = 49152;    // rows longer than this get 1024-thread CTAs, shorter ones 512 (two per SM)
 constexpr int kGatherThreads = 256;
 constexpr int kGatherChunk = 8;      // tiles claimed at once
 
@@ -44,9 +45,8 @@ static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { retur
 // fp32 score -> uint32 key with the same order (larger score = larger key); -0.0 and +0.0 compare equal
 // as they do as fp32 values.
 __device__ __forceinline__ uint32_t score_key(float x) {
-    uint32_t u = __float_as_uint(x);
-    if ((u << 1) == 0u) u = 0u;
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    const uint32_t u = __float_as_uint(x + 0.0f);  // -0 + 0 = +0 (round to nearest); every other value is unchanged
+    return u ^ (static_cast<uint32_t>(static_cast<int32_t>(u) >> 31) | 0x80000000u);
 }
 
 __global__ void __launch_bounds__(1024)
@@ -93,13 +93,40 @@ compact_prepare_kernel(const int4* __restrict__ seq_info, const int32_t* __restr
     }
 }
 
-__global__ void __launch_bounds__(kSelThreads)
+// Calls fn(key) for the aligned 16-byte groups [v0, v1) of a score row, in no particular order, U loads in
+// flight per thread.
+template <int NT, int U, typename F>
+__device__ __forceinline__ void for_each_key(const float4* __restrict__ sv, int v0, int v1, int tid, F&& fn) {
+    int i = v0 + tid;
+    for (; i + (U - 1) * NT < v1; i += U * NT) {
+        float4 x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) x[u] = __ldg(sv + i + u * NT);
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            fn(score_key(x[u].x)), fn(score_key(x[u].y)), fn(score_key(x[u].z)), fn(score_key(x[u].w));
+        }
+    }
+    for (; i < v1; i += NT) {
+        const float4 x = __ldg(sv + i);
+        fn(score_key(x.x)), fn(score_key(x.y)), fn(score_key(x.z)), fn(score_key(x.w));
+    }
+}
+
+// One CTA of NT threads per (request, KV head).  (A thread-block cluster per row with the histograms
+// exchanged through distributed shared memory was measured too: the remote loads and cluster barriers cost
+// more than the extra SMs bring -- 8b 40 -> 46 us with 2 CTAs per row, 220 us with 8.)
+template <int NT>
+__global__ void __launch_bounds__(NT, 1024 / NT)
 topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len,
                    const int32_t* __restrict__ keep_eff, int H, int32_t* __restrict__ idx_out) {
-    __shared__ uint32_t s_hist[kSelWarps][256];
-    __shared__ uint32_t s_total[256];
+    constexpr int kSelWarps = NT / 32;
+    constexpr int kSelBpt = kSelBins / NT;  // adjacent bins a thread owns in the scan
+    constexpr int kU = NT == 1024 ? 4 : 8;  // 16-byte loads in flight per thread (register budget: 64 / 32)
+    __shared__ uint32_t s_hist[kSelBins];
+    __shared__ uint32_t s_wsum[kSelWarps];
     __shared__ uint32_t s_prefix, s_krem;
-    __shared__ uint32_t s_wgt[kSelWarps], s_weq[kSelWarps];
+    __shared__ uint32_t s_cnt[2][kSelWarps];  // (greater, equal) counts of the warps' segments
     const int seq = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = ctx_len[seq / H];
     const int k = keep_eff[seq];
@@ -107,43 +134,48 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
     const float* s = scores + static_cast<size_t>(seq) * n_max;
     int32_t* idx = idx_out + static_cast<size_t>(seq) * n_max;
     if (k >= N) {  // everything is retained
-        for (int i = tid; i < N; i += kSelThreads) idx[i] = i;
+        for (int i = tid; i < N; i += NT) idx[i] = i;
         return;
     }
-    // ---- radix select of the k-th largest key
+    // The row is <= 3 head entries, nvec aligned float4 groups, <= 3 tail entries.
+    const int head = min(N, static_cast<int>((4u - (static_cast<uint32_t>(reinterpret_cast<uintptr_t>(s)) >> 2)) & 3u));
+    const int nvec = (N - head) >> 2;
+    const int tail0 = head + 4 * nvec;
+    const float4* sv = reinterpret_cast<const float4*>(s + head);
+
+    // ---- radix select of the k-th largest key: digits of 11, 11 and 10 bits from the top
     uint32_t prefix = 0, mask = 0, krem = static_cast<uint32_t>(k);
-    for (int pass = 0; pass < 4; ++pass) {
-        const int shift = 24 - 8 * pass;
-        for (int b = tid; b < kSelWarps * 256; b += kSelThreads) (&s_hist[0][0])[b] = 0u;
+#pragma unroll 1
+    for (int pass = 0; pass < 3; ++pass) {
+        const int shift = pass == 0 ? 21 : (pass == 1 ? 10 : 0);
+        const uint32_t dmask = pass == 2 ? 1023u : 2047u;
+        for (int b = tid; b < kSelBins; b += NT) s_hist[b] = 0u;
         __syncthreads();
-        for (int i = tid; i < N; i += kSelThreads) {
-            const uint32_t key = score_key(__ldg(s + i));
-            if ((key & mask) == prefix) atomicAdd(&s_hist[warp][(key >> shift) & 255u], 1u);
-        }
+        auto add = [&](uint32_t key) {
+            if ((key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & dmask], 1u);
+        };
+        if (tid < head) add(score_key(__ldg(s + tid)));
+        if (tid < N - tail0) add(score_key(__ldg(s + tail0 + tid)));
+        for_each_key<NT, kU>(sv, 0, nvec, tid, add);
         __syncthreads();
-        if (tid < 256) {
-            uint32_t t = 0;
-#pragma unroll 8
-            for (int w = 0; w < kSelWarps; ++w) t += s_hist[w][tid];
-            s_total[tid] = t;
-        }
-        __syncthreads();
-        if (warp == 0) {
-            // lane owns bins [8 lane, 8 lane + 8); `above` = entries in the bins of higher lanes
-            uint32_t c[8], mine = 0;
+        {   // thread owns bins kSelBpt tid ..; `gt` = entries in higher bins (block-wide suffix sum)
+            uint32_t c[kSelBpt], mine = 0;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) c[j] = s_total[8 * lane + j], mine += c[j];
-            uint32_t incl = mine;  // inclusive suffix sum over lanes
+            for (int j = 0; j < kSelBpt; ++j) c[j] = s_hist[kSelBpt * tid + j], mine += c[j];
+            uint32_t incl = mine;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const uint32_t v = __shfl_down_sync(0xffffffffu, incl, o);
                 if (lane + o < 32) incl += v;
             }
+            if (lane == 0) s_wsum[warp] = incl;
+            __syncthreads();
             uint32_t gt = incl - mine;
+            for (int w = warp + 1; w < kSelWarps; ++w) gt += s_wsum[w];
 #pragma unroll
-            for (int j = 7; j >= 0; --j) {
-                if (gt < krem && krem <= gt + c[j]) {  // exactly one (lane, j) satisfies this
-                    s_prefix = prefix | (static_cast<uint32_t>(8 * lane + j) << shift);
+            for (int j = kSelBpt - 1; j >= 0; --j) {
+                if (gt < krem && krem <= gt + c[j]) {  // exactly one bin of the row satisfies this
+                    s_prefix = prefix | (static_cast<uint32_t>(kSelBpt * tid + j) << shift);
                     s_krem = krem - gt;
                 }
                 gt += c[j];
@@ -151,39 +183,103 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
         }
         __syncthreads();
         prefix = s_prefix, krem = s_krem;
-        mask |= 255u << shift;
+        mask |= dmask << shift;
     }
     const uint32_t T = prefix, need = krem;  // keep every key > T and the first `need` entries with key == T
-    // ---- ordered pass: position of token i = #greater before i + min(#equal before i, need)
-    uint32_t run_gt = 0, run_eq = 0;
-    for (int base = 0; base < N; base += kSelThreads) {
-        const int i = base + tid;
-        uint32_t key = 0;
-        bool gt = false, eq = false;
-        if (i < N) {
-            key = score_key(__ldg(s + i));
-            gt = key > T, eq = key == T;
+
+    // ---- ordered pass: position of token i = #greater before i + min(#equal before i, need).
+    // Warp w owns the contiguous groups [v0, v1): it counts them (16-byte loads, 8 in flight), the counts of
+    // all warps are exchanged (the only block barrier of this part), then it walks its groups again 32 at a
+    // time: a lane holds four consecutive tokens and a packed (greater, equal) warp scan gives their positions.
+    const int wseg = ((nvec + kSelWarps - 1) / kSelWarps + 31) & ~31;
+    const int v0 = min(nvec, warp * wseg), v1 = min(nvec, v0 + wseg);
+    auto cnt4 = [&](const float4 x, uint32_t& g, uint32_t& e) {
+        const uint32_t a = score_key(x.x), b = score_key(x.y), c = score_key(x.z), d = score_key(x.w);
+        g += (a > T) + (b > T) + (c > T) + (d > T);
+        e += (a == T) + (b == T) + (c == T) + (d == T);
+    };
+    {
+        uint32_t cg_ = 0, ce_ = 0;
+        int v = v0 + lane;
+        for (; v + 7 * 32 < v1; v += 8 * 32) {
+            float4 x[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) x[u] = __ldg(sv + v + u * 32);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) cnt4(x[u], cg_, ce_);
         }
+        for (; v < v1; v += 32) cnt4(__ldg(sv + v), cg_, ce_);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cg_ += __shfl_xor_sync(0xffffffffu, cg_, o), ce_ += __shfl_xor_sync(0xffffffffu, ce_, o);
+        if (lane == 0) s_cnt[0][warp] = cg_, s_cnt[1][warp] = ce_;
+    }
+    __syncthreads();
+    const uint32_t lt = (1u << lane) - 1u;
+    // the head entries come first, the tail entries last; both are placed by warp 0 (lane j holds entry j)
+    uint32_t run_gt = 0, run_eq = 0;
+    {
+        const bool in_head = lane < head;
+        const uint32_t key = in_head ? score_key(__ldg(s + lane)) : 0u;
+        const bool gt = in_head && key > T, eq = in_head && key == T;
         const unsigned bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
-        if (lane == 0) s_wgt[warp] = __popc(bg), s_weq[warp] = __popc(be);
-        __syncthreads();
-        // every warp scans the 32 warp counts redundantly
-        uint32_t wg = s_wgt[lane], we = s_weq[lane];
-        uint32_t ig = wg, ie = we;
+        const uint32_t eq_before = __popc(be & lt);
+        if (warp == 0 && (gt || (eq && eq_before < need))) idx[__popc(bg & lt) + min(eq_before, need)] = lane;
+        run_gt = __popc(bg), run_eq = __popc(be);
+    }
+    uint32_t all_gt = run_gt, all_eq = run_eq;
+    {   // lane w reads warp w's counts
+        uint32_t ag_ = lane < kSelWarps ? s_cnt[0][lane] : 0u, ae_ = lane < kSelWarps ? s_cnt[1][lane] : 0u;
+        uint32_t bg_ = lane < warp ? ag_ : 0u, be_ = lane < warp ? ae_ : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            bg_ += __shfl_xor_sync(0xffffffffu, bg_, o), be_ += __shfl_xor_sync(0xffffffffu, be_, o);
+            ag_ += __shfl_xor_sync(0xffffffffu, ag_, o), ae_ += __shfl_xor_sync(0xffffffffu, ae_, o);
+        }
+        run_gt += bg_, run_eq += be_, all_gt += ag_, all_eq += ae_;
+    }
+    if (warp == 0) {
+        const bool in_tail = lane < N - tail0;
+        const uint32_t key = in_tail ? score_key(__ldg(s + tail0 + lane)) : 0u;
+        const bool gt = in_tail && key > T, eq = in_tail && key == T;
+        const unsigned bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
+        const uint32_t eq_before = all_eq + __popc(be & lt);
+        if (gt || (eq && eq_before < need)) idx[all_gt + __popc(bg & lt) + min(eq_before, need)] = tail0 + lane;
+    }
+    auto place4 = [&](const float4 x, int v) {  // group v of the row: tokens head + 4 v .. + 3, lane-major order
+        const uint32_t key[4] = {score_key(x.x), score_key(x.y), score_key(x.z), score_key(x.w)};
+        uint32_t p = 0;
+        if (v < v1) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) p += (key[j] > T) + ((key[j] == T) << 16);
+        }
+        if (!__any_sync(0xffffffffu, p != 0u)) return;  // nothing retained in these 128 tokens
+        uint32_t incl = p;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t vg = __shfl_up_sync(0xffffffffu, ig, o), ve = __shfl_up_sync(0xffffffffu, ie, o);
-            if (lane >= o) ig += vg, ie += ve;
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
         }
-        const uint32_t tot_g = __shfl_sync(0xffffffffu, ig, 31), tot_e = __shfl_sync(0xffffffffu, ie, 31);
-        const uint32_t warp_g = __shfl_sync(0xffffffffu, ig - wg, warp), warp_e = __shfl_sync(0xffffffffu, ie - we, warp);
-        const uint32_t lt = (1u << lane) - 1u;
-        const uint32_t gt_before = run_gt + warp_g + __popc(bg & lt);
-        const uint32_t eq_before = run_eq + warp_e + __popc(be & lt);
-        if (gt || (eq && eq_before < need)) idx[gt_before + min(eq_before, need)] = i;
-        run_gt += tot_g, run_eq += tot_e;
-        __syncthreads();  // s_wgt / s_weq are rewritten by the next chunk
+        const uint32_t tot = __shfl_sync(0xffffffffu, incl, 31);
+        uint32_t g = run_gt + ((incl - p) & 0xffffu), e = run_eq + ((incl - p) >> 16);
+        if (p) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const bool gt = key[j] > T, eq = key[j] == T;
+                if (gt || (eq && e < need)) idx[g + min(e, need)] = head + 4 * v + j;
+                g += gt, e += eq;
+            }
+        }
+        run_gt += tot & 0xffffu, run_eq += tot >> 16;
+    };
+    int v = v0;  // warp-uniform: rows of 32 groups
+    for (; v + 3 * 32 < v1; v += 4 * 32) {
+        float4 x[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) x[u] = v + u * 32 + lane < v1 ? __ldg(sv + v + u * 32 + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) place4(x[u], v + u * 32 + lane);
     }
+    for (; v < v1; v += 32) place4(v + lane < v1 ? __ldg(sv + v + lane) : make_float4(0.f, 0.f, 0.f, 0.f), v + lane);
 }
 
 template <int D>
@@ -270,7 +366,7 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: NULL argument");
     if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: head_dim %d not in {64, 128}", d);
     if (dp->P != kCPage) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: page size %d (kernels need 16)", dp->P);
-    if (n_max < 1 || n_max > INT32_MAX || n_pool_pages < 1)
+    if (n_max < 1 || n_max > (1 << 30) || n_pool_pages < 1)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: n_max=%lld n_pool_pages=%lld", (long long)n_max,
                     (long long)n_pool_pages);
     if (reinterpret_cast<uintptr_t>(k_dense) % 16 || reinterpret_cast<uintptr_t>(v_dense) % 16 ||
@@ -291,10 +387,12 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
                                                w.tile_indptr, clamped_dev);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
-    topk_select_kernel<<<n_seq, kSelThreads, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
+    if (n_max > kSelLongRow)
+        topk_select_kernel<1024><<<n_seq, 1024, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
+    else
+        topk_select_kernel<512><<<n_seq, 512, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "top-k select launch");
-
     static thread_local int grid128 = 0, grid64 = 0;
     int& grid = d == 128 ? grid128 : grid64;
     if (grid == 0) {

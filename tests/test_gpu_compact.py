@@ -54,9 +54,15 @@ def run_and_compare(wl, t, dp, n_pool, keep, scores, kd, vd, n_max):
 
 @pytest.mark.parametrize("seed,R,H,d,C,max_ctx,ties", [(21, 3, 4, 128, 2, 3000, "bf16"), (22, 2, 6, 64, 3, 2500, "none"),
                                                        (23, 4, 2, 128, 1, 700, "bf16"), (24, 2, 8, 64, 8, 5000, "bf16"),
-                                                       (25, 1, 4, 128, 4, 40, "none")])
+                                                       (25, 1, 4, 128, 4, 40, "none"),
+                                                       # rows long enough for clusters of 4 and 8 CTAs
+                                                       (26, 2, 2, 64, 2, 40000, "bf16"), (27, 1, 2, 64, 1, 70000, "bf16")])
 def test_compact_random_shapes_bit_exact(seed, R, H, d, C, max_ctx, ties):
     wl = I.make_random_workload(seed, R=R, H=H, G=1, d=d, C=C, max_ctx=max_ctx)
+    if max_ctx > 10000:
+        wl.ctx_len[0] = max_ctx - 5           # make sure the longest cluster shape is exercised
+        wl.demand = np.minimum(wl.demand, wl.ctx_len[:, None]).astype(np.int32)
+        wl.demand[0] = np.maximum(1, (wl.ctx_len[0] * np.linspace(0.02, 0.9, H))).astype(np.int32)
     B, res, kv, t, n_pool, dp = setup(wl)
     n_max = int(wl.ctx_len.max()) + 3
     scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda", ties=ties)
