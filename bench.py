@@ -366,6 +366,37 @@ def decode_loop(T, I, name, device, layers, steps, torch):
 
 
 # ------------------------------------------------------------------------------------------------
+# NEXT-2: per-head Top-k selection + compaction into the ragged pages (the step that fills the pool)
+# ------------------------------------------------------------------------------------------------
+def compact_topk_summary(T, I, name, device, steps, flush, torch, peak_gbs):
+    """tangram_compact_topk on the workload's shape: scores [R,H,n_max] f32 and the uncompressed cache
+    [R,H,n_max,d] bf16 are resident; one call = prepare + top-k select + gather (three launches).  The
+    gather is the HBM-bound part: 4d bytes read + 4d bytes written per retained token-head."""
+    S = setup_workload(T, I, name, device)
+    wl, kv = S["wl"], S["kv"]
+    dp = T.tangram_upload(S["tables"], S["plan"])
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, device)
+    ctx = torch.as_tensor(wl.ctx_len, device=device)
+    keep = torch.as_tensor(np.ascontiguousarray(kv, dtype=np.int32), device=device)
+    idx = torch.empty(wl.R, wl.H, n_max, dtype=torch.int32, device=device)
+    ws = torch.empty(T.tangram_compact_workspace_bytes(wl.R, wl.H), dtype=torch.uint8, device=device)
+    step = lambda: T.tangram_compact_topk(dp, scores, kd, vd, ctx, keep, S["pool"], idx_out=idx, workspace=ws)
+    ms = time_steps(step, steps, 3, flush, torch)
+    kept = int(kv.sum())
+    gather_bytes = kept * 4 * wl.d * 2 + kept * 4            # rows read + rows written + indices read
+    score_bytes = int(wl.ctx_len.astype(np.int64).sum()) * wl.H * 4
+    us = float(np.median(ms) * 1e3)
+    return {"workload": name, "us": us, "us_min": float(np.min(ms) * 1e3), "launches": 3,
+            "retained_token_heads": kept, "gather_bytes": gather_bytes, "score_bytes_one_pass": score_bytes,
+            "gbs_gather_bytes_over_total_time": gather_bytes / (us * 1e-6) / 1e9,
+            "pct_of_measured_copy": 100 * gather_bytes / (us * 1e-6) / 1e9 / peak_gbs,
+            "note": "whole call (select + gather) timed with CUDA events, L2 flushed; bytes = K/V rows read + "
+                    "written; the select kernel reads the scores five times (first pass from HBM, then L2); "
+                    "kernel shares: profiles/"}
+
+
+# ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
 def spread_of(T, S, torch, reps=5):
@@ -458,6 +489,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the other configs' summary lines")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-compact", action="store_true", help="skip the Top-k compaction (NEXT-2) summary")
     ap.add_argument("--dyn-permille", type=int, default=None, help="dynamic-tail share of the BALANCED plan")
     ap.add_argument("--dyn-rounds", type=int, default=None)
     ap.add_argument("--decode-loop-layers", type=int, default=8,
@@ -566,11 +598,16 @@ def main():
         line["per_config"] = per
         if args.decode_loop_layers > 0:
             line["decode_loop"] = decode_loop(T, I, args.workload, device, args.decode_loop_layers, 30, torch)
+            torch.cuda.empty_cache()
     elif not args.no_cpu_baseline and world == 1:
         from oracle import tangram_oracle as O
         O.build_c()
         S = setup_workload(T, I, args.workload, device)
         line["cpu_baseline"] = cpu_baseline(O, S)
+    if world == 1 and not args.no_compact:
+        S = None
+        torch.cuda.empty_cache()
+        line["compact_topk"] = compact_topk_summary(T, I, args.workload, device, 30, flush, torch, peak_gbs)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
