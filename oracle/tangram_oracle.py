@@ -19,6 +19,10 @@ What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.
      compact_topk         :57) written into the ragged pages (NEXT-2; tie rule = reading A30)
   O6 append_kv            one decode step's new K/V rows written into the ragged pages (NEXT-1;
                           page layout :190, capacity bound :176, reading A29)
+  O8 account_pages        pages / token-head slots a batch occupies under a grouping policy (monolithic,
+                          adjacent, Budget-Aware Clustering; Fig. 7 :168, Fig. 8 :186, Fig. 15 :316-320; NEXT-3)
+  O9 calibrate_budgets    mu, sigma of the recorded per-head implicit retention ratios and Eq. 5 (:156-158;
+                          population sigma = reading A10; NEXT-4)
   O1 attention*           plain softmax(q K~^T / sqrt(d)) V~ through the page tables (Eq. 1 :57)
 
 Pins (every function is pinned; nothing here is "parity unpinned"): tests/test_oracle_pins.py.
@@ -405,6 +409,86 @@ def compact_topk(pool_bits: np.ndarray, t: Tables, scores, k_dense_bits, v_dense
                 pool[page, sl, 0, pos % t.P, :] = k_dense_bits[r, h, tok, :]
                 pool[page, sl, 1, pos % t.P, :] = v_dense_bits[r, h, tok, :]
     return pool, out_idx
+
+
+# --------------------------------------------------------------------------------------------
+# O8  page accounting under a grouping policy (NEXT-3; Fig. 7 :168, :190, :235-242, Fig. 15 :316-320)
+# --------------------------------------------------------------------------------------------
+GROUP_CLUSTERED, GROUP_ADJACENT = 0, 1
+
+
+def account_pages(B, reserved, ctx_len, Hp: int, page_size: int, policy: int) -> dict:
+    """Memory a batch occupies when H_p heads share a page table sized by the group's largest reservation
+    (:190).  policy CLUSTERED groups H_p consecutive heads of the budget-sorted order (:227-233), ADJACENT
+    groups heads in index order ("naively grouping adjacent heads", :192); H_p = H is the monolithic page of
+    one layer (Fig. 7(a)).  Unit = token-head slot (one token of one head, K and V).
+      pages_alloc  = sum_r sum_groups ceil(max_{h in g} reserved[r][h] / P)   (pages of H_p x 2 x P x d elements)
+      slots_alloc  = H_p * P * pages_alloc
+      slots_exact  = sum_r sum_h P * ceil(reserved[r][h] / P)                 (every head its own table)
+      slots_full   = sum_r H * P * ceil(N_r / P)                              (uncompressed cache)
+      slots_used   = sum_r sum_h reserved[r][h]
+      tables       = R * H / H_p                                              (block tables to manage, :244)
+      reclaimed_frac = 1 - slots_alloc / slots_full   ("memory reclaimed, fraction of the full KV cache", Fig. 15)
+      fragmentation  = (slots_alloc - slots_used) / slots_alloc               (allocated slots holding no retained
+                                                                               token; reading A31)"""
+    B = np.asarray(B, dtype=np.float64)
+    res = np.asarray(reserved, dtype=np.int64)
+    R, H = res.shape
+    P = int(page_size)
+    if Hp < 1 or H % Hp != 0 or P < 1:
+        raise ValueError("bad H_p / page size")
+    if policy == GROUP_CLUSTERED:
+        order = sorted(range(H), key=lambda h: (B[h], h))
+    elif policy == GROUP_ADJACENT:
+        order = list(range(H))
+    else:
+        raise ValueError("bad policy")
+    pages = 0
+    exact = 0
+    full = 0
+    used = 0
+    for r in range(R):
+        for g in range(H // Hp):
+            longest = max(int(res[r, order[g * Hp + j]]) for j in range(Hp))
+            pages += -(-longest // P)
+        for h in range(H):
+            exact += P * (-(-int(res[r, h]) // P))
+            used += int(res[r, h])
+        full += H * P * (-(-int(ctx_len[r]) // P))
+    alloc = Hp * P * pages
+    return dict(pages_alloc=pages, slots_alloc=alloc, slots_exact=exact, slots_full=full, slots_used=used,
+                tables=R * (H // Hp), reclaimed_frac=1.0 - float(alloc) / float(full),
+                fragmentation=float(alloc - used) / float(alloc))
+
+
+# --------------------------------------------------------------------------------------------
+# O9  Budget Calibration (NEXT-4; :156-158, Eq. 5)
+# --------------------------------------------------------------------------------------------
+def calibrate_budgets(ratios, alpha: float):
+    """ratios[i][h] = implicit retention ratio head h received on calibration sample i (:156).  Returns
+    (mu, sigma, B): mu_h = (sum_i x_ih) / n and sigma_h = sqrt((sum_i (x_ih - mu_h)^2) / n) -- the
+    population standard deviation (reading A10: the paper says "standard deviation" only) -- both summed in
+    sample order in fp64, and B_h = min(1, mu_h + alpha * sigma_h) (Eq. 5)."""
+    x = np.asarray(ratios, dtype=np.float64)
+    n, H = x.shape
+    if n < 1:
+        raise ValueError("no samples")
+    mu = np.zeros(H)
+    sigma = np.zeros(H)
+    B = np.zeros(H)
+    for h in range(H):
+        acc = 0.0
+        for i in range(n):
+            acc = acc + float(x[i, h])
+        m = acc / float(n)
+        acc2 = 0.0
+        for i in range(n):
+            dlt = float(x[i, h]) - m
+            acc2 = acc2 + dlt * dlt
+        sd = math.sqrt(acc2 / float(n))
+        mu[h], sigma[h] = m, sd
+        B[h] = min(1.0, m + alpha * sd)
+    return mu, sigma, B
 
 
 # --------------------------------------------------------------------------------------------

@@ -568,3 +568,82 @@ def test_compact_topk_round_trip_against_dense_attention():
             assert np.allclose(out[r, j], ref.numpy(), rtol=0, atol=1e-12)
     with pytest.raises(ValueError):
         O.compact_topk(b0, t, scores, kb, vb, ctx, keep + 100)
+
+
+# ---------------------------------------------------------------------------- O8 page accounting (NEXT-3)
+def test_account_pages_hand_example_fig7():
+    """Fig. 7 (:168) in numbers: six heads, one request of 64 tokens, P = 16, two long heads (64) among short
+    ones (16).  Monolithic: every page blocked by a long head.  Adjacent groups of 3: each group holds a long
+    head, nothing freed.  Clustered: the short heads share a group and free their pages."""
+    res = np.array([[16, 64, 16, 16, 64, 16]])
+    B = res[0] / 64.0
+    ctx = [64]
+    mono = O.account_pages(B, res, ctx, 6, 16, O.GROUP_ADJACENT)
+    adj = O.account_pages(B, res, ctx, 3, 16, O.GROUP_ADJACENT)
+    clu = O.account_pages(B, res, ctx, 3, 16, O.GROUP_CLUSTERED)
+    one = O.account_pages(B, res, ctx, 1, 16, O.GROUP_CLUSTERED)
+    assert mono["slots_alloc"] == 6 * 64 and mono["pages_alloc"] == 4 and mono["reclaimed_frac"] == 0.0
+    assert adj["slots_alloc"] == 384 and adj["pages_alloc"] == 8 and adj["tables"] == 2
+    assert clu["slots_alloc"] == 3 * 16 + 3 * 64 == 240 and clu["reclaimed_frac"] == 1.0 - 240 / 384
+    assert one["slots_alloc"] == one["slots_exact"] == one["slots_used"] == 4 * 16 + 2 * 64 and one["fragmentation"] == 0.0
+    assert clu["fragmentation"] == (240 - 192) / 240 and one["tables"] == 6
+
+
+def test_account_pages_invariants_and_optimality():
+    rng = np.random.default_rng(8)
+    for _ in range(30):
+        H = int(rng.choice([4, 6, 8]))
+        R = int(rng.integers(1, 4))
+        P = int(rng.choice([1, 16]))
+        B = rng.uniform(0.05, 1.0, size=H)
+        ctx = rng.integers(50, 400, size=R)
+        res = np.ceil(B[None, :] * ctx[:, None]).astype(np.int64)
+        for Hp in [d for d in (1, 2, 4, 8, H) if H % d == 0]:
+            clu = O.account_pages(B, res, ctx, Hp, P, O.GROUP_CLUSTERED)
+            adj = O.account_pages(B, res, ctx, Hp, P, O.GROUP_ADJACENT)
+            assert clu["slots_exact"] == adj["slots_exact"] <= clu["slots_alloc"] <= adj["slots_alloc"] <= clu["slots_full"]
+            assert clu["slots_alloc"] == Hp * P * clu["pages_alloc"] and clu["tables"] == R * H // Hp
+            if Hp == 1:
+                assert clu["slots_alloc"] == clu["slots_exact"]
+            if Hp == H:                                   # one group: the policy cannot matter
+                assert clu["slots_alloc"] == adj["slots_alloc"] == H * P * sum(-(-int(m) // P) for m in res.max(1))
+            # the tables the pinned builder O3 makes use exactly this many pages
+            t, _ = O.build_ragged_tables(B, res.astype(np.int32), H // Hp, P, np.arange(10 ** 5, dtype=np.int32))
+            assert t.n_pages_used == clu["pages_alloc"]
+            if H <= 6 and Hp in (2, 3) and P == 1 and R == 1:   # brute force over all equal-size groupings
+                best = min(sum(max(res[0, list(g)]) for g in part) * Hp for part in _equal_partitions(list(range(H)), Hp))
+                assert clu["slots_alloc"] == best
+    same = O.account_pages(np.full(4, 0.5), np.full((2, 4), 100), [200, 200], 2, 16, O.GROUP_CLUSTERED)
+    assert same == O.account_pages(np.full(4, 0.5), np.full((2, 4), 100), [200, 200], 2, 16, O.GROUP_ADJACENT)
+
+
+def _equal_partitions(items, size):
+    if not items:
+        yield []
+        return
+    first, rest = items[0], items[1:]
+    import itertools
+    for mates in itertools.combinations(rest, size - 1):
+        left = [x for x in rest if x not in mates]
+        for tail in _equal_partitions(left, size):
+            yield [(first,) + mates] + tail
+
+
+# ---------------------------------------------------------------------------- O9 calibration (NEXT-4)
+def test_calibrate_budgets_closed_forms_and_library():
+    mu, sd, B = O.calibrate_budgets([[0.25, 0.5], [0.75, 0.5]], 1.0)
+    assert mu.tolist() == [0.5, 0.5] and sd.tolist() == [0.25, 0.0]        # population sigma (ddof = 0), not 0.3536
+    assert B.tolist() == [0.75, 0.5]
+    assert O.calibrate_budgets([[0.25], [0.75]], 2.0)[2].tolist() == [1.0]  # min(1, .) of Eq. 5
+    assert O.calibrate_budgets([[0.375]], 2.0)[2].tolist() == [0.375]       # one sample: sigma = 0
+    rng = np.random.default_rng(12)
+    x = rng.uniform(0.01, 1.0, size=(50, 8))                                # 50 samples (:262)
+    mu, sd, B = O.calibrate_budgets(x, 2.0)
+    assert np.allclose(mu, x.mean(0), rtol=1e-14, atol=0) and np.allclose(sd, x.std(0, ddof=0), rtol=1e-12, atol=0)
+    assert np.array_equal(B, np.minimum(1.0, mu + 2.0 * sd))
+    # feeds Eq. 5 of O2 unchanged: reserve_budgets(mu, sigma, alpha) reproduces B
+    B2, _, _ = O.reserve_budgets(mu, sd, 2.0, np.array([1000], dtype=np.int32))
+    assert np.array_equal(B, B2)
+    # Cantelli: at most 1/(1 + alpha^2) of the samples exceed mu + alpha * sigma (holds for the empirical
+    # distribution with the population sigma)
+    assert ((x > (mu + 2.0 * sd)[None, :]).mean(0) <= 0.2 + 1e-12).all()
