@@ -397,6 +397,25 @@ def compact_topk_summary(T, I, name, device, steps, flush, torch, peak_gbs):
 
 
 # ------------------------------------------------------------------------------------------------
+# NEXT-3: memory reclaimed vs heads per page, with and without Budget-Aware Clustering (host only)
+# ------------------------------------------------------------------------------------------------
+def page_accounting_summary(T, I, name):
+    """Fig. 12 / Fig. 15 quantities on the synthetic profile of the workload: fraction of the full KV cache
+    reclaimed when H_p heads share a page table, heads grouped by budget (clustered) or by index (adjacent)."""
+    wl = I.make_workload(name)
+    B, res, _ = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    out = {"workload": name, "unit": "fraction of the full (uncompressed, paged) KV cache of the layer"}
+    for Hp in [d for d in (1, 2, 4, 8) if wl.H % d == 0]:
+        clu = T.tangram_account_pages(B, res, wl.ctx_len, Hp, wl.P, T.GROUP_CLUSTERED)
+        adj = T.tangram_account_pages(B, res, wl.ctx_len, Hp, wl.P, T.GROUP_ADJACENT)
+        out[f"Hp{Hp}"] = {"reclaimed_clustered": clu["reclaimed_frac"], "reclaimed_adjacent": adj["reclaimed_frac"],
+                          "extra_from_clustering": clu["reclaimed_frac"] - adj["reclaimed_frac"],
+                          "fragmentation_clustered": clu["fragmentation"], "tables": clu["tables"],
+                          "pages": clu["pages_alloc"]}
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
 def spread_of(T, S, torch, reps=5):
@@ -604,6 +623,8 @@ def main():
         O.build_c()
         S = setup_workload(T, I, args.workload, device)
         line["cpu_baseline"] = cpu_baseline(O, S)
+    if world == 1:
+        line["page_accounting"] = page_accounting_summary(T, I, args.workload)
     if world == 1 and not args.no_compact:
         S = None
         torch.cuda.empty_cache()

@@ -282,6 +282,46 @@ int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, con
                          void* kv_pool, int64_t n_pool_pages, int32_t d, int32_t* idx_out, int32_t* clamped_dev,
                          void* workspace, size_t workspace_bytes, void* stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-3  Page accounting under a grouping policy (host, pure).  PAPER.md:168 (Fig. 7: a page is freed only when
+ * all heads sharing it are evicted; monolithic / ragged / clustered), :190 (a group's page table is sized by its
+ * largest budget), :192 ("naively grouping adjacent heads mixes dissimilar budgets"), :235-242 (H_p trade-off),
+ * :244 (block-table cost O(N_req x H / H_p)), :316-320 (Fig. 15: memory reclaimed as a fraction of the full KV cache).
+ *
+ *   B         host [H] f64   calibrated budgets (only their order is used: TANGRAM_GROUP_CLUSTERED sorts by them
+ *                            exactly as tangram_build_ragged_tables does)
+ *   reserved  host [R][H] i32 (from a1)      ctx_len  host [R] i32
+ *   heads_per_page  H_p, must divide H (H_p = H: the monolithic page of one layer)
+ *   policy    TANGRAM_GROUP_CLUSTERED (H_p consecutive heads of the budget-sorted order, :227-233) or
+ *             TANGRAM_GROUP_ADJACENT (H_p consecutive heads in index order)
+ *   out       unit = token-head slot (one token of one head, K and V):
+ *               pages_alloc = sum_r sum_groups ceil(max_{h in g} reserved[r][h] / P)
+ *               slots_alloc = H_p * P * pages_alloc;   slots_exact = sum_r sum_h P * ceil(reserved[r][h] / P)
+ *               slots_full  = sum_r H * P * ceil(N_r / P);   slots_used = sum reserved;   tables = R * H / H_p
+ *               reclaimed_frac = 1 - slots_alloc / slots_full;  fragmentation = (slots_alloc - slots_used) / slots_alloc
+ * Errors: INVALID_ARG (NULL, R/H < 1, H % H_p != 0, page_size < 1, reserved < 0, ctx_len < 1, unknown policy). */
+#define TANGRAM_GROUP_CLUSTERED 0
+#define TANGRAM_GROUP_ADJACENT 1
+typedef struct tangram_page_account {
+    int64_t pages_alloc, slots_alloc, slots_exact, slots_full, slots_used, tables;
+    double reclaimed_frac, fragmentation;
+} tangram_page_account;
+int tangram_account_pages(const double* B, const int32_t* reserved, const int32_t* ctx_len, int32_t R, int32_t H,
+                          int32_t heads_per_page, int32_t page_size, int32_t policy, tangram_page_account* out);
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-4  Budget Calibration (host, pure).  PAPER.md:156-158: on a small set of sample contexts the implicit
+ * per-head retention ratio of the global top-k selection is recorded and summarised by its mean and standard
+ * deviation; Eq. 5 fixes B = min(1, mu + alpha sigma) (50 samples, alpha = 2 in the paper, :262).
+ *
+ *   ratios    host [n_samples][H] f64   ratio head h received on sample i
+ *   mu_out, sigma_out, B_out   host [H] f64:  mu = (sum_i x_i) / n,  sigma = sqrt((sum_i (x_i - mu)^2) / n) -- the
+ *             POPULATION standard deviation (the paper does not say which) -- sums in sample order, fp64, no FMA;
+ *             B as in tangram_reserve_budgets (B_out may be NULL)
+ * Errors: INVALID_ARG (NULL, n_samples < 1, H < 1, a ratio that is not finite). */
+int tangram_calibrate_budgets(const double* ratios, int32_t n_samples, int32_t H, double alpha, double* mu_out,
+                              double* sigma_out, double* B_out);
+
 #ifdef __cplusplus
 }
 #endif

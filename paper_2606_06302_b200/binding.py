@@ -22,6 +22,7 @@ FILL_GROUP = 1
 MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
 # dynamic tail of the BALANCED plan used by bench.py / smoke (tuned on B200)
 DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 500, 6
+GROUP_CLUSTERED, GROUP_ADJACENT = 0, 1
 MODE_NAMES = {MODE_BALANCED: "balanced", MODE_SPLITMAP: "splitmap", MODE_STATIC_EVEN: "static_even"}
 
 if not os.path.exists(LIB_PATH):
@@ -67,13 +68,15 @@ _lib.tangram_compact_workspace_bytes.restype = C.c_size_t
 _lib.tangram_compact_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
 for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
-              "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk"):
+              "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk",
+              "tangram_account_pages", "tangram_calibrate_budgets"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
            "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
-           "tangram_compact_workspace_bytes", "tangram_compact_topk")
+           "tangram_compact_workspace_bytes", "tangram_compact_topk", "tangram_account_pages",
+           "tangram_calibrate_budgets")
 
 
 def _check(rc: int):
@@ -325,3 +328,29 @@ def tangram_compact_topk(dp: DevicePlan, scores, k_dense, v_dense, ctx_len, keep
                                      C.c_int64(kv_pool.shape[0]), C.c_int32(d), C.c_void_p(idx_out.data_ptr()), cl,
                                      C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), sp))
     return idx_out
+
+
+class _PageAccount(C.Structure):
+    _fields_ = [("pages_alloc", C.c_int64), ("slots_alloc", C.c_int64), ("slots_exact", C.c_int64),
+                ("slots_full", C.c_int64), ("slots_used", C.c_int64), ("tables", C.c_int64),
+                ("reclaimed_frac", C.c_double), ("fragmentation", C.c_double)]
+
+
+def tangram_account_pages(B, reserved, ctx_len, heads_per_page: int, page_size: int, policy: int) -> dict:
+    """NEXT-3: pages / token-head slots the batch occupies when heads_per_page heads share a page table."""
+    B, reserved, ctx = _np(B, np.float64), _np(reserved, np.int32), _np(ctx_len, np.int32)
+    R, H = reserved.shape
+    acc = _PageAccount()
+    _check(_lib.tangram_account_pages(_ptr(B), _ptr(reserved), _ptr(ctx), C.c_int32(R), C.c_int32(H),
+                                      C.c_int32(heads_per_page), C.c_int32(page_size), C.c_int32(policy), C.byref(acc)))
+    return {k: getattr(acc, k) for k, _ in _PageAccount._fields_}
+
+
+def tangram_calibrate_budgets(ratios, alpha: float):
+    """NEXT-4: (mu, sigma, B) from the recorded per-head implicit retention ratios [n_samples, H] (Eq. 5)."""
+    x = _np(ratios, np.float64)
+    n, H = x.shape
+    mu, sigma, B = np.zeros(H), np.zeros(H), np.zeros(H)
+    _check(_lib.tangram_calibrate_budgets(_ptr(x), C.c_int32(n), C.c_int32(H), C.c_double(alpha), _ptr(mu), _ptr(sigma),
+                                          _ptr(B)))
+    return mu, sigma, B

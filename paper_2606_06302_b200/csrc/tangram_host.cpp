@@ -289,3 +289,69 @@ extern "C" int tangram_plan_partitions(const tangram_tables* t, const double* B,
     }
     return TANGRAM_OK;
 }
+
+// ---- NEXT-3: page accounting under a grouping policy (Fig. 7 :168, :190, Fig. 15 :316-320)
+extern "C" int tangram_account_pages(const double* B, const int32_t* reserved, const int32_t* ctx_len, int32_t R,
+                                     int32_t H, int32_t heads_per_page, int32_t page_size, int32_t policy,
+                                     tangram_page_account* out) {
+    if (!B || !reserved || !ctx_len || !out) return fail(TANGRAM_ERR_INVALID_ARG, "account_pages: NULL argument");
+    const int32_t Hp = heads_per_page, P = page_size;
+    if (R < 1 || H < 1 || Hp < 1 || H % Hp != 0 || P < 1)
+        return fail(TANGRAM_ERR_INVALID_ARG, "account_pages: R=%d H=%d heads_per_page=%d page_size=%d", R, H, Hp, P);
+    if (policy != TANGRAM_GROUP_CLUSTERED && policy != TANGRAM_GROUP_ADJACENT)
+        return fail(TANGRAM_ERR_INVALID_ARG, "account_pages: policy=%d", policy);
+    std::vector<int32_t> order(H);
+    std::iota(order.begin(), order.end(), 0);
+    if (policy == TANGRAM_GROUP_CLUSTERED)  // the same stable sort as the table builder (:227-233)
+        std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return B[a] < B[b]; });
+    int64_t pages = 0, exact = 0, full = 0, used = 0;
+    for (int32_t r = 0; r < R; ++r) {
+        if (ctx_len[r] < 1) return fail(TANGRAM_ERR_INVALID_ARG, "account_pages: ctx_len[%d]=%d < 1", r, ctx_len[r]);
+        const int32_t* row = reserved + (size_t)r * H;
+        for (int32_t h = 0; h < H; ++h) {
+            if (row[h] < 0) return fail(TANGRAM_ERR_INVALID_ARG, "account_pages: reserved[%d][%d] < 0", r, h);
+            exact += (int64_t)P * ((row[h] + (int64_t)P - 1) / P);
+            used += row[h];
+        }
+        for (int32_t g = 0; g < H / Hp; ++g) {
+            int32_t longest = 0;
+            for (int32_t j = 0; j < Hp; ++j) longest = std::max(longest, row[order[g * Hp + j]]);
+            pages += (longest + (int64_t)P - 1) / P;
+        }
+        full += (int64_t)H * P * ((ctx_len[r] + (int64_t)P - 1) / P);
+    }
+    const int64_t alloc = (int64_t)Hp * P * pages;
+    out->pages_alloc = pages, out->slots_alloc = alloc, out->slots_exact = exact, out->slots_full = full;
+    out->slots_used = used, out->tables = (int64_t)R * (H / Hp);
+    out->reclaimed_frac = 1.0 - static_cast<double>(alloc) / static_cast<double>(full);
+    out->fragmentation = alloc > 0 ? static_cast<double>(alloc - used) / static_cast<double>(alloc) : 0.0;
+    return TANGRAM_OK;
+}
+
+// ---- NEXT-4: Budget Calibration (:156-158, Eq. 5); population sigma, sums in sample order
+extern "C" int tangram_calibrate_budgets(const double* ratios, int32_t n_samples, int32_t H, double alpha,
+                                         double* mu_out, double* sigma_out, double* B_out) {
+    if (!ratios || !mu_out || !sigma_out) return fail(TANGRAM_ERR_INVALID_ARG, "calibrate_budgets: NULL argument");
+    if (n_samples < 1 || H < 1) return fail(TANGRAM_ERR_INVALID_ARG, "calibrate_budgets: n_samples=%d H=%d", n_samples, H);
+    for (size_t i = 0; i < (size_t)n_samples * H; ++i)
+        if (!std::isfinite(ratios[i])) return fail(TANGRAM_ERR_INVALID_ARG, "calibrate_budgets: ratio %zu is not finite", i);
+    const double n = static_cast<double>(n_samples);
+    for (int32_t h = 0; h < H; ++h) {
+        double acc = 0.0;
+        for (int32_t i = 0; i < n_samples; ++i) acc = acc + ratios[(size_t)i * H + h];
+        const double m = acc / n;
+        double acc2 = 0.0;
+        for (int32_t i = 0; i < n_samples; ++i) {
+            const double dlt = ratios[(size_t)i * H + h] - m;
+            const double sq = dlt * dlt;
+            acc2 = acc2 + sq;
+        }
+        const double sd = std::sqrt(acc2 / n);
+        mu_out[h] = m, sigma_out[h] = sd;
+        if (B_out) {
+            const double margin = alpha * sd;
+            B_out[h] = std::min(1.0, m + margin);  // Eq. 5
+        }
+    }
+    return TANGRAM_OK;
+}

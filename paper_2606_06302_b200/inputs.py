@@ -191,3 +191,13 @@ def make_scores_and_dense_kv(wl: Workload, n_max: int, device: str = "cpu", *, t
         for r in range(wl.R):  # one request at a time: bounded fp32 scratch
             dst[r] = torch.randn(wl.H, n_max, wl.d, generator=gen, device=device, dtype=torch.float32).bfloat16()
     return scores, k, v
+
+
+def make_calibration_ratios(wl: Workload, n_samples: int = 50) -> np.ndarray:
+    """[n_samples, H] per-head implicit retention ratios as a calibration run would record them
+    (PAPER.md:156, 50 samples :262): the workload's nominal head ratio times the same uniform per-input
+    jitter the demand uses (half-width = sigma * sqrt(3) / mu), clipped to (0, 1]."""
+    rng = np.random.default_rng(wl.seed + 99991)
+    hw = np.where(wl.mu > 0, wl.sigma * math.sqrt(3.0) / np.maximum(wl.mu, 1e-300), 0.0)
+    u = rng.uniform(-1.0, 1.0, size=(n_samples, wl.H))
+    return np.clip(wl.mu[None, :] * (1.0 + hw[None, :] * u), 1e-6, 1.0)

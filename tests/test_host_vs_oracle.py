@@ -148,3 +148,64 @@ def test_skew_balance_numbers():
     ps = T.tangram_plan_partitions(tp, B, kv, 296, 64, 0, T.MODE_STATIC_EVEN)
     assert ps.split_map.tolist() == [3, 3]
     assert max(int(it[5] - it[4]) for it in ps.items) == 43712           # ceil(2048/3)=683 granules * 64
+
+
+# ---------------------------------------------------------------------------- NEXT-3 / NEXT-4 (host, bit-exact)
+@pytest.mark.parametrize("name", I.CONFIG_NAMES)
+def test_account_pages_bit_exact_on_the_configs(name):
+    wl = I.make_workload(name)
+    B, res, _ = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    for Hp in [d for d in (1, 2, 4, 8) if wl.H % d == 0]:
+        for pol in (T.GROUP_CLUSTERED, T.GROUP_ADJACENT):
+            got = T.tangram_account_pages(B, res, wl.ctx_len, Hp, wl.P, pol)
+            want = O.account_pages(B, res, wl.ctx_len, Hp, wl.P, pol)
+            assert got == want, (Hp, pol)                 # integers and the two fp64 ratios, bit for bit
+    # the tables the product builds occupy exactly the accounted pages
+    assert T.tangram_account_pages(B, res, wl.ctx_len, wl.Hp, wl.P, T.GROUP_CLUSTERED)["pages_alloc"] == \
+        T.tangram_pages_needed(B, res, wl.C, wl.P)
+
+
+@settings(max_examples=60, deadline=None)
+@given(st.integers(1, 5), st.sampled_from([2, 4, 6, 8, 12]), st.integers(0, 2 ** 31 - 1))
+def test_account_pages_random(R, H, seed):
+    rng = np.random.default_rng(seed)
+    B = np.round(rng.uniform(0.01, 1.0, size=H), 2)          # rounded: equal budgets (ties) do occur
+    ctx = rng.integers(1, 3000, size=R).astype(np.int32)
+    res = np.maximum(1, np.ceil(B[None, :] * ctx[:, None])).astype(np.int32)
+    P = int(rng.choice([1, 8, 16, 32]))
+    for Hp in [d for d in range(1, H + 1) if H % d == 0]:
+        for pol in (T.GROUP_CLUSTERED, T.GROUP_ADJACENT):
+            assert T.tangram_account_pages(B, res, ctx, Hp, P, pol) == O.account_pages(B, res, ctx, Hp, P, pol)
+
+
+def test_account_pages_error_contract():
+    B, res, ctx = np.array([0.5, 0.5]), np.array([[5, 5]], dtype=np.int32), np.array([10], dtype=np.int32)
+    for args in ((B, res, ctx, 3, 16, 0), (B, res, ctx, 2, 0, 0), (B, res, ctx, 2, 16, 7), (B, -res, ctx, 2, 16, 0),
+                 (B, res, ctx * 0, 2, 16, 0)):
+        with pytest.raises(T.TangramError) as e:
+            T.tangram_account_pages(*args)
+        assert e.value.code == T.ERR_INVALID_ARG
+
+
+@settings(max_examples=60, deadline=None)
+@given(st.integers(1, 60), st.integers(1, 9), st.integers(0, 2 ** 31 - 1), st.sampled_from([0.0, 1.0, 2.0, 2.5]))
+def test_calibrate_budgets_bit_exact(n, H, seed, alpha):
+    rng = np.random.default_rng(seed)
+    x = rng.uniform(0.0, 1.0, size=(n, H))
+    mo, so, Bo = O.calibrate_budgets(x, alpha)
+    mp, sp, Bp = T.tangram_calibrate_budgets(x, alpha)
+    assert mo.tobytes() == mp.tobytes() and so.tobytes() == sp.tobytes() and Bo.tobytes() == Bp.tobytes()
+
+
+def test_calibrate_then_reserve_pipeline_and_errors():
+    """Calibration feeds Budget Reservation: 50 synthetic samples of the 8b head profile (:262)."""
+    wl = I.make_workload("8b")
+    x = I.make_calibration_ratios(wl, 50)
+    mu, sigma, B = T.tangram_calibrate_budgets(x, wl.alpha)
+    B2, res, kv = T.tangram_reserve_budgets(mu, sigma, wl.alpha, wl.ctx_len, wl.demand)
+    assert B.tobytes() == B2.tobytes()
+    assert (np.abs(mu - wl.mu) < 0.1 * wl.mu).all()           # the samples were drawn around the nominal ratios
+    with pytest.raises(T.TangramError):
+        T.tangram_calibrate_budgets(np.array([[np.nan]]), 2.0)
+    with pytest.raises(T.TangramError):
+        T.tangram_calibrate_budgets(np.zeros((0, 3)), 2.0)
