@@ -165,7 +165,8 @@ size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan* p);
 /* Host-side view of an uploaded plan: sizes plus DEVICE pointers into the blob.  Plain data; valid
  * as long as the blob is. */
 typedef struct tangram_device_plan {
-    int32_t R, H, C, Hp, P, W /* work lists */, mode, n_static /* launch grid */;
+    int32_t R, H, C, Hp, P, W /* work lists on the device: the plan's, minus empty dynamic-tail lists */, mode,
+        n_static /* launch grid */;
     int64_t n_items, n_part_slots;
     int64_t n_merge_seqs;       /* sequences whose part count is not 1 */
     int64_t n_empty_seqs;       /* of these, the first n_empty_seqs have no part at all (kv_len 0) */

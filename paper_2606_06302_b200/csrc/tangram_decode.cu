@@ -891,10 +891,16 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
         if (p->part_indptr[sq + 1] - p->part_indptr[sq] > kMergeBigParts) push(sq);
     off += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);
     const size_t off_heads = off;
-    {   // list head = {item_begin, n_items, 0, 0, first item (8 words), its first 16 page ids, 0 x 4}
-        int32_t* hd = reinterpret_cast<int32_t*>(host.data() + off);
-        for (int32_t k = 0; k < p->W; ++k, hd += 32) {
+    int32_t n_dev_lists = 0;
+    {   // list head = {item_begin, n_items, 0, 0, first item (8 words), its first 16 page ids, 0 x 4}.
+        // The first n_static lists belong to the CTAs and are kept as they are; of the dynamic-tail lists only
+        // the non-empty ones are uploaded (in plan order): claiming an empty list costs a CTA an atomic and a
+        // dependent load for nothing, which is most of the tail on a small batch.
+        int32_t* heads = reinterpret_cast<int32_t*>(host.data() + off);
+        for (int32_t k = 0; k < p->W; ++k) {
             const int64_t ib = p->worker_indptr[k], ie = p->worker_indptr[k + 1];
+            if (k >= p->n_static && ie == ib) continue;
+            int32_t* hd = heads + 32 * n_dev_lists++;
             hd[0] = (int32_t)ib, hd[1] = (int32_t)(ie - ib);
             if (ie > ib) {
                 std::memcpy(hd + 4, &di[ib], sizeof(DeviceItem));
@@ -925,7 +931,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "upload: cudaStreamSynchronize");
     uint8_t* base = static_cast<uint8_t*>(dev_blob);
-    dp->R = t->R, dp->H = t->H, dp->C = t->C, dp->Hp = t->Hp, dp->P = t->P, dp->W = p->W, dp->mode = p->mode;
+    dp->R = t->R, dp->H = t->H, dp->C = t->C, dp->Hp = t->Hp, dp->P = t->P, dp->W = n_dev_lists, dp->mode = p->mode;
     dp->n_static = p->n_static;
     dp->sched = reinterpret_cast<int32_t*>(base + off_sched);
     dp->merge_seqs = reinterpret_cast<const int32_t*>(base + off_mseq);
