@@ -23,6 +23,8 @@ What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.
                           adjacent, Budget-Aware Clustering; Fig. 7 :168, Fig. 8 :186, Fig. 15 :316-320; NEXT-3)
   O9 calibrate_budgets    mu, sigma of the recorded per-head implicit retention ratios and Eq. 5 (:156-158;
                           population sigma = reading A10; NEXT-4)
+  O10 implicit_ratios     the per-head retention ratios a global flat Top-ceil(rho H N) selection implies (Eq. 3
+                          :68-77; what Budget Calibration records per sample, :156; NEXT-4)
   O1 attention*           plain softmax(q K~^T / sqrt(d)) V~ through the page tables (Eq. 1 :57)
 
 Pins (every function is pinned; nothing here is "parity unpinned"): tests/test_oracle_pins.py.
@@ -489,6 +491,31 @@ def calibrate_budgets(ratios, alpha: float):
         mu[h], sigma[h] = m, sd
         B[h] = min(1.0, m + alpha * sd)
     return mu, sigma, B
+
+
+# --------------------------------------------------------------------------------------------
+# O10  implicit per-head retention ratios of the global flat Top-k (NEXT-4; Eq. 3 :68-77, :156)
+# --------------------------------------------------------------------------------------------
+def implicit_ratios(scores, ctx_len, rho: float):
+    """I = Top(ceil(rho H N), s^flat) over the flattened scores of all H heads of a request (Eq. 3), and the
+    ratio |{(h, t) in I}| / N each head receives from it -- the quantity Budget Calibration records on every
+    sample context (:156).  s^flat is head-major (index h N + t); ties go to the lower flat index (reading
+    A30 applied to the flat vector).  scores [R][H][n_max] f32 (entries >= ctx_len[r] ignored).
+    Returns (counts [R][H] int64, ratios [R][H] f64 = counts / N_r)."""
+    sc = np.asarray(scores, dtype=np.float32)
+    R, H = sc.shape[0], sc.shape[1]
+    counts = np.zeros((R, H), dtype=np.int64)
+    ratios = np.zeros((R, H), dtype=np.float64)
+    for r in range(R):
+        N = int(ctx_len[r])
+        flat = np.concatenate([sc[r, h, :N] for h in range(H)])
+        k = int(math.ceil(rho * float(H * N)))
+        k = max(0, min(k, H * N))
+        for i in topk_indices(flat, k):
+            counts[r, int(i) // N] += 1
+        for h in range(H):
+            ratios[r, h] = float(counts[r, h]) / float(N)
+    return counts, ratios
 
 
 # --------------------------------------------------------------------------------------------

@@ -647,3 +647,37 @@ def test_calibrate_budgets_closed_forms_and_library():
     # Cantelli: at most 1/(1 + alpha^2) of the samples exceed mu + alpha * sigma (holds for the empirical
     # distribution with the population sigma)
     assert ((x > (mu + 2.0 * sd)[None, :]).mean(0) <= 0.2 + 1e-12).all()
+
+
+# ---------------------------------------------------------------------------- O10 implicit ratios (Eq. 3, NEXT-4)
+def test_implicit_ratios_brute_force_and_closed_forms():
+    rng = np.random.default_rng(17)
+    R, H, n_max = 3, 4, 37
+    ctx = np.array([37, 20, 5])
+    sc = rng.integers(0, 6, size=(R, H, n_max)).astype(np.float32)          # heavy ties across heads
+    for rho in (0.0, 0.13, 0.5, 0.99, 1.0):
+        cnt, rat = O.implicit_ratios(sc, ctx, rho)
+        for r in range(R):
+            N = int(ctx[r])
+            flat = [(float(sc[r, h, t]), h * N + t) for h in range(H) for t in range(N)]
+            k = min(H * N, max(0, math.ceil(rho * H * N)))
+            # definition: entry i is selected iff fewer than k entries beat it (higher score, or equal and lower flat index)
+            sel = [i for (v, i) in flat if sum(1 for (w, j) in flat if w > v or (w == v and j < i)) < k]
+            want = np.bincount(np.array(sel, dtype=np.int64) // N, minlength=H) if sel else np.zeros(H, int)
+            assert cnt[r].tolist() == want.tolist() and cnt[r].sum() == k
+            assert np.array_equal(rat[r], cnt[r] / N)
+    # heads on disjoint score bands: the flat selection eats the highest heads first
+    N = 10
+    band = np.stack([np.linspace(0, 0.9, N) + 10 * h for h in range(4)])[None].astype(np.float32)
+    cnt, rat = O.implicit_ratios(band, [N], 0.625)                          # k = 25
+    assert cnt[0].tolist() == [0, 5, 10, 10] and rat[0].tolist() == [0.0, 0.5, 1.0, 1.0]
+    # identical score vectors in every head, no ties inside a head: equal shares, the remainder to the lower heads
+    same = np.tile(np.arange(8, dtype=np.float32)[None, None, :], (1, 3, 1))
+    assert O.implicit_ratios(same, [8], 10 / 24)[0][0].tolist() == [4, 3, 3]
+    # mean over heads of the implicit ratios = k / (H N) >= rho  (Eq. 3 keeps the global budget exactly)
+    big = rng.normal(size=(2, 8, 300)).astype(np.float32)
+    cnt, rat = O.implicit_ratios(big, [300, 211], 0.3)
+    assert cnt.sum(1).tolist() == [math.ceil(0.3 * 8 * 300), math.ceil(0.3 * 8 * 211)]
+    # a global selection over ONE head is the per-head selection of Eq. 4
+    one = rng.normal(size=(1, 1, 50)).astype(np.float32)
+    assert O.implicit_ratios(one, [50], 0.2)[0][0, 0] == len(O.topk_indices(one[0, 0], 10))
