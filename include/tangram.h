@@ -323,6 +323,20 @@ int tangram_account_pages(const double* B, const int32_t* reserved, const int32_
 int tangram_calibrate_budgets(const double* ratios, int32_t n_samples, int32_t H, double alpha, double* mu_out,
                               double* sigma_out, double* B_out);
 
+/* NEXT-4 (device)  Implicit per-head retention ratios of the global flat Top-k -- PAPER.md:68-77 (Eq. 3:
+ * I_l = Top(ceil(rho H N), s^flat) over the scores of all H heads of a layer flattened together), :156 (Budget
+ * Calibration records the ratio each head receives from that selection on every sample context; the rows of
+ * tangram_calibrate_budgets' `ratios` input).
+ *
+ *   scores       device [R][H][n_max] f32 (entries >= ctx_len[r] ignored); H * n_max < 2^31
+ *   ctx_len_dev  device [R] i32, 1 <= ctx_len[r] <= n_max        rho in [0, 1]
+ *   counts_out   device [R][H] i32: entries of head h among the ceil(rho * H * N_r) highest-scoring ones of request
+ *                r; s^flat is head-major, scores compared as fp32 values (-0 == +0), ties to the lower flat index
+ *   ratios_out   device [R][H] f64 = counts / N_r
+ * Asynchronous on `stream` (one launch, one CTA per request).  Errors: INVALID_ARG, CUDA. */
+int tangram_implicit_ratios(const float* scores, int32_t R, int32_t H, int64_t n_max, const int32_t* ctx_len_dev,
+                            double rho, int32_t* counts_out, double* ratios_out, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -69,14 +69,14 @@ _lib.tangram_compact_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
 for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
               "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk",
-              "tangram_account_pages", "tangram_calibrate_budgets"):
+              "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
            "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
            "tangram_compact_workspace_bytes", "tangram_compact_topk", "tangram_account_pages",
-           "tangram_calibrate_budgets")
+           "tangram_calibrate_budgets", "tangram_implicit_ratios")
 
 
 def _check(rc: int):
@@ -354,3 +354,19 @@ def tangram_calibrate_budgets(ratios, alpha: float):
     _check(_lib.tangram_calibrate_budgets(_ptr(x), C.c_int32(n), C.c_int32(H), C.c_double(alpha), _ptr(mu), _ptr(sigma),
                                           _ptr(B)))
     return mu, sigma, B
+
+
+def tangram_implicit_ratios(scores, ctx_len, rho: float, stream=None):
+    """NEXT-4 (device): per-head (counts [R,H] int32, ratios [R,H] f64) of the global flat Top-ceil(rho H N)
+    selection (Eq. 3) on scores [R,H,n_max] f32 cuda; ctx_len [R] int32 cuda."""
+    import torch
+    R, H, n_max = scores.shape
+    assert scores.is_cuda and scores.dtype == torch.float32 and scores.is_contiguous()
+    assert ctx_len.is_cuda and ctx_len.dtype == torch.int32 and ctx_len.numel() == R and ctx_len.is_contiguous()
+    counts = torch.empty(R, H, dtype=torch.int32, device=scores.device)
+    ratios = torch.empty(R, H, dtype=torch.float64, device=scores.device)
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    _check(_lib.tangram_implicit_ratios(C.c_void_p(scores.data_ptr()), C.c_int32(R), C.c_int32(H), C.c_int64(n_max),
+                                        C.c_void_p(ctx_len.data_ptr()), C.c_double(rho), C.c_void_p(counts.data_ptr()),
+                                        C.c_void_p(ratios.data_ptr()), sp))
+    return counts, ratios

@@ -113,6 +113,69 @@ __device__ __forceinline__ void for_each_key(const float4* __restrict__ sv, int 
     }
 }
 
+// The same for a whole score row s[0..N): <= 3 entries before the first 16-byte boundary, the aligned groups,
+// <= 3 entries after the last one.
+template <int NT, int U, typename F>
+__device__ __forceinline__ void for_each_key_row(const float* __restrict__ s, int N, int tid, F&& fn) {
+    const int head = min(N, static_cast<int>((4u - (static_cast<uint32_t>(reinterpret_cast<uintptr_t>(s)) >> 2)) & 3u));
+    const int nvec = (N - head) >> 2;
+    const int tail0 = head + 4 * nvec;
+    if (tid < head) fn(score_key(__ldg(s + tid)));
+    if (tid < N - tail0) fn(score_key(__ldg(s + tail0 + tid)));
+    for_each_key<NT, U>(reinterpret_cast<const float4*>(s + head), 0, nvec, tid, fn);
+}
+
+// Block-wide radix select of the k-th largest key (1 <= k <= number of entries): digits of 11, 11 and 10 bits
+// from the top, one shared-memory atomic histogram per digit.  each_key(add) must call add(key) once for every
+// entry, the entries split among the NT threads in any way.  Returns, in every thread, the threshold key T and
+// `need` = how many of the entries equal to T belong to the k largest (1 <= need <= their number).
+template <int NT, typename EachKey>
+__device__ __forceinline__ void radix_select(EachKey&& each_key, uint32_t k, uint32_t* s_hist, uint32_t* s_wsum,
+                                             uint32_t* s_pick, uint32_t& T, uint32_t& need) {
+    constexpr int kWarps = NT / 32;
+    constexpr int kBpt = kSelBins / NT;  // adjacent bins a thread owns in the scan
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t prefix = 0, mask = 0, krem = k;
+#pragma unroll 1
+    for (int pass = 0; pass < 3; ++pass) {
+        const int shift = pass == 0 ? 21 : (pass == 1 ? 10 : 0);
+        const uint32_t dmask = pass == 2 ? 1023u : 2047u;
+        for (int b = tid; b < kSelBins; b += NT) s_hist[b] = 0u;
+        __syncthreads();
+        each_key([&](uint32_t key) {
+            if ((key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & dmask], 1u);
+        });
+        __syncthreads();
+        {   // thread owns bins kBpt tid ..; `gt` = entries in higher bins (block-wide suffix sum)
+            uint32_t c[kBpt], mine = 0;
+#pragma unroll
+            for (int j = 0; j < kBpt; ++j) c[j] = s_hist[kBpt * tid + j], mine += c[j];
+            uint32_t incl = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t v = __shfl_down_sync(0xffffffffu, incl, o);
+                if (lane + o < 32) incl += v;
+            }
+            if (lane == 0) s_wsum[warp] = incl;
+            __syncthreads();
+            uint32_t gt = incl - mine;
+            for (int w = warp + 1; w < kWarps; ++w) gt += s_wsum[w];
+#pragma unroll
+            for (int j = kBpt - 1; j >= 0; --j) {
+                if (gt < krem && krem <= gt + c[j]) {  // exactly one bin of the row satisfies this
+                    s_pick[0] = prefix | (static_cast<uint32_t>(kBpt * tid + j) << shift);
+                    s_pick[1] = krem - gt;
+                }
+                gt += c[j];
+            }
+        }
+        __syncthreads();
+        prefix = s_pick[0], krem = s_pick[1];
+        mask |= dmask << shift;
+    }
+    T = prefix, need = krem;
+}
+
 // One CTA of NT threads per (request, KV head).  (A thread-block cluster per row with the histograms
 // exchanged through distributed shared memory was measured too: the remote loads and cluster barriers cost
 // more than the extra SMs bring -- 8b 40 -> 46 us with 2 CTAs per row, 220 us with 8.)
@@ -121,11 +184,10 @@ __global__ void __launch_bounds__(NT, 1024 / NT)
 topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len,
                    const int32_t* __restrict__ keep_eff, int H, int32_t* __restrict__ idx_out) {
     constexpr int kSelWarps = NT / 32;
-    constexpr int kSelBpt = kSelBins / NT;  // adjacent bins a thread owns in the scan
     constexpr int kU = NT == 1024 ? 4 : 8;  // 16-byte loads in flight per thread (register budget: 64 / 32)
     __shared__ uint32_t s_hist[kSelBins];
     __shared__ uint32_t s_wsum[kSelWarps];
-    __shared__ uint32_t s_prefix, s_krem;
+    __shared__ uint32_t s_pick[2];
     __shared__ uint32_t s_cnt[2][kSelWarps];  // (greater, equal) counts of the warps' segments
     const int seq = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = ctx_len[seq / H];
@@ -137,55 +199,15 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
         for (int i = tid; i < N; i += NT) idx[i] = i;
         return;
     }
+    // keep every key > T and the first `need` entries with key == T
+    uint32_t T, need;
+    radix_select<NT>([&](auto&& add) { for_each_key_row<NT, kU>(s, N, tid, add); }, static_cast<uint32_t>(k), s_hist,
+                     s_wsum, s_pick, T, need);
     // The row is <= 3 head entries, nvec aligned float4 groups, <= 3 tail entries.
     const int head = min(N, static_cast<int>((4u - (static_cast<uint32_t>(reinterpret_cast<uintptr_t>(s)) >> 2)) & 3u));
     const int nvec = (N - head) >> 2;
     const int tail0 = head + 4 * nvec;
     const float4* sv = reinterpret_cast<const float4*>(s + head);
-
-    // ---- radix select of the k-th largest key: digits of 11, 11 and 10 bits from the top
-    uint32_t prefix = 0, mask = 0, krem = static_cast<uint32_t>(k);
-#pragma unroll 1
-    for (int pass = 0; pass < 3; ++pass) {
-        const int shift = pass == 0 ? 21 : (pass == 1 ? 10 : 0);
-        const uint32_t dmask = pass == 2 ? 1023u : 2047u;
-        for (int b = tid; b < kSelBins; b += NT) s_hist[b] = 0u;
-        __syncthreads();
-        auto add = [&](uint32_t key) {
-            if ((key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & dmask], 1u);
-        };
-        if (tid < head) add(score_key(__ldg(s + tid)));
-        if (tid < N - tail0) add(score_key(__ldg(s + tail0 + tid)));
-        for_each_key<NT, kU>(sv, 0, nvec, tid, add);
-        __syncthreads();
-        {   // thread owns bins kSelBpt tid ..; `gt` = entries in higher bins (block-wide suffix sum)
-            uint32_t c[kSelBpt], mine = 0;
-#pragma unroll
-            for (int j = 0; j < kSelBpt; ++j) c[j] = s_hist[kSelBpt * tid + j], mine += c[j];
-            uint32_t incl = mine;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t v = __shfl_down_sync(0xffffffffu, incl, o);
-                if (lane + o < 32) incl += v;
-            }
-            if (lane == 0) s_wsum[warp] = incl;
-            __syncthreads();
-            uint32_t gt = incl - mine;
-            for (int w = warp + 1; w < kSelWarps; ++w) gt += s_wsum[w];
-#pragma unroll
-            for (int j = kSelBpt - 1; j >= 0; --j) {
-                if (gt < krem && krem <= gt + c[j]) {  // exactly one bin of the row satisfies this
-                    s_prefix = prefix | (static_cast<uint32_t>(kSelBpt * tid + j) << shift);
-                    s_krem = krem - gt;
-                }
-                gt += c[j];
-            }
-        }
-        __syncthreads();
-        prefix = s_prefix, krem = s_krem;
-        mask |= dmask << shift;
-    }
-    const uint32_t T = prefix, need = krem;  // keep every key > T and the first `need` entries with key == T
 
     // ---- ordered pass: position of token i = #greater before i + min(#equal before i, need).
     // Warp w owns the contiguous groups [v0, v1): it counts them (16-byte loads, 8 in flight), the counts of
@@ -280,6 +302,64 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
         for (int u = 0; u < 4; ++u) place4(x[u], v + u * 32 + lane);
     }
     for (; v < v1; v += 32) place4(v + lane < v1 ? __ldg(sv + v + lane) : make_float4(0.f, 0.f, 0.f, 0.f), v + lane);
+}
+
+// NEXT-4: implicit per-head retention ratios of the global flat Top-k (Eq. 3; what Budget
+// Calibration records on every sample, :156).  One CTA per request: radix select over the flattened scores of
+// all H heads (head-major; ties to the lower flat index), then per-head counts of the entries above the
+// threshold; the entries equal to it are granted in head order until `need` of them are taken.
+template <int NT>
+__global__ void __launch_bounds__(NT, 1024 / NT)
+implicit_ratio_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len, int H,
+                      double rho, int32_t* __restrict__ counts_out, double* __restrict__ ratios_out) {
+    constexpr int kU = NT == 1024 ? 4 : 8;
+    extern __shared__ uint32_t s_ge[];  // [2][H]: entries greater than / equal to the threshold, per head
+    __shared__ uint32_t s_hist[kSelBins];
+    __shared__ uint32_t s_wsum[NT / 32];
+    __shared__ uint32_t s_pick[2];
+    const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const int N = ctx_len[r];
+    const float* s = scores + static_cast<size_t>(r) * H * n_max;
+    const double total_f = static_cast<double>(static_cast<int64_t>(H) * N);
+    const double want = ceil(rho * total_f);  // Eq. 3: ceil(rho H N)
+    const uint32_t total = static_cast<uint32_t>(H) * static_cast<uint32_t>(N);
+    const uint32_t k = want <= 0.0 ? 0u : (want >= total_f ? total : static_cast<uint32_t>(want));
+    if (k == 0u || k == total) {
+        for (int h = tid; h < H; h += NT) {
+            counts_out[r * H + h] = k ? N : 0;
+            ratios_out[r * H + h] = k ? 1.0 : 0.0;
+        }
+        return;
+    }
+    uint32_t T, need;
+    radix_select<NT>(
+        [&](auto&& add) {
+            for (int h = 0; h < H; ++h) for_each_key_row<NT, kU>(s + static_cast<size_t>(h) * n_max, N, tid, add);
+        },
+        k, s_hist, s_wsum, s_pick, T, need);
+    for (int h = tid; h < 2 * H; h += NT) s_ge[h] = 0u;
+    __syncthreads();
+    for (int h = 0; h < H; ++h) {
+        uint32_t g = 0, e = 0;
+        for_each_key_row<NT, kU>(s + static_cast<size_t>(h) * n_max, N, tid, [&](uint32_t key) { g += key > T, e += key == T; });
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) g += __shfl_xor_sync(0xffffffffu, g, o), e += __shfl_xor_sync(0xffffffffu, e, o);
+        if (lane == 0) {
+            if (g) atomicAdd(&s_ge[h], g);
+            if (e) atomicAdd(&s_ge[H + h], e);
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t left = need;
+        for (int h = 0; h < H; ++h) {
+            const uint32_t take = min(s_ge[H + h], left);
+            left -= take;
+            const uint32_t c = s_ge[h] + take;
+            counts_out[r * H + h] = static_cast<int32_t>(c);
+            ratios_out[r * H + h] = static_cast<double>(c) / static_cast<double>(N);
+        }
+    }
 }
 
 template <int D>
@@ -416,5 +496,25 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
                                                                    dp->Hp, n_seq, w.counter, w.keep_eff, w.tile_indptr);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact gather launch");
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_implicit_ratios(const float* scores, int32_t R, int32_t H, int64_t n_max,
+                                       const int32_t* ctx_len_dev, double rho, int32_t* counts_out,
+                                       double* ratios_out, void* stream) {
+    if (!scores || !ctx_len_dev || !counts_out || !ratios_out)
+        return fail(TANGRAM_ERR_INVALID_ARG, "implicit_ratios: NULL argument");
+    if (R < 1 || H < 1 || H > 4096 || n_max < 1 || (int64_t)H * n_max > INT32_MAX)
+        return fail(TANGRAM_ERR_INVALID_ARG, "implicit_ratios: R=%d H=%d n_max=%lld (H * n_max must fit 31 bits)", R, H,
+                    (long long)n_max);
+    if (!(rho >= 0.0 && rho <= 1.0)) return fail(TANGRAM_ERR_INVALID_ARG, "implicit_ratios: rho=%g not in [0, 1]", rho);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t smem = 2 * sizeof(uint32_t) * (size_t)H;
+    if ((int64_t)H * n_max > kSelLongRow)
+        implicit_ratio_kernel<1024><<<R, 1024, smem, st>>>(scores, n_max, ctx_len_dev, H, rho, counts_out, ratios_out);
+    else
+        implicit_ratio_kernel<512><<<R, 512, smem, st>>>(scores, n_max, ctx_len_dev, H, rho, counts_out, ratios_out);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail2(e, "implicit ratio launch");
     return TANGRAM_OK;
 }

@@ -187,3 +187,44 @@ def test_compact_full_size_sampled_and_properties():
             got_v = pool[pages, sl, 1].reshape(-1, wl.d)[:k]
             It = torch.from_numpy(I_).cuda()
             assert torch.equal(got_k, kd[r, h, It]) and torch.equal(got_v, vd[r, h, It])
+
+
+# ---------------------------------------------------------------------------- NEXT-4: implicit ratios (Eq. 3)
+@pytest.mark.parametrize("seed,R,H,n_max,ties", [(51, 3, 4, 700, True), (52, 2, 8, 3001, False), (53, 1, 2, 45000, True),
+                                                 (54, 4, 3, 64, True)])
+def test_implicit_ratios_bit_exact(seed, R, H, n_max, ties):
+    g = torch.Generator(device="cuda").manual_seed(seed)
+    scores = torch.randn(R, H, n_max, generator=g, device="cuda").exp_()
+    scores *= torch.linspace(0.5, 2.0, H, device="cuda")[None, :, None]       # heads of different importance
+    if ties:
+        scores = scores.bfloat16().float()
+    rng = np.random.default_rng(seed)
+    ctx = rng.integers(max(1, n_max // 3), n_max + 1, size=R).astype(np.int32)
+    ctx[0] = n_max
+    ctx_dev = torch.from_numpy(ctx).cuda()
+    for rho in (0.0, 0.3, 0.5, 1.0, 1e-9):
+        cnt, rat = T.tangram_implicit_ratios(scores, ctx_dev, rho)
+        torch.cuda.synchronize()
+        ref_cnt, ref_rat = O.implicit_ratios(scores.cpu().numpy(), ctx, rho)
+        assert np.array_equal(cnt.cpu().numpy(), ref_cnt), rho
+        assert rat.cpu().numpy().tobytes() == ref_rat.tobytes(), rho
+
+
+def test_calibration_pipeline_scores_to_budgets():
+    """Offline calibration end to end (:156-158): scores of 12 sample contexts -> Eq. 3 implicit ratios (CUDA) ->
+    mu, sigma, B (host C++) against the same chain through the oracle; the budgets then drive a1."""
+    H, n_max, n_samples, rho = 8, 2048, 12, 0.3
+    g = torch.Generator(device="cuda").manual_seed(77)
+    head_gain = torch.tensor([0.3, 0.5, 3.0, 0.4, 0.6, 2.5, 0.5, 0.7], device="cuda")   # two "retrieval" heads
+    scores = (torch.randn(n_samples, H, n_max, generator=g, device="cuda").exp_() * head_gain[None, :, None]).bfloat16().float()
+    ctx = np.random.default_rng(3).integers(700, n_max + 1, size=n_samples).astype(np.int32)
+    _, rat = T.tangram_implicit_ratios(scores, torch.from_numpy(ctx).cuda(), rho)
+    torch.cuda.synchronize()
+    mu, sigma, B = T.tangram_calibrate_budgets(rat.cpu().numpy(), 2.0)
+    _, ref_rat = O.implicit_ratios(scores.cpu().numpy(), ctx, rho)
+    mo, so, Bo = O.calibrate_budgets(ref_rat, 2.0)
+    assert mu.tobytes() == mo.tobytes() and sigma.tobytes() == so.tobytes() and B.tobytes() == Bo.tobytes()
+    assert abs(mu.mean() - rho) < 1e-3                      # Eq. 3 keeps the global budget: mean_h mu_h = rho (+ ceil)
+    assert set(np.argsort(B)[-2:]) == {2, 5}                # the high-gain heads get the large budgets
+    B2, res, _ = T.tangram_reserve_budgets(mu, sigma, 2.0, np.array([4096], dtype=np.int32))
+    assert B2.tobytes() == B.tobytes() and res.sum() >= math.ceil(rho * H * 4096) - H
