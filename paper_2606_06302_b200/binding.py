@@ -237,19 +237,22 @@ def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, wor
     """q [R,Hq,d] bf16 cuda, kv_pool [n_pages,Hp,2,P,d] bf16 cuda -> (out [R,Hq,d] bf16, lse [R,Hq] f32).
     Asynchronous on the current (or given) torch stream."""
     import torch
-    assert q.is_cuda and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
+    # q / out / lse may also be PINNED host tensors: page-locked memory is mapped into the device's address space
+    # (unified addressing), the kernels read q and write out / lse in place over the bus, no staging copy
+    assert (q.is_cuda or q.is_pinned()) and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
     assert q.is_contiguous() and kv_pool.is_contiguous()
     R, Hq, d = q.shape
     n_pages = kv_pool.shape[0]
     assert tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d) and R == dp.c.R
     G = Hq // dp.c.H
     if out is None:
-        out = torch.empty_like(q)
+        out = torch.empty(R, Hq, d, dtype=torch.bfloat16, device=kv_pool.device)
     if lse is None:
-        lse = torch.empty(R, Hq, dtype=torch.float32, device=q.device)
+        lse = torch.empty(R, Hq, dtype=torch.float32, device=kv_pool.device)
+    assert (out.is_cuda or out.is_pinned()) and (lse.is_cuda or lse.is_pinned())
     need = tangram_workspace_bytes(int(dp.c.n_part_slots), G, d)
     if workspace is None:
-        workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
+        workspace = torch.empty(need, dtype=torch.uint8, device=kv_pool.device)
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     wn = C.c_void_p(worker_ns.data_ptr()) if worker_ns is not None else None
     if kv_len is not None:

@@ -390,3 +390,23 @@ def test_multi_layer_decode_loop_under_one_cuda_graph():
         ro, rl, _ = O.attention(S["q"].cpu(), torch.from_numpy(rb.view(np.int16)).view(torch.bfloat16), ot, rk,
                                 S["wl"].Hq, S["wl"].d)
         check(S["out"], S["lse"], ro, rl, "multi-layer graph loop")
+
+
+def test_pinned_host_q_and_outputs_zero_copy():
+    """q, out and lse in pinned host memory passed straight through the C ABI (device-mapped): same bits as the
+    device-resident call, and within tolerance of the oracle."""
+    wl = I.make_workload("8b", R=3, ctx_div=8)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    pl = T.tangram_plan_partitions(t, B, kv, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dp = T.tangram_upload(t, pl)
+    out_d, lse_d = T.tangram_decode_attention(dp, q, pool)
+    q_h = q.cpu().pin_memory()
+    out_h = torch.zeros(q.shape, dtype=torch.bfloat16).pin_memory()
+    lse_h = torch.zeros(wl.R, wl.Hq, dtype=torch.float32).pin_memory()
+    for _ in range(2):
+        T.tangram_decode_attention(dp, q_h, pool, out_h, lse_h)
+        torch.cuda.synchronize()
+        assert torch.equal(out_h, out_d.cpu()) and torch.equal(lse_h, lse_d.cpu())
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    check(out_h, lse_h, ref_out, ref_lse, "pinned host buffers")
