@@ -228,3 +228,32 @@ def test_calibration_pipeline_scores_to_budgets():
     assert set(np.argsort(B)[-2:]) == {2, 5}                # the high-gain heads get the large budgets
     B2, res, _ = T.tangram_reserve_budgets(mu, sigma, 2.0, np.array([4096], dtype=np.int32))
     assert B2.tobytes() == B.tobytes() and res.sum() >= math.ceil(rho * H * 4096) - H
+
+
+def test_compact_topk_is_graph_capturable_and_repeatable():
+    """Three launches, no host work: captured once, replayed on fresh pools, same bytes every time."""
+    wl = I.make_random_workload(61, R=3, H=4, G=1, d=128, C=2, max_ctx=2000)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    _, pool0 = I.make_q_and_pool(wl, n_pool, "cuda")
+    pool = pool0.clone()
+    keep = torch.from_numpy(kv.astype(np.int32)).cuda()
+    ctx = torch.from_numpy(wl.ctx_len).cuda()
+    idx = torch.empty(wl.R, wl.H, n_max, dtype=torch.int32, device="cuda")
+    ws = torch.empty(T.tangram_compact_workspace_bytes(wl.R, wl.H), dtype=torch.uint8, device="cuda")
+    T.tangram_compact_topk(dp, scores, kd, vd, ctx, keep, pool, idx_out=idx, workspace=ws)
+    torch.cuda.synchronize()
+    want = bits(pool).copy()
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            T.tangram_compact_topk(dp, scores, kd, vd, ctx, keep, pool, idx_out=idx, workspace=ws, stream=st)
+        for _ in range(3):
+            pool.copy_(pool0)
+            g.replay()
+            st.synchronize()
+            assert np.array_equal(bits(pool), want)
+    torch.cuda.current_stream().wait_stream(st)
