@@ -302,8 +302,10 @@ def reference_arm(args):
             toks.append(tok)
     alg_bytes = sum(toks) / wl.G * 4 * wl.d
     tbs = alg_bytes / sum(times) / 1e12
-    sample = (f"each step = a random sample of (request, query head) rows of the {name} workload worth "
-              f"~{per_step_s:.2f} s of oracle time ({int(np.mean(toks))} token visits per step)")
+    n_rows = wl.R * wl.Hq
+    sample = (f"each step = {len(pairs)} of the {n_rows} (request, query head) rows of the {name} workload "
+              f"({int(np.mean(toks))} token visits, {np.mean(times):.3f} s of oracle time per step on {used} threads; "
+              f"the sample is capped at the whole workload or ~{per_step_s:.0f} s, whichever is smaller)")
     line = {"impl": "reference", "metric": METRIC, "value": tbs, "unit": "TB/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(times) * 1e3),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
