@@ -257,3 +257,33 @@ def test_compact_topk_is_graph_capturable_and_repeatable():
             st.synchronize()
             assert np.array_equal(bits(pool), want)
     torch.cuda.current_stream().wait_stream(st)
+
+
+def test_random_sweep_compaction_and_implicit_ratios():
+    """100 seeded cases (shapes, unaligned n_max, three score distributions incl. five-valued scores, empty heads):
+    index lists, every pool byte, implicit-ratio counts and fp64 ratios bit-exact against the oracle."""
+    rng = np.random.default_rng(20260631)
+    for case in range(100):
+        H, d = int(rng.choice([1, 2, 4, 8])), int(rng.choice([64, 128]))
+        C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
+        R = int(rng.integers(1, 4))
+        wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=1, d=d, C=C,
+                                    max_ctx=int(rng.choice([20, 200, 1100, 2100, 6000])))
+        if rng.random() < 0.3:
+            wl.demand[rng.integers(R), rng.integers(H)] = 0
+        B, res, kv, t, n_pool, dp = setup(wl)
+        n_max = int(wl.ctx_len.max()) + int(rng.integers(0, 5))
+        g = torch.Generator(device="cuda").manual_seed(int(rng.integers(1 << 30)))
+        kind = int(rng.integers(3))
+        if kind == 0:
+            scores = torch.randn(R, H, n_max, generator=g, device="cuda")
+        elif kind == 1:
+            scores = torch.randint(-2, 3, (R, H, n_max), generator=g, device="cuda").float()
+        else:
+            scores = torch.randn(R, H, n_max, generator=g, device="cuda").exp().bfloat16().float()
+        _, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+        run_and_compare(wl, t, dp, n_pool, kv, scores, kd, vd, n_max)
+        rho = float(rng.choice([0.0, 0.1, 0.37, 1.0]))
+        cnt, rat = T.tangram_implicit_ratios(scores, torch.from_numpy(wl.ctx_len).cuda(), rho)
+        ref_cnt, ref_rat = O.implicit_ratios(scores.cpu().numpy(), wl.ctx_len, rho)
+        assert np.array_equal(cnt.cpu().numpy(), ref_cnt) and rat.cpu().numpy().tobytes() == ref_rat.tobytes(), case

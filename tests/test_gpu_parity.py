@@ -410,3 +410,35 @@ def test_pinned_host_q_and_outputs_zero_copy():
         assert torch.equal(out_h, out_d.cpu()) and torch.equal(lse_h, lse_d.cpu())
     ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
     check(out_h, lse_h, ref_out, ref_lse, "pinned host buffers")
+
+
+def test_random_sweep_of_shapes_plans_and_runtime_lengths():
+    """300 seeded cases over (R, H, G 1..8, d, clusters, context, W, mode, c0, granule, dynamic tail, FILL_GROUP,
+    empty heads, open-ended run-time lengths), every one against the oracle at the BASELINE tolerances, each
+    plan launched twice (the scheduler counters re-arm themselves)."""
+    rng = np.random.default_rng(20260630)
+    for case in range(300):
+        H = int(rng.choice([1, 2, 4, 8]))
+        G, d = int(rng.integers(1, 9)), int(rng.choice([64, 128]))
+        C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
+        R = int(rng.integers(1, 6))
+        wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=G, d=d, C=C,
+                                    max_ctx=int(rng.choice([40, 300, 1500, 4000])))
+        if rng.random() < 0.3:
+            wl.demand[rng.integers(R), rng.integers(H)] = 0
+        B, res, kv, t, n_pool = setup(wl, flags=int(rng.random() < 0.2))
+        W = int(rng.choice([1, 2, 7, 33, 148, 148, 148, 200]))
+        mode, c0 = int(rng.choice([0, 0, 0, 1, 2])), int(rng.integers(0, 3))
+        dyn = (int(rng.integers(50, 950)), int(rng.integers(1, 9))) if mode == 0 and rng.random() < 0.6 else (0, 0)
+        pl = T.tangram_plan_partitions(t, B, kv, W, int(rng.choice([16, 64, 64, 128])), c0, mode, 0, dyn[0], dyn[1])
+        dp = T.tangram_upload(t, pl)
+        q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+        kv_run, kv_dev = kv, None
+        if rng.random() < 0.4:
+            kv_run = (kv * rng.uniform(0, 1, size=kv.shape)).astype(np.int32)
+            kv_dev = torch.from_numpy(kv_run).cuda()
+        ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv_run, wl.Hq, wl.d)
+        for _ in range(2):
+            out, lse = T.tangram_decode_attention(dp, q, pool, kv_len=kv_dev)
+            torch.cuda.synchronize()
+            check(out, lse, ref_out, ref_lse, f"case {case}: R={R} H={H} G={G} d={d} C={C} W={W} mode={mode} dyn={dyn}")
