@@ -529,7 +529,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--workload", default="8b", choices=["tiny", "8b", "32b", "skew", "uniform"])
+    ap.add_argument("--workload", default="8b", choices=["tiny", "8b", "32b", "skew", "uniform", "12b_d256"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the other configs' summary lines")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -634,7 +634,7 @@ def main():
         per = {}
         del S
         torch.cuda.empty_cache()
-        for name in ("tiny", "8b", "32b", "skew", "uniform"):
+        for name in ("tiny", "8b", "32b", "skew", "uniform", "12b_d256"):
             S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs, dyn=dyn)
             if name == args.workload and not args.no_cpu_baseline:
                 from oracle import tangram_oracle as O

@@ -372,6 +372,8 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
     constexpr int kChunks = D / 8;           // 16-byte chunks per row
     constexpr int kRowsPerLd = 32 / kChunks;  // rows one warp-wide load covers
     constexpr int kLds = kCPage / kRowsPerLd; // loads per lane for the K rows of a tile (same for V)
+    constexpr int kPasses = D == 256 ? 2 : 1;
+    constexpr int kLdsP = kLds / kPasses;
     const int lane = threadIdx.x & 31;
     const int sub = lane / kChunks, ch = lane % kChunks;
     const int total = __ldg(counter + 1);
@@ -398,26 +400,30 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
             const int page = __ldg(tbl_pages + si.x + tl);
             int my_tok = 0;
             if (lane < n_rows) my_tok = __ldg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
-            uint4 kreg[kLds], vreg[kLds];
-#pragma unroll
-            for (int j = 0; j < kLds; ++j) {
-                const int row = j * kRowsPerLd + sub;
-                const int tok = __shfl_sync(0xffffffffu, my_tok, row);
-                if (row < n_rows) {
-                    const size_t src = (static_cast<size_t>(seq) * n_max + tok) * kChunks + ch;
-                    kreg[j] = __ldcs(k_dense + src);
-                    vreg[j] = __ldcs(v_dense + src);
-                }
-            }
             // pool[page][slot][kv][token][d]
             const size_t dst_k = ((static_cast<size_t>(page) * Hp + si.z) * 2) * kCPage * kChunks;
             const size_t dst_v = dst_k + static_cast<size_t>(kCPage) * kChunks;
+            // (at d = 256 a tile goes in two halves of eight rows: 16 + 16 loads would not fit the register budget)
 #pragma unroll
-            for (int j = 0; j < kLds; ++j) {
-                const int row = j * kRowsPerLd + sub;
-                if (row < n_rows) {
-                    pool[dst_k + row * kChunks + ch] = kreg[j];
-                    pool[dst_v + row * kChunks + ch] = vreg[j];
+            for (int half = 0; half < kPasses; ++half) {
+                uint4 kreg[kLdsP], vreg[kLdsP];
+#pragma unroll
+                for (int j = 0; j < kLdsP; ++j) {
+                    const int row = (half * kLdsP + j) * kRowsPerLd + sub;
+                    const int tok = __shfl_sync(0xffffffffu, my_tok, row);
+                    if (row < n_rows) {
+                        const size_t src = (static_cast<size_t>(seq) * n_max + tok) * kChunks + ch;
+                        kreg[j] = __ldcs(k_dense + src);
+                        vreg[j] = __ldcs(v_dense + src);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < kLdsP; ++j) {
+                    const int row = (half * kLdsP + j) * kRowsPerLd + sub;
+                    if (row < n_rows) {
+                        pool[dst_k + row * kChunks + ch] = kreg[j];
+                        pool[dst_v + row * kChunks + ch] = vreg[j];
+                    }
                 }
             }
         }
@@ -444,7 +450,8 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
                                     void* stream) {
     if (!dp || !scores || !k_dense || !v_dense || !ctx_len_dev || !keep_dev || !kv_pool || !idx_out || !workspace)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: NULL argument");
-    if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: head_dim %d not in {64, 128}", d);
+    if (d != 64 && d != 128 && d != 256)
+        return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kCPage) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: page size %d (kernels need 16)", dp->P);
     if (n_max < 1 || n_max > (1 << 30) || n_pool_pages < 1)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: n_max=%lld n_pool_pages=%lld", (long long)n_max,
@@ -473,27 +480,27 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
         topk_select_kernel<512><<<n_seq, 512, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "top-k select launch");
-    static thread_local int grid128 = 0, grid64 = 0;
-    int& grid = d == 128 ? grid128 : grid64;
-    if (grid == 0) {
-        int dev = 0, sms = 0, per_sm = 0;
-        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail2(e, "cudaGetDevice");
-        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
-            return cuda_fail2(e, "cudaDeviceGetAttribute");
-        e = d == 128 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, compact_gather_kernel<128>, kGatherThreads, 0)
-                     : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, compact_gather_kernel<64>, kGatherThreads, 0);
-        if (e != cudaSuccess) return cuda_fail2(e, "occupancy query");
-        grid = sms * (per_sm > 0 ? per_sm : 1);
-    }
     const uint4* kd = static_cast<const uint4*>(k_dense);
     const uint4* vd = static_cast<const uint4*>(v_dense);
     uint4* pool = static_cast<uint4*>(kv_pool);
-    if (d == 128)
-        compact_gather_kernel<128><<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool,
-                                                                    dp->Hp, n_seq, w.counter, w.keep_eff, w.tile_indptr);
-    else
-        compact_gather_kernel<64><<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool,
-                                                                   dp->Hp, n_seq, w.counter, w.keep_eff, w.tile_indptr);
+    auto gather = [&](auto kernel, int& grid) -> cudaError_t {
+        if (grid == 0) {  // persistent grid: SMs x resident CTAs
+            int dev = 0, sms = 0, per_sm = 0;
+            cudaError_t e2 = cudaGetDevice(&dev);
+            if (e2 == cudaSuccess) e2 = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e2 == cudaSuccess) e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kGatherThreads, 0);
+            if (e2 != cudaSuccess) return e2;
+            grid = sms * (per_sm > 0 ? per_sm : 1);
+        }
+        kernel<<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool, dp->Hp, n_seq,
+                                                w.counter, w.keep_eff, w.tile_indptr);
+        return cudaSuccess;
+    };
+    static thread_local int grid256 = 0, grid128 = 0, grid64 = 0;
+    if (d == 256) e = gather(compact_gather_kernel<256>, grid256);
+    else if (d == 128) e = gather(compact_gather_kernel<128>, grid128);
+    else e = gather(compact_gather_kernel<64>, grid64);
+    if (e != cudaSuccess) return cuda_fail2(e, "compact gather setup");
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact gather launch");
     return TANGRAM_OK;

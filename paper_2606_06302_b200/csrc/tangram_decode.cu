@@ -36,8 +36,10 @@
 namespace tangram {
 
 constexpr int kPage = 16;          // tokens per page the kernels are specialised for
-constexpr int kNW = 8;             // consumer warps
-constexpr int kThreads = (kNW + 1) * 32;
+// consumer warps of the decode kernel: 8, or 4 at d = 256 where one (page, head) tile is 16 KB and eight
+// three-stage rings would not fit in shared memory
+template <int D>
+constexpr int consumer_warps() { return D == 256 ? 4 : 8; }
 constexpr int kQSlots = 2;         // item / query ring depth
 constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime <= this)
 constexpr int kMaxG = 8;
@@ -72,6 +74,8 @@ struct DecodeParams {
 // ------------------------------------------------------------------ shared-memory carve-up
 template <int D>
 struct Smem {
+    static constexpr int kNW = consumer_warps<D>();
+    static constexpr int kThreads = (kNW + 1) * 32;          // + the producer warp
     static constexpr int kTile = 2 * kPage * D * 2;          // K rows + V rows of one (page, head)
     static constexpr int kHalf = 2 * kPage * 128;            // one 64-element column block of the tile
     static constexpr int kRowF = D + 8;                      // padded fp32 row of the merge scratch
@@ -325,9 +329,10 @@ tangram_merge_kernel(const int32_t* __restrict__ merge_recs, int n_small, const 
 
 // ------------------------------------------------------------------ a4: split-KV decode kernel
 template <int D, bool TIMED>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(Smem<D>::kThreads, 1)
 tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeParams p) {
     using L = Smem<D>;
+    constexpr int kNW = L::kNW;
     constexpr int kTile = L::kTile, kHalf = L::kHalf, kRowF = L::kRowF;
     extern __shared__ uint8_t smem_raw[];
     // 128-byte-swizzled TMA tiles need a 1024-byte aligned base
@@ -384,7 +389,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         // dependent memory round trips away from the claim instead of four.
         int64_t cb, ce;
         DeviceItem next;
-        int head_pid_lo = 0, head_pid_hi = 0;  // page ids of tiles (lane - rot) & 7 and that + 8 of the list's first item
+        int head_pid_lo = 0, head_pid_hi = 0;  // page ids of tiles (lane - rot) mod NW and that + NW of the list's first item
         auto load_head = [&](int list) {
             const int w = __ldg(reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(list) * 32 + lane);
             cb = __shfl_sync(0xffffffffu, w, 0);
@@ -396,7 +401,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             if (p.kv_len) next.tok_end = min(next.tok_end, __ldg(p.kv_len + next.req * p.H + next.kv_head));
             const int i0 = (lane - (next.part_slot & (kNW - 1))) & (kNW - 1);
             head_pid_lo = __shfl_sync(0xffffffffu, w, 12 + i0);
-            head_pid_hi = __shfl_sync(0xffffffffu, w, 20 + i0);
+            head_pid_hi = __shfl_sync(0xffffffffu, w, 12 + kNW + i0);
         };
         load_head(blockIdx.x);
         int seq = 0;  // running item number = position in the item / query ring
@@ -740,7 +745,7 @@ static int max_coresident(int smem) {
     int dev = 0, sms = 0, per_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED>, kThreads, smem) !=
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED>, Smem<D>::kThreads, smem) !=
         cudaSuccess)
         return 0;
     return sms * per_sm;
@@ -755,11 +760,12 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     // The tail merge needs a grid barrier, i.e. a cooperative launch with every CTA resident.
     static thread_local int cached_smem = -1, cached_max = 0;
-    if (want_tail_merge && cached_smem != smem) cached_max = max_coresident<D, TIMED>(smem), cached_smem = smem;
-    prm.tail_merge = want_tail_merge && dp->n_static <= cached_max;
+    if (want_tail_merge && D <= 128 && cached_smem != smem) cached_max = max_coresident<D, TIMED>(smem), cached_smem = smem;
+    // (at d = 256 the grid has 128 consumer threads per CTA, fewer than a merge record has elements: stand-alone kernel)
+    prm.tail_merge = want_tail_merge && D <= 128 && dp->n_static <= cached_max;
     *merged = prm.tail_merge;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
+    cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(Smem<D>::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
@@ -801,27 +807,27 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+template <int D>
+static cudaError_t occupancy_of(int gqa, int* per_sm) {
+    const int smem = Smem<D>::total(Smem<D>::max_stages(gqa), gqa);
+    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false>, Smem<D>::kThreads, smem);
+}
+
 }  // namespace tangram
 
 using namespace tangram;
 
 extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa, int32_t* n_cta_out) {
-    if (!n_cta_out || (head_dim != 64 && head_dim != 128) || gqa < 1 || gqa > kMaxG)
+    if (!n_cta_out || (head_dim != 64 && head_dim != 128 && head_dim != 256) || gqa < 1 || gqa > kMaxG)
         return fail(TANGRAM_ERR_INVALID_ARG, "query_max_ctas: head_dim=%d gqa=%d", head_dim, gqa);
     int sms = 0, per_sm = 0;
     cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
-    if (head_dim == 128) {
-        const int smem = Smem<128>::total(Smem<128>::max_stages(gqa), gqa);
-        e = cudaFuncSetAttribute(tangram_decode_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<128, false>, kThreads, smem);
-    } else {
-        const int smem = Smem<64>::total(Smem<64>::max_stages(gqa), gqa);
-        e = cudaFuncSetAttribute(tangram_decode_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<64, false>, kThreads, smem);
-    }
+    if (head_dim == 256) e = occupancy_of<256>(gqa, &per_sm);
+    else if (head_dim == 128) e = occupancy_of<128>(gqa, &per_sm);
+    else e = occupancy_of<64>(gqa, &per_sm);
     if (e != cudaSuccess) return cuda_fail(e, "occupancy query");
     *n_cta_out = sms * per_sm;
     return TANGRAM_OK;
@@ -957,7 +963,8 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
                          const int32_t* kv_len_dev, int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
                          size_t workspace_bytes, uint64_t* worker_ns, void* stream, int which) {
     if (!dp || !q || !kv_pool || !out || !lse) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
-    if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128}", d);
+    if (d != 64 && d != 128 && d != 256)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d (kernels need 16)", dp->P);
     if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > kMaxG)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d)", Hq,
@@ -996,10 +1003,11 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.sched = dp->sched;
     prm.kv_len = kv_len_dev, prm.H = dp->H;
 
-    prm.n_stages = d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G);
+    prm.n_stages = d == 256 ? Smem<256>::max_stages(G) : (d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G));
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
     prm.scale_log2 = scale * 1.4426950408889634f;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (d == 256) return launch_decode<256>(dp, prm, map, st, which);
     return d == 128 ? launch_decode<128>(dp, prm, map, st, which) : launch_decode<64>(dp, prm, map, st, which);
 }
 
@@ -1031,7 +1039,8 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
                                  void* stream) {
     if (!dp || !k_new || !v_new || !kv_pool || !kv_len_dev)
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: NULL argument");
-    if (d != 64 && d != 128) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: head_dim %d not in {64, 128}", d);
+    if (d != 64 && d != 128 && d != 256)
+        return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: page size %d (kernels need 16)", dp->P);
     if (n_pool_pages < 1) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: empty pool");
     if (reinterpret_cast<uintptr_t>(k_new) % 16 || reinterpret_cast<uintptr_t>(v_new) % 16 ||

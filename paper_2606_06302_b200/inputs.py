@@ -21,6 +21,9 @@ import numpy as np
 
 SEED_BASE = 20260630
 CONFIG_NAMES = ("tiny", "8b", "32b", "skew", "uniform")
+# not a BASELINE.json config: the 8b recipe on Gemma-3-12B-shaped heads (16 query / 8 KV heads of 256 dims,
+# one of the paper's five models) -- exercises the d = 256 kernels at full size
+EXTRA_CONFIG_NAMES = ("12b_d256",)
 
 
 @dataclasses.dataclass
@@ -71,7 +74,7 @@ def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1, layer
     arguments give the full BASELINE.json configuration.  `layer` > 0 draws another layer of the
     same shape (its own head ratios, i.e. its own budgets, clusters and plan) for multi-layer
     decode loops: seed + 1000 * layer; the context lengths of layer 0 are kept (same requests)."""
-    idx = CONFIG_NAMES.index(name)
+    idx = (CONFIG_NAMES + EXTRA_CONFIG_NAMES).index(name)
     seed = SEED_BASE + idx
     if layer:
         base = make_workload(name, R=R, ctx_div=ctx_div)
@@ -84,8 +87,8 @@ def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1, layer
         R_ = R or R0
         ctx = np.full(R_, 512 // ctx_div, dtype=np.int32)
         ratio_h = np.array([1.0, 0.25])
-    elif name == "8b":
-        R0, Hq, H, d, C, hw = 32, 32, 8, 128, 4, 0.10
+    elif name in ("8b", "12b_d256"):
+        R0, Hq, H, d, C, hw = (32, 32, 8, 128, 4, 0.10) if name == "8b" else (32, 16, 8, 256, 4, 0.10)
         R_ = R or R0
         ctx = (rng.integers(8192, 32768 + 1, size=R_) // ctx_div).astype(np.int32)
         ratio_h = np.exp(rng.normal(math.log(0.2), 0.5, size=H))

@@ -54,7 +54,7 @@ def run_and_compare(wl, t, dp, n_pool, keep, scores, kd, vd, n_max):
 
 @pytest.mark.parametrize("seed,R,H,d,C,max_ctx,ties", [(21, 3, 4, 128, 2, 3000, "bf16"), (22, 2, 6, 64, 3, 2500, "none"),
                                                        (23, 4, 2, 128, 1, 700, "bf16"), (24, 2, 8, 64, 8, 5000, "bf16"),
-                                                       (25, 1, 4, 128, 4, 40, "none"),
+                                                       (25, 1, 4, 128, 4, 40, "none"), (28, 2, 4, 256, 2, 1800, "bf16"),
                                                        # rows long enough for clusters of 4 and 8 CTAs
                                                        (26, 2, 2, 64, 2, 40000, "bf16"), (27, 1, 2, 64, 1, 70000, "bf16")])
 def test_compact_random_shapes_bit_exact(seed, R, H, d, C, max_ctx, ties):
@@ -264,7 +264,7 @@ def test_random_sweep_compaction_and_implicit_ratios():
     index lists, every pool byte, implicit-ratio counts and fp64 ratios bit-exact against the oracle."""
     rng = np.random.default_rng(20260631)
     for case in range(100):
-        H, d = int(rng.choice([1, 2, 4, 8])), int(rng.choice([64, 128]))
+        H, d = int(rng.choice([1, 2, 4, 8])), int(rng.choice([64, 128, 256]))
         C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
         R = int(rng.integers(1, 4))
         wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=1, d=d, C=C,

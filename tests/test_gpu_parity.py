@@ -65,7 +65,7 @@ def n_cta(wl):
 
 def test_query_max_ctas():
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    for d, g in ((64, 2), (128, 4), (128, 5), (128, 8)):
+    for d, g in ((64, 2), (128, 4), (128, 5), (128, 8), (256, 2), (256, 8)):
         n = T.tangram_query_max_ctas(0, d, g)
         assert n >= sms and n % sms == 0
 
@@ -89,7 +89,10 @@ def test_scaled_configs(name, kw):
 
 @pytest.mark.parametrize("seed,R,H,G,d,C", [(1, 3, 4, 1, 64, 2), (2, 2, 4, 2, 128, 4), (3, 3, 2, 3, 128, 1),
                                             (4, 2, 6, 5, 128, 3), (5, 2, 2, 8, 64, 1), (6, 1, 8, 7, 128, 2),
-                                            (7, 4, 4, 6, 64, 4), (8, 2, 2, 8, 128, 2)])
+                                            (7, 4, 4, 6, 64, 4), (8, 2, 2, 8, 128, 2),
+                                            # d = 256 (Gemma-3-shaped heads): four consumer warps, 16 KB tiles
+                                            (9, 2, 4, 2, 256, 2), (10, 2, 2, 8, 256, 1), (11, 3, 8, 4, 256, 4),
+                                            (12, 1, 1, 5, 256, 1)])
 def test_random_shapes(seed, R, H, G, d, C):
     wl = I.make_random_workload(seed, R=R, H=H, G=G, d=d, C=C, max_ctx=900)
     B, res, kv, t, n_pool = setup(wl)
@@ -419,7 +422,7 @@ def test_random_sweep_of_shapes_plans_and_runtime_lengths():
     rng = np.random.default_rng(20260630)
     for case in range(300):
         H = int(rng.choice([1, 2, 4, 8]))
-        G, d = int(rng.integers(1, 9)), int(rng.choice([64, 128]))
+        G, d = int(rng.integers(1, 9)), int(rng.choice([64, 128, 256]))
         C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
         R = int(rng.integers(1, 6))
         wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=G, d=d, C=C,
@@ -442,3 +445,29 @@ def test_random_sweep_of_shapes_plans_and_runtime_lengths():
             out, lse = T.tangram_decode_attention(dp, q, pool, kv_len=kv_dev)
             torch.cuda.synchronize()
             check(out, lse, ref_out, ref_lse, f"case {case}: R={R} H={H} G={G} d={d} C={C} W={W} mode={mode} dyn={dyn}")
+
+
+def test_head_dim_256_gemma_shaped_layer_with_append():
+    """16 query / 8 KV heads of 256 dims (the Gemma-3-12B attention shape): attention in all three
+    plan modes, then KV append + open-ended plan, against the oracle."""
+    wl = I.make_random_workload(71, R=4, H=8, G=2, d=256, C=2, max_ctx=3000)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    run_modes(wl, B, kv, t, q, pool, Ws=(5, n_cta(wl)))
+    rows = np.arange(wl.R)[:, None] * t.C + t.cluster_of[None, :]
+    cap = ((t.tbl_indptr[rows + 1] - t.tbl_indptr[rows]) * wl.P).astype(np.int32)
+    pl = T.tangram_plan_partitions(t, B, cap, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dp = T.tangram_upload(t, pl)
+    kv_dev = torch.from_numpy(kv.copy()).cuda()
+    g = torch.Generator(device="cuda").manual_seed(5)
+    pool_bits, kv_ref = bits(pool).copy(), kv.copy()
+    for step in range(3):
+        k_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+        v_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+        T.tangram_append_kv(dp, k_new, v_new, pool, kv_dev)
+        pool_bits, kv_ref, _ = O.append_kv(pool_bits, oracle_tables(t), kv_ref, bits(k_new), bits(v_new))
+        out, lse = T.tangram_decode_attention(dp, q, pool, kv_len=kv_dev)
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(pool), pool_bits) and np.array_equal(kv_dev.cpu().numpy(), kv_ref)
+        ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv_ref, wl.Hq, wl.d)
+        check(out, lse, ref_out, ref_lse, f"d=256 decode step {step}")
