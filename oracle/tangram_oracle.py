@@ -17,6 +17,8 @@ What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.
   O5 merge                log-sum-exp merge of split-KV partials (implied by split-KV :91, :120)
   O7 topk_indices /       per-head Top-ceil(B N) selection (Eq. 4 :154) and K~ = K[I,:], V~ = V[I,:] (Eq. 1
      compact_topk         :57) written into the ragged pages (NEXT-2; tie rule = reading A30)
+  O11 compact_topk_chunk  the same for one prefill chunk, appended behind what the head already holds (compression
+                          fused into chunked prefill, :152; NEXT-2 extension)
   O6 append_kv            one decode step's new K/V rows written into the ragged pages (NEXT-1;
                           page layout :190, capacity bound :176, reading A29)
   O8 account_pages        pages / token-head slots a batch occupies under a grouping policy (monolithic,
@@ -411,6 +413,42 @@ def compact_topk(pool_bits: np.ndarray, t: Tables, scores, k_dense_bits, v_dense
                 pool[page, sl, 0, pos % t.P, :] = k_dense_bits[r, h, tok, :]
                 pool[page, sl, 1, pos % t.P, :] = v_dense_bits[r, h, tok, :]
     return pool, out_idx
+
+
+# --------------------------------------------------------------------------------------------
+# O11  per-chunk Top-k + compaction appended behind the retained tokens (:152 "each prefill chunk is compressed
+#      as soon as its KV cache is generated"; Eq. 4 applied to the chunk, Eq. 1 into the ragged pages)
+# --------------------------------------------------------------------------------------------
+def compact_topk_chunk(pool_bits: np.ndarray, t: Tables, scores, k_dense_bits, v_dense_bits, chunk_len, keep, kv_len):
+    """One prefill chunk of chunk_len[r] tokens per request: I = Top(keep[r][h], s_{r,h}[:chunk_len[r]]) and the
+    rows K[I,:], V[I,:] of the CHUNK written, in ascending token order, to token slots
+    kv_len[r][h] .. kv_len[r][h] + keep[r][h] - 1 of head h's ragged pages; the length grows by keep.
+    scores [R][H][n_max] f32, k/v_dense_bits uint16 [R][H][n_max][d] hold the chunk.  Raises if a head would
+    exceed its table capacity (:176) or keep > chunk_len.
+    Returns (pool', kv_len', indices) with indices[r][h] the retained token indices inside the chunk."""
+    pool = np.array(pool_bits, dtype=np.uint16, copy=True)
+    kv = np.array(kv_len, dtype=np.int32, copy=True)
+    out_idx = [[None] * t.H for _ in range(t.R)]
+    for r in range(t.R):
+        N = int(chunk_len[r])
+        for h in range(t.H):
+            k = int(keep[r][h])
+            if k > N:
+                raise ValueError("keep > chunk_len")
+            c, sl = int(t.cluster_of[h]), int(t.slot_of[h])
+            lo, hi = int(t.tbl_indptr[r * t.C + c]), int(t.tbl_indptr[r * t.C + c + 1])
+            base = int(kv[r, h])
+            if base + k > (hi - lo) * t.P:
+                raise ValueError("chunk exceeds the table capacity")
+            idx = topk_indices(np.asarray(scores[r][h])[:N], k)
+            out_idx[r][h] = idx
+            for j, tok in enumerate(idx):
+                pos = base + j
+                page = int(t.tbl_pages[lo + pos // t.P])
+                pool[page, sl, 0, pos % t.P, :] = k_dense_bits[r, h, tok, :]
+                pool[page, sl, 1, pos % t.P, :] = v_dense_bits[r, h, tok, :]
+            kv[r, h] = base + k
+    return pool, kv, out_idx
 
 
 # --------------------------------------------------------------------------------------------

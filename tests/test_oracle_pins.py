@@ -681,3 +681,47 @@ def test_implicit_ratios_brute_force_and_closed_forms():
     # a global selection over ONE head is the per-head selection of Eq. 4
     one = rng.normal(size=(1, 1, 50)).astype(np.float32)
     assert O.implicit_ratios(one, [50], 0.2)[0][0, 0] == len(O.topk_indices(one[0, 0], 10))
+
+
+# ---------------------------------------------------------------------------- O11 chunked compaction (:152)
+def test_compact_topk_chunk_round_trip_and_single_chunk_case():
+    """A context compressed chunk by chunk: attention over the resulting cache (pinned gather O1) equals dense
+    library attention over the union, in chunk order, of the per-chunk brute-force-pinned selections; with one
+    chunk and an empty cache the result is compact_topk's, byte for byte."""
+    R, H, G, d, P = 2, 4, 2, 64, 16
+    chunks = [np.array([40, 33]), np.array([25, 40]), np.array([7, 1])]
+    keeps = [np.array([[40, 10, 21, 1], [33, 0, 16, 9]]), np.array([[25, 6, 11, 0], [40, 3, 17, 16]]),
+             np.array([[7, 2, 3, 1], [1, 1, 0, 1]])]
+    total = sum(keeps)
+    B = np.array([1.0, 0.25, 0.5, 0.3])
+    t, _ = O.build_ragged_tables(B, total.astype(np.int32), 2, P, np.random.default_rng(6).permutation(80).astype(np.int32))
+    g = torch.Generator().manual_seed(44)
+    pool0 = torch.randn(80, t.Hp, 2, P, d, generator=g).bfloat16()
+    bits_ = lambda x: x.view(torch.int16).numpy().view(np.uint16)
+    pool, kv = bits_(pool0).copy(), np.zeros((R, H), dtype=np.int32)
+    kept_k = [[[] for _ in range(H)] for _ in range(R)]
+    kept_v = [[[] for _ in range(H)] for _ in range(R)]
+    for ci, (cl, kp) in enumerate(zip(chunks, keeps)):
+        n_max = int(cl.max())
+        sc = torch.randn(R, H, n_max, generator=g).numpy()
+        Kc, Vc = torch.randn(R, H, n_max, d, generator=g).bfloat16(), torch.randn(R, H, n_max, d, generator=g).bfloat16()
+        if ci == 0:
+            single, sidx = O.compact_topk(pool, t, sc, bits_(Kc), bits_(Vc), cl, kp)
+        pool, kv, idx = O.compact_topk_chunk(pool, t, sc, bits_(Kc), bits_(Vc), cl, kp, kv)
+        if ci == 0:
+            assert np.array_equal(pool, single) and all(np.array_equal(idx[r][h], sidx[r][h]) for r in range(R) for h in range(H))
+        for r in range(R):
+            for h in range(H):
+                assert idx[r][h].tolist() == O.topk_indices(sc[r, h, :cl[r]], kp[r, h]).tolist()
+                kept_k[r][h].append(Kc[r, h, idx[r][h]]), kept_v[r][h].append(Vc[r, h, idx[r][h]])
+    assert np.array_equal(kv, total)
+    assert (pool != bits_(pool0)).sum() <= int(total.sum()) * 2 * d
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    out, lse, _ = O.attention(q, torch.from_numpy(pool.view(np.int16)).view(torch.bfloat16), t, kv, H * G, d)
+    for r in range(R):
+        for j in range(H * G):
+            Kd, Vd = torch.cat(kept_k[r][j // G]).double(), torch.cat(kept_v[r][j // G]).double()
+            sc_ = (Kd @ q[r, j].double()) / math.sqrt(d)
+            assert np.allclose(out[r, j], (torch.softmax(sc_, 0) @ Vd).numpy(), rtol=0, atol=1e-12)
+    with pytest.raises(ValueError):                      # the tables are full now (:176)
+        O.compact_topk_chunk(pool, t, sc, bits_(Kc), bits_(Vc), chunks[-1], np.full((R, H), 1), kv + 200)
