@@ -283,6 +283,19 @@ int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, con
                          void* kv_pool, int64_t n_pool_pages, int32_t d, int32_t* idx_out, int32_t* clamped_dev,
                          void* workspace, size_t workspace_bytes, void* stream);
 
+/* The same for ONE PREFILL CHUNK -- PAPER.md:152 ("each prefill chunk is compressed as soon as its KV cache is
+ * generated, fully fusing compression into chunked prefill"): scores / k_dense / v_dense hold the chunk
+ * (chunk_len_dev[r] tokens of request r), the keep[r][h] highest-scoring tokens of the chunk are selected as above
+ * and their rows are written to token slots kv_len[r][h] .. kv_len[r][h] + keep - 1 of head h -- behind what the
+ * head already holds -- and kv_len_dev[r][h] (device [R][H] i32, read and updated) grows by keep.  keep is clamped
+ * into [0, min(chunk_len[r], pages(r, cluster) x P - kv_len[r][h])] and clamped heads are counted (:176).
+ * idx_out receives token indices inside the chunk.  All other arguments as for tangram_compact_topk, which is this
+ * call with every kv_len = 0 and no update. */
+int tangram_compact_topk_chunk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
+                               const void* v_dense, int64_t n_max, const int32_t* chunk_len_dev, const int32_t* keep_dev,
+                               int32_t* kv_len_dev, void* kv_pool, int64_t n_pool_pages, int32_t d, int32_t* idx_out,
+                               int32_t* clamped_dev, void* workspace, size_t workspace_bytes, void* stream);
+
 /* ------------------------------------------------------------------------------------------------
  * NEXT-3  Page accounting under a grouping policy (host, pure).  PAPER.md:168 (Fig. 7: a page is freed only when
  * all heads sharing it are evicted; monolithic / ragged / clustered), :190 (a group's page table is sized by its

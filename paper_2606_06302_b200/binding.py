@@ -69,14 +69,15 @@ _lib.tangram_compact_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
 for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram_plan_partitions",
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
               "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk",
-              "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios"):
+              "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios",
+              "tangram_compact_topk_chunk"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
            "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
            "tangram_compact_workspace_bytes", "tangram_compact_topk", "tangram_account_pages",
-           "tangram_calibrate_budgets", "tangram_implicit_ratios")
+           "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk")
 
 
 def _check(rc: int):
@@ -305,10 +306,12 @@ def tangram_compact_workspace_bytes(R: int, H: int) -> int:
 
 
 def tangram_compact_topk(dp: DevicePlan, scores, k_dense, v_dense, ctx_len, keep, kv_pool, idx_out=None,
-                         clamped=None, workspace=None, stream=None):
+                         clamped=None, workspace=None, stream=None, kv_len=None):
     """NEXT-2: per-head Top-keep[r][h] selection on `scores` ([R,H,n_max] f32) and compaction of the selected
     K/V rows ([R,H,n_max,d] bf16 each) into the ragged pages.  ctx_len [R] / keep [R,H] int32 cuda.
-    -> idx_out [R,H,n_max] int32 (first keep[r][h] entries of each row = retained token indices, ascending)."""
+    -> idx_out [R,H,n_max] int32 (first keep[r][h] entries of each row = retained token indices, ascending).
+    With kv_len ([R,H] int32 cuda, updated in place) the call is tangram_compact_topk_chunk: the tensors hold one
+    prefill chunk (ctx_len = chunk lengths) and the rows are appended behind the kv_len tokens already held."""
     import torch
     R, H, n_max, d = k_dense.shape
     assert scores.is_cuda and k_dense.is_cuda and v_dense.is_cuda and kv_pool.is_cuda and ctx_len.is_cuda and keep.is_cuda
@@ -325,12 +328,21 @@ def tangram_compact_topk(dp: DevicePlan, scores, k_dense, v_dense, ctx_len, keep
         workspace = torch.empty(need, dtype=torch.uint8, device=scores.device)
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     cl = C.c_void_p(clamped.data_ptr()) if clamped is not None else None
-    _check(_lib.tangram_compact_topk(C.byref(dp.c), C.c_void_p(scores.data_ptr()), C.c_void_p(k_dense.data_ptr()),
-                                     C.c_void_p(v_dense.data_ptr()), C.c_int64(n_max), C.c_void_p(ctx_len.data_ptr()),
-                                     C.c_void_p(keep.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
-                                     C.c_int64(kv_pool.shape[0]), C.c_int32(d), C.c_void_p(idx_out.data_ptr()), cl,
-                                     C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), sp))
+    tail = (C.c_void_p(kv_pool.data_ptr()), C.c_int64(kv_pool.shape[0]), C.c_int32(d), C.c_void_p(idx_out.data_ptr()), cl,
+            C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), sp)
+    head = (C.byref(dp.c), C.c_void_p(scores.data_ptr()), C.c_void_p(k_dense.data_ptr()), C.c_void_p(v_dense.data_ptr()),
+            C.c_int64(n_max), C.c_void_p(ctx_len.data_ptr()), C.c_void_p(keep.data_ptr()))
+    if kv_len is None:
+        _check(_lib.tangram_compact_topk(*head, *tail))
+    else:
+        assert kv_len.is_cuda and kv_len.dtype == torch.int32 and kv_len.is_contiguous() and kv_len.numel() == R * H
+        _check(_lib.tangram_compact_topk_chunk(*head, C.c_void_p(kv_len.data_ptr()), *tail))
     return idx_out
+
+
+def tangram_compact_topk_chunk(dp: DevicePlan, scores, k_dense, v_dense, chunk_len, keep, kv_len, kv_pool, **kw):
+    """One prefill chunk compressed and appended behind the kv_len tokens every head already holds."""
+    return tangram_compact_topk(dp, scores, k_dense, v_dense, chunk_len, keep, kv_pool, kv_len=kv_len, **kw)
 
 
 class _PageAccount(C.Structure):

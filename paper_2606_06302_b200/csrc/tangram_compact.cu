@@ -33,14 +33,15 @@ constexpr int kSelLongRow = 49152;    // rows longer than this get 1024-thread C
 constexpr int kGatherThreads = 256;
 constexpr int kGatherChunk = 8;      // tiles claimed at once
 
-// Workspace (int32 words): [0] chunk counter, [1] total tiles, [2..3] pad, then keep_eff[n_seq],
-// then tile_indptr[n_seq + 1].
+// Workspace (int32 words): [0] chunk counter, [1] total tiles, [2..3] pad, then keep_eff[n_seq], base[n_seq]
+// (tokens every head held before the call), then tile_indptr[n_seq + 1].
 struct CompactWs {
     int32_t* counter;
     int32_t* keep_eff;
+    int32_t* base;
     int32_t* tile_indptr;
 };
-static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 4 + (size_t)n_seq + (size_t)n_seq + 1; }
+static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 4 + 3 * (size_t)n_seq + 1; }
 
 // fp32 score -> uint32 key with the same order (larger score = larger key); -0.0 and +0.0 compare equal
 // as they do as fp32 values.
@@ -51,22 +52,26 @@ __device__ __forceinline__ uint32_t score_key(float x) {
 
 __global__ void __launch_bounds__(1024)
 compact_prepare_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ ctx_len,
-                       const int32_t* __restrict__ keep, int n_seq, int H, int32_t* __restrict__ counter,
-                       int32_t* __restrict__ keep_eff, int32_t* __restrict__ tile_indptr, int32_t* __restrict__ clamped) {
+                       const int32_t* __restrict__ keep, int32_t* __restrict__ kv_len, int n_seq, int H,
+                       int32_t* __restrict__ counter, int32_t* __restrict__ keep_eff, int32_t* __restrict__ base,
+                       int32_t* __restrict__ tile_indptr, int32_t* __restrict__ clamped) {
     __shared__ int s_warp[32];
     __shared__ int s_run, s_bad;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_run = 0, s_bad = 0;
     __syncthreads();
-    for (int base = 0; base < n_seq; base += blockDim.x) {
-        const int seq = base + tid;
+    for (int first = 0; first < n_seq; first += blockDim.x) {
+        const int seq = first + tid;
         int tiles = 0, bad = 0;
         if (seq < n_seq) {
             const int want = keep[seq];
-            const int cap = min(ctx_len[seq / H], seq_info[seq].y);  // {table row offset, capacity tokens, slot, -}
+            const int have = kv_len ? kv_len[seq] : 0;  // chunked prefill: the rows go behind what the head holds
+            const int cap = min(ctx_len[seq / H], seq_info[seq].y - have);  // {table row offset, capacity tokens, slot, -}
             const int k = max(0, min(want, cap));
             bad = k != want;
             keep_eff[seq] = k;
+            base[seq] = have;
+            if (kv_len) kv_len[seq] = have + k;
             tiles = (k + kCPage - 1) / kCPage;
         }
         int incl = tiles;
@@ -368,7 +373,7 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
                       const int32_t* __restrict__ idx, int64_t n_max, const uint4* __restrict__ k_dense,
                       const uint4* __restrict__ v_dense, uint4* __restrict__ pool, int Hp, int n_seq,
                       int32_t* __restrict__ counter, const int32_t* __restrict__ keep_eff,
-                      const int32_t* __restrict__ tile_indptr) {
+                      const int32_t* __restrict__ base, const int32_t* __restrict__ tile_indptr) {
     constexpr int kChunks = D / 8;           // 16-byte chunks per row
     constexpr int kRowsPerLd = 32 / kChunks;  // rows one warp-wide load covers
     constexpr int kLds = kCPage / kRowsPerLd; // loads per lane for the K rows of a tile (same for V)
@@ -394,15 +399,20 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
         int seq_end = __ldg(tile_indptr + seq + 1);
         for (int tile = first; tile < last; ++tile) {
             while (tile >= seq_end) ++seq, seq_end = __ldg(tile_indptr + seq + 1);  // skips heads that keep nothing
-            const int tl = tile - __ldg(tile_indptr + seq);  // tile inside the sequence = index of its page in the table row
+            const int tl = tile - __ldg(tile_indptr + seq);  // tile inside the sequence: its retained rows 16 tl ..
             const int4 si = __ldg(seq_info + seq);           // {table row offset, capacity tokens, slot, -}
             const int n_rows = min(kCPage, __ldg(keep_eff + seq) - tl * kCPage);
-            const int page = __ldg(tbl_pages + si.x + tl);
+            // lane j < n_rows: source token of the tile's row j and where it goes -- token slot base + 16 tl + j
+            // of the head (with base = 0 the tile is exactly one page; behind an earlier chunk it straddles two)
             int my_tok = 0;
-            if (lane < n_rows) my_tok = __ldg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
-            // pool[page][slot][kv][token][d]
-            const size_t dst_k = ((static_cast<size_t>(page) * Hp + si.z) * 2) * kCPage * kChunks;
-            const size_t dst_v = dst_k + static_cast<size_t>(kCPage) * kChunks;
+            uint32_t my_dst = 0;  // row index in the pool (rows of d elements): < 2^32 for pools up to 550 GB
+            if (lane < n_rows) {
+                my_tok = __ldg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
+                const int pos = __ldg(base + seq) + tl * kCPage + lane;
+                const int page = __ldg(tbl_pages + si.x + pos / kCPage);
+                // pool[page][slot][kv][token][d]: row index of the K row; the V row is kCPage rows further
+                my_dst = ((static_cast<uint32_t>(page) * Hp + si.z) * 2) * kCPage + pos % kCPage;
+            }
             // (at d = 256 a tile goes in two halves of eight rows: 16 + 16 loads would not fit the register budget)
 #pragma unroll
             for (int half = 0; half < kPasses; ++half) {
@@ -420,9 +430,10 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
 #pragma unroll
                 for (int j = 0; j < kLdsP; ++j) {
                     const int row = (half * kLdsP + j) * kRowsPerLd + sub;
+                    const uint32_t dst = __shfl_sync(0xffffffffu, my_dst, row);
                     if (row < n_rows) {
-                        pool[dst_k + row * kChunks + ch] = kreg[j];
-                        pool[dst_v + row * kChunks + ch] = vreg[j];
+                        pool[static_cast<size_t>(dst) * kChunks + ch] = kreg[j];
+                        pool[static_cast<size_t>(dst + kCPage) * kChunks + ch] = vreg[j];
                     }
                 }
             }
@@ -443,11 +454,10 @@ extern "C" size_t tangram_compact_workspace_bytes(int32_t R, int32_t H) {
     return (compact_ws_words((int64_t)R * H) * 4 + 255) / 256 * 256;
 }
 
-extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
-                                    const void* v_dense, int64_t n_max, const int32_t* ctx_len_dev,
-                                    const int32_t* keep_dev, void* kv_pool, int64_t n_pool_pages, int32_t d,
-                                    int32_t* idx_out, int32_t* clamped_dev, void* workspace, size_t workspace_bytes,
-                                    void* stream) {
+static int compact_impl(const tangram_device_plan* dp, const float* scores, const void* k_dense, const void* v_dense,
+                        int64_t n_max, const int32_t* ctx_len_dev, const int32_t* keep_dev, int32_t* kv_len_dev,
+                        void* kv_pool, int64_t n_pool_pages, int32_t d, int32_t* idx_out, int32_t* clamped_dev,
+                        void* workspace, size_t workspace_bytes, void* stream) {
     if (!dp || !scores || !k_dense || !v_dense || !ctx_len_dev || !keep_dev || !kv_pool || !idx_out || !workspace)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: NULL argument");
     if (d != 64 && d != 128 && d != 256)
@@ -467,11 +477,11 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
         return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "compact_topk: workspace %zu < %zu bytes", workspace_bytes, need);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int32_t* ws = static_cast<int32_t*>(workspace);
-    CompactWs w{ws, ws + 4, ws + 4 + n_seq};
+    CompactWs w{ws, ws + 4, ws + 4 + n_seq, ws + 4 + 2 * n_seq};
     const int4* seq_info = reinterpret_cast<const int4*>(dp->seq_info);
 
-    compact_prepare_kernel<<<1, 1024, 0, st>>>(seq_info, ctx_len_dev, keep_dev, n_seq, dp->H, w.counter, w.keep_eff,
-                                               w.tile_indptr, clamped_dev);
+    compact_prepare_kernel<<<1, 1024, 0, st>>>(seq_info, ctx_len_dev, keep_dev, kv_len_dev, n_seq, dp->H, w.counter,
+                                               w.keep_eff, w.base, w.tile_indptr, clamped_dev);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
     if (n_max > kSelLongRow)
@@ -493,7 +503,7 @@ extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* 
             grid = sms * (per_sm > 0 ? per_sm : 1);
         }
         kernel<<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool, dp->Hp, n_seq,
-                                                w.counter, w.keep_eff, w.tile_indptr);
+                                                w.counter, w.keep_eff, w.base, w.tile_indptr);
         return cudaSuccess;
     };
     static thread_local int grid256 = 0, grid128 = 0, grid64 = 0;
@@ -524,4 +534,23 @@ extern "C" int tangram_implicit_ratios(const float* scores, int32_t R, int32_t H
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "implicit ratio launch");
     return TANGRAM_OK;
+}
+
+extern "C" int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
+                                    const void* v_dense, int64_t n_max, const int32_t* ctx_len_dev,
+                                    const int32_t* keep_dev, void* kv_pool, int64_t n_pool_pages, int32_t d,
+                                    int32_t* idx_out, int32_t* clamped_dev, void* workspace, size_t workspace_bytes,
+                                    void* stream) {
+    return compact_impl(dp, scores, k_dense, v_dense, n_max, ctx_len_dev, keep_dev, nullptr, kv_pool, n_pool_pages, d,
+                        idx_out, clamped_dev, workspace, workspace_bytes, stream);
+}
+
+extern "C" int tangram_compact_topk_chunk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
+                                          const void* v_dense, int64_t n_max, const int32_t* chunk_len_dev,
+                                          const int32_t* keep_dev, int32_t* kv_len_dev, void* kv_pool,
+                                          int64_t n_pool_pages, int32_t d, int32_t* idx_out, int32_t* clamped_dev,
+                                          void* workspace, size_t workspace_bytes, void* stream) {
+    if (!kv_len_dev) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk_chunk: NULL kv_len_dev");
+    return compact_impl(dp, scores, k_dense, v_dense, n_max, chunk_len_dev, keep_dev, kv_len_dev, kv_pool, n_pool_pages,
+                        d, idx_out, clamped_dev, workspace, workspace_bytes, stream);
 }

@@ -287,3 +287,64 @@ def test_random_sweep_compaction_and_implicit_ratios():
         cnt, rat = T.tangram_implicit_ratios(scores, torch.from_numpy(wl.ctx_len).cuda(), rho)
         ref_cnt, ref_rat = O.implicit_ratios(scores.cpu().numpy(), wl.ctx_len, rho)
         assert np.array_equal(cnt.cpu().numpy(), ref_cnt) and rat.cpu().numpy().tobytes() == ref_rat.tobytes(), case
+
+
+@pytest.mark.parametrize("seed,d,C", [(81, 128, 2), (82, 64, 4), (83, 256, 1)])
+def test_chunked_prefill_compaction_bit_exact(seed, d, C):
+    """Compression fused into chunked prefill (:152): four chunks of ragged lengths compressed one after the other,
+    each appended behind the previous ones (chunk boundaries fall inside pages); pool, lengths and index lists
+    bit-exact against oracle O11 after every chunk; then decode attention over the result; then an over-full
+    chunk is clamped and counted."""
+    R, H = 3, 4
+    rng = np.random.default_rng(seed)
+    wl = I.make_random_workload(seed, R=R, H=H, G=2, d=d, C=C, max_ctx=100)
+    chunk_lens = [rng.integers(1, 700, size=R).astype(np.int32) for _ in range(4)]
+    ratios = rng.uniform(0.05, 1.0, size=H)
+    keeps = [np.minimum(cl[:, None], np.ceil(cl[:, None] * ratios[None, :] * rng.uniform(0.5, 1.0, size=(R, H)))).astype(np.int32)
+             for cl in chunk_lens]
+    keeps[1][0, 1] = 0
+    total = sum(keeps)
+    B = np.clip(total.max(0) / sum(chunk_lens).max(), 0.01, 1.0)
+    need = T.tangram_pages_needed(B, total, C, 16)
+    t, _ = T.tangram_build_ragged_tables(B, total, C, 16, np.random.default_rng(seed).permutation(need + 3).astype(np.int32))
+    pl = T.tangram_plan_partitions(t, B, total, 148, 64, 1, T.MODE_BALANCED, 0, T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS)
+    dp = T.tangram_upload(t, pl)
+    g = torch.Generator(device="cuda").manual_seed(seed)
+    pool = torch.randn(need + 3, t.Hp, 2, 16, d, generator=g, device="cuda").bfloat16()
+    ref_pool, ref_kv = bits(pool).copy(), np.zeros((R, H), dtype=np.int32)
+    kv_dev = torch.zeros(R, H, dtype=torch.int32, device="cuda")
+    clamped = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for cl, kp in zip(chunk_lens, keeps):
+        n_max = int(cl.max()) + 1
+        scores = torch.randn(R, H, n_max, generator=g, device="cuda").exp().bfloat16().float()
+        kd = torch.randn(R, H, n_max, d, generator=g, device="cuda").bfloat16()
+        vd = torch.randn(R, H, n_max, d, generator=g, device="cuda").bfloat16()
+        idx = torch.full((R, H, n_max), -7, dtype=torch.int32, device="cuda")
+        T.tangram_compact_topk_chunk(dp, scores, kd, vd, torch.from_numpy(cl).cuda(), torch.from_numpy(kp).cuda(), kv_dev,
+                                     pool, idx_out=idx, clamped=clamped)
+        torch.cuda.synchronize()
+        ref_pool, ref_kv, ref_idx = O.compact_topk_chunk(ref_pool, otables(t), scores.cpu().numpy(), bits(kd), bits(vd), cl,
+                                                         kp, ref_kv)
+        assert np.array_equal(bits(pool), ref_pool) and np.array_equal(kv_dev.cpu().numpy(), ref_kv)
+        gi = idx.cpu().numpy()
+        for r in range(R):
+            for h in range(H):
+                assert np.array_equal(gi[r, h, :kp[r, h]], ref_idx[r][h]) and (gi[r, h, kp[r, h]:] == -7).all()
+    assert int(clamped.item()) == 0 and np.array_equal(ref_kv, total)
+    q = torch.randn(R, H * 2, d, generator=g, device="cuda").bfloat16()
+    out, lse = T.tangram_decode_attention(dp, q, pool)
+    torch.cuda.synchronize()
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), otables(t), total, H * 2, d)
+    got = out.float().cpu().numpy().astype(np.float64)
+    assert np.abs(got - ref_out).max() <= 2e-2 and np.linalg.norm(got - ref_out) / np.linalg.norm(ref_out) <= 5e-3
+    assert np.abs(lse.cpu().numpy() - ref_lse).max() <= 1e-3
+    # one more chunk does not fit any more: every head is clamped to the room its table has left (:176)
+    rows = np.arange(R)[:, None] * t.C + t.cluster_of[None, :]
+    room = ((t.tbl_indptr[rows + 1] - t.tbl_indptr[rows]) * 16 - total).astype(np.int32)
+    cl, kp = chunk_lens[0], np.minimum(chunk_lens[0][:, None], room + 5).astype(np.int32)
+    eff = np.minimum(kp, room)
+    T.tangram_compact_topk_chunk(dp, scores[:, :, :int(cl.max())].contiguous(), kd[:, :, :int(cl.max())].contiguous(),
+                                 vd[:, :, :int(cl.max())].contiguous(), torch.from_numpy(cl).cuda(),
+                                 torch.from_numpy(kp).cuda(), kv_dev, pool, clamped=clamped)
+    torch.cuda.synchronize()
+    assert int(clamped.item()) == int((eff != kp).sum()) and np.array_equal(kv_dev.cpu().numpy(), total + eff)
