@@ -209,3 +209,17 @@ def test_calibrate_then_reserve_pipeline_and_errors():
         T.tangram_calibrate_budgets(np.array([[np.nan]]), 2.0)
     with pytest.raises(T.TangramError):
         T.tangram_calibrate_budgets(np.zeros((0, 3)), 2.0)
+
+
+def test_header_is_plain_c_and_host_path_runs_from_c(tmp_path):
+    """include/tangram.h compiles as strict C99 and a plain C program drives the host side of the path through
+    the shared library (no Python, no torch types): hand-evaluated values of a1 / a2 / a3 / NEXT-3 / NEXT-4."""
+    import subprocess
+    src = os.path.join(ROOT, "tests", "c_abi", "host_path.c")
+    exe = str(tmp_path / "host_path")
+    libdir = os.path.dirname(T.LIB_PATH)
+    subprocess.check_call(["gcc", "-std=c99", "-pedantic", "-Wall", "-Wextra", "-Werror", "-I", os.path.join(ROOT, "include"),
+                           src, "-o", exe, "-L", libdir, "-ltangram", "-Wl,-rpath," + libdir])
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0, out.stderr
+    assert "c_abi host path ok" in out.stdout
