@@ -471,3 +471,22 @@ def test_head_dim_256_gemma_shaped_layer_with_append():
         assert np.array_equal(bits(pool), pool_bits) and np.array_equal(kv_dev.cpu().numpy(), kv_ref)
         ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv_ref, wl.Hq, wl.d)
         check(out, lse, ref_out, ref_lse, f"d=256 decode step {step}")
+
+
+def test_whole_path_from_plain_c(tmp_path):
+    """The C ABI end to end from a plain C program (CUDA runtime C API + include/tangram.h, no Python / torch in
+    the process): closed-form outputs (q = 0, V_h = h + 1, NaN in every slot that is not a retained row)."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    src = os.path.join(root, "tests", "c_abi", "device_path.c")
+    exe = str(tmp_path / "device_path")
+    libdir = os.path.dirname(T.LIB_PATH)
+    cuda = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-I", os.path.join(root, "include"),
+                           "-I", os.path.join(cuda, "include"), src, "-o", exe, "-L", libdir, "-ltangram",
+                           "-L", os.path.join(cuda, "lib64"), "-lcudart", "-lm",
+                           "-Wl,-rpath," + libdir, "-Wl,-rpath," + os.path.join(cuda, "lib64")])
+    out = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0, out.stderr + out.stdout
+    assert "c_abi device path ok" in out.stdout
