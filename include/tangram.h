@@ -214,6 +214,8 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *             {start, end of its work lists, grid barrier passed, merges done} (the last two only when
  *             the merge runs inside the decode grid); the per-CTA elapsed-time spread of BASELINE.json
  *             is measured from the first two.
+ * A device plan carries the launch's scheduler counters: launches on the SAME plan must be ordered (one stream, or
+ * events between streams); different plans (e.g. one per layer) may run concurrently.
  * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
  * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G), BUFFER_TOO_SMALL (workspace), CUDA. */
