@@ -182,6 +182,8 @@ typedef struct tangram_device_plan {
     int32_t* sched;               /* device [4]: list-claim / CTAs-done counters of the dynamic tail and the
                                      grid-barrier counters of the in-kernel merge; zero between launches
                                      (the kernel re-arms them itself) */
+    int64_t min_pool_pages;       /* largest page id in the tables + 1: the device calls return INVALID_ARG for a
+                                     kv_pool with fewer pages */
 } tangram_device_plan;
 
 /* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte
@@ -218,7 +220,8 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  * events between streams); different plans (e.g. one per layer) may run concurrently.
  * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
- * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G), BUFFER_TOO_SMALL (workspace), CUDA. */
+ * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G / n_pool_pages <= a page id of the tables),
+ * BUFFER_TOO_SMALL (workspace), CUDA. */
 int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
                              int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d,
                              float sm_scale, void* out,

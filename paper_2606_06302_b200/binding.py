@@ -57,7 +57,8 @@ class _DevicePlan(C.Structure):
                 ("n_part_slots", C.c_int64), ("n_merge_seqs", C.c_int64), ("n_empty_seqs", C.c_int64), ("n_big_merge_seqs", C.c_int64),
                 ("merge_seqs", C.c_void_p),
                 ("items", C.c_void_p), ("worker_indptr", C.c_void_p), ("list_heads", C.c_void_p),
-                ("seq_info", C.c_void_p), ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p)]
+                ("seq_info", C.c_void_p), ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p),
+                ("min_pool_pages", C.c_int64)]
 
 
 _lib.tangram_last_error.restype = C.c_char_p

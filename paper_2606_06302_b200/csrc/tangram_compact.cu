@@ -463,7 +463,7 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kCPage) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: page size %d (kernels need 16)", dp->P);
-    if (n_max < 1 || n_max > (1 << 30) || n_pool_pages < 1)
+    if (n_max < 1 || n_max > (1 << 30) || n_pool_pages < 1 || n_pool_pages < dp->min_pool_pages)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: n_max=%lld n_pool_pages=%lld", (long long)n_max,
                     (long long)n_pool_pages);
     if (reinterpret_cast<uintptr_t>(k_dense) % 16 || reinterpret_cast<uintptr_t>(v_dense) % 16 ||

@@ -875,6 +875,11 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     off += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
     const size_t off_pages = off;
     std::memcpy(host.data() + off, t->tbl_pages, sizeof(int32_t) * (size_t)t->n_pages_used);
+    int64_t max_page = -1;
+    for (int64_t i = 0; i < t->n_pages_used; ++i) {
+        if (t->tbl_pages[i] < 0) return fail(TANGRAM_ERR_INVALID_ARG, "upload: negative page id in the tables");
+        max_page = std::max<int64_t>(max_page, t->tbl_pages[i]);
+    }
     off += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
     const size_t off_mseq = off;
     int32_t* mseq = reinterpret_cast<int32_t*>(host.data() + off);
@@ -939,6 +944,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     uint8_t* base = static_cast<uint8_t*>(dev_blob);
     dp->R = t->R, dp->H = t->H, dp->C = t->C, dp->Hp = t->Hp, dp->P = t->P, dp->W = n_dev_lists, dp->mode = p->mode;
     dp->n_static = p->n_static;
+    dp->min_pool_pages = max_page + 1;
     dp->sched = reinterpret_cast<int32_t*>(base + off_sched);
     dp->merge_seqs = reinterpret_cast<const int32_t*>(base + off_mseq);
     dp->n_merge_seqs = n_mseq;
@@ -970,6 +976,9 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d)", Hq,
                     dp->H, kMaxG);
     if (n_pool_pages < 1 || dp->W < 1 || dp->n_static < 1 || dp->n_static > dp->W) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool or plan");
+    if ((which & kRunSplit) && n_pool_pages < dp->min_pool_pages)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: kv_pool has %lld pages, the tables use page id %lld",
+                    (long long)n_pool_pages, (long long)dp->min_pool_pages - 1);
     if (reinterpret_cast<uintptr_t>(q) % 16 || reinterpret_cast<uintptr_t>(kv_pool) % 128 ||
         reinterpret_cast<uintptr_t>(out) % 16 || reinterpret_cast<uintptr_t>(workspace) % 16)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: misaligned pointer");
@@ -1042,7 +1051,9 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: page size %d (kernels need 16)", dp->P);
-    if (n_pool_pages < 1) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: empty pool");
+    if (n_pool_pages < 1 || n_pool_pages < dp->min_pool_pages)
+        return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: kv_pool has %lld pages, the tables need %lld", (long long)n_pool_pages,
+                    (long long)dp->min_pool_pages);
     if (reinterpret_cast<uintptr_t>(k_new) % 16 || reinterpret_cast<uintptr_t>(v_new) % 16 ||
         reinterpret_cast<uintptr_t>(kv_pool) % 16)
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: misaligned pointer");

@@ -228,6 +228,15 @@ def test_device_error_contract():
     with pytest.raises(T.TangramError) as e:
         T.tangram_decode_attention(dp, q3, pool)
     assert e.value.code == T.ERR_INVALID_ARG
+    short = pool[:int(t.tbl_pages.max())]                                          # one page fewer than the tables use
+    assert int(dp.c.min_pool_pages) == int(t.tbl_pages.max()) + 1
+    for call in (lambda: T.tangram_decode_attention(dp, q, short),
+                 lambda: T.tangram_append_kv(dp, torch.zeros(wl.R, wl.H, wl.d, device="cuda").bfloat16(),
+                                             torch.zeros(wl.R, wl.H, wl.d, device="cuda").bfloat16(), short,
+                                             torch.zeros(wl.R, wl.H, dtype=torch.int32, device="cuda"))):
+        with pytest.raises(T.TangramError) as e:
+            call()
+        assert e.value.code == T.ERR_INVALID_ARG
 
 
 @pytest.mark.parametrize("name", ["8b", "32b", "skew", "uniform"])
