@@ -348,3 +348,29 @@ def test_chunked_prefill_compaction_bit_exact(seed, d, C):
                                  torch.from_numpy(kp).cuda(), kv_dev, pool, clamped=clamped)
     torch.cuda.synchronize()
     assert int(clamped.item()) == int((eff != kp).sum()) and np.array_equal(kv_dev.cpu().numpy(), total + eff)
+
+
+def test_global_flat_topk_compression_as_a_composition():
+    """The non-uniform compressor of Eq. 3 run on the device: implicit per-head counts (tangram_implicit_ratios)
+    fed as `keep` into the per-head compaction reproduce the global flat Top-k selection (oracle: one flat sort)."""
+    wl = I.make_random_workload(91, R=3, H=4, G=1, d=64, C=1, max_ctx=1500)
+    wl.mu[:] = 1.0                                        # tables sized for the whole context: any split fits
+    wl.demand = np.repeat(wl.ctx_len[:, None], wl.H, 1).astype(np.int32)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    scores *= torch.tensor([0.4, 1.0, 2.5, 0.7], device="cuda")[None, :, None]
+    ctx_dev = torch.from_numpy(wl.ctx_len).cuda()
+    cnt, _ = T.tangram_implicit_ratios(scores, ctx_dev, 0.3)
+    _, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    idx = T.tangram_compact_topk(dp, scores, kd, vd, ctx_dev, cnt, pool)
+    torch.cuda.synchronize()
+    sc, gi, c = scores.cpu().numpy(), idx.cpu().numpy(), cnt.cpu().numpy()
+    for r in range(wl.R):
+        N = int(wl.ctx_len[r])
+        flat = np.concatenate([sc[r, h, :N] for h in range(wl.H)])
+        sel = O.topk_indices(flat, int(math.ceil(0.3 * wl.H * N)))
+        assert c[r].sum() == len(sel)
+        for h in range(wl.H):
+            mine = sel[(sel >= h * N) & (sel < (h + 1) * N)] - h * N
+            assert np.array_equal(gi[r, h, :c[r, h]], mine)

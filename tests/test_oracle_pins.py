@@ -725,3 +725,22 @@ def test_compact_topk_chunk_round_trip_and_single_chunk_case():
             assert np.allclose(out[r, j], (torch.softmax(sc_, 0) @ Vd).numpy(), rtol=0, atol=1e-12)
     with pytest.raises(ValueError):                      # the tables are full now (:176)
         O.compact_topk_chunk(pool, t, sc, bits_(Kc), bits_(Vc), chunks[-1], np.full((R, H), 1), kv + 200)
+
+
+def test_global_flat_topk_equals_per_head_topk_with_its_own_counts():
+    """Eq. 3 decomposes exactly: the global flat Top-k set, split by head, is each head's Top-(its implicit count)
+    under the same tie rule -- so the non-uniform compressor Tangram replaces (and Eq. 2, keep = ceil(rho N) for
+    every head) are the per-head selection of Eq. 4 with particular `keep` inputs."""
+    rng = np.random.default_rng(23)
+    R, H, n_max = 2, 5, 60
+    ctx = np.array([60, 41])
+    sc = rng.integers(0, 7, size=(R, H, n_max)).astype(np.float32) * rng.uniform(0.5, 2.0, size=(1, H, 1)).astype(np.float32)
+    for rho in (0.1, 0.45, 0.8):
+        cnt, _ = O.implicit_ratios(sc, ctx, rho)
+        for r in range(R):
+            N = int(ctx[r])
+            flat = np.concatenate([sc[r, h, :N] for h in range(H)])
+            sel = O.topk_indices(flat, int(cnt[r].sum()))
+            for h in range(H):
+                mine = sel[(sel >= h * N) & (sel < (h + 1) * N)] - h * N
+                assert mine.tolist() == O.topk_indices(sc[r, h, :N], int(cnt[r, h])).tolist()
