@@ -241,9 +241,12 @@ def test_compact_topk_is_graph_capturable_and_repeatable():
     keep = torch.from_numpy(kv.astype(np.int32)).cuda()
     ctx = torch.from_numpy(wl.ctx_len).cuda()
     idx = torch.empty(wl.R, wl.H, n_max, dtype=torch.int32, device="cuda")
-    ws = torch.empty(T.tangram_compact_workspace_bytes(wl.R, wl.H), dtype=torch.uint8, device="cuda")
+    need = T.tangram_compact_workspace_bytes(wl.R, wl.H)
+    ws_guarded = torch.full((need + 512,), 0xAB, dtype=torch.uint8, device="cuda")   # 256-byte guards on both sides
+    ws = ws_guarded[256:256 + need]
     T.tangram_compact_topk(dp, scores, kd, vd, ctx, keep, pool, idx_out=idx, workspace=ws)
     torch.cuda.synchronize()
+    assert bool((ws_guarded[:256] == 0xAB).all()) and bool((ws_guarded[256 + need:] == 0xAB).all())
     want = bits(pool).copy()
     st = torch.cuda.Stream()
     st.wait_stream(torch.cuda.current_stream())
