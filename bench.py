@@ -486,8 +486,9 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
     of the serving system (written by prefill, like weights) and stays in HBM.
     zero_copy=True: out / lse are HOST pointers passed straight into the C-ABI call -- pinned memory is mapped into
     the device's address space and the kernel's (posted) stores go over the bus, so the result never waits for a
-    copy engine; q is staged with one H2D copy (reading q in place from host memory works too, the binding and
-    tests cover it, but every item then waits a bus round trip for its query group: 154 us against 146 us).
+    copy engine; q is pulled from pinned host memory by tangram_stage_from_host (a kernel, not a copy-engine
+    transfer; reading q in place from host memory inside the decode kernel works too, the binding and tests
+    cover it, but every item then waits a bus round trip for its query group: 154 us).
     zero_copy=False: explicit staging copies around the call (one H2D, one D2H)."""
     q_host = S["q"].cpu().pin_memory()
     R, Hq, d = S["q"].shape
@@ -500,7 +501,7 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
         q_dev = torch.empty_like(S["q"])
 
         def step():
-            q_dev.copy_(q_host, non_blocking=True)
+            T.tangram_stage_from_host(q_dev, q_host)
             T.tangram_decode_attention(S["dp"], q_dev, S["pool"], out_host, lse_host, S["ws"])
     else:
         # out and lse live in ONE device allocation, so the result goes back with a single device->host copy
@@ -612,9 +613,10 @@ def main():
         "e2e": {"value": e_bytes / (e_ms * 1e-3) / 1e12, "unit": "TB/s", "us_per_layer_step": e_ms * 1e3,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "us_per_layer_step_staged_copies": float(np.mean(ems_staged) * 1e3),
-                "note": "every step: q copied from pinned host memory (H2D), out+lse written by the kernel straight "
-                        "into pinned, device-mapped host memory (host pointers passed to the C-ABI call), all inside "
-                        "the timed region; `staged_copies` = the same with an explicit D2H copy after the call; "
+                "note": "every step: q pulled from pinned host memory by tangram_stage_from_host (H2D over the bus), "
+                        "out+lse written by the kernel straight into pinned, device-mapped host memory (host pointers "
+                        "passed to the C-ABI call), all inside the timed region; `staged_copies` = the same with "
+                        "copy-engine transfers (one H2D before, one D2H after the call); "
                         "the KV page pool is resident serving state in HBM"},
         # one cooperative launch per step (the merge runs inside the decode grid); the stand-alone merge
         # kernel is only launched when the grid cannot be co-resident, which bench.py never asks for

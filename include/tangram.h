@@ -228,6 +228,15 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
                              float* lse, void* workspace, size_t workspace_bytes,
                              uint64_t* worker_ns, void* stream);
 
+/* Host buffers.  q, out and lse of tangram_decode_attention may be PINNED host memory (page-locked memory is mapped
+ * into the device's address space under unified addressing): the kernel then reads / writes them in place over the
+ * bus.  Writing out / lse that way costs nothing (posted stores); reading q in place makes every item wait a bus
+ * round trip for its query group, so for q this helper is the better way: it copies `bytes` (a multiple of 16) from
+ * pinned host memory `src_host` to device memory `dst_dev` with a kernel on `stream` -- for the few hundred KB of a
+ * decode step ~10 us sooner than a copy-engine transfer plus its stream hand-off.  Errors: INVALID_ARG (NULL,
+ * alignment, source not page-locked), CUDA. */
+int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream);
+
 /* The two kernels of tangram_decode_attention as separate calls (same arguments, same checks):
  * a4 alone (split-KV decode kernel: final outputs of single-part sequences, fp32 partials of the
  * others into `workspace`) and a5 alone (LSE merge of the partials in `workspace` into out / lse;

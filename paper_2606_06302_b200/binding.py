@@ -71,14 +71,15 @@ for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
               "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk",
               "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios",
-              "tangram_compact_topk_chunk"):
+              "tangram_compact_topk_chunk", "tangram_stage_from_host"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
            "tangram_plan_partitions", "tangram_query_max_ctas", "tangram_blob_bytes", "tangram_upload",
            "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
            "tangram_compact_workspace_bytes", "tangram_compact_topk", "tangram_account_pages",
-           "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk")
+           "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk",
+           "tangram_stage_from_host")
 
 
 def _check(rc: int):
@@ -386,3 +387,14 @@ def tangram_implicit_ratios(scores, ctx_len, rho: float, stream=None):
                                         C.c_void_p(ctx_len.data_ptr()), C.c_double(rho), C.c_void_p(counts.data_ptr()),
                                         C.c_void_p(ratios.data_ptr()), sp))
     return counts, ratios
+
+
+def tangram_stage_from_host(dst, src, stream=None):
+    """dst (cuda tensor) <- src (pinned host tensor of the same size), copied by a kernel on the stream."""
+    import torch
+    assert dst.is_cuda and src.is_pinned() and dst.is_contiguous() and src.is_contiguous()
+    nbytes = dst.numel() * dst.element_size()
+    assert nbytes == src.numel() * src.element_size()
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    _check(_lib.tangram_stage_from_host(C.c_void_p(dst.data_ptr()), C.c_void_p(src.data_ptr()), C.c_size_t(nbytes), sp))
+    return dst

@@ -700,6 +700,17 @@ tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
     if (lane == 0) kv_len[seq] = n + 1;
 }
 
+// ------------------------------------------------------------------ staging small host buffers
+// dst (device) <- src (pinned, device-mapped host memory), 16 bytes per thread and step.  For the few hundred KB of
+// a decode step's queries a kernel that pulls the bytes over the bus is ready ~10 us sooner than a copy-engine
+// transfer and its stream hand-off to the next kernel.
+__global__ void __launch_bounds__(256)
+tangram_stage_kernel(uint4* __restrict__ dst, const uint4* __restrict__ src, size_t n16) {
+    for (size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n16;
+         i += static_cast<size_t>(gridDim.x) * blockDim.x)
+        dst[i] = src[i];
+}
+
 // ------------------------------------------------------------------ host-side launch helpers
 static int cuda_fail(cudaError_t e, const char* what) {
     return fail(TANGRAM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
@@ -1063,5 +1074,25 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
         static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream) {
+    if (!dst_dev || !src_host) return fail(TANGRAM_ERR_INVALID_ARG, "stage_from_host: NULL argument");
+    if (bytes % 16 || reinterpret_cast<uintptr_t>(dst_dev) % 16 || reinterpret_cast<uintptr_t>(src_host) % 16)
+        return fail(TANGRAM_ERR_INVALID_ARG, "stage_from_host: pointers and size must be multiples of 16 bytes");
+    if (bytes == 0) return TANGRAM_OK;
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, src_host);
+    if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged && at.type != cudaMemoryTypeDevice)) {
+        (void)cudaGetLastError();
+        return fail(TANGRAM_ERR_INVALID_ARG, "stage_from_host: the source is not page-locked (device-mapped) memory");
+    }
+    const size_t n16 = bytes / 16;
+    const unsigned grid = static_cast<unsigned>(std::min<size_t>((n16 + 255) / 256, 592));
+    tangram_stage_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(static_cast<uint4*>(dst_dev),
+                                                                            static_cast<const uint4*>(src_host), n16);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "stage kernel launch");
     return TANGRAM_OK;
 }

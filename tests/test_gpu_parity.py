@@ -499,3 +499,18 @@ def test_whole_path_from_plain_c(tmp_path):
     out = subprocess.run([exe], capture_output=True, text=True, timeout=120)
     assert out.returncode == 0, out.stderr + out.stdout
     assert "c_abi device path ok" in out.stdout
+
+
+def test_stage_from_host():
+    src = torch.randn(3, 40, 128).bfloat16().pin_memory()
+    dst = torch.zeros(3, 40, 128, dtype=torch.bfloat16, device="cuda")
+    T.tangram_stage_from_host(dst, src)
+    torch.cuda.synchronize()
+    assert torch.equal(dst.cpu(), src)
+    big = torch.randint(0, 255, (5 << 20,), dtype=torch.uint8).pin_memory()       # more 16-byte words than threads
+    out = torch.zeros_like(big, device="cuda")
+    T.tangram_stage_from_host(out, big)
+    assert torch.equal(out.cpu(), big)
+    with pytest.raises(T.TangramError):                                              # pageable memory is refused
+        T._check(T._lib.tangram_stage_from_host(T.C.c_void_p(dst.data_ptr()), T.C.c_void_p(torch.zeros(64).data_ptr()),
+                                                T.C.c_size_t(64), None))
