@@ -19,14 +19,24 @@ def bits(x):
 
 
 def otables(t):
+    if getattr(t, "oracle_side", None) is not None:
+        return t.oracle_side
     return O.Tables(R=t.R, H=t.H, C=t.C, Hp=t.Hp, P=t.P, perm=t.perm, cluster_of=t.cluster_of, slot_of=t.slot_of,
                     tbl_indptr=t.tbl_indptr, tbl_pages=t.tbl_pages, n_pages_used=t.n_pages_used)
 
 
 def setup(wl):
+    """Tables through the product's C ABI and, independently, through the oracle (bit-exact agreement asserted);
+    the oracle later works on its own copy."""
     B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
     n_pool = int(math.ceil(1.05 * T.tangram_pages_needed(B, res, wl.C, wl.P))) + 1
-    t, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, I.make_free_pages(wl, n_pool), 0, kv)
+    free = I.make_free_pages(wl, n_pool)
+    t, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, free, 0, kv)
+    Bo, reso, kvo = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    to, kvo = O.build_ragged_tables(Bo, reso, wl.C, wl.P, free, 0, kvo)
+    assert np.array_equal(kvo, kv) and all(np.array_equal(getattr(to, f), getattr(t, f))
+                                           for f in ("perm", "cluster_of", "slot_of", "tbl_indptr", "tbl_pages"))
+    t.oracle_side = to          # the oracle's own, independently built tables
     pl = T.tangram_plan_partitions(t, B, kv, 8, wl.granule, 1, T.MODE_BALANCED)
     return B, res, kv, t, n_pool, T.tangram_upload(t, pl)
 

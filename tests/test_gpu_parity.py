@@ -19,15 +19,25 @@ DYN_PERMILLE, DYN_ROUNDS = T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS     # be
 
 
 def setup(wl, flags=0, identity=False):
+    """Budgets, tables through the product's C ABI -- and, independently, through the oracle: the two must agree
+    bit for bit, and everything the oracle is given later (tables, lengths) is the ORACLE's own copy."""
     B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
     need = T.tangram_pages_needed(B, res, wl.C, wl.P)
     n_pool = int(math.ceil(1.05 * need))
     free = I.make_free_pages(wl, n_pool, identity=identity)
     t, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, free, flags, kv)
+    Bo, reso, kvo = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    to, kvo = O.build_ragged_tables(Bo, reso, wl.C, wl.P, free, flags, kvo)
+    assert Bo.tobytes() == B.tobytes() and np.array_equal(reso, res) and np.array_equal(kvo, kv)
+    for f in ("perm", "cluster_of", "slot_of", "tbl_indptr", "tbl_pages"):
+        assert np.array_equal(getattr(to, f), getattr(t, f)), f
+    t.oracle_side = to          # the oracle's own, independently built tables
     return B, res, kv, t, n_pool
 
 
 def oracle_tables(t):
+    if getattr(t, "oracle_side", None) is not None:
+        return t.oracle_side
     return O.Tables(R=t.R, H=t.H, C=t.C, Hp=t.Hp, P=t.P, perm=t.perm, cluster_of=t.cluster_of, slot_of=t.slot_of,
                     tbl_indptr=t.tbl_indptr, tbl_pages=t.tbl_pages, n_pages_used=t.n_pages_used)
 
