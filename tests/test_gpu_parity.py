@@ -524,3 +524,39 @@ def test_stage_from_host():
     with pytest.raises(T.TangramError):                                              # pageable memory is refused
         T._check(T._lib.tangram_stage_from_host(T.C.c_void_p(dst.data_ptr()), T.C.c_void_p(torch.zeros(64).data_ptr()),
                                                 T.C.c_size_t(64), None))
+
+
+def test_page_ids_at_the_top_of_a_24_gb_pool():
+    """Maximum sizes: the tables point at the highest page ids of a 1.5 M-page (24.6 GB) pool, i.e. byte offsets far
+    beyond 2^32 and TMA row coordinates near 10^8; append, compaction and attention must address them correctly.
+    The oracle works on the small pool of the used pages with the same pages numbered 0, 1, 2, ... (page-permutation
+    invariance is one of its pins)."""
+    n_big = 1_500_000
+    wl = I.make_random_workload(101, R=2, H=4, G=4, d=128, C=2, max_ctx=3000)
+    B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    need = T.tangram_pages_needed(B, res, wl.C, wl.P)
+    top = np.arange(n_big - 1, n_big - 1 - need, -1, dtype=np.int32)            # highest ids first
+    t, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, top, 0, kv)
+    to, kvo = O.build_ragged_tables(*O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)[:2], wl.C, wl.P,
+                                    np.arange(need, dtype=np.int32), 0, kv.copy())
+    assert np.array_equal(t.tbl_pages, top[to.tbl_pages]) and np.array_equal(t.tbl_indptr, to.tbl_indptr)
+    q, small = I.make_q_and_pool(wl, need, "cuda")
+    big = torch.empty(n_big, t.Hp, 2, wl.P, wl.d, dtype=torch.bfloat16, device="cuda")
+    assert big.numel() * 2 > 24 * 10 ** 9
+    big[torch.from_numpy(top.astype(np.int64)).cuda()] = small
+    pl = T.tangram_plan_partitions(t, B, kv, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dp = T.tangram_upload(t, pl)
+    assert int(dp.c.min_pool_pages) == n_big
+    out, lse = T.tangram_decode_attention(dp, q, big)
+    torch.cuda.synchronize()
+    ref_out, ref_lse, _ = O.attention(q.cpu(), small.cpu(), to, kvo, wl.Hq, wl.d)
+    check(out, lse, ref_out, ref_lse, "24 GB pool")
+    # compaction writes to the same far pages: bit-exact against the oracle on the small pool
+    n_max = int(wl.ctx_len.max())
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    T.tangram_compact_topk(dp, scores, kd, vd, torch.from_numpy(wl.ctx_len).cuda(), torch.from_numpy(kv.astype(np.int32)).cuda(), big)
+    torch.cuda.synchronize()
+    ref_pool, _ = O.compact_topk(bits(small), to, scores.cpu().numpy(), bits(kd), bits(vd), wl.ctx_len, kvo)
+    assert np.array_equal(bits(big[torch.from_numpy(top.astype(np.int64)).cuda()]), ref_pool)
+    del big
+    torch.cuda.empty_cache()
