@@ -560,3 +560,23 @@ def test_page_ids_at_the_top_of_a_24_gb_pool():
     assert np.array_equal(bits(big[torch.from_numpy(top.astype(np.int64)).cuda()]), ref_pool)
     del big
     torch.cuda.empty_cache()
+
+
+def test_one_million_token_sequence():
+    """Maximum sizes: one KV head that retains 2^20 tokens (65 536 pages; the whole batch is one sequence cut into
+    ~1000 parts across all SMs, merged by the big-record path), GQA 8, against the oracle."""
+    wl = I.make_random_workload(111, R=1, H=1, G=8, d=128, C=1, max_ctx=10)
+    wl.ctx_len[:] = 1 << 20
+    wl.mu[:], wl.sigma[:] = 1.0, 0.0
+    wl.demand = np.full((1, 1), 1 << 20, dtype=np.int32)
+    B, res, kv, t, n_pool = setup(wl)
+    assert int(kv[0, 0]) == 1 << 20
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    pl = T.tangram_plan_partitions(t, B, kv, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    assert pl.n_items > 500
+    dp = T.tangram_upload(t, pl)
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    for _ in range(2):
+        out, lse = T.tangram_decode_attention(dp, q, pool)
+        torch.cuda.synchronize()
+        check(out, lse, ref_out, ref_lse, "2^20 tokens")
