@@ -182,6 +182,7 @@ typedef struct tangram_device_plan {
     int32_t* sched;               /* device [4]: list-claim / CTAs-done counters of the dynamic tail and the
                                      grid-barrier counters of the in-kernel merge; zero between launches
                                      (the kernel re-arms them itself) */
+    int64_t max_merge_parts;      /* most parts any sequence has (sizes the column split of the big-record merge) */
     int64_t min_pool_pages;       /* largest page id in the tables + 1: the device calls return INVALID_ARG for a
                                      kv_pool with fewer pages */
 } tangram_device_plan;

@@ -58,7 +58,7 @@ class _DevicePlan(C.Structure):
                 ("merge_seqs", C.c_void_p),
                 ("items", C.c_void_p), ("worker_indptr", C.c_void_p), ("list_heads", C.c_void_p),
                 ("seq_info", C.c_void_p), ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p),
-                ("min_pool_pages", C.c_int64)]
+                ("max_merge_parts", C.c_int64), ("min_pool_pages", C.c_int64)]
 
 
 _lib.tangram_last_error.restype = C.c_char_p

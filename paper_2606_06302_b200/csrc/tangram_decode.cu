@@ -67,7 +67,7 @@ struct DecodeParams {
     const int32_t* kv_len;      // [R*H] run-time lengths (open-ended plan) or nullptr: items are taken as planned
     int32_t H;
     int32_t Hq, G, Hp, n_stages, n_lists;
-    int32_t tail_merge, n_merge_units, n_merge_small;
+    int32_t tail_merge, n_merge_units, n_merge_small, merge_split;
     float scale_log2;
 };
 
@@ -188,12 +188,86 @@ constexpr int kMergeThreads = 512;
 constexpr int kMergeBigParts = 32;
 
 struct MergeUnit {
-    int seq, p0, n, g;  // g < 0: all query heads of the group
+    int seq, p0, n, g;  // g < 0: all query heads of the group (small record)
+    int c0, cb;         // big record: the unit's block of float4 columns [c0, c0 + cb) of the D/4 of a row
 };
-__device__ __forceinline__ MergeUnit unit_of(const int32_t* __restrict__ recs, int n_small, int u, int G) {
-    const int r = u < n_small ? u : n_small + (u - n_small) / G;
+// Units [0, n_small) are the small records; then every big record gives G * S units, S = column blocks per row.
+__device__ __forceinline__ MergeUnit unit_of(const int32_t* __restrict__ recs, int n_small, int u, int G, int S, int D4) {
+    const int v = u - n_small;
+    const int r = u < n_small ? u : n_small + v / (G * S);
     const int4 rec = reinterpret_cast<const int4*>(recs)[r];  // {seq, first part slot, parts, -}
-    return MergeUnit{rec.x, rec.y, rec.z, u < n_small ? -1 : (u - n_small) % G};
+    if (u < n_small) return MergeUnit{rec.x, rec.y, rec.z, -1, 0, D4};
+    return MergeUnit{rec.x, rec.y, rec.z, (v / S) % G, (v % S) * (D4 / S), D4 / S};
+}
+
+// One query head of a BIG record (a long sequence that the work lists dice into up to thousands of parts), one
+// block of cb float4 columns: thread (grp, c) accumulates parts grp, grp + PG, ... of column c0 + c with eight
+// loads in flight, PG = NT / cb part groups; the group states are then combined by a fixed binary tree through
+// shared memory.  The narrower the column block, the more part groups work on the record at once: with cb = 1 a
+// CTA covers 8 * NT parts per round trip, and a record's G * D/4 units spread over the whole grid -- a single
+// 2^20-token sequence in 1036 parts merges in ~3 us instead of ~15 us with one CTA per query head.  The order
+// of the additions is a function of (n, cb, NT) only: deterministic.
+template <int D, int NT, bool NAMED_BAR>
+__device__ __forceinline__ void merge_big_unit(const MergeUnit mu, int G, const float* __restrict__ part_o,
+                                               const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
+                                               float* __restrict__ lse, float (*s_part)[6], int tid) {
+    auto sync = [] {
+        if constexpr (NAMED_BAR) named_bar_sync(1, NT);
+        else __syncthreads();
+    };
+    const int cb = mu.cb, PG = NT / cb;
+    const int c = tid % cb, grp = tid / cb, c4 = mu.c0 + c, n = mu.n;
+    const size_t row = static_cast<size_t>(mu.seq) * G + mu.g;  // (r*H + h)*G + g = r*Hq + h*G + g
+    float m = -INFINITY, tot = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    {
+        const float* pl = part_lse + static_cast<size_t>(mu.p0) * G + mu.g;  // [part][g]
+        const float* po = part_o + (static_cast<size_t>(mu.p0) * G + mu.g) * D + c4 * 4;
+        const size_t stride = static_cast<size_t>(G) * D;
+        for (int i = grp; i < n; i += 8 * PG) {
+            float4 v[8];
+            float w[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int ii = i + u * PG;
+                const int ic = ii < n ? ii : i;
+                v[u] = __ldcg(reinterpret_cast<const float4*>(po + ic * stride));
+                w[u] = ii < n ? __ldcg(pl + ic * G) : -INFINITY;
+            }
+            float m_new = m;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
+            const float resc = m_new == -INFINITY ? 1.f : __expf(m - m_new);  // m = -inf on the first batch -> 0
+            tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
+            m = m_new;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float e = m == -INFINITY ? 0.f : __expf(w[u] - m);  // -inf -> 0; all parts empty so far -> 0
+                tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
+            }
+        }
+    }
+    float* mine = s_part[tid];
+    mine[0] = m, mine[1] = tot, mine[2] = a0, mine[3] = a1, mine[4] = a2, mine[5] = a3;
+    for (int half = PG >> 1; half >= 1; half >>= 1) {  // group grp takes in group grp + half
+        sync();
+        if (grp < half) {
+            const float* o = s_part[(grp + half) * cb + c];
+            const float M = fmaxf(m, o[0]);
+            const float sa = M == -INFINITY ? 0.f : __expf(m - M), sb = M == -INFINITY ? 0.f : __expf(o[0] - M);
+            tot = sa * tot + sb * o[1];
+            a0 = sa * a0 + sb * o[2], a1 = sa * a1 + sb * o[3], a2 = sa * a2 + sb * o[4], a3 = sa * a3 + sb * o[5];
+            m = M;
+            mine[0] = m, mine[1] = tot, mine[2] = a0, mine[3] = a1, mine[4] = a2, mine[5] = a3;
+        }
+    }
+    if (grp == 0) {
+        const float inv = tot > 0.f ? 1.f / tot : 0.f;
+        const __nv_bfloat162 lo = __floats2bfloat162_rn(a0 * inv, a1 * inv), hi = __floats2bfloat162_rn(a2 * inv, a3 * inv);
+        reinterpret_cast<uint2*>(out + row * D)[c4] =
+            make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
+        if (c4 == 0) lse[row] = tot > 0.f ? m + __logf(tot) : -INFINITY;
+    }
+    sync();  // s_part may be reused by the next unit
 }
 
 template <int D, int NT, bool NAMED_BAR>
@@ -319,12 +393,13 @@ template <int D>
 __global__ void __launch_bounds__(kMergeThreads)
 tangram_merge_kernel(const int32_t* __restrict__ merge_recs, int n_small, const float* __restrict__ part_o,
                      const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
-                     float* __restrict__ lse, int G) {
+                     float* __restrict__ lse, int G, int S) {
     __shared__ float s_part[kMergeThreads][6];
-    const MergeUnit mu = unit_of(merge_recs, n_small, blockIdx.x, G);
+    const MergeUnit mu = unit_of(merge_recs, n_small, blockIdx.x, G, S, D / 4);
     // everything above reads plan data only; the partials / outputs need the decode grid to be done
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    merge_unit<D, kMergeThreads, false>(mu, G, part_o, part_lse, out, lse, s_part, threadIdx.x);
+    if (mu.g < 0) merge_unit<D, kMergeThreads, false>(mu, G, part_o, part_lse, out, lse, s_part, threadIdx.x);
+    else merge_big_unit<D, kMergeThreads, false>(mu, G, part_o, part_lse, out, lse, s_part, threadIdx.x);
 }
 
 // ------------------------------------------------------------------ a4: split-KV decode kernel
@@ -655,8 +730,8 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
         float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
         for (int u = blockIdx.x; u < n_big_units; u += grid)
-            merge_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G), G, p.part_o,
-                                          p.part_lse, p.out, p.lse, s_part, threadIdx.x);
+            merge_big_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4),
+                                              G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
         if (sub < K)
             for (; sidx < p.n_merge_small; sidx += grid * K) {
                 merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
@@ -790,8 +865,24 @@ template <int D>
 static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map,
                          cudaStream_t stream, int which) {
     const int n_small = (int)(dp->n_merge_seqs - dp->n_big_merge_seqs);
-    const int n_units = n_small + (int)dp->n_big_merge_seqs * prm.G;
-    prm.merge_recs = dp->merge_seqs, prm.n_merge_small = n_small, prm.n_merge_units = n_units;
+    // Column blocks per row of a big record (a power of two <= D/4): more blocks = more part groups per record
+    // (fewer dependent round trips: a CTA of 256 threads covers 8 * 256 * S / (D/4) parts of one block per round)
+    // but also more units, i.e. more waves over the grid.  Cost model in units of one L2 round trip, measured on
+    // B200: a unit costs ~2.5 (record, reduction tree, store) + its rounds.
+    int S = 1;
+    {
+        const int64_t n_big = dp->n_big_merge_seqs, grid = std::max(1, dp->n_static);
+        double best = 1e30;
+        for (int cand = 1; cand <= D / 4 && n_big > 0; cand *= 2) {
+            const int64_t waves = (n_big * prm.G * cand + grid - 1) / grid;
+            const int64_t per_round = (int64_t)8 * 256 * cand / (D / 4);
+            const int64_t rounds = (dp->max_merge_parts + per_round - 1) / per_round;
+            const double cost = (double)waves * (2.5 + (double)rounds);
+            if (cost < best) best = cost, S = cand;
+        }
+    }
+    const int n_units = n_small + (int)dp->n_big_merge_seqs * prm.G * S;
+    prm.merge_recs = dp->merge_seqs, prm.n_merge_small = n_small, prm.n_merge_units = n_units, prm.merge_split = S;
     bool merged = false;
     if (which & kRunSplit) {
         const bool want = (which & kRunMerge) && n_units > 0;
@@ -811,7 +902,7 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
     const float* po = prm.part_o;
     const float* pl = prm.part_lse;
     cudaError_t e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, n_small, po, pl, prm.out, prm.lse,
-                                       (int)prm.G);
+                                       (int)prm.G, S);
     if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
     return TANGRAM_OK;
 }
@@ -963,6 +1054,9 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->list_heads = base + off_heads;
     dp->seq_info = reinterpret_cast<const int32_t*>(base + off_seqinfo);
     dp->n_big_merge_seqs = n_mseq - n_not_big;
+    dp->max_merge_parts = 0;
+    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)
+        dp->max_merge_parts = std::max<int64_t>(dp->max_merge_parts, p->part_indptr[sq + 1] - p->part_indptr[sq]);
     dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
     dp->items = base + off_items;
     dp->worker_indptr = reinterpret_cast<const int64_t*>(base + off_windptr);
@@ -1016,7 +1110,7 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.part_lse = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) +
                                             align_up((size_t)dp->n_part_slots * G * d * 4, 256));
     prm.worker_ns = reinterpret_cast<unsigned long long*>(worker_ns);
-    prm.tail_merge = 0, prm.merge_recs = nullptr, prm.n_merge_units = 0, prm.n_merge_small = 0;
+    prm.tail_merge = 0, prm.merge_recs = nullptr, prm.n_merge_units = 0, prm.n_merge_small = 0, prm.merge_split = 1;
     prm.Hq = Hq, prm.G = G, prm.Hp = dp->Hp;
     prm.n_lists = dp->W;
     prm.list_heads = dp->list_heads;
