@@ -161,11 +161,12 @@ def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None, layer=
     if W is None:
         W = T.tangram_query_max_ctas(torch.cuda.current_device(), wl.d, wl.G)
     t3 = time.perf_counter()
-    dyn = (T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS) if dyn is None else dyn
     kv_plan = kv
     if plan_capacity:      # open-ended plan: built once for the tables' capacity, serves every decode step
         rows = np.arange(wl.R)[:, None] * tb.C + tb.cluster_of[None, :]
         kv_plan = ((tb.tbl_indptr[rows + 1] - tb.tbl_indptr[rows]) * wl.P).astype(np.int32)
+    if dyn is None:        # the library's default: dynamic tail 500/6, or the static plan for a small batch
+        dyn = T.tangram_default_dynamic_tail(kv_plan, W, wl.granule, c0)
     plan = T.tangram_plan_partitions(tb, B, kv_plan, W, wl.granule, c0, T.MODE_BALANCED if mode is None else mode, 0,
                                      dyn[0], dyn[1])
     t4 = time.perf_counter()

@@ -149,6 +149,14 @@ int tangram_plan_partitions(const tangram_tables* t, const double* B, const int3
                             int32_t mode, int32_t static_splits, int32_t dyn_permille, int32_t dyn_rounds,
                             tangram_plan* out);
 
+/* Default dynamic tail for tangram_plan_partitions (a measured tuning rule, not from the paper): (500, 6) when the
+ * batch has at least 32 cost units (granules of granule_tokens + overhead_granules per non-empty sequence) per
+ * worker, else (0, 0) -- with little work per CTA the purely static plan is faster (no list claims, fewer parts to
+ * merge: 8b-shaped batch of 1: 18.5 us against 22.5 us; 32 requests: the tail wins, 127 us against 140 us).
+ * kv_len host [R][H] i32.  Errors: INVALID_ARG. */
+int tangram_default_dynamic_tail(const int32_t* kv_len, int32_t R, int32_t H, int32_t n_workers, int32_t granule_tokens,
+                                 int32_t overhead_granules, int32_t* dyn_permille_out, int32_t* dyn_rounds_out);
+
 /* ------------------------------------------------------------------------------------------------
  * Device side.  One upload of tables + plan per (batch, layer); then one
  * tangram_decode_attention per decode step with no host planning (:254 "zero runtime planning").

@@ -251,6 +251,18 @@ def list_weights(n_workers: int, dyn_permille: int, dyn_rounds: int) -> List[int
     return w
 
 
+def default_dynamic_tail(kv_len, n_workers: int, granule: int, overhead_granules: int) -> Tuple[int, int]:
+    """Default (dyn_permille, dyn_rounds) of the BALANCED plan (reading A32, a measured tuning rule, not
+    from the paper): the dynamic tail (500, 6) pays off once a CTA streams long enough for the per-SM bandwidth
+    differences to matter; with fewer than 32 cost units (granules + per-sequence overhead) per worker the purely
+    static plan (0, 0) is faster (no claims, fewer parts to merge)."""
+    total = 0
+    for n in np.asarray(kv_len, dtype=np.int64).reshape(-1):
+        u = -(-int(n) // granule)
+        total += u + (overhead_granules if u > 0 else 0)
+    return (500, 6) if total >= 32 * n_workers else (0, 0)
+
+
 def plan_partitions(t: Tables, B, kv_len, n_workers: int, granule: int, overhead_granules: int,
                     mode: int, static_splits: int = 0, dyn_permille: int = 0, dyn_rounds: int = 0) -> Plan:
     """Offline deterministic planner (§4.3).  Sequences are visited r-major, then in `perm`

@@ -71,7 +71,7 @@ for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
               "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk",
               "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios",
-              "tangram_compact_topk_chunk", "tangram_stage_from_host"):
+              "tangram_compact_topk_chunk", "tangram_stage_from_host", "tangram_default_dynamic_tail"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
@@ -79,7 +79,7 @@ EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragge
            "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
            "tangram_compact_workspace_bytes", "tangram_compact_topk", "tangram_account_pages",
            "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk",
-           "tangram_stage_from_host")
+           "tangram_stage_from_host", "tangram_default_dynamic_tail")
 
 
 def _check(rc: int):
@@ -398,3 +398,13 @@ def tangram_stage_from_host(dst, src, stream=None):
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     _check(_lib.tangram_stage_from_host(C.c_void_p(dst.data_ptr()), C.c_void_p(src.data_ptr()), C.c_size_t(nbytes), sp))
     return dst
+
+
+def tangram_default_dynamic_tail(kv_len, n_workers: int, granule_tokens: int, overhead_granules: int = 1):
+    """-> (dyn_permille, dyn_rounds): the library's default dynamic tail for this batch (static plan for small ones)."""
+    kv = _np(kv_len, np.int32)
+    R, H = kv.shape
+    a, b = C.c_int32(0), C.c_int32(0)
+    _check(_lib.tangram_default_dynamic_tail(_ptr(kv), C.c_int32(R), C.c_int32(H), C.c_int32(n_workers),
+                                             C.c_int32(granule_tokens), C.c_int32(overhead_granules), C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)

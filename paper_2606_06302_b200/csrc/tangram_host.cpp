@@ -355,3 +355,21 @@ extern "C" int tangram_calibrate_budgets(const double* ratios, int32_t n_samples
     }
     return TANGRAM_OK;
 }
+
+// ---- default dynamic tail of the BALANCED plan (measured tuning rule, reading A32)
+extern "C" int tangram_default_dynamic_tail(const int32_t* kv_len, int32_t R, int32_t H, int32_t n_workers,
+                                            int32_t granule_tokens, int32_t overhead_granules,
+                                            int32_t* dyn_permille_out, int32_t* dyn_rounds_out) {
+    if (!kv_len || !dyn_permille_out || !dyn_rounds_out || R < 1 || H < 1 || n_workers < 1 || granule_tokens < 1 ||
+        overhead_granules < 0)
+        return fail(TANGRAM_ERR_INVALID_ARG, "default_dynamic_tail: bad argument");
+    int64_t total = 0;
+    for (int64_t i = 0; i < (int64_t)R * H; ++i) {
+        if (kv_len[i] < 0) return fail(TANGRAM_ERR_INVALID_ARG, "default_dynamic_tail: kv_len < 0");
+        const int64_t u = (kv_len[i] + (int64_t)granule_tokens - 1) / granule_tokens;
+        total += u + (u > 0 ? overhead_granules : 0);
+    }
+    const bool tail = total >= (int64_t)32 * n_workers;
+    *dyn_permille_out = tail ? 500 : 0, *dyn_rounds_out = tail ? 6 : 0;
+    return TANGRAM_OK;
+}

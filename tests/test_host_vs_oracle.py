@@ -223,3 +223,20 @@ def test_header_is_plain_c_and_host_path_runs_from_c(tmp_path):
     out = subprocess.run([exe], capture_output=True, text=True)
     assert out.returncode == 0, out.stderr
     assert "c_abi host path ok" in out.stdout
+
+
+def test_default_dynamic_tail_rule():
+    for name in I.CONFIG_NAMES:
+        wl = I.make_workload(name)
+        _, _, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+        for W in (1, 148, 296):
+            assert T.tangram_default_dynamic_tail(kv, W, wl.granule, 1) == O.default_dynamic_tail(kv, W, wl.granule, 1)
+    wl = I.make_workload("tiny")
+    _, _, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    assert T.tangram_default_dynamic_tail(kv, 148, 64, 1) == (0, 0)                      # little work per CTA: static
+    wl = I.make_workload("8b")
+    _, _, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    assert T.tangram_default_dynamic_tail(kv, 148, 64, 1) == (T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS)
+    edge = np.full((1, 1), 64 * 31, dtype=np.int32)                                       # 31 granules + 1 overhead = 32
+    assert T.tangram_default_dynamic_tail(edge, 1, 64, 1) == O.default_dynamic_tail(edge, 1, 64, 1) == (500, 6)
+    assert T.tangram_default_dynamic_tail(edge - 64, 1, 64, 1) == O.default_dynamic_tail(edge - 64, 1, 64, 1) == (0, 0)
