@@ -5,13 +5,16 @@
 //   1. compact_prepare_kernel   one CTA: clamps keep[r][h] to [0, min(N_r, table capacity)] (the reserved
 //      budget is a hard capacity bound, :176), counts the clamped heads, and scans ceil(keep / P) into a
 //      tile index (tile = the P token slots of one (page, head)); zeroes the gather kernel's chunk counter.
-//   2. topk_select_kernel       one CTA (512 or 1024 threads, by row length) per (request, KV head): radix select (digits of 11, 11
-//      and 10 bits, shared-memory atomic histograms, 16-byte loads) over a monotone integer image of the
-//      fp32 score finds the threshold key T and how many of the entries equal to T are kept (the lowest
-//      token indices first, reading A30).  An ordered pass then writes the retained token indices in ascending order: the entry at token i goes
-//      to position (#greater before i) + min(#equal before i, need); every warp owns a contiguous segment,
-//      so that pass needs one block barrier in total.  Integer work on fp32 bit patterns: the result is the
-//      unique Top-k under the tie rule, bit-exact against the sort-based oracle.
+//   2. topk_select_kernel       one CTA (512 or 1024 threads, by row length) per (request, KV head): radix select
+//      (digits of 11, 11 and 10 bits, shared-memory atomic histograms, 16-byte loads) over a monotone integer image
+//      of the fp32 score finds the threshold key T and how many of the entries equal to T are kept (the lowest
+//      token indices first, reading A30).  After the first digit the entries that share the threshold's digit are
+//      usually few (<= 4096): one more pass over the row buffers them in shared memory, where the other two digits
+//      are resolved; otherwise the kernel falls back to whole-row passes.  An ordered pass then writes the retained
+//      token indices in ascending order: the entry at token i goes to position (#greater before i) +
+//      min(#equal before i, need); every warp owns a contiguous segment, so that pass needs one block barrier in
+//      total.  Integer work on fp32 bit patterns: the result is the unique Top-k under the tie rule, bit-exact
+//      against the sort-based oracle.
 //   3. compact_gather_kernel    persistent grid, warps claim chunks of tiles from a global counter (the same
 //      run-time balancing as the decode kernel's dynamic tail: per-SM bandwidth differs on B200).  A warp
 //      moves one tile: up to P K rows and P V rows of d bf16 each, gathered with 16-byte loads (16 in
@@ -29,6 +32,7 @@ namespace tangram {
 
 constexpr int kCPage = 16;           // tokens per page (the kernels are specialised for P = 16)
 constexpr int kSelBins = 2048;        // 11-bit digits
+constexpr int kSelCand = 4096;        // candidates (entries in the first digit's bin) the select kernel buffers
 constexpr int kSelLongRow = 49152;    // rows longer than this get 1024-thread CTAs, shorter ones 512 (two per SM)
 constexpr int kGatherThreads = 256;
 constexpr int kGatherChunk = 8;      // tiles claimed at once
@@ -131,20 +135,26 @@ __device__ __forceinline__ void for_each_key_row(const float* __restrict__ s, in
 }
 
 // Block-wide radix select of the k-th largest key (1 <= k <= number of entries): digits of 11, 11 and 10 bits
-// from the top, one shared-memory atomic histogram per digit.  each_key(add) must call add(key) once for every
-// entry, the entries split among the NT threads in any way.  Returns, in every thread, the threshold key T and
-// `need` = how many of the entries equal to T belong to the k largest (1 <= need <= their number).
+// from the top, one shared-memory atomic histogram per digit.  radix_passes runs digits [pass_begin, pass_end):
+// each_key(add) must call add(key) once for every entry (split among the NT threads in any way; entries whose
+// higher digits do not match the prefix found so far are ignored).  State, the same in every thread: `prefix` /
+// `mask` = the digits fixed so far, `krem` = rank still to be found among the entries that match them, `cand` =
+// how many entries match.  After the last digit prefix is the threshold key T and krem = how many of the entries
+// equal to T belong to the k largest.
+struct RadixState {
+    uint32_t prefix, mask, krem, cand;
+};
 template <int NT, typename EachKey>
-__device__ __forceinline__ void radix_select(EachKey&& each_key, uint32_t k, uint32_t* s_hist, uint32_t* s_wsum,
-                                             uint32_t* s_pick, uint32_t& T, uint32_t& need) {
+__device__ __forceinline__ void radix_passes(EachKey&& each_key, int pass_begin, int pass_end, RadixState& st,
+                                             uint32_t* s_hist, uint32_t* s_wsum, uint32_t* s_pick) {
     constexpr int kWarps = NT / 32;
     constexpr int kBpt = kSelBins / NT;  // adjacent bins a thread owns in the scan
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    uint32_t prefix = 0, mask = 0, krem = k;
 #pragma unroll 1
-    for (int pass = 0; pass < 3; ++pass) {
+    for (int pass = pass_begin; pass < pass_end; ++pass) {
         const int shift = pass == 0 ? 21 : (pass == 1 ? 10 : 0);
         const uint32_t dmask = pass == 2 ? 1023u : 2047u;
+        const uint32_t prefix = st.prefix, mask = st.mask, krem = st.krem;
         for (int b = tid; b < kSelBins; b += NT) s_hist[b] = 0u;
         __syncthreads();
         each_key([&](uint32_t key) {
@@ -167,18 +177,18 @@ __device__ __forceinline__ void radix_select(EachKey&& each_key, uint32_t k, uin
             for (int w = warp + 1; w < kWarps; ++w) gt += s_wsum[w];
 #pragma unroll
             for (int j = kBpt - 1; j >= 0; --j) {
-                if (gt < krem && krem <= gt + c[j]) {  // exactly one bin of the row satisfies this
+                if (gt < krem && krem <= gt + c[j]) {  // exactly one bin satisfies this
                     s_pick[0] = prefix | (static_cast<uint32_t>(kBpt * tid + j) << shift);
                     s_pick[1] = krem - gt;
+                    s_pick[2] = c[j];
                 }
                 gt += c[j];
             }
         }
         __syncthreads();
-        prefix = s_pick[0], krem = s_pick[1];
-        mask |= dmask << shift;
+        st.prefix = s_pick[0], st.krem = s_pick[1], st.cand = s_pick[2];
+        st.mask = mask | (dmask << shift);
     }
-    T = prefix, need = krem;
 }
 
 // One CTA of NT threads per (request, KV head).  (A thread-block cluster per row with the histograms
@@ -192,8 +202,10 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
     constexpr int kU = NT == 1024 ? 4 : 8;  // 16-byte loads in flight per thread (register budget: 64 / 32)
     __shared__ uint32_t s_hist[kSelBins];
     __shared__ uint32_t s_wsum[kSelWarps];
-    __shared__ uint32_t s_pick[2];
+    __shared__ uint32_t s_pick[3];
     __shared__ uint32_t s_cnt[2][kSelWarps];  // (greater, equal) counts of the warps' segments
+    __shared__ uint32_t s_ckey[kSelCand], s_cidx[kSelCand];  // candidates: entries in the first digit's bin
+    __shared__ uint32_t s_ncand;
     const int seq = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = ctx_len[seq / H];
     const int k = keep_eff[seq];
@@ -204,28 +216,86 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
         for (int i = tid; i < N; i += NT) idx[i] = i;
         return;
     }
-    // keep every key > T and the first `need` entries with key == T
-    uint32_t T, need;
-    radix_select<NT>([&](auto&& add) { for_each_key_row<NT, kU>(s, N, tid, add); }, static_cast<uint32_t>(k), s_hist,
-                     s_wsum, s_pick, T, need);
-    // The row is <= 3 head entries, nvec aligned float4 groups, <= 3 tail entries.
+    // The row is <= 3 head entries, nvec aligned float4 groups, <= 3 tail entries.  Warp w owns the contiguous
+    // groups [v0, v1) in the ordered parts below.
     const int head = min(N, static_cast<int>((4u - (static_cast<uint32_t>(reinterpret_cast<uintptr_t>(s)) >> 2)) & 3u));
     const int nvec = (N - head) >> 2;
     const int tail0 = head + 4 * nvec;
     const float4* sv = reinterpret_cast<const float4*>(s + head);
-
-    // ---- ordered pass: position of token i = #greater before i + min(#equal before i, need).
-    // Warp w owns the contiguous groups [v0, v1): it counts them (16-byte loads, 8 in flight), the counts of
-    // all warps are exchanged (the only block barrier of this part), then it walks its groups again 32 at a
-    // time: a lane holds four consecutive tokens and a packed (greater, equal) warp scan gives their positions.
     const int wseg = ((nvec + kSelWarps - 1) / kSelWarps + 31) & ~31;
     const int v0 = min(nvec, warp * wseg), v1 = min(nvec, v0 + wseg);
+
+    // ---- threshold: keep every key > T and the first `need` entries with key == T
+    auto whole_row = [&](auto&& add) { for_each_key_row<NT, kU>(s, N, tid, add); };
+    RadixState st{0u, 0u, static_cast<uint32_t>(k), static_cast<uint32_t>(N)};
+    radix_passes<NT>(whole_row, 0, 1, st, s_hist, s_wsum, s_pick);  // first digit: one pass over the row (from HBM)
+    const bool buffered = st.cand <= static_cast<uint32_t>(kSelCand);
+    if (buffered) {
+        // Usual case: few entries share the threshold's first digit.  ONE more pass over the row collects them
+        // in shared memory and counts, per warp segment, the entries above that digit (certainly retained); the
+        // remaining two digits and the (greater, equal) split of the candidates are then found in shared memory.
+        // Three passes over the row in total (this one, the first digit, the placement) instead of five.
+        if (tid == 0) s_ncand = 0u;
+        __syncthreads();
+        const uint32_t top = st.prefix >> 21;
+        auto collect = [&](uint32_t key, int token) {
+            if ((key >> 21) == top) {
+                const uint32_t slot = atomicAdd(&s_ncand, 1u);
+                s_ckey[slot] = key, s_cidx[slot] = static_cast<uint32_t>(token);
+            }
+        };
+        if (tid < head) collect(score_key(__ldg(s + tid)), tid);
+        if (tid < N - tail0) collect(score_key(__ldg(s + tail0 + tid)), tail0 + tid);
+        uint32_t cg_ = 0;
+        auto scan4 = [&](const float4 x, int v) {
+            const uint32_t key[4] = {score_key(x.x), score_key(x.y), score_key(x.z), score_key(x.w)};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                cg_ += (key[j] >> 21) > top;
+                collect(key[j], head + 4 * v + j);
+            }
+        };
+        int v = v0 + lane;
+        for (; v + 7 * 32 < v1; v += 8 * 32) {
+            float4 x[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) x[u] = __ldg(sv + v + u * 32);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) scan4(x[u], v + u * 32);
+        }
+        for (; v < v1; v += 32) scan4(__ldg(sv + v), v);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cg_ += __shfl_xor_sync(0xffffffffu, cg_, o);
+        if (lane == 0) s_cnt[0][warp] = cg_, s_cnt[1][warp] = 0u;
+        __syncthreads();
+        const int n_cand = static_cast<int>(s_ncand);  // == st.cand
+        radix_passes<NT>([&](auto&& add) { for (int i = tid; i < n_cand; i += NT) add(s_ckey[i]); }, 1, 3, st, s_hist,
+                         s_wsum, s_pick);
+        // candidates above / at the threshold, added to their warp segment's counts (head and tail entries are
+        // placed separately below)
+        for (int i = tid; i < n_cand; i += NT) {
+            const int token = static_cast<int>(s_cidx[i]);
+            if (token < head || token >= tail0) continue;
+            const int w = ((token - head) >> 2) / wseg;
+            if (s_ckey[i] > st.prefix) atomicAdd(&s_cnt[0][w], 1u);
+            else if (s_ckey[i] == st.prefix) atomicAdd(&s_cnt[1][w], 1u);
+        }
+    } else {
+        radix_passes<NT>(whole_row, 1, 3, st, s_hist, s_wsum, s_pick);
+    }
+    const uint32_t T = st.prefix, need = st.krem;
+
+    // ---- ordered pass: position of token i = #greater before i + min(#equal before i, need).
+    // Every warp needs the (greater, equal) counts of the segments before its own: from the buffered path above, or
+    // by counting its groups (16-byte loads, 8 in flight); after the only block barrier of this part it walks its
+    // groups 32 at a time: a lane holds four consecutive tokens and a packed (greater, equal) warp scan gives their
+    // positions.
     auto cnt4 = [&](const float4 x, uint32_t& g, uint32_t& e) {
         const uint32_t a = score_key(x.x), b = score_key(x.y), c = score_key(x.z), d = score_key(x.w);
         g += (a > T) + (b > T) + (c > T) + (d > T);
         e += (a == T) + (b == T) + (c == T) + (d == T);
     };
-    {
+    if (!buffered) {
         uint32_t cg_ = 0, ce_ = 0;
         int v = v0 + lane;
         for (; v + 7 * 32 < v1; v += 8 * 32) {
@@ -321,7 +391,7 @@ implicit_ratio_kernel(const float* __restrict__ scores, int64_t n_max, const int
     extern __shared__ uint32_t s_ge[];  // [2][H]: entries greater than / equal to the threshold, per head
     __shared__ uint32_t s_hist[kSelBins];
     __shared__ uint32_t s_wsum[NT / 32];
-    __shared__ uint32_t s_pick[2];
+    __shared__ uint32_t s_pick[3];
     const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
     const int N = ctx_len[r];
     const float* s = scores + static_cast<size_t>(r) * H * n_max;
@@ -336,12 +406,13 @@ implicit_ratio_kernel(const float* __restrict__ scores, int64_t n_max, const int
         }
         return;
     }
-    uint32_t T, need;
-    radix_select<NT>(
+    RadixState st{0u, 0u, k, total};
+    radix_passes<NT>(
         [&](auto&& add) {
             for (int h = 0; h < H; ++h) for_each_key_row<NT, kU>(s + static_cast<size_t>(h) * n_max, N, tid, add);
         },
-        k, s_hist, s_wsum, s_pick, T, need);
+        0, 3, st, s_hist, s_wsum, s_pick);
+    const uint32_t T = st.prefix, need = st.krem;
     for (int h = tid; h < 2 * H; h += NT) s_ge[h] = 0u;
     __syncthreads();
     for (int h = 0; h < H; ++h) {

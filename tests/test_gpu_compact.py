@@ -387,3 +387,24 @@ def test_global_flat_topk_compression_as_a_composition():
         for h in range(wl.H):
             mine = sel[(sel >= h * N) & (sel < (h + 1) * N)] - h * N
             assert np.array_equal(gi[r, h, :c[r, h]], mine)
+
+
+def test_select_paths_buffered_and_fallback():
+    """The select kernel buffers the entries that share the threshold's first radix digit when there are at most
+    4096 of them, and falls back to whole-row passes otherwise: rows of 9 000 - 20 000 tokens with all-equal scores,
+    three-valued scores (fallback), well-spread scores (buffered), and a row whose candidates are exactly the
+    buffer size."""
+    wl = I.make_random_workload(95, R=5, H=2, G=1, d=64, C=1, max_ctx=100)
+    wl.ctx_len[:] = [9000, 20000, 12000, 4096, 16000]
+    wl.mu[:] = 1.0
+    wl.demand = (wl.ctx_len[:, None] * np.array([[0.3, 0.77]])).astype(np.int32)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    n_max = 20000
+    g = torch.Generator(device="cuda").manual_seed(95)
+    scores = torch.randn(wl.R, wl.H, n_max, generator=g, device="cuda")
+    scores[0] = 1.25                                                               # all equal: N candidates
+    scores[1] = torch.randint(0, 3, (wl.H, n_max), generator=g, device="cuda").float()   # ~6 700 per value
+    scores[3] = 3.0                                                                # exactly 4096 candidates
+    scores[4, 0] = scores[4, 0].bfloat16().float()                                 # bf16-rounded normal scores
+    _, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda")
+    run_and_compare(wl, t, dp, n_pool, kv, scores, kd, vd, n_max)
