@@ -204,11 +204,13 @@ int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blo
 /* Workspace for the split-KV partials: n_part_slots x G x (d + 1) fp32, rounded up. */
 size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_dim);
 
-/* a4 + a5  One layer, whole batch: split-KV decode kernel over the work list, then the LSE merge
- * kernel.  Asynchronous on `stream`; CUDA-graph capturable; no host work besides the two launches.
+/* a4 + a5  One layer, whole batch: split-KV decode kernel over the work lists, then the LSE merge -- inside the
+ * same persistent grid after a grid barrier (ONE cooperative launch); the stand-alone merge kernel follows as a
+ * second launch only when the grid cannot be co-resident (n_workers > SMs x occupancy) or d = 256.
+ * Asynchronous on `stream`; CUDA-graph capturable; no host work besides the launch.
  *
  *   dp        from tangram_upload (host struct holding device pointers)
- *   q         device [R][Hq][d] bf16, 16-byte aligned
+ *   q         device (or pinned host, see "Host buffers" below) [R][Hq][d] bf16, 16-byte aligned
  *   kv_pool   device [n_pool_pages][Hp][2][P][d] bf16, 128-byte aligned (Ragged page, :190)
  *   kv_len_dev device [R][H] i32 or NULL.  NULL: the items are executed exactly as planned.  Otherwise the
  *             plan is OPEN-ENDED: every item covers tokens [tok_begin, min(tok_end, kv_len_dev[r][h])), so a
