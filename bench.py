@@ -395,7 +395,7 @@ def compact_topk_summary(T, I, name, device, steps, flush, torch, peak_gbs):
             "gbs_gather_bytes_over_total_time": gather_bytes / (us * 1e-6) / 1e9,
             "pct_of_measured_copy": 100 * gather_bytes / (us * 1e-6) / 1e9 / peak_gbs,
             "note": "whole call (select + gather) timed with CUDA events, L2 flushed; bytes = K/V rows read + "
-                    "written; the select kernel reads the scores five times (first pass from HBM, then L2); "
+                    "written; the select kernel reads the scores three times (first pass from HBM, then L2); "
                     "kernel shares: profiles/"}
 
 
