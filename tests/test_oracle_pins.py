@@ -744,3 +744,17 @@ def test_global_flat_topk_equals_per_head_topk_with_its_own_counts():
             for h in range(H):
                 mine = sel[(sel >= h * N) & (sel < (h + 1) * N)] - h * N
                 assert mine.tolist() == O.topk_indices(sc[r, h, :N], int(cnt[r, h])).tolist()
+
+
+def test_topk_indices_against_a_stable_library_sort():
+    """O7 once more against a library routine: a stable descending argsort keeps equal scores in index order, so its
+    first k entries are the oracle's selection (random rows with ties, +-0, infinities)."""
+    rng = np.random.default_rng(77)
+    for _ in range(200):
+        n = int(rng.integers(1, 400))
+        s = rng.choice([rng.normal(size=n), rng.integers(-3, 4, size=n).astype(float)]).astype(np.float32)
+        if n > 4:
+            s[rng.integers(n)], s[rng.integers(n)], s[rng.integers(n)] = 0.0, -0.0, np.inf
+        k = int(rng.integers(0, n + 1))
+        want = np.sort(np.argsort(-s.astype(np.float64), kind="stable")[:k])
+        assert O.topk_indices(s, k).tolist() == want.tolist()
