@@ -7,7 +7,8 @@
  * KV head h = floor(j / G) through that head's cluster page table (Ragged Paging, PAPER.md:190
  * "a page holds H_p x 2 x P x d elements for the H_p heads of one group in one layer"; Eq. 1,
  * PAPER.md:57-58, K~ = K[I,:], V~ = V[I,:]) and evaluate softmax(q K~^T / sqrt(d)) V~ in fp64.
- * The paper never writes softmax attention out; scale 1/sqrt(d) and natural-log LSE are
+ * The paper never writes softmax attention out; the softmax scale (1/sqrt(d) unless the caller
+ * gives another one, as tangram_decode_attention's sm_scale argument does) and natural-log LSE are
  * DESIGN.md readings A19/A20/A21.  Element order inside a page is reading A4:
  * pool[page][slot][kv][token][d], kv 0 = K, 1 = V, bf16.
  *
@@ -38,6 +39,7 @@ typedef struct {
     const int32_t* cluster_of;  /* [H] */
     const int32_t* slot_of;     /* [H] */
     int32_t R, H, Hq, C, Hp, P, d;
+    double scale;               /* softmax scale: x_t = (q . k_t) * scale; <= 0 means 1/sqrt(d) (reading A19) */
 } oracle_ctx;
 
 /* Attention of query head j of request r over tokens [t0, t1) of its KV head.
@@ -60,14 +62,14 @@ static void attend_range(const oracle_ctx* c, int r, int j, int t0, int t1, doub
     const int32_t* row = c->tbl_pages + c->tbl_indptr[(size_t)r * c->C + cl];
     const size_t page_elems = (size_t)c->Hp * 2 * P * d;
     double* x = (double*)malloc(sizeof(double) * (size_t)n);
-    const double inv_sqrt_d = 1.0 / sqrt((double)d);
-    /* pass 1: x_t = (q . k_t) / sqrt(d) */
+    const double scale = c->scale > 0.0 ? c->scale : 1.0 / sqrt((double)d);
+    /* pass 1: x_t = (q . k_t) * scale   (scale = 1/sqrt(d) by default) */
     for (int t = t0; t < t1; ++t) {
         const size_t page = (size_t)row[t / P];
         const uint16_t* k = c->pool + page * page_elems + (((size_t)s * 2 + 0) * P + (t % P)) * d;
         double acc = 0.0;
         for (int e = 0; e < d; ++e) acc += bf16_to_f64(qv[e]) * bf16_to_f64(k[e]);
-        x[t - t0] = acc * inv_sqrt_d;
+        x[t - t0] = acc * scale;
     }
     /* pass 2: m = max x, l = sum exp(x - m) */
     double m = x[0];
@@ -91,23 +93,23 @@ void tangram_oracle_attend_range(const uint16_t* q, const uint16_t* pool, const 
                                  const int32_t* tbl_pages, const int32_t* cluster_of,
                                  const int32_t* slot_of, int32_t R, int32_t H, int32_t Hq, int32_t C,
                                  int32_t Hp, int32_t P, int32_t d, int32_t r, int32_t j, int32_t t0,
-                                 int32_t t1, double* out, double* lse) {
-    oracle_ctx c = {q, pool, tbl_indptr, tbl_pages, cluster_of, slot_of, R, H, Hq, C, Hp, P, d};
+                                 int32_t t1, double scale, double* out, double* lse) {
+    oracle_ctx c = {q, pool, tbl_indptr, tbl_pages, cluster_of, slot_of, R, H, Hq, C, Hp, P, d, scale};
     attend_range(&c, r, j, t0, t1, out, lse);
 }
 
 /* Attention for a list of (request, query head) pairs: pairs[2*i] = r, pairs[2*i+1] = j.
  * out [n_pairs][d], lse [n_pairs].  kv_len [R][H].  A plain `parallel for` over the pairs
- * (each pair is independent); n_threads <= 0 keeps the OpenMP default.  Returns the number of
- * threads used. */
+ * (each pair is independent); n_threads <= 0 keeps the OpenMP default; scale <= 0 means 1/sqrt(d).
+ * Returns the number of threads used. */
 int tangram_oracle_attention_pairs(const uint16_t* q, const uint16_t* pool,
                                    const int64_t* tbl_indptr, const int32_t* tbl_pages,
                                    const int32_t* cluster_of, const int32_t* slot_of,
                                    const int32_t* kv_len, int32_t R, int32_t H, int32_t Hq,
                                    int32_t C, int32_t Hp, int32_t P, int32_t d,
-                                   const int32_t* pairs, int64_t n_pairs, double* out, double* lse,
-                                   int32_t n_threads) {
-    oracle_ctx c = {q, pool, tbl_indptr, tbl_pages, cluster_of, slot_of, R, H, Hq, C, Hp, P, d};
+                                   const int32_t* pairs, int64_t n_pairs, double scale, double* out,
+                                   double* lse, int32_t n_threads) {
+    oracle_ctx c = {q, pool, tbl_indptr, tbl_pages, cluster_of, slot_of, R, H, Hq, C, Hp, P, d, scale};
     const int G = Hq / H;
     int used = 1;
 #ifdef _OPENMP

@@ -20,7 +20,10 @@ What each function follows (citations are PAPER.md lines; "reading Ax" = DESIGN.
   O11 compact_topk_chunk  the same for one prefill chunk, appended behind what the head already holds (compression
                           fused into chunked prefill, :152; NEXT-2 extension)
   O6 append_kv            one decode step's new K/V rows written into the ragged pages (NEXT-1;
-                          page layout :190, capacity bound :176, reading A29)
+                          page layout :190, reading A29: a row is dropped only when its table has no page for it)
+  O12 extend_tables       block-table growth during decode (NEXT-4; :85-89 "for every iteration, the scheduler
+                          allocates pages", :244 per-group block mappings updated for all groups at once;
+                          reading A33)
   O8 account_pages        pages / token-head slots a batch occupies under a grouping policy (monolithic,
                           adjacent, Budget-Aware Clustering; Fig. 7 :168, Fig. 8 :186, Fig. 15 :316-320; NEXT-3)
   O9 calibrate_budgets    mu, sigma of the recorded per-head implicit retention ratios and Eq. 5 (:156-158;
@@ -100,9 +103,16 @@ class Tables:
     perm: np.ndarray        # [H]  pi: sorted position -> head
     cluster_of: np.ndarray  # [H]  head -> cluster
     slot_of: np.ndarray     # [H]  head -> slot inside the cluster's pages
-    tbl_indptr: np.ndarray  # [R*C+1] int64, row = r*C + c
-    tbl_pages: np.ndarray   # [n_pages_used] int32
-    n_pages_used: int
+    tbl_indptr: np.ndarray  # [R*C+1] int64, row = r*C + c; a row owns the page SLOTS [indptr[row], indptr[row+1])
+    tbl_pages: np.ndarray   # [indptr[-1]] int32 page id of every slot; -1 = slot not assigned yet (growth headroom)
+    n_pages_used: int       # pages taken from the free list so far
+    row_pages: Optional[np.ndarray] = None   # [R*C] int32 assigned pages per row (None: every slot is assigned)
+
+    def assigned(self, row: int) -> int:
+        """Pages row `row` holds (its first `assigned` slots)."""
+        if self.row_pages is None:
+            return int(self.tbl_indptr[row + 1] - self.tbl_indptr[row])
+        return int(self.row_pages[row])
 
 
 def cluster_heads(B, n_clusters: int):
@@ -123,10 +133,12 @@ def cluster_heads(B, n_clusters: int):
 
 
 def build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages,
-                        flags: int = 0, kv_len=None):
+                        flags: int = 0, kv_len=None, headroom_pages: int = 0):
     """Returns (Tables, kv_len').  Row (r, c) of the tables has ceil(max_{h in c} reserved / P)
     pages (:190) and takes the next entries of `free_pages` in order (reading A27).  With
-    FLAG_FILL_GROUP every head's kv_len is raised to its cluster's max reserved (:235)."""
+    FLAG_FILL_GROUP every head's kv_len is raised to its cluster's max reserved (:235).
+    headroom_pages > 0 (reading A33): every row is followed by that many page slots that hold no
+    page yet (-1) -- room for extend_tables to grow the row during decode without moving it."""
     reserved = np.asarray(reserved)
     R, H = reserved.shape
     if page_size <= 0:
@@ -135,6 +147,7 @@ def build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages
     C, Hp = n_clusters, H // n_clusters
     indptr = [0]
     pages: List[int] = []
+    row_pages: List[int] = []
     cursor = 0
     gmax = np.zeros((R, C), dtype=np.int64)
     for r in range(R):
@@ -146,8 +159,10 @@ def build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages
             if cursor + n_pg > len(free_pages):
                 raise MemoryError("out of pages")
             pages.extend(int(free_pages[cursor + i]) for i in range(n_pg))
+            pages.extend([-1] * int(headroom_pages))
             cursor += n_pg
-            indptr.append(cursor)
+            row_pages.append(n_pg)
+            indptr.append(len(pages))
     kv_out = None if kv_len is None else np.array(kv_len, dtype=np.int32, copy=True)
     if (flags & FLAG_FILL_GROUP) and kv_out is not None:
         for r in range(R):
@@ -155,8 +170,50 @@ def build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages
                 kv_out[r, h] = gmax[r, cluster_of[h]]
     t = Tables(R=R, H=H, C=C, Hp=Hp, P=page_size, perm=perm, cluster_of=cluster_of,
                slot_of=slot_of, tbl_indptr=np.array(indptr, dtype=np.int64),
-               tbl_pages=np.array(pages, dtype=np.int32), n_pages_used=cursor)
+               tbl_pages=np.array(pages, dtype=np.int32), n_pages_used=cursor,
+               row_pages=np.array(row_pages, dtype=np.int32) if headroom_pages else None)
     return t, kv_out
+
+
+# --------------------------------------------------------------------------------------------
+# O12  block-table growth during decode (NEXT-4; :85-89, :244; reading A33)
+# --------------------------------------------------------------------------------------------
+def extend_tables(t: Tables, kv_len, free_pages):
+    """One block-table update for ALL (request, cluster) rows of a batch, run between two decode steps
+    ("between consecutive forward passes, a scheduling step requests the pages required for the next
+    pass", :89; the per-group block mappings of all groups updated together, :244).
+
+    Reading A33: the free list is the one the tables were built from; its first t.n_pages_used entries are
+    taken.  The rows are visited r-major then by cluster.  A row whose LONGEST head has filled the row's
+    pages (max_{h in c} kv_len[r][h] >= assigned pages x P) has no room for the next token; it takes the
+    next free page, free_pages[n_pages_used], into its first unassigned slot.  A row with no unassigned
+    slot left, or reached after the free list ran out, stays as it is and is counted as starved (its full
+    heads then drop their next row: append_kv).  At most one page per row and call: a decode step appends
+    one token per head.
+    Returns (Tables' (a modified copy), n_starved)."""
+    if t.row_pages is None:
+        raise ValueError("tables were built without growth headroom")
+    kv = np.asarray(kv_len)
+    P, C, Hp = t.P, t.C, t.Hp
+    pages = np.array(t.tbl_pages, dtype=np.int32, copy=True)
+    row_pages = np.array(t.row_pages, dtype=np.int32, copy=True)
+    cursor = int(t.n_pages_used)
+    starved = 0
+    for r in range(t.R):
+        for c in range(C):
+            row = r * C + c
+            longest = max(int(kv[r, int(t.perm[c * Hp + k])]) for k in range(Hp))
+            have = int(row_pages[row])
+            if longest < have * P:
+                continue                                  # the next token of every head still fits
+            lo, hi = int(t.tbl_indptr[row]), int(t.tbl_indptr[row + 1])
+            if have >= hi - lo or cursor >= len(free_pages):
+                starved += 1
+                continue
+            pages[lo + have] = int(free_pages[cursor])
+            cursor += 1
+            row_pages[row] = have + 1
+    return dataclasses.replace(t, tbl_pages=pages, row_pages=row_pages, n_pages_used=cursor), starved
 
 
 # --------------------------------------------------------------------------------------------
@@ -363,9 +420,10 @@ def append_kv(pool_bits: np.ndarray, t: Tables, kv_len, k_new_bits: np.ndarray, 
     pool_bits  uint16 [n_pages][Hp][2][P][d] (raw bf16 bits; a modified COPY is returned)
     k_new_bits, v_new_bits  uint16 [R][H][d]
     Rule (reading A29): the row goes to token index n = kv_len[r][h] of head h, i.e. to
-    pool[tbl_pages[tbl_indptr[r*C + c] + n // P]][slot][kv][n % P]; kv_len[r][h] becomes n + 1.  The
-    reserved budget is a hard capacity bound (:176): if n already equals the capacity of the
-    (request, cluster) table (its pages x P) the row is dropped and counted as an overflow.
+    pool[tbl_pages[tbl_indptr[r*C + c] + n // P]][slot][kv][n % P]; kv_len[r][h] becomes n + 1.  If the
+    (request, cluster) table holds no page for token n (n >= its assigned pages x P: a table without
+    growth headroom that is full, or a row that extend_tables could not serve) the row is dropped and
+    counted as an overflow.
     Returns (pool', kv_len', n_overflow)."""
     pool = np.array(pool_bits, dtype=np.uint16, copy=True)
     kv = np.array(kv_len, dtype=np.int32, copy=True)
@@ -373,9 +431,9 @@ def append_kv(pool_bits: np.ndarray, t: Tables, kv_len, k_new_bits: np.ndarray, 
     for r in range(t.R):
         for h in range(t.H):
             c, s = int(t.cluster_of[h]), int(t.slot_of[h])
-            lo, hi = int(t.tbl_indptr[r * t.C + c]), int(t.tbl_indptr[r * t.C + c + 1])
+            lo = int(t.tbl_indptr[r * t.C + c])
             n = int(kv[r, h])
-            if n >= (hi - lo) * t.P:
+            if n >= t.assigned(r * t.C + c) * t.P:
                 over += 1
                 continue
             page = int(t.tbl_pages[lo + n // t.P])
@@ -416,7 +474,7 @@ def compact_topk(pool_bits: np.ndarray, t: Tables, scores, k_dense_bits, v_dense
                 raise ValueError("keep > ctx_len")
             c, sl = int(t.cluster_of[h]), int(t.slot_of[h])
             lo, hi = int(t.tbl_indptr[r * t.C + c]), int(t.tbl_indptr[r * t.C + c + 1])
-            if k > (hi - lo) * t.P:
+            if k > t.assigned(r * t.C + c) * t.P:
                 raise ValueError("keep exceeds the table capacity")
             idx = topk_indices(np.asarray(scores[r][h])[:N], k)
             out_idx[r][h] = idx
@@ -450,7 +508,7 @@ def compact_topk_chunk(pool_bits: np.ndarray, t: Tables, scores, k_dense_bits, v
             c, sl = int(t.cluster_of[h]), int(t.slot_of[h])
             lo, hi = int(t.tbl_indptr[r * t.C + c]), int(t.tbl_indptr[r * t.C + c + 1])
             base = int(kv[r, h])
-            if base + k > (hi - lo) * t.P:
+            if base + k > t.assigned(r * t.C + c) * t.P:
                 raise ValueError("chunk exceeds the table capacity")
             idx = topk_indices(np.asarray(scores[r][h])[:N], k)
             out_idx[r][h] = idx
@@ -606,8 +664,10 @@ def _p(a: np.ndarray):
     return a.ctypes.data_as(ctypes.c_void_p)
 
 
-def attention_pairs(q, pool, t: Tables, kv_len, Hq: int, d: int, pairs, n_threads: int = 0):
-    """Attention for the listed (r, j) pairs.  Returns (out [n,d] f64, lse [n] f64, threads)."""
+def attention_pairs(q, pool, t: Tables, kv_len, Hq: int, d: int, pairs, n_threads: int = 0,
+                    sm_scale: Optional[float] = None):
+    """Attention for the listed (r, j) pairs.  Returns (out [n,d] f64, lse [n] f64, threads).
+    sm_scale: softmax scale (the scores are (q . k) * sm_scale); None = 1/sqrt(d) (reading A19)."""
     qb, pb = _u16(q), _u16(pool)
     pairs = np.ascontiguousarray(np.asarray(pairs, dtype=np.int32).reshape(-1, 2))
     kv = np.ascontiguousarray(np.asarray(kv_len, dtype=np.int32))
@@ -622,18 +682,20 @@ def attention_pairs(q, pool, t: Tables, kv_len, Hq: int, d: int, pairs, n_thread
         _p(qb), _p(pb), _p(ip), _p(pg), _p(co), _p(so), _p(kv),
         ctypes.c_int32(t.R), ctypes.c_int32(t.H), ctypes.c_int32(Hq), ctypes.c_int32(t.C),
         ctypes.c_int32(t.Hp), ctypes.c_int32(t.P), ctypes.c_int32(d), _p(pairs),
-        ctypes.c_int64(n), _p(out), _p(lse), ctypes.c_int32(n_threads))
+        ctypes.c_int64(n), ctypes.c_double(0.0 if sm_scale is None else float(sm_scale)), _p(out), _p(lse),
+        ctypes.c_int32(n_threads))
     return out, lse, int(used)
 
 
-def attention(q, pool, t: Tables, kv_len, Hq: int, d: int, n_threads: int = 0):
+def attention(q, pool, t: Tables, kv_len, Hq: int, d: int, n_threads: int = 0, sm_scale: Optional[float] = None):
     """Whole batch: out [R][Hq][d] f64, lse [R][Hq] f64."""
     pairs = [(r, j) for r in range(t.R) for j in range(Hq)]
-    out, lse, used = attention_pairs(q, pool, t, kv_len, Hq, d, pairs, n_threads)
+    out, lse, used = attention_pairs(q, pool, t, kv_len, Hq, d, pairs, n_threads, sm_scale)
     return out.reshape(t.R, Hq, d), lse.reshape(t.R, Hq), used
 
 
-def attend_range(q, pool, t: Tables, Hq: int, d: int, r: int, j: int, t0: int, t1: int):
+def attend_range(q, pool, t: Tables, Hq: int, d: int, r: int, j: int, t0: int, t1: int,
+                 sm_scale: Optional[float] = None):
     """Attention of (r, j) over tokens [t0, t1) only: (o [d] normalised in the range, lse)."""
     qb, pb = _u16(q), _u16(pool)
     out = np.zeros(d, dtype=np.float64)
@@ -646,5 +708,6 @@ def attend_range(q, pool, t: Tables, Hq: int, d: int, r: int, j: int, t0: int, t
         _p(qb), _p(pb), _p(ip), _p(pg), _p(co), _p(so),
         ctypes.c_int32(t.R), ctypes.c_int32(t.H), ctypes.c_int32(Hq), ctypes.c_int32(t.C),
         ctypes.c_int32(t.Hp), ctypes.c_int32(t.P), ctypes.c_int32(d), ctypes.c_int32(r),
-        ctypes.c_int32(j), ctypes.c_int32(t0), ctypes.c_int32(t1), _p(out), ctypes.byref(lse))
+        ctypes.c_int32(j), ctypes.c_int32(t0), ctypes.c_int32(t1),
+        ctypes.c_double(0.0 if sm_scale is None else float(sm_scale)), _p(out), ctypes.byref(lse))
     return out, float(lse.value)

@@ -410,6 +410,19 @@ def test_attention_closed_forms():
     pool2 = scatter_dense_into_pool(Kc, Vc, [[2, 2]], t2, npg)
     out, lse, _ = O.attention(qq, pool2, t2, [[2, 2]], H * G, d)
     assert np.allclose(out, cf[0]["w0"], rtol=0, atol=1e-15) and np.allclose(lse, cf[0]["lse"], rtol=0, atol=1e-15)
+    # the same inputs under a caller-supplied scale (sm_scale of tangram.h): x = [8 * 0.25, 0] = [2, 0]
+    out, lse, _ = O.attention(qq, pool2, t2, [[2, 2]], H * G, d, sm_scale=cf[2]["sm_scale"])
+    assert np.allclose(out, cf[2]["w0"], rtol=0, atol=1e-15) and np.allclose(lse, cf[2]["lse"], rtol=0, atol=1e-15)
+    o_r, l_r = O.attend_range(qq, pool2, t2, H * G, d, 0, 1, 0, 2, sm_scale=cf[2]["sm_scale"])
+    assert np.allclose(o_r, cf[2]["w0"], rtol=0, atol=1e-15) and abs(l_r - cf[2]["lse"]) < 1e-15
+    # and against dense library attention at a third scale on random data
+    q3, K3, V3, t3, pool3 = dense_case(2, 2, 3, d, [[37, 90], [64, 5]], seed=131)
+    out3, lse3, _ = O.attention(q3, pool3, t3, [[37, 90], [64, 5]], 6, d, sm_scale=0.05)
+    for r in range(2):
+        for j in range(6):
+            sc = (K3[r][j // 3].double() @ q3[r, j].double()) * 0.05
+            assert np.allclose(out3[r, j], (torch.softmax(sc, 0) @ V3[r][j // 3].double()).numpy(), rtol=0, atol=1e-12)
+            assert abs(lse3[r, j] - float(torch.logsumexp(sc, 0))) < 1e-12
     # V_h == h + 1 => out_j = floor(j / G) + 1 (pins the GQA map, reading A20) -- G = 3, H = 4
     H4, G3 = 4, 3
     lens = [[40, 9, 23, 31]]
@@ -758,3 +771,109 @@ def test_topk_indices_against_a_stable_library_sort():
         k = int(rng.integers(0, n + 1))
         want = np.sort(np.argsort(-s.astype(np.float64), kind="stable")[:k])
         assert O.topk_indices(s, k).tolist() == want.tolist()
+
+
+# ---------------------------------------------------------------------------- O12 block-table growth (NEXT-4)
+def test_extend_tables_hand_example():
+    """Hand-evaluated updates (tests/golden): which rows take a page, from where in the free list, and which starve."""
+    for case in GOLD["extend_tables"]:
+        free = np.array(case["free_pages"], dtype=np.int32)
+        t, _ = O.build_ragged_tables(np.array(case["B"]), np.array(case["reserved"], dtype=np.int32), case["n_clusters"],
+                                     case["P"], free, headroom_pages=case["headroom_pages"])
+        b = case["built"]
+        assert t.tbl_indptr.tolist() == b["tbl_indptr"] and t.tbl_pages.tolist() == b["tbl_pages"]
+        assert t.row_pages.tolist() == b["row_pages"] and t.n_pages_used == b["n_pages_used"]
+        for u in case["updates"]:
+            t, starved = O.extend_tables(t, np.array(u["kv_len"], dtype=np.int32), free)
+            assert t.tbl_pages.tolist() == u["tbl_pages"] and t.row_pages.tolist() == u["row_pages"]
+            assert t.n_pages_used == u["n_pages_used"] and starved == u["starved"]
+            assert t.tbl_indptr.tolist() == b["tbl_indptr"]                       # rows never move
+
+
+def test_headroom_zero_is_the_tight_table_and_slots_do_not_change_the_gather():
+    """headroom_pages = 0 reproduces the pinned builder bit for bit; with headroom the assigned pages are the same
+    ones in the same order (only -1 slots are interleaved), so the pinned gather O1 reads the same bytes."""
+    R, H, G, d = 2, 4, 2, 64
+    lens = np.array([[100, 20, 64, 3], [16, 90, 33, 48]], dtype=np.int32)
+    B = np.array([0.9, 0.2, 0.6, 0.3])
+    free = np.random.default_rng(5).permutation(64).astype(np.int32)
+    t0, _ = O.build_ragged_tables(B, lens, 2, 16, free)
+    t1, _ = O.build_ragged_tables(B, lens, 2, 16, free, headroom_pages=3)
+    assert t0.row_pages is None and t1.n_pages_used == t0.n_pages_used
+    assert t1.tbl_pages[t1.tbl_pages >= 0].tolist() == t0.tbl_pages.tolist()
+    for row in range(R * 2):
+        n = t0.tbl_indptr[row + 1] - t0.tbl_indptr[row]
+        assert t1.row_pages[row] == n == t1.assigned(row) and t1.tbl_indptr[row + 1] - t1.tbl_indptr[row] == n + 3
+        assert np.array_equal(t1.tbl_pages[t1.tbl_indptr[row]:t1.tbl_indptr[row] + n],
+                              t0.tbl_pages[t0.tbl_indptr[row]:t0.tbl_indptr[row + 1]])
+        assert np.all(t1.tbl_pages[t1.tbl_indptr[row] + n:t1.tbl_indptr[row + 1]] == -1)
+    g = torch.Generator().manual_seed(6)
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    pool = torch.randn(64, 2, 2, 16, d, generator=g).bfloat16()
+    a, b = O.attention(q, pool, t0, lens, H * G, d)[:2], O.attention(q, pool, t1, lens, H * G, d)[:2]
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_extend_then_append_round_trip_through_page_boundaries():
+    """A decode loop of 70 steps (extend the tables, then append one row per head) crosses several page
+    boundaries in every row and drops nothing; the pinned gather O1 then finds the prefill rows followed by all
+    appended rows: attention = dense library attention over them.  The pages are a duplicate-free prefix of the
+    free list, and every row ends with exactly the pages the pinned builder gives a batch whose reservation is
+    the final length + 1 (the same tables up to which physical page sits where)."""
+    R, H, G, d, P, steps, C = 2, 4, 2, 64, 16, 70, 2
+    B = np.array([0.9, 0.2, 0.6, 0.3])
+    lens0 = np.array([[40, 10, 33, 16], [16, 5, 20, 7]], dtype=np.int32)
+    free = np.random.default_rng(8).permutation(80).astype(np.int32)
+    t, _ = O.build_ragged_tables(B, lens0, C, P, free, headroom_pages=6)
+    g = torch.Generator().manual_seed(9)
+    K0 = [[torch.randn(int(lens0[r][h]), d, generator=g).bfloat16() for h in range(H)] for r in range(R)]
+    V0 = [[torch.randn(int(lens0[r][h]), d, generator=g).bfloat16() for h in range(H)] for r in range(R)]
+    pool = scatter_dense_into_pool(K0, V0, lens0, t, 80, seed=10)
+    bits = pool.view(torch.int16).numpy().view(np.uint16).copy()
+    Ks = torch.randn(steps, R, H, d, generator=g).bfloat16()
+    Vs = torch.randn(steps, R, H, d, generator=g).bfloat16()
+    kv = lens0.copy()
+    for s_ in range(steps):
+        t, starved = O.extend_tables(t, kv, free)
+        assert starved == 0
+        bits, kv, over = O.append_kv(bits, t, kv, Ks[s_].view(torch.int16).numpy().view(np.uint16),
+                                     Vs[s_].view(torch.int16).numpy().view(np.uint16))
+        assert over == 0
+    assert np.array_equal(kv, lens0 + steps)
+    used = t.tbl_pages[t.tbl_pages >= 0]
+    assert len(set(used.tolist())) == len(used) == t.n_pages_used
+    assert sorted(used.tolist()) == sorted(free[:t.n_pages_used].tolist())
+    tight, _ = O.build_ragged_tables(B, kv, C, P, free)          # reservation = final length: ceil(n / P) pages
+    for row in range(R * C):
+        # the row grew when its longest head filled a page, i.e. it holds floor((longest - 1) / P) + 1 pages
+        # (the page of the last appended token) -- the pinned builder's count for these lengths
+        assert t.assigned(row) == tight.tbl_indptr[row + 1] - tight.tbl_indptr[row]
+    q = torch.randn(R, H * G, d, generator=g).bfloat16()
+    out, lse, _ = O.attention(q, torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16), t, kv, H * G, d)
+    for r in range(R):
+        for j in range(H * G):
+            h = j // G
+            Kd = torch.cat([K0[r][h], Ks[:, r, h]]).double()
+            Vd = torch.cat([V0[r][h], Vs[:, r, h]]).double()
+            sc = (Kd @ q[r, j].double()) / math.sqrt(d)
+            assert np.allclose(out[r, j], (torch.softmax(sc, 0) @ Vd).numpy(), rtol=0, atol=1e-12)
+            assert abs(lse[r, j] - float(torch.logsumexp(sc, 0))) < 1e-12
+
+
+def test_extend_tables_starvation_drops_exactly_the_unserved_rows():
+    """Free list shorter than the growth: rows are served in (request, cluster) order until it runs out; the heads
+    of an unserved row that are full drop their row and are counted (reading A29), the others keep growing."""
+    R, H, P, C, d = 2, 2, 16, 2, 8
+    B = np.array([0.3, 0.8])
+    lens0 = np.array([[16, 32], [16, 16]], dtype=np.int32)        # every row is exactly full
+    free = np.arange(100, 107, dtype=np.int32)                    # 5 pages to build with, 2 left for 4 rows
+    t, _ = O.build_ragged_tables(B, lens0, C, P, free, headroom_pages=2)
+    assert t.n_pages_used == 5
+    t, starved = O.extend_tables(t, lens0, free)
+    assert starved == 2 and t.row_pages.tolist() == [2, 3, 1, 1] and t.n_pages_used == 7
+    bits = np.zeros((107, 1, 2, P, d), dtype=np.uint16)
+    k = np.full((R, H, d), 7, dtype=np.uint16)
+    _, kv, over = O.append_kv(bits, t, lens0, k, k)
+    assert over == 2 and kv.tolist() == [[17, 33], [16, 16]]
+    t2, starved2 = O.extend_tables(t, kv, free)                   # nothing left: the same two rows starve again
+    assert starved2 == 2 and np.array_equal(t2.tbl_pages, t.tbl_pages)
