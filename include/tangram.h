@@ -67,26 +67,39 @@ int tangram_reserve_budgets(const double* mu, const double* sigma, double alpha,
  * takes the next entries of free_pages in order, rows visited r-major then c.  Page layout in the
  * pool (bf16): pool[page][slot][kv][token][d], kv 0 = K, 1 = V, slot = slot_of[head].
  *
+ * Growth during decode (NEXT-4, "a scheduling step requests the pages required for the
+ * next pass", :244 Vectorized Block Table): with out->headroom_pages = h > 0 every row is followed by
+ * h page SLOTS that hold no page yet (tbl_pages = -1), so that tangram_extend_tables /
+ * tangram_extend_tables_device can hand a row its next page without moving any row; out->row_pages
+ * (required then) receives the pages each row holds.  With headroom_pages = 0 and row_pages = NULL
+ * the tables are tight (every slot holds a page), as :172 reserves them at admission.
+ *
  *   B            host [H] f64 (from a1)            reserved  host [R][H] i32 (from a1)
  *   free_pages   host [n_free] i32 page ids the caller's allocator hands out (not modified)
  *   flags        TANGRAM_FILL_GROUP: kv_len_inout[r][h] := max reserved of h's cluster (:235)
  *   kv_len_inout host [R][H] i32 or NULL (only touched with TANGRAM_FILL_GROUP)
  *   out          caller-filled: perm/cluster_of/slot_of [H], tbl_indptr [R*C+1], tbl_pages
- *                [tbl_pages_cap] (or tbl_pages == NULL to query: only n_pages_used is written).
- *                On success R,H,C,Hp,P, the arrays and n_pages_used are written.
- * Errors: INVALID_ARG (H % n_clusters != 0, page_size <= 0, ...); OUT_OF_PAGES if the free list is
- * too short (n_pages_used = pages needed; arrays untouched); BUFFER_TOO_SMALL if tbl_pages_cap <
- * pages needed (n_pages_used = pages needed). */
+ *                [tbl_pages_cap] (or tbl_pages == NULL to query: only n_pages_used / n_slots are
+ *                written), headroom_pages (in), row_pages [R*C] (or NULL if headroom_pages == 0).
+ *                On success R,H,C,Hp,P, the arrays, n_pages_used and n_slots are written.
+ * Errors: INVALID_ARG (H % n_clusters != 0, page_size <= 0, headroom_pages < 0 or > 0 without
+ * row_pages, ...); OUT_OF_PAGES if the free list is too short (n_pages_used = pages needed; arrays
+ * untouched); BUFFER_TOO_SMALL if tbl_pages_cap < n_slots (n_pages_used / n_slots = needed). */
 #define TANGRAM_FILL_GROUP 1u
 typedef struct tangram_tables {
     int32_t R, H, C, Hp, P;
     int32_t* perm;        /* host [H]  sorted position -> head (pi of :229) */
     int32_t* cluster_of;  /* host [H]  head -> cluster */
     int32_t* slot_of;     /* host [H]  head -> slot inside the cluster's pages */
-    int64_t* tbl_indptr;  /* host [R*C+1]  CSR row pointer, row = r*C + c */
-    int32_t* tbl_pages;   /* host [tbl_pages_cap]  page ids, row after row */
+    int64_t* tbl_indptr;  /* host [R*C+1]  CSR row pointer, row = r*C + c: the row owns page slots
+                             [tbl_indptr[row], tbl_indptr[row+1]) */
+    int32_t* tbl_pages;   /* host [tbl_pages_cap]  page id of every slot, row after row; -1 = no page yet */
     int64_t tbl_pages_cap;
-    int64_t n_pages_used;
+    int64_t n_pages_used; /* pages taken from the free list so far (the free list's cursor) */
+    int32_t headroom_pages; /* in: unassigned slots kept behind every row for growth (0 = tight tables) */
+    int32_t reserved_;
+    int32_t* row_pages;   /* host [R*C] pages each row holds (its first row_pages slots), or NULL: all slots */
+    int64_t n_slots;      /* out: tbl_indptr[R*C] = entries of tbl_pages = n_pages_used + R*C*headroom at build */
 } tangram_tables;
 int tangram_build_ragged_tables(const double* B, const int32_t* reserved, int32_t R, int32_t H,
                                 int32_t n_clusters, int32_t page_size, const int32_t* free_pages,
@@ -184,15 +197,24 @@ typedef struct tangram_device_plan {
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
     const int64_t* worker_indptr; /* device [W+1] */
     const void* list_heads;       /* device [W] 128-byte list heads: item range, first item, its first 16 page ids */
-    const int32_t* seq_info;      /* device [R*H][4]: {page-table row offset, capacity in tokens, slot, 0} */
+    const int32_t* seq_info;      /* device [R*H][4]: {first slot of the head's row, slot capacity in tokens, slot in
+                                     the page, row index r*C + c} */
     const int64_t* part_indptr;   /* device [R*H+1] */
     const int32_t* tbl_pages;     /* device page ids */
     int32_t* sched;               /* device [4]: list-claim / CTAs-done counters of the dynamic tail and the
                                      grid-barrier counters of the in-kernel merge; zero between launches
                                      (the kernel re-arms them itself) */
     int64_t max_merge_parts;      /* most parts any sequence has (sizes the column split of the big-record merge) */
-    int64_t min_pool_pages;       /* largest page id in the tables + 1: the device calls return INVALID_ARG for a
-                                     kv_pool with fewer pages */
+    int64_t min_pool_pages;       /* largest page id in the tables at upload + 1: the device calls return INVALID_ARG
+                                     for a kv_pool with fewer pages */
+    /* block-table state on the device (NEXT-4); all arrays live in the blob */
+    int64_t n_slots;              /* entries of tbl_pages (assigned pages + growth slots) */
+    const int32_t* row_ptr;       /* device [R*C+1]: first slot of every (request, cluster) row */
+    int32_t* row_pages;           /* device [R*C]: pages each row holds */
+    const int32_t* perm;          /* device [H]: sorted position -> head (cluster c = perm[c*Hp .. (c+1)*Hp)) */
+    int32_t* seq_cap;             /* device [R*H]: tokens the pages of head h's row hold (row_pages x P) */
+    const int32_t* plan_cover;    /* device [R*H]: largest tok_end any item of the plan has for the sequence */
+    int32_t* grow_state;          /* device [4]: {free-list cursor, rows starved so far, 0, 0} */
 } tangram_device_plan;
 
 /* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte
@@ -200,6 +222,11 @@ typedef struct tangram_device_plan {
  * arrays may be freed when the call returns. */
 int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
                    void* stream, tangram_device_plan* dp);
+
+/* Zeroes the launch-state counters of an uploaded plan (dp->sched) on `stream`.  The kernels re-arm the counters
+ * themselves at the end of every launch that runs to completion; this call is for recovery after a launch that
+ * did not (an aborted process, a fault), or after two launches on one plan were wrongly overlapped. */
+int tangram_reset_plan(const tangram_device_plan* dp, void* stream);
 
 /* Workspace for the split-KV partials: n_part_slots x G x (d + 1) fp32, rounded up. */
 size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_dim);
@@ -265,8 +292,9 @@ int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d,
 /* ------------------------------------------------------------------------------------------------
  * NEXT-1  KV append of one decode step.  The new K row and V row of every (request,
  * KV head) are written behind its retained tokens in the ragged pages (:190 page layout), and its length
- * grows by one.  The reserved budget is a hard capacity bound (:176): a head whose (request, cluster)
- * table is full (pages x P tokens) keeps its length, its row is dropped and counted.
+ * grows by one.  A head whose (request, cluster) row holds no page for the new token (row_pages x P tokens
+ * are full: tight tables, or a row the table growth above could not serve) keeps its length; its row is
+ * dropped and counted.
  *
  *   dp            from tangram_upload (uses the tables only)
  *   k_new, v_new  device [R][H][d] bf16, 16-byte aligned
@@ -277,6 +305,78 @@ int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d,
 int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const void* v_new, void* kv_pool,
                       int64_t n_pool_pages, int32_t d, int32_t* kv_len_dev, int32_t* overflow_dev,
                       void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-4 (second half)  Vectorized Block Table: growing the page tables during decode.
+ * PAPER.md:89 ("between consecutive forward passes, a scheduling step requests the pages required for the next
+ * pass from the Block Pool"), :244 (the per-group block mappings of all groups are aggregated into a Vectorized
+ * Block Table and updated together -- OpenMP across head groups, SIMD inside a group -- because the cost grows with
+ * the number of groups, O(N_req x H / H_p)), :176 (what overflow means: truncation of the compressor's selection,
+ * not the loss of decode tokens).
+ *
+ * One update visits every (request, cluster) row, r-major then by cluster.  A row whose LONGEST head has filled
+ * the row's pages (max_{h in c} kv_len[r][h] >= row_pages x P) takes the next page of the free list -- the list
+ * the tables were built from, whose first n_pages_used entries are taken -- into its first unassigned slot.  A row
+ * with no unassigned slot left (headroom used up), or reached after the free list ran out, stays as it is and is
+ * counted as starved; only then does tangram_append_kv / tangram_decode_step drop that row's next token.  At most
+ * one page per row and call (a decode step appends one token per head).  Results are bit-exact against the oracle
+ * (O12) on either path.
+ *
+ * Host path (a scheduler that owns the tables): tangram_extend_tables updates *t in place; the rows that need a
+ * page are found for all groups at once (OpenMP across (cluster, block of requests), AVX-512 gathers / max /
+ * compare inside a block when the CPU has it, else the same loop in scalar code), then the pages are handed out
+ * in row order.  tangram_sync_tables copies the tables' current state over the device copy of an uploaded plan.
+ *   t           tables built with headroom_pages > 0 (row_pages present); updated in place
+ *   kv_len      host [R][H] i32 current lengths          free_pages host [n_free] i32, the build's free list
+ *   n_threads   OpenMP threads for the row scan; <= 0: one thread per 2048 rows, at most the OpenMP default
+ *   n_extended_out / n_starved_out  host, may be NULL: rows that took a page / rows that needed one and got none
+ * Errors: INVALID_ARG.
+ *
+ * Device path (zero host work per step, CUDA-graph capturable): tangram_extend_tables_device runs the same update
+ * on the device copy (one small kernel: a block-wide ordered scan over the rows); the free-list cursor and the
+ * starved count live in dp->grow_state.  tangram_decode_step below runs it inside the decode kernel.
+ *   free_pages_dev  device [n_free] i32: the free list the tables were built from (every entry must be a page of
+ *                   the pool the attention calls are given; the device calls cannot check that)
+ * tangram_download_tables copies the device state (tbl_pages, row_pages, n_pages_used) back into *t (host arrays
+ * sized as at build time) and synchronises the stream. */
+int tangram_extend_tables(tangram_tables* t, const int32_t* kv_len, const int32_t* free_pages, int64_t n_free,
+                          int32_t n_threads, int64_t* n_extended_out, int64_t* n_starved_out);
+int tangram_extend_tables_device(const tangram_device_plan* dp, const int32_t* kv_len_dev, const int32_t* free_pages_dev,
+                                 int64_t n_free, void* stream);
+int tangram_sync_tables(const tangram_tables* t, const tangram_device_plan* dp, void* stream);
+int tangram_download_tables(const tangram_device_plan* dp, tangram_tables* t, int64_t* n_starved_out, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * One decode step of one layer in ONE launch: KV append (NEXT-1) + split-KV attention (a4) + LSE merge (a5) +
+ * block-table update for the next step (NEXT-4), on an OPEN-ENDED plan (built for the tables' slot capacity).
+ *
+ *   1. append   the new K / V row of every (request, KV head) goes to token index n = kv_len[r][h] of its ragged
+ *               pages if its row holds a page for that token (n < row_pages x P), else it is dropped and counted
+ *               in *overflow_dev.  The row is written by the CTA whose work item covers token n, just before it
+ *               streams that item -- no extra launch, no grid-wide dependency.
+ *   2. attend   exactly as tangram_decode_attention over the n + 1 tokens (the new one included).
+ *   3. lengths  kv_len_dev[r][h] becomes n + 1 (unchanged for a dropped row).
+ *   4. grow     if free_pages_dev != NULL: the block-table update described above, with the new lengths, so that
+ *               the NEXT step's token has a page.  (Run tangram_extend_tables_device once before the first step.)
+ * Steps 3 and 4 run after the grid barrier of the in-kernel merge, on one CTA, while the others merge; when the
+ * grid cannot be launched cooperatively (or d = 256) they run in a small follow-up kernel.
+ * The composition is bit-exact against the oracle's extend_tables -> append_kv -> attention for the pool, the
+ * lengths, the tables and the counters; the attention output is within the a4 tolerances.
+ *
+ *   k_new, v_new  device [R][H][d] bf16, 16-byte aligned          kv_pool  device, read and written
+ *   kv_len_dev    device [R][H] i32 (required), read, then incremented
+ *   flags         TANGRAM_STEP_OVERLAP: the caller guarantees that the work preceding this call on the stream
+ *                 writes nothing this call reads except q, k_new and v_new (true for the layers of one decode
+ *                 step).  The kernel is then launched with programmatic stream serialization and fetches its
+ *                 work lists, page ids and first KV tiles while its predecessor drains; it waits for the
+ *                 predecessor (griddepcontrol.wait) before touching q / k_new / v_new.
+ *   all other arguments as for tangram_decode_attention.
+ * Errors: as tangram_decode_attention, plus INVALID_ARG for kv_len_dev == NULL. */
+#define TANGRAM_STEP_OVERLAP 1u
+int tangram_decode_step(const tangram_device_plan* dp, const void* q, const void* k_new, const void* v_new,
+                        void* kv_pool, int64_t n_pool_pages, int32_t* kv_len_dev, const int32_t* free_pages_dev,
+                        int64_t n_free, int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
+                        size_t workspace_bytes, int32_t* overflow_dev, uint32_t flags, uint64_t* worker_ns, void* stream);
 
 /* ------------------------------------------------------------------------------------------------
  * NEXT-2  Per-head Top-k selection + compaction into the ragged pages.

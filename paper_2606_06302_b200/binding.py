@@ -41,7 +41,8 @@ class _Tables(C.Structure):
     _fields_ = [("R", C.c_int32), ("H", C.c_int32), ("C", C.c_int32), ("Hp", C.c_int32), ("P", C.c_int32),
                 ("perm", C.c_void_p), ("cluster_of", C.c_void_p), ("slot_of", C.c_void_p),
                 ("tbl_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("tbl_pages_cap", C.c_int64),
-                ("n_pages_used", C.c_int64)]
+                ("n_pages_used", C.c_int64), ("headroom_pages", C.c_int32), ("reserved_", C.c_int32),
+                ("row_pages", C.c_void_p), ("n_slots", C.c_int64)]
 
 
 class _Plan(C.Structure):
@@ -58,7 +59,9 @@ class _DevicePlan(C.Structure):
                 ("merge_seqs", C.c_void_p),
                 ("items", C.c_void_p), ("worker_indptr", C.c_void_p), ("list_heads", C.c_void_p),
                 ("seq_info", C.c_void_p), ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p),
-                ("max_merge_parts", C.c_int64), ("min_pool_pages", C.c_int64)]
+                ("max_merge_parts", C.c_int64), ("min_pool_pages", C.c_int64), ("n_slots", C.c_int64),
+                ("row_ptr", C.c_void_p), ("row_pages", C.c_void_p), ("perm", C.c_void_p), ("seq_cap", C.c_void_p),
+                ("plan_cover", C.c_void_p), ("grow_state", C.c_void_p)]
 
 
 _lib.tangram_last_error.restype = C.c_char_p
@@ -71,7 +74,9 @@ for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram
               "tangram_query_max_ctas", "tangram_upload", "tangram_decode_attention", "tangram_decode_partials",
               "tangram_merge_partials", "tangram_append_kv", "tangram_compact_topk",
               "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios",
-              "tangram_compact_topk_chunk", "tangram_stage_from_host", "tangram_default_dynamic_tail"):
+              "tangram_compact_topk_chunk", "tangram_stage_from_host", "tangram_default_dynamic_tail",
+              "tangram_extend_tables", "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables",
+              "tangram_decode_step", "tangram_reset_plan"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
@@ -79,7 +84,10 @@ EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragge
            "tangram_workspace_bytes", "tangram_decode_attention", "tangram_decode_partials", "tangram_merge_partials", "tangram_append_kv",
            "tangram_compact_workspace_bytes", "tangram_compact_topk", "tangram_account_pages",
            "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk",
-           "tangram_stage_from_host", "tangram_default_dynamic_tail")
+           "tangram_stage_from_host", "tangram_default_dynamic_tail", "tangram_extend_tables",
+           "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables", "tangram_decode_step",
+           "tangram_reset_plan")
+STEP_OVERLAP = 1
 
 
 def _check(rc: int):
@@ -120,14 +128,16 @@ class Tables:
     perm: np.ndarray
     cluster_of: np.ndarray
     slot_of: np.ndarray
-    tbl_indptr: np.ndarray
-    tbl_pages: np.ndarray
-    n_pages_used: int
+    tbl_indptr: np.ndarray     # [R*C+1] i64: row r*C+c owns the page slots [indptr[row], indptr[row+1])
+    tbl_pages: np.ndarray      # [n_slots] i32 page id per slot, -1 = no page yet (growth headroom)
+    n_pages_used: int          # pages taken from the free list so far
+    headroom_pages: int = 0
+    row_pages: Optional[np.ndarray] = None   # [R*C] i32 pages each row holds (None: tight tables, every slot)
 
     def _c(self) -> _Tables:
         return _Tables(self.R, self.H, self.C, self.Hp, self.P, _ptr(self.perm), _ptr(self.cluster_of),
                        _ptr(self.slot_of), _ptr(self.tbl_indptr), _ptr(self.tbl_pages), len(self.tbl_pages),
-                       self.n_pages_used)
+                       self.n_pages_used, self.headroom_pages, 0, _ptr(self.row_pages), len(self.tbl_pages))
 
 
 def tangram_pages_needed(B, reserved, n_clusters: int, page_size: int) -> int:
@@ -143,23 +153,39 @@ def tangram_pages_needed(B, reserved, n_clusters: int, page_size: int) -> int:
 
 
 def tangram_build_ragged_tables(B, reserved, n_clusters: int, page_size: int, free_pages, flags: int = 0,
-                                kv_len=None):
-    """-> (Tables, kv_len').  kv_len' is a copy of kv_len (raised to the cluster capacity with FILL_GROUP)."""
+                                kv_len=None, headroom_pages: int = 0):
+    """-> (Tables, kv_len').  kv_len' is a copy of kv_len (raised to the cluster capacity with FILL_GROUP).
+    headroom_pages > 0: growable tables (every row followed by that many empty page slots, row_pages filled)."""
     B, reserved = _np(B, np.float64), _np(reserved, np.int32)
     free = _np(free_pages, np.int32)
     R, H = reserved.shape
     kv = None if kv_len is None else _np(kv_len, np.int32).reshape(R, H).copy()
     need = tangram_pages_needed(B, reserved, n_clusters, page_size)
+    n_rows = R * max(1, n_clusters)
+    n_slots = need + n_rows * max(0, headroom_pages)
     t = Tables(R, H, n_clusters, H // max(1, n_clusters), page_size, np.zeros(H, np.int32), np.zeros(H, np.int32),
-               np.zeros(H, np.int32), np.zeros(R * n_clusters + 1, np.int64), np.zeros(max(need, 1), np.int32), 0)
+               np.zeros(H, np.int32), np.zeros(R * n_clusters + 1, np.int64), np.zeros(max(n_slots, 1), np.int32), 0,
+               headroom_pages, np.zeros(n_rows, np.int32) if headroom_pages > 0 else None)
     ct = t._c()
     _check(_lib.tangram_build_ragged_tables(_ptr(B), _ptr(reserved), C.c_int32(R), C.c_int32(H),
                                             C.c_int32(n_clusters), C.c_int32(page_size), _ptr(free),
                                             C.c_int64(free.shape[0]), C.c_uint32(flags), _ptr(kv), C.byref(ct)))
     t.n_pages_used = int(ct.n_pages_used)
-    t.tbl_pages = t.tbl_pages[:t.n_pages_used]
+    t.tbl_pages = t.tbl_pages[:int(ct.n_slots)]
     t.Hp, t.C = int(ct.Hp), int(ct.C)
     return t, kv
+
+
+def tangram_extend_tables(t: Tables, kv_len, free_pages, n_threads: int = 0):
+    """NEXT-4 (host): one Vectorized Block Table update of `t` in place -> (rows extended, rows starved)."""
+    kv, free = _np(kv_len, np.int32), _np(free_pages, np.int32)
+    assert kv.shape == (t.R, t.H) and t.row_pages is not None
+    ct = t._c()
+    ext, starved = C.c_int64(0), C.c_int64(0)
+    _check(_lib.tangram_extend_tables(C.byref(ct), _ptr(kv), _ptr(free), C.c_int64(free.shape[0]), C.c_int32(n_threads),
+                                      C.byref(ext), C.byref(starved)))
+    t.n_pages_used = int(ct.n_pages_used)
+    return int(ext.value), int(starved.value)
 
 
 # ------------------------------------------------------------------------------------------ a3
@@ -283,6 +309,75 @@ def tangram_merge_partials(dp: DevicePlan, out, lse, workspace, stream=None):
     _check(_lib.tangram_merge_partials(C.byref(dp.c), C.c_int32(Hq), C.c_int32(d), C.c_void_p(out.data_ptr()),
                                        C.c_void_p(lse.data_ptr()), C.c_void_p(workspace.data_ptr()),
                                        C.c_size_t(workspace.numel()), sp))
+    return out, lse
+
+
+def _stream_ptr(stream):
+    import torch
+    return C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+
+
+def tangram_extend_tables_device(dp: DevicePlan, kv_len, free_pages, stream=None):
+    """NEXT-4 (device): the same update on the uploaded tables; kv_len [R,H] / free_pages [n_free] int32 cuda."""
+    import torch
+    assert kv_len.is_cuda and kv_len.dtype == torch.int32 and kv_len.is_contiguous() and kv_len.numel() == dp.c.R * dp.c.H
+    assert free_pages.is_cuda and free_pages.dtype == torch.int32 and free_pages.is_contiguous()
+    _check(_lib.tangram_extend_tables_device(C.byref(dp.c), C.c_void_p(kv_len.data_ptr()), C.c_void_p(free_pages.data_ptr()),
+                                             C.c_int64(free_pages.numel()), _stream_ptr(stream)))
+
+
+def tangram_sync_tables(t: Tables, dp: DevicePlan, stream=None):
+    """Host tables -> device copy of an uploaded plan (after tangram_extend_tables on the host)."""
+    ct = t._c()
+    _check(_lib.tangram_sync_tables(C.byref(ct), C.byref(dp.c), _stream_ptr(stream)))
+
+
+def tangram_download_tables(dp: DevicePlan, t: Tables, stream=None) -> int:
+    """Device state (tbl_pages, row_pages, free-list cursor) -> `t` in place; returns the rows starved so far."""
+    assert t.row_pages is not None
+    ct = t._c()
+    starved = C.c_int64(0)
+    _check(_lib.tangram_download_tables(C.byref(dp.c), C.byref(ct), C.byref(starved), _stream_ptr(stream)))
+    t.n_pages_used = int(ct.n_pages_used)
+    return int(starved.value)
+
+
+def tangram_reset_plan(dp: DevicePlan, stream=None):
+    _check(_lib.tangram_reset_plan(C.byref(dp.c), _stream_ptr(stream)))
+
+
+def tangram_decode_step(dp: DevicePlan, q, k_new, v_new, kv_pool, kv_len, free_pages=None, out=None, lse=None,
+                        workspace=None, sm_scale: float = 0.0, overflow=None, flags: int = 0, worker_ns=None, stream=None):
+    """One decode step of one layer in one launch: KV append + attention + merge + length update + table growth
+    for the next step (include/tangram.h).  kv_len [R,H] int32 cuda is incremented in place."""
+    import torch
+    assert (q.is_cuda or q.is_pinned()) and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
+    assert q.is_contiguous() and kv_pool.is_contiguous()
+    R, Hq, d = q.shape
+    H = dp.c.H
+    assert tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d) and R == dp.c.R
+    for x in (k_new, v_new):
+        assert x.is_cuda and x.dtype == torch.bfloat16 and x.is_contiguous() and tuple(x.shape) == (R, H, d)
+    assert kv_len.is_cuda and kv_len.dtype == torch.int32 and kv_len.is_contiguous() and kv_len.numel() == R * H
+    G = Hq // H
+    if out is None:
+        out = torch.empty(R, Hq, d, dtype=torch.bfloat16, device=kv_pool.device)
+    if lse is None:
+        lse = torch.empty(R, Hq, dtype=torch.float32, device=kv_pool.device)
+    if workspace is None:
+        workspace = torch.empty(tangram_workspace_bytes(int(dp.c.n_part_slots), G, d), dtype=torch.uint8, device=kv_pool.device)
+    fp, nf = None, 0
+    if free_pages is not None:
+        assert free_pages.is_cuda and free_pages.dtype == torch.int32 and free_pages.is_contiguous()
+        fp, nf = C.c_void_p(free_pages.data_ptr()), free_pages.numel()
+    ov = C.c_void_p(overflow.data_ptr()) if overflow is not None else None
+    wn = C.c_void_p(worker_ns.data_ptr()) if worker_ns is not None else None
+    _check(_lib.tangram_decode_step(C.byref(dp.c), C.c_void_p(q.data_ptr()), C.c_void_p(k_new.data_ptr()),
+                                    C.c_void_p(v_new.data_ptr()), C.c_void_p(kv_pool.data_ptr()), C.c_int64(kv_pool.shape[0]),
+                                    C.c_void_p(kv_len.data_ptr()), fp, C.c_int64(nf), C.c_int32(Hq), C.c_int32(d),
+                                    C.c_float(sm_scale), C.c_void_p(out.data_ptr()), C.c_void_p(lse.data_ptr()),
+                                    C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), ov, C.c_uint32(flags),
+                                    wn, _stream_ptr(stream)))
     return out, lse
 
 

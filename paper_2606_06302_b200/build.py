@@ -33,8 +33,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
     cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-           "-Xcompiler", "-fPIC,-ffp-contract=off", "-Xptxas", "-v" if verbose else "-O3",
-           "-shared", "-o", LIB, "-I", os.path.join(ROOT, "include"), "-I", CSRC] + SOURCES
+           "-Xcompiler", "-fPIC,-ffp-contract=off,-fopenmp", "-Xptxas", "-v" if verbose else "-O3",
+           "-shared", "-lgomp", "-o", LIB, "-I", os.path.join(ROOT, "include"), "-I", CSRC] + SOURCES
     if verbose:
         print(" ".join(cmd))
     subprocess.check_call(cmd)

@@ -55,7 +55,7 @@ __device__ __forceinline__ uint32_t score_key(float x) {
 }
 
 __global__ void __launch_bounds__(1024)
-compact_prepare_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ ctx_len,
+compact_prepare_kernel(const int32_t* __restrict__ seq_cap, const int32_t* __restrict__ ctx_len,
                        const int32_t* __restrict__ keep, int32_t* __restrict__ kv_len, int n_seq, int H,
                        int32_t* __restrict__ counter, int32_t* __restrict__ keep_eff, int32_t* __restrict__ base,
                        int32_t* __restrict__ tile_indptr, int32_t* __restrict__ clamped) {
@@ -70,7 +70,7 @@ compact_prepare_kernel(const int4* __restrict__ seq_info, const int32_t* __restr
         if (seq < n_seq) {
             const int want = keep[seq];
             const int have = kv_len ? kv_len[seq] : 0;  // chunked prefill: the rows go behind what the head holds
-            const int cap = min(ctx_len[seq / H], seq_info[seq].y - have);  // {table row offset, capacity tokens, slot, -}
+            const int cap = min(ctx_len[seq / H], seq_cap[seq] - have);  // seq_cap: tokens the pages of the head's row hold
             const int k = max(0, min(want, cap));
             bad = k != want;
             keep_eff[seq] = k;
@@ -551,7 +551,7 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
     CompactWs w{ws, ws + 4, ws + 4 + n_seq, ws + 4 + 2 * n_seq};
     const int4* seq_info = reinterpret_cast<const int4*>(dp->seq_info);
 
-    compact_prepare_kernel<<<1, 1024, 0, st>>>(seq_info, ctx_len_dev, keep_dev, kv_len_dev, n_seq, dp->H, w.counter,
+    compact_prepare_kernel<<<1, 1024, 0, st>>>(dp->seq_cap, ctx_len_dev, keep_dev, kv_len_dev, n_seq, dp->H, w.counter,
                                                w.keep_eff, w.base, w.tile_indptr, clamped_dev);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");

@@ -40,7 +40,9 @@ constexpr int kPage = 16;          // tokens per page the kernels are specialise
 // three-stage rings would not fit in shared memory
 template <int D>
 constexpr int consumer_warps() { return D == 256 ? 4 : 8; }
-constexpr int kQSlots = 2;         // item / query ring depth
+constexpr int kMinQSlots = 2;      // item / query ring depth: as deep as shared memory allows, 2 .. 8 (runtime).  A deep
+constexpr int kMaxQSlots = 8;      // ring lets the producer fetch query groups several items ahead, which is what hides
+                                   // the bus round trip when q lives in pinned host memory
 constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime <= this)
 constexpr int kMaxG = 8;
 constexpr int kSmemLimit = 232448; // 227 KB opt-in limit per CTA
@@ -49,6 +51,21 @@ constexpr int kRunSplit = 1, kRunMerge = 2;
 #define TANGRAM_CLAIM_TILES 16
 #endif
 constexpr int kClaimTiles = TANGRAM_CLAIM_TILES;  // how many tiles before the end of a list its successor is claimed
+
+// Block-table state of an uploaded plan as the growth code sees it (NEXT-4).
+struct GrowParams {
+    const int32_t* row_ptr;      // [n_rows + 1] first slot of every (request, cluster) row
+    int32_t* row_pages;          // [n_rows] pages a row holds
+    const int32_t* perm;         // [H]
+    int32_t* tbl_pages;          // page id per slot, -1 = none yet
+    int32_t* seq_cap;            // [R*H] row_pages x P of the head's row
+    const int32_t* plan_cover;   // [R*H] tokens the plan's items cover
+    int32_t* kv_len;             // [R*H]
+    int32_t* grow_state;         // {free-list cursor, rows starved so far}
+    const int32_t* free_pages;   // [n_free] or nullptr: no growth
+    int32_t* overflow;           // dropped rows, or nullptr
+    int32_t n_free, n_rows, R, H, C, Hp;
+};
 
 struct DecodeParams {
     const DeviceItem* items;
@@ -66,9 +83,18 @@ struct DecodeParams {
     const void* list_heads;     // [n_lists] 128-byte list heads
     const int32_t* kv_len;      // [R*H] run-time lengths (open-ended plan) or nullptr: items are taken as planned
     int32_t H;
-    int32_t Hq, G, Hp, n_stages, n_lists;
+    int32_t Hq, G, Hp, n_stages, n_qslots, n_lists;
     int32_t tail_merge, n_merge_units, n_merge_small, merge_split;
     float scale_log2;
+    // fused decode step (tangram_decode_step): KV append by the CTA that streams the sequence's last item, the
+    // length update and the block-table growth for the next step after the grid barrier; all nullptr / 0 otherwise
+    const uint4* k_new;          // [R*H][d/8] or nullptr: no append
+    const uint4* v_new;
+    uint4* pool_w;               // the page pool, writable view
+    const int32_t* seq_cap;      // [R*H] tokens the row's pages hold
+    int32_t* kv_len_w;           // = kv_len, writable
+    GrowParams grow;
+    int32_t pdl;                 // launched with programmatic stream serialization: wait before reading q / k_new / v_new
 };
 
 // ------------------------------------------------------------------ shared-memory carve-up
@@ -81,22 +107,29 @@ struct Smem {
     static constexpr int kRowF = D + 8;                      // padded fp32 row of the merge scratch
     __host__ __device__ static int q_slot(int G) { return (G * D * 2 + 127) & ~127; }
     __host__ __device__ static int off_q(int ns) { return kNW * ns * kTile; }
-    __host__ __device__ static int off_desc(int ns, int G) { return off_q(ns) + kQSlots * q_slot(G); }
-    __host__ __device__ static int off_scratch(int ns, int G) { return off_desc(ns, G) + kQSlots * 32; }
+    __host__ __device__ static int off_desc(int ns, int G, int nq) { return off_q(ns) + nq * q_slot(G); }
+    __host__ __device__ static int off_scratch(int ns, int G, int nq) { return off_desc(ns, G, nq) + nq * 32; }
     // merge scratch: 8 warp states of G padded rows; also reused by the tail merge (256 threads x 6 floats)
     __host__ __device__ static int scratch_bytes(int G) {
         return kNW * G * kRowF * 4 > kNW * 32 * 6 * 4 ? kNW * G * kRowF * 4 : kNW * 32 * 6 * 4;
     }
-    __host__ __device__ static int off_ml(int ns, int G) { return off_scratch(ns, G) + scratch_bytes(G); }
-    __host__ __device__ static int off_bar(int ns, int G) { return (off_ml(ns, G) + kNW * G * 8 + 15) & ~15; }
-    __host__ __device__ static int off_flag(int ns, int G) { return off_bar(ns, G) + (2 * kNW * kMaxStages + 2 * kQSlots) * 8; }
-    __host__ __device__ static int total(int ns, int G) {
-        return off_flag(ns, G) + 16 + 1024 /* base alignment slack */;
+    __host__ __device__ static int off_ml(int ns, int G, int nq) { return off_scratch(ns, G, nq) + scratch_bytes(G); }
+    __host__ __device__ static int off_bar(int ns, int G, int nq) { return (off_ml(ns, G, nq) + kNW * G * 8 + 15) & ~15; }
+    __host__ __device__ static int off_flag(int ns, int G, int nq) {
+        return off_bar(ns, G, nq) + (2 * kNW * kMaxStages + 2 * kMaxQSlots) * 8;
+    }
+    __host__ __device__ static int total(int ns, int G, int nq) {
+        return off_flag(ns, G, nq) + 16 + 1024 /* base alignment slack */;
     }
     static int max_stages(int G) {
         int ns = kMaxStages;
-        while (ns > 1 && total(ns, G) > kSmemLimit) --ns;
+        while (ns > 1 && total(ns, G, kMinQSlots) > kSmemLimit) --ns;
         return ns;
+    }
+    static int max_qslots(int ns, int G) {  // what is left after the tile rings goes to the query ring
+        int nq = kMaxQSlots;
+        while (nq > kMinQSlots && total(ns, G, nq) > kSmemLimit) --nq;
+        return nq;
     }
 };
 
@@ -402,6 +435,84 @@ tangram_merge_kernel(const int32_t* __restrict__ merge_recs, int n_small, const 
     else merge_big_unit<D, kMergeThreads, false>(mu, G, part_o, part_lse, out, lse, s_part, threadIdx.x);
 }
 
+// ------------------------------------------------------------------ NEXT-4: block-table growth on the device
+// The lengths of one decode step and the Vectorized Block Table update by ONE thread block of
+// NT threads (a power of two): thread i owns rows i, i + NT, ...  A row that needs a page and has a free slot takes
+// free_pages[cursor + (number of such rows before it)] -- a block-wide exclusive scan keeps the oracle's row order.
+template <int NT, bool NAMED_BAR>
+__device__ __forceinline__ void block_sync() {
+    if constexpr (NAMED_BAR) named_bar_sync(1, NT);
+    else __syncthreads();
+}
+
+// kv_len[seq] += 1 for every sequence whose appended row was stored (its row holds a page for token n and the plan
+// has an item covering it); the others are counted as dropped.
+template <int NT, bool NAMED_BAR>
+__device__ __forceinline__ void step_lengths(const GrowParams& g, int tid) {
+    for (int seq = tid; seq < g.R * g.H; seq += NT) {
+        const int n = g.kv_len[seq];
+        if (n < g.seq_cap[seq] && n < g.plan_cover[seq]) g.kv_len[seq] = n + 1;
+        else if (g.overflow) atomicAdd(g.overflow, 1);
+    }
+    block_sync<NT, NAMED_BAR>();
+}
+
+template <int NT, bool NAMED_BAR>
+__device__ __forceinline__ void extend_rows(const GrowParams& g, int page_tokens, int tid, int* s_scan /* >= 33 ints */) {
+    const int lane = tid & 31, wid = tid >> 5;
+    const int cursor0 = g.grow_state[0];
+    int granted = 0;  // pages asked for by the rows of earlier chunks (same value in every thread)
+    for (int row0 = 0; row0 < g.n_rows; row0 += NT) {
+        const int row = row0 + tid;
+        bool want = false, can = false;
+        int have = 0, lo = 0, r = 0, c = 0;
+        if (row < g.n_rows) {
+            r = row / g.C, c = row % g.C;
+            int longest = 0;
+            for (int k = 0; k < g.Hp; ++k) longest = max(longest, g.kv_len[r * g.H + g.perm[c * g.Hp + k]]);
+            have = g.row_pages[row], lo = g.row_ptr[row];
+            want = longest >= have * page_tokens;
+            can = want && have < g.row_ptr[row + 1] - lo;
+        }
+        // block-wide exclusive scan of `can`
+        const unsigned bal = __ballot_sync(0xffffffffu, can);
+        if (lane == 0) s_scan[wid] = __popc(bal);
+        block_sync<NT, NAMED_BAR>();
+        if (wid == 0) {
+            const int v = lane < NT / 32 ? s_scan[lane] : 0;
+            int inc = v;
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            s_scan[lane] = inc - v;                      // exclusive prefix of the warp totals
+            if (lane == 31) s_scan[32] = inc;            // chunk total
+        }
+        block_sync<NT, NAMED_BAR>();
+        const int idx = cursor0 + granted + s_scan[wid] + __popc(bal & ((1u << lane) - 1u));
+        const int total = s_scan[32];
+        const bool ok = can && idx < g.n_free;
+        if (ok) {
+            g.tbl_pages[lo + have] = g.free_pages[idx];
+            g.row_pages[row] = have + 1;
+            for (int k = 0; k < g.Hp; ++k) g.seq_cap[r * g.H + g.perm[c * g.Hp + k]] = (have + 1) * page_tokens;
+        }
+        if (want && !ok) atomicAdd(g.grow_state + 1, 1);
+        granted += total;
+        block_sync<NT, NAMED_BAR>();                     // s_scan is reused by the next chunk
+    }
+    if (tid == 0) g.grow_state[0] = min(cursor0 + granted, max(cursor0, g.n_free));
+}
+
+// Stand-alone: tangram_extend_tables_device (do_lengths = 0) and the follow-up of tangram_decode_step when the
+// decode grid cannot run its tail phase (do_lengths = 1).
+__global__ void __launch_bounds__(1024) tangram_grow_kernel(const GrowParams g, int page_tokens, int do_lengths) {
+    __shared__ int s_scan[33];
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (do_lengths) step_lengths<1024, false>(g, threadIdx.x);
+    if (g.free_pages) extend_rows<1024, false>(g, page_tokens, threadIdx.x, s_scan);
+}
+
 // ------------------------------------------------------------------ a4: split-KV decode kernel
 template <int D, bool TIMED>
 __global__ void __launch_bounds__(Smem<D>::kThreads, 1)
@@ -413,35 +524,41 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     // 128-byte-swizzled TMA tiles need a 1024-byte aligned base
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
 
-    const int NS = p.n_stages, G = p.G;
+    const int NS = p.n_stages, NQ = p.n_qslots, G = p.G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t tiles = smem_u32(smem);
     uint8_t* q_ring = smem + L::off_q(NS);
-    uint8_t* desc_ring = smem + L::off_desc(NS, G);
-    float* scratch_o = reinterpret_cast<float*>(smem + L::off_scratch(NS, G));
-    float* scratch_ml = reinterpret_cast<float*>(smem + L::off_ml(NS, G));
-    const uint32_t bars = smem_u32(smem + L::off_bar(NS, G));
+    uint8_t* desc_ring = smem + L::off_desc(NS, G, NQ);
+    float* scratch_o = reinterpret_cast<float*>(smem + L::off_scratch(NS, G, NQ));
+    float* scratch_ml = reinterpret_cast<float*>(smem + L::off_ml(NS, G, NQ));
+    const uint32_t bars = smem_u32(smem + L::off_bar(NS, G, NQ));
     const int q_slot_bytes = L::q_slot(G);
     auto full_bar = [&](int w, int s) { return bars + (w * kMaxStages + s) * 8; };
     auto empty_bar = [&](int w, int s) { return bars + (kNW * kMaxStages + w * kMaxStages + s) * 8; };
     auto qfull_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + s) * 8; };
-    auto qempty_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + kQSlots + s) * 8; };
+    auto qempty_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + kMaxQSlots + s) * 8; };
 
     if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x] = globaltimer();
+    // The CTA's own list head (plan data) is on its way while the barriers are set up: the first TMA of the CTA
+    // is then one memory round trip behind the start of the CTA, not two.
+    int head_word = 0;
+    if (warp == kNW) {
+        head_word = __ldg(reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(blockIdx.x) * 32 + lane);
+        if (lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&kv_map) : "memory");
+    }
     if (threadIdx.x == 0) {
         for (int w = 0; w < kNW; ++w)
             for (int s = 0; s < NS; ++s) {
                 mbar_init(full_bar(w, s), 1);
                 mbar_init(empty_bar(w, s), 1);
             }
-        for (int s = 0; s < kQSlots; ++s) {
+        for (int s = 0; s < NQ; ++s) {
             mbar_init(qfull_bar(s), 1);
             mbar_init(qempty_bar(s), kNW);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    asm volatile("griddepcontrol.launch_dependents;");  // lets the merge grid's launch overlap this kernel
 
     if (warp == kNW) {
         // ============================== producer warp ==============================
@@ -459,41 +576,107 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             if (lane == 0) v = atomicAdd(p.sched, 1) + static_cast<int>(gridDim.x);
             return v;
         };
+        // Open-ended plan: an item ends where its sequence ends NOW.  In a fused decode step (k_new given) the
+        // sequence gains one token in this launch if its row holds a page for it; the item that covers that
+        // token index is the sequence's TAIL item, and the CTA that runs it stores the new K / V row first.
+        auto open_end = [&](DeviceItem& it, bool& tail) {
+            tail = false;
+            if (!p.kv_len) return;
+            const int sq = it.req * p.H + it.kv_head;
+            int n = __ldcg(p.kv_len + sq);
+            if (p.k_new) {
+                const bool room = n < __ldcg(p.seq_cap + sq);
+                tail = room && it.tok_begin <= n && n < it.tok_end;
+                n += room ? 1 : 0;
+            }
+            it.tok_end = min(it.tok_end, n);
+        };
         // One 128-byte list head (a single coalesced load, lane L reads word L) carries the list's item
         // range, its first item and that item's first 16 page ids, so the first TMA of a list is two
         // dependent memory round trips away from the claim instead of four.
         int64_t cb, ce;
         DeviceItem next;
+        bool next_tail = false;
         int head_pid_lo = 0, head_pid_hi = 0;  // page ids of tiles (lane - rot) mod NW and that + NW of the list's first item
-        auto load_head = [&](int list) {
-            const int w = __ldg(reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(list) * 32 + lane);
+        auto take_head = [&](int w) {
             cb = __shfl_sync(0xffffffffu, w, 0);
             ce = cb + __shfl_sync(0xffffffffu, w, 1);
             next.req = __shfl_sync(0xffffffffu, w, 4), next.kv_head = __shfl_sync(0xffffffffu, w, 5);
             next.tbl_row = __shfl_sync(0xffffffffu, w, 6), next.slot = __shfl_sync(0xffffffffu, w, 7);
             next.tok_begin = __shfl_sync(0xffffffffu, w, 8), next.tok_end = __shfl_sync(0xffffffffu, w, 9);
             next.part_slot = __shfl_sync(0xffffffffu, w, 10), next.n_parts = __shfl_sync(0xffffffffu, w, 11);
-            if (p.kv_len) next.tok_end = min(next.tok_end, __ldg(p.kv_len + next.req * p.H + next.kv_head));
+            if (ce > cb) open_end(next, next_tail);
             const int i0 = (lane - (next.part_slot & (kNW - 1))) & (kNW - 1);
             head_pid_lo = __shfl_sync(0xffffffffu, w, 12 + i0);
             head_pid_hi = __shfl_sync(0xffffffffu, w, 12 + kNW + i0);
         };
-        load_head(blockIdx.x);
+        auto load_head = [&](int list) {
+            take_head(__ldg(reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(list) * 32 + lane));
+        };
+        take_head(head_word);
+        // Programmatic dependent launch (tangram_decode_step with TANGRAM_STEP_OVERLAP): everything up to here read
+        // plan data, lengths and tables, which the predecessor on the stream does not write.  The producer may
+        // also fill its (empty) tile rings with the first item's KV tiles -- the cache is not the predecessor's
+        // either -- and only then waits for the predecessor, before the first q / k_new / v_new access.
+        bool pdl_wait = p.pdl != 0;
+        int prefilled = 0;              // tiles of the first item already issued per lane (0 .. NS)
+        int pre_pid = 0;                // page id of the lane's next tile after the prefill
+        if (pdl_wait) {
+            if (ce > cb && !next_tail && lane < kNW) {
+                const int n_tiles = max(0, next.tok_end - next.tok_begin + kPage - 1) / kPage;
+                const int32_t* ids = p.tbl_pages + next.tbl_row + next.tok_begin / kPage;
+                int i = (lane - (next.part_slot & (kNW - 1))) & (kNW - 1);
+                int pid = head_pid_lo;
+                if (i < n_tiles && pid < 0) pid = __ldg(ids + i);
+                while (i < n_tiles && prefilled < NS) {
+                    const int i_next = i + kNW;
+                    int pid_next = i_next < 2 * kNW ? head_pid_hi : 0;
+                    if (i_next < n_tiles && (i_next >= 2 * kNW || pid_next < 0)) pid_next = __ldg(ids + i_next);
+                    mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
+                    tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
+                                  (pid * p.Hp + next.slot) * (2 * kPage), policy);
+                    if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
+                    i = i_next, pid = pid_next, ++prefilled;
+                }
+                pre_pid = pid;
+            }
+            __syncwarp();
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+        }
+        asm volatile("griddepcontrol.launch_dependents;");  // the next launch on the stream may be scheduled
         int seq = 0;  // running item number = position in the item / query ring
         for (;;) {
             int fut = 0;
             if (dynamic && cb == ce) fut = claim();
             for (int64_t it = cb; it < ce; ++it, ++seq) {
                 const DeviceItem item = next;
+                const bool tail = next_tail;
                 const bool head_item = it == cb;
                 if (it + 1 < ce) {
                     next = p.items[it + 1];
-                    // open-ended plan: the item ends where the sequence ends NOW (it may be empty)
-                    if (p.kv_len) next.tok_end = min(next.tok_end, __ldg(p.kv_len + next.req * p.H + next.kv_head));
+                    open_end(next, next_tail);
                 }
                 const bool claim_here = dynamic && it + 1 == ce;  // last item of the list: claim the next list
-                const int qs = seq % kQSlots;
-                const uint32_t qpar = (seq / kQSlots) & 1;
+                const int qs = seq % NQ;
+                const uint32_t qpar = (seq / NQ) & 1;
+                if (tail) {
+                    // fused KV append: token index tok_end - 1 is the new one.  16-byte chunks of the K row then
+                    // the V row; the proxy fence orders these generic-proxy stores before the TMA (async proxy)
+                    // reads of the same page issued below by this warp.
+                    const int n = item.tok_end - 1;
+                    const int page = __ldg(p.tbl_pages + item.tbl_row + n / kPage);
+                    const size_t row_k = ((static_cast<size_t>(page) * p.Hp + item.slot) * 2) * kPage + n % kPage;
+                    const size_t sq = static_cast<size_t>(item.req) * p.H + item.kv_head;
+                    constexpr int chunks = D / 8;
+                    for (int c = lane; c < 2 * chunks; c += 32) {
+                        const bool is_v = c >= chunks;
+                        const int cc = is_v ? c - chunks : c;
+                        const uint4 val = __ldcg((is_v ? p.v_new : p.k_new) + sq * chunks + cc);
+                        p.pool_w[(row_k + (is_v ? kPage : 0)) * chunks + cc] = val;
+                    }
+                    asm volatile("fence.proxy.async;" ::: "memory");
+                    __syncwarp();
+                }
                 if (lane == 0) {
                     mbar_wait(qempty_bar(qs), qpar ^ 1);
                     *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = item;
@@ -508,7 +691,15 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 if (lane < kNW) {
                     const int32_t* ids = p.tbl_pages + item.tbl_row + item.tok_begin / kPage;
                     int i = (lane - rot) & (kNW - 1);
-                    int pid = head_item ? head_pid_lo : (i < n_tiles ? __ldg(ids + i) : 0);
+                    int pid;
+                    if (prefilled) {  // (first item of a PDL launch: its first tiles are already in flight)
+                        i += prefilled * kNW, pid = pre_pid, prefilled = 0;
+                    } else {
+                        pid = head_item ? head_pid_lo : 0;
+                        // a list head caches the page ids its first item had at upload time; a slot that got its
+                        // page later (table growth) is read from the table
+                        if (i < n_tiles && (!head_item || pid < 0)) pid = __ldg(ids + i);
+                    }
                     // lane 0 issues the claim kClaimTiles tiles before the end of the item's TMA issue: late
                     // enough that the CTA does not hoard a list, early enough to cover the claim -> list
                     // head -> first TMA chain (~3 us) with tiles that are still being issued
@@ -519,8 +710,8 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                             to_claim = false;
                         }
                         const int i_next = i + kNW;
-                        const int pid_next =
-                            head_item && i_next < 2 * kNW ? head_pid_hi : (i_next < n_tiles ? __ldg(ids + i_next) : 0);
+                        int pid_next = head_item && i_next < 2 * kNW ? head_pid_hi : 0;
+                        if (i_next < n_tiles && (!head_item || i_next >= 2 * kNW || pid_next < 0)) pid_next = __ldg(ids + i_next);
                         mbar_wait(empty_bar(lane, stage), phase ^ 1);
                         mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
                         tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
@@ -530,6 +721,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     }
                     if (to_claim) fut = atomicAdd(p.sched, 1) + static_cast<int>(gridDim.x);
                 }
+                prefilled = 0;
                 __syncwarp();
             }
             if (!dynamic) break;
@@ -539,8 +731,8 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         }
         if (lane == 0) {
             // end-of-work sentinel for the consumers
-            const int qs = seq % kQSlots;
-            mbar_wait(qempty_bar(qs), ((seq / kQSlots) & 1) ^ 1);
+            const int qs = seq % NQ;
+            mbar_wait(qempty_bar(qs), ((seq / NQ) & 1) ^ 1);
             DeviceItem stop{};
             stop.n_parts = -1;
             *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = stop;
@@ -561,8 +753,8 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     constexpr float kNegInf = -INFINITY;
 
     for (int it = 0;; ++it) {
-        const int qs = it % kQSlots;
-        mbar_wait(qfull_bar(qs), (it / kQSlots) & 1);
+        const int qs = it % NQ;
+        mbar_wait(qfull_bar(qs), (it / NQ) & 1);
         const DeviceItem item = *reinterpret_cast<const DeviceItem*>(desc_ring + qs * 32);
         if (item.n_parts < 0) break;  // producer's end-of-work sentinel
         uint32_t qa[D / 16][2];
@@ -702,19 +894,24 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
 
     if (p.tail_merge) {
         // a5 inside the persistent grid (cooperative launch: all CTAs are co-resident).  Grid barrier over
-        // the consumer threads, then CTA b merges units b, b + gridDim.x, ... -- no second launch, and the
+        // the consumer threads, then CTA b merges units b, b + grid, ... -- no second launch, and the
         // merges of many sequences run on all SMs at once.
-        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*gridDim.x)*K + sub, no
+        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*grid)*K + sub, no
         // barrier inside; the first record is fetched BEFORE the grid barrier (plan data).  Big records
         // (more than kMergeBigParts parts) go first, one query head per unit, CTAs 0 .. n_big_units-1 ...
+        // In a fused decode step the LAST CTA of the grid does not merge: it updates the lengths and grows the
+        // block tables for the next step while the others merge (`grid` = the CTAs that merge).
+        const bool fused = p.k_new != nullptr;
+        const int grid_all = static_cast<int>(gridDim.x);
+        const int grid = fused && grid_all > 1 ? grid_all - 1 : grid_all;
+        const bool merger = static_cast<int>(blockIdx.x) < grid;
         const int n_elem = G * (D / 4), K = (kNW * 32) / n_elem, sub = threadIdx.x / n_elem;
         const int n_big_units = p.n_merge_units - p.n_merge_small;
-        const int grid = static_cast<int>(gridDim.x);
         // ... so the small records start at the CTA after the last one holding a big unit
         const int first = (static_cast<int>(blockIdx.x) - n_big_units % grid + grid) % grid;
         int sidx = first * K + sub;
         int4 rec = make_int4(0, 0, 0, 0);
-        if (sub < K && sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
+        if (merger && sub < K && sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
         __threadfence();
         named_bar_sync(1, kNW * 32);
         if (threadIdx.x == 0) {
@@ -722,41 +919,50 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             int seen;
             do {
                 asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
-                if (seen < grid) __nanosleep(32);
-            } while (seen < grid);
+                if (seen < grid_all) __nanosleep(32);
+            } while (seen < grid_all);
             __threadfence();
         }
         named_bar_sync(1, kNW * 32);
         if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
         float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
-        for (int u = blockIdx.x; u < n_big_units; u += grid)
-            merge_big_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4),
-                                              G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
-        if (sub < K)
-            for (; sidx < p.n_merge_small; sidx += grid * K) {
-                merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
-                if (sidx + grid * K < p.n_merge_small)
-                    rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
-            }
+        if (merger) {
+            for (int u = blockIdx.x; u < n_big_units; u += grid)
+                merge_big_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4),
+                                                  G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
+            if (sub < K)
+                for (; sidx < p.n_merge_small; sidx += grid * K) {
+                    merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
+                    if (sidx + grid * K < p.n_merge_small)
+                        rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
+                }
+        }
+        if (fused && (!merger || grid_all == 1)) {
+            // every append of this step happened before the barrier: lengths, then the pages of the next step
+            named_bar_sync(1, kNW * 32);
+            step_lengths<kNW * 32, true>(p.grow, threadIdx.x);
+            if (p.grow.free_pages) extend_rows<kNW * 32, true>(p.grow, kPage, threadIdx.x, reinterpret_cast<int*>(scratch_o));
+        }
         if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
-        if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == static_cast<int>(gridDim.x) - 1)
+        if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == grid_all - 1)
             p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
     }
 }
 
 // ------------------------------------------------------------------ NEXT-1: KV append
 // One warp per (request, KV head): the new K row and V row (d bf16 each) go to token index
-// n = kv_len[r][h] of the head's ragged pages; kv_len becomes n + 1.  A head whose table is full keeps its
-// length (the reserved budget is a hard capacity bound) and the row is counted in *overflow.
+// n = kv_len[r][h] of the head's ragged pages; kv_len becomes n + 1.  A head whose row holds no page for
+// token n (seq_cap = row_pages x P tokens are full) keeps its length and the row is counted in *overflow.
 __global__ void __launch_bounds__(128)
-tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ tbl_pages,
+tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ seq_cap,
+                      const int32_t* __restrict__ tbl_pages,
                       const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, uint4* __restrict__ pool,
                       int32_t* __restrict__ kv_len, int32_t* __restrict__ overflow, int n_seq, int Hp, int d) {
     const int seq = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (seq >= n_seq) return;
-    const int4 si = seq_info[seq];  // {table row offset, capacity tokens, slot, -}
+    const int4 si = seq_info[seq];  // {first slot of the row, slot capacity in tokens, slot, row}
     const int n = kv_len[seq];
-    if (n >= si.y) {
+    if (n >= seq_cap[seq]) {
         if (lane == 0 && overflow) atomicAdd(overflow, 1);
         return;
     }
@@ -827,9 +1033,8 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
 
 // CTAs of the decode kernel that can be co-resident on the current device (SMs x occupancy).
 template <int D, bool TIMED>
-static int max_coresident(int smem) {
-    int dev = 0, sms = 0, per_sm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+static int max_coresident(int dev, int smem) {
+    int sms = 0, per_sm = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED>, Smem<D>::kThreads, smem) !=
         cudaSuccess)
@@ -841,22 +1046,34 @@ template <int D, bool TIMED>
 static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map, cudaStream_t stream,
                         bool want_tail_merge, bool* merged) {
     using L = Smem<D>;
-    const int smem = L::total(prm.n_stages, prm.G);
+    const int smem = L::total(prm.n_stages, prm.G, prm.n_qslots);
     cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, TIMED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
-    // The tail merge needs a grid barrier, i.e. a cooperative launch with every CTA resident.
-    static thread_local int cached_smem = -1, cached_max = 0;
-    if (want_tail_merge && D <= 128 && cached_smem != smem) cached_max = max_coresident<D, TIMED>(smem), cached_smem = smem;
+    // The tail merge needs a grid barrier, i.e. a cooperative launch with every CTA resident.  The answer is
+    // cached per (device, shared-memory size).
+    static thread_local int cached_dev = -1, cached_smem = -1, cached_max = 0;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (want_tail_merge && D <= 128 && (cached_smem != smem || cached_dev != dev))
+        cached_max = max_coresident<D, TIMED>(dev, smem), cached_smem = smem, cached_dev = dev;
     // (at d = 256 the grid has 128 consumer threads per CTA, fewer than a merge record has elements: stand-alone kernel)
     prm.tail_merge = want_tail_merge && D <= 128 && dp->n_static <= cached_max;
     *merged = prm.tail_merge;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(Smem<D>::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
-    cfg.attrs = attr, cfg.numAttrs = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
     e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+    if (e != cudaSuccess && prm.pdl) {
+        // the two attributes together are refused: launch without the overlap (the kernel then must not wait)
+        (void)cudaGetLastError();
+        prm.pdl = 0, cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+    }
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
     return TANGRAM_OK;
 }
@@ -883,27 +1100,36 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
     }
     const int n_units = n_small + (int)dp->n_big_merge_seqs * prm.G * S;
     prm.merge_recs = dp->merge_seqs, prm.n_merge_small = n_small, prm.n_merge_units = n_units, prm.merge_split = S;
+    const bool fused = prm.k_new != nullptr;
     bool merged = false;
     if (which & kRunSplit) {
-        const bool want = (which & kRunMerge) && n_units > 0;
+        // a fused step always wants the tail phase (lengths + table growth), even with nothing to merge
+        const bool want = (which & kRunMerge) && (n_units > 0 || fused);
         const int rc = prm.worker_ns ? launch_split<D, true>(dp, prm, map, stream, want, &merged)
                                      : launch_split<D, false>(dp, prm, map, stream, want, &merged);
         if (rc != TANGRAM_OK) return rc;
     }
-    if (!(which & kRunMerge) || merged || n_units == 0) return TANGRAM_OK;
-    // Stand-alone merge kernel by programmatic dependent launch: its grid is scheduled while the decode
-    // grid drains and blocks in griddepcontrol.wait until that grid has completed and flushed its writes.
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)n_units), cfg.blockDim = dim3(kMergeThreads), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr, cfg.numAttrs = 1;
-    const float* po = prm.part_o;
-    const float* pl = prm.part_lse;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, n_small, po, pl, prm.out, prm.lse,
-                                       (int)prm.G, S);
-    if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
+    if (!(which & kRunMerge) || merged) return TANGRAM_OK;
+    if (n_units > 0) {
+        // Stand-alone merge kernel by programmatic dependent launch: its grid is scheduled while the decode
+        // grid drains and blocks in griddepcontrol.wait until that grid has completed and flushed its writes.
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)n_units), cfg.blockDim = dim3(kMergeThreads), cfg.dynamicSmemBytes = 0, cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr, cfg.numAttrs = 1;
+        const float* po = prm.part_o;
+        const float* pl = prm.part_lse;
+        cudaError_t e = cudaLaunchKernelEx(&cfg, tangram_merge_kernel<D>, dp->merge_seqs, n_small, po, pl, prm.out, prm.lse,
+                                           (int)prm.G, S);
+        if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
+    }
+    if (fused) {  // lengths + table growth of a fused step whose grid could not run its tail phase
+        tangram_grow_kernel<<<1, 1024, 0, stream>>>(prm.grow, kPage, 1);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "grow kernel launch");
+    }
     return TANGRAM_OK;
 }
 
@@ -911,7 +1137,8 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 template <int D>
 static cudaError_t occupancy_of(int gqa, int* per_sm) {
-    const int smem = Smem<D>::total(Smem<D>::max_stages(gqa), gqa);
+    const int ns = Smem<D>::max_stages(gqa);
+    const int smem = Smem<D>::total(ns, gqa, Smem<D>::max_qslots(ns, gqa));
     cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false>, Smem<D>::kThreads, smem);
@@ -935,56 +1162,84 @@ extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa,
     return TANGRAM_OK;
 }
 
+// Blob layout (all sections 256-byte aligned), shared by tangram_blob_bytes and tangram_upload.
+namespace {
+struct BlobLayout {
+    size_t items, windptr, pindptr, pages, mseq, heads, seqinfo, row_ptr, row_pages, perm, seq_cap, cover, grow, sched, total;
+};
+int64_t table_slots(const tangram_tables* t) {
+    return t->tbl_indptr ? t->tbl_indptr[(int64_t)t->R * t->C] : t->n_pages_used;
+}
+BlobLayout blob_layout(const tangram_tables* t, const tangram_plan* p) {
+    BlobLayout b{};
+    const size_t n_seq = (size_t)t->R * t->H, n_rows = (size_t)t->R * t->C;
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t at = off;
+        off += align_up(bytes, 256);
+        return at;
+    };
+    b.items = take(sizeof(DeviceItem) * (size_t)p->n_items);
+    b.windptr = take(sizeof(int64_t) * ((size_t)p->W + 1));
+    b.pindptr = take(sizeof(int64_t) * (n_seq + 1));
+    b.pages = take(sizeof(int32_t) * (size_t)table_slots(t));
+    b.mseq = take(4 * sizeof(int32_t) * n_seq);  // merge records (upper bound)
+    b.heads = take(128 * (size_t)p->W);          // list heads
+    b.seqinfo = take(16 * n_seq);                // per-sequence table info (KV append, compaction)
+    b.row_ptr = take(sizeof(int32_t) * (n_rows + 1));
+    b.row_pages = take(sizeof(int32_t) * n_rows);
+    b.perm = take(sizeof(int32_t) * (size_t)t->H);
+    b.seq_cap = take(sizeof(int32_t) * n_seq);
+    b.cover = take(sizeof(int32_t) * n_seq);
+    b.grow = take(16);
+    b.sched = take(16);
+    b.total = off + 256;
+    return b;
+}
+}  // namespace
+
 extern "C" size_t tangram_blob_bytes(const tangram_tables* t, const tangram_plan* p) {
     if (!t || !p) return 0;
-    size_t b = 0;
-    b += align_up(sizeof(DeviceItem) * (size_t)p->n_items, 256);
-    b += align_up(sizeof(int64_t) * ((size_t)p->W + 1), 256);
-    b += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
-    b += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
-    b += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);  // merge records (upper bound)
-    b += align_up(128 * (size_t)p->W, 256);                          // list heads
-    b += align_up(16 * (size_t)t->R * t->H, 256);                    // per-sequence table info (KV append)
-    return b + 256 /* scheduler counters */ + 256;
+    return blob_layout(t, p).total;
 }
 
 extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
                               void* stream, tangram_device_plan* dp) {
     if (!t || !p || !dev_blob || !dp || !p->items || !p->worker_indptr || !p->part_indptr || !t->tbl_pages ||
-        !t->tbl_indptr || !t->cluster_of || !t->slot_of)
+        !t->tbl_indptr || !t->cluster_of || !t->slot_of || !t->perm)
         return fail(TANGRAM_ERR_INVALID_ARG, "upload: NULL argument");
     if (p->n_items > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: more than 2^31 items");
-    const size_t need = tangram_blob_bytes(t, p);
+    const BlobLayout lay = blob_layout(t, p);
+    const size_t need = lay.total;
     if (bytes < need) return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "upload: blob %zu < %zu bytes", bytes, need);
     if (reinterpret_cast<uintptr_t>(dev_blob) % 256 != 0)
         return fail(TANGRAM_ERR_INVALID_ARG, "upload: dev_blob must be 256-byte aligned");
+    const int64_t n_seq = (int64_t)t->R * t->H, n_rows = (int64_t)t->R * t->C, n_slots = table_slots(t);
+    if (n_slots > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: page table larger than 2^31 entries");
     std::vector<uint8_t> host(need, 0);
-    size_t off = 0;
-    const size_t off_items = off;
-    DeviceItem* di = reinterpret_cast<DeviceItem*>(host.data() + off);
+    DeviceItem* di = reinterpret_cast<DeviceItem*>(host.data() + lay.items);
+    int32_t* cover = reinterpret_cast<int32_t*>(host.data() + lay.cover);
     for (int64_t i = 0; i < p->n_items; ++i) {
         const tangram_item& s = p->items[i];
         const int64_t row_off = t->tbl_indptr[(int64_t)s.req * t->C + s.cluster];
-        if (row_off > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: page table larger than 2^31 entries");
         di[i] = DeviceItem{s.req, s.kv_head, (int32_t)row_off, s.slot, s.tok_begin, s.tok_end, s.part_slot, s.n_parts};
+        int32_t& cv = cover[(int64_t)s.req * t->H + s.kv_head];
+        cv = std::max(cv, s.tok_end);
     }
-    off += align_up(sizeof(DeviceItem) * (size_t)p->n_items, 256);
-    const size_t off_windptr = off;
-    std::memcpy(host.data() + off, p->worker_indptr, sizeof(int64_t) * ((size_t)p->W + 1));
-    off += align_up(sizeof(int64_t) * ((size_t)p->W + 1), 256);
-    const size_t off_pindptr = off;
-    std::memcpy(host.data() + off, p->part_indptr, sizeof(int64_t) * ((size_t)t->R * t->H + 1));
-    off += align_up(sizeof(int64_t) * ((size_t)t->R * t->H + 1), 256);
-    const size_t off_pages = off;
-    std::memcpy(host.data() + off, t->tbl_pages, sizeof(int32_t) * (size_t)t->n_pages_used);
+    std::memcpy(host.data() + lay.windptr, p->worker_indptr, sizeof(int64_t) * ((size_t)p->W + 1));
+    std::memcpy(host.data() + lay.pindptr, p->part_indptr, sizeof(int64_t) * ((size_t)n_seq + 1));
+    std::memcpy(host.data() + lay.pages, t->tbl_pages, sizeof(int32_t) * (size_t)n_slots);
     int64_t max_page = -1;
-    for (int64_t i = 0; i < t->n_pages_used; ++i) {
-        if (t->tbl_pages[i] < 0) return fail(TANGRAM_ERR_INVALID_ARG, "upload: negative page id in the tables");
-        max_page = std::max<int64_t>(max_page, t->tbl_pages[i]);
+    for (int64_t row = 0; row < n_rows; ++row) {
+        const int64_t lo = t->tbl_indptr[row], hi = t->tbl_indptr[row + 1];
+        const int64_t have = t->row_pages ? t->row_pages[row] : hi - lo;
+        if (have < 0 || have > hi - lo) return fail(TANGRAM_ERR_INVALID_ARG, "upload: row_pages[%lld] out of range", (long long)row);
+        for (int64_t i = lo; i < lo + have; ++i) {
+            if (t->tbl_pages[i] < 0) return fail(TANGRAM_ERR_INVALID_ARG, "upload: negative page id in the tables");
+            max_page = std::max<int64_t>(max_page, t->tbl_pages[i]);
+        }
     }
-    off += align_up(sizeof(int32_t) * (size_t)t->n_pages_used, 256);
-    const size_t off_mseq = off;
-    int32_t* mseq = reinterpret_cast<int32_t*>(host.data() + off);
+    int32_t* mseq = reinterpret_cast<int32_t*>(host.data() + lay.mseq);
     int64_t n_mseq = 0;
     int64_t n_empty = 0;
     auto push = [&](int64_t sq) {  // record = {sequence, first part slot, parts, 0}
@@ -992,24 +1247,23 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
         rec[0] = (int32_t)sq, rec[1] = (int32_t)p->part_indptr[sq];
         rec[2] = (int32_t)(p->part_indptr[sq + 1] - p->part_indptr[sq]), rec[3] = 0;
     };
-    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // empty sequences first ...
+    for (int64_t sq = 0; sq < n_seq; ++sq)  // empty sequences first ...
         if (p->part_indptr[sq + 1] - p->part_indptr[sq] == 0) push(sq);
     n_empty = n_mseq;
-    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq) {  // ... then the small multi-part ones
+    for (int64_t sq = 0; sq < n_seq; ++sq) {  // ... then the small multi-part ones
         const int64_t np = p->part_indptr[sq + 1] - p->part_indptr[sq];
         if (np > 1 && np <= kMergeBigParts) push(sq);
     }
     const int64_t n_not_big = n_mseq;
-    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)  // ... then the big ones (one merge unit per query head)
+    for (int64_t sq = 0; sq < n_seq; ++sq)  // ... then the big ones (one merge unit per query head)
         if (p->part_indptr[sq + 1] - p->part_indptr[sq] > kMergeBigParts) push(sq);
-    off += align_up(4 * sizeof(int32_t) * (size_t)t->R * t->H, 256);
-    const size_t off_heads = off;
     int32_t n_dev_lists = 0;
     {   // list head = {item_begin, n_items, 0, 0, first item (8 words), its first 16 page ids, 0 x 4}.
         // The first n_static lists belong to the CTAs and are kept as they are; of the dynamic-tail lists only
         // the non-empty ones are uploaded (in plan order): claiming an empty list costs a CTA an atomic and a
-        // dependent load for nothing, which is most of the tail on a small batch.
-        int32_t* heads = reinterpret_cast<int32_t*>(host.data() + off);
+        // dependent load for nothing, which is most of the tail on a small batch.  A slot without a page yet
+        // (-1, growth headroom) stays -1 here and is read from the table at run time.
+        int32_t* heads = reinterpret_cast<int32_t*>(host.data() + lay.heads);
         for (int32_t k = 0; k < p->W; ++k) {
             const int64_t ib = p->worker_indptr[k], ie = p->worker_indptr[k + 1];
             if (k >= p->n_static && ie == ib) continue;
@@ -1024,20 +1278,29 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
             }
         }
     }
-    off += align_up(128 * (size_t)p->W, 256);
-    const size_t off_seqinfo = off;
-    {   // {page-table row offset, capacity in tokens, slot, 0} of every (request, KV head)
-        int32_t* si = reinterpret_cast<int32_t*>(host.data() + off);
+    {   // {first slot of the row, slot capacity in tokens, slot, row} and the tokens the row's pages hold
+        int32_t* si = reinterpret_cast<int32_t*>(host.data() + lay.seqinfo);
+        int32_t* cap = reinterpret_cast<int32_t*>(host.data() + lay.seq_cap);
         for (int32_t r = 0; r < t->R; ++r)
             for (int32_t h = 0; h < t->H; ++h, si += 4) {
                 const int64_t row = (int64_t)r * t->C + t->cluster_of[h];
+                const int64_t slots = t->tbl_indptr[row + 1] - t->tbl_indptr[row];
                 si[0] = (int32_t)t->tbl_indptr[row];
-                si[1] = (int32_t)((t->tbl_indptr[row + 1] - t->tbl_indptr[row]) * t->P);
-                si[2] = t->slot_of[h], si[3] = 0;
+                si[1] = (int32_t)(slots * t->P);
+                si[2] = t->slot_of[h], si[3] = (int32_t)row;
+                cap[(int64_t)r * t->H + h] = (int32_t)((t->row_pages ? t->row_pages[row] : slots) * t->P);
             }
     }
-    off += align_up(16 * (size_t)t->R * t->H, 256);
-    const size_t off_sched = off;
+    {
+        int32_t* rp = reinterpret_cast<int32_t*>(host.data() + lay.row_ptr);
+        int32_t* rg = reinterpret_cast<int32_t*>(host.data() + lay.row_pages);
+        for (int64_t row = 0; row <= n_rows; ++row) rp[row] = (int32_t)t->tbl_indptr[row];
+        for (int64_t row = 0; row < n_rows; ++row)
+            rg[row] = t->row_pages ? t->row_pages[row] : (int32_t)(t->tbl_indptr[row + 1] - t->tbl_indptr[row]);
+        std::memcpy(host.data() + lay.perm, t->perm, sizeof(int32_t) * (size_t)t->H);
+        int32_t* gs = reinterpret_cast<int32_t*>(host.data() + lay.grow);
+        gs[0] = (int32_t)t->n_pages_used;  // the free list's cursor
+    }
     // pageable source: the runtime stages it before returning, so `host` may die at scope exit
     cudaError_t e = cudaMemcpyAsync(dev_blob, host.data(), need, cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "upload: cudaMemcpyAsync");
@@ -1047,21 +1310,35 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->R = t->R, dp->H = t->H, dp->C = t->C, dp->Hp = t->Hp, dp->P = t->P, dp->W = n_dev_lists, dp->mode = p->mode;
     dp->n_static = p->n_static;
     dp->min_pool_pages = max_page + 1;
-    dp->sched = reinterpret_cast<int32_t*>(base + off_sched);
-    dp->merge_seqs = reinterpret_cast<const int32_t*>(base + off_mseq);
+    dp->sched = reinterpret_cast<int32_t*>(base + lay.sched);
+    dp->merge_seqs = reinterpret_cast<const int32_t*>(base + lay.mseq);
     dp->n_merge_seqs = n_mseq;
     dp->n_empty_seqs = n_empty;
-    dp->list_heads = base + off_heads;
-    dp->seq_info = reinterpret_cast<const int32_t*>(base + off_seqinfo);
+    dp->list_heads = base + lay.heads;
+    dp->seq_info = reinterpret_cast<const int32_t*>(base + lay.seqinfo);
     dp->n_big_merge_seqs = n_mseq - n_not_big;
     dp->max_merge_parts = 0;
-    for (int64_t sq = 0; sq < (int64_t)t->R * t->H; ++sq)
+    for (int64_t sq = 0; sq < n_seq; ++sq)
         dp->max_merge_parts = std::max<int64_t>(dp->max_merge_parts, p->part_indptr[sq + 1] - p->part_indptr[sq]);
     dp->n_items = p->n_items, dp->n_part_slots = p->n_part_slots;
-    dp->items = base + off_items;
-    dp->worker_indptr = reinterpret_cast<const int64_t*>(base + off_windptr);
-    dp->part_indptr = reinterpret_cast<const int64_t*>(base + off_pindptr);
-    dp->tbl_pages = reinterpret_cast<const int32_t*>(base + off_pages);
+    dp->items = base + lay.items;
+    dp->worker_indptr = reinterpret_cast<const int64_t*>(base + lay.windptr);
+    dp->part_indptr = reinterpret_cast<const int64_t*>(base + lay.pindptr);
+    dp->tbl_pages = reinterpret_cast<const int32_t*>(base + lay.pages);
+    dp->n_slots = n_slots;
+    dp->row_ptr = reinterpret_cast<const int32_t*>(base + lay.row_ptr);
+    dp->row_pages = reinterpret_cast<int32_t*>(base + lay.row_pages);
+    dp->perm = reinterpret_cast<const int32_t*>(base + lay.perm);
+    dp->seq_cap = reinterpret_cast<int32_t*>(base + lay.seq_cap);
+    dp->plan_cover = reinterpret_cast<const int32_t*>(base + lay.cover);
+    dp->grow_state = reinterpret_cast<int32_t*>(base + lay.grow);
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_reset_plan(const tangram_device_plan* dp, void* stream) {
+    if (!dp || !dp->sched) return fail(TANGRAM_ERR_INVALID_ARG, "reset_plan: NULL argument");
+    const cudaError_t e = cudaMemsetAsync(dp->sched, 0, 16, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e, "reset_plan: cudaMemsetAsync");
     return TANGRAM_OK;
 }
 
@@ -1070,21 +1347,46 @@ extern "C" size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int
     return align_up((size_t)n_part_slots * gqa * head_dim * 4, 256) + align_up((size_t)n_part_slots * gqa * 4, 256) + 256;
 }
 
+static GrowParams grow_params(const tangram_device_plan* dp, int32_t* kv_len_dev, const int32_t* free_pages_dev,
+                              int64_t n_free, int32_t* overflow_dev) {
+    GrowParams g{};
+    g.row_ptr = dp->row_ptr, g.row_pages = dp->row_pages, g.perm = dp->perm;
+    g.tbl_pages = const_cast<int32_t*>(dp->tbl_pages), g.seq_cap = dp->seq_cap, g.plan_cover = dp->plan_cover;
+    g.kv_len = kv_len_dev, g.grow_state = dp->grow_state, g.free_pages = free_pages_dev, g.overflow = overflow_dev;
+    g.n_free = (int32_t)std::min<int64_t>(n_free, INT32_MAX), g.n_rows = dp->R * dp->C;
+    g.R = dp->R, g.H = dp->H, g.C = dp->C, g.Hp = dp->Hp;
+    return g;
+}
+
+// Arguments of a fused decode step beyond those of plain attention (all null / 0 for tangram_decode_attention).
+struct StepArgs {
+    const void* k_new = nullptr;
+    const void* v_new = nullptr;
+    int32_t* kv_len_w = nullptr;
+    const int32_t* free_pages = nullptr;
+    int64_t n_free = 0;
+    int32_t* overflow = nullptr;
+    uint32_t flags = 0;
+};
+
 static int run_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool, int64_t n_pool_pages,
                          const int32_t* kv_len_dev, int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
-                         size_t workspace_bytes, uint64_t* worker_ns, void* stream, int which) {
-    if (!dp || !q || !kv_pool || !out || !lse) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
+                         size_t workspace_bytes, uint64_t* worker_ns, void* stream, int which, const StepArgs& step = StepArgs()) {
+    const bool split = (which & kRunSplit) != 0;
+    if (!dp || !out || !lse || (split && (!q || !kv_pool))) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d (kernels need 16)", dp->P);
     if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > kMaxG)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d)", Hq,
                     dp->H, kMaxG);
-    if (n_pool_pages < 1 || dp->W < 1 || dp->n_static < 1 || dp->n_static > dp->W) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool or plan");
-    if ((which & kRunSplit) && n_pool_pages < dp->min_pool_pages)
+    if (dp->W < 1 || dp->n_static < 1 || dp->n_static > dp->W) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty plan");
+    if (split && n_pool_pages < 1) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool");
+    if (split && n_pool_pages < dp->min_pool_pages)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: kv_pool has %lld pages, the tables use page id %lld",
                     (long long)n_pool_pages, (long long)dp->min_pool_pages - 1);
-    if (reinterpret_cast<uintptr_t>(q) % 16 || reinterpret_cast<uintptr_t>(kv_pool) % 128 ||
+    // q and kv_pool are read by the split kernel only: the merge-only entry point checks out / workspace alone
+    if ((split && (reinterpret_cast<uintptr_t>(q) % 16 || reinterpret_cast<uintptr_t>(kv_pool) % 128)) ||
         reinterpret_cast<uintptr_t>(out) % 16 || reinterpret_cast<uintptr_t>(workspace) % 16)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: misaligned pointer");
     const int G = Hq / dp->H;
@@ -1094,12 +1396,12 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
 
     CUtensorMap map;
     std::memset(&map, 0, sizeof map);
-    if (which & kRunSplit) {
+    if (split) {
         const int rc = make_kv_map(&map, kv_pool, n_pool_pages, dp->Hp, d);
         if (rc != TANGRAM_OK) return rc;
     }
 
-    DecodeParams prm;
+    DecodeParams prm{};
     prm.items = static_cast<const DeviceItem*>(dp->items);
     prm.worker_indptr = dp->worker_indptr;
     prm.tbl_pages = dp->tbl_pages;
@@ -1116,8 +1418,17 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.list_heads = dp->list_heads;
     prm.sched = dp->sched;
     prm.kv_len = kv_len_dev, prm.H = dp->H;
+    if (step.k_new) {
+        prm.k_new = static_cast<const uint4*>(step.k_new), prm.v_new = static_cast<const uint4*>(step.v_new);
+        prm.pool_w = static_cast<uint4*>(const_cast<void*>(kv_pool));
+        prm.seq_cap = dp->seq_cap, prm.kv_len_w = step.kv_len_w;
+        prm.grow = grow_params(dp, step.kv_len_w, step.free_pages, step.n_free, step.overflow);
+        prm.pdl = (step.flags & TANGRAM_STEP_OVERLAP) ? 1 : 0;
+    }
 
-    prm.n_stages = d == 256 ? Smem<256>::max_stages(G) : (d == 128 ? Smem<128>::max_stages(G) : Smem<64>::max_stages(G));
+    if (d == 256) prm.n_stages = Smem<256>::max_stages(G), prm.n_qslots = Smem<256>::max_qslots(prm.n_stages, G);
+    else if (d == 128) prm.n_stages = Smem<128>::max_stages(G), prm.n_qslots = Smem<128>::max_qslots(prm.n_stages, G);
+    else prm.n_stages = Smem<64>::max_stages(G), prm.n_qslots = Smem<64>::max_qslots(prm.n_stages, G);
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
     prm.scale_log2 = scale * 1.4426950408889634f;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -1143,9 +1454,78 @@ extern "C" int tangram_decode_partials(const tangram_device_plan* dp, const void
 
 extern "C" int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d, void* out, float* lse,
                                       void* workspace, size_t workspace_bytes, void* stream) {
-    // q / kv_pool are not read by the merge kernel; pass aligned dummies through the shared validation
-    return run_attention(dp, out, out, 1, nullptr, Hq, d, 0.f, out, lse, workspace, workspace_bytes, nullptr, stream,
+    return run_attention(dp, nullptr, nullptr, 0, nullptr, Hq, d, 0.f, out, lse, workspace, workspace_bytes, nullptr, stream,
                          kRunMerge);
+}
+
+extern "C" int tangram_decode_step(const tangram_device_plan* dp, const void* q, const void* k_new, const void* v_new,
+                                   void* kv_pool, int64_t n_pool_pages, int32_t* kv_len_dev, const int32_t* free_pages_dev,
+                                   int64_t n_free, int32_t Hq, int32_t d, float sm_scale, void* out, float* lse,
+                                   void* workspace, size_t workspace_bytes, int32_t* overflow_dev, uint32_t flags,
+                                   uint64_t* worker_ns, void* stream) {
+    if (!k_new || !v_new || !kv_len_dev) return fail(TANGRAM_ERR_INVALID_ARG, "decode_step: NULL argument");
+    if (reinterpret_cast<uintptr_t>(k_new) % 16 || reinterpret_cast<uintptr_t>(v_new) % 16)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_step: misaligned pointer");
+    if (n_free < 0 || (flags & ~TANGRAM_STEP_OVERLAP)) return fail(TANGRAM_ERR_INVALID_ARG, "decode_step: bad n_free / flags");
+    StepArgs step;
+    step.k_new = k_new, step.v_new = v_new, step.kv_len_w = kv_len_dev, step.free_pages = free_pages_dev;
+    step.n_free = n_free, step.overflow = overflow_dev, step.flags = flags;
+    return run_attention(dp, q, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, workspace, workspace_bytes,
+                         worker_ns, stream, kRunSplit | kRunMerge, step);
+}
+
+extern "C" int tangram_extend_tables_device(const tangram_device_plan* dp, const int32_t* kv_len_dev,
+                                            const int32_t* free_pages_dev, int64_t n_free, void* stream) {
+    if (!dp || !kv_len_dev || !free_pages_dev || n_free < 0)
+        return fail(TANGRAM_ERR_INVALID_ARG, "extend_tables_device: NULL argument");
+    const GrowParams g = grow_params(dp, const_cast<int32_t*>(kv_len_dev), free_pages_dev, n_free, nullptr);
+    tangram_grow_kernel<<<1, 1024, 0, static_cast<cudaStream_t>(stream)>>>(g, dp->P, 0);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "grow kernel launch");
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_sync_tables(const tangram_tables* t, const tangram_device_plan* dp, void* stream) {
+    if (!t || !dp || !t->tbl_pages || !t->tbl_indptr || !t->cluster_of)
+        return fail(TANGRAM_ERR_INVALID_ARG, "sync_tables: NULL argument");
+    const int64_t n_rows = (int64_t)t->R * t->C, n_seq = (int64_t)t->R * t->H;
+    if (t->R != dp->R || t->H != dp->H || t->C != dp->C || t->P != dp->P || table_slots(t) != dp->n_slots)
+        return fail(TANGRAM_ERR_INVALID_ARG, "sync_tables: the tables do not have the shape of the uploaded ones");
+    std::vector<int32_t> rows((size_t)n_rows), cap((size_t)n_seq);
+    for (int64_t row = 0; row < n_rows; ++row) {
+        rows[(size_t)row] = t->row_pages ? t->row_pages[row] : (int32_t)(t->tbl_indptr[row + 1] - t->tbl_indptr[row]);
+    }
+    for (int32_t r = 0; r < t->R; ++r)
+        for (int32_t h = 0; h < t->H; ++h)
+            cap[(size_t)r * t->H + h] = rows[(size_t)r * t->C + t->cluster_of[h]] * t->P;
+    const int32_t gs[4] = {(int32_t)t->n_pages_used, 0, 0, 0};
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemcpyAsync(const_cast<int32_t*>(dp->tbl_pages), t->tbl_pages, sizeof(int32_t) * (size_t)dp->n_slots,
+                                    cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dp->row_pages, rows.data(), sizeof(int32_t) * rows.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dp->seq_cap, cap.data(), sizeof(int32_t) * cap.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dp->grow_state, gs, 4, cudaMemcpyHostToDevice, st);  // cursor only
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // the sources are host temporaries
+    if (e != cudaSuccess) return cuda_fail(e, "sync_tables");
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_download_tables(const tangram_device_plan* dp, tangram_tables* t, int64_t* n_starved_out, void* stream) {
+    if (!t || !dp || !t->tbl_pages || !t->row_pages)
+        return fail(TANGRAM_ERR_INVALID_ARG, "download_tables: NULL argument (row_pages is required)");
+    if (t->R != dp->R || t->C != dp->C || t->tbl_pages_cap < dp->n_slots)
+        return fail(TANGRAM_ERR_INVALID_ARG, "download_tables: the host tables are smaller than the uploaded ones");
+    int32_t gs[4] = {0, 0, 0, 0};
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemcpyAsync(t->tbl_pages, dp->tbl_pages, sizeof(int32_t) * (size_t)dp->n_slots, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(t->row_pages, dp->row_pages, sizeof(int32_t) * (size_t)dp->R * dp->C, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(gs, dp->grow_state, sizeof gs, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e, "download_tables");
+    t->n_pages_used = gs[0];
+    if (n_starved_out) *n_starved_out = gs[1];
+    return TANGRAM_OK;
 }
 
 extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const void* v_new, void* kv_pool,
@@ -1164,7 +1544,7 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: misaligned pointer");
     const int n_seq = dp->R * dp->H;
     tangram_append_kernel<<<(n_seq + 3) / 4, 128, 0, static_cast<cudaStream_t>(stream)>>>(
-        reinterpret_cast<const int4*>(dp->seq_info), dp->tbl_pages, static_cast<const uint4*>(k_new),
+        reinterpret_cast<const int4*>(dp->seq_info), dp->seq_cap, dp->tbl_pages, static_cast<const uint4*>(k_new),
         static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");

@@ -9,6 +9,12 @@
 #include <cstring>
 #include <numeric>
 #include <vector>
+#if defined(__x86_64__) && defined(__GNUC__)
+#include <immintrin.h>
+#endif
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 #include "tangram.h"
 #include "tangram_internal.h"
@@ -101,6 +107,9 @@ extern "C" int tangram_build_ragged_tables(const double* B, const int32_t* reser
     if (n_free < 0 || (n_free > 0 && !free_pages))
         return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: bad free list");
     const int32_t C = n_clusters, Hp = H / C;
+    const int32_t headroom = out->headroom_pages;
+    if (headroom < 0 || headroom > (1 << 20))
+        return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: headroom_pages=%d", headroom);
 
     // Budget-Aware Clustering (:227-233): stable ascending sort on B only.
     std::vector<int32_t> order(H);
@@ -123,32 +132,131 @@ extern "C" int tangram_build_ragged_tables(const double* B, const int32_t* reser
         }
     out->R = R, out->H = H, out->C = C, out->Hp = Hp, out->P = page_size;
     out->n_pages_used = need;
+    const int64_t n_slots = need + (int64_t)R * C * headroom;
+    out->n_slots = n_slots;
     if (need > n_free)
         return fail(TANGRAM_ERR_OUT_OF_PAGES, "build_ragged_tables: need %lld pages, free list has %lld",
                     (long long)need, (long long)n_free);
     if (!out->tbl_pages) return TANGRAM_OK;  // query
     if (!out->perm || !out->cluster_of || !out->slot_of || !out->tbl_indptr)
         return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: NULL output array");
-    if (out->tbl_pages_cap < need)
+    if (headroom > 0 && !out->row_pages)
+        return fail(TANGRAM_ERR_INVALID_ARG, "build_ragged_tables: headroom_pages > 0 needs the row_pages array");
+    if (out->tbl_pages_cap < n_slots)
         return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "build_ragged_tables: tbl_pages_cap %lld < %lld",
-                    (long long)out->tbl_pages_cap, (long long)need);
+                    (long long)out->tbl_pages_cap, (long long)n_slots);
     for (int32_t j = 0; j < H; ++j) {
         out->perm[j] = order[j];
         out->cluster_of[order[j]] = j / Hp;
         out->slot_of[order[j]] = j % Hp;
     }
-    int64_t cur = 0;
+    int64_t cur = 0, slot = 0;  // next free-list entry, next table slot
     out->tbl_indptr[0] = 0;
     for (int64_t row = 0; row < (int64_t)R * C; ++row) {
         const int64_t n = (cap[row] + page_size - 1) / page_size;
-        std::memcpy(out->tbl_pages + cur, free_pages + cur, sizeof(int32_t) * (size_t)n);
-        cur += n;
-        out->tbl_indptr[row + 1] = cur;
+        std::memcpy(out->tbl_pages + slot, free_pages + cur, sizeof(int32_t) * (size_t)n);
+        std::fill(out->tbl_pages + slot + n, out->tbl_pages + slot + n + headroom, -1);  // growth slots: no page yet
+        cur += n, slot += n + headroom;
+        out->tbl_indptr[row + 1] = slot;
+        if (out->row_pages) out->row_pages[row] = (int32_t)n;
     }
     if ((flags & TANGRAM_FILL_GROUP) && kv_len_inout)
         for (int32_t r = 0; r < R; ++r)
             for (int32_t h = 0; h < H; ++h)
                 kv_len_inout[(size_t)r * H + h] = cap[(size_t)r * C + out->cluster_of[h]];
+    return TANGRAM_OK;
+}
+
+// ---- NEXT-4: Vectorized Block Table update (:244): every (request, cluster) row whose longest head has filled
+// the row's pages takes the next free page.  Pass 1 finds those rows for all groups at once -- OpenMP across
+// (cluster, block of 16 requests), AVX-512 inside a block: one gather of the H_p member lengths per lane, a
+// vector max, a compare against pages x P -- and leaves one mask bit per row; pass 2 hands out the pages in row
+// order (the free list is consumed in (request, cluster) order, so it is a sequential walk over the set bits).
+namespace tangram {
+
+static void rows_needing_a_page_scalar(const tangram_tables* t, const int32_t* kv_len, int32_t c, int32_t r0,
+                                       int32_t r1, uint8_t* need) {
+    const int32_t H = t->H, C = t->C, Hp = t->Hp, P = t->P;
+    for (int32_t r = r0; r < r1; ++r) {
+        int32_t longest = 0;
+        for (int32_t k = 0; k < Hp; ++k) longest = std::max(longest, kv_len[(size_t)r * H + t->perm[c * Hp + k]]);
+        const int64_t row = (int64_t)r * C + c;
+        need[row] = (int64_t)longest >= (int64_t)t->row_pages[row] * P;
+    }
+}
+
+#if defined(__x86_64__) && defined(__GNUC__)
+__attribute__((target("avx512f"))) static void rows_needing_a_page_avx512(const tangram_tables* t, const int32_t* kv_len,
+                                                                         int32_t c, int32_t r0, int32_t r1, uint8_t* need) {
+    const int32_t H = t->H, C = t->C, Hp = t->Hp, P = t->P;
+    const __m512i lane = _mm512_setr_epi32(0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15);
+    int32_t r = r0;
+    // 16 requests per step; the 32-bit gather indices must not overflow
+    if ((int64_t)t->R * H < INT32_MAX && (int64_t)t->R * C < INT32_MAX)
+        for (; r + 16 <= r1; r += 16) {
+            const __m512i rr = _mm512_add_epi32(_mm512_set1_epi32(r), lane);
+            const __m512i seq0 = _mm512_mullo_epi32(rr, _mm512_set1_epi32(H));
+            __m512i longest = _mm512_setzero_si512();
+            for (int32_t k = 0; k < Hp; ++k) {
+                const __m512i idx = _mm512_add_epi32(seq0, _mm512_set1_epi32(t->perm[c * Hp + k]));
+                longest = _mm512_max_epi32(longest, _mm512_i32gather_epi32(idx, kv_len, 4));
+            }
+            const __m512i row = _mm512_add_epi32(_mm512_mullo_epi32(rr, _mm512_set1_epi32(C)), _mm512_set1_epi32(c));
+            const __m512i have = _mm512_i32gather_epi32(row, t->row_pages, 4);
+            // longest >= have * P  (lengths and capacities are far below 2^31)
+            const __mmask16 m = _mm512_cmpge_epi32_mask(longest, _mm512_mullo_epi32(have, _mm512_set1_epi32(P)));
+            for (int32_t i = 0; i < 16; ++i) need[((int64_t)r + i) * C + c] = (m >> i) & 1;
+        }
+    rows_needing_a_page_scalar(t, kv_len, c, r, r1, need);
+}
+static bool have_avx512() { return __builtin_cpu_supports("avx512f"); }
+#else
+static bool have_avx512() { return false; }
+#endif
+
+}  // namespace tangram
+
+extern "C" int tangram_extend_tables(tangram_tables* t, const int32_t* kv_len, const int32_t* free_pages, int64_t n_free,
+                                     int32_t n_threads, int64_t* n_extended_out, int64_t* n_starved_out) {
+    if (!t || !kv_len || (n_free > 0 && !free_pages) || n_free < 0)
+        return fail(TANGRAM_ERR_INVALID_ARG, "extend_tables: NULL argument");
+    if (!t->row_pages || !t->tbl_indptr || !t->tbl_pages || !t->perm)
+        return fail(TANGRAM_ERR_INVALID_ARG, "extend_tables: the tables were built without row_pages (growth headroom)");
+    const int32_t R = t->R, C = t->C;
+    const int64_t n_rows = (int64_t)R * C;
+    std::vector<uint8_t> need((size_t)n_rows, 0);
+    const bool simd = have_avx512();
+    const int32_t blocks = (R + 255) / 256;  // 256 requests = 16 vector steps per task
+    const int64_t n_tasks = (int64_t)C * blocks;
+#ifdef _OPENMP
+    const int nt = n_threads > 0 ? n_threads : std::min<int64_t>(omp_get_max_threads(), std::max<int64_t>(1, n_rows / 2048));
+#pragma omp parallel for schedule(static) num_threads(nt) if (nt > 1)
+#endif
+    for (int64_t task = 0; task < n_tasks; ++task) {
+        const int32_t c = (int32_t)(task / blocks), r0 = (int32_t)(task % blocks) * 256, r1 = std::min(R, r0 + 256);
+#if defined(__x86_64__) && defined(__GNUC__)
+        if (simd) rows_needing_a_page_avx512(t, kv_len, c, r0, r1, need.data());
+        else
+#endif
+            rows_needing_a_page_scalar(t, kv_len, c, r0, r1, need.data());
+    }
+    (void)simd, (void)n_threads;
+    int64_t cursor = t->n_pages_used, extended = 0, starved = 0;
+    for (int64_t row = 0; row < n_rows; ++row) {
+        if (!need[(size_t)row]) continue;
+        const int64_t lo = t->tbl_indptr[row], slots = t->tbl_indptr[row + 1] - lo;
+        const int32_t have = t->row_pages[row];
+        if (have >= slots || cursor >= n_free) {
+            ++starved;
+            continue;
+        }
+        t->tbl_pages[lo + have] = free_pages[cursor++];
+        t->row_pages[row] = have + 1;
+        ++extended;
+    }
+    t->n_pages_used = cursor;
+    if (n_extended_out) *n_extended_out = extended;
+    if (n_starved_out) *n_starved_out = starved;
     return TANGRAM_OK;
 }
 

@@ -240,3 +240,96 @@ def test_default_dynamic_tail_rule():
     edge = np.full((1, 1), 64 * 31, dtype=np.int32)                                       # 31 granules + 1 overhead = 32
     assert T.tangram_default_dynamic_tail(edge, 1, 64, 1) == O.default_dynamic_tail(edge, 1, 64, 1) == (500, 6)
     assert T.tangram_default_dynamic_tail(edge - 64, 1, 64, 1) == O.default_dynamic_tail(edge - 64, 1, 64, 1) == (0, 0)
+
+
+# ---------------------------------------------------------------------------- NEXT-4: growable tables (host path)
+def tables_equal(to, tp):
+    for f in ("tbl_indptr", "tbl_pages", "row_pages"):
+        a, b = getattr(to, f), getattr(tp, f)
+        assert a.dtype == b.dtype and np.array_equal(a, b), f
+    assert to.n_pages_used == tp.n_pages_used
+
+
+@pytest.mark.parametrize("name,Hp", [("8b", 1), ("8b", 2), ("8b", 8), ("32b", 1), ("32b", 4), ("uniform", 8), ("skew", 4)])
+def test_growable_tables_and_vectorized_update_bit_exact(name, Hp):
+    """Tables with growth headroom and 60 block-table updates of a decode loop (lengths + 1 per step, every head
+    started a few tokens before its page boundary) on the full-size configs at several heads per page: slot
+    layout, page ids, row_pages, free-list cursor and the extended / starved counts equal the oracle's, with one
+    thread and with four (the OpenMP row scan) -- and the AVX-512 path equals the scalar path wherever it runs."""
+    wl = I.make_workload(name)
+    C = wl.H // Hp
+    Bo, reso, kvo = O.reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    need = T.tangram_pages_needed(Bo, reso, C, wl.P)
+    free = I.make_free_pages(wl, need + 2 * wl.R * C + 3)            # short: every row wants 3 more pages, some a 4th
+    to, _ = O.build_ragged_tables(Bo, reso, C, wl.P, free, 0, kvo, headroom_pages=3)
+    tp, _ = T.tangram_build_ragged_tables(Bo, reso, C, wl.P, free, 0, kvo, headroom_pages=3)
+    tp4, _ = T.tangram_build_ragged_tables(Bo, reso, C, wl.P, free, 0, kvo, headroom_pages=3)
+    tables_equal(to, tp)
+    rng = np.random.default_rng(7)
+    # every row starts between 0 and 20 tokens before the end of its pages
+    rows = np.arange(wl.R)[:, None] * C + to.cluster_of[None, :]
+    kv = np.maximum(to.row_pages[rows] * wl.P - rng.integers(0, 21, size=(wl.R, wl.H)), 0).astype(np.int32)
+    tot_ext = tot_starved = 0
+    for step in range(60):
+        to, starved = O.extend_tables(to, kv, free)
+        ext_p, starved_p = T.tangram_extend_tables(tp, kv, free, n_threads=1)
+        ext_4, starved_4 = T.tangram_extend_tables(tp4, kv, free, n_threads=4)
+        assert starved == starved_p == starved_4 and ext_p == ext_4
+        tables_equal(to, tp)
+        tables_equal(to, tp4)
+        tot_ext, tot_starved = tot_ext + ext_p, tot_starved + starved
+        cap = to.row_pages[rows] * wl.P
+        kv = np.minimum(kv + 1, cap).astype(np.int32)                # what append_kv leaves (full rows drop)
+    assert tot_ext == to.n_pages_used - need and tot_ext > 0 and tot_starved > 0
+    assert to.n_pages_used == len(free)                              # the free list was used up, in order
+    used = to.tbl_pages[to.tbl_pages >= 0]
+    assert sorted(used.tolist()) == sorted(free.tolist())
+
+
+@settings(max_examples=40, deadline=None)
+@given(seed=st.integers(0, 10 ** 6), R=st.integers(1, 40), Hp=st.sampled_from([1, 2, 3, 4]), C=st.integers(1, 4),
+       headroom=st.integers(1, 3), P=st.sampled_from([1, 4, 16]))
+def test_growable_tables_random_shapes(seed, R, Hp, C, headroom, P):
+    rng = np.random.default_rng(seed)
+    H = Hp * C
+    B = rng.uniform(0.05, 1.0, size=H)
+    res = rng.integers(1, 70, size=(R, H)).astype(np.int32)
+    need = T.tangram_pages_needed(B, res, C, P)
+    free = rng.permutation(need + int(rng.integers(0, 2 * R * C + 1))).astype(np.int32)
+    to, _ = O.build_ragged_tables(B, res, C, P, free, headroom_pages=headroom)
+    tp, _ = T.tangram_build_ragged_tables(B, res, C, P, free, headroom_pages=headroom)
+    tables_equal(to, tp)
+    kv = res.copy()
+    for step in range(3 * P + 2):
+        to, starved = O.extend_tables(to, kv, free)
+        ext, starved_p = T.tangram_extend_tables(tp, kv, free, n_threads=int(rng.integers(0, 3)))
+        assert starved == starved_p
+        tables_equal(to, tp)
+        rows = np.arange(R)[:, None] * C + to.cluster_of[None, :]
+        kv = np.minimum(kv + rng.integers(0, 2, size=kv.shape), to.row_pages[rows] * P).astype(np.int32)
+
+
+def test_growable_tables_error_contract():
+    B = np.array([0.5, 0.25])
+    res = np.array([[20, 10]], dtype=np.int32)
+    free = np.arange(10, dtype=np.int32)
+    tight, _ = T.tangram_build_ragged_tables(B, res, 2, 16, free)
+    assert tight.row_pages is None and len(tight.tbl_pages) == tight.n_pages_used == 3
+    with pytest.raises(T.TangramError) as e:                          # no headroom, no row_pages: nothing to grow into
+        T._check(T._lib.tangram_extend_tables(ctypes.byref(tight._c()), T._ptr(res), T._ptr(free), ctypes.c_int64(10),
+                                              ctypes.c_int32(0), None, None))
+    assert e.value.code == T.ERR_INVALID_ARG
+    ct = tight._c()
+    ct.headroom_pages = 2                                             # headroom asked for without the row_pages array
+    rc = T._lib.tangram_build_ragged_tables(T._ptr(B), T._ptr(res), 1, 2, 2, 16, T._ptr(free), ctypes.c_int64(10), 0, None,
+                                            ctypes.byref(ct))
+    assert rc == T.ERR_INVALID_ARG
+    ct.headroom_pages = -1
+    rc = T._lib.tangram_build_ragged_tables(T._ptr(B), T._ptr(res), 1, 2, 2, 16, T._ptr(free), ctypes.c_int64(10), 0, None,
+                                            ctypes.byref(ct))
+    assert rc == T.ERR_INVALID_ARG
+    grow, _ = T.tangram_build_ragged_tables(B, res, 2, 16, free, headroom_pages=2)
+    assert len(grow.tbl_pages) == 3 + 2 * 2 and grow.row_pages.tolist() == [1, 2]
+    # the planner accepts lengths up to the slot capacity (an open-ended plan covers the growth)
+    pl = T.tangram_plan_partitions(grow, B, np.array([[64, 48]], dtype=np.int32), 4, 64, 1, T.MODE_BALANCED)
+    assert int(pl.items[:, 5].max()) == 64
