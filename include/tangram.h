@@ -275,6 +275,11 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
  * alignment, source not page-locked), CUDA. */
 int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream);
 
+/* Measurement aid: reads `bytes` (a multiple of 16) of device memory once with 16-byte streaming loads on all SMs
+ * and discards them -- a read-only HBM stream, the ceiling a4 can be held against (bench.py `roofline.read_peak_gbs`).
+ * sink_dev: device u32 scratch.  Errors: INVALID_ARG, CUDA. */
+int tangram_read_stream(const void* src_dev, size_t bytes, uint32_t* sink_dev, void* stream);
+
 /* The two kernels of tangram_decode_attention as separate calls (same arguments, same checks):
  * a4 alone (split-KV decode kernel: final outputs of single-part sequences, fp32 partials of the
  * others into `workspace`) and a5 alone (LSE merge of the partials in `workspace` into out / lse;

@@ -76,7 +76,7 @@ for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram
               "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios",
               "tangram_compact_topk_chunk", "tangram_stage_from_host", "tangram_default_dynamic_tail",
               "tangram_extend_tables", "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables",
-              "tangram_decode_step", "tangram_reset_plan"):
+              "tangram_decode_step", "tangram_reset_plan", "tangram_read_stream"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
@@ -86,7 +86,7 @@ EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragge
            "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk",
            "tangram_stage_from_host", "tangram_default_dynamic_tail", "tangram_extend_tables",
            "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables", "tangram_decode_step",
-           "tangram_reset_plan")
+           "tangram_reset_plan", "tangram_read_stream")
 STEP_OVERLAP = 1
 
 
@@ -340,6 +340,12 @@ def tangram_download_tables(dp: DevicePlan, t: Tables, stream=None) -> int:
     _check(_lib.tangram_download_tables(C.byref(dp.c), C.byref(ct), C.byref(starved), _stream_ptr(stream)))
     t.n_pages_used = int(ct.n_pages_used)
     return int(starved.value)
+
+
+def tangram_read_stream(src, sink, nbytes=None, stream=None):
+    """Measurement aid: one read-only pass over `src` (cuda tensor) with 16-byte loads; sink = uint32/int32[1] cuda."""
+    n = src.numel() * src.element_size() if nbytes is None else nbytes
+    _check(_lib.tangram_read_stream(C.c_void_p(src.data_ptr()), C.c_size_t(n), C.c_void_p(sink.data_ptr()), _stream_ptr(stream)))
 
 
 def tangram_reset_plan(dp: DevicePlan, stream=None):

@@ -992,6 +992,26 @@ tangram_stage_kernel(uint4* __restrict__ dst, const uint4* __restrict__ src, siz
         dst[i] = src[i];
 }
 
+// ------------------------------------------------------------------ measurement aid: a read-only HBM stream
+// 16-byte streaming loads, four in flight per thread, grid-stride; the xor keeps the loads alive.  This is the
+// ceiling a read-only kernel such as a4 can be held against (MEASURED_PEAKS.json's copy is a read+write stream).
+__global__ void __launch_bounds__(512)
+tangram_read_stream_kernel(const uint4* __restrict__ src, size_t n16, uint32_t* __restrict__ sink) {
+    uint32_t acc = 0;
+    size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const size_t stride = static_cast<size_t>(gridDim.x) * blockDim.x;
+    for (; i + 3 * stride < n16; i += 4 * stride) {
+        const uint4 a = __ldcs(src + i), b = __ldcs(src + i + stride), c = __ldcs(src + i + 2 * stride),
+                    d = __ldcs(src + i + 3 * stride);
+        acc ^= a.x ^ a.y ^ a.z ^ a.w ^ b.x ^ b.y ^ b.z ^ b.w ^ c.x ^ c.y ^ c.z ^ c.w ^ d.x ^ d.y ^ d.z ^ d.w;
+    }
+    for (; i < n16; i += stride) {
+        const uint4 a = __ldcs(src + i);
+        acc ^= a.x ^ a.y ^ a.z ^ a.w;
+    }
+    if (acc == 0x9e3779b9u) atomicAdd(sink, 1u);  // practically never; only keeps `acc` observable
+}
+
 // ------------------------------------------------------------------ host-side launch helpers
 static int cuda_fail(cudaError_t e, const char* what) {
     return fail(TANGRAM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
@@ -1066,12 +1086,15 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
+    // Programmatic dependent launch next to the cooperative attribute: if the driver refuses the pair once, it is
+    // not asked again (a failing launch inside a stream capture would invalidate the capture).
+    static int pdl_refused = 0;
+    if (pdl_refused) prm.pdl = 0;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
     e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
     if (e != cudaSuccess && prm.pdl) {
-        // the two attributes together are refused: launch without the overlap (the kernel then must not wait)
         (void)cudaGetLastError();
-        prm.pdl = 0, cfg.numAttrs = 1;
+        pdl_refused = 1, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
         e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
     }
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
@@ -1548,6 +1571,20 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
         static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_read_stream(const void* src_dev, size_t bytes, uint32_t* sink_dev, void* stream) {
+    if (!src_dev || !sink_dev || bytes % 16 || reinterpret_cast<uintptr_t>(src_dev) % 16)
+        return fail(TANGRAM_ERR_INVALID_ARG, "read_stream: NULL / misaligned argument");
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e, "read_stream: device query");
+    tangram_read_stream_kernel<<<sms * 16, 512, 0, static_cast<cudaStream_t>(stream)>>>(static_cast<const uint4*>(src_dev),
+                                                                                        bytes / 16, sink_dev);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "read_stream launch");
     return TANGRAM_OK;
 }
 
