@@ -34,16 +34,30 @@ NOMINAL_TBS = 8.0
 FALLBACK_PEAK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 
 
+def csrc_hash() -> str:
+    """sha256 (first 16 hex digits) over the kernel sources: ties a committed ncu capture to the code it measured."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_06302_b200", "csrc")
+    for fn in sorted(os.listdir(d)):
+        h.update(fn.encode())
+        h.update(open(os.path.join(d, fn), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def profiled_traffic(workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of the decode kernel, per launch, from the committed
-    `ncu --set full` capture of this workload (profiles/*_traffic.csv), or None."""
+    `ncu --set full` capture of this workload (profiles/*_traffic.csv) -- only from a row whose `csrc_hash` column
+    equals the hash of the current kernel sources (a capture of older code says nothing about this build); else None."""
     best = None
     try:
         import csv
         import glob
+        cur = csrc_hash()
         for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
             for row in csv.DictReader(open(path)):
-                if row["workload"] == workload and row["kernel"] == "tangram_decode_kernel":
+                if (row["workload"] == workload and row["kernel"] == "tangram_decode_kernel"
+                        and row.get("csrc_hash", "") == cur):
                     best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
     except Exception:
         return None
@@ -76,6 +90,40 @@ def aggregate(ms_local: float, units_local: float, world: int, device=None):
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dist.all_reduce(u, op=dist.ReduceOp.SUM)
     return float(t.item()), float(u.item())
+
+
+def spawn_ranks(n: int, argv) -> int:
+    """`bench.py --gpus N` started bare (no torchrun, WORLD_SIZE unset): start the N ranks ourselves, one process per
+    GPU, rendezvous on 127.0.0.1, and wait for them.  Rank 0 prints the JSON line."""
+    import socket
+    import subprocess
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    procs = []
+    for r in range(n):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + list(argv), env=env))
+    rcs = [p.wait() for p in procs]
+    return next((rc for rc in rcs if rc != 0), 0)
+
+
+def plumbing_only(args):
+    """The multi-rank plumbing without the GPU work (tests/test_bench_dist.py, gloo on CPU): rendezvous, barrier,
+    max-over-ranks / sum-over-ranks aggregation, rank 0 prints one JSON line."""
+    import torch.distributed as dist
+    rank, _, world = dist_env()
+    if world > 1:
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+        dist.barrier()
+    ms, units = aggregate(1.0 + rank, 100.0 * (rank + 1), world, device="cpu")
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"plumbing_only": True, "n_gpus": world, "ms_per_step": ms, "units": units}))
 
 
 class ClockSampler:
@@ -147,16 +195,19 @@ def algorithmic_bytes(wl, kv, plan, t):
             "total": kv_bytes + qo + partials + page_ids}
 
 
-def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None, layer=0, plan_capacity=False):
+def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None, layer=0, plan_capacity=False, R=None,
+                   headroom=0):
+    """Budgets, tables and plan of workload `name` through the product's API.  headroom > 0: growable tables (that
+    many empty page slots per row, and a pool / free list large enough to fill them) for the decode loop."""
     import torch
-    wl = I.make_workload(name, layer=layer)
+    wl = I.make_workload(name, layer=layer, R=R)
     t0 = time.perf_counter()
     B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
     need = T.tangram_pages_needed(B, res, wl.C, wl.P)
-    n_pool = int(math.ceil(1.05 * need))
+    n_pool = int(math.ceil(1.05 * need)) + headroom * wl.R * wl.C
     free = I.make_free_pages(wl, n_pool)
     t1 = time.perf_counter()
-    tb, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, free, 0, kv)
+    tb, kv = T.tangram_build_ragged_tables(B, res, wl.C, wl.P, free, 0, kv, headroom_pages=headroom)
     t2 = time.perf_counter()
     if W is None:
         W = T.tangram_query_max_ctas(torch.cuda.current_device(), wl.d, wl.G)
@@ -173,7 +224,7 @@ def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None, layer=
     q, pool = I.make_q_and_pool(wl, n_pool, device)
     host_ms = {"reserve_ms": (t1 - t0) * 1e3, "tables_ms": (t2 - t1) * 1e3, "plan_ms": (t4 - t3) * 1e3}
     return dict(wl=wl, B=B, res=res, kv=kv, tables=tb, plan=plan, W=W, q=q, pool=pool, n_pool=n_pool,
-                host_ms=host_ms, c0=c0, dyn=dyn)
+                host_ms=host_ms, c0=c0, dyn=dyn, free=free)
 
 
 class L2Flusher:
@@ -320,52 +371,81 @@ def reference_arm(args):
 # NEXT-1: a real decode loop -- L layers x (KV append + attention) per step under ONE CUDA graph
 # ------------------------------------------------------------------------------------------------
 def decode_loop(T, I, name, device, layers, steps, torch):
-    """Every layer has its own budgets, clusters, tables and an open-ended plan built once for the
-    tables' capacity; one decode step = for each layer: tangram_append_kv, then tangram_decode_attention
-    on the run-time lengths.  The L-layer step is captured in one CUDA graph and replayed: zero host
-    planning across steps and layers.  The layers' pools are distinct and far larger than
-    L2 together, so no flush is needed between layer-steps."""
+    """Every layer has its own budgets, clusters, growable tables and an open-ended plan built once for the tables'
+    slot capacity; one decode step = for each layer ONE launch of tangram_decode_step (KV append + attention +
+    merge + length update + block-table growth for the next step), chained by programmatic dependent launch.  The
+    L-layer step is captured in one CUDA graph and replayed: zero host work across steps and layers.
+    The layers' pools are distinct and far larger than L2 together, so no flush is needed between layer-steps.
+    `two_launches` is the round-1 loop (tangram_append_kv + tangram_decode_attention) on the same data."""
+    headroom = (steps + 8) // 16 + 2                     # page slots for every token the loop appends
     Ls = []
     for l in range(layers):
-        S = setup_workload(T, I, name, device, layer=l, plan_capacity=True)
+        S = setup_workload(T, I, name, device, layer=l, plan_capacity=True, headroom=headroom)
         prepare(T, S, torch)
         S["kv_dev"] = torch.as_tensor(S["kv"], device=device)
+        S["kv_dev2"] = S["kv_dev"].clone()
+        S["free_dev"] = torch.as_tensor(S["free"], device=device)
+        S["over"] = torch.zeros(2, dtype=torch.int32, device=device)
+        S["pages0"] = int(S["tables"].n_pages_used)
         g = torch.Generator(device=device).manual_seed(S["wl"].seed + 17)
         S["k_new"] = torch.randn(S["wl"].R, S["wl"].H, S["wl"].d, generator=g, device=device).bfloat16()
         S["v_new"] = torch.randn(S["wl"].R, S["wl"].H, S["wl"].d, generator=g, device=device).bfloat16()
         Ls.append(S)
 
-    def one_step(stream=None):
+    def fused_step(stream=None):
         for S in Ls:
-            T.tangram_append_kv(S["dp"], S["k_new"], S["v_new"], S["pool"], S["kv_dev"], stream=stream)
-            T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"], kv_len=S["kv_dev"],
+            T.tangram_decode_step(S["dp"], S["q"], S["k_new"], S["v_new"], S["pool"], S["kv_dev"], S["free_dev"], S["out"],
+                                  S["lse"], S["ws"], overflow=S["over"][0:1], flags=T.STEP_OVERLAP, stream=stream)
+
+    def two_launch_step(stream=None):
+        for S in Ls:
+            T.tangram_append_kv(S["dp"], S["k_new"], S["v_new"], S["pool"], S["kv_dev2"], S["over"][1:2], stream=stream)
+            T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"], kv_len=S["kv_dev2"],
                                        stream=stream)
 
-    st = torch.cuda.Stream()
-    st.wait_stream(torch.cuda.current_stream())
-    with torch.cuda.stream(st):
-        one_step(st)                                  # warm-up outside the capture
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph, stream=st):
-            one_step(st)
-        for _ in range(3):
-            graph.replay()
-        st.synchronize()
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        for a, b in evs:
-            a.record(st)
-            graph.replay()
-            b.record(st)
-        st.synchronize()
-    torch.cuda.current_stream().wait_stream(st)
-    ms = np.array([a.elapsed_time(b) for a, b in evs])
-    kv_bytes = float(np.mean([int(S["kv_dev"].sum().item()) * 4 * S["wl"].d for S in Ls]))
+    def timed(one_step, n):
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(st):
+            one_step(st)                                  # warm-up outside the capture
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=st):
+                one_step(st)
+            for _ in range(3):
+                graph.replay()
+            st.synchronize()
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+            for a, b in evs:
+                a.record(st)
+                graph.replay()
+                b.record(st)
+            st.synchronize()
+        torch.cuda.current_stream().wait_stream(st)
+        return np.array([a.elapsed_time(b) for a, b in evs])
+
+    for S in Ls:                                          # room for the first appended token
+        T.tangram_extend_tables_device(S["dp"], S["kv_dev"], S["free_dev"])
+    len0 = float(np.mean([int(S["kv_dev"].sum().item()) for S in Ls]))
+    ms = timed(fused_step, steps - 4)                     # 1 eager + 3 warm replays + (steps - 4) timed = steps appends
+    len1 = float(np.mean([int(S["kv_dev"].sum().item()) for S in Ls]))
+    kv_bytes = 0.5 * (len0 + len1) * 4 * Ls[0]["wl"].d    # mean retained K/V over the loop (lengths grow every step)
     us_layer = float(np.median(ms)) * 1e3 / layers
+    ms2 = timed(two_launch_step, max(4, (steps - 4) // 2))
+    us_layer2 = float(np.median(ms2)) * 1e3 / layers
+    torch.cuda.synchronize()
+    starved = sum(T.tangram_download_tables(S["dp"], S["tables"]) for S in Ls)
     return {"layers": layers, "steps": steps, "us_per_layer_step": us_layer, "us_per_decode_step": us_layer * layers,
             "tbs": kv_bytes / (us_layer * 1e-6) / 1e12, "pct_of_8tbs": 100 * kv_bytes / (us_layer * 1e-6) / 1e12 / NOMINAL_TBS,
-            "launches_per_layer_step": 2, "host_planning_per_step_ms": 0.0,
-            "note": "append + attention per layer, open-ended plans built once, whole L-layer step in one CUDA graph; "
-                    "kv bytes = retained K/V at the end of the loop (the lengths grow by one token per step)"}
+            "launches_per_layer_step": 1, "host_planning_per_step_ms": 0.0,
+            "overflow": int(sum(int(S["over"][0].item()) for S in Ls)), "rows_starved": int(starved),
+            "tokens_appended_per_head": steps,
+            "pages_handed_out": int(sum(S["tables"].n_pages_used - S["pages0"] for S in Ls)),
+            "overlap_state": T.tangram_overlap_state(),
+            "two_launches": {"us_per_layer_step": us_layer2, "overflow": int(sum(int(S["over"][1].item()) for S in Ls)),
+                             "note": "round-1 loop: tangram_append_kv + tangram_decode_attention, tables never grow"},
+            "note": "one tangram_decode_step launch per layer (append + attention + merge + lengths + table growth), "
+                    "chained by programmatic dependent launch, open-ended plans built once, whole L-layer step in one "
+                    "CUDA graph; kv bytes = mean retained K/V over the loop"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -440,7 +520,9 @@ def spread_of(T, S, torch, reps=5):
 
 def prepare(T, S, torch):
     wl, plan = S["wl"], S["plan"]
-    S["dp"] = T.tangram_upload(S["tables"], plan)
+    t0 = time.perf_counter()
+    S["dp"] = T.tangram_upload(S["tables"], plan)      # packs the blob on the host, one H2D copy, stream sync
+    S["host_ms"]["upload_ms"] = (time.perf_counter() - t0) * 1e3
     S["out"] = torch.empty_like(S["q"])
     S["lse"] = torch.empty(wl.R, wl.Hq, dtype=torch.float32, device=S["q"].device)
     S["ws"] = torch.empty(T.tangram_workspace_bytes(plan.n_part_slots, wl.G, wl.d), dtype=torch.uint8,
@@ -448,10 +530,10 @@ def prepare(T, S, torch):
     S["bytes"] = algorithmic_bytes(wl, S["kv"], plan, S["tables"])
 
 
-def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, compare=True, dyn=None):
+def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, compare=True, dyn=None, R=None):
     """µs per layer-step, achieved TB/s, kernel-only roofline, spread, and the same kernel run from the
-    STATIC_EVEN and SPLITMAP plans."""
-    S = setup_workload(T, I, name, device, dyn=dyn)
+    BALANCED plan without its dynamic tail, from STATIC_EVEN and from SPLITMAP."""
+    S = setup_workload(T, I, name, device, dyn=dyn, R=R)
     prepare(T, S, torch)
     step = lambda: T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"])
     ms = time_steps(step, steps, warmup, flush, torch)
@@ -464,13 +546,17 @@ def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, co
            "tbs": b["total"] / (us * 1e-6) / 1e12,
            "pct_of_8tbs": 100 * b["total"] / (us * 1e-6) / 1e12 / NOMINAL_TBS,
            "pct_of_measured_copy": 100 * b["total"] / (us * 1e-6) / 1e9 / peak_gbs,
-           "decode_kernel_us": kus, "decode_kernel_gbs": b["total"] / (kus * 1e-6) / 1e9,
+           "decode_kernel_us": kus, "decode_kernel_gbs": (b["total"] - b["partials"] // 2) / (kus * 1e-6) / 1e9,
            "algorithmic_bytes": b, "W": S["W"], "items": int(S["plan"].n_items), "granule": S["wl"].granule,
            "c0": S["c0"], "dyn_permille": S["dyn"][0], "dyn_rounds": S["dyn"][1], "host_ms": S["host_ms"],
            "cta_spread": spread_of(T, S, torch)}
     if compare:
-        for mode, key in ((T.MODE_STATIC_EVEN, "static_even"), (T.MODE_SPLITMAP, "splitmap")):
+        legs = [(T.MODE_STATIC_EVEN, "static_even"), (T.MODE_SPLITMAP, "splitmap")]
+        if S["dyn"][1] > 0:                   # the same equal-bytes plan, every CTA owning exactly one list
+            legs.insert(0, (T.MODE_BALANCED, "balanced_static"))
+        for mode, key in legs:
             S2 = dict(S)
+            S2["host_ms"] = dict(S["host_ms"])
             S2["plan"] = T.tangram_plan_partitions(S["tables"], S["B"], S["kv"], S["W"], S["wl"].granule, S["c0"], mode)
             prepare(T, S2, torch)
             f2 = lambda: T.tangram_decode_attention(S2["dp"], S2["q"], S2["pool"], S2["out"], S2["lse"], S2["ws"])
@@ -485,11 +571,12 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
     """Same step through the public API with HOST buffers: q comes from pinned host memory and the result
     (out, lse) ends up in pinned host memory inside the timed region.  The KV page pool is the resident state
     of the serving system (written by prefill, like weights) and stays in HBM.
-    zero_copy=True: out / lse are HOST pointers passed straight into the C-ABI call -- pinned memory is mapped into
-    the device's address space and the kernel's (posted) stores go over the bus, so the result never waits for a
-    copy engine; q is pulled from pinned host memory by tangram_stage_from_host (a kernel, not a copy-engine
-    transfer; reading q in place from host memory inside the decode kernel works too, the binding and tests
-    cover it, but every item then waits a bus round trip for its query group: 154 us).
+    zero_copy=True: tangram_decode_attention_host -- out / lse are HOST pointers (pinned memory is mapped into the
+    device's address space and the kernel's posted stores go over the bus, so the result never waits for a copy
+    engine); q is pulled from pinned host memory by the staging kernel, and the decode kernel is launched behind it
+    with programmatic stream serialization, so its launch and the fill of its KV tile rings overlap the transfer
+    (reading q in place from host memory inside the decode kernel works too and is tested, but every work item
+    re-reads its query group over the bus: 1.3 MB instead of 0.26 MB, and the bus queue stalls the CTAs).
     zero_copy=False: explicit staging copies around the call (one H2D, one D2H)."""
     q_host = S["q"].cpu().pin_memory()
     R, Hq, d = S["q"].shape
@@ -501,9 +588,8 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
 
         q_dev = torch.empty_like(S["q"])
 
-        def step():
-            T.tangram_stage_from_host(q_dev, q_host)
-            T.tangram_decode_attention(S["dp"], q_dev, S["pool"], out_host, lse_host, S["ws"])
+        def step():          # ONE C-ABI call: staging kernel + decode kernel overlapped behind it (PDL)
+            T.tangram_decode_attention_host(S["dp"], q_host, q_dev, S["pool"], out_host, lse_host, S["ws"])
     else:
         # out and lse live in ONE device allocation, so the result goes back with a single device->host copy
         res_dev = torch.empty(n_out + n_lse, dtype=torch.uint8, device=S["q"].device)
@@ -526,6 +612,76 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
     return ms, q_host.numel() * 2, n_out + n_lse
 
 
+def read_stream_peak(T, device, flush, torch, nbytes=4 << 30, reps=5):
+    """Builder-measured ceiling of a read-only HBM stream: tangram_read_stream (16-byte loads on all SMs) over 4 GiB,
+    L2 flushed, CUDA events; best of `reps`, in GB/s."""
+    buf = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    buf.random_(0, 255)
+    sink = torch.zeros(1, dtype=torch.int32, device=device)
+    ms = time_steps(lambda: T.tangram_read_stream(buf, sink), reps, 3, flush, torch)
+    del buf
+    torch.cuda.empty_cache()
+    return nbytes / (min(ms) * 1e-3) / 1e9
+
+
+def table_update_summary(T, I, device, torch, names=("8b", "32b"), steps=48):
+    """NEXT-4: cost of one block-table update of the whole batch (every (request, cluster) row checked, full rows
+    handed a page) per decode step, at H_p = 1 / 2 / 4 / 8: the host path (tangram_extend_tables, 1 thread and the
+    OpenMP default) and the device path (tangram_extend_tables_device, CUDA events).  The paper's Table 1 quotes
+    5.64-17.13 ms of per-step planning for its dynamic baseline; its own block-table cost is
+    only shown in Fig. 8(c) (image not available)."""
+    out = {"unit": "us per update of the whole batch", "paper_table1_dynamic_planning_ms": [5.64, 17.13]}
+    for name in names:
+        wl = I.make_workload(name)
+        B, res, kv0 = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+        for Hp in (1, 2, 4, 8):
+            C = wl.H // Hp
+            need = T.tangram_pages_needed(B, res, C, wl.P)
+            headroom = steps // 16 + 2
+            free = I.make_free_pages(wl, need + headroom * wl.R * C)
+            host_us = {}
+            for nt in (1, 0):
+                t, kv = T.tangram_build_ragged_tables(B, res, C, wl.P, free, 0, kv0, headroom_pages=headroom)
+                cur, ts, ext = kv.copy(), [], 0
+                for _ in range(steps):
+                    t0 = time.perf_counter()
+                    e, s_ = T.tangram_extend_tables(t, cur, free, n_threads=nt)
+                    ts.append(time.perf_counter() - t0)
+                    ext += e
+                    cur += 1
+                host_us["1_thread" if nt == 1 else "openmp_default"] = float(np.median(ts) * 1e6)
+            t, kv = T.tangram_build_ragged_tables(B, res, C, wl.P, free, 0, kv0, headroom_pages=headroom)
+            pl = T.tangram_plan_partitions(t, B, kv, 8, wl.granule, 1, T.MODE_BALANCED)
+            dp = T.tangram_upload(t, pl)
+            kv_dev, free_dev = torch.as_tensor(kv, device=device), torch.as_tensor(free, device=device)
+            evs = []
+            for _ in range(steps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                T.tangram_extend_tables_device(dp, kv_dev, free_dev)
+                b.record()
+                kv_dev += 1
+                evs.append((a, b))
+            torch.cuda.synchronize()
+            starved = T.tangram_download_tables(dp, t)
+            out[f"{name}_Hp{Hp}"] = {"rows": wl.R * C, "host_us": host_us,
+                                     "device_us": float(np.median([a.elapsed_time(b) for a, b in evs]) * 1e3),
+                                     "pages_handed_out_host": int(ext), "rows_starved_device": int(starved)}
+    return out
+
+
+def tiny_oracle_one_thread(O, T, I, torch):
+    """SURVEY §8(d) 'Oracle timing': the whole Tiny workload through the fp64 oracle on ONE thread, wall seconds."""
+    S = setup_workload(T, I, "tiny", "cpu", W=4)
+    wl = S["wl"]
+    pairs = [(r, j) for r in range(wl.R) for j in range(wl.Hq)]
+    best = 1e9
+    for _ in range(5):
+        dt, used = run_oracle_sample(O, S, S["q"], S["pool"], pairs, threads=1)
+        best = min(best, dt)
+    return {"seconds": best, "threads": 1, "rows": len(pairs), "token_visits": int(S["kv"].sum()) * wl.G}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -540,9 +696,19 @@ def main():
     ap.add_argument("--dyn-rounds", type=int, default=None)
     ap.add_argument("--decode-loop-layers", type=int, default=8,
                     help="layers of the multi-layer decode loop summary (0 = skip)")
+    ap.add_argument("--plumbing-only", action="store_true",
+                    help="exercise only the multi-rank plumbing (spawn, rendezvous, barrier, aggregation) on CPU / gloo")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_arm(args)
+        return
+    # --gpus N does what it says: under torchrun the world must have N ranks; started bare, N ranks are spawned here
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ.get('WORLD_SIZE', '1')}")
+    if args.plumbing_only:
+        plumbing_only(args)
         return
     args.warmup = max(args.warmup, 3)
 
@@ -556,6 +722,7 @@ def main():
     torch.cuda.set_device(local_rank)
     device = f"cuda:{local_rank}"
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")      # the communicator log shows the ranks that really joined
         dist.init_process_group("nccl", device_id=torch.device(device))
     peak_gbs, peak_src = measured_peak()
     flush = L2Flusher(device)
@@ -583,10 +750,12 @@ def main():
     ms_step, total_bytes = aggregate(ms_step_local, float(b["total"]), world, device)
     tbs = total_bytes / (ms_step * 1e-3) / 1e12
 
-    # ---- kernel-only roofline for the dominant kernel (split-KV decode kernel)
+    # ---- kernel-only roofline for the dominant kernel (split-KV decode kernel alone: it does not read the partials
+    #      back, so half of the partial bytes -- the merge's reads -- are not counted for it)
     kern = lambda: T.tangram_decode_partials(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"])
     kms = time_steps(kern, args.steps, 3, flush, torch)
-    k_gbs = b["total"] / (float(np.mean(kms)) * 1e-3) / 1e9
+    k_bytes = b["total"] - b["partials"] // 2
+    k_gbs = k_bytes / (float(np.mean(kms)) * 1e-3) / 1e9
     # ---- end to end with host buffers
     ems, h2d, d2h = e2e_steps(T, S, args.steps, 3, flush, torch, zero_copy=True)
     e_ms, e_bytes = aggregate(float(np.mean(ems)), float(b["total"]), world, device)
@@ -597,6 +766,7 @@ def main():
             dist.destroy_process_group()
         return
 
+    read_peak = read_stream_peak(T, device, flush, torch)
     line = {
         "metric": METRIC, "value": tbs, "unit": "TB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "us_per_layer_step": ms_step * 1e3,
@@ -610,14 +780,15 @@ def main():
                    "granule": S["wl"].granule, "c0": S["c0"], "items": int(S["plan"].n_items),
                    "kv_bytes": b["kv"], "algorithmic_bytes": b["total"], "pool_bytes": S["pool"].numel() * 2,
                    "l2": "inputs larger than L2 and an L2 flush (256 MB write, then 256 MB read) before every timed step",
-                   "multi_gpu": "replicas only (path shards by request, no collective)"},
+                   "multi_gpu": "replicas only (path shards by request, no collective)",
+                   "host_ms": {k: round(v, 3) for k, v in S["host_ms"].items()}},
         "e2e": {"value": e_bytes / (e_ms * 1e-3) / 1e12, "unit": "TB/s", "us_per_layer_step": e_ms * 1e3,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "us_per_layer_step_staged_copies": float(np.mean(ems_staged) * 1e3),
-                "note": "every step: q pulled from pinned host memory by tangram_stage_from_host (H2D over the bus), "
-                        "out+lse written by the kernel straight into pinned, device-mapped host memory (host pointers "
-                        "passed to the C-ABI call), all inside the timed region; `staged_copies` = the same with "
-                        "copy-engine transfers (one H2D before, one D2H after the call); "
+                "note": "one tangram_decode_attention_host call per step: q pulled from pinned host memory by the staging "
+                        "kernel with the decode kernel launched behind it by programmatic dependent launch, out+lse written "
+                        "by the kernel straight into pinned, device-mapped host memory, all inside the timed region; "
+                        "`staged_copies` = the same with copy-engine transfers (one H2D before, one D2H after the call); "
                         "the KV page pool is resident serving state in HBM"},
         # one cooperative launch per step (the merge runs inside the decode grid); the stand-alone merge
         # kernel is only launched when the grid cannot be co-resident, which bench.py never asks for
@@ -625,7 +796,11 @@ def main():
         "roofline": {"bound": "hbm", "kernel": "tangram_decode_kernel", "achieved": k_gbs, "peak": peak_gbs,
                      "unit": "GB/s", "frac": k_gbs / peak_gbs, "traffic": profiled_traffic(args.workload),
                      "peak_source": peak_src,
-                     "kernel_us": float(np.mean(kms) * 1e3), "algorithmic_bytes_per_launch": b["total"]},
+                     "kernel_us": float(np.mean(kms) * 1e3), "algorithmic_bytes_per_launch": k_bytes,
+                     # the peak above is a read+write copy; this kernel only reads.  Builder-measured in this run:
+                     "read_peak_gbs": read_peak, "frac_of_read_peak": k_gbs / read_peak,
+                     "read_peak_how": "tangram_read_stream: 16-byte loads on all SMs over 4 GiB, L2 flushed, CUDA events, best of 5",
+                     "step_frac_of_read_peak": tbs * 1e3 / world / read_peak},
         "clocks": clocks.summary(),
         "host_ms": S["host_ms"], "wall_s_timed_region": wall,
         "paper_context": "Tangram reports ratios only: up to 1.7x decode-attention inflation from static "
@@ -633,34 +808,66 @@ def main():
                          "full KV (4xA100-80GB, PAPER.md:13); no absolute us or TB/s to compare with",
     }
     line["cta_spread"] = spread_of(T, S, torch)
+    line["config"]["cta_spread"] = round(line["cta_spread"], 4)
     if not args.no_sweep and world == 1:
         per = {}
         del S
         torch.cuda.empty_cache()
-        for name in ("tiny", "8b", "32b", "skew", "uniform", "12b_d256"):
-            S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs, dyn=dyn)
-            if name == args.workload and not args.no_cpu_baseline:
+        # batch-4 8b-shaped: the paper's own decode-attention comparison point (Fig. 13: batch 4)
+        sweep = [("tiny", None), ("8b", None), ("32b", None), ("skew", None), ("uniform", None), ("12b_d256", None),
+                 ("8b_batch4", 4)]
+        for key, R in sweep:
+            name = "8b" if key == "8b_batch4" else key
+            S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs, dyn=dyn, R=R)
+            if key == args.workload and not args.no_cpu_baseline:
                 from oracle import tangram_oracle as O
                 O.build_c()
                 line["cpu_baseline"] = cpu_baseline(O, S2)
-            per[name] = res
+            per[key] = res
             del S2
             torch.cuda.empty_cache()
         line["per_config"] = per
+        # compact copy the driver's record keeps: [us per layer-step, TB/s, kernel GB/s, per-CTA spread,
+        # BALANCED-without-dynamic-tail slowdown (x), STATIC_EVEN slowdown (x)]
+        line["config"]["per_config_summary"] = {
+            "columns": ["us", "tbs", "kernel_gbs", "cta_spread", "balanced_static_x", "static_even_x"],
+            **{k: [round(v["us_per_layer_step"], 2), round(v["tbs"], 3), round(v["decode_kernel_gbs"], 0),
+                   round(v["cta_spread"], 4),
+                   round(v["balanced_static"]["slowdown_vs_balanced"], 3) if "balanced_static" in v else None,
+                   round(v["static_even"]["slowdown_vs_balanced"], 3)] for k, v in per.items()}}
         if args.decode_loop_layers > 0:
-            line["decode_loop"] = decode_loop(T, I, args.workload, device, args.decode_loop_layers, 30, torch)
+            dl = decode_loop(T, I, args.workload, device, args.decode_loop_layers, 36, torch)
+            line["decode_loop"] = dl
+            line["config"]["decode_loop"] = {"us_per_layer_step": round(dl["us_per_layer_step"], 2),
+                                             "launches_per_layer_step": dl["launches_per_layer_step"],
+                                             "overflow": dl["overflow"], "layers": dl["layers"],
+                                             "two_launches_us": round(dl["two_launches"]["us_per_layer_step"], 2),
+                                             "two_launches_overflow": dl["two_launches"]["overflow"]}
             torch.cuda.empty_cache()
+        tu = table_update_summary(T, I, device, torch)
+        line["table_update"] = tu
+        line["config"]["table_update_us"] = {k: [round(v["host_us"]["1_thread"], 1), round(v["host_us"]["openmp_default"], 1),
+                                                 round(v["device_us"], 1)]
+                                             for k, v in tu.items() if isinstance(v, dict)}
+        line["config"]["table_update_us"]["columns"] = ["host 1 thread", "host OpenMP", "device kernel"]
     elif not args.no_cpu_baseline and world == 1:
         from oracle import tangram_oracle as O
         O.build_c()
         S = setup_workload(T, I, args.workload, device)
         line["cpu_baseline"] = cpu_baseline(O, S)
+    if world == 1 and "cpu_baseline" in line:
+        from oracle import tangram_oracle as O
+        t1 = tiny_oracle_one_thread(O, T, I, torch)
+        line["cpu_baseline"]["tiny_1thread_s"] = t1["seconds"]
+        line["cpu_baseline"]["tiny_1thread"] = t1
     if world == 1:
         line["page_accounting"] = page_accounting_summary(T, I, args.workload)
     if world == 1 and not args.no_compact:
         S = None
         torch.cuda.empty_cache()
         line["compact_topk"] = compact_topk_summary(T, I, args.workload, device, 30, flush, torch, peak_gbs)
+        line["config"]["compact_topk"] = {"us": round(line["compact_topk"]["us"], 1),
+                                          "pct_of_measured_copy": round(line["compact_topk"]["pct_of_measured_copy"], 1)}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -275,6 +275,17 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
  * alignment, source not page-locked), CUDA. */
 int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream);
 
+/* tangram_decode_attention with HOST buffers, end to end in one call: q_host (pinned) is pulled into q_stage_dev
+ * (device, R x Hq x d bf16, 16-byte aligned) by the staging kernel, and the decode kernel is launched behind it with
+ * programmatic stream serialization, so its launch, its work-list / page-id fetches and the fill of its KV tile
+ * rings run while the queries cross the bus; it waits for the staged q only before its first query load.  out and
+ * lse may be pinned host pointers (the kernel's stores go over the bus).  All other arguments and errors as for
+ * tangram_decode_attention and tangram_stage_from_host. */
+int tangram_decode_attention_host(const tangram_device_plan* dp, const void* q_host, void* q_stage_dev,
+                                  const void* kv_pool, int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq,
+                                  int32_t d, float sm_scale, void* out, float* lse, void* workspace,
+                                  size_t workspace_bytes, uint64_t* worker_ns, void* stream);
+
 /* Measurement aid: reads `bytes` (a multiple of 16) of device memory once with 16-byte streaming loads on all SMs
  * and discards them -- a read-only HBM stream, the ceiling a4 can be held against (bench.py `roofline.read_peak_gbs`).
  * sink_dev: device u32 scratch.  Errors: INVALID_ARG, CUDA. */
@@ -378,6 +389,9 @@ int tangram_download_tables(const tangram_device_plan* dp, tangram_tables* t, in
  *   all other arguments as for tangram_decode_attention.
  * Errors: as tangram_decode_attention, plus INVALID_ARG for kv_len_dev == NULL. */
 #define TANGRAM_STEP_OVERLAP 1u
+/* 1 once a launch with TANGRAM_STEP_OVERLAP was accepted by the driver, 0 if it was refused (the flag is then
+ * ignored and the steps run back to back), -1 before the first such launch. */
+int tangram_overlap_state(void);
 int tangram_decode_step(const tangram_device_plan* dp, const void* q, const void* k_new, const void* v_new,
                         void* kv_pool, int64_t n_pool_pages, int32_t* kv_len_dev, const int32_t* free_pages_dev,
                         int64_t n_free, int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,

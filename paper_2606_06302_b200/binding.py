@@ -76,7 +76,8 @@ for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram
               "tangram_account_pages", "tangram_calibrate_budgets", "tangram_implicit_ratios",
               "tangram_compact_topk_chunk", "tangram_stage_from_host", "tangram_default_dynamic_tail",
               "tangram_extend_tables", "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables",
-              "tangram_decode_step", "tangram_reset_plan", "tangram_read_stream"):
+              "tangram_decode_step", "tangram_reset_plan", "tangram_read_stream", "tangram_overlap_state",
+              "tangram_decode_attention_host"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
@@ -86,13 +87,18 @@ EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragge
            "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk",
            "tangram_stage_from_host", "tangram_default_dynamic_tail", "tangram_extend_tables",
            "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables", "tangram_decode_step",
-           "tangram_reset_plan", "tangram_read_stream")
+           "tangram_reset_plan", "tangram_read_stream", "tangram_overlap_state", "tangram_decode_attention_host")
 STEP_OVERLAP = 1
 
 
 def _check(rc: int):
     if rc != OK:
         raise TangramError(rc, _lib.tangram_last_error().decode())
+
+
+def _stream_ptr(stream):
+    import torch
+    return C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
 
 
 def _np(a, dtype) -> np.ndarray:
@@ -294,6 +300,25 @@ def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, wor
     return out, lse
 
 
+def tangram_decode_attention_host(dp: DevicePlan, q_host, q_stage, kv_pool, out, lse, workspace, sm_scale: float = 0.0,
+                                  stream=None, kv_len=None):
+    """End to end with host buffers: q_host (pinned) -> q_stage (cuda) by the staging kernel, decode kernel overlapped
+    behind it; out / lse may be pinned host tensors."""
+    import torch
+    assert q_host.is_pinned() and q_stage.is_cuda and kv_pool.is_cuda and q_host.dtype == torch.bfloat16
+    assert q_host.is_contiguous() and q_stage.is_contiguous() and q_stage.shape == q_host.shape and q_stage.dtype == q_host.dtype
+    R, Hq, d = q_host.shape
+    assert tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d) and R == dp.c.R
+    assert (out.is_cuda or out.is_pinned()) and (lse.is_cuda or lse.is_pinned())
+    kvl = C.c_void_p(kv_len.data_ptr()) if kv_len is not None else None
+    _check(_lib.tangram_decode_attention_host(C.byref(dp.c), C.c_void_p(q_host.data_ptr()), C.c_void_p(q_stage.data_ptr()),
+                                              C.c_void_p(kv_pool.data_ptr()), C.c_int64(kv_pool.shape[0]), kvl, C.c_int32(Hq),
+                                              C.c_int32(d), C.c_float(sm_scale), C.c_void_p(out.data_ptr()),
+                                              C.c_void_p(lse.data_ptr()), C.c_void_p(workspace.data_ptr()),
+                                              C.c_size_t(workspace.numel()), None, _stream_ptr(stream)))
+    return out, lse
+
+
 def tangram_decode_partials(dp: DevicePlan, q, kv_pool, out=None, lse=None, workspace=None, sm_scale: float = 0.0,
                             worker_ns=None, stream=None, kv_len=None):
     """a4 alone: the split-KV decode kernel (see include/tangram.h)."""
@@ -310,11 +335,6 @@ def tangram_merge_partials(dp: DevicePlan, out, lse, workspace, stream=None):
                                        C.c_void_p(lse.data_ptr()), C.c_void_p(workspace.data_ptr()),
                                        C.c_size_t(workspace.numel()), sp))
     return out, lse
-
-
-def _stream_ptr(stream):
-    import torch
-    return C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
 
 
 def tangram_extend_tables_device(dp: DevicePlan, kv_len, free_pages, stream=None):
@@ -346,6 +366,10 @@ def tangram_read_stream(src, sink, nbytes=None, stream=None):
     """Measurement aid: one read-only pass over `src` (cuda tensor) with 16-byte loads; sink = uint32/int32[1] cuda."""
     n = src.numel() * src.element_size() if nbytes is None else nbytes
     _check(_lib.tangram_read_stream(C.c_void_p(src.data_ptr()), C.c_size_t(n), C.c_void_p(sink.data_ptr()), _stream_ptr(stream)))
+
+
+def tangram_overlap_state() -> int:
+    return int(_lib.tangram_overlap_state())
 
 
 def tangram_reset_plan(dp: DevicePlan, stream=None):

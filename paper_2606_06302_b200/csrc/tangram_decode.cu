@@ -219,6 +219,13 @@ __device__ __forceinline__ unsigned long long globaltimer() {
 // (n, G, D, thread count) only, so the result is deterministic.
 constexpr int kMergeThreads = 512;
 constexpr int kMergeBigParts = 32;
+#ifndef TANGRAM_MERGE_BATCH
+#define TANGRAM_MERGE_BATCH 8
+#endif
+constexpr int kMergeBatch = TANGRAM_MERGE_BATCH;  // partial rows a thread of the small-record merge keeps in flight
+#ifndef TANGRAM_BARRIER_NANOSLEEP
+#define TANGRAM_BARRIER_NANOSLEEP 32
+#endif
 
 struct MergeUnit {
     int seq, p0, n, g;  // g < 0: all query heads of the group (small record)
@@ -381,6 +388,7 @@ template <int D>
 __device__ __forceinline__ void merge_small(const int4 rec, int G, const float* __restrict__ part_o,
                                             const float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
                                             float* __restrict__ lse, int e4) {
+    constexpr int kB = kMergeBatch;  // loads in flight per thread
     const int n = rec.z, g = e4 / (D / 4), c4 = e4 % (D / 4);
     const size_t row = static_cast<size_t>(rec.x) * G + g;
     if (n == 0) {
@@ -392,23 +400,23 @@ __device__ __forceinline__ void merge_small(const int4 rec, int G, const float* 
     const float* po = part_o + (static_cast<size_t>(rec.y) * G + g) * D + c4 * 4;
     const size_t stride = static_cast<size_t>(G) * D;
     float m = -INFINITY, tot = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-    for (int i = 0; i < n; i += 8) {
-        float4 v[8];
-        float w[8];
+    for (int i = 0; i < n; i += kB) {
+        float4 v[kB];
+        float w[kB];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
+        for (int u = 0; u < kB; ++u) {
             const int ic = i + u < n ? i + u : i;
             v[u] = __ldcg(reinterpret_cast<const float4*>(po + ic * stride));
             w[u] = i + u < n ? __ldcg(pl + ic * G) : -INFINITY;
         }
         float m_new = m;
 #pragma unroll
-        for (int u = 0; u < 8; ++u) m_new = fmaxf(m_new, w[u]);
+        for (int u = 0; u < kB; ++u) m_new = fmaxf(m_new, w[u]);
         const float resc = m_new == -INFINITY ? 1.f : __expf(m - m_new);
         tot *= resc, a0 *= resc, a1 *= resc, a2 *= resc, a3 *= resc;
         m = m_new;
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
+        for (int u = 0; u < kB; ++u) {
             const float e = m == -INFINITY ? 0.f : __expf(w[u] - m);  // parts of an open-ended plan may be empty
             tot += e, a0 += e * v[u].x, a1 += e * v[u].y, a2 += e * v[u].z, a3 += e * v[u].w;
         }
@@ -919,7 +927,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             int seen;
             do {
                 asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
-                if (seen < grid_all) __nanosleep(32);
+                if (TANGRAM_BARRIER_NANOSLEEP > 0 && seen < grid_all) __nanosleep(TANGRAM_BARRIER_NANOSLEEP);
             } while (seen < grid_all);
             __threadfence();
         }
@@ -987,6 +995,7 @@ tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
 // transfer and its stream hand-off to the next kernel.
 __global__ void __launch_bounds__(256)
 tangram_stage_kernel(uint4* __restrict__ dst, const uint4* __restrict__ src, size_t n16) {
+    asm volatile("griddepcontrol.launch_dependents;");  // a dependent decode kernel may start its prologue now
     for (size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n16;
          i += static_cast<size_t>(gridDim.x) * blockDim.x)
         dst[i] = src[i];
@@ -1051,6 +1060,10 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
     return TANGRAM_OK;
 }
 
+// -1: TANGRAM_STEP_OVERLAP not tried yet; 1: the driver took programmatic stream serialization next to the
+// cooperative attribute; 0: it refused (the flag is then ignored)
+static int g_overlap_state = -1;
+
 // CTAs of the decode kernel that can be co-resident on the current device (SMs x occupancy).
 template <int D, bool TIMED>
 static int max_coresident(int dev, int smem) {
@@ -1088,14 +1101,16 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     // Programmatic dependent launch next to the cooperative attribute: if the driver refuses the pair once, it is
     // not asked again (a failing launch inside a stream capture would invalidate the capture).
-    static int pdl_refused = 0;
-    if (pdl_refused) prm.pdl = 0;
+    if (g_overlap_state == 0) prm.pdl = 0;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
     e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
-    if (e != cudaSuccess && prm.pdl) {
-        (void)cudaGetLastError();
-        pdl_refused = 1, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
-        e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+    if (prm.pdl) {
+        if (e == cudaSuccess) g_overlap_state = 1;
+        else {
+            (void)cudaGetLastError();
+            g_overlap_state = 0, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
+            e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+        }
     }
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
     return TANGRAM_OK;
@@ -1358,6 +1373,8 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     return TANGRAM_OK;
 }
 
+extern "C" int tangram_overlap_state(void) { return g_overlap_state; }
+
 extern "C" int tangram_reset_plan(const tangram_device_plan* dp, void* stream) {
     if (!dp || !dp->sched) return fail(TANGRAM_ERR_INVALID_ARG, "reset_plan: NULL argument");
     const cudaError_t e = cudaMemsetAsync(dp->sched, 0, 16, static_cast<cudaStream_t>(stream));
@@ -1446,8 +1463,8 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
         prm.pool_w = static_cast<uint4*>(const_cast<void*>(kv_pool));
         prm.seq_cap = dp->seq_cap, prm.kv_len_w = step.kv_len_w;
         prm.grow = grow_params(dp, step.kv_len_w, step.free_pages, step.n_free, step.overflow);
-        prm.pdl = (step.flags & TANGRAM_STEP_OVERLAP) ? 1 : 0;
     }
+    prm.pdl = (step.flags & TANGRAM_STEP_OVERLAP) ? 1 : 0;
 
     if (d == 256) prm.n_stages = Smem<256>::max_stages(G), prm.n_qslots = Smem<256>::max_qslots(prm.n_stages, G);
     else if (d == 128) prm.n_stages = Smem<128>::max_stages(G), prm.n_qslots = Smem<128>::max_qslots(prm.n_stages, G);
@@ -1586,6 +1603,20 @@ extern "C" int tangram_read_stream(const void* src_dev, size_t bytes, uint32_t* 
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "read_stream launch");
     return TANGRAM_OK;
+}
+
+extern "C" int tangram_decode_attention_host(const tangram_device_plan* dp, const void* q_host, void* q_stage_dev,
+                                             const void* kv_pool, int64_t n_pool_pages, const int32_t* kv_len_dev,
+                                             int32_t Hq, int32_t d, float sm_scale, void* out, float* lse, void* workspace,
+                                             size_t workspace_bytes, uint64_t* worker_ns, void* stream) {
+    if (!dp || !q_host || !q_stage_dev || Hq < 1 || d < 1)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_host: NULL argument");
+    const int rc = tangram_stage_from_host(q_stage_dev, q_host, (size_t)dp->R * Hq * d * 2, stream);
+    if (rc != TANGRAM_OK) return rc;
+    StepArgs step;
+    step.flags = TANGRAM_STEP_OVERLAP;  // the staging kernel writes q only: the decode kernel may start under it
+    return run_attention(dp, q_stage_dev, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, workspace,
+                         workspace_bytes, worker_ns, stream, kRunSplit | kRunMerge, step);
 }
 
 extern "C" int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream) {

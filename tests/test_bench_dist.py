@@ -47,3 +47,26 @@ def test_aggregate_single_rank_is_identity():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.aggregate(3.5, 7.0, 1) == (3.5, 7.0)
+
+
+def test_gpus_flag_spawns_the_ranks_itself():
+    """`bench.py --gpus 2` started bare (no torchrun): two rank processes are spawned, rendezvous over gloo, and
+    rank 0 prints the aggregate (max of the times, sum of the units) for a world of 2."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--plumbing-only"], env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    rec = json.loads(lines[0])
+    assert rec == {"plumbing_only": True, "n_gpus": 2, "ms_per_step": 2.0, "units": 300.0}
+
+
+def test_gpus_flag_must_match_the_world():
+    import subprocess
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--plumbing-only"], env=env,
+                         capture_output=True, text=True, timeout=120)
+    assert out.returncode != 0 and "WORLD_SIZE" in out.stderr
