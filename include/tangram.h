@@ -215,6 +215,7 @@ typedef struct tangram_device_plan {
     int32_t* seq_cap;             /* device [R*H]: tokens the pages of head h's row hold (row_pages x P) */
     const int32_t* plan_cover;    /* device [R*H]: largest tok_end any item of the plan has for the sequence */
     int32_t* grow_state;          /* device [4]: {free-list cursor, rows starved so far, 0, 0} */
+    int32_t* q_flags;             /* device [R*H]: staging flags of tangram_decode_attention_host (launch numbers) */
 } tangram_device_plan;
 
 /* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte
@@ -275,11 +276,13 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
  * alignment, source not page-locked), CUDA. */
 int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream);
 
-/* tangram_decode_attention with HOST buffers, end to end in one call: q_host (pinned) is pulled into q_stage_dev
- * (device, R x Hq x d bf16, 16-byte aligned) by the staging kernel, and the decode kernel is launched behind it with
- * programmatic stream serialization, so its launch, its work-list / page-id fetches and the fill of its KV tile
- * rings run while the queries cross the bus; it waits for the staged q only before its first query load.  out and
- * lse may be pinned host pointers (the kernel's stores go over the bus).  All other arguments and errors as for
+/* tangram_decode_attention with HOST buffers, end to end in ONE launch: the consumer warps of CTA b copy the query
+ * blocks b, b + grid, ... (G x d bf16 per (request, KV head)) from q_host (pinned) to q_stage_dev (device, R x Hq x d
+ * bf16, 16-byte aligned) when the CTA starts -- every block crosses the bus once, while the producer warps already
+ * stream KV tiles -- and publish a per-block flag (dp->q_flags); a producer waits for the flag of the block its item
+ * needs.  out and lse may be pinned host pointers (the kernel's stores go over the bus).  When the grid cannot be
+ * launched cooperatively (or d = 256) the staging kernel of tangram_stage_from_host runs first and the decode kernel
+ * is launched behind it with programmatic stream serialization.  All other arguments and errors as for
  * tangram_decode_attention and tangram_stage_from_host. */
 int tangram_decode_attention_host(const tangram_device_plan* dp, const void* q_host, void* q_stage_dev,
                                   const void* kv_pool, int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq,

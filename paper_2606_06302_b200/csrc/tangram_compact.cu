@@ -23,6 +23,7 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
 
 #include "tangram.h"
@@ -34,18 +35,24 @@ constexpr int kCPage = 16;           // tokens per page (the kernels are special
 constexpr int kSelBins = 2048;        // 11-bit digits
 constexpr int kSelCand = 4096;        // candidates (entries in the first digit's bin) the select kernel buffers
 constexpr int kSelLongRow = 49152;    // rows longer than this get 1024-thread CTAs, shorter ones 512 (two per SM)
+#ifndef TANGRAM_SEL_WIDE_ROWS
+#define TANGRAM_SEL_WIDE_ROWS 4
+#endif
+constexpr int kSelWideRows = TANGRAM_SEL_WIDE_ROWS;  // ... unless the batch has fewer rows than this per SM
 constexpr int kGatherThreads = 256;
 constexpr int kGatherChunk = 8;      // tiles claimed at once
 
-// Workspace (int32 words): [0] chunk counter, [1] total tiles, [2..3] pad, then keep_eff[n_seq], base[n_seq]
-// (tokens every head held before the call), then tile_indptr[n_seq + 1].
+// Workspace (int32 words): [0] chunk counter of the gather, [1] total tiles, [2] row counter of the select, [3] pad,
+// then keep_eff[n_seq], base[n_seq] (tokens every head held before the call), tile_indptr[n_seq + 1] and
+// order[n_seq] (the rows, longest context first: the select kernel's queue).
 struct CompactWs {
     int32_t* counter;
     int32_t* keep_eff;
     int32_t* base;
     int32_t* tile_indptr;
+    int32_t* order;
 };
-static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 4 + 3 * (size_t)n_seq + 1; }
+static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 4 + 4 * (size_t)n_seq + 1; }
 
 // fp32 score -> uint32 key with the same order (larger score = larger key); -0.0 and +0.0 compare equal
 // as they do as fp32 values.
@@ -58,7 +65,7 @@ __global__ void __launch_bounds__(1024)
 compact_prepare_kernel(const int32_t* __restrict__ seq_cap, const int32_t* __restrict__ ctx_len,
                        const int32_t* __restrict__ keep, int32_t* __restrict__ kv_len, int n_seq, int H,
                        int32_t* __restrict__ counter, int32_t* __restrict__ keep_eff, int32_t* __restrict__ base,
-                       int32_t* __restrict__ tile_indptr, int32_t* __restrict__ clamped) {
+                       int32_t* __restrict__ tile_indptr, int32_t* __restrict__ order, int32_t* __restrict__ clamped) {
     __shared__ int s_warp[32];
     __shared__ int s_run, s_bad;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -97,8 +104,20 @@ compact_prepare_kernel(const int32_t* __restrict__ seq_cap, const int32_t* __res
     }
     if (tid == 0) {
         tile_indptr[n_seq] = s_run;
-        counter[0] = 0, counter[1] = s_run;
+        counter[0] = 0, counter[1] = s_run, counter[2] = 0;
         if (clamped && s_bad) atomicAdd(clamped, s_bad);
+    }
+    // The select kernel's queue: requests by context length, longest first (ties: lower request first), all H rows
+    // of a request together -- longest-processing-time-first over the persistent select CTAs.
+    const int R = n_seq / H;
+    for (int r = tid; r < R; r += blockDim.x) {
+        const int n = ctx_len[r];
+        int rank = 0;
+        for (int o = 0; o < R; ++o) {
+            const int m = ctx_len[o];
+            rank += (m > n) || (m == n && o < r);
+        }
+        for (int h = 0; h < H; ++h) order[rank * H + h] = r * H + h;
     }
 }
 
@@ -191,22 +210,34 @@ __device__ __forceinline__ void radix_passes(EachKey&& each_key, int pass_begin,
     }
 }
 
-// One CTA of NT threads per (request, KV head).  (A thread-block cluster per row with the histograms
+// One (request, KV head) row by one CTA of NT threads.  (A thread-block cluster per row with the histograms
 // exchanged through distributed shared memory was measured too: the remote loads and cluster barriers cost
 // more than the extra SMs bring -- 8b 40 -> 46 us with 2 CTAs per row, 220 us with 8.)
 template <int NT>
-__global__ void __launch_bounds__(NT, 1024 / NT)
-topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len,
-                   const int32_t* __restrict__ keep_eff, int H, int32_t* __restrict__ idx_out) {
+struct SelectSmem {
+    uint32_t hist[kSelBins];
+    uint32_t wsum[NT / 32];
+    uint32_t pick[3];
+    uint32_t cnt[2][NT / 32];                   // (greater, equal) counts of the warps' segments
+    uint32_t ckey[kSelCand], cidx[kSelCand];    // candidates: entries in the first digit's bin
+    uint32_t ncand;
+    int row;                                    // the row the CTA claimed
+};
+
+template <int NT>
+__device__ __forceinline__ void select_row(SelectSmem<NT>& sm, const int seq, const float* __restrict__ scores,
+                                           int64_t n_max, const int32_t* __restrict__ ctx_len,
+                                           const int32_t* __restrict__ keep_eff, int H, int32_t* __restrict__ idx_out) {
     constexpr int kSelWarps = NT / 32;
     constexpr int kU = NT == 1024 ? 4 : 8;  // 16-byte loads in flight per thread (register budget: 64 / 32)
-    __shared__ uint32_t s_hist[kSelBins];
-    __shared__ uint32_t s_wsum[kSelWarps];
-    __shared__ uint32_t s_pick[3];
-    __shared__ uint32_t s_cnt[2][kSelWarps];  // (greater, equal) counts of the warps' segments
-    __shared__ uint32_t s_ckey[kSelCand], s_cidx[kSelCand];  // candidates: entries in the first digit's bin
-    __shared__ uint32_t s_ncand;
-    const int seq = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t* s_hist = sm.hist;
+    uint32_t* s_wsum = sm.wsum;
+    uint32_t* s_pick = sm.pick;
+    uint32_t(*s_cnt)[kSelWarps] = sm.cnt;
+    uint32_t* s_ckey = sm.ckey;
+    uint32_t* s_cidx = sm.cidx;
+    uint32_t& s_ncand = sm.ncand;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = ctx_len[seq / H];
     const int k = keep_eff[seq];
     if (k <= 0) return;
@@ -379,6 +410,26 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
     for (; v < v1; v += 32) place4(v + lane < v1 ? __ldg(sv + v + lane) : make_float4(0.f, 0.f, 0.f, 0.f), v + lane);
 }
 
+// Persistent grid: every CTA claims rows from the queue `order` (longest context first) until it is empty.  The
+// select is bound by instruction issue and latency per row, not by bandwidth, so what matters is that no SM ends
+// up with two long rows while another holds two short ones (round 1: one CTA per row in launch order, SM busy
+// cycles min / avg / max = 5.7 K / 45 K / 63 K on 8b).
+template <int NT>
+__global__ void __launch_bounds__(NT, 1024 / NT)
+topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len,
+                   const int32_t* __restrict__ keep_eff, int H, int n_seq, const int32_t* __restrict__ order,
+                   int32_t* __restrict__ row_counter, int32_t* __restrict__ idx_out) {
+    __shared__ SelectSmem<NT> sm;
+    for (;;) {
+        __syncthreads();  // the previous row is done with the shared state
+        if (threadIdx.x == 0) sm.row = atomicAdd(row_counter, 1);
+        __syncthreads();
+        const int slot = sm.row;
+        if (slot >= n_seq) return;
+        select_row<NT>(sm, order[slot], scores, n_max, ctx_len, keep_eff, H, idx_out);
+    }
+}
+
 // NEXT-4: implicit per-head retention ratios of the global flat Top-k (Eq. 3; what Budget
 // Calibration records on every sample, :156).  One CTA per request: radix select over the flattened scores of
 // all H heads (head-major; ties to the lower flat index), then per-head counts of the entries above the
@@ -548,17 +599,29 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
         return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "compact_topk: workspace %zu < %zu bytes", workspace_bytes, need);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int32_t* ws = static_cast<int32_t*>(workspace);
-    CompactWs w{ws, ws + 4, ws + 4 + n_seq, ws + 4 + 2 * n_seq};
+    CompactWs w{ws, ws + 4, ws + 4 + n_seq, ws + 4 + 2 * n_seq, ws + 4 + 3 * n_seq + 1};
     const int4* seq_info = reinterpret_cast<const int4*>(dp->seq_info);
 
     compact_prepare_kernel<<<1, 1024, 0, st>>>(dp->seq_cap, ctx_len_dev, keep_dev, kv_len_dev, n_seq, dp->H, w.counter,
-                                               w.keep_eff, w.base, w.tile_indptr, clamped_dev);
+                                               w.keep_eff, w.base, w.tile_indptr, w.order, clamped_dev);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
-    if (n_max > kSelLongRow)
-        topk_select_kernel<1024><<<n_seq, 1024, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
+    // Persistent select grid fed longest-row-first.  Few rows per SM (or very long rows): one 1024-thread CTA per SM,
+    // so that a row gets a whole SM and the queue can even out the SMs; many short rows: two 512-thread CTAs per SM.
+    static thread_local int sms_dev = -1, sms = 0;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail2(e, "cudaGetDevice");
+    if (dev != sms_dev) {
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+            return cuda_fail2(e, "cudaDeviceGetAttribute");
+        sms_dev = dev;
+    }
+    if (n_max > kSelLongRow || n_seq <= kSelWideRows * sms)
+        topk_select_kernel<1024><<<std::min(n_seq, sms), 1024, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, n_seq,
+                                                                       w.order, w.counter + 2, idx_out);
     else
-        topk_select_kernel<512><<<n_seq, 512, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, idx_out);
+        topk_select_kernel<512><<<std::min(n_seq, 2 * sms), 512, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, n_seq,
+                                                                         w.order, w.counter + 2, idx_out);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "top-k select launch");
     const uint4* kd = static_cast<const uint4*>(k_dense);
@@ -577,7 +640,8 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
                                                 w.counter, w.keep_eff, w.base, w.tile_indptr);
         return cudaSuccess;
     };
-    static thread_local int grid256 = 0, grid128 = 0, grid64 = 0;
+    static thread_local int grid_dev = -1, grid256 = 0, grid128 = 0, grid64 = 0;  // cached per (thread, device)
+    if (grid_dev != dev) grid_dev = dev, grid256 = grid128 = grid64 = 0;
     if (d == 256) e = gather(compact_gather_kernel<256>, grid256);
     else if (d == 128) e = gather(compact_gather_kernel<128>, grid128);
     else e = gather(compact_gather_kernel<64>, grid64);

@@ -78,11 +78,12 @@ struct DecodeParams {
     float* part_lse;
     unsigned long long* worker_ns;
     int* sched;  // [0] next list to claim (relative to gridDim.x), [1] CTAs done claiming, [2] grid-barrier
-                 // arrivals, [3] CTAs done merging; all 0 between launches (the kernel re-arms them)
+                 // arrivals, [3] CTAs done merging; all 0 between launches (the kernel re-arms them);
+                 // [4] launches that staged host queries on this plan (the epoch of q_flags)
     const int32_t* merge_recs;  // merge records (see a5)
     const void* list_heads;     // [n_lists] 128-byte list heads
     const int32_t* kv_len;      // [R*H] run-time lengths (open-ended plan) or nullptr: items are taken as planned
-    int32_t H;
+    int32_t H, R;
     int32_t Hq, G, Hp, n_stages, n_qslots, n_lists;
     int32_t tail_merge, n_merge_units, n_merge_small, merge_split;
     float scale_log2;
@@ -95,6 +96,11 @@ struct DecodeParams {
     int32_t* kv_len_w;           // = kv_len, writable
     GrowParams grow;
     int32_t pdl;                 // launched with programmatic stream serialization: wait before reading q / k_new / v_new
+    // host-resident queries (tangram_decode_attention_host, cooperative launch only): the consumer warps of CTA b
+    // copy query blocks b, b + grid, ... from pinned host memory to `q` (device) when the CTA starts and publish each
+    // block's flag; a producer waits for the flag of the block its item needs.  nullptr otherwise.
+    const uint4* q_host;
+    int32_t* q_flags;            // [R*H] launch number (epoch) in which the block was staged last
 };
 
 // ------------------------------------------------------------------ shared-memory carve-up
@@ -652,6 +658,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             asm volatile("griddepcontrol.wait;" ::: "memory");
         }
         asm volatile("griddepcontrol.launch_dependents;");  // the next launch on the stream may be scheduled
+        const int q_epoch = p.q_host ? __ldcg(p.sched + 4) + 1 : 0;
         int seq = 0;  // running item number = position in the item / query ring
         for (;;) {
             int fut = 0;
@@ -688,6 +695,14 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 if (lane == 0) {
                     mbar_wait(qempty_bar(qs), qpar ^ 1);
                     *reinterpret_cast<DeviceItem*>(desc_ring + qs * 32) = item;
+                    if (p.q_host) {  // the item's query block is staged by some CTA's consumer warps: wait for its flag
+                        const int32_t* flag = p.q_flags + item.req * p.H + item.kv_head;
+                        int seen;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(flag) : "memory");
+                        } while (seen != q_epoch);
+                        asm volatile("fence.proxy.async;" ::: "memory");  // generic-proxy stores -> bulk (async proxy) read
+                    }
                     const uint32_t qbytes = static_cast<uint32_t>(G * D * 2);
                     mbar_arrive_expect_tx(qfull_bar(qs), qbytes);
                     bulk_load(smem_u32(q_ring + qs * q_slot_bytes),
@@ -754,6 +769,21 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     }
 
     // ================================ consumer warps ================================
+    if (p.q_host) {
+        // Queries in pinned host memory: this CTA's share of the R*H query blocks (G x d bf16 each) crosses the bus
+        // once, now, while the producer already streams KV tiles; sched[4] counts the launches on this plan.
+        const int epoch = __ldcg(p.sched + 4) + 1;
+        const int n_blocks = p.R * p.H, v16 = G * D / 8;  // 16-byte words per block
+        for (int blk = static_cast<int>(blockIdx.x) + warp * static_cast<int>(gridDim.x); blk < n_blocks;
+             blk += kNW * static_cast<int>(gridDim.x)) {
+            const uint4* src = p.q_host + static_cast<size_t>(blk) * v16;
+            uint4* dst = reinterpret_cast<uint4*>(const_cast<__nv_bfloat16*>(p.q)) + static_cast<size_t>(blk) * v16;
+            for (int i = lane; i < v16; i += 32) dst[i] = src[i];
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.q_flags + blk), "r"(epoch) : "memory");
+        }
+    }
     const int row = lane >> 2;  // query head inside the GQA group held by this quad (valid if < G)
     const int qd = lane & 3;
     const bool row_ok = row < G;
@@ -952,8 +982,10 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             if (p.grow.free_pages) extend_rows<kNW * 32, true>(p.grow, kPage, threadIdx.x, reinterpret_cast<int*>(scratch_o));
         }
         if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
-        if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == grid_all - 1)
+        if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == grid_all - 1) {
             p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
+            if (p.q_host) p.sched[4] += 1;   // ... and closes this launch's query-staging epoch
+        }
     }
 }
 
@@ -1092,6 +1124,13 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     // (at d = 256 the grid has 128 consumer threads per CTA, fewer than a merge record has elements: stand-alone kernel)
     prm.tail_merge = want_tail_merge && D <= 128 && dp->n_static <= cached_max;
     *merged = prm.tail_merge;
+    if (prm.q_host && !prm.tail_merge) {
+        // no co-resident grid, no in-kernel staging: the staging kernel runs first and the decode kernel is
+        // launched behind it with programmatic stream serialization (it waits before its first query load)
+        const int rc = tangram_stage_from_host(const_cast<__nv_bfloat16*>(prm.q), prm.q_host, (size_t)prm.R * prm.Hq * D * 2, stream);
+        if (rc != TANGRAM_OK) return rc;
+        prm.q_host = nullptr, prm.pdl = 1;
+    }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(Smem<D>::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
     cudaLaunchAttribute attr[2];
@@ -1142,7 +1181,7 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
     bool merged = false;
     if (which & kRunSplit) {
         // a fused step always wants the tail phase (lengths + table growth), even with nothing to merge
-        const bool want = (which & kRunMerge) && (n_units > 0 || fused);
+        const bool want = (which & kRunMerge) && (n_units > 0 || fused || prm.q_host);
         const int rc = prm.worker_ns ? launch_split<D, true>(dp, prm, map, stream, want, &merged)
                                      : launch_split<D, false>(dp, prm, map, stream, want, &merged);
         if (rc != TANGRAM_OK) return rc;
@@ -1203,7 +1242,7 @@ extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa,
 // Blob layout (all sections 256-byte aligned), shared by tangram_blob_bytes and tangram_upload.
 namespace {
 struct BlobLayout {
-    size_t items, windptr, pindptr, pages, mseq, heads, seqinfo, row_ptr, row_pages, perm, seq_cap, cover, grow, sched, total;
+    size_t items, windptr, pindptr, pages, mseq, heads, seqinfo, row_ptr, row_pages, perm, seq_cap, cover, q_flags, grow, sched, total;
 };
 int64_t table_slots(const tangram_tables* t) {
     return t->tbl_indptr ? t->tbl_indptr[(int64_t)t->R * t->C] : t->n_pages_used;
@@ -1229,8 +1268,9 @@ BlobLayout blob_layout(const tangram_tables* t, const tangram_plan* p) {
     b.perm = take(sizeof(int32_t) * (size_t)t->H);
     b.seq_cap = take(sizeof(int32_t) * n_seq);
     b.cover = take(sizeof(int32_t) * n_seq);
+    b.q_flags = take(sizeof(int32_t) * n_seq);
     b.grow = take(16);
-    b.sched = take(16);
+    b.sched = take(32);
     b.total = off + 256;
     return b;
 }
@@ -1370,6 +1410,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->seq_cap = reinterpret_cast<int32_t*>(base + lay.seq_cap);
     dp->plan_cover = reinterpret_cast<const int32_t*>(base + lay.cover);
     dp->grow_state = reinterpret_cast<int32_t*>(base + lay.grow);
+    dp->q_flags = reinterpret_cast<int32_t*>(base + lay.q_flags);
     return TANGRAM_OK;
 }
 
@@ -1377,7 +1418,9 @@ extern "C" int tangram_overlap_state(void) { return g_overlap_state; }
 
 extern "C" int tangram_reset_plan(const tangram_device_plan* dp, void* stream) {
     if (!dp || !dp->sched) return fail(TANGRAM_ERR_INVALID_ARG, "reset_plan: NULL argument");
-    const cudaError_t e = cudaMemsetAsync(dp->sched, 0, 16, static_cast<cudaStream_t>(stream));
+    cudaError_t e = cudaMemsetAsync(dp->sched, 0, 32, static_cast<cudaStream_t>(stream));
+    if (e == cudaSuccess && dp->q_flags)
+        e = cudaMemsetAsync(dp->q_flags, 0, sizeof(int32_t) * (size_t)dp->R * dp->H, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "reset_plan: cudaMemsetAsync");
     return TANGRAM_OK;
 }
@@ -1407,6 +1450,7 @@ struct StepArgs {
     int64_t n_free = 0;
     int32_t* overflow = nullptr;
     uint32_t flags = 0;
+    const void* q_host = nullptr;  // queries in pinned host memory, staged into q (device) by the kernel itself
 };
 
 static int run_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool, int64_t n_pool_pages,
@@ -1457,7 +1501,8 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.n_lists = dp->W;
     prm.list_heads = dp->list_heads;
     prm.sched = dp->sched;
-    prm.kv_len = kv_len_dev, prm.H = dp->H;
+    prm.kv_len = kv_len_dev, prm.H = dp->H, prm.R = dp->R;
+    prm.q_host = static_cast<const uint4*>(step.q_host), prm.q_flags = dp->q_flags;
     if (step.k_new) {
         prm.k_new = static_cast<const uint4*>(step.k_new), prm.v_new = static_cast<const uint4*>(step.v_new);
         prm.pool_w = static_cast<uint4*>(const_cast<void*>(kv_pool));
@@ -1611,10 +1656,15 @@ extern "C" int tangram_decode_attention_host(const tangram_device_plan* dp, cons
                                              size_t workspace_bytes, uint64_t* worker_ns, void* stream) {
     if (!dp || !q_host || !q_stage_dev || Hq < 1 || d < 1)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_host: NULL argument");
-    const int rc = tangram_stage_from_host(q_stage_dev, q_host, (size_t)dp->R * Hq * d * 2, stream);
-    if (rc != TANGRAM_OK) return rc;
+    if (reinterpret_cast<uintptr_t>(q_host) % 16) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_host: misaligned q_host");
+    cudaPointerAttributes at;
+    const cudaError_t e = cudaPointerGetAttributes(&at, q_host);
+    if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged && at.type != cudaMemoryTypeDevice)) {
+        (void)cudaGetLastError();
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_host: q_host is not page-locked (device-mapped) memory");
+    }
     StepArgs step;
-    step.flags = TANGRAM_STEP_OVERLAP;  // the staging kernel writes q only: the decode kernel may start under it
+    step.q_host = q_host;
     return run_attention(dp, q_stage_dev, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, workspace,
                          workspace_bytes, worker_ns, stream, kRunSplit | kRunMerge, step);
 }

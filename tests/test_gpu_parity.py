@@ -721,3 +721,38 @@ def test_full_size_constant_v_per_head_is_exact(name):
     want = (torch.arange(wl.Hq, device="cuda") // wl.G + 1).to(torch.bfloat16)[None, :, None].expand(wl.R, wl.Hq, wl.d)
     assert torch.equal(out, want), f"{name}: {int((out != want).sum())} output elements differ from floor(j/G)+1"
     assert torch.isfinite(lse).all()
+
+
+@pytest.mark.parametrize("d,W", [(128, None), (64, None), (128, 200), (256, None)])
+def test_decode_attention_host_entry(d, W):
+    """tangram_decode_attention_host: q in pinned host memory staged by the decode kernel itself (per-block flags,
+    cooperative grid) or, when the grid cannot be co-resident (W = 200) or d = 256, by the staging kernel with the
+    decode kernel overlapped behind it; out / lse in pinned host memory.  Same bits as the device-resident call,
+    launch after launch (the staging epoch advances), also after a device-resident launch in between and with a
+    different q every time; within tolerance of the oracle."""
+    wl = I.make_random_workload(600 + d, R=5, H=4, G=4 if d != 256 else 2, d=d, C=2, max_ctx=3000)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    W = W or n_cta(wl)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, 300, 3)
+    dp = T.tangram_upload(t, pl)
+    ws = torch.empty(T.tangram_workspace_bytes(pl.n_part_slots, wl.G, wl.d), dtype=torch.uint8, device="cuda")
+    q_stage = torch.zeros_like(q)
+    out_h = torch.zeros(q.shape, dtype=torch.bfloat16).pin_memory()
+    lse_h = torch.zeros(wl.R, wl.Hq, dtype=torch.float32).pin_memory()
+    g = torch.Generator(device="cuda").manual_seed(3)
+    for rep in range(4):
+        q_new = torch.randn(q.shape, generator=g, device="cuda").bfloat16()
+        out_d, lse_d = T.tangram_decode_attention(dp, q_new, pool)              # device-resident launch in between
+        q_h = q_new.cpu().pin_memory()
+        q_stage.fill_(float("nan"))
+        T.tangram_decode_attention_host(dp, q_h, q_stage, pool, out_h, lse_h, ws)
+        torch.cuda.synchronize()
+        assert torch.equal(q_stage, q_new)
+        assert torch.equal(out_h, out_d.cpu()) and torch.equal(lse_h, lse_d.cpu()), f"rep {rep}"
+    ref_out, ref_lse, _ = O.attention(q_new.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    check(out_h, lse_h, ref_out, ref_lse, "host entry point")
+    T.tangram_reset_plan(dp)                                                    # recovery call: state zeroed, still correct
+    T.tangram_decode_attention_host(dp, q_h, q_stage, pool, out_h, lse_h, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(out_h, out_d.cpu())
