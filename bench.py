@@ -501,21 +501,35 @@ def page_accounting_summary(T, I, name):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def spread_of(T, S, torch, reps=5):
+def spread_of(T, S, torch, reps=5, detail=False):
     """Per-CTA elapsed-time spread (max - min) / mean of the worker CTAs' busy time, from the
-    globaltimer stamps of the instrumented build (median over reps)."""
+    globaltimer stamps of the instrumented build (median over reps).  detail=True also returns the quantiles of the
+    busy times (us), the spread of the bytes the plan assigned to the CTAs' own lists, and how stable the ranking of
+    fast and slow CTAs (= SMs: one CTA per SM) is from launch to launch (correlation of the busy times)."""
     W = S["plan"].n_static
     ns = torch.zeros(W, 4, dtype=torch.int64, device=S["q"].device)
     dp = S["dp"]
-    vals = []
+    vals, runs = [], []
+    live = np.diff(S["plan"].worker_indptr)[:W] > 0
     for _ in range(reps):
         T.tangram_decode_partials(dp, S["q"], S["pool"], S["out"], S["lse"], S["ws"], worker_ns=ns)
         torch.cuda.synchronize()
         a = ns.cpu().numpy().astype(np.float64)
-        busy = a[:, 1] - a[:, 0]
-        busy = busy[np.diff(S["plan"].worker_indptr)[:W] > 0]
+        busy = (a[:, 1] - a[:, 0])[live]
+        runs.append(busy)
         vals.append(float((busy.max() - busy.min()) / busy.mean()))
-    return float(np.median(vals))
+    if not detail:
+        return float(np.median(vals))
+    b = runs[-1] / 1e3
+    items, wi = S["plan"].items, S["plan"].worker_indptr
+    own = np.array([int((items[wi[k]:wi[k + 1], 5] - items[wi[k]:wi[k + 1], 4]).sum()) for k in range(W)], dtype=np.float64)[live]
+    corr = [float(np.corrcoef(runs[i], runs[i + 1])[0, 1]) for i in range(len(runs) - 1)] if b.size > 2 else []
+    return float(np.median(vals)), {
+        "busy_us": {"min": float(b.min()), "p10": float(np.percentile(b, 10)), "median": float(np.median(b)),
+                    "p90": float(np.percentile(b, 90)), "max": float(b.max())},
+        "own_list_tokens_spread": float((own.max() - own.min()) / own.mean()) if own.size else 0.0,
+        "busy_vs_own_tokens_corr": float(np.corrcoef(b, own)[0, 1]) if b.size > 2 and own.std() > 0 else None,
+        "launch_to_launch_corr": corr}
 
 
 def prepare(T, S, torch):
@@ -564,6 +578,8 @@ def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, co
             res[key] = {"us_per_layer_step": float(np.median(m2) * 1e3), "items": int(S2["plan"].n_items),
                         "split_map": S2["plan"].split_map.tolist(), "cta_spread": spread_of(T, S2, torch, 3),
                         "slowdown_vs_balanced": float(np.median(m2) * 1e3) / us}
+            if key == "balanced_static":  # the evidence behind the dynamic tail: equal bytes per CTA != equal time
+                res[key]["cta_spread"], res[key]["per_cta"] = spread_of(T, S2, torch, 4, detail=True)
     return S, res, ms, kms
 
 
@@ -696,6 +712,8 @@ def main():
     ap.add_argument("--dyn-rounds", type=int, default=None)
     ap.add_argument("--decode-loop-layers", type=int, default=8,
                     help="layers of the multi-layer decode loop summary (0 = skip)")
+    ap.add_argument("--decode-loop-only", action="store_true",
+                    help="after the timed steps run only the multi-layer decode loop summary (short runs under ncu)")
     ap.add_argument("--plumbing-only", action="store_true",
                     help="exercise only the multi-rank plumbing (spawn, rendezvous, barrier, aggregation) on CPU / gloo")
     args = ap.parse_args()
@@ -809,6 +827,12 @@ def main():
     }
     line["cta_spread"] = spread_of(T, S, torch)
     line["config"]["cta_spread"] = round(line["cta_spread"], 4)
+    if args.decode_loop_only and world == 1:
+        del S
+        torch.cuda.empty_cache()
+        line["decode_loop"] = decode_loop(T, I, args.workload, device, args.decode_loop_layers or 2, 12, torch)
+        print(json.dumps(line))
+        return
     if not args.no_sweep and world == 1:
         per = {}
         del S

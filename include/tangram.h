@@ -177,7 +177,7 @@ int tangram_default_dynamic_tail(const int32_t* kv_len, int32_t R, int32_t H, in
 
 /* N_CTA of :252 ("CUDAMaxOccupancy API ... CTAs the GPU can execute concurrently for the attention
  * kernel") = SM count x resident CTAs per SM of the decode kernel for this head_dim / GQA group.
- * Needs a CUDA device.  head_dim in {64, 128, 256}, 1 <= gqa <= 8. */
+ * Needs a CUDA device.  head_dim in {64, 128, 256}, 1 <= gqa <= 16 (<= 8 at head_dim 256). */
 int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa, int32_t* n_cta_out);
 
 /* Bytes of the device blob that tangram_upload fills for these tables + plan. */
@@ -245,7 +245,7 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *             plan built once for lengths >= the run-time ones (e.g. the tables' capacity) serves every
  *             decode step while tangram_append_kv grows the cache; items beyond the current length are
  *             empty and a head with length 0 yields out = 0, lse = -inf.
- *   Hq        query heads, Hq % H == 0, G = Hq / H <= 8 (query head j uses KV head floor(j / G))
+ *   Hq        query heads, Hq % H == 0, G = Hq / H <= 16 (<= 8 at d = 256; query head j uses KV head floor(j / G))
  *   d         64, 128 or 256;  P must be 16
  *   sm_scale  softmax scale; 0 means 1/sqrt(d)
  *   out       device [R][Hq][d] bf16;  lse device [R][Hq] f32 (natural log of sum exp(scaled score);

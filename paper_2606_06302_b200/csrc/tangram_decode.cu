@@ -44,7 +44,7 @@ constexpr int kMinQSlots = 2;      // item / query ring depth: as deep as shared
 constexpr int kMaxQSlots = 8;      // ring lets the producer fetch query groups several items ahead, which is what hides
                                    // the bus round trip when q lives in pinned host memory
 constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime <= this)
-constexpr int kMaxG = 8;
+constexpr int kMaxG = 16;         // GQA groups above 8 use both halves of the 16-row A operand (d <= 128)
 constexpr int kSmemLimit = 232448; // 227 KB opt-in limit per CTA
 constexpr int kRunSplit = 1, kRunMerge = 2;
 #ifndef TANGRAM_CLAIM_TILES
@@ -198,6 +198,13 @@ __device__ __forceinline__ void mma_rows07(float& c0, float& c1, uint32_t a0, ui
         : "+f"(c0), "+f"(c1), "=f"(d2), "=f"(d3)
         : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1), "f"(0.f));
     (void)d2, (void)d3;
+}
+// The full 16-row form (GQA groups of 9..16 query heads): rows 0..7 accumulate into (c0, c1), rows 8..15 into (c2, c3).
+__device__ __forceinline__ void mma_rows16(float& c0, float& c1, float& c2, float& c3, uint32_t a0, uint32_t a1, uint32_t a2,
+                                           uint32_t a3, uint32_t b0, uint32_t b1) {
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c0), "+f"(c1), "+f"(c2), "+f"(c3)
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     uint32_t r;
@@ -528,7 +535,7 @@ __global__ void __launch_bounds__(1024) tangram_grow_kernel(const GrowParams g, 
 }
 
 // ------------------------------------------------------------------ a4: split-KV decode kernel
-template <int D, bool TIMED>
+template <int D, bool TIMED, int NH>
 __global__ void __launch_bounds__(Smem<D>::kThreads, 1)
 tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeParams p) {
     using L = Smem<D>;
@@ -774,19 +781,31 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         // once, now, while the producer already streams KV tiles; sched[4] counts the launches on this plan.
         const int epoch = __ldcg(p.sched + 4) + 1;
         const int n_blocks = p.R * p.H, v16 = G * D / 8;  // 16-byte words per block
-        for (int blk = static_cast<int>(blockIdx.x) + warp * static_cast<int>(gridDim.x); blk < n_blocks;
-             blk += kNW * static_cast<int>(gridDim.x)) {
+        auto stage = [&](int blk) {
             const uint4* src = p.q_host + static_cast<size_t>(blk) * v16;
             uint4* dst = reinterpret_cast<uint4*>(const_cast<__nv_bfloat16*>(p.q)) + static_cast<size_t>(blk) * v16;
             for (int i = lane; i < v16; i += 32) dst[i] = src[i];
             __threadfence();
             __syncwarp();
             if (lane == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.q_flags + blk), "r"(epoch) : "memory");
+        };
+        if (warp == kNW - 1) {
+            // the block this CTA's own first item needs goes first (several CTAs may fetch the same block: harmless),
+            // so that no CTA's start waits behind the whole batch on the bus
+            const int* hd = reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(blockIdx.x) * 32;
+            if (__ldg(hd + 1) > 0) stage(__ldg(hd + 4) * p.H + __ldg(hd + 5));
         }
+        for (int blk = static_cast<int>(blockIdx.x) + warp * static_cast<int>(gridDim.x); blk < n_blocks;
+             blk += kNW * static_cast<int>(gridDim.x))
+            stage(blk);
     }
-    const int row = lane >> 2;  // query head inside the GQA group held by this quad (valid if < G)
+    // Query head `row + 8 hf` of the GQA group is held by this quad in half hf of the 16-row A operand: NH = 1 uses
+    // rows 0..7 only (G <= 8: the upper rows are fed zeros and their accumulators dropped), NH = 2 all sixteen.
+    const int row = lane >> 2;
     const int qd = lane & 3;
-    const bool row_ok = row < G;
+    bool row_ok[NH];
+#pragma unroll
+    for (int hf = 0; hf < NH; ++hf) row_ok[hf] = row + 8 * hf < G;
     uint32_t stage = 0, phase = 0;
     constexpr float kNegInf = -INFINITY;
 
@@ -795,13 +814,14 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         mbar_wait(qfull_bar(qs), (it / NQ) & 1);
         const DeviceItem item = *reinterpret_cast<const DeviceItem*>(desc_ring + qs * 32);
         if (item.n_parts < 0) break;  // producer's end-of-work sentinel
-        uint32_t qa[D / 16][2];
-        {
-            const uint8_t* qrow = q_ring + qs * q_slot_bytes + row * D * 2;
+        uint32_t qa[NH][D / 16][2];
+#pragma unroll
+        for (int hf = 0; hf < NH; ++hf) {
+            const uint8_t* qrow = q_ring + qs * q_slot_bytes + (row + 8 * hf) * D * 2;
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
-                qa[ks][0] = row_ok ? *reinterpret_cast<const uint32_t*>(qrow + (ks * 16 + qd * 2) * 2) : 0u;
-                qa[ks][1] = row_ok ? *reinterpret_cast<const uint32_t*>(qrow + (ks * 16 + 8 + qd * 2) * 2) : 0u;
+                qa[hf][ks][0] = row_ok[hf] ? *reinterpret_cast<const uint32_t*>(qrow + (ks * 16 + qd * 2) * 2) : 0u;
+                qa[hf][ks][1] = row_ok[hf] ? *reinterpret_cast<const uint32_t*>(qrow + (ks * 16 + 8 + qd * 2) * 2) : 0u;
             }
         }
         __syncwarp();
@@ -810,10 +830,14 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         const int n_tok = max(0, item.tok_end - item.tok_begin);  // 0: an open-ended item beyond the current length
         const int n_tiles = (n_tok + kPage - 1) / kPage;
         const int rot = item.part_slot & (kNW - 1);  // a function of the item only: results do not depend on which CTA runs it
-        float m = kNegInf, l = 0.f;
-        float o[D / 8][2];
+        float m[NH], l[NH];
+        float o[NH][D / 8][2];
 #pragma unroll
-        for (int nt = 0; nt < D / 8; ++nt) o[nt][0] = o[nt][1] = 0.f;
+        for (int hf = 0; hf < NH; ++hf) {
+            m[hf] = kNegInf, l[hf] = 0.f;
+#pragma unroll
+            for (int nt = 0; nt < D / 8; ++nt) o[hf][nt][0] = o[hf][nt][1] = 0.f;
+        }
 
         for (int i = (warp - rot) & (kNW - 1); i < n_tiles; i += kNW) {
             mbar_wait(full_bar(warp, stage), phase);
@@ -830,8 +854,10 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                                      : "memory");
                 __syncwarp();
             }
-            // ---- S = Q K^T : 16 (8 used) query rows x 16 tokens
-            float s[2][2] = {{0.f, 0.f}, {0.f, 0.f}};
+            // ---- S = Q K^T : 16 query rows (8 or 16 used) x 16 tokens
+            float s[NH][2][2];
+#pragma unroll
+            for (int hf = 0; hf < NH; ++hf) s[hf][0][0] = s[hf][0][1] = s[hf][1][0] = s[hf][1][1] = 0.f;
             {
                 const int tok = ((lane >> 4) << 3) + (lane & 7);
                 const uint32_t rbase = tb + tok * 128;
@@ -840,34 +866,54 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     const int ck = ((ks & 3) << 1) + ((lane >> 3) & 1);
                     uint32_t b0, b1, b2, b3;
                     ldsm_x4(rbase + (ks >> 2) * kHalf + ((ck ^ (tok & 7)) << 4), b0, b1, b2, b3);
-                    mma_rows07(s[0][0], s[0][1], qa[ks][0], qa[ks][1], b0, b1);
-                    mma_rows07(s[1][0], s[1][1], qa[ks][0], qa[ks][1], b2, b3);
+                    if constexpr (NH == 1) {
+                        mma_rows07(s[0][0][0], s[0][0][1], qa[0][ks][0], qa[0][ks][1], b0, b1);
+                        mma_rows07(s[0][1][0], s[0][1][1], qa[0][ks][0], qa[0][ks][1], b2, b3);
+                    } else {
+                        mma_rows16(s[0][0][0], s[0][0][1], s[NH - 1][0][0], s[NH - 1][0][1], qa[0][ks][0], qa[NH - 1][ks][0],
+                                   qa[0][ks][1], qa[NH - 1][ks][1], b0, b1);
+                        mma_rows16(s[0][1][0], s[0][1][1], s[NH - 1][1][0], s[NH - 1][1][1], qa[0][ks][0], qa[NH - 1][ks][0],
+                                   qa[0][ks][1], qa[NH - 1][ks][1], b2, b3);
+                    }
                 }
             }
             // ---- online softmax (exp2 domain)
-            float tmax = kNegInf;
+            float m_new[NH];
+            bool grew = false;
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt)
+            for (int hf = 0; hf < NH; ++hf) {
+                float tmax = kNegInf;
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const float x = s[nt][e] * p.scale_log2;
-                    s[nt][e] = (nt * 8 + qd * 2 + e < valid) ? x : kNegInf;
-                    tmax = fmaxf(tmax, s[nt][e]);
-                }
-            tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
-            tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
-            const float m_new = fmaxf(m, tmax);
-            if (__any_sync(0xffffffffu, m_new > m)) {
-                const float corr = exp2f(m - m_new);  // m = -inf on the first tile -> 0
-                l *= corr;
+                for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
-                for (int nt = 0; nt < D / 8; ++nt) o[nt][0] *= corr, o[nt][1] *= corr;
-                m = m_new;
+                    for (int e = 0; e < 2; ++e) {
+                        const float x = s[hf][nt][e] * p.scale_log2;
+                        s[hf][nt][e] = (nt * 8 + qd * 2 + e < valid) ? x : kNegInf;
+                        tmax = fmaxf(tmax, s[hf][nt][e]);
+                    }
+                tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
+                tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
+                m_new[hf] = fmaxf(m[hf], tmax);
+                grew = grew || m_new[hf] > m[hf];
             }
-            const float p00 = exp2f(s[0][0] - m), p01 = exp2f(s[0][1] - m);
-            const float p10 = exp2f(s[1][0] - m), p11 = exp2f(s[1][1] - m);
-            l += (p00 + p01) + (p10 + p11);
-            const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);
+            if (__any_sync(0xffffffffu, grew)) {
+#pragma unroll
+                for (int hf = 0; hf < NH; ++hf) {
+                    const float corr = exp2f(m[hf] - m_new[hf]);  // m = -inf on the first tile -> 0
+                    l[hf] *= corr;
+#pragma unroll
+                    for (int nt = 0; nt < D / 8; ++nt) o[hf][nt][0] *= corr, o[hf][nt][1] *= corr;
+                    m[hf] = m_new[hf];
+                }
+            }
+            uint32_t pa[NH][2];
+#pragma unroll
+            for (int hf = 0; hf < NH; ++hf) {
+                const float p00 = exp2f(s[hf][0][0] - m[hf]), p01 = exp2f(s[hf][0][1] - m[hf]);
+                const float p10 = exp2f(s[hf][1][0] - m[hf]), p11 = exp2f(s[hf][1][1] - m[hf]);
+                l[hf] += (p00 + p01) + (p10 + p11);
+                pa[hf][0] = pack_bf16(p00, p01), pa[hf][1] = pack_bf16(p10, p11);
+            }
             // ---- O += P V
             {
                 const int vrow = kPage + (((lane >> 3) & 1) << 3) + (lane & 7);
@@ -877,8 +923,15 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     const int ck = (cg & 7) + (lane >> 4);
                     uint32_t v0, v1, v2, v3;
                     ldsm_x4_t(rbase + (cg >> 3) * kHalf + ((ck ^ (vrow & 7)) << 4), v0, v1, v2, v3);
-                    mma_rows07(o[cg][0], o[cg][1], pa0, pa2, v0, v1);
-                    mma_rows07(o[cg + 1][0], o[cg + 1][1], pa0, pa2, v2, v3);
+                    if constexpr (NH == 1) {
+                        mma_rows07(o[0][cg][0], o[0][cg][1], pa[0][0], pa[0][1], v0, v1);
+                        mma_rows07(o[0][cg + 1][0], o[0][cg + 1][1], pa[0][0], pa[0][1], v2, v3);
+                    } else {
+                        mma_rows16(o[0][cg][0], o[0][cg][1], o[NH - 1][cg][0], o[NH - 1][cg][1], pa[0][0], pa[NH - 1][0], pa[0][1],
+                                   pa[NH - 1][1], v0, v1);
+                        mma_rows16(o[0][cg + 1][0], o[0][cg + 1][1], o[NH - 1][cg + 1][0], o[NH - 1][cg + 1][1], pa[0][0],
+                                   pa[NH - 1][0], pa[0][1], pa[NH - 1][1], v2, v3);
+                    }
                 }
             }
             if (valid < kPage) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -888,13 +941,17 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         }
 
         // ---- combine the eight warp states of this item
-        l += __shfl_xor_sync(0xffffffffu, l, 1);
-        l += __shfl_xor_sync(0xffffffffu, l, 2);
-        if (row_ok) {
-            float* so = scratch_o + (warp * G + row) * kRowF + qd * 2;
 #pragma unroll
-            for (int nt = 0; nt < D / 8; ++nt) *reinterpret_cast<float2*>(so + nt * 8) = make_float2(o[nt][0], o[nt][1]);
-            if (qd == 0) *reinterpret_cast<float2*>(scratch_ml + (warp * G + row) * 2) = make_float2(m, l);
+        for (int hf = 0; hf < NH; ++hf) {
+            l[hf] += __shfl_xor_sync(0xffffffffu, l[hf], 1);
+            l[hf] += __shfl_xor_sync(0xffffffffu, l[hf], 2);
+            if (row_ok[hf]) {
+                float* so = scratch_o + (warp * G + row + 8 * hf) * kRowF + qd * 2;
+#pragma unroll
+                for (int nt = 0; nt < D / 8; ++nt)
+                    *reinterpret_cast<float2*>(so + nt * 8) = make_float2(o[hf][nt][0], o[hf][nt][1]);
+                if (qd == 0) *reinterpret_cast<float2*>(scratch_ml + (warp * G + row + 8 * hf) * 2) = make_float2(m[hf], l[hf]);
+            }
         }
         named_bar_sync(1, kNW * 32);
         for (int idx = threadIdx.x; idx < G * (D / 2); idx += kNW * 32) {
@@ -1097,32 +1154,34 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
 static int g_overlap_state = -1;
 
 // CTAs of the decode kernel that can be co-resident on the current device (SMs x occupancy).
-template <int D, bool TIMED>
+template <int D, bool TIMED, int NH>
 static int max_coresident(int dev, int smem) {
     int sms = 0, per_sm = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED>, Smem<D>::kThreads, smem) !=
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED, NH>, Smem<D>::kThreads, smem) !=
         cudaSuccess)
         return 0;
     return sms * per_sm;
 }
 
-template <int D, bool TIMED>
+template <int D, bool TIMED, int NH>
 static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map, cudaStream_t stream,
                         bool want_tail_merge, bool* merged) {
     using L = Smem<D>;
     const int smem = L::total(prm.n_stages, prm.G, prm.n_qslots);
-    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, TIMED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, TIMED, NH>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     // The tail merge needs a grid barrier, i.e. a cooperative launch with every CTA resident.  The answer is
     // cached per (device, shared-memory size).
     static thread_local int cached_dev = -1, cached_smem = -1, cached_max = 0;
     int dev = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
-    if (want_tail_merge && D <= 128 && (cached_smem != smem || cached_dev != dev))
-        cached_max = max_coresident<D, TIMED>(dev, smem), cached_smem = smem, cached_dev = dev;
-    // (at d = 256 the grid has 128 consumer threads per CTA, fewer than a merge record has elements: stand-alone kernel)
-    prm.tail_merge = want_tail_merge && D <= 128 && dp->n_static <= cached_max;
+    // the in-grid merge gives every thread one float4 of a record: it needs G * d/4 <= consumer threads (d = 256,
+    // or d = 128 with G > 8, use the stand-alone merge kernel)
+    const bool fits = D <= 128 && prm.G * (D / 4) <= Smem<D>::kNW * 32;
+    if (want_tail_merge && fits && (cached_smem != smem || cached_dev != dev))
+        cached_max = max_coresident<D, TIMED, NH>(dev, smem), cached_smem = smem, cached_dev = dev;
+    prm.tail_merge = want_tail_merge && fits && dp->n_static <= cached_max;
     *merged = prm.tail_merge;
     if (prm.q_host && !prm.tail_merge) {
         // no co-resident grid, no in-kernel staging: the staging kernel runs first and the decode kernel is
@@ -1142,13 +1201,13 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     // not asked again (a failing launch inside a stream capture would invalidate the capture).
     if (g_overlap_state == 0) prm.pdl = 0;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
-    e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+    e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH>, map, prm);
     if (prm.pdl) {
         if (e == cudaSuccess) g_overlap_state = 1;
         else {
             (void)cudaGetLastError();
             g_overlap_state = 0, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
-            e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED>, map, prm);
+            e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH>, map, prm);
         }
     }
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
@@ -1182,8 +1241,18 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
     if (which & kRunSplit) {
         // a fused step always wants the tail phase (lengths + table growth), even with nothing to merge
         const bool want = (which & kRunMerge) && (n_units > 0 || fused || prm.q_host);
-        const int rc = prm.worker_ns ? launch_split<D, true>(dp, prm, map, stream, want, &merged)
-                                     : launch_split<D, false>(dp, prm, map, stream, want, &merged);
+        int rc;
+        if constexpr (D <= 128) {
+            if (prm.G > 8)
+                rc = prm.worker_ns ? launch_split<D, true, 2>(dp, prm, map, stream, want, &merged)
+                                   : launch_split<D, false, 2>(dp, prm, map, stream, want, &merged);
+            else
+                rc = prm.worker_ns ? launch_split<D, true, 1>(dp, prm, map, stream, want, &merged)
+                                   : launch_split<D, false, 1>(dp, prm, map, stream, want, &merged);
+        } else {
+            rc = prm.worker_ns ? launch_split<D, true, 1>(dp, prm, map, stream, want, &merged)
+                               : launch_split<D, false, 1>(dp, prm, map, stream, want, &merged);
+        }
         if (rc != TANGRAM_OK) return rc;
     }
     if (!(which & kRunMerge) || merged) return TANGRAM_OK;
@@ -1212,13 +1281,24 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Largest GQA group: 16 query heads per KV head (both halves of the mma A operand) at d <= 128; at d = 256 the
+// accumulators of 16 rows do not fit the register file, so 8.
+static int max_gqa(int head_dim) { return head_dim == 256 ? 8 : kMaxG; }
+
 template <int D>
 static cudaError_t occupancy_of(int gqa, int* per_sm) {
     const int ns = Smem<D>::max_stages(gqa);
     const int smem = Smem<D>::total(ns, gqa, Smem<D>::max_qslots(ns, gqa));
-    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (D <= 128 && gqa > 8) {
+        if constexpr (D <= 128) {
+            cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e != cudaSuccess) return e;
+            return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false, 2>, Smem<D>::kThreads, smem);
+        }
+    }
+    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false>, Smem<D>::kThreads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false, 1>, Smem<D>::kThreads, smem);
 }
 
 }  // namespace tangram
@@ -1226,8 +1306,9 @@ static cudaError_t occupancy_of(int gqa, int* per_sm) {
 using namespace tangram;
 
 extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa, int32_t* n_cta_out) {
-    if (!n_cta_out || (head_dim != 64 && head_dim != 128 && head_dim != 256) || gqa < 1 || gqa > kMaxG)
-        return fail(TANGRAM_ERR_INVALID_ARG, "query_max_ctas: head_dim=%d gqa=%d", head_dim, gqa);
+    if (!n_cta_out || (head_dim != 64 && head_dim != 128 && head_dim != 256) || gqa < 1 || gqa > max_gqa(head_dim))
+        return fail(TANGRAM_ERR_INVALID_ARG, "query_max_ctas: head_dim=%d gqa=%d (GQA groups up to %d at this head_dim)",
+                    head_dim, gqa, max_gqa(head_dim));
     int sms = 0, per_sm = 0;
     cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
@@ -1287,6 +1368,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
         !t->tbl_indptr || !t->cluster_of || !t->slot_of || !t->perm)
         return fail(TANGRAM_ERR_INVALID_ARG, "upload: NULL argument");
     if (p->n_items > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: more than 2^31 items");
+    if (t->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "upload: page size %d (kernels need 16)", t->P);
     const BlobLayout lay = blob_layout(t, p);
     const size_t need = lay.total;
     if (bytes < need) return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "upload: blob %zu < %zu bytes", bytes, need);
@@ -1461,9 +1543,9 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128, 256}", d);
     if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d (kernels need 16)", dp->P);
-    if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > kMaxG)
-        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d)", Hq,
-                    dp->H, kMaxG);
+    if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > max_gqa(d))
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d at head_dim %d)", Hq,
+                    dp->H, max_gqa(d), d);
     if (dp->W < 1 || dp->n_static < 1 || dp->n_static > dp->W) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty plan");
     if (split && n_pool_pages < 1) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: empty pool");
     if (split && n_pool_pages < dp->min_pool_pages)

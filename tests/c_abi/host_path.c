@@ -78,6 +78,31 @@ int main(void) {
         CHECK(tangram_calibrate_budgets(x, 2, 1, 1.0, &m, &sd, &b) == TANGRAM_OK);
         CHECK(m == 0.5 && sd == 0.25 && b == 0.75);
     }
+    /* NEXT-4 (block tables): the hand-evaluated growth example of tests/golden/hand_examples.json "extend_tables":
+     * B = [.9,.2,.6,.3] -> clusters {1,3} and {2,0}; 2 growth slots per row; 7 pages built, 4 more handed out */
+    {
+        const double Bg[4] = {0.9, 0.2, 0.6, 0.3};
+        const int32_t res[8] = {40, 10, 33, 16, 16, 5, 20, 7};
+        const int32_t fl[11] = {50, 7, 23, 41, 8, 15, 16, 42, 4, 99, 3};
+        const int32_t kv1[8] = {40, 10, 33, 16, 16, 5, 20, 7}, kv2[8] = {48, 10, 33, 32, 16, 16, 32, 7};
+        const int32_t want1[15] = {50, 42, -1, 7, 23, 41, -1, -1, 8, -1, -1, 15, 16, -1, -1};
+        const int32_t want2[15] = {50, 42, 4, 7, 23, 41, 99, -1, 8, 3, -1, 15, 16, -1, -1};
+        int32_t pm[4], co[4], so[4], pages[15], rows[4];
+        int64_t ip[5], ext = -1, starved = -1;
+        tangram_tables g;
+        memset(&g, 0, sizeof g);
+        g.perm = pm, g.cluster_of = co, g.slot_of = so, g.tbl_indptr = ip, g.tbl_pages = pages, g.tbl_pages_cap = 15;
+        g.headroom_pages = 2, g.row_pages = rows;
+        CHECK(tangram_build_ragged_tables(Bg, res, 2, 4, 2, 16, fl, 11, 0u, NULL, &g) == TANGRAM_OK);
+        CHECK(g.n_pages_used == 7 && g.n_slots == 15 && ip[4] == 15 && rows[0] == 1 && rows[1] == 3 && rows[3] == 2);
+        CHECK(tangram_extend_tables(&g, kv1, fl, 11, 1, &ext, &starved) == TANGRAM_OK);
+        CHECK(ext == 1 && starved == 0 && g.n_pages_used == 8 && memcmp(pages, want1, sizeof want1) == 0);
+        CHECK(tangram_extend_tables(&g, kv2, fl, 11, 0, &ext, &starved) == TANGRAM_OK);
+        CHECK(ext == 3 && starved == 1 && g.n_pages_used == 11 && memcmp(pages, want2, sizeof want2) == 0);
+        CHECK(rows[0] == 3 && rows[1] == 4 && rows[2] == 2 && rows[3] == 2);
+        g.row_pages = NULL;
+        CHECK(tangram_extend_tables(&g, kv2, fl, 11, 0, NULL, NULL) == TANGRAM_ERR_INVALID_ARG);
+    }
     printf("c_abi host path ok\n");
     return 0;
 }

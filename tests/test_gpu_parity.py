@@ -87,9 +87,12 @@ def n_cta(wl):
 
 def test_query_max_ctas():
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    for d, g in ((64, 2), (128, 4), (128, 5), (128, 8), (256, 2), (256, 8)):
+    for d, g in ((64, 2), (128, 4), (128, 5), (128, 8), (256, 2), (256, 8), (128, 9), (128, 16), (64, 12)):
         n = T.tangram_query_max_ctas(0, d, g)
         assert n >= sms and n % sms == 0
+    for d, g in ((128, 17), (256, 9), (64, 0)):                 # GQA groups: up to 16 at d <= 128, up to 8 at d = 256
+        with pytest.raises(T.TangramError):
+            T.tangram_query_max_ctas(0, d, g)
 
 
 def test_tiny_full_config():
@@ -114,7 +117,10 @@ def test_scaled_configs(name, kw):
                                             (7, 4, 4, 6, 64, 4), (8, 2, 2, 8, 128, 2),
                                             # d = 256 (Gemma-3-shaped heads): four consumer warps, 16 KB tiles
                                             (9, 2, 4, 2, 256, 2), (10, 2, 2, 8, 256, 1), (11, 3, 8, 4, 256, 4),
-                                            (12, 1, 1, 5, 256, 1)])
+                                            (12, 1, 1, 5, 256, 1),
+                                            # GQA groups of 9..16 query heads: both halves of the mma A operand
+                                            (13, 2, 2, 9, 128, 1), (14, 2, 4, 16, 128, 2), (15, 3, 2, 12, 64, 2),
+                                            (16, 1, 1, 16, 64, 1), (17, 2, 2, 13, 128, 2)])
 def test_random_shapes(seed, R, H, G, d, C):
     wl = I.make_random_workload(seed, R=R, H=H, G=G, d=d, C=C, max_ctx=900)
     B, res, kv, t, n_pool = setup(wl)
@@ -246,7 +252,7 @@ def test_device_error_contract():
     with pytest.raises(T.TangramError) as e:
         T.tangram_decode_attention(dp, q, pool, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
     assert e.value.code == T.ERR_BUFFER_TOO_SMALL
-    q3 = torch.randn(wl.R, 3 * wl.H * 3, wl.d, device="cuda").bfloat16()          # G = 9 > 8
+    q3 = torch.randn(wl.R, 17 * wl.H, wl.d, device="cuda").bfloat16()             # G = 17 > 16
     with pytest.raises(T.TangramError) as e:
         T.tangram_decode_attention(dp, q3, pool)
     assert e.value.code == T.ERR_INVALID_ARG
@@ -447,13 +453,14 @@ def test_pinned_host_q_and_outputs_zero_copy():
 
 
 def test_random_sweep_of_shapes_plans_and_runtime_lengths():
-    """300 seeded cases over (R, H, G 1..8, d, clusters, context, W, mode, c0, granule, dynamic tail, FILL_GROUP,
+    """300 seeded cases over (R, H, G 1..16 (1..8 at d = 256), d, clusters, context, W, mode, c0, granule, dynamic tail, FILL_GROUP,
     empty heads, open-ended run-time lengths), every one against the oracle at the BASELINE tolerances, each
     plan launched twice (the scheduler counters re-arm themselves)."""
     rng = np.random.default_rng(20260630)
     for case in range(300):
         H = int(rng.choice([1, 2, 4, 8]))
-        G, d = int(rng.integers(1, 9)), int(rng.choice([64, 128, 256]))
+        d = int(rng.choice([64, 128, 256]))
+        G = int(rng.integers(1, 9 if d == 256 else 17))
         C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
         R = int(rng.integers(1, 6))
         wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=G, d=d, C=C,

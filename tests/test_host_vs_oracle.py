@@ -225,6 +225,26 @@ def test_header_is_plain_c_and_host_path_runs_from_c(tmp_path):
     assert "c_abi host path ok" in out.stdout
 
 
+def test_host_code_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """the host side (tangram_host.cpp: reserve, tables, growth, planner, accounting, calibration) built
+    with -fsanitize=address,undefined together with the plain-C caller and run: no report, same hand-evaluated
+    values.  The CUDA side cannot be built this way; it is covered by guard regions / NaN poison on the GPU."""
+    import subprocess
+    csrc = os.path.join(ROOT, "paper_2606_06302_b200", "csrc")
+    san = ["-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer", "-g", "-O1"]
+    obj_c, obj_cpp, exe = str(tmp_path / "host_path.o"), str(tmp_path / "tangram_host.o"), str(tmp_path / "host_path_san")
+    subprocess.check_call(["gcc", "-std=c99", "-pedantic", "-Wall", "-Wextra", "-Werror", *san, "-I", os.path.join(ROOT, "include"),
+                           "-c", os.path.join(ROOT, "tests", "c_abi", "host_path.c"), "-o", obj_c])
+    subprocess.check_call(["g++", "-std=c++17", "-Wall", "-Wextra", "-ffp-contract=off", "-fopenmp", *san,
+                           "-I", os.path.join(ROOT, "include"), "-I", csrc, "-c", os.path.join(csrc, "tangram_host.cpp"),
+                           "-o", obj_cpp])
+    subprocess.check_call(["g++", *san, "-fopenmp", obj_c, obj_cpp, "-o", exe])
+    env = dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", UBSAN_OPTIONS="print_stacktrace=1")
+    out = subprocess.run([exe], capture_output=True, text=True, env=env, timeout=120)
+    assert out.returncode == 0, out.stderr + out.stdout
+    assert "c_abi host path ok" in out.stdout and "runtime error" not in out.stderr and "AddressSanitizer" not in out.stderr
+
+
 def test_default_dynamic_tail_rule():
     for name in I.CONFIG_NAMES:
         wl = I.make_workload(name)
