@@ -658,12 +658,19 @@ def table_update_summary(T, I, device, torch, names=("8b", "32b"), steps=48):
             host_us = {}
             for nt in (1, 0):
                 t, kv = T.tangram_build_ragged_tables(B, res, C, wl.P, free, 0, kv0, headroom_pages=headroom)
-                cur, ts, ext = kv.copy(), [], 0
+                # the C call itself, arguments marshalled once (the binding's per-call numpy -> ctypes conversion
+                # costs ~15 us, more than the update)
+                import ctypes
+                ct, cur, ts, ext = t._c(), np.ascontiguousarray(kv, dtype=np.int32).copy(), [], 0
+                e_out, s_out = ctypes.c_int64(0), ctypes.c_int64(0)
+                args = (ctypes.byref(ct), cur.ctypes.data_as(ctypes.c_void_p), free.ctypes.data_as(ctypes.c_void_p),
+                        ctypes.c_int64(free.shape[0]), ctypes.c_int32(nt), ctypes.byref(e_out), ctypes.byref(s_out))
                 for _ in range(steps):
                     t0 = time.perf_counter()
-                    e, s_ = T.tangram_extend_tables(t, cur, free, n_threads=nt)
+                    rc = T._lib.tangram_extend_tables(*args)
                     ts.append(time.perf_counter() - t0)
-                    ext += e
+                    assert rc == 0
+                    ext += int(e_out.value)
                     cur += 1
                 host_us["1_thread" if nt == 1 else "openmp_default"] = float(np.median(ts) * 1e6)
             t, kv = T.tangram_build_ragged_tables(B, res, C, wl.P, free, 0, kv0, headroom_pages=headroom)
