@@ -532,6 +532,31 @@ def spread_of(T, S, torch, reps=5, detail=False):
         "launch_to_launch_corr": corr}
 
 
+def timeline_of(T, S, torch, flush, reps=5):
+    """Where a step's time goes, from the instrumented kernel's globaltimer stamps (us after the first CTA starts,
+    median over reps): the first and the last CTA running out of work lists, the grid barrier passed by the last
+    CTA, the last merge done.  The CUDA-event time of the same launch adds the launch / completion floor."""
+    W = S["plan"].n_static
+    ns = torch.zeros(W, 4, dtype=torch.int64, device=S["q"].device)
+    rows = []
+    for _ in range(reps):
+        flush()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"], worker_ns=ns)
+        b.record()
+        torch.cuda.synchronize()
+        w = ns.cpu().numpy().astype(np.float64)
+        t0 = w[:, 0].min()
+        merged = w[:, 3].max() if w[:, 3].max() > 0 else w[:, 1].max()
+        barrier = w[:, 2].max() if w[:, 2].max() > 0 else w[:, 1].max()
+        rows.append([(w[:, 0].max() - t0) / 1e3, (w[:, 1].min() - t0) / 1e3, (w[:, 1].max() - t0) / 1e3,
+                     (barrier - t0) / 1e3, (merged - t0) / 1e3, a.elapsed_time(b) * 1e3])
+    m = np.median(np.array(rows), axis=0)
+    return {"last_cta_start_us": float(m[0]), "first_cta_out_of_work_us": float(m[1]), "last_cta_out_of_work_us": float(m[2]),
+            "barrier_passed_us": float(m[3]), "merges_done_us": float(m[4]), "cuda_event_us": float(m[5])}
+
+
 def prepare(T, S, torch):
     wl, plan = S["wl"], S["plan"]
     t0 = time.perf_counter()
@@ -563,7 +588,7 @@ def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, co
            "decode_kernel_us": kus, "decode_kernel_gbs": (b["total"] - b["partials"] // 2) / (kus * 1e-6) / 1e9,
            "algorithmic_bytes": b, "W": S["W"], "items": int(S["plan"].n_items), "granule": S["wl"].granule,
            "c0": S["c0"], "dyn_permille": S["dyn"][0], "dyn_rounds": S["dyn"][1], "host_ms": S["host_ms"],
-           "cta_spread": spread_of(T, S, torch)}
+           "cta_spread": spread_of(T, S, torch), "timeline": timeline_of(T, S, torch, flush)}
     if compare:
         legs = [(T.MODE_STATIC_EVEN, "static_even"), (T.MODE_SPLITMAP, "splitmap")]
         if S["dyn"][1] > 0:                   # the same equal-bytes plan, every CTA owning exactly one list
@@ -862,6 +887,11 @@ def main():
         # BALANCED-without-dynamic-tail slowdown (x), STATIC_EVEN slowdown (x)]
         line["config"]["per_config_summary"] = {
             "columns": ["us", "tbs", "kernel_gbs", "cta_spread", "balanced_static_x", "static_even_x"],
+            "timeline_columns": ["first CTA out of work", "last CTA out of work", "barrier passed", "merges done",
+                                 "CUDA events"],
+            "timeline_us": {k: [round(v["timeline"][c], 1) for c in ("first_cta_out_of_work_us", "last_cta_out_of_work_us",
+                                                                      "barrier_passed_us", "merges_done_us", "cuda_event_us")]
+                            for k, v in per.items()},
             **{k: [round(v["us_per_layer_step"], 2), round(v["tbs"], 3), round(v["decode_kernel_gbs"], 0),
                    round(v["cta_spread"], 4),
                    round(v["balanced_static"]["slowdown_vs_balanced"], 3) if "balanced_static" in v else None,
