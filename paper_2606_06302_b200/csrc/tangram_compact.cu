@@ -192,8 +192,15 @@ __device__ __forceinline__ void radix_passes(EachKey&& each_key, int pass_begin,
             }
             if (lane == 0) s_wsum[warp] = incl;
             __syncthreads();
-            uint32_t gt = incl - mine;
-            for (int w = warp + 1; w < kWarps; ++w) gt += s_wsum[w];
+            // entries in the warps after this one: a warp-wide suffix sum over the (<= 32) warp totals
+            uint32_t after = lane < kWarps ? s_wsum[lane] : 0u;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t v = __shfl_down_sync(0xffffffffu, after, o);
+                if (lane + o < 32) after += v;
+            }
+            const uint32_t warp_incl = __shfl_sync(0xffffffffu, after, warp);  // totals of warps warp .. kWarps-1
+            uint32_t gt = incl - mine + (warp_incl - s_wsum[warp]);
 #pragma unroll
             for (int j = kBpt - 1; j >= 0; --j) {
                 if (gt < krem && krem <= gt + c[j]) {  // exactly one bin satisfies this
@@ -388,13 +395,16 @@ __device__ __forceinline__ void select_row(SelectSmem<NT>& sm, const int seq, co
             if (lane >= o) incl += t;
         }
         const uint32_t tot = __shfl_sync(0xffffffffu, incl, 31);
-        uint32_t g = run_gt + ((incl - p) & 0xffffu), e = run_eq + ((incl - p) >> 16);
         if (p) {
+            // the lane's retained tokens take consecutive positions from (#greater before) + min(#equal before, need)
+            uint32_t e = run_eq + ((incl - p) >> 16);
+            uint32_t pos = run_gt + ((incl - p) & 0xffffu) + min(e, need);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                const bool gt = key[j] > T, eq = key[j] == T;
-                if (gt || (eq && e < need)) idx[g + min(e, need)] = head + 4 * v + j;
-                g += gt, e += eq;
+                const bool eq = key[j] == T;
+                const bool keep = key[j] > T || (eq && e < need);
+                if (keep) idx[pos] = head + 4 * v + j;
+                pos += keep, e += eq;
             }
         }
         run_gt += tot & 0xffffu, run_eq += tot >> 16;
