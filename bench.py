@@ -196,11 +196,11 @@ def algorithmic_bytes(wl, kv, plan, t):
 
 
 def setup_workload(T, I, name, device, W=None, mode=None, c0=1, dyn=None, layer=0, plan_capacity=False, R=None,
-                   headroom=0):
+                   headroom=0, page_size=None):
     """Budgets, tables and plan of workload `name` through the product's API.  headroom > 0: growable tables (that
     many empty page slots per row, and a pool / free list large enough to fill them) for the decode loop."""
     import torch
-    wl = I.make_workload(name, layer=layer, R=R)
+    wl = I.make_workload(name, layer=layer, R=R, page_size=page_size)
     t0 = time.perf_counter()
     B, res, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
     need = T.tangram_pages_needed(B, res, wl.C, wl.P)
@@ -569,10 +569,11 @@ def prepare(T, S, torch):
     S["bytes"] = algorithmic_bytes(wl, S["kv"], plan, S["tables"])
 
 
-def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, compare=True, dyn=None, R=None):
+def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, compare=True, dyn=None, R=None,
+                   page_size=None):
     """µs per layer-step, achieved TB/s, kernel-only roofline, spread, and the same kernel run from the
     BALANCED plan without its dynamic tail, from STATIC_EVEN and from SPLITMAP."""
-    S = setup_workload(T, I, name, device, dyn=dyn, R=R)
+    S = setup_workload(T, I, name, device, dyn=dyn, R=R, page_size=page_size)
     prepare(T, S, torch)
     step = lambda: T.tangram_decode_attention(S["dp"], S["q"], S["pool"], S["out"], S["lse"], S["ws"])
     ms = time_steps(step, steps, warmup, flush, torch)
@@ -870,11 +871,12 @@ def main():
         del S
         torch.cuda.empty_cache()
         # batch-4 8b-shaped: the paper's own decode-attention comparison point (Fig. 13: batch 4)
-        sweep = [("tiny", None), ("8b", None), ("32b", None), ("skew", None), ("uniform", None), ("12b_d256", None),
-                 ("8b_batch4", 4)]
-        for key, R in sweep:
-            name = "8b" if key == "8b_batch4" else key
-            S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs, dyn=dyn, R=R)
+        sweep = [("tiny", None, None), ("8b", None, None), ("32b", None, None), ("skew", None, None), ("uniform", None, None),
+                 ("12b_d256", None, None), ("8b_batch4", 4, None), ("8b_page32", None, 32)]
+        for key, R, P in sweep:
+            name = "8b" if key in ("8b_batch4", "8b_page32") else key
+            S2, res, _, _ = measure_config(T, I, name, device, min(args.steps, 100), 5, flush, torch, peak_gbs, dyn=dyn, R=R,
+                                           page_size=P)
             if key == args.workload and not args.no_cpu_baseline:
                 from oracle import tangram_oracle as O
                 O.build_c()

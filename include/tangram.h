@@ -246,7 +246,7 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *             decode step while tangram_append_kv grows the cache; items beyond the current length are
  *             empty and a head with length 0 yields out = 0, lse = -inf.
  *   Hq        query heads, Hq % H == 0, G = Hq / H <= 16 (<= 8 at d = 256; query head j uses KV head floor(j / G))
- *   d         64, 128 or 256;  P must be 16
+ *   d         64, 128 or 256;  page size P 16, or 32 at d <= 128 (tangram_upload refuses any other P)
  *   sm_scale  softmax scale; 0 means 1/sqrt(d)
  *   out       device [R][Hq][d] bf16;  lse device [R][Hq] f32 (natural log of sum exp(scaled score);
  *             -inf and out = 0 for a head with kv_len 0)
@@ -259,7 +259,7 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  * events between streams); different plans (e.g. one per layer) may run concurrently.
  * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
- * Errors: INVALID_ARG (shape / alignment / P != 16 / d / G / n_pool_pages <= a page id of the tables),
+ * Errors: INVALID_ARG (shape / alignment / unsupported P / d / G / n_pool_pages <= a page id of the tables),
  * BUFFER_TOO_SMALL (workspace), CUDA. */
 int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
                              int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d,

@@ -31,7 +31,7 @@
 
 namespace tangram {
 
-constexpr int kCPage = 16;           // tokens per page (the kernels are specialised for P = 16)
+constexpr int kCPage = 16;           // rows of a gather tile (= one page at P = 16, half a page at P = 32)
 constexpr int kSelBins = 2048;        // 11-bit digits
 constexpr int kSelCand = 4096;        // candidates (entries in the first digit's bin) the select kernel buffers
 constexpr int kSelLongRow = 49152;    // rows longer than this get 1024-thread CTAs, shorter ones 512 (two per SM)
@@ -505,7 +505,7 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
                       const int32_t* __restrict__ idx, int64_t n_max, const uint4* __restrict__ k_dense,
                       const uint4* __restrict__ v_dense, uint4* __restrict__ pool, int Hp, int n_seq,
                       int32_t* __restrict__ counter, const int32_t* __restrict__ keep_eff,
-                      const int32_t* __restrict__ base, const int32_t* __restrict__ tile_indptr) {
+                      const int32_t* __restrict__ base, const int32_t* __restrict__ tile_indptr, int P) {
     constexpr int kChunks = D / 8;           // 16-byte chunks per row
     constexpr int kRowsPerLd = 32 / kChunks;  // rows one warp-wide load covers
     constexpr int kLds = kCPage / kRowsPerLd; // loads per lane for the K rows of a tile (same for V)
@@ -541,9 +541,9 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
             if (lane < n_rows) {
                 my_tok = __ldg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
                 const int pos = __ldg(base + seq) + tl * kCPage + lane;
-                const int page = __ldg(tbl_pages + si.x + pos / kCPage);
-                // pool[page][slot][kv][token][d]: row index of the K row; the V row is kCPage rows further
-                my_dst = ((static_cast<uint32_t>(page) * Hp + si.z) * 2) * kCPage + pos % kCPage;
+                const int page = __ldg(tbl_pages + si.x + pos / P);
+                // pool[page][slot][kv][token][d]: row index of the K row; the V row is P rows further
+                my_dst = ((static_cast<uint32_t>(page) * Hp + si.z) * 2) * P + pos % P;
             }
             // (at d = 256 a tile goes in two halves of eight rows: 16 + 16 loads would not fit the register budget)
 #pragma unroll
@@ -565,7 +565,7 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
                     const uint32_t dst = __shfl_sync(0xffffffffu, my_dst, row);
                     if (row < n_rows) {
                         pool[static_cast<size_t>(dst) * kChunks + ch] = kreg[j];
-                        pool[static_cast<size_t>(dst + kCPage) * kChunks + ch] = vreg[j];
+                        pool[static_cast<size_t>(dst + P) * kChunks + ch] = vreg[j];
                     }
                 }
             }
@@ -594,7 +594,8 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: NULL argument");
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: head_dim %d not in {64, 128, 256}", d);
-    if (dp->P != kCPage) return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: page size %d (kernels need 16)", dp->P);
+    if (dp->P != 16 && !(dp->P == 32 && d <= 128))
+        return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: page size %d at head_dim %d (kernels need 16, or 32 at head_dim <= 128)", dp->P, d);
     if (n_max < 1 || n_max > (1 << 30) || n_pool_pages < 1 || n_pool_pages < dp->min_pool_pages)
         return fail(TANGRAM_ERR_INVALID_ARG, "compact_topk: n_max=%lld n_pool_pages=%lld", (long long)n_max,
                     (long long)n_pool_pages);
@@ -647,7 +648,7 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
             grid = sms * (per_sm > 0 ? per_sm : 1);
         }
         kernel<<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool, dp->Hp, n_seq,
-                                                w.counter, w.keep_eff, w.base, w.tile_indptr);
+                                                w.counter, w.keep_eff, w.base, w.tile_indptr, dp->P);
         return cudaSuccess;
     };
     static thread_local int grid_dev = -1, grid256 = 0, grid128 = 0, grid64 = 0;  // cached per (thread, device)

@@ -35,11 +35,13 @@
 
 namespace tangram {
 
-constexpr int kPage = 16;          // tokens per page the kernels are specialised for
-// consumer warps of the decode kernel: 8, or 4 at d = 256 where one (page, head) tile is 16 KB and eight
-// three-stage rings would not fit in shared memory
-template <int D>
-constexpr int consumer_warps() { return D == 256 ? 4 : 8; }
+// Page sizes (tokens per page) the kernels are instantiated for: 16 and 32.  One TMA box = the 2 P rows (K then V)
+// of one (page, head): 8 KB at P = 16, d = 128; 16 KB at P = 32, d = 128 or P = 16, d = 256.
+static bool page_supported(int P, int d) { return P == 16 || (P == 32 && d <= 128); }
+// consumer warps of the decode kernel: 8, or 4 where one (page, head) tile is 16 KB and eight three-stage rings
+// would not fit in shared memory
+template <int D, int PAGE>
+constexpr int consumer_warps() { return 2 * PAGE * D * 2 >= 16384 ? 4 : 8; }
 constexpr int kMinQSlots = 2;      // item / query ring depth: as deep as shared memory allows, 2 .. 8 (runtime).  A deep
 constexpr int kMaxQSlots = 8;      // ring lets the producer fetch query groups several items ahead, which is what hides
                                    // the bus round trip when q lives in pinned host memory
@@ -104,12 +106,12 @@ struct DecodeParams {
 };
 
 // ------------------------------------------------------------------ shared-memory carve-up
-template <int D>
+template <int D, int PAGE>
 struct Smem {
-    static constexpr int kNW = consumer_warps<D>();
+    static constexpr int kNW = consumer_warps<D, PAGE>();
     static constexpr int kThreads = (kNW + 1) * 32;          // + the producer warp
-    static constexpr int kTile = 2 * kPage * D * 2;          // K rows + V rows of one (page, head)
-    static constexpr int kHalf = 2 * kPage * 128;            // one 64-element column block of the tile
+    static constexpr int kTile = 2 * PAGE * D * 2;           // K rows + V rows of one (page, head)
+    static constexpr int kHalf = 2 * PAGE * 128;             // one 64-element column block of the tile
     static constexpr int kRowF = D + 8;                      // padded fp32 row of the merge scratch
     __host__ __device__ static int q_slot(int G) { return (G * D * 2 + 127) & ~127; }
     __host__ __device__ static int off_q(int ns) { return kNW * ns * kTile; }
@@ -535,10 +537,11 @@ __global__ void __launch_bounds__(1024) tangram_grow_kernel(const GrowParams g, 
 }
 
 // ------------------------------------------------------------------ a4: split-KV decode kernel
-template <int D, bool TIMED, int NH>
-__global__ void __launch_bounds__(Smem<D>::kThreads, 1)
+template <int D, bool TIMED, int NH, int PAGE>
+__global__ void __launch_bounds__(Smem<D, PAGE>::kThreads, 1)
 tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeParams p) {
-    using L = Smem<D>;
+    using L = Smem<D, PAGE>;
+    constexpr int kPage = PAGE;
     constexpr int kNW = L::kNW;
     constexpr int kTile = L::kTile, kHalf = L::kHalf, kRowF = L::kRowF;
     extern __shared__ uint8_t smem_raw[];
@@ -842,24 +845,29 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         for (int i = (warp - rot) & (kNW - 1); i < n_tiles; i += kNW) {
             mbar_wait(full_bar(warp, stage), phase);
             const uint32_t tb = tiles + (warp * NS + stage) * kTile;
-            const int valid = min(kPage, n_tok - i * kPage);
-            if (valid < kPage) {
+            const int tile_valid = min(kPage, n_tok - i * kPage);  // retained tokens in this (page, head) tile
+            if (tile_valid < kPage) {
                 // ragged tail: V rows of tokens that are not retained may hold anything (NaN
                 // included) and 0 * NaN would poison the PV product -- zero them.
                 if (lane < 8 * (D / 64))
-                    for (int rr = kPage + valid; rr < 2 * kPage; ++rr)
+                    for (int rr = kPage + tile_valid; rr < 2 * kPage; ++rr)
                         asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(tb + (lane >> 3) * kHalf + rr * 128 +
                                                                                    (lane & 7) * 16),
                                      "r"(0u)
                                      : "memory");
                 __syncwarp();
             }
+            // a tile is processed 16 tokens at a time (one pass at P = 16, two at P = 32)
+#pragma unroll 1
+            for (int sb = 0; sb < kPage / 16; ++sb) {
+            const int valid = min(16, tile_valid - sb * 16);
+            if (valid <= 0) break;
             // ---- S = Q K^T : 16 query rows (8 or 16 used) x 16 tokens
             float s[NH][2][2];
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) s[hf][0][0] = s[hf][0][1] = s[hf][1][0] = s[hf][1][1] = 0.f;
             {
-                const int tok = ((lane >> 4) << 3) + (lane & 7);
+                const int tok = sb * 16 + ((lane >> 4) << 3) + (lane & 7);
                 const uint32_t rbase = tb + tok * 128;
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks) {
@@ -916,7 +924,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             }
             // ---- O += P V
             {
-                const int vrow = kPage + (((lane >> 3) & 1) << 3) + (lane & 7);
+                const int vrow = kPage + sb * 16 + (((lane >> 3) & 1) << 3) + (lane & 7);
                 const uint32_t rbase = tb + vrow * 128;
 #pragma unroll
                 for (int cg = 0; cg < D / 8; cg += 2) {
@@ -934,7 +942,8 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     }
                 }
             }
-            if (valid < kPage) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }  // 16-token passes
+            if (tile_valid < kPage) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(warp, stage));
             if (++stage == static_cast<uint32_t>(NS)) stage = 0, phase ^= 1;
@@ -1054,7 +1063,7 @@ __global__ void __launch_bounds__(128)
 tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ seq_cap,
                       const int32_t* __restrict__ tbl_pages,
                       const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, uint4* __restrict__ pool,
-                      int32_t* __restrict__ kv_len, int32_t* __restrict__ overflow, int n_seq, int Hp, int d) {
+                      int32_t* __restrict__ kv_len, int32_t* __restrict__ overflow, int n_seq, int Hp, int d, int kPage) {
     const int seq = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (seq >= n_seq) return;
     const int4 si = seq_info[seq];  // {first slot of the row, slot capacity in tokens, slot, row}
@@ -1134,7 +1143,7 @@ static EncodeTiledFn encode_tiled_fn() {
 // The pool [n_pages][Hp][2][P][d] bf16 seen as rows of d elements: dim0 = 64 elements (128 B, the
 // swizzle span), dim1 = row, dim2 = which 64-element half of the row.  One box = the 2P rows (K then
 // V) of one (page, slot).
-static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages, int Hp, int d) {
+static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages, int Hp, int d, int kPage) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return fail(TANGRAM_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
     const cuuint64_t rows = static_cast<cuuint64_t>(n_pool_pages) * Hp * 2 * kPage;
@@ -1154,22 +1163,22 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
 static int g_overlap_state = -1;
 
 // CTAs of the decode kernel that can be co-resident on the current device (SMs x occupancy).
-template <int D, bool TIMED, int NH>
+template <int D, bool TIMED, int NH, int PAGE>
 static int max_coresident(int dev, int smem) {
     int sms = 0, per_sm = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED, NH>, Smem<D>::kThreads, smem) !=
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tangram_decode_kernel<D, TIMED, NH, PAGE>, Smem<D, PAGE>::kThreads, smem) !=
         cudaSuccess)
         return 0;
     return sms * per_sm;
 }
 
-template <int D, bool TIMED, int NH>
+template <int D, bool TIMED, int NH, int PAGE>
 static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map, cudaStream_t stream,
                         bool want_tail_merge, bool* merged) {
-    using L = Smem<D>;
+    using L = Smem<D, PAGE>;
     const int smem = L::total(prm.n_stages, prm.G, prm.n_qslots);
-    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, TIMED, NH>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, TIMED, NH, PAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     // The tail merge needs a grid barrier, i.e. a cooperative launch with every CTA resident.  The answer is
     // cached per (device, shared-memory size).
@@ -1178,9 +1187,9 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
     // the in-grid merge gives every thread one float4 of a record: it needs G * d/4 <= consumer threads (d = 256,
     // or d = 128 with G > 8, use the stand-alone merge kernel)
-    const bool fits = D <= 128 && prm.G * (D / 4) <= Smem<D>::kNW * 32;
+    const bool fits = D <= 128 && prm.G * (D / 4) <= L::kNW * 32;
     if (want_tail_merge && fits && (cached_smem != smem || cached_dev != dev))
-        cached_max = max_coresident<D, TIMED, NH>(dev, smem), cached_smem = smem, cached_dev = dev;
+        cached_max = max_coresident<D, TIMED, NH, PAGE>(dev, smem), cached_smem = smem, cached_dev = dev;
     prm.tail_merge = want_tail_merge && fits && dp->n_static <= cached_max;
     *merged = prm.tail_merge;
     if (prm.q_host && !prm.tail_merge) {
@@ -1191,7 +1200,7 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
         prm.q_host = nullptr, prm.pdl = 1;
     }
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(Smem<D>::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
+    cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(L::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
@@ -1201,20 +1210,20 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     // not asked again (a failing launch inside a stream capture would invalidate the capture).
     if (g_overlap_state == 0) prm.pdl = 0;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
-    e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH>, map, prm);
+    e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH, PAGE>, map, prm);
     if (prm.pdl) {
         if (e == cudaSuccess) g_overlap_state = 1;
         else {
             (void)cudaGetLastError();
             g_overlap_state = 0, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
-            e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH>, map, prm);
+            e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH, PAGE>, map, prm);
         }
     }
     if (e != cudaSuccess) return cuda_fail(e, "decode kernel launch");
     return TANGRAM_OK;
 }
 
-template <int D>
+template <int D, int PAGE>
 static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const CUtensorMap& map,
                          cudaStream_t stream, int which) {
     const int n_small = (int)(dp->n_merge_seqs - dp->n_big_merge_seqs);
@@ -1244,14 +1253,14 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
         int rc;
         if constexpr (D <= 128) {
             if (prm.G > 8)
-                rc = prm.worker_ns ? launch_split<D, true, 2>(dp, prm, map, stream, want, &merged)
-                                   : launch_split<D, false, 2>(dp, prm, map, stream, want, &merged);
+                rc = prm.worker_ns ? launch_split<D, true, 2, PAGE>(dp, prm, map, stream, want, &merged)
+                                   : launch_split<D, false, 2, PAGE>(dp, prm, map, stream, want, &merged);
             else
-                rc = prm.worker_ns ? launch_split<D, true, 1>(dp, prm, map, stream, want, &merged)
-                                   : launch_split<D, false, 1>(dp, prm, map, stream, want, &merged);
+                rc = prm.worker_ns ? launch_split<D, true, 1, PAGE>(dp, prm, map, stream, want, &merged)
+                                   : launch_split<D, false, 1, PAGE>(dp, prm, map, stream, want, &merged);
         } else {
-            rc = prm.worker_ns ? launch_split<D, true, 1>(dp, prm, map, stream, want, &merged)
-                               : launch_split<D, false, 1>(dp, prm, map, stream, want, &merged);
+            rc = prm.worker_ns ? launch_split<D, true, 1, PAGE>(dp, prm, map, stream, want, &merged)
+                               : launch_split<D, false, 1, PAGE>(dp, prm, map, stream, want, &merged);
         }
         if (rc != TANGRAM_OK) return rc;
     }
@@ -1272,7 +1281,7 @@ static int launch_decode(const tangram_device_plan* dp, DecodeParams prm, const 
         if (e != cudaSuccess) return cuda_fail(e, "merge kernel launch");
     }
     if (fused) {  // lengths + table growth of a fused step whose grid could not run its tail phase
-        tangram_grow_kernel<<<1, 1024, 0, stream>>>(prm.grow, kPage, 1);
+        tangram_grow_kernel<<<1, 1024, 0, stream>>>(prm.grow, PAGE, 1);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "grow kernel launch");
     }
@@ -1285,20 +1294,21 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // accumulators of 16 rows do not fit the register file, so 8.
 static int max_gqa(int head_dim) { return head_dim == 256 ? 8 : kMaxG; }
 
-template <int D>
+template <int D, int PAGE>
 static cudaError_t occupancy_of(int gqa, int* per_sm) {
-    const int ns = Smem<D>::max_stages(gqa);
-    const int smem = Smem<D>::total(ns, gqa, Smem<D>::max_qslots(ns, gqa));
+    using L = Smem<D, PAGE>;
+    const int ns = L::max_stages(gqa);
+    const int smem = L::total(ns, gqa, L::max_qslots(ns, gqa));
     if (D <= 128 && gqa > 8) {
         if constexpr (D <= 128) {
-            cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false, 2, PAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
             if (e != cudaSuccess) return e;
-            return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false, 2>, Smem<D>::kThreads, smem);
+            return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false, 2, PAGE>, L::kThreads, smem);
         }
     }
-    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(tangram_decode_kernel<D, false, 1, PAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false, 1>, Smem<D>::kThreads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, tangram_decode_kernel<D, false, 1, PAGE>, L::kThreads, smem);
 }
 
 }  // namespace tangram
@@ -1312,9 +1322,9 @@ extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa,
     int sms = 0, per_sm = 0;
     cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
-    if (head_dim == 256) e = occupancy_of<256>(gqa, &per_sm);
-    else if (head_dim == 128) e = occupancy_of<128>(gqa, &per_sm);
-    else e = occupancy_of<64>(gqa, &per_sm);
+    if (head_dim == 256) e = occupancy_of<256, 16>(gqa, &per_sm);
+    else if (head_dim == 128) e = occupancy_of<128, 16>(gqa, &per_sm);
+    else e = occupancy_of<64, 16>(gqa, &per_sm);
     if (e != cudaSuccess) return cuda_fail(e, "occupancy query");
     *n_cta_out = sms * per_sm;
     return TANGRAM_OK;
@@ -1368,7 +1378,8 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
         !t->tbl_indptr || !t->cluster_of || !t->slot_of || !t->perm)
         return fail(TANGRAM_ERR_INVALID_ARG, "upload: NULL argument");
     if (p->n_items > INT32_MAX) return fail(TANGRAM_ERR_INVALID_ARG, "upload: more than 2^31 items");
-    if (t->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "upload: page size %d (kernels need 16)", t->P);
+    if (t->P != 16 && t->P != 32) return fail(TANGRAM_ERR_INVALID_ARG, "upload: page size %d (kernels need 16 or 32)", t->P);
+    const int kPage = t->P;
     const BlobLayout lay = blob_layout(t, p);
     const size_t need = lay.total;
     if (bytes < need) return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "upload: blob %zu < %zu bytes", bytes, need);
@@ -1542,7 +1553,9 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     if (!dp || !out || !lse || (split && (!q || !kv_pool))) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: NULL argument");
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: head_dim %d not in {64, 128, 256}", d);
-    if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d (kernels need 16)", dp->P);
+    if (!page_supported(dp->P, d))
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: page size %d at head_dim %d (kernels need 16, or 32 at head_dim <= 128)",
+                    dp->P, d);
     if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || Hq / dp->H > max_gqa(d))
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: Hq=%d H=%d (need Hq %% H == 0 and Hq/H <= %d at head_dim %d)", Hq,
                     dp->H, max_gqa(d), d);
@@ -1563,7 +1576,7 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     CUtensorMap map;
     std::memset(&map, 0, sizeof map);
     if (split) {
-        const int rc = make_kv_map(&map, kv_pool, n_pool_pages, dp->Hp, d);
+        const int rc = make_kv_map(&map, kv_pool, n_pool_pages, dp->Hp, d, dp->P);
         if (rc != TANGRAM_OK) return rc;
     }
 
@@ -1593,14 +1606,21 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     }
     prm.pdl = (step.flags & TANGRAM_STEP_OVERLAP) ? 1 : 0;
 
-    if (d == 256) prm.n_stages = Smem<256>::max_stages(G), prm.n_qslots = Smem<256>::max_qslots(prm.n_stages, G);
-    else if (d == 128) prm.n_stages = Smem<128>::max_stages(G), prm.n_qslots = Smem<128>::max_qslots(prm.n_stages, G);
-    else prm.n_stages = Smem<64>::max_stages(G), prm.n_qslots = Smem<64>::max_qslots(prm.n_stages, G);
     const float scale = sm_scale != 0.f ? sm_scale : 1.f / std::sqrt(static_cast<float>(d));
     prm.scale_log2 = scale * 1.4426950408889634f;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (d == 256) return launch_decode<256>(dp, prm, map, st, which);
-    return d == 128 ? launch_decode<128>(dp, prm, map, st, which) : launch_decode<64>(dp, prm, map, st, which);
+    auto go = [&](auto tag) {
+        using L = decltype(tag);
+        prm.n_stages = L::max_stages(G), prm.n_qslots = L::max_qslots(prm.n_stages, G);
+        return 0;
+    };
+    if (dp->P == 32) {
+        if (d == 128) return go(Smem<128, 32>()), launch_decode<128, 32>(dp, prm, map, st, which);
+        return go(Smem<64, 32>()), launch_decode<64, 32>(dp, prm, map, st, which);
+    }
+    if (d == 256) return go(Smem<256, 16>()), launch_decode<256, 16>(dp, prm, map, st, which);
+    if (d == 128) return go(Smem<128, 16>()), launch_decode<128, 16>(dp, prm, map, st, which);
+    return go(Smem<64, 16>()), launch_decode<64, 16>(dp, prm, map, st, which);
 }
 
 extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const void* kv_pool,
@@ -1702,7 +1722,8 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: NULL argument");
     if (d != 64 && d != 128 && d != 256)
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: head_dim %d not in {64, 128, 256}", d);
-    if (dp->P != kPage) return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: page size %d (kernels need 16)", dp->P);
+    if (!page_supported(dp->P, d))
+        return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: page size %d at head_dim %d (kernels need 16, or 32 at head_dim <= 128)", dp->P, d);
     if (n_pool_pages < 1 || n_pool_pages < dp->min_pool_pages)
         return fail(TANGRAM_ERR_INVALID_ARG, "append_kv: kv_pool has %lld pages, the tables need %lld", (long long)n_pool_pages,
                     (long long)dp->min_pool_pages);
@@ -1712,7 +1733,7 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
     const int n_seq = dp->R * dp->H;
     tangram_append_kernel<<<(n_seq + 3) / 4, 128, 0, static_cast<cudaStream_t>(stream)>>>(
         reinterpret_cast<const int4*>(dp->seq_info), dp->seq_cap, dp->tbl_pages, static_cast<const uint4*>(k_new),
-        static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d);
+        static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d, dp->P);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
     return TANGRAM_OK;

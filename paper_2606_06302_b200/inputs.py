@@ -68,19 +68,21 @@ def _jitter(rng: np.random.Generator, ratio_h: np.ndarray, R: int, hw: float) ->
     return np.minimum(1.0, ratio_h[None, :] * (1.0 + u))
 
 
-def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1, layer: int = 0) -> Workload:
+def make_workload(name: str, *, R: Optional[int] = None, ctx_div: int = 1, layer: int = 0,
+                  page_size: Optional[int] = None) -> Workload:
     """Build config `name` (one of CONFIG_NAMES).  `R` overrides the batch size and
     `ctx_div` divides every context length (scaled-down parity cases); the default
     arguments give the full BASELINE.json configuration.  `layer` > 0 draws another layer of the
     same shape (its own head ratios, i.e. its own budgets, clusters and plan) for multi-layer
-    decode loops: seed + 1000 * layer; the context lengths of layer 0 are kept (same requests)."""
+    decode loops: seed + 1000 * layer; the context lengths of layer 0 are kept (same requests).
+    `page_size` overrides P = 16 (BASELINE.json) for the P = 32 variants of the configs."""
     idx = (CONFIG_NAMES + EXTRA_CONFIG_NAMES).index(name)
     seed = SEED_BASE + idx
     if layer:
-        base = make_workload(name, R=R, ctx_div=ctx_div)
+        base = make_workload(name, R=R, ctx_div=ctx_div, page_size=page_size)
         seed += 1000 * layer
     rng = np.random.default_rng(seed)
-    P, alpha, g = 16, 2.0, 64
+    P, alpha, g = page_size or 16, 2.0, 64
 
     if name == "tiny":
         R0, Hq, H, d, C, hw = 2, 4, 2, 64, 2, 0.05

@@ -281,7 +281,8 @@ def test_random_sweep_compaction_and_implicit_ratios():
         C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
         R = int(rng.integers(1, 4))
         wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=1, d=d, C=C,
-                                    max_ctx=int(rng.choice([20, 200, 1100, 2100, 6000])))
+                                    max_ctx=int(rng.choice([20, 200, 1100, 2100, 6000])),
+                                    P=int(rng.choice([16, 32])) if d <= 128 else 16)
         if rng.random() < 0.3:
             wl.demand[rng.integers(R), rng.integers(H)] = 0
         B, res, kv, t, n_pool, dp = setup(wl)
@@ -302,15 +303,15 @@ def test_random_sweep_compaction_and_implicit_ratios():
         assert np.array_equal(cnt.cpu().numpy(), ref_cnt) and rat.cpu().numpy().tobytes() == ref_rat.tobytes(), case
 
 
-@pytest.mark.parametrize("seed,d,C", [(81, 128, 2), (82, 64, 4), (83, 256, 1)])
-def test_chunked_prefill_compaction_bit_exact(seed, d, C):
+@pytest.mark.parametrize("seed,d,C,P", [(81, 128, 2, 16), (82, 64, 4, 16), (83, 256, 1, 16), (84, 128, 2, 32), (85, 64, 1, 32)])
+def test_chunked_prefill_compaction_bit_exact(seed, d, C, P):
     """Compression fused into chunked prefill (:152): four chunks of ragged lengths compressed one after the other,
     each appended behind the previous ones (chunk boundaries fall inside pages); pool, lengths and index lists
     bit-exact against oracle O11 after every chunk; then decode attention over the result; then an over-full
     chunk is clamped and counted."""
     R, H = 3, 4
     rng = np.random.default_rng(seed)
-    wl = I.make_random_workload(seed, R=R, H=H, G=2, d=d, C=C, max_ctx=100)
+    wl = I.make_random_workload(seed, R=R, H=H, G=2, d=d, C=C, max_ctx=100, P=P)
     chunk_lens = [rng.integers(1, 700, size=R).astype(np.int32) for _ in range(4)]
     ratios = rng.uniform(0.05, 1.0, size=H)
     keeps = [np.minimum(cl[:, None], np.ceil(cl[:, None] * ratios[None, :] * rng.uniform(0.5, 1.0, size=(R, H)))).astype(np.int32)
@@ -318,12 +319,12 @@ def test_chunked_prefill_compaction_bit_exact(seed, d, C):
     keeps[1][0, 1] = 0
     total = sum(keeps)
     B = np.clip(total.max(0) / sum(chunk_lens).max(), 0.01, 1.0)
-    need = T.tangram_pages_needed(B, total, C, 16)
-    t, _ = T.tangram_build_ragged_tables(B, total, C, 16, np.random.default_rng(seed).permutation(need + 3).astype(np.int32))
+    need = T.tangram_pages_needed(B, total, C, P)
+    t, _ = T.tangram_build_ragged_tables(B, total, C, P, np.random.default_rng(seed).permutation(need + 3).astype(np.int32))
     pl = T.tangram_plan_partitions(t, B, total, 148, 64, 1, T.MODE_BALANCED, 0, T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS)
     dp = T.tangram_upload(t, pl)
     g = torch.Generator(device="cuda").manual_seed(seed)
-    pool = torch.randn(need + 3, t.Hp, 2, 16, d, generator=g, device="cuda").bfloat16()
+    pool = torch.randn(need + 3, t.Hp, 2, P, d, generator=g, device="cuda").bfloat16()
     ref_pool, ref_kv = bits(pool).copy(), np.zeros((R, H), dtype=np.int32)
     kv_dev = torch.zeros(R, H, dtype=torch.int32, device="cuda")
     clamped = torch.zeros(1, dtype=torch.int32, device="cuda")
@@ -353,7 +354,7 @@ def test_chunked_prefill_compaction_bit_exact(seed, d, C):
     assert np.abs(lse.cpu().numpy() - ref_lse).max() <= 1e-3
     # one more chunk does not fit any more: every head is clamped to the room its table has left (:176)
     rows = np.arange(R)[:, None] * t.C + t.cluster_of[None, :]
-    room = ((t.tbl_indptr[rows + 1] - t.tbl_indptr[rows]) * 16 - total).astype(np.int32)
+    room = ((t.tbl_indptr[rows + 1] - t.tbl_indptr[rows]) * P - total).astype(np.int32)
     cl, kp = chunk_lens[0], np.minimum(chunk_lens[0][:, None], room + 5).astype(np.int32)
     eff = np.minimum(kp, room)
     T.tangram_compact_topk_chunk(dp, scores[:, :, :int(cl.max())].contiguous(), kd[:, :, :int(cl.max())].contiguous(),

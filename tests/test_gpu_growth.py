@@ -153,6 +153,14 @@ def test_decode_step_equals_extend_append_attend(name, kw):
     assert over == 0 and starved == 0 and np.array_equal(ref_kv, kv + 40)
 
 
+def test_decode_step_page_size_32():
+    """The fused step on 32-token pages: growth hands out a page every 32 tokens per row."""
+    wl = I.make_workload("8b", R=3, ctx_div=32, page_size=32)
+    B, kv, t, to, free = growable_setup(wl, headroom=3)
+    ref_kv, over, starved = run_decode_steps(wl, B, kv, t, to, free, steps=70)
+    assert over == 0 and starved == 0
+
+
 def test_decode_step_small_grid_and_static_plan():
     """W = 1 (the single CTA merges AND grows) and W = 5 with a static plan."""
     wl = I.make_random_workload(41, R=3, H=4, G=2, d=128, C=2, max_ctx=300)

@@ -121,8 +121,11 @@ def test_scaled_configs(name, kw):
                                             # GQA groups of 9..16 query heads: both halves of the mma A operand
                                             (13, 2, 2, 9, 128, 1), (14, 2, 4, 16, 128, 2), (15, 3, 2, 12, 64, 2),
                                             (16, 1, 1, 16, 64, 1), (17, 2, 2, 13, 128, 2)])
-def test_random_shapes(seed, R, H, G, d, C):
-    wl = I.make_random_workload(seed, R=R, H=H, G=G, d=d, C=C, max_ctx=900)
+@pytest.mark.parametrize("P", [16, 32])
+def test_random_shapes(seed, R, H, G, d, C, P):
+    if P == 32 and d == 256:
+        pytest.skip("P = 32 is instantiated for d <= 128")
+    wl = I.make_random_workload(seed, R=R, H=H, G=G, d=d, C=C, max_ctx=900, P=P)
     B, res, kv, t, n_pool = setup(wl)
     q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
     run_modes(wl, B, kv, t, q, pool, Ws=(3, 40))
@@ -453,7 +456,7 @@ def test_pinned_host_q_and_outputs_zero_copy():
 
 
 def test_random_sweep_of_shapes_plans_and_runtime_lengths():
-    """300 seeded cases over (R, H, G 1..16 (1..8 at d = 256), d, clusters, context, W, mode, c0, granule, dynamic tail, FILL_GROUP,
+    """300 seeded cases over (R, H, G 1..16 (1..8 at d = 256), d, page size 16 / 32 (16 at d = 256), clusters, context, W, mode, c0, granule, dynamic tail, FILL_GROUP,
     empty heads, open-ended run-time lengths), every one against the oracle at the BASELINE tolerances, each
     plan launched twice (the scheduler counters re-arm themselves)."""
     rng = np.random.default_rng(20260630)
@@ -463,15 +466,16 @@ def test_random_sweep_of_shapes_plans_and_runtime_lengths():
         G = int(rng.integers(1, 9 if d == 256 else 17))
         C = int(rng.choice([c for c in (1, 2, 4, 8) if H % c == 0]))
         R = int(rng.integers(1, 6))
+        P = int(rng.choice([16, 32])) if d <= 128 else 16
         wl = I.make_random_workload(int(rng.integers(1 << 30)), R=R, H=H, G=G, d=d, C=C,
-                                    max_ctx=int(rng.choice([40, 300, 1500, 4000])))
+                                    max_ctx=int(rng.choice([40, 300, 1500, 4000])), P=P)
         if rng.random() < 0.3:
             wl.demand[rng.integers(R), rng.integers(H)] = 0
         B, res, kv, t, n_pool = setup(wl, flags=int(rng.random() < 0.2))
         W = int(rng.choice([1, 2, 7, 33, 148, 148, 148, 200]))
         mode, c0 = int(rng.choice([0, 0, 0, 1, 2])), int(rng.integers(0, 3))
         dyn = (int(rng.integers(50, 950)), int(rng.integers(1, 9))) if mode == 0 and rng.random() < 0.6 else (0, 0)
-        pl = T.tangram_plan_partitions(t, B, kv, W, int(rng.choice([16, 64, 64, 128])), c0, mode, 0, dyn[0], dyn[1])
+        pl = T.tangram_plan_partitions(t, B, kv, W, int(rng.choice([P, 64, 64, 128])), c0, mode, 0, dyn[0], dyn[1])
         dp = T.tangram_upload(t, pl)
         q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
         kv_run, kv_dev = kv, None
@@ -763,3 +767,34 @@ def test_decode_attention_host_entry(d, W):
     T.tangram_decode_attention_host(dp, q_h, q_stage, pool, out_h, lse_h, ws)
     torch.cuda.synchronize()
     assert torch.equal(out_h, out_d.cpu())
+
+
+@pytest.mark.parametrize("name,kw", [("8b", dict(R=4, ctx_div=8)), ("32b", dict(R=6, ctx_div=8)), ("skew", dict(R=2, ctx_div=8))])
+def test_scaled_configs_page_size_32(name, kw):
+    """The scaled BASELINE configs with 32-token pages (one 16 KB TMA box per (page, head) at d = 128, four consumer
+    warps, two 16-token passes per tile), all plan modes; then append + open-ended plan through page boundaries."""
+    wl = I.make_workload(name, page_size=32, **kw)
+    B, res, kv, t, n_pool = setup(wl)
+    assert t.P == 32
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    run_modes(wl, B, kv, t, q, pool, Ws=(7, n_cta(wl)))
+    rows = np.arange(wl.R)[:, None] * t.C + t.cluster_of[None, :]
+    cap = ((t.tbl_indptr[rows + 1] - t.tbl_indptr[rows]) * wl.P).astype(np.int32)
+    pl = T.tangram_plan_partitions(t, B, cap, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dp = T.tangram_upload(t, pl)
+    kv_dev = torch.from_numpy(np.maximum(cap - 3, 0).astype(np.int32)).cuda()
+    over = torch.zeros(1, dtype=torch.int32, device="cuda")
+    g = torch.Generator(device="cuda").manual_seed(5)
+    pool_bits, kv_ref, n_over = bits(pool).copy(), np.maximum(cap - 3, 0).astype(np.int32), 0
+    for step in range(5):
+        k_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+        v_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+        T.tangram_append_kv(dp, k_new, v_new, pool, kv_dev, over)
+        pool_bits, kv_ref, o = O.append_kv(pool_bits, oracle_tables(t), kv_ref, bits(k_new), bits(v_new))
+        n_over += o
+        out, lse = T.tangram_decode_attention(dp, q, pool, kv_len=kv_dev)
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(pool), pool_bits) and np.array_equal(kv_dev.cpu().numpy(), kv_ref) and int(over.item()) == n_over
+        ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv_ref, wl.Hq, wl.d)
+        check(out, lse, ref_out, ref_lse, f"P=32 decode step {step}")
+    assert n_over > 0
