@@ -386,7 +386,8 @@ int tangram_download_tables(const tangram_device_plan* dp, tangram_tables* t, in
  *   kv_len_dev    device [R][H] i32 (required), read, then incremented
  *   flags         TANGRAM_STEP_OVERLAP: the caller guarantees that the work preceding this call on the stream
  *                 writes nothing this call reads except q, k_new and v_new (true for the layers of one decode
- *                 step).  The kernel is then launched with programmatic stream serialization and fetches its
+ *                 step, each with its own plan, pool and lengths; NOT true when the preceding launch is a step
+ *                 on the same plan -- it writes this call's lengths, tables and pool).  The kernel is then launched with programmatic stream serialization and fetches its
  *                 work lists, page ids and first KV tiles while its predecessor drains; it waits for the
  *                 predecessor (griddepcontrol.wait) before touching q / k_new / v_new.
  *   all other arguments as for tangram_decode_attention.

@@ -182,6 +182,27 @@ def test_split_then_merge_entry_points():
         check(out2, lse2, ref_out, ref_lse, f"decode_attention dyn={dyn}")
 
 
+def test_merge_partials_takes_16_byte_aligned_outputs():
+    """tangram_merge_partials reads neither q nor the pool: an `out` that is 16-byte but not 128-byte aligned (legal
+    per tangram.h) must be accepted (round 1 ran it through the pool's alignment check)."""
+    wl = I.make_workload("8b", R=2, ctx_div=16)
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    pl = T.tangram_plan_partitions(t, B, kv, 19, wl.granule, 1, T.MODE_BALANCED)
+    dp = T.tangram_upload(t, pl)
+    ws = torch.zeros(T.tangram_workspace_bytes(pl.n_part_slots, wl.G, wl.d), dtype=torch.uint8, device="cuda")
+    raw = torch.zeros(q.numel() * 2 + 256, dtype=torch.uint8, device="cuda")
+    off = (16 - raw.data_ptr() % 128) % 128                       # data_ptr + off is 16 (mod 128)
+    out = raw[off:off + q.numel() * 2].view(torch.bfloat16).view(q.shape)
+    assert out.data_ptr() % 128 == 16
+    lse = torch.zeros(wl.R, wl.Hq, device="cuda")
+    T.tangram_decode_partials(dp, q, pool, out, lse, ws)
+    T.tangram_merge_partials(dp, out, lse, ws)
+    torch.cuda.synchronize()
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    check(out, lse, ref_out, ref_lse, "merge into a 16-byte aligned buffer")
+
+
 def test_fill_group_policy():
     wl = I.make_workload("8b", R=2, ctx_div=16)
     B, res, kv, t, n_pool = setup(wl, flags=T.FILL_GROUP, identity=True)
