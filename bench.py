@@ -35,11 +35,12 @@ FALLBACK_PEAK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 
 
 def csrc_hash() -> str:
-    """sha256 (first 16 hex digits) over the kernel sources: ties a committed ncu capture to the code it measured."""
+    """sha256 (first 16 hex digits) over the decode kernel's sources (tangram_decode.cu + tangram_internal.h): ties a
+    committed ncu capture of that kernel to the code it measured."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2606_06302_b200", "csrc")
-    for fn in sorted(os.listdir(d)):
+    for fn in ("tangram_decode.cu", "tangram_internal.h"):
         h.update(fn.encode())
         h.update(open(os.path.join(d, fn), "rb").read())
     return h.hexdigest()[:16]

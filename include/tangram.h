@@ -162,10 +162,12 @@ int tangram_plan_partitions(const tangram_tables* t, const double* B, const int3
                             int32_t mode, int32_t static_splits, int32_t dyn_permille, int32_t dyn_rounds,
                             tangram_plan* out);
 
-/* Default dynamic tail for tangram_plan_partitions (a measured tuning rule, not from the paper): (500, 6) when the
- * batch has at least 32 cost units (granules of granule_tokens + overhead_granules per non-empty sequence) per
- * worker, else (0, 0) -- with little work per CTA the purely static plan is faster (no list claims, fewer parts to
- * merge: 8b-shaped batch of 1: 18.5 us against 22.5 us; 32 requests: the tail wins, 127 us against 140 us).
+/* Default dynamic tail for tangram_plan_partitions (a measured tuning rule, not from the paper), by the cost units
+ * (granules of granule_tokens + overhead_granules per non-empty sequence) a worker gets: fewer than 48 -> (0, 0), the
+ * purely static plan (with little work per CTA the claims and the extra parts to merge cost more than the balance
+ * brings: 8b shape, 4 requests: 30.7 us static against 34.8 us with a tail); 48 .. 383 -> (500, 4); 384 and more ->
+ * (500, 6) (round-2 sweep on B200, reading A32: e.g. 32b shape with 16 requests 113 us with (500, 4), 119 us
+ * with (500, 6), 127 us static).
  * kv_len host [R][H] i32.  Errors: INVALID_ARG. */
 int tangram_default_dynamic_tail(const int32_t* kv_len, int32_t R, int32_t H, int32_t n_workers, int32_t granule_tokens,
                                  int32_t overhead_granules, int32_t* dyn_permille_out, int32_t* dyn_rounds_out);

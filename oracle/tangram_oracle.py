@@ -310,14 +310,18 @@ def list_weights(n_workers: int, dyn_permille: int, dyn_rounds: int) -> List[int
 
 def default_dynamic_tail(kv_len, n_workers: int, granule: int, overhead_granules: int) -> Tuple[int, int]:
     """Default (dyn_permille, dyn_rounds) of the BALANCED plan (reading A32, a measured tuning rule, not
-    from the paper): the dynamic tail (500, 6) pays off once a CTA streams long enough for the per-SM bandwidth
-    differences to matter; with fewer than 32 cost units (granules + per-sequence overhead) per worker the purely
-    static plan (0, 0) is faster (no claims, fewer parts to merge)."""
+    from the paper), by the cost units (granules + per-sequence overhead) a worker gets: fewer than 48 -- the purely
+    static plan (0, 0) (no claims, fewer parts to merge); 48 to 383 -- half of the cost axis handed out in 4 rounds;
+    384 and more -- in 6 rounds (the longer a CTA streams, the finer the last lists may be)."""
     total = 0
     for n in np.asarray(kv_len, dtype=np.int64).reshape(-1):
         u = -(-int(n) // granule)
         total += u + (overhead_granules if u > 0 else 0)
-    return (500, 6) if total >= 32 * n_workers else (0, 0)
+    if total < 48 * n_workers:
+        return (0, 0)
+    if total < 384 * n_workers:
+        return (500, 4)
+    return (500, 6)
 
 
 def plan_partitions(t: Tables, B, kv_len, n_workers: int, granule: int, overhead_granules: int,

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libtangram.so")
 OK, ERR_INVALID_ARG, ERR_OUT_OF_PAGES, ERR_BUFFER_TOO_SMALL, ERR_CUDA = 0, -1, -2, -3, -4
 FILL_GROUP = 1
 MODE_BALANCED, MODE_SPLITMAP, MODE_STATIC_EVEN = 0, 1, 2
-# dynamic tail of the BALANCED plan used by bench.py / smoke (tuned on B200)
+# the finest dynamic tail tangram_default_dynamic_tail picks (large batches; tuned on B200)
 DEFAULT_DYN_PERMILLE, DEFAULT_DYN_ROUNDS = 500, 6
 GROUP_CLUSTERED, GROUP_ADJACENT = 0, 1
 MODE_NAMES = {MODE_BALANCED: "balanced", MODE_SPLITMAP: "splitmap", MODE_STATIC_EVEN: "static_even"}

@@ -477,7 +477,9 @@ extern "C" int tangram_default_dynamic_tail(const int32_t* kv_len, int32_t R, in
         const int64_t u = (kv_len[i] + (int64_t)granule_tokens - 1) / granule_tokens;
         total += u + (u > 0 ? overhead_granules : 0);
     }
-    const bool tail = total >= (int64_t)32 * n_workers;
-    *dyn_permille_out = tail ? 500 : 0, *dyn_rounds_out = tail ? 6 : 0;
+    // fewer than 48 cost units per worker: static; up to 384: half of the axis in 4 rounds; above: in 6 rounds
+    if (total < (int64_t)48 * n_workers) *dyn_permille_out = 0, *dyn_rounds_out = 0;
+    else if (total < (int64_t)384 * n_workers) *dyn_permille_out = 500, *dyn_rounds_out = 4;
+    else *dyn_permille_out = 500, *dyn_rounds_out = 6;
     return TANGRAM_OK;
 }

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 
 MAX_ABS, REL_L2, LSE_TOL = 2e-2, 5e-3, 1e-3
 ROW_REL_L2 = 5e-3      # the same relative-L2 bound applied to EVERY (request, query head) output row on its own
-DYN_PERMILLE, DYN_ROUNDS = T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS     # bench.py's launch configuration
+DYN_PERMILLE, DYN_ROUNDS = T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS     # the finest tail the default rule uses
 
 
 def setup(wl, flags=0, identity=False):
@@ -300,7 +300,8 @@ def test_full_size_sampled(name):
     B, res, kv, t, n_pool = setup(wl)
     q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
     W = n_cta(wl)
-    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    dyn = T.tangram_default_dynamic_tail(kv, W, wl.granule, 1)            # what bench.py plans with
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, *dyn)
     dp = T.tangram_upload(t, pl)
     out, lse = T.tangram_decode_attention(dp, q, pool)
     torch.cuda.synchronize()
@@ -746,7 +747,8 @@ def test_full_size_constant_v_per_head_is_exact(name):
             if int(t.cluster_of[h]) == c:
                 pool[pg, int(t.slot_of[h]), 1] = float(h + 1)
     W = n_cta(wl)
-    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, DYN_PERMILLE, DYN_ROUNDS)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0,
+                                   *T.tangram_default_dynamic_tail(kv, W, wl.granule, 1))
     dp = T.tangram_upload(t, pl)
     out, lse = T.tangram_decode_attention(dp, q, pool)
     torch.cuda.synchronize()

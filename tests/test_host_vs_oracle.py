@@ -256,10 +256,13 @@ def test_default_dynamic_tail_rule():
     assert T.tangram_default_dynamic_tail(kv, 148, 64, 1) == (0, 0)                      # little work per CTA: static
     wl = I.make_workload("8b")
     _, _, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
-    assert T.tangram_default_dynamic_tail(kv, 148, 64, 1) == (T.DEFAULT_DYN_PERMILLE, T.DEFAULT_DYN_ROUNDS)
-    edge = np.full((1, 1), 64 * 31, dtype=np.int32)                                       # 31 granules + 1 overhead = 32
-    assert T.tangram_default_dynamic_tail(edge, 1, 64, 1) == O.default_dynamic_tail(edge, 1, 64, 1) == (500, 6)
-    assert T.tangram_default_dynamic_tail(edge - 64, 1, 64, 1) == O.default_dynamic_tail(edge - 64, 1, 64, 1) == (0, 0)
+    assert T.tangram_default_dynamic_tail(kv, 148, 64, 1) == (500, 4)                    # 167 cost units per CTA
+    wl = I.make_workload("uniform")
+    _, _, kv = T.tangram_reserve_budgets(wl.mu, wl.sigma, wl.alpha, wl.ctx_len, wl.demand)
+    assert T.tangram_default_dynamic_tail(kv, 148, 64, 1) == (500, 6)                    # 900 cost units per CTA
+    for units, want in ((47, (0, 0)), (48, (500, 4)), (383, (500, 4)), (384, (500, 6))):
+        edge = np.full((1, 1), 64 * (units - 1), dtype=np.int32)                          # units - 1 granules + 1 overhead
+        assert T.tangram_default_dynamic_tail(edge, 1, 64, 1) == O.default_dynamic_tail(edge, 1, 64, 1) == want
 
 
 # ---------------------------------------------------------------------------- NEXT-4: growable tables (host path)
