@@ -255,7 +255,8 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *   workspace device, >= tangram_workspace_bytes(dp->n_part_slots, G, d), 16-byte aligned
  *   worker_ns device [n_static][4] u64 or NULL: if given, every CTA stores its globaltimer stamps
  *             {start, end of its work lists, grid barrier passed, merges done} (the last two only when
- *             the merge runs inside the decode grid); the per-CTA elapsed-time spread of BASELINE.json
+ *             the merge runs inside the decode grid; without it -- tangram_decode_partials -- the third slot
+ *             holds the id of the SM the CTA ran on, %smid); the per-CTA elapsed-time spread of BASELINE.json
  *             is measured from the first two.
  * A device plan carries the launch's scheduler counters: launches on the SAME plan must be ordered (one stream, or
  * events between streams); different plans (e.g. one per layer) may run concurrently.

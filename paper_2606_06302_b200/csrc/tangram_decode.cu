@@ -562,7 +562,12 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     auto qfull_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + s) * 8; };
     auto qempty_bar = [&](int s) { return bars + (2 * kNW * kMaxStages + kMaxQSlots + s) * 8; };
 
-    if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x] = globaltimer();
+    if (TIMED && threadIdx.x == 0) {
+        p.worker_ns[4 * blockIdx.x] = globaltimer();
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        p.worker_ns[4 * blockIdx.x + 2] = smid;  // kept by tangram_decode_partials; the in-grid merge overwrites it
+    }
     // The CTA's own list head (plan data) is on its way while the barriers are set up: the first TMA of the CTA
     // is then one memory round trip behind the start of the CTA, not two.
     int head_word = 0;
