@@ -203,9 +203,9 @@ typedef struct tangram_device_plan {
                                      the page, row index r*C + c} */
     const int64_t* part_indptr;   /* device [R*H+1] */
     const int32_t* tbl_pages;     /* device page ids */
-    int32_t* sched;               /* device [4]: list-claim / CTAs-done counters of the dynamic tail and the
-                                     grid-barrier counters of the in-kernel merge; zero between launches
-                                     (the kernel re-arms them itself) */
+    int32_t* sched;               /* device [8]: list-claim / CTAs-done counters of the dynamic tail, the grid-barrier
+                                     counters of the in-kernel merge (zero between launches; the kernel re-arms
+                                     them itself) and the launch number of the host-query staging */
     int64_t max_merge_parts;      /* most parts any sequence has (sizes the column split of the big-record merge) */
     int64_t min_pool_pages;       /* largest page id in the tables at upload + 1: the device calls return INVALID_ARG
                                      for a kv_pool with fewer pages */
@@ -226,7 +226,7 @@ typedef struct tangram_device_plan {
 int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
                    void* stream, tangram_device_plan* dp);
 
-/* Zeroes the launch-state counters of an uploaded plan (dp->sched) on `stream`.  The kernels re-arm the counters
+/* Zeroes the launch-state counters of an uploaded plan (dp->sched, dp->q_flags) on `stream`.  The kernels re-arm the counters
  * themselves at the end of every launch that runs to completion; this call is for recovery after a launch that
  * did not (an aborted process, a fault), or after two launches on one plan were wrongly overlapped. */
 int tangram_reset_plan(const tangram_device_plan* dp, void* stream);
@@ -236,7 +236,8 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
 
 /* a4 + a5  One layer, whole batch: split-KV decode kernel over the work lists, then the LSE merge -- inside the
  * same persistent grid after a grid barrier (ONE cooperative launch); the stand-alone merge kernel follows as a
- * second launch only when the grid cannot be co-resident (n_workers > SMs x occupancy) or d = 256.
+ * second launch only when the grid cannot be co-resident (n_workers > SMs x occupancy), at d = 256, or when a merge
+ * record is wider than the CTA (G x d/4 > consumer threads: d = 128 with G > 8, or G > 4 on 32-token pages).
  * Asynchronous on `stream`; CUDA-graph capturable; no host work besides the launch.
  *
  *   dp        from tangram_upload (host struct holding device pointers)
