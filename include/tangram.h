@@ -235,9 +235,10 @@ int tangram_reset_plan(const tangram_device_plan* dp, void* stream);
 size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_dim);
 
 /* a4 + a5  One layer, whole batch: split-KV decode kernel over the work lists, then the LSE merge -- inside the
- * same persistent grid after a grid barrier (ONE cooperative launch); the stand-alone merge kernel follows as a
- * second launch only when the grid cannot be co-resident (n_workers > SMs x occupancy), at d = 256, or when a merge
- * record is wider than the CTA (G x d/4 > consumer threads: d = 128 with G > 8, or G > 4 on 32-token pages).
+ * same persistent grid after a grid barrier (ONE launch: cooperative when the grid fits on the device, else the
+ * last SMs x occupancy CTAs to finish do the merging); the stand-alone merge kernel follows as a second launch only
+ * at d = 256 or when a merge record is wider than the CTA (G x d/4 > consumer threads: d = 128 with G > 8, or G > 4
+ * on 32-token pages).
  * Asynchronous on `stream`; CUDA-graph capturable; no host work besides the launch.
  *
  *   dp        from tangram_upload (host struct holding device pointers)

@@ -87,7 +87,7 @@ struct DecodeParams {
     const int32_t* kv_len;      // [R*H] run-time lengths (open-ended plan) or nullptr: items are taken as planned
     int32_t H, R;
     int32_t Hq, G, Hp, n_stages, n_qslots, n_lists;
-    int32_t tail_merge, n_merge_units, n_merge_small, merge_split;
+    int32_t tail_merge, n_merge_units, n_merge_small, merge_split, merge_ctas;
     float scale_log2;
     // fused decode step (tangram_decode_step): KV append by the CTA that streams the sequence's last item, the
     // length update and the block-table growth for the next step after the grid barrier; all nullptr / 0 otherwise
@@ -1002,57 +1002,68 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
     if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 1] = globaltimer();
 
     if (p.tail_merge) {
-        // a5 inside the persistent grid (cooperative launch: all CTAs are co-resident).  Grid barrier over
-        // the consumer threads, then CTA b merges units b, b + grid, ... -- no second launch, and the
-        // merges of many sequences run on all SMs at once.
-        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*grid)*K + sub, no
-        // barrier inside; the first record is fetched BEFORE the grid barrier (plan data).  Big records
-        // (more than kMergeBigParts parts) go first, one query head per unit, CTAs 0 .. n_big_units-1 ...
-        // In a fused decode step the LAST CTA of the grid does not merge: it updates the lengths and grows the
-        // block tables for the next step while the others merge (`grid` = the CTAs that merge).
+        // a5 inside the persistent grid.  Every CTA takes a ticket when its work lists are done (its partials are
+        // published by the fence before the ticket).  The last `merge_ctas` arrivals stay: they wait until all
+        // tickets are taken -- the grid barrier -- and merge unit rank, rank + M, ... among themselves; earlier
+        // arrivals, if any, leave at once.  With merge_ctas = grid (the normal case) this is a plain grid barrier
+        // followed by merges on all SMs.  The wait cannot deadlock as long as merge_ctas CTAs fit on the device
+        // together (checked by the launcher): whoever waits is running, and whoever has not arrived yet is running or
+        // will be scheduled on a slot a finished CTA left.  The launcher still asks for a cooperative launch, except
+        // behind a programmatic dependency, where the plain launch saves ~2 us per layer-step.
+        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*M)*K + sub, no barrier inside; the
+        // first record is fetched before the wait (plan data).  Big records (more than kMergeBigParts parts) go
+        // first, one query head per unit.
+        // In a fused decode step the very last arrival does not merge: it updates the lengths and grows the
+        // block tables for the next step while the others merge.
         const bool fused = p.k_new != nullptr;
         const int grid_all = static_cast<int>(gridDim.x);
-        const int grid = fused && grid_all > 1 ? grid_all - 1 : grid_all;
-        const bool merger = static_cast<int>(blockIdx.x) < grid;
-        const int n_elem = G * (D / 4), K = (kNW * 32) / n_elem, sub = threadIdx.x / n_elem;
-        const int n_big_units = p.n_merge_units - p.n_merge_small;
-        // ... so the small records start at the CTA after the last one holding a big unit
-        const int first = (static_cast<int>(blockIdx.x) - n_big_units % grid + grid) % grid;
-        int sidx = first * K + sub;
-        int4 rec = make_int4(0, 0, 0, 0);
-        if (merger && sub < K && sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
+        const int n_late = min(grid_all, p.merge_ctas);  // CTAs that stay for the tail phase
+        int* s_ticket = reinterpret_cast<int*>(smem + L::off_flag(NS, G, NQ));
         __threadfence();
         named_bar_sync(1, kNW * 32);
-        if (threadIdx.x == 0) {
-            atomicAdd(p.sched + 2, 1);
-            int seen;
-            do {
-                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
-                if (TANGRAM_BARRIER_NANOSLEEP > 0 && seen < grid_all) __nanosleep(TANGRAM_BARRIER_NANOSLEEP);
-            } while (seen < grid_all);
-            __threadfence();
-        }
+        if (threadIdx.x == 0) *s_ticket = atomicAdd(p.sched + 2, 1);
         named_bar_sync(1, kNW * 32);
-        if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
-        float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
-        if (merger) {
-            for (int u = blockIdx.x; u < n_big_units; u += grid)
-                merge_big_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4),
-                                                  G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
-            if (sub < K)
-                for (; sidx < p.n_merge_small; sidx += grid * K) {
-                    merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
-                    if (sidx + grid * K < p.n_merge_small)
-                        rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
-                }
-        }
-        if (fused && (!merger || grid_all == 1)) {
-            // every append of this step happened before the barrier: lengths, then the pages of the next step
+        const int rank = *s_ticket - (grid_all - n_late);  // < 0: an early arrival
+        if (rank >= 0) {
+            const int grid = fused && n_late > 1 ? n_late - 1 : n_late;  // the CTAs that merge
+            const bool merger = rank < grid;
+            const int n_elem = G * (D / 4), K = (kNW * 32) / n_elem, sub = threadIdx.x / n_elem;
+            const int n_big_units = p.n_merge_units - p.n_merge_small;
+            // ... so the small records start at the CTA after the last one holding a big unit
+            const int first = (rank - n_big_units % grid + grid) % grid;
+            int sidx = first * K + sub;
+            int4 rec = make_int4(0, 0, 0, 0);
+            if (merger && sub < K && sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
+            if (threadIdx.x == 0) {
+                int seen;
+                do {
+                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
+                    if (TANGRAM_BARRIER_NANOSLEEP > 0 && seen < grid_all) __nanosleep(TANGRAM_BARRIER_NANOSLEEP);
+                } while (seen < grid_all);
+                __threadfence();
+            }
             named_bar_sync(1, kNW * 32);
-            step_lengths<kNW * 32, true>(p.grow, threadIdx.x);
-            if (p.grow.free_pages) extend_rows<kNW * 32, true>(p.grow, kPage, threadIdx.x, reinterpret_cast<int*>(scratch_o));
+            if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
+            float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
+            if (merger) {
+                for (int u = rank; u < n_big_units; u += grid)
+                    merge_big_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4),
+                                                      G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
+                if (sub < K)
+                    for (; sidx < p.n_merge_small; sidx += grid * K) {
+                        merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
+                        if (sidx + grid * K < p.n_merge_small)
+                            rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
+                    }
+            }
+            if (fused && (!merger || n_late == 1)) {
+                // every append of this step happened before the barrier: lengths, then the pages of the next step
+                named_bar_sync(1, kNW * 32);
+                step_lengths<kNW * 32, true>(p.grow, threadIdx.x);
+                if (p.grow.free_pages) extend_rows<kNW * 32, true>(p.grow, kPage, threadIdx.x, reinterpret_cast<int*>(scratch_o));
+            }
+            if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
         }
-        if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
         if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == grid_all - 1) {
             p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
             if (p.q_host) p.sched[4] += 1;   // ... and closes this launch's query-staging epoch
@@ -1163,8 +1174,8 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
     return TANGRAM_OK;
 }
 
-// -1: TANGRAM_STEP_OVERLAP not tried yet; 1: the driver took programmatic stream serialization next to the
-// cooperative attribute; 0: it refused (the flag is then ignored)
+// -1: TANGRAM_STEP_OVERLAP not tried yet; 1: the driver took the programmatic stream serialization attribute;
+// 0: it refused (the flag is then ignored)
 static int g_overlap_state = -1;
 
 // CTAs of the decode kernel that can be co-resident on the current device (SMs x occupancy).
@@ -1195,9 +1206,13 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     const bool fits = D <= 128 && prm.G * (D / 4) <= L::kNW * 32;
     if (want_tail_merge && fits && (cached_smem != smem || cached_dev != dev))
         cached_max = max_coresident<D, TIMED, NH, PAGE>(dev, smem), cached_smem = smem, cached_dev = dev;
-    prm.tail_merge = want_tail_merge && fits && dp->n_static <= cached_max;
+    // The ticket scheme of the tail phase only needs the CTAs that WAIT to fit on the device together: with a grid
+    // larger than that, the last `cached_max` arrivals merge (plain launch: a cooperative one would be refused).
+    const bool coresident = dp->n_static <= cached_max;
+    prm.tail_merge = want_tail_merge && fits && cached_max > 0;
+    prm.merge_ctas = std::min(dp->n_static, cached_max);
     *merged = prm.tail_merge;
-    if (prm.q_host && !prm.tail_merge) {
+    if (prm.q_host && !(prm.tail_merge && coresident)) {
         // no co-resident grid, no in-kernel staging: the staging kernel runs first and the decode kernel is
         // launched behind it with programmatic stream serialization (it waits before its first query load)
         const int rc = tangram_stage_from_host(const_cast<__nv_bfloat16*>(prm.q), prm.q_host, (size_t)prm.R * prm.Hq * D * 2, stream);
@@ -1206,14 +1221,16 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)dp->n_static), cfg.blockDim = dim3(L::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = stream;
+    // Programmatic dependent launch: if the driver refuses the attribute once, it is not asked again (a failing
+    // launch inside a stream capture would invalidate the capture).
+    if (g_overlap_state == 0) prm.pdl = 0;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeCooperative;
-    attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
+    // cooperative: the formal co-residency guarantee for the in-grid barrier; a plain launch behind a programmatic
+    // dependency (the barrier's ticket scheme only needs the grid to FIT, which was checked above)
+    attr[0].val.cooperative = (prm.tail_merge && coresident && !prm.pdl) ? 1 : 0;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
-    // Programmatic dependent launch next to the cooperative attribute: if the driver refuses the pair once, it is
-    // not asked again (a failing launch inside a stream capture would invalidate the capture).
-    if (g_overlap_state == 0) prm.pdl = 0;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
     e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH, PAGE>, map, prm);
     if (prm.pdl) {
@@ -1221,6 +1238,7 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
         else {
             (void)cudaGetLastError();
             g_overlap_state = 0, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
+            attr[0].val.cooperative = (prm.tail_merge && coresident) ? 1 : 0;
             e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH, PAGE>, map, prm);
         }
     }
