@@ -1,10 +1,14 @@
 // NEXT-2 of SURVEY.md §8(f): per-head Top-k selection (Eq. 4: I = Top(ceil(B N), s)) and
 // compaction K~ = K[I,:], V~ = V[I,:] (Eq. 1) into the ragged pages (:190).  Contract:
-// include/tangram.h (tangram_compact_topk).  Three launches on the caller's stream:
+// include/tangram.h (tangram_compact_topk).  Three launches on the caller's stream; the third is launched behind
+// the second by programmatic dependent launch and the two OVERLAP: a row's gather starts when that row's select is
+// done (per-row ready flags), so the issue-bound select hides behind the HBM-bound gather:
 //
 //   1. compact_prepare_kernel   one CTA: clamps keep[r][h] to [0, min(N_r, table capacity)] (the reserved
 //      budget is a hard capacity bound, :176), counts the clamped heads, and scans ceil(keep / P) into a
-//      tile index (tile = the P token slots of one (page, head)); zeroes the gather kernel's chunk counter.
+//      tile index (tile = the P token slots of one (page, head)) in QUEUE order -- the order in which the select
+//      kernel takes the rows and the gather kernel moves them; zeroes the counters and the rows' ready flags, and
+//      decides from the batch whether the call is gather-heavy (select and gather then share every SM).
 //   2. topk_select_kernel       one CTA (512 or 1024 threads, by row length) per (request, KV head): radix select
 //      (digits of 11, 11 and 10 bits, shared-memory atomic histograms, 16-byte loads) over a monotone integer image
 //      of the fp32 score finds the threshold key T and how many of the entries equal to T are kept (the lowest
@@ -14,17 +18,19 @@
 //      token indices in ascending order: the entry at token i goes to position (#greater before i) +
 //      min(#equal before i, need); every warp owns a contiguous segment, so that pass needs one block barrier in
 //      total.  Integer work on fp32 bit patterns: the result is the unique Top-k under the tie rule, bit-exact
-//      against the sort-based oracle.
+//      against the sort-based oracle.  A finished row is published with a release store to its ready flag.
 //   3. compact_gather_kernel    persistent grid, warps claim chunks of tiles from a global counter (the same
 //      run-time balancing as the decode kernel's dynamic tail: per-SM bandwidth differs on B200).  A warp
 //      moves one tile: up to P K rows and P V rows of d bf16 each, gathered with 16-byte loads (16 in
 //      flight per lane) and stored as two contiguous runs of the page.  HBM-bound: 4*d bytes read +
-//      4*d bytes written per retained token-head.
+//      4*d bytes written per retained token-head.  Before the first tile of a row the warp waits for the row's
+//      ready flag (acquire); the kernel's CTAs become resident as soon as every select CTA has started.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
 #include <cstdint>
+#include <cstdlib>
 
 #include "tangram.h"
 #include "tangram_internal.h"
@@ -35,24 +41,29 @@ constexpr int kCPage = 16;           // rows of a gather tile (= one page at P =
 constexpr int kSelBins = 2048;        // 11-bit digits
 constexpr int kSelCand = 4096;        // candidates (entries in the first digit's bin) the select kernel buffers
 constexpr int kSelLongRow = 49152;    // rows longer than this get 1024-thread CTAs, shorter ones 512 (two per SM)
-#ifndef TANGRAM_SEL_WIDE_ROWS
-#define TANGRAM_SEL_WIDE_ROWS 4
-#endif
-constexpr int kSelWideRows = TANGRAM_SEL_WIDE_ROWS;  // ... unless the batch has fewer rows than this per SM
 constexpr int kGatherThreads = 256;
 constexpr int kGatherChunk = 8;      // tiles claimed at once
 
-// Workspace (int32 words): [0] chunk counter of the gather, [1] total tiles, [2] row counter of the select, [3] pad,
-// then keep_eff[n_seq], base[n_seq] (tokens every head held before the call), tile_indptr[n_seq + 1] and
-// order[n_seq] (the rows, longest context first: the select kernel's queue).
+constexpr int kMaxSms = 256;          // per-SM slots of the workspace (B200: 148 SMs)
+// Cost model behind the gather-heavy decision (measured on B200, 8b shapes): the select kernel alone handles
+// ~150 scores per ns on the whole device, the gather moves ~6400 bytes per ns.
+constexpr long long kSelScoresPerNs = 150, kGatherBytesPerNs = 6400;
+
+// Workspace (int32 words): [0] chunk counter of the gather, [1] total tiles, [2] row counter of the select,
+// [3] 1 = gather-heavy call (one select CTA per SM stays, the others leave their registers to the gather), [4..7] pad;
+// then keep_eff[n_seq], base[n_seq] (tokens every head held before the call), tile_indptr[n_seq + 1] (first tile of
+// every QUEUE POSITION), order[n_seq] (the row at every queue position), ready[n_seq] (1 = the row's indices are
+// written) and sm_first[kMaxSms] (select CTAs that arrived on every SM).
 struct CompactWs {
     int32_t* counter;
     int32_t* keep_eff;
     int32_t* base;
     int32_t* tile_indptr;
     int32_t* order;
+    int32_t* ready;
+    int32_t* sm_first;
 };
-static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 4 + 4 * (size_t)n_seq + 1; }
+static __host__ __device__ inline size_t compact_ws_words(int64_t n_seq) { return 8 + 5 * (size_t)n_seq + 1 + kMaxSms; }
 
 // fp32 score -> uint32 key with the same order (larger score = larger key); -0.0 and +0.0 compare equal
 // as they do as fp32 values.
@@ -61,30 +72,77 @@ __device__ __forceinline__ uint32_t score_key(float x) {
     return u ^ (static_cast<uint32_t>(static_cast<int32_t>(u) >> 31) | 0x80000000u);
 }
 
+// overlap: 0 = never share the SMs (the select keeps all its CTAs), 1 = always, 2 = decide from the batch
 __global__ void __launch_bounds__(1024)
 compact_prepare_kernel(const int32_t* __restrict__ seq_cap, const int32_t* __restrict__ ctx_len,
                        const int32_t* __restrict__ keep, int32_t* __restrict__ kv_len, int n_seq, int H,
                        int32_t* __restrict__ counter, int32_t* __restrict__ keep_eff, int32_t* __restrict__ base,
-                       int32_t* __restrict__ tile_indptr, int32_t* __restrict__ order, int32_t* __restrict__ clamped) {
+                       int32_t* __restrict__ tile_indptr, int32_t* __restrict__ order, int32_t* __restrict__ ready,
+                       int32_t* __restrict__ sm_first, int32_t* __restrict__ clamped, int row_bytes, int overlap) {
     __shared__ int s_warp[32];
-    __shared__ int s_run, s_bad;
+    __shared__ int s_run, s_bad, s_heavy;
+    __shared__ unsigned long long s_kept, s_scored;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_run = 0, s_bad = 0;
+    if (tid == 0) s_run = 0, s_bad = 0, s_kept = 0ull, s_scored = 0ull;
+    for (int i = tid; i < kMaxSms; i += blockDim.x) sm_first[i] = 0;
     __syncthreads();
-    for (int first = 0; first < n_seq; first += blockDim.x) {
-        const int seq = first + tid;
-        int tiles = 0, bad = 0;
-        if (seq < n_seq) {
-            const int want = keep[seq];
-            const int have = kv_len ? kv_len[seq] : 0;  // chunked prefill: the rows go behind what the head holds
-            const int cap = min(ctx_len[seq / H], seq_cap[seq] - have);  // seq_cap: tokens the pages of the head's row hold
-            const int k = max(0, min(want, cap));
-            bad = k != want;
-            keep_eff[seq] = k;
-            base[seq] = have;
-            if (kv_len) kv_len[seq] = have + k;
-            tiles = (k + kCPage - 1) / kCPage;
+    // ---- per row: the clamped keep, where its rows go, the new length; batch totals for the cost model
+    unsigned long long kept = 0ull, scored = 0ull;
+    int bad = 0;
+    for (int seq = tid; seq < n_seq; seq += blockDim.x) {
+        const int want = keep[seq];
+        const int have = kv_len ? kv_len[seq] : 0;  // chunked prefill: the rows go behind what the head holds
+        const int N = ctx_len[seq / H];
+        const int cap = min(N, seq_cap[seq] - have);  // seq_cap: tokens the pages of the head's row hold
+        const int k = max(0, min(want, cap));
+        bad += k != want;
+        keep_eff[seq] = k;
+        base[seq] = have;
+        ready[seq] = 0;
+        if (kv_len) kv_len[seq] = have + k;
+        kept += static_cast<unsigned long long>(k);
+        if (k > 0 && k < N) scored += static_cast<unsigned long long>(N);  // rows that need a selection
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        kept += __shfl_xor_sync(0xffffffffu, kept, o), scored += __shfl_xor_sync(0xffffffffu, scored, o);
+        bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if (lane == 0) {
+        if (kept) atomicAdd(&s_kept, kept);
+        if (scored) atomicAdd(&s_scored, scored);
+        if (bad) atomicAdd(&s_bad, bad);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        // gather-heavy: the gather's estimated time is at least three times the select's.  Then one select CTA per SM
+        // is enough (at half the threads and next to a gather CTA it takes ~2.2 x as long: 8b 37 -> 77 us, and still
+        // ends long before the gather) and the gather gets the other half of the SM's registers from the start.
+        const unsigned long long gather_ns = s_kept * static_cast<unsigned long long>(row_bytes) / kGatherBytesPerNs;
+        const unsigned long long select_ns = s_scored / kSelScoresPerNs;
+        s_heavy = overlap == 1 || (overlap == 2 && gather_ns >= 3 * select_ns);
+    }
+    __syncthreads();
+    const bool heavy = s_heavy != 0;
+    // ---- the queue: requests by context length, all H rows of a request together (ties: lower request first).
+    // Gather-heavy: SHORTEST first, so that the first rows are ready after a few microseconds and the select's own
+    // tail (the long rows) hides behind the gather.  Otherwise longest first: longest-processing-time-first over the
+    // persistent select CTAs.
+    const int R = n_seq / H;
+    for (int r = tid; r < R; r += blockDim.x) {
+        const int n = ctx_len[r];
+        int rank = 0;
+        for (int o = 0; o < R; ++o) {
+            const int m = ctx_len[o];
+            rank += (heavy ? m < n : m > n) || (m == n && o < r);
         }
+        for (int h = 0; h < H; ++h) order[rank * H + h] = r * H + h;
+    }
+    __syncthreads();
+    // ---- exclusive scan of the tiles over the queue positions
+    for (int first = 0; first < n_seq; first += blockDim.x) {
+        const int pos = first + tid;
+        const int tiles = pos < n_seq ? (keep_eff[order[pos]] + kCPage - 1) / kCPage : 0;
         int incl = tiles;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -92,32 +150,18 @@ compact_prepare_kernel(const int32_t* __restrict__ seq_cap, const int32_t* __res
             if (lane >= o) incl += v;
         }
         if (lane == 31) s_warp[warp] = incl;
-        const unsigned badmask = __ballot_sync(0xffffffffu, bad);
-        if (lane == 0 && badmask) atomicAdd(&s_bad, __popc(badmask));
         __syncthreads();
         int before = s_run;
         for (int w = 0; w < warp; ++w) before += s_warp[w];
-        if (seq < n_seq) tile_indptr[seq] = before + incl - tiles;
+        if (pos < n_seq) tile_indptr[pos] = before + incl - tiles;
         __syncthreads();
         if (tid == blockDim.x - 1) s_run = before + incl;
         __syncthreads();
     }
     if (tid == 0) {
         tile_indptr[n_seq] = s_run;
-        counter[0] = 0, counter[1] = s_run, counter[2] = 0;
+        counter[0] = 0, counter[1] = s_run, counter[2] = 0, counter[3] = heavy ? 1 : 0;
         if (clamped && s_bad) atomicAdd(clamped, s_bad);
-    }
-    // The select kernel's queue: requests by context length, longest first (ties: lower request first), all H rows
-    // of a request together -- longest-processing-time-first over the persistent select CTAs.
-    const int R = n_seq / H;
-    for (int r = tid; r < R; r += blockDim.x) {
-        const int n = ctx_len[r];
-        int rank = 0;
-        for (int o = 0; o < R; ++o) {
-            const int m = ctx_len[o];
-            rank += (m > n) || (m == n && o < r);
-        }
-        for (int h = 0; h < H; ++h) order[rank * H + h] = r * H + h;
     }
 }
 
@@ -420,23 +464,45 @@ __device__ __forceinline__ void select_row(SelectSmem<NT>& sm, const int seq, co
     for (; v < v1; v += 32) place4(v + lane < v1 ? __ldg(sv + v + lane) : make_float4(0.f, 0.f, 0.f, 0.f), v + lane);
 }
 
-// Persistent grid: every CTA claims rows from the queue `order` (longest context first) until it is empty.  The
-// select is bound by instruction issue and latency per row, not by bandwidth, so what matters is that no SM ends
-// up with two long rows while another holds two short ones (round 1: one CTA per row in launch order, SM busy
-// cycles min / avg / max = 5.7 K / 45 K / 63 K on 8b).
+// Persistent grid: every CTA claims rows from the queue `order` until it is empty.  The select is bound by
+// instruction issue and latency per row, not by bandwidth, so what matters is that no SM ends up with two long rows
+// while another holds two short ones (round 1: one CTA per row in launch order, SM busy cycles min / avg / max =
+// 5.7 K / 45 K / 63 K on 8b).  The gather kernel is launched behind this one programmatically: its CTAs may become
+// resident once every CTA here has started, and they wait row by row for `ready`.  On a gather-heavy call
+// (counter[3], two 512-thread CTAs per SM launched) only the first CTA to arrive on an SM stays: the other leaves
+// its half of the register file to a gather CTA.
 template <int NT>
 __global__ void __launch_bounds__(NT, 1024 / NT)
 topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_t* __restrict__ ctx_len,
                    const int32_t* __restrict__ keep_eff, int H, int n_seq, const int32_t* __restrict__ order,
-                   int32_t* __restrict__ row_counter, int32_t* __restrict__ idx_out) {
+                   int32_t* __restrict__ counter, int32_t* __restrict__ ready, int32_t* __restrict__ sm_first,
+                   int32_t* __restrict__ idx_out) {
     __shared__ SelectSmem<NT> sm;
+    asm volatile("griddepcontrol.launch_dependents;");
+    if (NT < 1024 && __ldcg(counter + 3)) {
+        if (threadIdx.x == 0) {
+            unsigned smid;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            sm.row = atomicAdd(sm_first + (smid % kMaxSms), 1);
+        }
+        __syncthreads();
+        if (sm.row > 0) return;
+    }
+    int done = -1;  // the row whose indices this CTA wrote last
     for (;;) {
-        __syncthreads();  // the previous row is done with the shared state
-        if (threadIdx.x == 0) sm.row = atomicAdd(row_counter, 1);
+        __syncthreads();  // the previous row is done with the shared state, and all its indices are written
+        if (threadIdx.x == 0) {
+            if (done >= 0) {
+                __threadfence();
+                asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(ready + done), "r"(1) : "memory");
+            }
+            sm.row = atomicAdd(counter + 2, 1);
+        }
         __syncthreads();
         const int slot = sm.row;
         if (slot >= n_seq) return;
-        select_row<NT>(sm, order[slot], scores, n_max, ctx_len, keep_eff, H, idx_out);
+        done = order[slot];
+        select_row<NT>(sm, done, scores, n_max, ctx_len, keep_eff, H, idx_out);
     }
 }
 
@@ -505,7 +571,8 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
                       const int32_t* __restrict__ idx, int64_t n_max, const uint4* __restrict__ k_dense,
                       const uint4* __restrict__ v_dense, uint4* __restrict__ pool, int Hp, int n_seq,
                       int32_t* __restrict__ counter, const int32_t* __restrict__ keep_eff,
-                      const int32_t* __restrict__ base, const int32_t* __restrict__ tile_indptr, int P) {
+                      const int32_t* __restrict__ base, const int32_t* __restrict__ tile_indptr,
+                      const int32_t* __restrict__ order, const int32_t* __restrict__ ready, int P) {
     constexpr int kChunks = D / 8;           // 16-byte chunks per row
     constexpr int kRowsPerLd = 32 / kChunks;  // rows one warp-wide load covers
     constexpr int kLds = kCPage / kRowsPerLd; // loads per lane for the K rows of a tile (same for V)
@@ -514,24 +581,37 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
     const int lane = threadIdx.x & 31;
     const int sub = lane / kChunks, ch = lane % kChunks;
     const int total = __ldg(counter + 1);
+    // The select kernel may still be running: a row's indices are read only after its ready flag (acquire by lane 0,
+    // then a warp barrier) and through L2 (ld.cg), never through the non-coherent path.
+    auto wait_row = [&](int seq) {
+        if (lane == 0) {
+            int seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(ready + seq) : "memory");
+            } while (seen == 0);
+        }
+        __syncwarp();
+    };
     for (;;) {
         int first = 0;
         if (lane == 0) first = atomicAdd(counter, kGatherChunk);
         first = __shfl_sync(0xffffffffu, first, 0);
         if (first >= total) break;
         const int last = min(first + kGatherChunk, total);
-        // sequence of the chunk's first tile: largest seq with tile_indptr[seq] <= first
+        // queue position of the chunk's first tile: largest pos with tile_indptr[pos] <= first
         int lo = 0, hi = n_seq;
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
             if (__ldg(tile_indptr + mid) <= first) lo = mid;
             else hi = mid;
         }
-        int seq = lo;
-        int seq_end = __ldg(tile_indptr + seq + 1);
+        int pos = lo;
+        int pos_end = __ldg(tile_indptr + pos + 1);
+        int seq = -1;
         for (int tile = first; tile < last; ++tile) {
-            while (tile >= seq_end) ++seq, seq_end = __ldg(tile_indptr + seq + 1);  // skips heads that keep nothing
-            const int tl = tile - __ldg(tile_indptr + seq);  // tile inside the sequence: its retained rows 16 tl ..
+            while (tile >= pos_end) ++pos, pos_end = __ldg(tile_indptr + pos + 1), seq = -1;  // skips heads that keep nothing
+            if (seq < 0) seq = __ldg(order + pos), wait_row(seq);
+            const int tl = tile - __ldg(tile_indptr + pos);  // tile inside the sequence: its retained rows 16 tl ..
             const int4 si = __ldg(seq_info + seq);           // {table row offset, capacity tokens, slot, -}
             const int n_rows = min(kCPage, __ldg(keep_eff + seq) - tl * kCPage);
             // lane j < n_rows: source token of the tile's row j and where it goes -- token slot base + 16 tl + j
@@ -539,11 +619,11 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
             int my_tok = 0;
             uint32_t my_dst = 0;  // row index in the pool (rows of d elements): < 2^32 for pools up to 550 GB
             if (lane < n_rows) {
-                my_tok = __ldg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
-                const int pos = __ldg(base + seq) + tl * kCPage + lane;
-                const int page = __ldg(tbl_pages + si.x + pos / P);
+                my_tok = __ldcg(idx + static_cast<size_t>(seq) * n_max + tl * kCPage + lane);
+                const int slot = __ldg(base + seq) + tl * kCPage + lane;
+                const int page = __ldg(tbl_pages + si.x + slot / P);
                 // pool[page][slot][kv][token][d]: row index of the K row; the V row is P rows further
-                my_dst = ((static_cast<uint32_t>(page) * Hp + si.z) * 2) * P + pos % P;
+                my_dst = ((static_cast<uint32_t>(page) * Hp + si.z) * 2) * P + slot % P;
             }
             // (at d = 256 a tile goes in two halves of eight rows: 16 + 16 loads would not fit the register budget)
 #pragma unroll
@@ -571,6 +651,8 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
             }
         }
     }
+    // the grid ends after the select grid: whatever follows on the stream sees both complete
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 static int cuda_fail2(cudaError_t e, const char* what) {
@@ -610,54 +692,82 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
         return fail(TANGRAM_ERR_BUFFER_TOO_SMALL, "compact_topk: workspace %zu < %zu bytes", workspace_bytes, need);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int32_t* ws = static_cast<int32_t*>(workspace);
-    CompactWs w{ws, ws + 4, ws + 4 + n_seq, ws + 4 + 2 * n_seq, ws + 4 + 3 * n_seq + 1};
+    CompactWs w{ws, ws + 8, ws + 8 + n_seq, ws + 8 + 2 * n_seq, ws + 8 + 3 * n_seq + 1, ws + 8 + 4 * n_seq + 1,
+                ws + 8 + 5 * n_seq + 1};
     const int4* seq_info = reinterpret_cast<const int4*>(dp->seq_info);
-
-    compact_prepare_kernel<<<1, 1024, 0, st>>>(dp->seq_cap, ctx_len_dev, keep_dev, kv_len_dev, n_seq, dp->H, w.counter,
-                                               w.keep_eff, w.base, w.tile_indptr, w.order, clamped_dev);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
-    // Persistent select grid fed longest-row-first.  Few rows per SM (or very long rows): one 1024-thread CTA per SM,
-    // so that a row gets a whole SM and the queue can even out the SMs; many short rows: two 512-thread CTAs per SM.
     static thread_local int sms_dev = -1, sms = 0;
     int dev = 0;
+    cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail2(e, "cudaGetDevice");
     if (dev != sms_dev) {
         if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
             return cuda_fail2(e, "cudaDeviceGetAttribute");
         sms_dev = dev;
     }
-    if (n_max > kSelLongRow || n_seq <= kSelWideRows * sms)
+    // Select grid: rows of ordinary length get two 512-thread CTAs per SM (and, on a gather-heavy call, give one of
+    // them up to the gather: the decision is the prepare kernel's, from the batch).  Very long rows get one
+    // 1024-thread CTA per SM: a row then has a whole SM, and the gather follows as the select CTAs leave.
+    // TANGRAM_COMPACT_OVERLAP = 0 / 1 forces the decision (measurement aid); default: decide from the batch.
+    const bool wide = n_max > kSelLongRow;
+    const char* ov = getenv("TANGRAM_COMPACT_OVERLAP");
+    const int overlap_env = ov && (ov[0] == '0' || ov[0] == '1') && !ov[1] ? ov[0] - '0' : 2;
+    compact_prepare_kernel<<<1, 1024, 0, st>>>(dp->seq_cap, ctx_len_dev, keep_dev, kv_len_dev, n_seq, dp->H, w.counter,
+                                               w.keep_eff, w.base, w.tile_indptr, w.order, w.ready, w.sm_first, clamped_dev,
+                                               8 * d, wide ? 0 : overlap_env);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
+    if (wide)
         topk_select_kernel<1024><<<std::min(n_seq, sms), 1024, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, n_seq,
-                                                                       w.order, w.counter + 2, idx_out);
+                                                                       w.order, w.counter, w.ready, w.sm_first, idx_out);
     else
         topk_select_kernel<512><<<std::min(n_seq, 2 * sms), 512, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, n_seq,
-                                                                         w.order, w.counter + 2, idx_out);
+                                                                         w.order, w.counter, w.ready, w.sm_first, idx_out);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "top-k select launch");
     const uint4* kd = static_cast<const uint4*>(k_dense);
     const uint4* vd = static_cast<const uint4*>(v_dense);
     uint4* pool = static_cast<uint4*>(kv_pool);
+    // The gather is launched behind the select with programmatic stream serialization and never waits for the whole
+    // select grid, only for the rows it is about to move.  If the driver refuses the attribute once it is not asked
+    // again (a failing launch inside a stream capture would invalidate the capture); a plain launch is correct too.
+    static int pdl_state = -1;  // -1 not tried, 1 accepted, 0 refused
     auto gather = [&](auto kernel, int& grid) -> cudaError_t {
         if (grid == 0) {  // persistent grid: SMs x resident CTAs
-            int dev = 0, sms = 0, per_sm = 0;
-            cudaError_t e2 = cudaGetDevice(&dev);
-            if (e2 == cudaSuccess) e2 = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (e2 == cudaSuccess) e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kGatherThreads, 0);
+            int per_sm = 0;
+            const cudaError_t e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kGatherThreads, 0);
             if (e2 != cudaSuccess) return e2;
             grid = sms * (per_sm > 0 ? per_sm : 1);
         }
-        kernel<<<grid, kGatherThreads, 0, st>>>(seq_info, dp->tbl_pages, idx_out, n_max, kd, vd, pool, dp->Hp, n_seq,
-                                                w.counter, w.keep_eff, w.base, w.tile_indptr, dp->P);
-        return cudaSuccess;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)grid), cfg.blockDim = dim3(kGatherThreads), cfg.dynamicSmemBytes = 0, cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr, cfg.numAttrs = pdl_state != 0 ? 1 : 0;
+        const int64_t n_max_ = n_max;
+        const int Hp = dp->Hp, P = dp->P;
+        const int32_t* tbl = dp->tbl_pages;
+        const int32_t* idx_c = idx_out;
+        cudaError_t e2 = cudaLaunchKernelEx(&cfg, kernel, seq_info, tbl, idx_c, n_max_, kd, vd, pool, Hp, n_seq, w.counter,
+                                            (const int32_t*)w.keep_eff, (const int32_t*)w.base, (const int32_t*)w.tile_indptr,
+                                            (const int32_t*)w.order, (const int32_t*)w.ready, P);
+        if (cfg.numAttrs == 1) {
+            if (e2 == cudaSuccess) pdl_state = 1;
+            else {
+                (void)cudaGetLastError();
+                pdl_state = 0, cfg.numAttrs = 0;
+                e2 = cudaLaunchKernelEx(&cfg, kernel, seq_info, tbl, idx_c, n_max_, kd, vd, pool, Hp, n_seq, w.counter,
+                                        (const int32_t*)w.keep_eff, (const int32_t*)w.base, (const int32_t*)w.tile_indptr,
+                                        (const int32_t*)w.order, (const int32_t*)w.ready, P);
+            }
+        }
+        return e2;
     };
     static thread_local int grid_dev = -1, grid256 = 0, grid128 = 0, grid64 = 0;  // cached per (thread, device)
     if (grid_dev != dev) grid_dev = dev, grid256 = grid128 = grid64 = 0;
     if (d == 256) e = gather(compact_gather_kernel<256>, grid256);
     else if (d == 128) e = gather(compact_gather_kernel<128>, grid128);
     else e = gather(compact_gather_kernel<64>, grid64);
-    if (e != cudaSuccess) return cuda_fail2(e, "compact gather setup");
-    e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact gather launch");
     return TANGRAM_OK;
 }

@@ -79,6 +79,25 @@ def test_compact_random_shapes_bit_exact(seed, R, H, d, C, max_ctx, ties):
     run_and_compare(wl, t, dp, n_pool, kv, scores, kd, vd, n_max)
 
 
+@pytest.mark.parametrize("overlap", ["0", "1"])
+@pytest.mark.parametrize("seed,R,H,d,C,max_ctx", [(41, 40, 8, 128, 4, 900), (42, 3, 4, 64, 2, 6000), (43, 2, 4, 256, 2, 1200)])
+def test_compact_select_and_gather_overlap_modes(monkeypatch, overlap, seed, R, H, d, C, max_ctx):
+    """The gather is launched behind the select programmatically and waits row by row for ready flags.  Both
+    queue orders / occupancies (TANGRAM_COMPACT_OVERLAP = 0: the select keeps every CTA, longest row first; 1: one
+    select CTA per SM, shortest row first, the gather co-resident from the start) must give the oracle's bytes;
+    320 rows make the select queue several waves deep.  Empty and fully retained rows are in the mix."""
+    monkeypatch.setenv("TANGRAM_COMPACT_OVERLAP", overlap)
+    wl = I.make_random_workload(seed, R=R, H=H, G=1, d=d, C=C, max_ctx=max_ctx)
+    B, res, kv, t, n_pool, dp = setup(wl)
+    keep = kv.copy()
+    keep[0, 0] = 0                                     # a row that keeps nothing
+    keep[R - 1, H - 1] = min(int(wl.ctx_len[R - 1]), int(keep[R - 1, H - 1]))
+    n_max = int(wl.ctx_len.max()) + 1
+    scores, kd, vd = I.make_scores_and_dense_kv(wl, n_max, "cuda", ties="bf16")
+    for _ in range(2):                                 # the second call re-arms flags and counters from the first
+        run_and_compare(wl, t, dp, n_pool, keep, scores, kd, vd, n_max)
+
+
 def test_compact_edge_keeps_and_heavy_ties():
     """keep in {0, 1, N-1, N, page multiples}; scores with four distinct values only, +-0, +-inf."""
     wl = I.make_random_workload(31, R=3, H=4, G=1, d=64, C=2, max_ctx=1500)
