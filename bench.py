@@ -535,7 +535,7 @@ def spread_of(T, S, torch, reps=5, detail=False):
 
 def timeline_of(T, S, torch, flush, reps=5):
     """Where a step's time goes, from the instrumented kernel's globaltimer stamps (us after the first CTA starts,
-    median over reps): the first and the last CTA running out of work lists, the grid barrier passed by the last
+    median over reps): the first and the last CTA running out of work lists, the last wait for a record's parts ended (in-grid merge),
     CTA, the last merge done.  The CUDA-event time of the same launch adds the launch / completion floor."""
     W = S["plan"].n_static
     ns = torch.zeros(W, 4, dtype=torch.int64, device=S["q"].device)
@@ -550,12 +550,13 @@ def timeline_of(T, S, torch, flush, reps=5):
         w = ns.cpu().numpy().astype(np.float64)
         t0 = w[:, 0].min()
         merged = w[:, 3].max() if w[:, 3].max() > 0 else w[:, 1].max()
-        barrier = w[:, 2].max() if w[:, 2].max() > 0 else w[:, 1].max()
+        # slot 2: when a CTA's last wait for a record's parts ended (in-grid merge); it holds the SM id otherwise
+        barrier = w[:, 2].max() if w[:, 2].max() >= t0 else w[:, 1].max()
         rows.append([(w[:, 0].max() - t0) / 1e3, (w[:, 1].min() - t0) / 1e3, (w[:, 1].max() - t0) / 1e3,
                      (barrier - t0) / 1e3, (merged - t0) / 1e3, a.elapsed_time(b) * 1e3])
     m = np.median(np.array(rows), axis=0)
     return {"last_cta_start_us": float(m[0]), "first_cta_out_of_work_us": float(m[1]), "last_cta_out_of_work_us": float(m[2]),
-            "barrier_passed_us": float(m[3]), "merges_done_us": float(m[4]), "cuda_event_us": float(m[5])}
+            "last_wait_passed_us": float(m[3]), "merges_done_us": float(m[4]), "cuda_event_us": float(m[5])}
 
 
 def prepare(T, S, torch):
@@ -890,10 +891,10 @@ def main():
         # BALANCED-without-dynamic-tail slowdown (x), STATIC_EVEN slowdown (x)]
         line["config"]["per_config_summary"] = {
             "columns": ["us", "tbs", "kernel_gbs", "cta_spread", "balanced_static_x", "static_even_x"],
-            "timeline_columns": ["first CTA out of work", "last CTA out of work", "barrier passed", "merges done",
+            "timeline_columns": ["first CTA out of work", "last CTA out of work", "last wait for parts passed", "merges done",
                                  "CUDA events"],
             "timeline_us": {k: [round(v["timeline"][c], 1) for c in ("first_cta_out_of_work_us", "last_cta_out_of_work_us",
-                                                                      "barrier_passed_us", "merges_done_us", "cuda_event_us")]
+                                                                      "last_wait_passed_us", "merges_done_us", "cuda_event_us")]
                             for k, v in per.items()},
             **{k: [round(v["us_per_layer_step"], 2), round(v["tbs"], 3), round(v["decode_kernel_gbs"], 0),
                    round(v["cta_spread"], 4),

@@ -193,7 +193,7 @@ typedef struct tangram_device_plan {
     int64_t n_items, n_part_slots;
     int64_t n_merge_seqs;       /* sequences whose part count is not 1 */
     int64_t n_empty_seqs;       /* of these, the first n_empty_seqs have no part at all (kv_len 0) */
-    int64_t n_big_merge_seqs;   /* ... and the last n_big_merge_seqs have more than 32 parts */
+    int64_t n_big_merge_seqs;   /* ... and the last n_big_merge_seqs have more than 16 parts */
     const int32_t* merge_seqs;  /* device [n_merge_seqs][4]: {r * H + h, first part slot, parts, 0}, empty
                                    sequences first, then by part count <= 32 / > 32 */
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
@@ -218,6 +218,8 @@ typedef struct tangram_device_plan {
     const int32_t* plan_cover;    /* device [R*H]: largest tok_end any item of the plan has for the sequence */
     int32_t* grow_state;          /* device [4]: {free-list cursor, rows starved so far, 0, 0} */
     int32_t* q_flags;             /* device [R*H]: staging flags of tangram_decode_attention_host (launch numbers) */
+    uint32_t* seq_done;           /* device [R*H]: parts of each sequence written so far, summed over the launches that
+                                     merged in-grid on this plan (the in-grid merge waits for launches x parts) */
 } tangram_device_plan;
 
 /* Packs tables + plan and copies them into dev_blob (device, >= tangram_blob_bytes, 256-byte
@@ -226,7 +228,7 @@ typedef struct tangram_device_plan {
 int tangram_upload(const tangram_tables* t, const tangram_plan* p, void* dev_blob, size_t bytes,
                    void* stream, tangram_device_plan* dp);
 
-/* Zeroes the launch-state counters of an uploaded plan (dp->sched, dp->q_flags) on `stream`.  The kernels re-arm the counters
+/* Zeroes the launch-state counters of an uploaded plan (dp->sched, dp->q_flags, dp->seq_done) on `stream`.  The kernels re-arm the counters
  * themselves at the end of every launch that runs to completion; this call is for recovery after a launch that
  * did not (an aborted process, a fault), or after two launches on one plan were wrongly overlapped. */
 int tangram_reset_plan(const tangram_device_plan* dp, void* stream);

@@ -61,7 +61,8 @@ class _DevicePlan(C.Structure):
                 ("seq_info", C.c_void_p), ("part_indptr", C.c_void_p), ("tbl_pages", C.c_void_p), ("sched", C.c_void_p),
                 ("max_merge_parts", C.c_int64), ("min_pool_pages", C.c_int64), ("n_slots", C.c_int64),
                 ("row_ptr", C.c_void_p), ("row_pages", C.c_void_p), ("perm", C.c_void_p), ("seq_cap", C.c_void_p),
-                ("plan_cover", C.c_void_p), ("grow_state", C.c_void_p), ("q_flags", C.c_void_p)]
+                ("plan_cover", C.c_void_p), ("grow_state", C.c_void_p), ("q_flags", C.c_void_p),
+                ("seq_done", C.c_void_p)]
 
 
 _lib.tangram_last_error.restype = C.c_char_p

@@ -79,9 +79,11 @@ struct DecodeParams {
     float* part_o;
     float* part_lse;
     unsigned long long* worker_ns;
-    int* sched;  // [0] next list to claim (relative to gridDim.x), [1] CTAs done claiming, [2] grid-barrier
-                 // arrivals, [3] CTAs done merging; all 0 between launches (the kernel re-arms them);
-                 // [4] launches that staged host queries on this plan (the epoch of q_flags)
+    int* sched;  // [0] next list to claim (relative to gridDim.x), [1] CTAs done claiming, [2] tickets taken (CTAs
+                 // out of work), [3] CTAs done merging; all 0 between launches (the kernel re-arms them);
+                 // [4] launches that staged host queries on this plan (the epoch of q_flags); [5] launches that
+                 // merged in-grid on this plan (the epoch of seq_done)
+    unsigned* seq_done;  // [R*H] parts written so far, summed over the in-grid-merging launches on this plan
     const int32_t* merge_recs;  // merge records (see a5)
     const void* list_heads;     // [n_lists] 128-byte list heads
     const int32_t* kv_len;      // [R*H] run-time lengths (open-ended plan) or nullptr: items are taken as planned
@@ -233,7 +235,10 @@ __device__ __forceinline__ unsigned long long globaltimer() {
 // pass); the group sums are then combined in group order.  The summation order is a function of
 // (n, G, D, thread count) only, so the result is deterministic.
 constexpr int kMergeThreads = 512;
-constexpr int kMergeBigParts = 32;
+#ifndef TANGRAM_MERGE_BIG_PARTS
+#define TANGRAM_MERGE_BIG_PARTS 16
+#endif
+constexpr int kMergeBigParts = TANGRAM_MERGE_BIG_PARTS;  // records with more parts are merged by whole-CTA units
 #ifndef TANGRAM_MERGE_BATCH
 #define TANGRAM_MERGE_BATCH 8
 #endif
@@ -998,23 +1003,34 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             }
         }
         named_bar_sync(1, kNW * 32);  // scratch may be overwritten by the next item
+        // In-grid merge: the part is published with one fire-and-forget release (every thread's stores precede the
+        // barrier above, the release is cumulative) -- nobody waits for it here.
+        if (p.tail_merge && item.n_parts != 1 && threadIdx.x == 0)
+            asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p.seq_done + item.req * p.H + item.kv_head), "r"(1u)
+                         : "memory");
     }
     if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 1] = globaltimer();
 
     if (p.tail_merge) {
-        // a5 inside the persistent grid.  Every CTA takes a ticket when its work lists are done (its partials are
-        // published by the fence before the ticket).  The last `merge_ctas` arrivals stay: they wait until all
-        // tickets are taken -- the grid barrier -- and merge unit rank, rank + M, ... among themselves; earlier
-        // arrivals, if any, leave at once.  With merge_ctas = grid (the normal case) this is a plain grid barrier
-        // followed by merges on all SMs.  The wait cannot deadlock as long as merge_ctas CTAs fit on the device
-        // together (checked by the launcher): whoever waits is running, and whoever has not arrived yet is running or
-        // will be scheduled on a slot a finished CTA left.  The launcher still asks for a cooperative launch, except
-        // behind a programmatic dependency, where the plain launch saves ~2 us per layer-step.
-        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*M)*K + sub, no barrier inside; the
-        // first record is fetched before the wait (plan data).  Big records (more than kMergeBigParts parts) go
-        // first, one query head per unit.
-        // In a fused decode step the very last arrival does not merge: it updates the lengths and grows the
-        // block tables for the next step while the others merge.
+        // a5 inside the persistent grid, without a grid barrier.  Every multi-part item was published by a release
+        // add on its sequence's counter (above); a CTA that is out of work lists merges its share of the records,
+        // waiting record by record until the counter shows all the parts of THIS launch: (launches so far + 1) x parts
+        // (the counters are never reset; unsigned wrap-around is harmless because a counter is only compared for
+        // equality with a target it cannot overshoot).  Records are visited in sequence order -- the order in which
+        // the work lists complete them -- so a CTA that runs out of work early merges what is already complete while
+        // the others still stream, and after the last part of the launch is written only the records that contain
+        // parts of the last lists remain.
+        // Who may wait: every CTA takes a ticket when its lists are done; the last `merge_ctas` arrivals stay and
+        // merge, earlier arrivals (grids larger than the device) leave at once.  A waiting CTA waits for parts that
+        // a running CTA writes or that a CTA not yet scheduled will write on a slot a finished CTA left, so the waits
+        // end whenever merge_ctas CTAs fit on the device together (checked by the launcher, which still asks for a
+        // cooperative launch except behind a programmatic dependency).
+        // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*M)*K + sub, every thread polls
+        // and merges on its own, no barrier inside.  Big records (more than kMergeBigParts parts: the sequences the
+        // last rounds of the dynamic tail dice finely) come after the small ones, one (query head, column block)
+        // per unit.
+        // In a fused decode step the very last arrival does not merge: all CTAs are out of work then, every append
+        // has happened, and it updates the lengths and grows the block tables for the next step.
         const bool fused = p.k_new != nullptr;
         const int grid_all = static_cast<int>(gridDim.x);
         const int n_late = min(grid_all, p.merge_ctas);  // CTAs that stay for the tail phase
@@ -1029,35 +1045,44 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             const bool merger = rank < grid;
             const int n_elem = G * (D / 4), K = (kNW * 32) / n_elem, sub = threadIdx.x / n_elem;
             const int n_big_units = p.n_merge_units - p.n_merge_small;
-            // ... so the small records start at the CTA after the last one holding a big unit
-            const int first = (rank - n_big_units % grid + grid) % grid;
-            int sidx = first * K + sub;
-            int4 rec = make_int4(0, 0, 0, 0);
-            if (merger && sub < K && sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
-            if (threadIdx.x == 0) {
-                int seen;
-                do {
-                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.sched + 2) : "memory");
-                    if (TANGRAM_BARRIER_NANOSLEEP > 0 && seen < grid_all) __nanosleep(TANGRAM_BARRIER_NANOSLEEP);
-                } while (seen < grid_all);
-                __threadfence();
-            }
-            named_bar_sync(1, kNW * 32);
-            if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();
+            // the previous launch on this plan is complete (the producer waited for it before the first item)
+            const unsigned epoch1 = static_cast<unsigned>(__ldcg(p.sched + 5)) + 1u;
+            auto wait_parts = [&](int seq, int n) {  // every thread for itself: acquire, then its own loads
+                const unsigned want = epoch1 * static_cast<unsigned>(n);
+                unsigned seen;
+                for (;;) {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(p.seq_done + seq) : "memory");
+                    if (seen == want) break;
+                    if (TANGRAM_BARRIER_NANOSLEEP > 0) __nanosleep(TANGRAM_BARRIER_NANOSLEEP);
+                }
+                if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();  // the CTA's last wait passed
+            };
             float(*s_part)[6] = reinterpret_cast<float(*)[6]>(scratch_o);
             if (merger) {
-                for (int u = rank; u < n_big_units; u += grid)
-                    merge_big_unit<D, kNW * 32, true>(unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4),
-                                                      G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
-                if (sub < K)
+                // ... the small records start at the CTA after the last one holding a big unit
+                const int first = (rank - n_big_units % grid + grid) % grid;
+                if (sub < K) {
+                    int sidx = first * K + sub;
+                    int4 rec = make_int4(0, 0, 0, 0);
+                    if (sidx < p.n_merge_small) rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx);
                     for (; sidx < p.n_merge_small; sidx += grid * K) {
-                        merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
+                        int4 nxt = make_int4(0, 0, 0, 0);
                         if (sidx + grid * K < p.n_merge_small)
-                            rec = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
+                            nxt = __ldg(reinterpret_cast<const int4*>(p.merge_recs) + sidx + grid * K);
+                        if (rec.z > 0) wait_parts(rec.x, rec.z);
+                        merge_small<D>(rec, G, p.part_o, p.part_lse, p.out, p.lse, threadIdx.x - sub * n_elem);
+                        rec = nxt;
                     }
+                }
+                if (n_big_units > 0) named_bar_sync(1, kNW * 32);  // the merge scratch is shared by the whole CTA
+                for (int u = rank; u < n_big_units; u += grid) {
+                    const MergeUnit mu = unit_of(p.merge_recs, p.n_merge_small, p.n_merge_small + u, G, p.merge_split, D / 4);
+                    wait_parts(mu.seq, mu.n);
+                    merge_big_unit<D, kNW * 32, true>(mu, G, p.part_o, p.part_lse, p.out, p.lse, s_part, threadIdx.x);
+                }
             }
             if (fused && (!merger || n_late == 1)) {
-                // every append of this step happened before the barrier: lengths, then the pages of the next step
+                // the last ticket: every CTA is out of work, every append of this step has happened
                 named_bar_sync(1, kNW * 32);
                 step_lengths<kNW * 32, true>(p.grow, threadIdx.x);
                 if (p.grow.free_pages) extend_rows<kNW * 32, true>(p.grow, kPage, threadIdx.x, reinterpret_cast<int*>(scratch_o));
@@ -1065,8 +1090,9 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
         }
         if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == grid_all - 1) {
-            p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the barrier for the next launch
-            if (p.q_host) p.sched[4] += 1;   // ... and closes this launch's query-staging epoch
+            p.sched[2] = 0, p.sched[3] = 0;  // last CTA out re-arms the tickets for the next launch
+            p.sched[5] += 1;                 // ... closes this launch's merge epoch
+            if (p.q_host) p.sched[4] += 1;   // ... and its query-staging epoch
         }
     }
 }
@@ -1356,7 +1382,7 @@ extern "C" int tangram_query_max_ctas(int device, int32_t head_dim, int32_t gqa,
 // Blob layout (all sections 256-byte aligned), shared by tangram_blob_bytes and tangram_upload.
 namespace {
 struct BlobLayout {
-    size_t items, windptr, pindptr, pages, mseq, heads, seqinfo, row_ptr, row_pages, perm, seq_cap, cover, q_flags, grow, sched, total;
+    size_t items, windptr, pindptr, pages, mseq, heads, seqinfo, row_ptr, row_pages, perm, seq_cap, cover, q_flags, seq_done, grow, sched, total;
 };
 int64_t table_slots(const tangram_tables* t) {
     return t->tbl_indptr ? t->tbl_indptr[(int64_t)t->R * t->C] : t->n_pages_used;
@@ -1383,6 +1409,7 @@ BlobLayout blob_layout(const tangram_tables* t, const tangram_plan* p) {
     b.seq_cap = take(sizeof(int32_t) * n_seq);
     b.cover = take(sizeof(int32_t) * n_seq);
     b.q_flags = take(sizeof(int32_t) * n_seq);
+    b.seq_done = take(sizeof(uint32_t) * n_seq);
     b.grow = take(16);
     b.sched = take(32);
     b.total = off + 256;
@@ -1527,6 +1554,7 @@ extern "C" int tangram_upload(const tangram_tables* t, const tangram_plan* p, vo
     dp->plan_cover = reinterpret_cast<const int32_t*>(base + lay.cover);
     dp->grow_state = reinterpret_cast<int32_t*>(base + lay.grow);
     dp->q_flags = reinterpret_cast<int32_t*>(base + lay.q_flags);
+    dp->seq_done = reinterpret_cast<uint32_t*>(base + lay.seq_done);
     return TANGRAM_OK;
 }
 
@@ -1537,6 +1565,8 @@ extern "C" int tangram_reset_plan(const tangram_device_plan* dp, void* stream) {
     cudaError_t e = cudaMemsetAsync(dp->sched, 0, 32, static_cast<cudaStream_t>(stream));
     if (e == cudaSuccess && dp->q_flags)
         e = cudaMemsetAsync(dp->q_flags, 0, sizeof(int32_t) * (size_t)dp->R * dp->H, static_cast<cudaStream_t>(stream));
+    if (e == cudaSuccess && dp->seq_done)
+        e = cudaMemsetAsync(dp->seq_done, 0, sizeof(uint32_t) * (size_t)dp->R * dp->H, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e, "reset_plan: cudaMemsetAsync");
     return TANGRAM_OK;
 }
@@ -1619,6 +1649,7 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     prm.n_lists = dp->W;
     prm.list_heads = dp->list_heads;
     prm.sched = dp->sched;
+    prm.seq_done = dp->seq_done;
     prm.kv_len = kv_len_dev, prm.H = dp->H, prm.R = dp->R;
     prm.q_host = static_cast<const uint4*>(step.q_host), prm.q_flags = dp->q_flags;
     if (step.k_new) {
