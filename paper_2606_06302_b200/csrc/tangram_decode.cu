@@ -197,11 +197,10 @@ __device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t&
 // D(16x8) += A(16x16) B(16x8), bf16 inputs, fp32 accumulate.  Only rows 0..7 of A are populated
 // (the GQA group), so a1 = a3 = 0 and the row 8..15 halves of the accumulator are discarded.
 __device__ __forceinline__ void mma_rows07(float& c0, float& c1, uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
-    float d2, d3;
+    [[maybe_unused]] float d2, d3;
     asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%10,%10};"
         : "+f"(c0), "+f"(c1), "=f"(d2), "=f"(d3)
         : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1), "f"(0.f));
-    (void)d2, (void)d3;
 }
 // The full 16-row form (GQA groups of 9..16 query heads): rows 0..7 accumulate into (c0, c1), rows 8..15 into (c2, c3).
 __device__ __forceinline__ void mma_rows16(float& c0, float& c1, float& c2, float& c3, uint32_t a0, uint32_t a1, uint32_t a2,
@@ -1191,7 +1190,7 @@ static int make_kv_map(CUtensorMap* map, const void* pool, int64_t n_pool_pages,
     const cuuint64_t rows = static_cast<cuuint64_t>(n_pool_pages) * Hp * 2 * kPage;
     const cuuint64_t gdim[3] = {64, rows, static_cast<cuuint64_t>(d / 64)};
     const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(d) * 2, 128};
-    const cuuint32_t box[3] = {64, 2 * kPage, static_cast<cuuint32_t>(d / 64)};
+    const cuuint32_t box[3] = {64, static_cast<cuuint32_t>(2 * kPage), static_cast<cuuint32_t>(d / 64)};
     const cuuint32_t estride[3] = {1, 1, 1};
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(pool), gdim, gstride, box,
                            estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,

@@ -821,3 +821,57 @@ def test_scaled_configs_page_size_32(name, kw):
         ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv_ref, wl.Hq, wl.d)
         check(out, lse, ref_out, ref_lse, f"P=32 decode step {step}")
     assert n_over > 0
+
+
+def blob_words(dp, ptr, n_words):
+    """int32 view of `n_words` words of the uploaded blob at device address `ptr` (a field of the device plan)."""
+    off = int(ptr) - dp.blob.data_ptr()
+    assert 0 <= off and off + 4 * n_words <= dp.blob.numel()
+    return dp.blob[off:off + 4 * n_words].view(torch.int32)
+
+
+@pytest.mark.parametrize("d,G,W,dyn", [(128, 4, None, (500, 6)), (64, 2, 300, (500, 4)), (128, 5, None, (300, 3)), (128, 4, 40, (0, 0))])
+def test_in_grid_merge_counters_epochs_wrap_and_recovery(d, G, W, dyn):
+    """The in-grid merge has no grid barrier: every multi-part item adds one to its sequence's counter (release), and
+    a record is merged when the counter reads (launches so far + 1) x parts.  Checked here: the counters and the
+    epoch after a launch; launches across the 2^32 wrap of both (counters preset as if 2^32 - 2 launches had run)
+    give the same bits as the first launch; tangram_reset_plan recovers from garbage state; small records, records
+    above 16 parts (whole-CTA units) and grids larger than the device (W = 300: early arrivals leave, the last 148
+    merge) are all in the mix; the result is within tolerance of the oracle."""
+    wl = I.make_random_workload(700 + d + G, R=3, H=4, G=G, d=d, C=2, max_ctx=9000)
+    wl.ctx_len[0] = 9000
+    wl.demand = np.minimum(np.maximum(wl.demand, 1), wl.ctx_len[:, None]).astype(np.int32)
+    wl.demand[0, 0] = 8800                                  # one long sequence: many parts
+    wl.mu[:] = 1.0
+    B, res, kv, t, n_pool = setup(wl)
+    q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
+    W = W or n_cta(wl)
+    pl = T.tangram_plan_partitions(t, B, kv, W, wl.granule, 1, T.MODE_BALANCED, 0, *dyn)
+    parts = np.diff(pl.part_indptr).astype(np.int64)
+    counted = np.where(parts != 1, parts, 0)                # single-part sequences are written by the decode kernel
+    assert (parts > 16).any() or dyn == (0, 0)
+    assert ((parts > 1) & (parts <= 16)).any()
+    dp = T.tangram_upload(t, pl)
+    sched, done = blob_words(dp, dp.c.sched, 8), blob_words(dp, dp.c.seq_done, wl.R * wl.H)
+    out0, lse0 = T.tangram_decode_attention(dp, q, pool)
+    torch.cuda.synchronize()
+    ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
+    check(out0, lse0, ref_out, ref_lse, "first launch")
+    s = sched.cpu().numpy()
+    assert s[5] == 1 and not s[[0, 1, 2, 3, 6, 7]].any(), s
+    assert np.array_equal(done.cpu().numpy().astype(np.int64), counted)
+    E = 2 ** 32 - 2                                         # as if 2^32 - 2 launches had merged on this plan
+    sched[5] = int(np.array(E, dtype=np.uint64).astype(np.uint32).view(np.int32))
+    done.copy_(torch.from_numpy(((counted.astype(np.uint64) * np.uint64(E)) & np.uint64(0xFFFFFFFF)).astype(np.uint32).view(np.int32)).cuda())
+    for rep in range(4):
+        out, lse = T.tangram_decode_attention(dp, q, pool)
+        torch.cuda.synchronize()
+        assert torch.equal(out, out0) and torch.equal(lse, lse0), f"launch {E + rep} (mod 2^32)"
+    assert int(sched.cpu().numpy().view(np.uint32)[5]) == (E + 4) % 2 ** 32 == 2
+    assert np.array_equal(done.cpu().numpy().view(np.uint32).astype(np.int64), (counted * 2) % 2 ** 32)
+    done.fill_(12345)                                       # an aborted launch leaves anything behind
+    sched[2], sched[3], sched[5] = 7, 3, 99
+    T.tangram_reset_plan(dp)
+    out, lse = T.tangram_decode_attention(dp, q, pool)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out0) and torch.equal(lse, lse0)
