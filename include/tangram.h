@@ -203,9 +203,10 @@ typedef struct tangram_device_plan {
                                      the page, row index r*C + c} */
     const int64_t* part_indptr;   /* device [R*H+1] */
     const int32_t* tbl_pages;     /* device page ids */
-    int32_t* sched;               /* device [8]: list-claim / CTAs-done counters of the dynamic tail, the grid-barrier
-                                     counters of the in-kernel merge (zero between launches; the kernel re-arms
-                                     them itself) and the launch number of the host-query staging */
+    int32_t* sched;               /* device [8]: list-claim / CTAs-done counters of the dynamic tail, the ticket and
+                                     exit counters of the in-kernel merge (zero between launches; the kernel re-arms
+                                     them itself), the launch number of the host-query staging and the number of
+                                     launches that merged in-grid on this plan (the epoch of seq_done) */
     int64_t max_merge_parts;      /* most parts any sequence has (sizes the column split of the big-record merge) */
     int64_t min_pool_pages;       /* largest page id in the tables at upload + 1: the device calls return INVALID_ARG
                                      for a kv_pool with fewer pages */
@@ -237,10 +238,12 @@ int tangram_reset_plan(const tangram_device_plan* dp, void* stream);
 size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_dim);
 
 /* a4 + a5  One layer, whole batch: split-KV decode kernel over the work lists, then the LSE merge -- inside the
- * same persistent grid after a grid barrier (ONE launch: cooperative when the grid fits on the device, else the
- * last SMs x occupancy CTAs to finish do the merging); the stand-alone merge kernel follows as a second launch only
- * at d = 256 or when a merge record is wider than the CTA (G x d/4 > consumer threads: d = 128 with G > 8, or G > 4
- * on 32-token pages).
+ * same persistent grid and without a grid barrier: every part of a multi-part sequence is published by a release add
+ * on the sequence's counter (dp->seq_done), and a CTA that is out of work lists merges its share of the sequences,
+ * each as soon as the counter shows all parts of this launch (ONE launch: cooperative when the grid fits on the
+ * device, else the last SMs x occupancy CTAs to finish do the merging); the stand-alone merge kernel follows as a
+ * second launch only at d = 256 or when a merge record is wider than the CTA (G x d/4 > consumer threads: d = 128
+ * with G > 8, or G > 4 on 32-token pages).
  * Asynchronous on `stream`; CUDA-graph capturable; no host work besides the launch.
  *
  *   dp        from tangram_upload (host struct holding device pointers)
@@ -258,7 +261,7 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *             -inf and out = 0 for a head with kv_len 0)
  *   workspace device, >= tangram_workspace_bytes(dp->n_part_slots, G, d), 16-byte aligned
  *   worker_ns device [n_static][4] u64 or NULL: if given, every CTA stores its globaltimer stamps
- *             {start, end of its work lists, grid barrier passed, merges done} (the last two only when
+ *             {start, end of its work lists, its last wait for a sequence's parts ended, merges done} (the last two only when
  *             the merge runs inside the decode grid; without it -- tangram_decode_partials -- the third slot
  *             holds the id of the SM the CTA ran on, %smid); the per-CTA elapsed-time spread of BASELINE.json
  *             is measured from the first two.
@@ -384,8 +387,9 @@ int tangram_download_tables(const tangram_device_plan* dp, tangram_tables* t, in
  *   3. lengths  kv_len_dev[r][h] becomes n + 1 (unchanged for a dropped row).
  *   4. grow     if free_pages_dev != NULL: the block-table update described above, with the new lengths, so that
  *               the NEXT step's token has a page.  (Run tangram_extend_tables_device once before the first step.)
- * Steps 3 and 4 run after the grid barrier of the in-kernel merge, on one CTA, while the others merge; when the
- * grid cannot be launched cooperatively (or d = 256) they run in a small follow-up kernel.
+ * Steps 3 and 4 run on the CTA that is the last to run out of work lists (every append has happened then), while the
+ * others merge; when the in-kernel merge is not available (d = 256, wide merge records) they run in a small
+ * follow-up kernel.
  * The composition is bit-exact against the oracle's extend_tables -> append_kv -> attention for the pool, the
  * lengths, the tables and the counters; the attention output is within the a4 tolerances.
  *
@@ -431,7 +435,11 @@ int tangram_decode_step(const tangram_device_plan* dp, const void* q, const void
  *                 token indices in ascending order (the set I of Eq. 4); the rest is not touched
  *   clamped_dev   device i32 or NULL: incremented by the number of clamped heads
  *   workspace     device, >= tangram_compact_workspace_bytes(R, H), 16-byte aligned
- * Asynchronous on `stream` (three launches); graph capturable.  Errors: INVALID_ARG, BUFFER_TOO_SMALL, CUDA. */
+ * Asynchronous on `stream`; graph capturable.  Three launches (prepare, select, gather); the gather is launched
+ * behind the select programmatically and moves a row as soon as that row's selection is written (per-row ready
+ * flags), so the two overlap; the call is complete when the gather grid is.  TANGRAM_COMPACT_OVERLAP = 0 / 1 in the
+ * environment forces the gather-heavy decision (whether the select leaves half of every SM to the gather), a
+ * measurement aid; by default it is taken from the batch.  Errors: INVALID_ARG, BUFFER_TOO_SMALL, CUDA. */
 size_t tangram_compact_workspace_bytes(int32_t R, int32_t H);
 int tangram_compact_topk(const tangram_device_plan* dp, const float* scores, const void* k_dense,
                          const void* v_dense, int64_t n_max, const int32_t* ctx_len_dev, const int32_t* keep_dev,
