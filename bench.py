@@ -617,10 +617,11 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
     of the serving system (written by prefill, like weights) and stays in HBM.
     zero_copy=True: tangram_decode_attention_host -- out / lse are HOST pointers (pinned memory is mapped into the
     device's address space and the kernel's posted stores go over the bus, so the result never waits for a copy
-    engine); q is pulled from pinned host memory by the staging kernel, and the decode kernel is launched behind it
-    with programmatic stream serialization, so its launch and the fill of its KV tile rings overlap the transfer
-    (reading q in place from host memory inside the decode kernel works too and is tested, but every work item
-    re-reads its query group over the bus: 1.3 MB instead of 0.26 MB, and the bus queue stalls the CTAs).
+    engine); q is pulled from pinned host memory by the decode kernel itself: the consumer warps of CTA b stage query
+    blocks b, b + grid, ... into device memory when the CTA starts and publish per-block flags, a producer waits for
+    the flag of the block its item needs -- one launch, every block crosses the bus once, and the KV tile rings fill
+    meanwhile (reading q in place from host memory works too and is tested, but every work item re-reads its query
+    group over the bus: 1.3 MB instead of 0.26 MB, and the bus queue stalls the CTAs).
     zero_copy=False: explicit staging copies around the call (one H2D, one D2H)."""
     q_host = S["q"].cpu().pin_memory()
     R, Hq, d = S["q"].shape
@@ -632,7 +633,7 @@ def e2e_steps(T, S, steps, warmup, flush, torch, zero_copy):
 
         q_dev = torch.empty_like(S["q"])
 
-        def step():          # ONE C-ABI call: staging kernel + decode kernel overlapped behind it (PDL)
+        def step():          # ONE C-ABI call, ONE launch: the decode kernel stages q itself
             T.tangram_decode_attention_host(S["dp"], q_host, q_dev, S["pool"], out_host, lse_host, S["ws"])
     else:
         # out and lse live in ONE device allocation, so the result goes back with a single device->host copy
@@ -838,8 +839,8 @@ def main():
         "e2e": {"value": e_bytes / (e_ms * 1e-3) / 1e12, "unit": "TB/s", "us_per_layer_step": e_ms * 1e3,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "us_per_layer_step_staged_copies": float(np.mean(ems_staged) * 1e3),
-                "note": "one tangram_decode_attention_host call per step: q pulled from pinned host memory by the staging "
-                        "kernel with the decode kernel launched behind it by programmatic dependent launch, out+lse written "
+                "note": "one tangram_decode_attention_host call (one launch) per step: q pulled from pinned host memory by "
+                        "the decode kernel's own consumer warps (per-block flags), out+lse written "
                         "by the kernel straight into pinned, device-mapped host memory, all inside the timed region; "
                         "`staged_copies` = the same with copy-engine transfers (one H2D before, one D2H after the call); "
                         "the KV page pool is resident serving state in HBM"},
