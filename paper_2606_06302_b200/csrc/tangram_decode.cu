@@ -100,6 +100,7 @@ struct DecodeParams {
     int32_t* kv_len_w;           // = kv_len, writable
     GrowParams grow;
     int32_t pdl;                 // launched with programmatic stream serialization: wait before reading q / k_new / v_new
+    int32_t early_trigger;       // 1: dependents may be launched while this grid runs (griddepcontrol.launch_dependents)
     // host-resident queries (tangram_decode_attention_host, cooperative launch only): the consumer warps of CTA b
     // copy query blocks b, b + grid, ... from pinned host memory to `q` (device) when the CTA starts and publish each
     // block's flag; a producer waits for the flag of the block its item needs.  nullptr otherwise.
@@ -676,7 +677,10 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             __syncwarp();
             asm volatile("griddepcontrol.wait;" ::: "memory");
         }
-        asm volatile("griddepcontrol.launch_dependents;");  // the next launch on the stream may be scheduled
+        // The next launch on the stream may be scheduled -- unless this grid waits inside (in-grid merge) and is NOT
+        // gang-scheduled: CTAs of a dependent grid that became resident early would sit on SMs (waiting for this grid
+        // to complete) that CTAs of this grid still need, and the waits in the tail phase would never end.
+        if (p.early_trigger) asm volatile("griddepcontrol.launch_dependents;");
         const int q_epoch = p.q_host ? __ldcg(p.sched + 4) + 1 : 0;
         int seq = 0;  // running item number = position in the item / query ring
         for (;;) {
@@ -1251,9 +1255,15 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     if (g_overlap_state == 0) prm.pdl = 0;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeCooperative;
-    // cooperative: the formal co-residency guarantee for the in-grid barrier; a plain launch behind a programmatic
-    // dependency (the barrier's ticket scheme only needs the grid to FIT, which was checked above)
-    attr[0].val.cooperative = (prm.tail_merge && coresident && !prm.pdl) ? 1 : 0;
+    // A grid whose CTAs wait for one another (in-grid merge) is launched cooperatively whenever it fits on the device:
+    // gang scheduling is what makes the waits safe next to OTHER grids -- in particular next to a programmatically
+    // dependent successor, whose CTAs become resident while this grid still runs.  (A plain launch behind a
+    // programmatic dependency was 1.8 us per layer-step faster in the graph loop and deadlocked about once in three
+    // runs of the 200-step graph test: dependent CTAs took SMs that CTAs of this grid had not reached yet.)  A grid
+    // larger than the device cannot be gang-scheduled: it runs as a plain launch, only its last `merge_ctas` CTAs
+    // wait, and it does not let its dependents start early.
+    attr[0].val.cooperative = (prm.tail_merge && coresident) ? 1 : 0;
+    prm.early_trigger = (!prm.tail_merge || coresident) ? 1 : 0;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
