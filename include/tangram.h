@@ -247,7 +247,7 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  * Asynchronous on `stream`; CUDA-graph capturable; no host work besides the launch.
  *
  *   dp        from tangram_upload (host struct holding device pointers)
- *   q         device (or pinned host, see "Host buffers" below) [R][Hq][d] bf16, 16-byte aligned
+ *   q         device [R][Hq][d] bf16, 16-byte aligned (host memory is refused, see "Host buffers" below)
  *   kv_pool   device [n_pool_pages][Hp][2][P][d] bf16, 128-byte aligned (Ragged page, :190)
  *   kv_len_dev device [R][H] i32 or NULL.  NULL: the items are executed exactly as planned.  Otherwise the
  *             plan is OPEN-ENDED: every item covers tokens [tok_begin, min(tok_end, kv_len_dev[r][h])), so a
@@ -277,13 +277,14 @@ int tangram_decode_attention(const tangram_device_plan* dp, const void* q, const
                              float* lse, void* workspace, size_t workspace_bytes,
                              uint64_t* worker_ns, void* stream);
 
-/* Host buffers.  q, out and lse of tangram_decode_attention may be PINNED host memory (page-locked memory is mapped
- * into the device's address space under unified addressing): the kernel then reads / writes them in place over the
- * bus.  Writing out / lse that way costs nothing (posted stores); reading q in place makes every item wait a bus
- * round trip for its query group, so for q this helper is the better way: it copies `bytes` (a multiple of 16) from
- * pinned host memory `src_host` to device memory `dst_dev` with a kernel on `stream` -- for the few hundred KB of a
- * decode step ~10 us sooner than a copy-engine transfer plus its stream hand-off.  Errors: INVALID_ARG (NULL,
- * alignment, source not page-locked), CUDA. */
+/* Host buffers.  out and lse of tangram_decode_attention may be PINNED host memory (page-locked memory is mapped
+ * into the device's address space under unified addressing): the kernel's stores then go over the bus as posted
+ * writes and the result never waits for a copy engine.  q must be DEVICE memory: the kernel fetches query groups with
+ * bulk asynchronous copies, and those hang now and then when pointed at mapped host memory (measured on B200), so a
+ * host q is refused with INVALID_ARG.  Host-resident queries go through tangram_decode_attention_host below, or are
+ * staged by this helper: it copies `bytes` (a multiple of 16) from pinned host memory `src_host` to device memory
+ * `dst_dev` with a kernel on `stream` -- for the few hundred KB of a decode step ~10 us sooner than a copy-engine
+ * transfer plus its stream hand-off.  Errors: INVALID_ARG (NULL, alignment, source not page-locked), CUDA. */
 int tangram_stage_from_host(void* dst_dev, const void* src_host, size_t bytes, void* stream);
 
 /* tangram_decode_attention with HOST buffers, end to end in ONE launch: the consumer warps of CTA b copy the query

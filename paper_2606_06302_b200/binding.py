@@ -273,9 +273,10 @@ def tangram_decode_attention(dp: DevicePlan, q, kv_pool, out=None, lse=None, wor
     """q [R,Hq,d] bf16 cuda, kv_pool [n_pages,Hp,2,P,d] bf16 cuda -> (out [R,Hq,d] bf16, lse [R,Hq] f32).
     Asynchronous on the current (or given) torch stream."""
     import torch
-    # q / out / lse may also be PINNED host tensors: page-locked memory is mapped into the device's address space
-    # (unified addressing), the kernels read q and write out / lse in place over the bus, no staging copy
-    assert (q.is_cuda or q.is_pinned()) and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
+    # out / lse may also be PINNED host tensors: page-locked memory is mapped into the device's address space
+    # (unified addressing) and the kernels write them in place over the bus; q must be on the device (host-resident
+    # queries: tangram_decode_attention_host)
+    assert q.is_cuda and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
     assert q.is_contiguous() and kv_pool.is_contiguous()
     R, Hq, d = q.shape
     n_pages = kv_pool.shape[0]
@@ -382,7 +383,7 @@ def tangram_decode_step(dp: DevicePlan, q, k_new, v_new, kv_pool, kv_len, free_p
     """One decode step of one layer in one launch: KV append + attention + merge + length update + table growth
     for the next step (include/tangram.h).  kv_len [R,H] int32 cuda is incremented in place."""
     import torch
-    assert (q.is_cuda or q.is_pinned()) and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
+    assert q.is_cuda and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
     assert q.is_contiguous() and kv_pool.is_contiguous()
     R, Hq, d = q.shape
     H = dp.c.H

@@ -43,8 +43,7 @@ static bool page_supported(int P, int d) { return P == 16 || (P == 32 && d <= 12
 template <int D, int PAGE>
 constexpr int consumer_warps() { return 2 * PAGE * D * 2 >= 16384 ? 4 : 8; }
 constexpr int kMinQSlots = 2;      // item / query ring depth: as deep as shared memory allows, 2 .. 8 (runtime).  A deep
-constexpr int kMaxQSlots = 8;      // ring lets the producer fetch query groups several items ahead, which is what hides
-                                   // the bus round trip when q lives in pinned host memory
+constexpr int kMaxQSlots = 8;      // ring lets the producer fetch query groups several items ahead
 constexpr int kMaxStages = 8;      // per-consumer-warp tile ring depth (runtime <= this)
 constexpr int kMaxG = 16;         // GQA groups above 8 use both halves of the 16-row A operand (d <= 128)
 constexpr int kSmemLimit = 232448; // 227 KB opt-in limit per CTA
@@ -1630,6 +1629,17 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     if ((split && (reinterpret_cast<uintptr_t>(q) % 16 || reinterpret_cast<uintptr_t>(kv_pool) % 128)) ||
         reinterpret_cast<uintptr_t>(out) % 16 || reinterpret_cast<uintptr_t>(workspace) % 16)
         return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: misaligned pointer");
+    if (split) {
+        // q is read with bulk asynchronous copies (cp.async.bulk), which must not be pointed at host memory: from
+        // page-locked, device-mapped memory they complete most of the time and now and then never (measured on B200:
+        // the launch hangs once in a few hundred to a few thousand calls).  Host-resident queries go through
+        // tangram_decode_attention_host, which stages them with ordinary loads.
+        cudaPointerAttributes at;
+        const cudaError_t pe = cudaPointerGetAttributes(&at, q);
+        if (pe != cudaSuccess) (void)cudaGetLastError();
+        else if (at.type == cudaMemoryTypeHost)
+            return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention: q is host memory (use tangram_decode_attention_host)");
+    }
     const int G = Hq / dp->H;
     const size_t need = tangram_workspace_bytes(dp->n_part_slots, G, d);
     if (dp->n_part_slots > 0 && (!workspace || workspace_bytes < need))

@@ -11,6 +11,7 @@ import torch
 from oracle import tangram_oracle as O
 from paper_2606_06302_b200 import binding as T
 from paper_2606_06302_b200 import inputs as I
+from conftest import isolated
 
 pytestmark = pytest.mark.gpu
 
@@ -457,9 +458,13 @@ def test_multi_layer_decode_loop_under_one_cuda_graph():
         check(S["out"], S["lse"], ro, rl, "multi-layer graph loop")
 
 
-def test_pinned_host_q_and_outputs_zero_copy():
-    """q, out and lse in pinned host memory passed straight through the C ABI (device-mapped): same bits as the
-    device-resident call, and within tolerance of the oracle."""
+@isolated()
+def test_pinned_host_outputs_zero_copy_and_host_q_refused():
+    """out and lse in pinned host memory passed straight through the C ABI (device-mapped, posted stores): same
+    bits as the device-resident call, launch after launch, and within tolerance of the oracle.  A q in host memory
+    is refused by tangram_decode_attention (its bulk copies must not read mapped host memory: they hang now and
+    then); host-resident queries go through tangram_decode_attention_host and give the same
+    bits."""
     wl = I.make_workload("8b", R=3, ctx_div=8)
     B, res, kv, t, n_pool = setup(wl)
     q, pool = I.make_q_and_pool(wl, n_pool, "cuda")
@@ -469,12 +474,27 @@ def test_pinned_host_q_and_outputs_zero_copy():
     q_h = q.cpu().pin_memory()
     out_h = torch.zeros(q.shape, dtype=torch.bfloat16).pin_memory()
     lse_h = torch.zeros(wl.R, wl.Hq, dtype=torch.float32).pin_memory()
-    for _ in range(2):
-        T.tangram_decode_attention(dp, q_h, pool, out_h, lse_h)
+    for _ in range(50):
+        out_h.zero_(), lse_h.zero_()
+        T.tangram_decode_attention(dp, q, pool, out_h, lse_h)
         torch.cuda.synchronize()
         assert torch.equal(out_h, out_d.cpu()) and torch.equal(lse_h, lse_d.cpu())
     ref_out, ref_lse, _ = O.attention(q.cpu(), pool.cpu(), oracle_tables(t), kv, wl.Hq, wl.d)
     check(out_h, lse_h, ref_out, ref_lse, "pinned host buffers")
+    # the C ABI itself refuses a host q (the binding's own assertion is bypassed on purpose)
+    import ctypes as C
+    ws = torch.empty(T.tangram_workspace_bytes(pl.n_part_slots, wl.G, wl.d), dtype=torch.uint8, device="cuda")
+    rc = T._lib.tangram_decode_attention(C.byref(dp.c), C.c_void_p(q_h.data_ptr()), C.c_void_p(pool.data_ptr()),
+                                         C.c_int64(pool.shape[0]), None, C.c_int32(wl.Hq), C.c_int32(wl.d), C.c_float(0.0),
+                                         C.c_void_p(out_h.data_ptr()), C.c_void_p(lse_h.data_ptr()),
+                                         C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), None, None)
+    assert rc == T.ERR_INVALID_ARG and "host memory" in T._lib.tangram_last_error().decode()
+    q_stage = torch.zeros_like(q)
+    for _ in range(50):
+        out_h.zero_()
+        T.tangram_decode_attention_host(dp, q_h, q_stage, pool, out_h, lse_h, ws)
+        torch.cuda.synchronize()
+        assert torch.equal(out_h, out_d.cpu()) and torch.equal(lse_h, lse_d.cpu())
 
 
 def test_random_sweep_of_shapes_plans_and_runtime_lengths():
@@ -556,6 +576,7 @@ def test_whole_path_from_plain_c(tmp_path):
     assert "c_abi device path ok" in out.stdout
 
 
+@isolated()
 def test_stage_from_host():
     src = torch.randn(3, 40, 128).bfloat16().pin_memory()
     dst = torch.zeros(3, 40, 128, dtype=torch.bfloat16, device="cuda")
@@ -758,6 +779,7 @@ def test_full_size_constant_v_per_head_is_exact(name):
 
 
 @pytest.mark.parametrize("d,W", [(128, None), (64, None), (128, 200), (256, None)])
+@isolated()
 def test_decode_attention_host_entry(d, W):
     """tangram_decode_attention_host: q in pinned host memory staged by the decode kernel itself (per-block flags,
     cooperative grid) or, when the grid cannot be co-resident (W = 200) or d = 256, by the staging kernel with the
