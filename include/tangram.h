@@ -266,7 +266,10 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  *             holds the id of the SM the CTA ran on, %smid); the per-CTA elapsed-time spread of BASELINE.json
  *             is measured from the first two.
  * A device plan carries the launch's scheduler counters: launches on the SAME plan must be ordered (one stream, or
- * events between streams); different plans (e.g. one per layer) may run concurrently.
+ * events between streams); different plans (e.g. one per layer) may run concurrently.  A grid that fits the device
+ * (n_static <= SMs x occupancy: tangram_query_max_ctas) is launched cooperatively, so its in-grid waits are safe next
+ * to any other work; a larger grid is a plain launch whose last CTAs wait for the others -- run such a plan alone
+ * on the device (it is what the tests use to exercise the path, not a serving configuration).
  * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
  * Errors: INVALID_ARG (shape / alignment / unsupported P / d / G / n_pool_pages <= a page id of the tables),

@@ -1025,8 +1025,9 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         // Who may wait: every CTA takes a ticket when its lists are done; the last `merge_ctas` arrivals stay and
         // merge, earlier arrivals (grids larger than the device) leave at once.  A waiting CTA waits for parts that
         // a running CTA writes or that a CTA not yet scheduled will write on a slot a finished CTA left, so the waits
-        // end whenever merge_ctas CTAs fit on the device together (checked by the launcher, which still asks for a
-        // cooperative launch except behind a programmatic dependency).
+        // end whenever merge_ctas CTAs fit on the device together (checked by the launcher, which launches a grid that
+        // fits cooperatively -- gang scheduling keeps the CTAs of other grids, a programmatically dependent successor
+        // in particular, off the SMs this grid still needs).
         // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*M)*K + sub, every thread polls
         // and merges on its own, no barrier inside.  Big records (more than kMergeBigParts parts: the sequences the
         // last rounds of the dynamic tail dice finely) come after the small ones, one (query head, column block)
