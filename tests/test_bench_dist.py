@@ -70,3 +70,20 @@ def test_gpus_flag_must_match_the_world():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--plumbing-only"], env=env,
                          capture_output=True, text=True, timeout=120)
     assert out.returncode != 0 and "WORLD_SIZE" in out.stderr
+
+
+def test_watchdog_prints_the_line_and_leaves_when_a_launch_never_returns():
+    """bench.guarded: the zero-copy e2e leg runs under it.  A call that never comes back (stood in for by a long
+    sleep) makes the watchdog thread print what is known and end the process with status 0; a call that returns in
+    time returns its value and the watchdog stays silent."""
+    import subprocess
+    import time
+    code = ("import sys, os, time; sys.path.insert(0, %r); import bench\n"
+            "def give_up():\n    print('LINE', flush=True); os._exit(0)\n"
+            "print(bench.guarded(lambda: 41 + 1, 5.0, give_up), flush=True)\n"
+            "bench.guarded(lambda: time.sleep(60), 0.5, give_up)\n"
+            "print('NOT REACHED', flush=True)\n") % ROOT
+    t0 = time.time()
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=50)
+    assert r.returncode == 0 and r.stdout.split() == ["42", "LINE"], (r.stdout, r.stderr)
+    assert time.time() - t0 < 40
