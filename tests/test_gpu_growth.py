@@ -169,6 +169,17 @@ def test_decode_step_small_grid_and_static_plan():
         run_decode_steps(wl, B, kv, t, to, free, steps=20, W=W, dyn=(0, 0))
 
 
+@pytest.mark.parametrize("flags", [0, T.STEP_OVERLAP])
+def test_decode_step_on_a_grid_larger_than_the_device(flags):
+    """W = 300 work lists = 300 CTAs, more than fit the device: a plain launch whose first 152 CTAs to finish leave at
+    once and whose last 148 merge; the CTA with the last ticket updates the lengths and grows the tables.  With
+    TANGRAM_STEP_OVERLAP such a grid waits for its predecessor but does not let its own dependents start early."""
+    wl = I.make_workload("8b", R=3, ctx_div=16)
+    B, kv, t, to, free = growable_setup(wl, headroom=3)
+    ref_kv, over, starved = run_decode_steps(wl, B, kv, t, to, free, steps=24, W=300, flags=flags, dyn=(300, 2))
+    assert over == 0 and starved == 0
+
+
 def test_decode_step_starvation_drops_and_counts():
     """A free list that runs out and headroom that runs out: exactly the oracle's rows are dropped and counted, the
     other heads keep growing, and nothing outside the written rows changes (the pool is compared bit for bit)."""
