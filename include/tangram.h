@@ -439,9 +439,10 @@ int tangram_decode_step(const tangram_device_plan* dp, const void* q, const void
  *                 token indices in ascending order (the set I of Eq. 4); the rest is not touched
  *   clamped_dev   device i32 or NULL: incremented by the number of clamped heads
  *   workspace     device, >= tangram_compact_workspace_bytes(R, H), 16-byte aligned
- * Asynchronous on `stream`; graph capturable.  Three launches (prepare, select, gather); the gather is launched
- * behind the select programmatically and moves a row as soon as that row's selection is written (per-row ready
- * flags), so the two overlap; the call is complete when the gather grid is.  TANGRAM_COMPACT_OVERLAP = 0 / 1 in the
+ * Asynchronous on `stream`; graph capturable.  Three launches (prepare, select, gather), each behind its predecessor
+ * programmatically: the select is set up while the prepare kernel runs and waits for its results; the gather moves a
+ * row as soon as that row's selection is written (per-row ready flags), so select and gather overlap; the call is
+ * complete when the gather grid is.  TANGRAM_COMPACT_OVERLAP = 0 / 1 in the
  * environment forces the gather-heavy decision (whether the select leaves half of every SM to the gather), a
  * measurement aid; by default it is taken from the batch.  Errors: INVALID_ARG, BUFFER_TOO_SMALL, CUDA. */
 size_t tangram_compact_workspace_bytes(int32_t R, int32_t H);

@@ -81,6 +81,7 @@ compact_prepare_kernel(const int32_t* __restrict__ seq_cap, const int32_t* __res
                        int32_t* __restrict__ sm_first, int32_t* __restrict__ clamped, int row_bytes, int overlap) {
     __shared__ int s_warp[32];
     __shared__ int s_run, s_bad, s_heavy;
+    asm volatile("griddepcontrol.launch_dependents;");  // the select grid may be set up while this CTA works
     __shared__ unsigned long long s_kept, s_scored;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_run = 0, s_bad = 0, s_kept = 0ull, s_scored = 0ull;
@@ -478,6 +479,8 @@ topk_select_kernel(const float* __restrict__ scores, int64_t n_max, const int32_
                    int32_t* __restrict__ counter, int32_t* __restrict__ ready, int32_t* __restrict__ sm_first,
                    int32_t* __restrict__ idx_out) {
     __shared__ SelectSmem<NT> sm;
+    // launched behind the prepare kernel programmatically: wait for its results, then let the gather in
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;");
     if (NT < 1024 && __ldcg(counter + 3)) {
         if (threadIdx.x == 0) {
@@ -716,13 +719,36 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
                                                8 * d, wide ? 0 : overlap_env);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail2(e, "compact prepare launch");
-    if (wide)
-        topk_select_kernel<1024><<<std::min(n_seq, sms), 1024, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, n_seq,
-                                                                       w.order, w.counter, w.ready, w.sm_first, idx_out);
-    else
-        topk_select_kernel<512><<<std::min(n_seq, 2 * sms), 512, 0, st>>>(scores, n_max, ctx_len_dev, w.keep_eff, dp->H, n_seq,
-                                                                         w.order, w.counter, w.ready, w.sm_first, idx_out);
-    e = cudaGetLastError();
+    static int pdl_state = -1;  // programmatic stream serialization: -1 not tried, 1 accepted, 0 refused
+    {
+        cudaLaunchConfig_t cfg{};
+        cfg.blockDim = dim3(wide ? 1024 : 512), cfg.gridDim = dim3((unsigned)(wide ? std::min(n_seq, sms) : std::min(n_seq, 2 * sms)));
+        cfg.dynamicSmemBytes = 0, cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        const int64_t n_max_ = n_max;
+        const int H_ = dp->H;
+        const int32_t* keep_c = w.keep_eff;
+        const int32_t* order_c = w.order;
+        auto go = [&]() {
+            return wide ? cudaLaunchKernelEx(&cfg, topk_select_kernel<1024>, scores, n_max_, ctx_len_dev, keep_c, H_, n_seq, order_c,
+                                             w.counter, w.ready, w.sm_first, idx_out)
+                        : cudaLaunchKernelEx(&cfg, topk_select_kernel<512>, scores, n_max_, ctx_len_dev, keep_c, H_, n_seq, order_c,
+                                             w.counter, w.ready, w.sm_first, idx_out);
+        };
+        cfg.numAttrs = pdl_state != 0 ? 1 : 0;
+        e = go();
+        if (cfg.numAttrs == 1) {
+            if (e == cudaSuccess) pdl_state = 1;
+            else {
+                (void)cudaGetLastError();
+                pdl_state = 0, cfg.numAttrs = 0;
+                e = go();
+            }
+        }
+    }
     if (e != cudaSuccess) return cuda_fail2(e, "top-k select launch");
     const uint4* kd = static_cast<const uint4*>(k_dense);
     const uint4* vd = static_cast<const uint4*>(v_dense);
@@ -730,7 +756,6 @@ static int compact_impl(const tangram_device_plan* dp, const float* scores, cons
     // The gather is launched behind the select with programmatic stream serialization and never waits for the whole
     // select grid, only for the rows it is about to move.  If the driver refuses the attribute once it is not asked
     // again (a failing launch inside a stream capture would invalidate the capture); a plain launch is correct too.
-    static int pdl_state = -1;  // -1 not tried, 1 accepted, 0 refused
     auto gather = [&](auto kernel, int& grid) -> cudaError_t {
         if (grid == 0) {  // persistent grid: SMs x resident CTAs
             int per_sm = 0;
