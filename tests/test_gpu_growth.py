@@ -153,6 +153,19 @@ def test_decode_step_equals_extend_append_attend(name, kw):
     assert over == 0 and starved == 0 and np.array_equal(ref_kv, kv + 40)
 
 
+def test_decode_step_full_size_8b_in_the_decode_loop_configuration():
+    """The fused step at BASELINE.json's full 8b size in the configuration bench.py's decode loop times (W = N_CTA,
+    open-ended plan over the tables' capacity, default dynamic tail, TANGRAM_STEP_OVERLAP): after each of three steps
+    the whole 0.9 GB pool, the lengths, the tables and the counters equal the oracle's bit for bit and every output
+    row is within tolerance of the oracle's attention over the grown cache."""
+    wl = I.make_workload("8b")
+    B, kv, t, to, free = growable_setup(wl, headroom=2)
+    W = n_cta(wl)
+    dyn = T.tangram_default_dynamic_tail(slot_capacity(t, wl), W, wl.granule, 1)
+    ref_kv, over, starved = run_decode_steps(wl, B, kv, t, to, free, steps=3, flags=T.STEP_OVERLAP, W=W, dyn=dyn)
+    assert over == 0 and starved == 0 and np.array_equal(ref_kv, kv + 3)
+
+
 def test_decode_step_page_size_32():
     """The fused step on 32-token pages: growth hands out a page every 32 tokens per row."""
     wl = I.make_workload("8b", R=3, ctx_div=32, page_size=32)
