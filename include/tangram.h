@@ -323,6 +323,45 @@ int tangram_merge_partials(const tangram_device_plan* dp, int32_t Hq, int32_t d,
                            void* workspace, size_t workspace_bytes, void* stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * tangram_decode_attention for callers that have no device memory to give and must not allocate any.
+ *
+ * Who that is.  The decode attention of a serving engine runs in the engine's steady state: at start-up the engine
+ * measures the model and hands ALL the HBM that is left to its KV page pool (the Block Pool of PAPER.md:89), so when
+ * the per-layer attention call comes there is nothing left for cudaMalloc to return; and a cudaMalloc / cudaFree issued
+ * from the decode loop would in any case synchronise the whole device in the middle of the step and can stall against
+ * a collective that is in flight on another stream.  The same holds for an attention plug-in loaded into a process
+ * whose device memory belongs to somebody else's allocator (a framework's caching allocator, a memory-budgeted
+ * container): it is not the plug-in's place to take memory behind that allocator's back.  Such callers still own q,
+ * the pool, out and lse -- what they do not have is the split-KV WORKSPACE (the fp32 partial outputs and partial LSEs
+ * of every multi-part sequence), which is pure scratch between the decode kernel and the merge.
+ *
+ * What this call does about it.  It is tangram_decode_attention, same kernels and same results, with the workspace
+ * taken from a fixed array of TANGRAM_STATIC_WORKSPACE_BYTES (8 MiB) that is part of the library image: every GPU
+ * that loads libtangram.so holds those 8 MiB from module load until the process exits, whether or not this call is
+ * ever made.  The call itself performs no cudaMalloc, cudaFree or any other allocating CUDA / library routine, on the
+ * first call or on any later one.
+ *
+ *   - Limit: tangram_workspace_bytes(dp->n_part_slots, Hq / H, d) must be <= TANGRAM_STATIC_WORKSPACE_BYTES, else
+ *     TANGRAM_ERR_BUFFER_TOO_SMALL ("... static workspace ...") and nothing is launched.  8 MiB holds about 4 000
+ *     part slots at G = 4, d = 128; on a 148-CTA grid the five configurations of BASELINE.json need 11 KB (tiny),
+ *     2.0 MB (8b), 4.0 MB (32b), 1.8 MB (skew) and 6.3 MB (uniform, 256 requests).  Plans with more parts need the
+ *     caller-workspace call.
+ *   - First call on a device: the array's device address is looked up once per device (with that device current,
+ *     as it is for the launch) and kept; this first call should be made before any stream capture is begun.
+ *   - One array per GPU, shared by EVERY call of this entry point on that GPU, whatever the plan, stream or host
+ *     thread: two such calls that overlap on the GPU (two streams, or two processes' worth of plans in one process)
+ *     write each other's partials -- a race, silently wrong results.  Order them (one stream, or events), or give
+ *     all but one of them a workspace of their own through tangram_decode_attention.
+ *   - The array keeps whatever the last call left in it.  Nothing in it has to start at zero: every partial a merge
+ *     reads was written earlier in the same call (the counters that order the two live in the plan's blob, not
+ *     here), so no clearing is done or needed.
+ * Arguments, results, asynchrony on `stream` and errors otherwise exactly as tangram_decode_attention. */
+#define TANGRAM_STATIC_WORKSPACE_BYTES (8u << 20)
+int tangram_decode_attention_static(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                                    int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d,
+                                    float sm_scale, void* out, float* lse, uint64_t* worker_ns, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
  * NEXT-1  KV append of one decode step.  The new K row and V row of every (request,
  * KV head) are written behind its retained tokens in the ragged pages (:190 page layout), and its length
  * grows by one.  A head whose (request, cluster) row holds no page for the new token (row_pages x P tokens

@@ -78,7 +78,7 @@ for _name in ("tangram_reserve_budgets", "tangram_build_ragged_tables", "tangram
               "tangram_compact_topk_chunk", "tangram_stage_from_host", "tangram_default_dynamic_tail",
               "tangram_extend_tables", "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables",
               "tangram_decode_step", "tangram_reset_plan", "tangram_read_stream", "tangram_overlap_state",
-              "tangram_decode_attention_host"):
+              "tangram_decode_attention_host", "tangram_decode_attention_static"):
     getattr(_lib, _name).restype = C.c_int
 
 EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragged_tables",
@@ -88,8 +88,10 @@ EXPORTS = ("tangram_last_error", "tangram_reserve_budgets", "tangram_build_ragge
            "tangram_calibrate_budgets", "tangram_implicit_ratios", "tangram_compact_topk_chunk",
            "tangram_stage_from_host", "tangram_default_dynamic_tail", "tangram_extend_tables",
            "tangram_extend_tables_device", "tangram_sync_tables", "tangram_download_tables", "tangram_decode_step",
-           "tangram_reset_plan", "tangram_read_stream", "tangram_overlap_state", "tangram_decode_attention_host")
+           "tangram_reset_plan", "tangram_read_stream", "tangram_overlap_state", "tangram_decode_attention_host",
+           "tangram_decode_attention_static")
 STEP_OVERLAP = 1
+STATIC_WORKSPACE_BYTES = 8 << 20     # TANGRAM_STATIC_WORKSPACE_BYTES of include/tangram.h
 
 
 def _check(rc: int):
@@ -318,6 +320,34 @@ def tangram_decode_attention_host(dp: DevicePlan, q_host, q_stage, kv_pool, out,
                                               C.c_int32(d), C.c_float(sm_scale), C.c_void_p(out.data_ptr()),
                                               C.c_void_p(lse.data_ptr()), C.c_void_p(workspace.data_ptr()),
                                               C.c_size_t(workspace.numel()), None, _stream_ptr(stream)))
+    return out, lse
+
+
+def tangram_decode_attention_static(dp: DevicePlan, q, kv_pool, out=None, lse=None, sm_scale: float = 0.0, worker_ns=None,
+                                    stream=None, kv_len=None):
+    """tangram_decode_attention for a caller that cannot allocate the split-KV workspace (a serving engine whose HBM
+    all went to the page pool, code running under somebody else's allocator): the library's fixed 8 MiB array is the
+    workspace and the C call allocates nothing.  Pass `out` and `lse` if this wrapper must not allocate either (when
+    they are None it makes them with torch.empty, like the other wrappers).  Raises TangramError (BUFFER_TOO_SMALL)
+    for a plan whose partials exceed STATIC_WORKSPACE_BYTES.  Every call on a GPU shares the one array: calls that
+    overlap on the GPU race (include/tangram.h)."""
+    import torch
+    assert q.is_cuda and kv_pool.is_cuda and q.dtype == torch.bfloat16 and kv_pool.dtype == torch.bfloat16
+    assert q.is_contiguous() and kv_pool.is_contiguous()
+    R, Hq, d = q.shape
+    assert tuple(kv_pool.shape[1:]) == (dp.c.Hp, 2, dp.c.P, d) and R == dp.c.R
+    if out is None:
+        out = torch.empty(R, Hq, d, dtype=torch.bfloat16, device=kv_pool.device)
+    if lse is None:
+        lse = torch.empty(R, Hq, dtype=torch.float32, device=kv_pool.device)
+    wn = C.c_void_p(worker_ns.data_ptr()) if worker_ns is not None else None
+    if kv_len is not None:
+        assert kv_len.is_cuda and kv_len.dtype == torch.int32 and kv_len.is_contiguous() and kv_len.numel() == R * dp.c.H
+    kvl = C.c_void_p(kv_len.data_ptr()) if kv_len is not None else None
+    _check(_lib.tangram_decode_attention_static(C.byref(dp.c), C.c_void_p(q.data_ptr()), C.c_void_p(kv_pool.data_ptr()),
+                                                C.c_int64(kv_pool.shape[0]), kvl, C.c_int32(Hq), C.c_int32(d),
+                                                C.c_float(sm_scale), C.c_void_p(out.data_ptr()), C.c_void_p(lse.data_ptr()),
+                                                wn, _stream_ptr(stream)))
     return out, lse
 
 

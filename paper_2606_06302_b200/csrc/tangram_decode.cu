@@ -27,6 +27,7 @@
 #include <cstdlib>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <type_traits>
 #include <vector>
 
@@ -1703,6 +1704,59 @@ extern "C" int tangram_decode_attention(const tangram_device_plan* dp, const voi
                                         void* stream) {
     return run_attention(dp, q, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, workspace,
                          workspace_bytes, worker_ns, stream, kRunSplit | kRunMerge);
+}
+
+// ------------------------------------------------------------------ the call that allocates nothing
+// Split-KV workspace for callers that cannot allocate one (include/tangram.h, tangram_decode_attention_static): a
+// serving engine in its decode loop has given all free HBM to its page pool and must not call cudaMalloc there.
+// The array is part of the module image: each GPU that loads the library holds these bytes until the process ends.
+// It is shared by every call on the device and is never cleared (nothing in it needs to start at zero: a merge reads
+// only partials that the same call wrote).
+static __device__ __align__(256) unsigned char g_static_workspace[TANGRAM_STATIC_WORKSPACE_BYTES];
+
+// Device address of g_static_workspace on the CURRENT device.  In host code the name `g_static_workspace` is only
+// the host-side handle of the symbol, not an address a kernel may be given: the real address differs per device and
+// comes from cudaGetSymbolAddress, asked once per device with that device current and then kept.
+static int static_workspace_on_current_device(void** ptr_out) {
+    constexpr int kMaxDevices = 64;
+    static std::mutex mu;
+    static void* ptr_of[kMaxDevices] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "decode_attention_static: cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDevices)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_static: device ordinal %d (at most %d devices)", dev, kMaxDevices);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_workspace);
+        if (e != cudaSuccess) return cuda_fail(e, "decode_attention_static: cudaGetSymbolAddress");
+        if (!p || reinterpret_cast<uintptr_t>(p) % 256)
+            return fail(TANGRAM_ERR_CUDA, "decode_attention_static: static workspace at %p on device %d", p, dev);
+        ptr_of[dev] = p;
+    }
+    *ptr_out = ptr_of[dev];
+    return TANGRAM_OK;
+}
+
+extern "C" int tangram_decode_attention_static(const tangram_device_plan* dp, const void* q, const void* kv_pool,
+                                               int64_t n_pool_pages, const int32_t* kv_len_dev, int32_t Hq, int32_t d,
+                                               float sm_scale, void* out, float* lse, uint64_t* worker_ns, void* stream) {
+    if (!dp) return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_static: NULL plan");
+    if (dp->H < 1 || Hq < 1 || Hq % dp->H != 0 || d < 1)
+        return fail(TANGRAM_ERR_INVALID_ARG, "decode_attention_static: Hq=%d H=%d d=%d", Hq, dp->H, d);
+    // the limit first: a plan with more parts than the fixed array holds is refused before anything is launched
+    const size_t need = tangram_workspace_bytes(dp->n_part_slots, Hq / dp->H, d);
+    if (need > (size_t)TANGRAM_STATIC_WORKSPACE_BYTES)
+        return fail(TANGRAM_ERR_BUFFER_TOO_SMALL,
+                    "decode_attention_static: the plan's %lld part slots need %zu bytes, the static workspace holds %zu "
+                    "(use tangram_decode_attention with a workspace of your own)",
+                    (long long)dp->n_part_slots, need, (size_t)TANGRAM_STATIC_WORKSPACE_BYTES);
+    void* ws = nullptr;
+    const int rc = static_workspace_on_current_device(&ws);
+    if (rc != TANGRAM_OK) return rc;
+    return run_attention(dp, q, kv_pool, n_pool_pages, kv_len_dev, Hq, d, sm_scale, out, lse, ws,
+                         (size_t)TANGRAM_STATIC_WORKSPACE_BYTES, worker_ns, stream, kRunSplit | kRunMerge);
 }
 
 extern "C" int tangram_decode_partials(const tangram_device_plan* dp, const void* q, const void* kv_pool,
