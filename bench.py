@@ -34,35 +34,127 @@ NOMINAL_TBS = 8.0
 FALLBACK_PEAK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
 
 
-def csrc_hash() -> str:
-    """sha256 (first 16 hex digits) over the decode kernel's sources (tangram_decode.cu + tangram_internal.h): ties a
-    committed ncu capture of that kernel to the code it measured."""
+def csrc_hash(files=("tangram_decode.cu", "tangram_internal.h")) -> str:
+    """sha256 (first 16 hex digits) over a kernel's sources (by default the decode kernel's: tangram_decode.cu +
+    tangram_internal.h): ties a committed ncu capture of that kernel to the code it measured."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2606_06302_b200", "csrc")
-    for fn in ("tangram_decode.cu", "tangram_internal.h"):
+    for fn in files:
         h.update(fn.encode())
         h.update(open(os.path.join(d, fn), "rb").read())
     return h.hexdigest()[:16]
 
 
-def profiled_traffic(workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the decode kernel, per launch, from the committed
-    `ncu --set full` capture of this workload (profiles/*_traffic.csv) -- only from a row whose `csrc_hash` column
-    equals the hash of the current kernel sources (a capture of older code says nothing about this build); else None."""
+KERNEL_SOURCES = {"tangram_decode_kernel": ("tangram_decode.cu", "tangram_internal.h"),
+                  "tangram_compact_topk": ("tangram_compact.cu", "tangram_internal.h")}
+
+
+def profiled_traffic(workload: str, kernel: str = "tangram_decode_kernel"):
+    """dram__bytes_read.sum + dram__bytes_write.sum of a kernel (for tangram_compact_topk: of the call's three kernels
+    together), per launch, from the committed `ncu --set full` capture of this workload (profiles/*_traffic.csv) --
+    only from a row whose `csrc_hash` column equals the hash of the current sources of that kernel (a capture of
+    older code says nothing about this build); else None."""
     best = None
     try:
         import csv
         import glob
-        cur = csrc_hash()
+        cur = csrc_hash(KERNEL_SOURCES[kernel])
         for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
             for row in csv.DictReader(open(path)):
-                if (row["workload"] == workload and row["kernel"] == "tangram_decode_kernel"
-                        and row.get("csrc_hash", "") == cur):
+                if row["workload"] == workload and row["kernel"] == kernel and row.get("csrc_hash", "") == cur:
                     best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
     except Exception:
         return None
     return best
+
+
+def sig(x, n=4):
+    """x rounded to n significant digits (None, bools, ints and strings pass through)."""
+    if isinstance(x, bool) or not isinstance(x, float):
+        return x
+    if x == 0 or not math.isfinite(x):
+        return x
+    return round(x, n - 1 - int(math.floor(math.log10(abs(x)))))
+
+
+COMPACT_LINE_LIMIT = 4096      # bytes; the driver's record kept round 1's 10.6 KB line and lost round 2's 21.6 KB one
+
+
+def compact_line(line: dict) -> dict:
+    """The ONE JSON line the driver keeps, built from the verbose record: the contract's keys, `roofline`,
+    `cpu_baseline`, `e2e`, `clocks`, `gpu_launches` and a `config` that names the workload, the plan and one summary row
+    per configuration -- numbers to 3-4 significant digits, no prose, nothing twice.  Everything else stays in the
+    verbose record (the BENCH_DETAIL line printed before it, gpurun_out/bench_detail.json)."""
+    cfg = line.get("config", {})
+    out = {k: sig(line[k], 6) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step",
+                                        "higher_is_better", "scaling", "vs_baseline", "dtype", "data") if k in line}
+    if "impl" in line:
+        out["impl"] = line["impl"]
+    out["us_per_layer_step"] = sig(line.get("us_per_layer_step"))
+    out["pct_of_8tbs_nominal"] = sig(line.get("pct_of_8tbs_nominal"))
+    c = {k: cfg[k] for k in ("workload", "R", "Hq", "H", "d", "page_size", "clusters", "plan", "W", "dyn_permille",
+                             "dyn_rounds", "granule", "c0", "items", "kv_bytes", "algorithmic_bytes") if k in cfg}
+    c["l2"] = "inputs > L2 and an L2 flush before every timed step"
+    c["multi_gpu"] = "replicas only"
+    if "cta_spread" in line:
+        c["cta_spread"] = sig(line["cta_spread"], 3)
+    per = line.get("per_config")
+    if per:
+        cols = ["us", "tbs", "pct_of_8tbs", "kernel_gbs", "cta_spread", "static_even_x", "traffic_ratio"]
+        rows = {}
+        for k, v in per.items():
+            rows[k] = [sig(v.get("us_per_layer_step"), 4), sig(v.get("tbs"), 3), sig(v.get("pct_of_8tbs"), 3),
+                       sig(v.get("decode_kernel_gbs"), 4), sig(v.get("cta_spread"), 2),
+                       sig(v.get("static_even", {}).get("slowdown_vs_balanced"), 3), sig(v.get("traffic_ratio"), 4)]
+        c["per_config_summary"] = {"columns": cols, **rows}
+    dl = line.get("decode_loop")
+    if dl:
+        c["decode_loop"] = {"us_per_layer_step": sig(dl.get("us_per_layer_step")), "layers": dl.get("layers"),
+                            "launches_per_layer_step": dl.get("launches_per_layer_step"), "overflow": dl.get("overflow")}
+    ct = line.get("compact_topk")
+    if ct:
+        c["compact_topk"] = {"us": sig(ct.get("us")), "pct_of_measured_copy": sig(ct.get("pct_of_measured_copy"), 3),
+                             "roofline": {k: sig(v) for k, v in ct.get("roofline", {}).items()}}
+    out["config"] = c
+    r = line.get("roofline", {})
+    out["roofline"] = {k: sig(r[k], 5) for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic",
+                                                 "kernel_us", "algorithmic_bytes_per_launch", "read_peak_gbs",
+                                                 "frac_of_read_peak") if k in r}
+    if "peak_source" in r:
+        out["roofline"]["peak_source"] = "measured" if str(r["peak_source"]).startswith("measured") else "fallback"
+    cb = line.get("cpu_baseline")
+    if cb:
+        out["cpu_baseline"] = {k: sig(cb[k]) for k in ("value", "unit", "cores", "kind") if k in cb}
+        out["cpu_baseline"]["sample"] = str(cb.get("sample", ""))[:160]
+        if "us_per_layer_step_extrapolated" in cb:
+            out["cpu_baseline"]["us_per_layer_step_extrapolated"] = sig(cb["us_per_layer_step_extrapolated"])
+    e = line.get("e2e")
+    if e:
+        out["e2e"] = {k: sig(e[k]) for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "us_per_layer_step",
+                                             "us_per_layer_step_staged_copies", "zero_copy", "zero_copy_hung") if k in e}
+    if "clocks" in line:
+        out["clocks"] = line["clocks"]
+    if "gpu_launches" in line:
+        out["gpu_launches"] = line["gpu_launches"]
+    out["detail"] = "BENCH_DETAIL line above; gpurun_out/bench_detail.json"
+    return out
+
+
+def emit(line: dict):
+    """Prints the verbose record on a line of its own behind a non-JSON prefix (and writes it to
+    gpurun_out/bench_detail.json when that folder can be written), then -- LAST -- the compact JSON line."""
+    detail = json.dumps(line)
+    print("BENCH_DETAIL " + detail, flush=True)
+    try:
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, "gpurun_out", "bench_detail.json"), "w") as f:
+            f.write(detail + "\n")
+    except OSError:
+        pass
+    text = json.dumps(compact_line(line), separators=(",", ":"))
+    assert "\n" not in text and len(text.encode()) <= COMPACT_LINE_LIMIT, f"compact bench line is {len(text.encode())} bytes"
+    print(text, flush=True)
 
 
 def measured_peak():
@@ -471,7 +563,10 @@ def compact_topk_summary(T, I, name, device, steps, flush, torch, peak_gbs):
     gather_bytes = kept * 4 * wl.d * 2 + kept * 4            # rows read + rows written + indices read
     score_bytes = int(wl.ctx_len.astype(np.int64).sum()) * wl.H * 4
     us = float(np.median(ms) * 1e3)
-    return {"workload": name, "us": us, "us_min": float(np.min(ms) * 1e3), "launches": 3,
+    gbs = gather_bytes / (us * 1e-6) / 1e9
+    roof = {"bound": "hbm", "achieved": gbs, "peak": peak_gbs, "unit": "GB/s", "frac": gbs / peak_gbs,
+            "traffic": profiled_traffic(name, "tangram_compact_topk")}
+    return {"workload": name, "us": us, "us_min": float(np.min(ms) * 1e3), "launches": 3, "roofline": roof,
             "retained_token_heads": kept, "gather_bytes": gather_bytes, "score_bytes_one_pass": score_bytes,
             "gbs_gather_bytes_over_total_time": gather_bytes / (us * 1e-6) / 1e9,
             "pct_of_measured_copy": 100 * gather_bytes / (us * 1e-6) / 1e9 / peak_gbs,
@@ -592,6 +687,10 @@ def measure_config(T, I, name, device, steps, warmup, flush, torch, peak_gbs, co
            "algorithmic_bytes": b, "W": S["W"], "items": int(S["plan"].n_items), "granule": S["wl"].granule,
            "c0": S["c0"], "dyn_permille": S["dyn"][0], "dyn_rounds": S["dyn"][1], "host_ms": S["host_ms"],
            "cta_spread": spread_of(T, S, torch), "timeline": timeline_of(T, S, torch, flush)}
+    # DRAM bytes of the committed ncu capture of this configuration / the kernel's algorithmic bytes (None: no capture
+    # of the current sources); only for the configuration as BASELINE.json names it
+    tr = profiled_traffic(name) if R is None and page_size is None else None
+    res["traffic_ratio"] = tr / (b["total"] - b["partials"] // 2) if tr else None
     if compare:
         legs = [(T.MODE_STATIC_EVEN, "static_even"), (T.MODE_SPLITMAP, "splitmap")]
         if S["dyn"][1] > 0:                   # the same equal-bytes plan, every CTA owning exactly one list
@@ -852,7 +951,8 @@ def main():
                     + "; the KV page pool is resident serving state in HBM")
         return {"value": e_bytes / (ms_ * 1e-3) / 1e12, "unit": "TB/s", "us_per_layer_step": ms_ * 1e3,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "us_per_layer_step_staged_copies": e_ms_staged * 1e3, "zero_copy": zero_copy_ms is not None, "note": note}
+                "us_per_layer_step_staged_copies": e_ms_staged * 1e3, "zero_copy": zero_copy_ms is not None,
+                "zero_copy_hung": bool(hung), "note": note}
 
     if rank != 0:
         if world > 1:
@@ -899,7 +999,7 @@ def main():
         del S
         torch.cuda.empty_cache()
         line["decode_loop"] = decode_loop(T, I, args.workload, device, args.decode_loop_layers or 2, 12, torch)
-        print(json.dumps(line))
+        emit(line)
         return
     if not args.no_sweep and world == 1:
         per = {}
@@ -975,12 +1075,12 @@ def main():
         prepare(T, S, torch)
 
         def give_up():
-            line["e2e"] = e2e_entry(None, hung=True)
-            print(json.dumps(line), flush=True)
+            line["e2e"] = e2e_entry(None, hung=True)      # e2e.zero_copy_hung = true: the fall-back is on the record
+            emit(line)
             os._exit(0)
         ems = guarded(lambda: e2e_steps(T, S, args.steps, 3, flush, torch, zero_copy=True)[0], 180.0, give_up)
         line["e2e"] = e2e_entry(float(np.mean(ems)))
-    print(json.dumps(line))
+    emit(line)
     if world > 1:
         dist.destroy_process_group()
 

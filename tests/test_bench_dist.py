@@ -87,3 +87,51 @@ def test_watchdog_prints_the_line_and_leaves_when_a_launch_never_returns():
     r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=50)
     assert r.returncode == 0 and r.stdout.split() == ["42", "LINE"], (r.stdout, r.stderr)
     assert time.time() - t0 < 40
+
+
+def test_compact_bench_line_is_small_single_line_and_complete(capsys, tmp_path, monkeypatch):
+    """The line the driver keeps: bench.compact_line on a canned verbose record (tests/golden/bench_verbose_record.json
+    = the 21.6 KB line of round 2, which the driver could not keep) must be one line of JSON under 4 KB that round-trips
+    and still carries the contract's keys, `roofline`, `cpu_baseline`, `e2e`, `clocks` and the per-configuration summary;
+    emit() prints the verbose record first, behind a non-JSON prefix, and the compact line LAST."""
+    import json
+    sys.path.insert(0, ROOT)
+    import bench
+    rec = json.load(open(os.path.join(ROOT, "tests", "golden", "bench_verbose_record.json")))
+    assert len(json.dumps(rec)) > 20000
+    rec["e2e"]["zero_copy_hung"] = False
+    for v in rec["per_config"].values():
+        v["traffic_ratio"] = 1.00369
+    rec["compact_topk"]["roofline"] = {"bound": "hbm", "achieved": 5771.123, "peak": 6533.2, "unit": "GB/s",
+                                       "frac": 0.88335, "traffic": 1601234567}
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))          # emit() writes gpurun_out/bench_detail.json under ROOT
+    bench.emit(rec)
+    lines = capsys.readouterr().out.strip("\n").split("\n")
+    assert len(lines) == 2 and lines[0].startswith("BENCH_DETAIL {")
+    assert json.loads(lines[0][len("BENCH_DETAIL "):]) == rec
+    assert json.loads(open(tmp_path / "gpurun_out" / "bench_detail.json").read()) == rec
+    last = lines[-1]
+    assert len(last.encode()) < 4096 and "\n" not in last
+    c = json.loads(last)
+    assert c == bench.compact_line(rec)
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "clocks", "gpu_launches"):
+        assert k in c, k
+    assert c["value"] > 0 and c["metric"] == rec["metric"] and c["config"]["workload"] == "8b"
+    for k in ("bound", "achieved", "peak", "unit", "frac", "traffic"):
+        assert k in c["roofline"], k
+    assert abs(c["roofline"]["frac"] - rec["roofline"]["frac"]) < 1e-3
+    for k in ("value", "unit", "cores", "kind", "sample"):
+        assert k in c["cpu_baseline"], k
+    for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "zero_copy_hung"):
+        assert k in c["e2e"], k
+    summ = c["config"]["per_config_summary"]
+    for name in ("tiny", "8b", "32b", "skew", "uniform"):                  # the five configurations of BASELINE.json
+        assert len(summ[name]) == len(summ["columns"])
+    assert abs(summ["32b"][summ["columns"].index("pct_of_8tbs")] - rec["per_config"]["32b"]["pct_of_8tbs"]) < 0.1
+    assert summ["skew"][summ["columns"].index("cta_spread")] == bench.sig(rec["per_config"]["skew"]["cta_spread"], 2)
+    # a record with every optional block missing (multi-rank run) still gives a valid line
+    small = {k: rec[k] for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                                 "scaling", "vs_baseline", "dtype", "data", "roofline", "e2e", "clocks", "gpu_launches")}
+    small["config"] = {"workload": "8b"}
+    assert len(json.dumps(bench.compact_line(small))) < 2048
