@@ -78,7 +78,9 @@ int tangram_reserve_budgets(const double* mu, const double* sigma, double alpha,
  *   free_pages   host [n_free] i32 page ids the caller's allocator hands out (not modified)
  *   flags        TANGRAM_FILL_GROUP: kv_len_inout[r][h] := max reserved of h's cluster (:235)
  *   kv_len_inout host [R][H] i32 or NULL (only touched with TANGRAM_FILL_GROUP)
- *   out          caller-filled: perm/cluster_of/slot_of [H], tbl_indptr [R*C+1], tbl_pages
+ *   out          ZERO-INITIALISE the struct first (memset / = {0}): it carries inputs (headroom_pages, row_pages,
+ *                tbl_pages_cap) next to outputs and has no version field, so a field a caller does not know about
+ *                must read as 0.  Then caller-filled: perm/cluster_of/slot_of [H], tbl_indptr [R*C+1], tbl_pages
  *                [tbl_pages_cap] (or tbl_pages == NULL to query: only n_pages_used / n_slots are
  *                written), headroom_pages (in), row_pages [R*C] (or NULL if headroom_pages == 0).
  *                On success R,H,C,Hp,P, the arrays, n_pages_used and n_slots are written.
@@ -195,7 +197,7 @@ typedef struct tangram_device_plan {
     int64_t n_empty_seqs;       /* of these, the first n_empty_seqs have no part at all (kv_len 0) */
     int64_t n_big_merge_seqs;   /* ... and the last n_big_merge_seqs have more than 16 parts */
     const int32_t* merge_seqs;  /* device [n_merge_seqs][4]: {r * H + h, first part slot, parts, 0}, empty
-                                   sequences first, then by part count <= 32 / > 32 */
+                                   sequences first, then by part count <= 16 / > 16 */
     const void* items;          /* device: 32-byte device items (cluster replaced by the table row offset) */
     const int64_t* worker_indptr; /* device [W+1] */
     const void* list_heads;       /* device [W] 128-byte list heads: item range, first item, its first 16 page ids */
@@ -240,10 +242,10 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
 /* a4 + a5  One layer, whole batch: split-KV decode kernel over the work lists, then the LSE merge -- inside the
  * same persistent grid and without a grid barrier: every part of a multi-part sequence is published by a release add
  * on the sequence's counter (dp->seq_done), and a CTA that is out of work lists merges its share of the sequences,
- * each as soon as the counter shows all parts of this launch (ONE launch: cooperative when the grid fits on the
- * device, else the last SMs x occupancy CTAs to finish do the merging); the stand-alone merge kernel follows as a
- * second launch only at d = 256 or when a merge record is wider than the CTA (G x d/4 > consumer threads: d = 128
- * with G > 8, or G > 4 on 32-token pages).
+ * each as soon as the counter shows all parts of this launch (ONE cooperative launch whenever the grid fits on the
+ * device: n_static <= tangram_query_max_ctas); the stand-alone merge kernel follows as a second launch when the grid
+ * is larger than that (CTAs that wait for one another must be gang-scheduled), at d = 256, or when a merge record is
+ * wider than the CTA (G x d/4 > consumer threads: d = 128 with G > 8, or G > 4 on 32-token pages).
  * Asynchronous on `stream`; CUDA-graph capturable; no host work besides the launch.
  *
  *   dp        from tangram_upload (host struct holding device pointers)
@@ -268,8 +270,8 @@ size_t tangram_workspace_bytes(int64_t n_part_slots, int32_t gqa, int32_t head_d
  * A device plan carries the launch's scheduler counters: launches on the SAME plan must be ordered (one stream, or
  * events between streams); different plans (e.g. one per layer) may run concurrently.  A grid that fits the device
  * (n_static <= SMs x occupancy: tangram_query_max_ctas) is launched cooperatively, so its in-grid waits are safe next
- * to any other work; a larger grid is a plain launch whose last CTAs wait for the others -- run such a plan alone
- * on the device (it is what the tests use to exercise the path, not a serving configuration).
+ * to any other work; a larger grid is a plain launch with no wait inside (merge, lengths and table growth run in
+ * follow-up kernels), safe next to other work as well, just slower -- not a serving configuration.
  * Computes, for every (r, j): softmax(q_j K~^T * sm_scale) V~ over exactly the kv_len retained
  * tokens of its KV head (Eq. 1, :57), fp32 accumulation, bf16 output.
  * Errors: INVALID_ARG (shape / alignment / unsupported P / d / G / n_pool_pages <= a page id of the tables),
@@ -407,8 +409,13 @@ int tangram_append_kv(const tangram_device_plan* dp, const void* k_new, const vo
  * Device path (zero host work per step, CUDA-graph capturable): tangram_extend_tables_device runs the same update
  * on the device copy (one small kernel: a block-wide ordered scan over the rows); the free-list cursor and the
  * starved count live in dp->grow_state.  tangram_decode_step below runs it inside the decode kernel.
- *   free_pages_dev  device [n_free] i32: the free list the tables were built from (every entry must be a page of
- *                   the pool the attention calls are given; the device calls cannot check that)
+ *   free_pages_dev  device [n_free] i32: the free list the tables were built from.  Every entry must be a page of
+ *                   the pool the attention calls are given.  tangram_decode_step knows the pool's size and hands out
+ *                   no entry outside [0, n_pool_pages) (the row counts as starved instead);
+ *                   tangram_extend_tables_device and tangram_sync_tables do not know it and cannot check, so as the
+ *                   last line of defence tangram_append_kv and the fused append never STORE through a page id outside
+ *                   the pool they are given (tangram_append_kv keeps the length and counts the row in overflow_dev;
+ *                   reads of such a page are clamped by the hardware).
  * tangram_download_tables copies the device state (tbl_pages, row_pages, n_pages_used) back into *t (host arrays
  * sized as at build time) and synchronises the stream. */
 int tangram_extend_tables(tangram_tables* t, const int32_t* kv_len, const int32_t* free_pages, int64_t n_free,

@@ -67,6 +67,8 @@ struct GrowParams {
     const int32_t* free_pages;   // [n_free] or nullptr: no growth
     int32_t* overflow;           // dropped rows, or nullptr
     int32_t n_free, n_rows, R, H, C, Hp;
+    int32_t n_pool_pages;        // pages of the pool the caller passed (INT32_MAX: not known to this call): a free-list
+                                 // entry outside [0, n_pool_pages) is not handed out -- the row counts as starved
 };
 
 struct DecodeParams {
@@ -96,6 +98,7 @@ struct DecodeParams {
     const uint4* k_new;          // [R*H][d/8] or nullptr: no append
     const uint4* v_new;
     uint4* pool_w;               // the page pool, writable view
+    int32_t n_pool_pages;        // its pages: an appended row is only stored to a page id inside [0, n_pool_pages)
     const int32_t* seq_cap;      // [R*H] tokens the row's pages hold
     int32_t* kv_len_w;           // = kv_len, writable
     GrowParams grow;
@@ -519,9 +522,12 @@ __device__ __forceinline__ void extend_rows(const GrowParams& g, int page_tokens
         block_sync<NT, NAMED_BAR>();
         const int idx = cursor0 + granted + s_scan[wid] + __popc(bal & ((1u << lane) - 1u));
         const int total = s_scan[32];
-        const bool ok = can && idx < g.n_free;
+        // a free-list entry that is not a page of the pool is never written into the tables (the appends store through
+        // the tables without a hardware bound, unlike the TMA reads): the row is starved instead
+        const int new_page = can && idx < g.n_free ? g.free_pages[idx] : -1;
+        const bool ok = new_page >= 0 && new_page < g.n_pool_pages;
         if (ok) {
-            g.tbl_pages[lo + have] = g.free_pages[idx];
+            g.tbl_pages[lo + have] = new_page;
             g.row_pages[row] = have + 1;
             for (int k = 0; k < g.Hp; ++k) g.seq_cap[r * g.H + g.perm[c * g.Hp + k]] = (have + 1) * page_tokens;
         }
@@ -644,6 +650,10 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             head_pid_lo = __shfl_sync(0xffffffffu, w, 12 + i0);
             head_pid_hi = __shfl_sync(0xffffffffu, w, 12 + kNW + i0);
         };
+        // Page ids: through the read-only (non-coherent) path only in launches that cannot write the tables; a fused
+        // decode step grows them in its tail phase (extend_rows), so there they are read from L2.
+        const bool tables_grow = p.k_new != nullptr;
+        auto load_pid = [&](const int32_t* a) { return tables_grow ? __ldcg(a) : __ldg(a); };
         auto load_head = [&](int list) {
             take_head(__ldg(reinterpret_cast<const int*>(p.list_heads) + static_cast<size_t>(list) * 32 + lane));
         };
@@ -661,11 +671,11 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 const int32_t* ids = p.tbl_pages + next.tbl_row + next.tok_begin / kPage;
                 int i = (lane - (next.part_slot & (kNW - 1))) & (kNW - 1);
                 int pid = head_pid_lo;
-                if (i < n_tiles && pid < 0) pid = __ldg(ids + i);
+                if (i < n_tiles && pid < 0) pid = load_pid(ids + i);
                 while (i < n_tiles && prefilled < NS) {
                     const int i_next = i + kNW;
                     int pid_next = i_next < 2 * kNW ? head_pid_hi : 0;
-                    if (i_next < n_tiles && (i_next >= 2 * kNW || pid_next < 0)) pid_next = __ldg(ids + i_next);
+                    if (i_next < n_tiles && (i_next >= 2 * kNW || pid_next < 0)) pid_next = load_pid(ids + i_next);
                     mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
                     tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
                                   (pid * p.Hp + next.slot) * (2 * kPage), policy);
@@ -702,11 +712,13 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     // the V row; the proxy fence orders these generic-proxy stores before the TMA (async proxy)
                     // reads of the same page issued below by this warp.
                     const int n = item.tok_end - 1;
-                    const int page = __ldg(p.tbl_pages + item.tbl_row + n / kPage);
+                    const int page = __ldcg(p.tbl_pages + item.tbl_row + n / kPage);
                     const size_t row_k = ((static_cast<size_t>(page) * p.Hp + item.slot) * 2) * kPage + n % kPage;
                     const size_t sq = static_cast<size_t>(item.req) * p.H + item.kv_head;
                     constexpr int chunks = D / 8;
-                    for (int c = lane; c < 2 * chunks; c += 32) {
+                    // (a page id outside the pool -- tables synced from a host that was given a wrong free list --
+                    // is never stored through; the TMA reads of such a page are clamped by the tensor map)
+                    for (int c = lane; c < 2 * chunks && static_cast<unsigned>(page) < static_cast<unsigned>(p.n_pool_pages); c += 32) {
                         const bool is_v = c >= chunks;
                         const int cc = is_v ? c - chunks : c;
                         const uint4 val = __ldcg((is_v ? p.v_new : p.k_new) + sq * chunks + cc);
@@ -744,7 +756,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                         pid = head_item ? head_pid_lo : 0;
                         // a list head caches the page ids its first item had at upload time; a slot that got its
                         // page later (table growth) is read from the table
-                        if (i < n_tiles && (!head_item || pid < 0)) pid = __ldg(ids + i);
+                        if (i < n_tiles && (!head_item || pid < 0)) pid = load_pid(ids + i);
                     }
                     // lane 0 issues the claim kClaimTiles tiles before the end of the item's TMA issue: late
                     // enough that the CTA does not hoard a list, early enough to cover the claim -> list
@@ -757,7 +769,7 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                         }
                         const int i_next = i + kNW;
                         int pid_next = head_item && i_next < 2 * kNW ? head_pid_hi : 0;
-                        if (i_next < n_tiles && (!head_item || i_next >= 2 * kNW || pid_next < 0)) pid_next = __ldg(ids + i_next);
+                        if (i_next < n_tiles && (!head_item || i_next >= 2 * kNW || pid_next < 0)) pid_next = load_pid(ids + i_next);
                         mbar_wait(empty_bar(lane, stage), phase ^ 1);
                         mbar_arrive_expect_tx(full_bar(lane, stage), kTile);
                         tma_load_tile(tiles + (lane * NS + stage) * kTile, &kv_map, full_bar(lane, stage),
@@ -1023,12 +1035,11 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
         // the work lists complete them -- so a CTA that runs out of work early merges what is already complete while
         // the others still stream, and after the last part of the launch is written only the records that contain
         // parts of the last lists remain.
-        // Who may wait: every CTA takes a ticket when its lists are done; the last `merge_ctas` arrivals stay and
-        // merge, earlier arrivals (grids larger than the device) leave at once.  A waiting CTA waits for parts that
-        // a running CTA writes or that a CTA not yet scheduled will write on a slot a finished CTA left, so the waits
-        // end whenever merge_ctas CTAs fit on the device together (checked by the launcher, which launches a grid that
-        // fits cooperatively -- gang scheduling keeps the CTAs of other grids, a programmatically dependent successor
-        // in particular, off the SMs this grid still needs).
+        // Who may wait: a waiting CTA waits for parts that another CTA of the grid writes, so every CTA of the grid
+        // must be resident: the launcher enables this phase only for a grid that fits on the device and launches it
+        // cooperatively -- gang scheduling also keeps the CTAs of other grids, a programmatically dependent successor
+        // in particular, off the SMs this grid still needs.  Every CTA takes a ticket when its
+        // lists are done (merge_ctas = the grid; the ticket decides who does the step's bookkeeping below).
         // Small records: sub-group `sub` of G*D/4 threads takes records (first + j*M)*K + sub, every thread polls
         // and merges on its own, no barrier inside.  Big records (more than kMergeBigParts parts: the sequences the
         // last rounds of the dynamic tail dice finely) come after the small ones, one (query head, column block)
@@ -1091,6 +1102,9 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                 step_lengths<kNW * 32, true>(p.grow, threadIdx.x);
                 if (p.grow.free_pages) extend_rows<kNW * 32, true>(p.grow, kPage, threadIdx.x, reinterpret_cast<int*>(scratch_o));
             }
+            // every merge thread of the CTA is done before "merges done" is stamped and the exit counter moves (the
+            // last CTA out re-arms the tickets and closes the epoch)
+            named_bar_sync(1, kNW * 32);
             if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 3] = globaltimer();
         }
         if (threadIdx.x == 0 && atomicAdd(p.sched + 3, 1) == grid_all - 1) {
@@ -1109,7 +1123,8 @@ __global__ void __launch_bounds__(128)
 tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restrict__ seq_cap,
                       const int32_t* __restrict__ tbl_pages,
                       const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, uint4* __restrict__ pool,
-                      int32_t* __restrict__ kv_len, int32_t* __restrict__ overflow, int n_seq, int Hp, int d, int kPage) {
+                      int32_t* __restrict__ kv_len, int32_t* __restrict__ overflow, int n_seq, int Hp, int d, int kPage,
+                      int n_pool_pages) {
     const int seq = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (seq >= n_seq) return;
     const int4 si = seq_info[seq];  // {first slot of the row, slot capacity in tokens, slot, row}
@@ -1120,6 +1135,10 @@ tangram_append_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
     }
     const int chunks = d / 8;  // 16-byte chunks per row
     const int page = tbl_pages[si.x + n / kPage];
+    if (static_cast<unsigned>(page) >= static_cast<unsigned>(n_pool_pages)) {  // not a page of this pool: never stored to
+        if (lane == 0 && overflow) atomicAdd(overflow, 1);
+        return;
+    }
     // pool[page][slot][kv][token][d]
     const size_t row_k = ((static_cast<size_t>(page) * Hp + si.z) * 2 + 0) * kPage + n % kPage;
     const size_t row_v = ((static_cast<size_t>(page) * Hp + si.z) * 2 + 1) * kPage + n % kPage;
@@ -1236,13 +1255,17 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     const bool fits = D <= 128 && prm.G * (D / 4) <= L::kNW * 32;
     if (want_tail_merge && fits && (cached_smem != smem || cached_dev != dev))
         cached_max = max_coresident<D, TIMED, NH, PAGE>(dev, smem), cached_smem = smem, cached_dev = dev;
-    // The ticket scheme of the tail phase only needs the CTAs that WAIT to fit on the device together: with a grid
-    // larger than that, the last `cached_max` arrivals merge (plain launch: a cooperative one would be refused).
-    const bool coresident = dp->n_static <= cached_max;
-    prm.tail_merge = want_tail_merge && fits && cached_max > 0;
-    prm.merge_ctas = std::min(dp->n_static, cached_max);
+    // The CTAs of the tail phase wait for parts that other CTAs write, so the whole grid must be resident at once:
+    // the in-grid merge is used only in a grid that fits on the device and is therefore launched cooperatively
+    // (gang-scheduled).  A larger grid runs as a plain launch with no wait inside and is followed by the stand-alone
+    // merge kernel (and, for a fused step, the length / table-growth kernel): the occupancy figure assumes a free
+    // device, and with another plan's grid, any long kernel, MPS or an SM-limited context next to it the waiters of a
+    // plain launch could hold every slot the not-yet-scheduled CTAs need.
+    const bool coresident = cached_max > 0 && dp->n_static <= cached_max;
+    prm.tail_merge = want_tail_merge && fits && coresident;
+    prm.merge_ctas = dp->n_static;
     *merged = prm.tail_merge;
-    if (prm.q_host && !(prm.tail_merge && coresident)) {
+    if (prm.q_host && !prm.tail_merge) {
         // no co-resident grid, no in-kernel staging: the staging kernel runs first and the decode kernel is
         // launched behind it with programmatic stream serialization (it waits before its first query load)
         const int rc = tangram_stage_from_host(const_cast<__nv_bfloat16*>(prm.q), prm.q_host, (size_t)prm.R * prm.Hq * D * 2, stream);
@@ -1261,10 +1284,9 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
     // dependent successor, whose CTAs become resident while this grid still runs.  (A plain launch behind a
     // programmatic dependency was 1.8 us per layer-step faster in the graph loop and deadlocked about once in three
     // runs of the 200-step graph test: dependent CTAs took SMs that CTAs of this grid had not reached yet.)  A grid
-    // larger than the device cannot be gang-scheduled: it runs as a plain launch, only its last `merge_ctas` CTAs
-    // wait, and it does not let its dependents start early.
-    attr[0].val.cooperative = (prm.tail_merge && coresident) ? 1 : 0;
-    prm.early_trigger = (!prm.tail_merge || coresident) ? 1 : 0;
+    // larger than the device cannot be gang-scheduled: it runs as a plain launch without the tail phase (above).
+    attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
+    prm.early_trigger = 1;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr, cfg.numAttrs = prm.pdl ? 2 : 1;
@@ -1274,7 +1296,7 @@ static int launch_split(const tangram_device_plan* dp, DecodeParams prm, const C
         else {
             (void)cudaGetLastError();
             g_overlap_state = 0, prm.pdl = 0, cfg.numAttrs = 1;  // the kernel then must not wait for a predecessor
-            attr[0].val.cooperative = (prm.tail_merge && coresident) ? 1 : 0;
+            attr[0].val.cooperative = prm.tail_merge ? 1 : 0;
             e = cudaLaunchKernelEx(&cfg, tangram_decode_kernel<D, TIMED, NH, PAGE>, map, prm);
         }
     }
@@ -1594,6 +1616,7 @@ static GrowParams grow_params(const tangram_device_plan* dp, int32_t* kv_len_dev
     g.kv_len = kv_len_dev, g.grow_state = dp->grow_state, g.free_pages = free_pages_dev, g.overflow = overflow_dev;
     g.n_free = (int32_t)std::min<int64_t>(n_free, INT32_MAX), g.n_rows = dp->R * dp->C;
     g.R = dp->R, g.H = dp->H, g.C = dp->C, g.Hp = dp->Hp;
+    g.n_pool_pages = INT32_MAX;  // the pool's size is not known here; tangram_decode_step fills it in
     return g;
 }
 
@@ -1676,8 +1699,10 @@ static int run_attention(const tangram_device_plan* dp, const void* q, const voi
     if (step.k_new) {
         prm.k_new = static_cast<const uint4*>(step.k_new), prm.v_new = static_cast<const uint4*>(step.v_new);
         prm.pool_w = static_cast<uint4*>(const_cast<void*>(kv_pool));
+        prm.n_pool_pages = (int32_t)std::min<int64_t>(n_pool_pages, INT32_MAX);
         prm.seq_cap = dp->seq_cap, prm.kv_len_w = step.kv_len_w;
         prm.grow = grow_params(dp, step.kv_len_w, step.free_pages, step.n_free, step.overflow);
+        prm.grow.n_pool_pages = prm.n_pool_pages;
     }
     prm.pdl = (step.flags & TANGRAM_STEP_OVERLAP) ? 1 : 0;
 
@@ -1861,7 +1886,8 @@ extern "C" int tangram_append_kv(const tangram_device_plan* dp, const void* k_ne
     const int n_seq = dp->R * dp->H;
     tangram_append_kernel<<<(n_seq + 3) / 4, 128, 0, static_cast<cudaStream_t>(stream)>>>(
         reinterpret_cast<const int4*>(dp->seq_info), dp->seq_cap, dp->tbl_pages, static_cast<const uint4*>(k_new),
-        static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d, dp->P);
+        static_cast<const uint4*>(v_new), static_cast<uint4*>(kv_pool), kv_len_dev, overflow_dev, n_seq, dp->Hp, d, dp->P,
+        (int)std::min<int64_t>(n_pool_pages, INT32_MAX));
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
     return TANGRAM_OK;

@@ -322,3 +322,93 @@ def test_200_decode_steps_on_a_3_layer_graph_through_page_boundaries():
         assert grew.min() >= steps // 16 - 2                               # every row crossed at least 10 page boundaries
         ro, rl, _ = O.attention(S["q"].cpu(), torch.from_numpy(rb.view(np.int16)).view(torch.bfloat16), to, rk, wl.Hq, wl.d)
         check(S["out"], S["lse"], ro, rl, "200-step graph loop")
+
+
+def _poisoned_free_list(wl, headroom):
+    """Growable tables from a valid free list whose NOT YET USED part then gets entries that are no pages of the pool
+    (beyond its end, huge, negative) mixed in; -> (B, kv, tables, free list, pages of the pool, the bad entries)."""
+    B, kv, t, to, free = growable_setup(wl, headroom=headroom)
+    n_pages = int(free.max()) + 1
+    free = free.copy()
+    tail = np.arange(t.n_pages_used, free.shape[0])
+    bad_at = tail[::3][:12]
+    bad = np.array([n_pages, n_pages + 5, 2 ** 30, -7, 2 ** 31 - 1, n_pages + 1] * 2, dtype=np.int64)[:bad_at.shape[0]]
+    free[bad_at] = bad.astype(np.int32)
+    return B, kv, t, free, n_pages, set(int(x) for x in bad)
+
+
+def test_decode_step_never_hands_out_a_free_list_entry_outside_the_pool():
+    """The appends store through the page tables without a hardware bound (the TMA reads are clamped, plain stores are
+    not), so a wrong free-list entry must not become a store address.  tangram_decode_step knows the pool's size: a
+    free-list entry outside [0, n_pool_pages) is consumed but never written into the tables, the row counts as starved
+    and takes the next entry at the next step.  Checked: guard pages behind the pool and every page no table names
+    keep their bits; the tables hold only pages of the pool; rows were starved; and the attention result of the last
+    step equals the oracle's over the final pool, tables and lengths."""
+    wl = I.make_random_workload(46, R=4, H=4, G=2, d=64, C=2, max_ctx=200)
+    B, kv, t, free, n_pages, bad = _poisoned_free_list(wl, headroom=6)
+    n_guard = 6
+    g = torch.Generator(device="cuda").manual_seed(9)
+    big = torch.randn(n_pages + n_guard, t.Hp, 2, wl.P, wl.d, generator=g, device="cuda").bfloat16()
+    pool = big[:n_pages]                                              # the pool the calls are told about
+    before = bits(big).copy()
+    q = torch.randn(wl.R, wl.Hq, wl.d, generator=g, device="cuda").bfloat16()
+    cap = slot_capacity(t, wl)
+    pl = T.tangram_plan_partitions(t, B, cap, n_cta(wl), wl.granule, 1, T.MODE_BALANCED, 0, 300, 3)
+    dp = T.tangram_upload(t, pl)
+    free_dev, kv_dev = torch.from_numpy(free).cuda(), torch.from_numpy(kv.copy()).cuda()
+    over = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for step in range(70):                                            # through several page boundaries of every row
+        k_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+        v_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+        out, lse = T.tangram_decode_step(dp, q, k_new, v_new, pool, kv_dev, free_dev, overflow=over)
+    torch.cuda.synchronize()
+    starved = T.tangram_download_tables(dp, t)
+    assert t.n_pages_used > int(np.flatnonzero(np.isin(free, list(bad)))[0]), "no bad entry was reached"
+    assert starved > 0
+    held = t.tbl_pages[t.tbl_pages >= 0]
+    assert held.max() < n_pages and not np.isin(held, list(bad)).any()
+    after = bits(big)
+    assert np.array_equal(after[n_pages:], before[n_pages:]), "a guard page behind the pool was written"
+    unnamed = np.setdiff1d(np.arange(n_pages), held)
+    assert np.array_equal(after[unnamed], before[unnamed]), "a page that no table names was written"
+    kv_now = kv_dev.cpu().numpy()
+    assert (kv_now > kv).all()
+    to = O.Tables(R=t.R, H=t.H, C=t.C, Hp=t.Hp, P=t.P, perm=t.perm, cluster_of=t.cluster_of, slot_of=t.slot_of,
+                  tbl_indptr=t.tbl_indptr, tbl_pages=t.tbl_pages, n_pages_used=t.n_pages_used)
+    ro, rl, _ = O.attention(q.cpu(), pool.cpu(), to, kv_now, wl.Hq, wl.d)
+    check(out, lse, ro, rl, "last step after poisoned free-list entries")
+
+
+def test_append_kv_never_stores_through_a_page_id_outside_the_pool():
+    """tangram_extend_tables_device does not know the pool's size, so a wrong free-list entry can reach the tables;
+    tangram_append_kv then keeps the row's length, counts it in overflow and stores nothing for it."""
+    wl = I.make_random_workload(47, R=3, H=4, G=2, d=128, C=2, max_ctx=150)
+    B, kv, t, free, n_pages, bad = _poisoned_free_list(wl, headroom=4)
+    # full rows, so that the very next token of every row needs the page handed out below
+    full = slot_capacity(t, wl) - 4 * wl.P
+    g = torch.Generator(device="cuda").manual_seed(10)
+    big = torch.randn(n_pages + 4, t.Hp, 2, wl.P, wl.d, generator=g, device="cuda").bfloat16()
+    pool = big[:n_pages]
+    before = bits(big).copy()
+    pl = T.tangram_plan_partitions(t, B, slot_capacity(t, wl), 8, wl.granule, 1, T.MODE_BALANCED, 0, 0, 0)
+    dp = T.tangram_upload(t, pl)
+    kv_dev = torch.from_numpy(full.astype(np.int32)).cuda()
+    T.tangram_extend_tables_device(dp, kv_dev, torch.from_numpy(free).cuda())
+    T.tangram_download_tables(dp, t)
+    rows = np.arange(wl.R)[:, None] * t.C + t.cluster_of[None, :]
+    new_page = t.tbl_pages[t.tbl_indptr[rows] + full // wl.P]            # the page every head's next token falls in
+    is_bad = (new_page < 0) | (new_page >= n_pages)
+    assert is_bad.any() and not is_bad.all()
+    k_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+    v_new = torch.randn(wl.R, wl.H, wl.d, generator=g, device="cuda").bfloat16()
+    over = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T.tangram_append_kv(dp, k_new, v_new, pool, kv_dev, overflow=over)
+    torch.cuda.synchronize()
+    assert np.array_equal(kv_dev.cpu().numpy(), full + (~is_bad).astype(np.int32))
+    assert int(over.item()) == int(is_bad.sum())
+    after = bits(big)
+    assert np.array_equal(after[n_pages:], before[n_pages:])
+    good_pages = np.unique(new_page[~is_bad])
+    untouched = np.setdiff1d(np.arange(n_pages), good_pages)
+    assert np.array_equal(after[untouched], before[untouched])
+    assert not np.array_equal(after[good_pages], before[good_pages])
