@@ -15,7 +15,9 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtangram.so")
+# TANGRAM_LIB selects another build of the same library (the debug build with bounded spin loops,
+# paper_2606_06302_b200/build.py --spin-limit); there is still no fallback: the named file must exist.
+LIB_PATH = os.environ.get("TANGRAM_LIB") or os.path.join(_HERE, "libtangram.so")
 
 OK, ERR_INVALID_ARG, ERR_OUT_OF_PAGES, ERR_BUFFER_TOO_SMALL, ERR_CUDA = 0, -1, -2, -3, -4
 FILL_GROUP = 1

@@ -589,8 +589,10 @@ compact_gather_kernel(const int4* __restrict__ seq_info, const int32_t* __restri
     auto wait_row = [&](int seq) {
         if (lane == 0) {
             int seen;
+            TANGRAM_SPIN_INIT;
             do {
                 asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(ready + seq) : "memory");
+                TANGRAM_SPIN_POLL(TANGRAM_WAIT_ROW_READY, seq);
             } while (seen == 0);
         }
         __syncwarp();

@@ -733,8 +733,10 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
                     if (p.q_host) {  // the item's query block is staged by some CTA's consumer warps: wait for its flag
                         const int32_t* flag = p.q_flags + item.req * p.H + item.kv_head;
                         int seen;
+                        TANGRAM_SPIN_INIT;
                         do {
                             asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(flag) : "memory");
+                            TANGRAM_SPIN_POLL(TANGRAM_WAIT_Q_FLAG, item.req * p.H + item.kv_head);
                         } while (seen != q_epoch);
                         asm volatile("fence.proxy.async;" ::: "memory");  // generic-proxy stores -> bulk (async proxy) read
                     }
@@ -1065,9 +1067,11 @@ tangram_decode_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodePa
             auto wait_parts = [&](int seq, int n) {  // every thread for itself: acquire, then its own loads
                 const unsigned want = epoch1 * static_cast<unsigned>(n);
                 unsigned seen;
+                TANGRAM_SPIN_INIT;
                 for (;;) {
                     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(p.seq_done + seq) : "memory");
                     if (seen == want) break;
+                    TANGRAM_SPIN_POLL(TANGRAM_WAIT_SEQ_PARTS, seq);
                     if (TANGRAM_BARRIER_NANOSLEEP > 0) __nanosleep(TANGRAM_BARRIER_NANOSLEEP);
                 }
                 if (TIMED && threadIdx.x == 0) p.worker_ns[4 * blockIdx.x + 2] = globaltimer();  // the CTA's last wait passed
