@@ -563,6 +563,24 @@ def test_head_dim_256_gemma_shaped_layer_with_append():
         check(out, lse, ref_out, ref_lse, f"d=256 decode step {step}")
 
 
+def test_host_read_reproducer_torch_free(tmp_path):
+    """tests/c_abi/host_read_repro.cu: the skeleton of tangram_decode_attention_host (cooperative grid, consumer warps
+    copying blocks from cudaHostAlloc-ed memory, producers spinning on ld.acquire.gpu flags and fetching the staged
+    block with cp.async.bulk, posted stores to host memory, CPU work between launches) without torch, without the
+    library, under its own watchdog.  20 000 launches here; the tally of the long runs is in DESIGN.md section 8.
+    A launch that never completes is reported by the program itself (exit code 2), so this test cannot hang."""
+    import os
+    import subprocess
+    from paper_2606_06302_b200 import build as Bd
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe = str(tmp_path / "host_read_repro")
+    subprocess.check_call([Bd.nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "-o", exe,
+                           os.path.join(root, "tests", "c_abi", "host_read_repro.cu")])
+    out = subprocess.run([exe, "20000", "20"], capture_output=True, text=True, timeout=400)
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert "launches=20000 hangs=0 mismatches=0" in out.stdout
+
+
 def test_whole_path_from_plain_c(tmp_path):
     """The C ABI end to end from a plain C program (CUDA runtime C API + include/tangram.h, no Python / torch in
     the process): closed-form outputs (q = 0, V_h = h + 1, NaN in every slot that is not a retained row)."""
